@@ -1,0 +1,471 @@
+// oracle/lbo.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, fp64 CPU oracle for the two-component colour-gradient D3Q19 lattice
+// Boltzmann step with near-contact repulsion (arxiv 2005.12764).  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load it.
+// It shares no code with the CUDA path (paper_2005_12764_b200/csrc) and neither includes
+// the other.
+//
+// What it follows, step by step, in the paper's order (PAPER.md = /root/reference/PAPER.md):
+//   S0 init         Eq. 2 per component with the common u
+//   S1 moments      rho_k = sum_i f^k_i, m = sum_i c_i f_i         PAPER.md:96 (Eq. 3)
+//   S2 gradient     G = 3 sum_i w_i c_i phi(x+c_i)                 stencil of Eq. 10
+//   S3 near contact F_rep = -A_h[h] n delta_I                      PAPER.md:221-223 (Eq. 11)
+//   S4 force, u     Guo half-force shift (north_star; S_i role PAPER.md:92)
+//   S5 omega_eff    Eq. 7-8, sign of Eq. 7 fixed by Eq. 4
+//   S6 BGK + source Eq. 1 on the total f = f^r + f^b
+//   S7 perturbation colour-gradient surface tension (north_star; not in the paper's text)
+//   S8 recolouring  Latva-Kokko (north_star; not in the paper's text)
+//   S9 streaming    exact shift + link-wise bounce-back
+// Readings of everything the paper leaves open are G1-G24 of SURVEY.md section 8(c), restated
+// in DESIGN.md.
+//
+// Pins (tests/test_oracle_*.py): P1 constants, P2 equilibrium fixed point, P3 mass, P4 momentum,
+// P5 shear-wave viscosity (Eq. 4), P6 mixture viscosity (Eq. 8), P7 Poiseuille, P8 Laplace,
+// P9 near-contact sign/size, P10 film table A_h(h), P11 lattice symmetry, P12 brute-force numpy
+// twin, P13 Taylor-Green decay.
+// PARITY UNPINNED against the paper (pinned only against DESIGN.md's reading): the discrete
+// contact search (G10), H_MAX, the wall rule for phi (G8), the guard eps (G7).
+//
+// Deliberately nothing clever: loops over sites and over the 19 directions, two full
+// population arrays, OpenMP on the outermost site loop only.
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace {
+
+constexpr int Q = 19;
+// Velocity order; the paper numbers i = 1..19 and fixes no order.
+const int CX[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+const int CY[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+const int CZ[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+const int OPP[Q] = {0, 2, 1, 4, 3, 6, 5, 8, 7, 10, 9, 12, 11, 14, 13, 16, 15, 18, 17};
+// "weights normalized to unity" PAPER.md:90; values are the standard D3Q19 ones (G2).
+const double W[Q] = {1.0 / 3, 1.0 / 18, 1.0 / 18, 1.0 / 18, 1.0 / 18, 1.0 / 18, 1.0 / 18,
+                     1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36,
+                     1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36};
+// Perturbation constants B_i (G5): sum B_i = 1/3, sum B_i c_ia c_ib = delta_ab / 3.
+const double B[Q] = {-1.0 / 3, 1.0 / 18, 1.0 / 18, 1.0 / 18, 1.0 / 18, 1.0 / 18, 1.0 / 18,
+                     1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36,
+                     1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36};
+constexpr double EPS_G = 1e-12;  // guard on |G| (G7)
+constexpr int H_MIN = 3;         // "h_min = 3-4 lattice units" PAPER.md:223 (G10)
+constexpr int H_MAX = 4;         // outer cut-off of the probe (G10)
+
+struct Oracle {
+  int nx = 0, ny = 0, nz = 0;
+  size_t S = 0;
+  double tau_r = 1, tau_b = 1, A = 0, beta = 0, A_nc = 0;
+  double g[3] = {0, 0, 0};
+  double phi_c = 0.9;
+  int nc_mode = 0;  // 0 = probe (S3), 1 = test hook: every |phi|<phi_c site in contact with A_h = A_nc
+  bool two = true;
+  bool inited = false;
+  bool any_solid = false;
+  std::vector<uint8_t> solid;            // S, 1 = solid
+  std::vector<double> f[2], fpost[2];    // [k][site*19 + i], pre- and post-collision
+  std::vector<double> rho_r, rho_b, phi; // per site (S1)
+  std::vector<double> mx, my, mz;        // bare momentum (S1)
+  std::vector<double> Fx, Fy, Fz;        // total force of the last evaluation (S4)
+  std::vector<double> Gx, Gy, Gz;        // colour gradient of the last evaluation (S2)
+  std::vector<int> hcontact;             // contact distance found by the probe, 0 = none
+  std::vector<double> margin;            // smallest margin of any discrete decision (G12)
+  std::string err;
+
+  size_t idx(int x, int y, int z) const { return (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * (size_t)z); }
+  static int wrap(int a, int n) {  // periodic image; loops so that boxes with n = 1 work (G22)
+    while (a < 0) a += n;
+    while (a >= n) a -= n;
+    return a;
+  }
+  size_t nbr(int x, int y, int z, int dx, int dy, int dz) const {
+    return idx(wrap(x + dx, nx), wrap(y + dy, ny), wrap(z + dz, nz));
+  }
+};
+
+double feq(int i, double rho, double ux, double uy, double uz) {
+  // Eq. 2 PAPER.md:87-90 with c_s^2 = 1/3: w_i rho (1 + 3 c.u + 4.5 (c.u)^2 - 1.5 u.u)
+  double cu = CX[i] * ux + CY[i] * uy + CZ[i] * uz;
+  double uu = ux * ux + uy * uy + uz * uz;
+  return W[i] * rho * (1.0 + 3.0 * cu + 4.5 * cu * cu - 1.5 * uu);
+}
+
+// S1 for every fluid site.
+void moments(Oracle& o) {
+  const size_t S = o.S;
+#pragma omp parallel for schedule(static)
+  for (long long sll = 0; sll < (long long)S; ++sll) {
+    size_t s = (size_t)sll;
+    if (o.solid[s]) {
+      o.rho_r[s] = o.rho_b[s] = o.phi[s] = 0.0;
+      o.mx[s] = o.my[s] = o.mz[s] = 0.0;
+      continue;
+    }
+    double rr = 0, rb = 0, mx = 0, my = 0, mz = 0;
+    for (int i = 0; i < Q; ++i) {
+      double fr = o.f[0][s * Q + i];
+      double fb = o.two ? o.f[1][s * Q + i] : 0.0;
+      rr += fr;
+      rb += fb;
+      mx += CX[i] * (fr + fb);
+      my += CY[i] * (fr + fb);
+      mz += CZ[i] * (fr + fb);
+    }
+    o.rho_r[s] = rr;
+    o.rho_b[s] = rb;
+    o.phi[s] = (rr - rb) / (rr + rb);
+    o.mx[s] = mx;
+    o.my[s] = my;
+    o.mz[s] = mz;
+  }
+}
+
+// S2-S4 at one fluid site: gradient, near-contact force, total force. Returns via refs.
+void force_at(Oracle& o, int x, int y, int z, double& Gx, double& Gy, double& Gz, double& Fx,
+              double& Fy, double& Fz) {
+  const size_t s = o.idx(x, y, z);
+  const double rho = o.rho_r[s] + o.rho_b[s];
+  Gx = Gy = Gz = 0.0;
+  double Fncx = 0, Fncy = 0, Fncz = 0;
+  int hfound = 0;
+  double marg = 1e300;
+  if (o.two) {
+    const double phi0 = o.phi[s];
+    // S2: G = 3 sum_{i>=1} w_i c_i phi~(x+c_i); a solid neighbour contributes phi(x) (G8).
+    for (int i = 1; i < Q; ++i) {
+      size_t n = o.nbr(x, y, z, CX[i], CY[i], CZ[i]);
+      double p = o.solid[n] ? phi0 : o.phi[n];
+      Gx += 3.0 * W[i] * CX[i] * p;
+      Gy += 3.0 * W[i] * CY[i] * p;
+      Gz += 3.0 * W[i] * CZ[i] * p;
+    }
+    const double Gn = std::sqrt(Gx * Gx + Gy * Gy + Gz * Gz);
+    // S3: near-contact force, Eq. 11 PAPER.md:221 with delta_I = |G|/2 (G9), n = -G/|G| (G10).
+    if (o.A_nc != 0.0) {
+      marg = std::fabs(std::fabs(phi0) - o.phi_c);
+      if (std::fabs(phi0) < o.phi_c && Gn > EPS_G) {
+        double Ah = 0.0;
+        if (o.nc_mode == 1) {
+          Ah = o.A_nc;
+          hfound = 1;
+        } else {
+          const double n[3] = {-Gx / Gn, -Gy / Gn, -Gz / Gn};
+          for (int k = 1; k <= H_MAX; ++k) {
+            int d[3];
+            for (int a = 0; a < 3; ++a) {
+              double v = k * n[a];
+              d[a] = (int)std::lround(v);  // round half away from zero
+              double fr = std::fabs(v) - std::floor(std::fabs(v));
+              marg = std::fmin(marg, std::fabs(fr - 0.5));
+            }
+            size_t p = o.nbr(x, y, z, d[0], d[1], d[2]);
+            if (o.solid[p]) break;  // wall in the way: no contact
+            if (k >= 2) {
+              marg = std::fmin(marg, std::fabs(o.phi[p] - phi0));
+              if (o.phi[p] >= phi0) {
+                hfound = k;
+                break;
+              }
+            }
+          }
+          if (hfound > 0) {
+            // A_h = A for h <= h_min, decays as h^-3 beyond.
+            Ah = hfound <= H_MIN ? o.A_nc
+                                 : o.A_nc * std::pow((double)H_MIN / (double)hfound, 3.0);
+          }
+        }
+        // -A_h n delta_I = -A_h (-G/|G|) (|G|/2) = +A_h G / 2
+        Fncx = 0.5 * Ah * Gx;
+        Fncy = 0.5 * Ah * Gy;
+        Fncz = 0.5 * Ah * Gz;
+      }
+    }
+  }
+  // S4: F = rho g + F_nc (G13).
+  Fx = rho * o.g[0] + Fncx;
+  Fy = rho * o.g[1] + Fncy;
+  Fz = rho * o.g[2] + Fncz;
+  o.Gx[s] = Gx; o.Gy[s] = Gy; o.Gz[s] = Gz;
+  o.Fx[s] = Fx; o.Fy[s] = Fy; o.Fz[s] = Fz;
+  o.hcontact[s] = hfound;
+  o.margin[s] = marg;
+}
+
+// S5-S8 at one fluid site; writes fpost.
+void collide_at(Oracle& o, int x, int y, int z) {
+  const size_t S = o.S;
+  const size_t s = o.idx(x, y, z);
+  double Gx, Gy, Gz, Fx, Fy, Fz;
+  force_at(o, x, y, z, Gx, Gy, Gz, Fx, Fy, Fz);
+  const double rr = o.rho_r[s], rb = o.rho_b[s];
+  const double rho = rr + rb;
+  // S4: u = (m + F/2)/rho
+  const double ux = (o.mx[s] + 0.5 * Fx) / rho;
+  const double uy = (o.my[s] + 0.5 * Fy) / rho;
+  const double uz = (o.mz[s] + 0.5 * Fz) / rho;
+  // S5: relaxation rate. Eq. 8, then omega = 1/(3 nu + 1/2) which is Eq. 4
+  // PAPER.md:102 inverted (the minus sign printed in Eq. 7 contradicts Eq. 4: G1).
+  double omega;
+  if (!o.two || o.tau_r == o.tau_b) {
+    omega = 1.0 / o.tau_r;
+  } else {
+    double nu_r = (o.tau_r - 0.5) / 3.0, nu_b = (o.tau_b - 0.5) / 3.0;
+    double inv_nu = (rr / rho) / nu_r + (rb / rho) / nu_b;
+    double nu = 1.0 / inv_nu;
+    omega = 1.0 / (3.0 * nu + 0.5);
+  }
+  const double Gn = std::sqrt(Gx * Gx + Gy * Gy + Gz * Gz);
+  const bool aniso = o.two && Gn > EPS_G;
+  double fstar[Q];
+  for (int i = 0; i < Q; ++i) {
+    // S6: collide the total (G3), Eq. 1 PAPER.md:78 with S_i the Guo term (G4).
+    double fi = o.f[0][s * Q + i] + (o.two ? o.f[1][s * Q + i] : 0.0);
+    double fe = feq(i, rho, ux, uy, uz);
+    double cu = CX[i] * ux + CY[i] * uy + CZ[i] * uz;
+    double sx = 3.0 * (CX[i] - ux) + 9.0 * cu * CX[i];
+    double sy = 3.0 * (CY[i] - uy) + 9.0 * cu * CY[i];
+    double sz = 3.0 * (CZ[i] - uz) + 9.0 * cu * CZ[i];
+    double guo = (1.0 - 0.5 * omega) * W[i] * (sx * Fx + sy * Fy + sz * Fz);
+    double v = fi - omega * (fi - fe) + guo;
+    // S7: colour-gradient perturbation (G5).
+    if (aniso) {
+      double cg = CX[i] * Gx + CY[i] * Gy + CZ[i] * Gz;
+      v += o.A * (W[i] * cg * cg / Gn - B[i] * Gn);
+    }
+    fstar[i] = v;
+  }
+  if (!o.two) {
+    for (int i = 0; i < Q; ++i) o.fpost[0][s * Q + i] = fstar[i];
+    return;
+  }
+  // S8: Latva-Kokko recolouring (G6); blue by subtraction so that f^r + f^b = f* exactly.
+  for (int i = 0; i < Q; ++i) {
+    double fr = (rr / rho) * fstar[i];
+    if (aniso && i > 0) {
+      double cg = CX[i] * Gx + CY[i] * Gy + CZ[i] * Gz;
+      double cnorm = std::sqrt((double)(CX[i] * CX[i] + CY[i] * CY[i] + CZ[i] * CZ[i]));
+      fr += o.beta * (rr * rb / rho) * W[i] * cg / (cnorm * Gn);
+    }
+    o.fpost[0][s * Q + i] = fr;
+    o.fpost[1][s * Q + i] = fstar[i] - fr;
+  }
+}
+
+// S9: f^k_i(x,t+1) = f^k*_i(x-c_i) if x-c_i is fluid, else f^k*_opp(i)(x) (G21).
+void stream(Oracle& o) {
+  const size_t S = o.S;
+  const int nk = o.two ? 2 : 1;
+#pragma omp parallel for schedule(static)
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x) {
+        size_t s = o.idx(x, y, z);
+        if (o.solid[s]) continue;
+        for (int i = 0; i < Q; ++i) {
+          size_t n = o.nbr(x, y, z, -CX[i], -CY[i], -CZ[i]);
+          for (int k = 0; k < nk; ++k)
+            o.f[k][s * Q + i] = o.solid[n] ? o.fpost[k][s * Q + OPP[i]] : o.fpost[k][n * Q + i];
+        }
+      }
+}
+
+void one_step(Oracle& o) {
+  moments(o);
+#pragma omp parallel for schedule(static)
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x)
+        if (!o.solid[o.idx(x, y, z)]) collide_at(o, x, y, z);
+  stream(o);
+}
+
+void eval_forces(Oracle& o) {
+  moments(o);
+#pragma omp parallel for schedule(static)
+  for (int z = 0; z < o.nz; ++z)
+    for (int y = 0; y < o.ny; ++y)
+      for (int x = 0; x < o.nx; ++x) {
+        size_t s = o.idx(x, y, z);
+        if (o.solid[s]) {
+          o.Fx[s] = o.Fy[s] = o.Fz[s] = 0;
+          o.Gx[s] = o.Gy[s] = o.Gz[s] = 0;
+          o.hcontact[s] = 0;
+          o.margin[s] = 1e300;
+          continue;
+        }
+        double a, b, c, d, e, f;
+        force_at(o, x, y, z, a, b, c, d, e, f);
+      }
+}
+
+}  // namespace
+
+extern "C" {
+
+enum { LBO_OK = 0, LBO_EINVAL = -1, LBO_ENOMEM = -2, LBO_ESTATE = -4 };
+
+// params = {tau_r, tau_b, A, beta, A_nc} (order fixed by north_star)
+int lbo_create(int nx, int ny, int nz, const double* params, void** out) {
+  if (!out || !params || nx < 1 || ny < 1 || nz < 1) return LBO_EINVAL;
+  if (!(params[0] > 0.5) || !(params[1] > 0.5)) return LBO_EINVAL;  // G17
+  Oracle* o = new (std::nothrow) Oracle();
+  if (!o) return LBO_ENOMEM;
+  o->nx = nx; o->ny = ny; o->nz = nz;
+  o->S = (size_t)nx * ny * nz;
+  o->tau_r = params[0]; o->tau_b = params[1]; o->A = params[2]; o->beta = params[3]; o->A_nc = params[4];
+  try {
+    o->solid.assign(o->S, 0);
+    for (auto* v : {&o->rho_r, &o->rho_b, &o->phi, &o->mx, &o->my, &o->mz, &o->Fx, &o->Fy, &o->Fz,
+                    &o->Gx, &o->Gy, &o->Gz, &o->margin})
+      v->assign(o->S, 0.0);
+    o->hcontact.assign(o->S, 0);
+  } catch (...) {
+    delete o;
+    return LBO_ENOMEM;
+  }
+  *out = o;
+  return LBO_OK;
+}
+
+void lbo_destroy(void* h) { delete static_cast<Oracle*>(h); }
+
+int lbo_set_geometry(void* h, const uint8_t* mask) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  if (o->inited) return LBO_ESTATE;
+  o->any_solid = false;
+  for (size_t s = 0; s < o->S; ++s) {
+    o->solid[s] = mask ? (mask[s] != 0) : 0;
+    o->any_solid |= o->solid[s] != 0;
+  }
+  return LBO_OK;
+}
+
+int lbo_set_body_force(void* h, double gx, double gy, double gz) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  o->g[0] = gx; o->g[1] = gy; o->g[2] = gz;
+  return LBO_OK;
+}
+
+int lbo_set_nc_cutoff(void* h, double phi_c) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  o->phi_c = phi_c;
+  return LBO_OK;
+}
+
+int lbo_set_nc_mode(void* h, int mode) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (mode != 0 && mode != 1)) return LBO_EINVAL;
+  o->nc_mode = mode;
+  return LBO_OK;
+}
+
+// S0. rho_b == NULL selects single-component mode. u is [3][z][y][x].
+int lbo_init(void* h, const double* rho_r, const double* rho_b, const double* u) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || !rho_r || !u) return LBO_EINVAL;
+  const size_t S = o->S;
+  o->two = rho_b != nullptr;
+  const int nk = o->two ? 2 : 1;
+  try {
+    for (int k = 0; k < nk; ++k) {
+      o->f[k].assign(Q * S, 0.0);
+      o->fpost[k].assign(Q * S, 0.0);
+    }
+  } catch (...) {
+    return LBO_ENOMEM;
+  }
+  for (size_t s = 0; s < S; ++s) {
+    if (o->solid[s]) continue;
+    for (int i = 0; i < Q; ++i) {
+      o->f[0][s * Q + i] = feq(i, rho_r[s], u[s], u[S + s], u[2 * S + s]);
+      if (o->two) o->f[1][s * Q + i] = feq(i, rho_b[s], u[s], u[S + s], u[2 * S + s]);
+    }
+  }
+  o->inited = true;
+  return LBO_OK;
+}
+
+int lbo_step(void* h, int nsteps) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || nsteps < 0) return LBO_EINVAL;
+  if (!o->inited) return LBO_ESTATE;
+  for (int t = 0; t < nsteps; ++t) one_step(*o);
+  return LBO_OK;
+}
+
+// rho_r, rho_b and the half-force-shifted velocity (G16); zeros on solid sites.
+int lbo_get_macros(void* h, double* rho_r, double* rho_b, double* u) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  if (!o->inited) return LBO_ESTATE;
+  eval_forces(*o);
+  const size_t S = o->S;
+  for (size_t s = 0; s < S; ++s) {
+    double rho = o->rho_r[s] + o->rho_b[s];
+    bool sol = o->solid[s];
+    if (rho_r) rho_r[s] = sol ? 0.0 : o->rho_r[s];
+    if (rho_b && o->two) rho_b[s] = sol ? 0.0 : o->rho_b[s];
+    if (u) {
+      u[s] = sol ? 0.0 : (o->mx[s] + 0.5 * o->Fx[s]) / rho;
+      u[S + s] = sol ? 0.0 : (o->my[s] + 0.5 * o->Fy[s]) / rho;
+      u[2 * S + s] = sol ? 0.0 : (o->mz[s] + 0.5 * o->Fz[s]) / rho;
+    }
+  }
+  return LBO_OK;
+}
+
+// Debug accessors. Pre-collision populations f^k_i(x,t), layout [i][z][y][x].
+int lbo_get_populations(void* h, int comp, double* f) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || !f || comp < 0 || comp > (o->two ? 1 : 0)) return LBO_EINVAL;
+  if (!o->inited) return LBO_ESTATE;
+  for (size_t s = 0; s < o->S; ++s)
+    for (int i = 0; i < Q; ++i) f[i * o->S + s] = o->f[comp][s * Q + i];
+  return LBO_OK;
+}
+
+int lbo_set_populations(void* h, int comp, const double* f) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || !f || comp < 0 || comp > (o->two ? 1 : 0)) return LBO_EINVAL;
+  if (!o->inited) return LBO_ESTATE;
+  for (size_t s = 0; s < o->S; ++s)
+    for (int i = 0; i < Q; ++i) o->f[comp][s * Q + i] = f[i * o->S + s];
+  return LBO_OK;
+}
+
+// Fields of the current state: phi, G[3][S], F[3][S] (total force), contact distance h
+// (0 = none), and the smallest decision margin (G12). Any pointer may be NULL.
+int lbo_get_fields(void* h, double* phi, double* G, double* F, int* hcontact, double* margin) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  if (!o->inited) return LBO_ESTATE;
+  eval_forces(*o);
+  const size_t S = o->S;
+  for (size_t s = 0; s < S; ++s) {
+    if (phi) phi[s] = o->phi[s];
+    if (G) { G[s] = o->Gx[s]; G[S + s] = o->Gy[s]; G[2 * S + s] = o->Gz[s]; }
+    if (F) { F[s] = o->Fx[s]; F[S + s] = o->Fy[s]; F[2 * S + s] = o->Fz[s]; }
+    if (hcontact) hcontact[s] = o->hcontact[s];
+    if (margin) margin[s] = o->margin[s];
+  }
+  return LBO_OK;
+}
+
+// Lattice constants, for pin P1: c[19][3], opp[19], w[19], B[19].
+void lbo_constants(int* c, int* opp, double* w, double* b) {
+  for (int i = 0; i < Q; ++i) {
+    if (c) { c[3 * i] = CX[i]; c[3 * i + 1] = CY[i]; c[3 * i + 2] = CZ[i]; }
+    if (opp) opp[i] = OPP[i];
+    if (w) w[i] = W[i];
+    if (b) b[i] = B[i];
+  }
+}
+
+}  // extern "C"

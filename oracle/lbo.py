@@ -1,0 +1,151 @@
+"""ctypes binding of the fp64 CPU oracle (oracle/lbo.cpp) -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from paper_2005_12764_b200 and vice versa.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lbo.cpp")
+_LIB = os.path.join(_HERE, "liblbo.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/lbo.cpp to oracle/liblbo.so with g++ -O2 -fopenmp (no GPU needed)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(
+            ["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        vp, dp, ip, u8p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.POINTER(C.c_uint8)
+        lib.lbo_create.argtypes = [C.c_int, C.c_int, C.c_int, dp, C.POINTER(vp)]
+        lib.lbo_destroy.argtypes = [vp]
+        lib.lbo_destroy.restype = None
+        lib.lbo_set_geometry.argtypes = [vp, u8p]
+        lib.lbo_set_body_force.argtypes = [vp, C.c_double, C.c_double, C.c_double]
+        lib.lbo_set_nc_cutoff.argtypes = [vp, C.c_double]
+        lib.lbo_set_nc_mode.argtypes = [vp, C.c_int]
+        lib.lbo_init.argtypes = [vp, dp, dp, dp]
+        lib.lbo_step.argtypes = [vp, C.c_int]
+        lib.lbo_get_macros.argtypes = [vp, dp, dp, dp]
+        lib.lbo_get_populations.argtypes = [vp, C.c_int, dp]
+        lib.lbo_set_populations.argtypes = [vp, C.c_int, dp]
+        lib.lbo_get_fields.argtypes = [vp, dp, dp, dp, ip, dp]
+        lib.lbo_constants.argtypes = [ip, ip, dp, dp]
+        lib.lbo_constants.restype = None
+        _lib = lib
+    return _lib
+
+
+def _dptr(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def constants():
+    """(c[19,3], opp[19], w[19], B[19]) as the oracle holds them."""
+    lib = _load()
+    c = np.zeros((19, 3), np.int32)
+    opp = np.zeros(19, np.int32)
+    w = np.zeros(19)
+    b = np.zeros(19)
+    lib.lbo_constants(c.ctypes.data_as(C.POINTER(C.c_int)), opp.ctypes.data_as(C.POINTER(C.c_int)),
+                      _dptr(w), _dptr(b))
+    return c, opp, w, b
+
+
+class Oracle:
+    """Scalar fields are [nz, ny, nx] (x fastest); u is [3, nz, ny, nx]; populations [19, nz, ny, nx]."""
+
+    def __init__(self, nx, ny, nz, tau_r=1.0, tau_b=1.0, A=0.0, beta=0.0, A_nc=0.0):
+        self.lib = _load()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self.two = True
+        p = np.array([tau_r, tau_b, A, beta, A_nc], np.float64)
+        h = C.c_void_p()
+        rc = self.lib.lbo_create(self.nx, self.ny, self.nz, _dptr(p), C.byref(h))
+        if rc != 0:
+            raise ValueError("lbo_create failed: %d" % rc)
+        self.h = h
+
+    def _ck(self, rc, what):
+        if rc != 0:
+            raise RuntimeError("%s failed: %d" % (what, rc))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.lbo_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def set_geometry(self, mask):
+        if mask is None:
+            self._ck(self.lib.lbo_set_geometry(self.h, None), "lbo_set_geometry")
+            return
+        m = np.ascontiguousarray(mask, dtype=np.uint8).reshape(self.shape)
+        self._ck(self.lib.lbo_set_geometry(self.h, m.ctypes.data_as(C.POINTER(C.c_uint8))), "lbo_set_geometry")
+
+    def set_body_force(self, gx, gy, gz):
+        self._ck(self.lib.lbo_set_body_force(self.h, gx, gy, gz), "lbo_set_body_force")
+
+    def set_nc_cutoff(self, phi_c):
+        self._ck(self.lib.lbo_set_nc_cutoff(self.h, phi_c), "lbo_set_nc_cutoff")
+
+    def set_nc_mode(self, mode):
+        self._ck(self.lib.lbo_set_nc_mode(self.h, mode), "lbo_set_nc_mode")
+
+    def init(self, rho_r, rho_b, u):
+        rr = _f64(rho_r).reshape(self.shape)
+        rb = None if rho_b is None else _f64(rho_b).reshape(self.shape)
+        uu = _f64(u).reshape((3,) + self.shape)
+        self.two = rb is not None
+        self._ck(self.lib.lbo_init(self.h, _dptr(rr), _dptr(rb), _dptr(uu)), "lbo_init")
+
+    def step(self, n=1):
+        self._ck(self.lib.lbo_step(self.h, int(n)), "lbo_step")
+
+    def get_macros(self):
+        rr = np.zeros(self.shape)
+        rb = np.zeros(self.shape) if self.two else None
+        u = np.zeros((3,) + self.shape)
+        self._ck(self.lib.lbo_get_macros(self.h, _dptr(rr), _dptr(rb), _dptr(u)), "lbo_get_macros")
+        return rr, rb, u
+
+    def get_populations(self, comp):
+        f = np.zeros((19,) + self.shape)
+        self._ck(self.lib.lbo_get_populations(self.h, comp, _dptr(f)), "lbo_get_populations")
+        return f
+
+    def set_populations(self, comp, f):
+        ff = _f64(f).reshape((19,) + self.shape)
+        self._ck(self.lib.lbo_set_populations(self.h, comp, _dptr(ff)), "lbo_set_populations")
+
+    def get_fields(self):
+        """dict(phi, G[3], F[3], h (contact distance, 0 = none), margin (G12))."""
+        phi = np.zeros(self.shape)
+        G = np.zeros((3,) + self.shape)
+        F = np.zeros((3,) + self.shape)
+        h = np.zeros(self.shape, np.int32)
+        m = np.zeros(self.shape)
+        self._ck(self.lib.lbo_get_fields(self.h, _dptr(phi), _dptr(G), _dptr(F),
+                                         h.ctypes.data_as(C.POINTER(C.c_int)), _dptr(m)), "lbo_get_fields")
+        return dict(phi=phi, G=G, F=F, h=h, margin=m)

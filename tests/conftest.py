@@ -1,0 +1,21 @@
+"""pytest configuration: the `gpu` marker and the repo root on sys.path."""
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on a B200)")
+
+
+@pytest.fixture(scope="session")
+def lbo():
+    """The fp64 CPU oracle binding (oracle/lbo.py); compiles oracle/lbo.cpp on first use."""
+    from oracle import lbo as mod
+    mod.build()
+    return mod

@@ -1,0 +1,115 @@
+"""Brute-force numpy restatement of one colour-gradient LB step (pin P12).
+
+Independent of oracle/lbo.cpp: whole-array operations with np.roll, streaming in PUSH form
+with masks for walls, near-contact probe by Python loops.  Written from the equations
+(Eq. 1-8, Eq. 11) and the readings in DESIGN.md, not from
+the oracle's source.  Test infrastructure only.
+"""
+import numpy as np
+
+C = np.array([[0, 0, 0], [1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1],
+              [1, 1, 0], [-1, -1, 0], [1, -1, 0], [-1, 1, 0], [1, 0, 1], [-1, 0, -1], [1, 0, -1],
+              [-1, 0, 1], [0, 1, 1], [0, -1, -1], [0, 1, -1], [0, -1, 1]])
+WT = np.array([12] + [2] * 6 + [1] * 12) / 36.0
+BB = np.array([-12] + [2] * 6 + [1] * 12) / 36.0
+
+
+def opposite(i):
+    return int(np.where((C == -C[i]).all(1))[0][0])
+
+
+def shift(a, c):
+    """result(x) = a(x - c) for arrays indexed [z, y, x]."""
+    return np.roll(a, shift=(int(c[2]), int(c[1]), int(c[0])), axis=(0, 1, 2))
+
+
+def half_away(v):
+    return np.sign(v) * np.floor(np.abs(v) + 0.5)
+
+
+def step(fr, fb, solid, tau_r, tau_b, A, beta, A_nc=0.0, g=(0.0, 0.0, 0.0), phi_c=0.9,
+         h_min=3, h_max=4, eps=1e-12):
+    """One time step. fr, fb: [19, nz, ny, nx] pre-collision; solid: bool [nz, ny, nx]."""
+    nz, ny, nx = solid.shape
+    fluid = ~solid
+    rr, rb = fr.sum(0), fb.sum(0)
+    rho = np.where(fluid, rr + rb, 1.0)
+    phi = np.where(fluid, (rr - rb) / rho, 0.0)
+    ftot = fr + fb
+    m = np.stack([(ftot * C[:, a, None, None, None]).sum(0) for a in range(3)])
+    G = np.zeros((3, nz, ny, nx))
+    for i in range(1, 19):
+        ph_n = shift(phi, -C[i])
+        so_n = shift(solid, -C[i])
+        ph_n = np.where(so_n, phi, ph_n)
+        for a in range(3):
+            G[a] += 3.0 * WT[i] * C[i, a] * ph_n
+    Gn = np.sqrt((G ** 2).sum(0))
+    Fnc = np.zeros_like(G)
+    if A_nc != 0.0:
+        for z in range(nz):
+            for y in range(ny):
+                for x in range(nx):
+                    if solid[z, y, x] or not (abs(phi[z, y, x]) < phi_c and Gn[z, y, x] > eps):
+                        continue
+                    n = -G[:, z, y, x] / Gn[z, y, x]
+                    h = 0
+                    for k in range(1, h_max + 1):
+                        d = half_away(k * n).astype(int)
+                        p = ((z + d[2]) % nz, (y + d[1]) % ny, (x + d[0]) % nx)
+                        if solid[p]:
+                            break
+                        if k >= 2 and phi[p] >= phi[z, y, x]:
+                            h = k
+                            break
+                    if h:
+                        Ah = A_nc if h <= h_min else A_nc * (h_min / h) ** 3
+                        Fnc[:, z, y, x] = 0.5 * Ah * G[:, z, y, x]
+    F = np.stack([rho * g[a] + Fnc[a] for a in range(3)])
+    u = (m + 0.5 * F) / rho
+    if tau_r == tau_b:
+        omega = np.full(rho.shape, 1.0 / tau_r)
+    else:
+        nur, nub = (tau_r - 0.5) / 3, (tau_b - 0.5) / 3
+        nubar = 1.0 / ((rr / rho) / nur + (rb / rho) / nub)
+        omega = 1.0 / (3.0 * nubar + 0.5)
+    uu = (u ** 2).sum(0)
+    aniso = Gn > eps
+    Gs = np.where(aniso, Gn, 1.0)
+    post_r = np.zeros_like(fr)
+    post_b = np.zeros_like(fb)
+    for i in range(19):
+        cu = sum(C[i, a] * u[a] for a in range(3))
+        feq = WT[i] * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * uu)
+        guo = (1 - 0.5 * omega) * WT[i] * sum((3 * (C[i, a] - u[a]) + 9 * cu * C[i, a]) * F[a] for a in range(3))
+        fs = ftot[i] - omega * (ftot[i] - feq) + guo
+        cg = sum(C[i, a] * G[a] for a in range(3))
+        fs = fs + np.where(aniso, A * (WT[i] * cg ** 2 / Gs - BB[i] * Gn), 0.0)
+        r = (rr / rho) * fs
+        if i > 0:
+            r = r + np.where(aniso, beta * (rr * rb / rho) * WT[i] * cg / (np.sqrt((C[i] ** 2).sum()) * Gs), 0.0)
+        post_r[i] = r
+        post_b[i] = fs - r
+    # streaming, push form: what leaves x along c_i lands on x + c_i, or comes back reversed
+    new_r = np.zeros_like(fr)
+    new_b = np.zeros_like(fb)
+    for i in range(19):
+        o = opposite(i)
+        dest_solid = shift(solid, -C[i])          # is x + c_i solid?
+        for post, new in ((post_r, new_r), (post_b, new_b)):
+            go = np.where(fluid & ~dest_solid, post[i], 0.0)
+            new[i] += shift(go, C[i])
+            new[o] += np.where(fluid & dest_solid, post[i], 0.0)
+    new_r *= fluid
+    new_b *= fluid
+    return new_r, new_b
+
+
+def equilibrium(rho, u):
+    """[19, nz, ny, nx] equilibrium of Eq. 2."""
+    uu = (u ** 2).sum(0)
+    out = []
+    for i in range(19):
+        cu = sum(C[i, a] * u[a] for a in range(3))
+        out.append(WT[i] * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * uu))
+    return np.stack(out)

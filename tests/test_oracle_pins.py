@@ -1,0 +1,385 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix (CPU only).
+
+Each test names the pin (P1-P13 of DESIGN.md / SURVEY.md 8(c)) and the passage it rests on.
+None of them compares the oracle with itself: expected values are closed forms, invariants,
+an independent numpy restatement (tests/np_twin.py) or hand-built fields.
+"""
+import numpy as np
+import pytest
+
+import np_twin as tw
+
+
+def droplet(n, R, centre=None):
+    c = (n - 1) / 2.0 if centre is None else centre
+    z, y, x = np.meshgrid(*(np.arange(n),) * 3, indexing="ij")
+    d = [np.minimum(np.abs(a - c), n - np.abs(a - c)) for a in (x, y, z)]
+    r = np.sqrt(d[0] ** 2 + d[1] ** 2 + d[2] ** 2)
+    phi = np.tanh((R - r) / 2.0)
+    return (1 + phi) / 2, (1 - phi) / 2, r
+
+
+# ---------------------------------------------------------------------------------- P1
+def test_P1_lattice_constants(lbo):
+    """D3Q19 isotropy identities (PAPER.md:90 'weights normalized to unity'; G2, G5)."""
+    c, opp, w, b = lbo.constants()
+    assert len({tuple(v) for v in c}) == 19 and (np.abs(c).max(1) <= 1).all()
+    assert ((c ** 2).sum(1) <= 2).all()                       # D3Q19: no (1,1,1) links
+    for i in range(19):
+        assert (c[opp[i]] == -c[i]).all() and opp[opp[i]] == i
+    assert (c == tw.C).all()                                   # order N4
+    assert abs(w.sum() - 1) < 1e-15 and abs(b.sum() - 1 / 3) < 1e-15
+    assert np.abs((w[:, None] * c).sum(0)).max() < 1e-15
+    for arr in (w, b):
+        m2 = np.einsum("i,ia,ib->ab", arr, c, c)
+        assert np.abs(m2 - np.eye(3) / 3).max() < 1e-15
+    assert abs((w * c[:, 0] ** 4).sum() - 1 / 3) < 1e-15
+    assert abs((w * c[:, 0] ** 2 * c[:, 1] ** 2).sum() - 1 / 9) < 1e-15
+    rng = np.random.default_rng(1)
+    for _ in range(5):
+        G = rng.normal(size=3)
+        Gn = np.linalg.norm(G)
+        cn = np.sqrt((c ** 2).sum(1))
+        assert abs((w[1:] * (c[1:] @ G) / (cn[1:] * Gn)).sum()) < 1e-15
+        assert abs((w * (c @ G) ** 2 / Gn - b * Gn).sum()) < 1e-15
+
+
+# ---------------------------------------------------------------------------------- P2
+def test_P2_equilibrium_is_fixed_point(lbo):
+    """Uniform equilibrium is invariant under collide+stream (Eq. 1-2)."""
+    nx, ny, nz = 8, 6, 4
+    o = lbo.Oracle(nx, ny, nz, 0.8, 1.3, 0.01, 0.7, 0.0)
+    u = np.zeros((3, nz, ny, nx))
+    u[0], u[1], u[2] = 0.03, -0.02, 0.01
+    o.init(np.full((nz, ny, nx), 0.3), np.full((nz, ny, nx), 0.7), u)
+    f0 = [o.get_populations(k) for k in (0, 1)]
+    # closed form, typed here independently of the oracle's feq
+    for k, rho in ((0, 0.3), (1, 0.7)):
+        for i in range(19):
+            cu = tw.C[i] @ np.array([0.03, -0.02, 0.01])
+            e = tw.WT[i] * rho * (1 + 3 * cu + 4.5 * cu * cu - 1.5 * (0.03 ** 2 + 0.02 ** 2 + 0.01 ** 2))
+            assert np.abs(f0[k][i] - e).max() < 1e-16
+    o.step(1)
+    for k in (0, 1):
+        assert np.abs(o.get_populations(k) - f0[k]).max() < 1e-14
+    rr, rb, uu = o.get_macros()
+    assert np.abs(uu[0] - 0.03).max() < 1e-14 and np.abs(rb - 0.7).max() < 1e-14
+
+
+# ---------------------------------------------------------------------------------- P3, P4
+def test_P3_P4_mass_and_momentum_C1(lbo):
+    """Per-component mass and (zero force) momentum are conserved: config C1, 100 steps.
+    Collision is local and conserving, streaming exact."""
+    n = 32
+    rr0, rb0, _ = droplet(n, 8.0)
+    o = lbo.Oracle(n, n, n, 1.0, 1.0, 0.01, 0.7, 0.0)
+    rng = np.random.default_rng(3)
+    u0 = 1e-3 * rng.normal(size=(3, n, n, n))
+    o.init(rr0, rb0, u0)
+    rr, rb, u = o.get_macros()
+    M0 = (rr.sum(), rb.sum())
+    P0 = np.array([((rr + rb) * u[a]).sum() for a in range(3)])
+    o.step(100)
+    rr, rb, u = o.get_macros()
+    assert abs(rr.sum() - M0[0]) / M0[0] < 1e-12 and abs(rb.sum() - M0[1]) / M0[1] < 1e-12
+    P1 = np.array([((rr + rb) * u[a]).sum() for a in range(3)])
+    assert np.abs(P1 - P0).max() / n ** 3 < 1e-12
+    assert np.abs(u).max() > 1e-5           # something actually moved
+
+
+def test_P3_mass_with_walls_and_force(lbo):
+    """Mass per component with bounce-back walls, a droplet touching the wall, g != 0 and the
+    near-contact force on (PAPER.md:367 bounce-back; G21)."""
+    nx, ny, nz = 16, 12, 10
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    solid = (y == 0) | (y == ny - 1) | ((x == 5) & (z == 4) & (y < 4))
+    r = np.sqrt((x - 7.3) ** 2 + (y - 2.2) ** 2 + (z - 4.6) ** 2)
+    phi = np.tanh((4.0 - r) / 2)
+    o = lbo.Oracle(nx, ny, nz, 0.9, 1.2, 0.01, 0.7, 0.02)
+    o.set_geometry(solid)
+    o.set_body_force(1e-5, 2e-6, -1e-6)
+    o.init((1 + phi) / 2, (1 - phi) / 2, np.zeros((3, nz, ny, nx)))
+    rr, rb, _ = o.get_macros()
+    assert rr[solid].max() == 0 and rb[solid].max() == 0
+    M0 = (rr.sum(), rb.sum())
+    o.step(200)
+    rr, rb, u = o.get_macros()
+    assert abs(rr.sum() - M0[0]) / M0[0] < 1e-12 and abs(rb.sum() - M0[1]) / M0[1] < 1e-12
+    assert np.isfinite(u).all() and u[0][~solid].mean() > 0
+
+
+# ---------------------------------------------------------------------------------- P5, P6
+def _shear_wave_nu(lbo, tau_r, tau_b, rho_r, rho_b, steps=500):
+    nx, ny, nz = 4, 64, 4
+    o = lbo.Oracle(nx, ny, nz, tau_r, tau_b, 0.0, 0.0, 0.0)
+    yy = np.arange(ny)[None, :, None] * np.ones((nz, ny, nx))
+    k = 2 * np.pi / ny
+    u = np.zeros((3, nz, ny, nx))
+    u[0] = 1e-3 * np.sin(k * yy)
+    o.init(np.full((nz, ny, nx), rho_r), None if rho_b is None else np.full((nz, ny, nx), rho_b), u)
+    amp = []
+    for _ in range(5):
+        o.step(steps // 5)
+        _, _, uu = o.get_macros()
+        amp.append(2 * (uu[0] * np.sin(k * yy)).mean())
+    t = np.arange(1, 6) * (steps // 5)
+    slope = np.polyfit(t, np.log(amp), 1)[0]
+    return -slope / k ** 2
+
+
+@pytest.mark.parametrize("tau", [0.6, 1.0])
+def test_P5_shear_wave_viscosity(lbo, tau):
+    """nu = c_s^2 (1/omega - 1/2) (Eq. 4), single component, within 1 %."""
+    nu = _shear_wave_nu(lbo, tau, tau, 1.0, None)
+    assert abs(nu - (tau - 0.5) / 3) / ((tau - 0.5) / 3) < 0.01
+
+
+def test_P5_printed_rate():
+    """The decay rate quoted for tau = 1: nu k^2 = 1.6064e-3 per step."""
+    assert abs((1.0 - 0.5) / 3 * (2 * np.pi / 64) ** 2 - 1.6064e-3) < 1e-7
+
+
+def test_P6_mixture_viscosity(lbo):
+    """Harmonic mixing (Eq. 8) and Eq. 7 with the sign Eq. 4 demands (G1):
+    rho_r = 0.3, rho_b = 0.7, tau_r = 0.8, tau_b = 1.4 -> nu = 0.1875."""
+    nu = _shear_wave_nu(lbo, 0.8, 1.4, 0.3, 0.7)
+    assert abs(nu - 0.1875) / 0.1875 < 0.01
+    # the printed minus sign would give omega = 2 c_s^2/(2 nu - c_s^2) = 16 -> unstable, nu < 0
+    assert abs(1 / (0.3 / 0.1 + 0.7 / 0.3) - 0.1875) < 1e-15
+
+
+# ---------------------------------------------------------------------------------- P7
+def test_P7_poiseuille(lbo):
+    """Body-force driven channel between half-way bounce-back walls:
+    u_x(y) = g/(2 nu) (y - 1/2)(32.5 - y), nu = 1/6, peak 7.68e-4; 1 % of peak everywhere."""
+    nx, ny, nz = 4, 34, 4
+    g = 1e-6
+    o = lbo.Oracle(nx, ny, nz, 1.0, 1.0, 0.0, 0.0, 0.0)
+    solid = np.zeros((nz, ny, nx), bool)
+    solid[:, 0, :] = solid[:, -1, :] = True
+    o.set_geometry(solid)
+    o.set_body_force(g, 0, 0)
+    o.init(np.ones((nz, ny, nx)), None, np.zeros((3, nz, ny, nx)))
+    o.step(20000)
+    _, _, u = o.get_macros()
+    y = np.arange(ny)
+    exact = g / (2 * (1 / 6)) * (y - 0.5) * (32.5 - y)
+    peak = exact.max()
+    assert abs(peak - 7.68e-4) < 1e-6
+    prof = u[0][2, :, 1]
+    assert np.abs(prof[1:-1] - exact[1:-1]).max() < 0.01 * peak
+    assert prof[0] == 0 and prof[-1] == 0
+    assert np.abs(u[1]).max() < 1e-12 and np.abs(u[2]).max() < 1e-12
+
+
+# ---------------------------------------------------------------------------------- P8, P9
+def _laplace(lbo, n, R, steps, A_nc=0.0, nc_mode=0):
+    rr0, rb0, r = droplet(n, R)
+    o = lbo.Oracle(n, n, n, 1.0, 1.0, 0.01, 0.7, A_nc)
+    if nc_mode:
+        o.set_nc_mode(1)
+    o.init(rr0, rb0, np.zeros((3, n, n, n)))
+    o.step(steps)
+    rr, rb, u = o.get_macros()
+    rho = rr + rb
+    dp = (rho[r < R / 2].mean() - rho[r > n / 2 - 2].mean()) / 3      # p = c_s^2 rho
+    phi = (rr - rb) / rho
+    c = int((n - 1) / 2)
+    radii = []
+    for line in (phi[c, c, :], phi[c, :, c], phi[:, c, c]):
+        i = np.where((line[:-1] > 0) & (line[1:] <= 0))[0][0]
+        xr = i + line[i] / (line[i] - line[i + 1])
+        i = np.where((line[:-1] <= 0) & (line[1:] > 0))[0][0]
+        xl = i + (-line[i]) / (line[i + 1] - line[i])
+        radii.append((xr - xl) / 2)
+    return dp, float(np.mean(radii)), float(np.abs(u).max())
+
+
+@pytest.fixture(scope="module")
+def laplace_runs(lbo):
+    return {R: _laplace(lbo, n, R, steps) for n, R, steps in LAPLACE_CASES}
+
+
+LAPLACE_CASES = [(32, 6.0, 1000), (40, 8.0, 1500), (48, 12.0, 1500)]
+
+
+def test_P8_laplace_law(laplace_runs):
+    """Static droplets: dp * R is the same for R = 6, 8, 12 within 3 % (north_star), and
+    close to 2 sigma = (8/9) A tau (secondary, 10 %; G5)."""
+    prod = [dp * R for dp, R, _ in laplace_runs.values()]
+    assert (max(prod) - min(prod)) / np.mean(prod) < 0.03, prod
+    assert abs(np.mean(prod) - 8 / 9 * 0.01) / (8 / 9 * 0.01) < 0.10, prod
+    assert all(v[2] < 5e-4 for v in laplace_runs.values())       # spurious currents stay small
+
+
+def test_P9_near_contact_sign_and_size(lbo, laplace_runs):
+    """With nc_mode = 1 the near-contact force is grad(A_nc/2 clamp(phi)), an exact gradient,
+    so the droplet pressure rises by A_nc * phi_c = 0.018 (Eq. 11, G9)."""
+    dp1, R1, _ = _laplace(lbo, 40, 8.0, 1000, A_nc=0.02, nc_mode=1)
+    dp0 = laplace_runs[8.0][0]
+    assert abs((dp1 - dp0) - 0.018) < 0.05 * 0.018, (dp1, dp0)
+
+
+# ---------------------------------------------------------------------------------- P10
+@pytest.mark.parametrize("h", [2, 3, 4, 5, 6])
+def test_P10_film_table(lbo, h):
+    """A_h[h]: constant A for h <= h_min = 3, A (h_min/h)^3 beyond, nothing past H_MAX = 4
+    (G10), on a hand-built quasi-1-D film of thickness h; the force pushes
+    both interfaces away from the film (sign of Eq. 11)."""
+    nx = 64
+    A_nc = 0.02
+    phi = np.ones(nx)
+    x0 = 20
+    phi[x0] = 0.5
+    phi[x0 + 1:x0 + h] = -0.8
+    phi[x0 + h] = 0.5
+    o = lbo.Oracle(nx, 1, 1, 1.0, 1.0, 0.01, 0.7, A_nc)
+    p3 = phi.reshape(1, 1, nx)
+    o.init((1 + p3) / 2, (1 - p3) / 2, np.zeros((3, 1, 1, nx)))
+    fl = o.get_fields()
+    assert np.abs(fl["phi"].ravel() - phi).max() < 1e-15
+    Gx = fl["G"][0].ravel()
+    # central difference: the D3Q19 stencil reduces to (phi(x+1) - phi(x-1))/2 in 1-D
+    assert abs(Gx[x0] - (phi[x0 + 1] - phi[x0 - 1]) / 2) < 1e-15
+    hc = fl["h"].ravel()
+    Fx = fl["F"][0].ravel()
+    expect_h = h if h <= 4 else 0
+    table = {2: A_nc, 3: A_nc, 4: A_nc * 0.421875, 0: 0.0}
+    for site, sign in ((x0, -1.0), (x0 + h, +1.0)):
+        assert hc[site] == expect_h
+        assert abs(Fx[site] - 0.5 * table[expect_h] * Gx[site]) < 1e-17
+        if expect_h:
+            assert np.sign(Fx[site]) == sign                 # away from the film
+    # sites deep in a phase (|phi| >= phi_c) feel nothing
+    assert np.abs(Fx[np.abs(phi) >= 0.9]).max() == 0
+
+
+def test_P10_wall_blocks_probe(lbo):
+    """A solid node on the probe path means no contact (G10)."""
+    nx = 32
+    phi = np.ones(nx)
+    x0 = 10
+    phi[x0], phi[x0 + 1], phi[x0 + 2], phi[x0 + 3] = 0.5, -0.8, -0.8, 0.5
+    solid = np.zeros(nx, bool)
+    o = lbo.Oracle(nx, 1, 1, 1.0, 1.0, 0.01, 0.7, 0.02)
+    solid[x0 + 2] = True
+    o.set_geometry(solid.reshape(1, 1, nx))
+    p3 = phi.reshape(1, 1, nx)
+    o.init((1 + p3) / 2, (1 - p3) / 2, np.zeros((3, 1, 1, nx)))
+    fl = o.get_fields()
+    assert fl["h"].ravel()[x0] == 0 and fl["F"][0].ravel()[x0] == 0
+
+
+# ---------------------------------------------------------------------------------- P11
+def _transform(f, perm_axes, mirror_x):
+    """Apply x->y->z->x rotation (perm_axes) then mirror x to a [19, nz, ny, nx] array."""
+    out = f
+    cmap = tw.C.copy()
+    if perm_axes:
+        # new coordinates (x', y', z') = (z, x, y): array axes [z', y', x'] = [y, x, z]
+        out = np.transpose(out, (0, 2, 3, 1))
+        cmap = cmap[:, [2, 0, 1]]
+    if mirror_x:
+        out = out[..., ::-1]
+        cmap = cmap * np.array([-1, 1, 1])
+    idx = [int(np.where((tw.C == cmap[i]).all(1))[0][0]) for i in range(19)]
+    res = np.empty_like(out)
+    for i in range(19):
+        res[idx[i]] = out[i]
+    return np.ascontiguousarray(res)
+
+
+def _transform_scalar(a, perm_axes, mirror_x):
+    out = a
+    if perm_axes:
+        out = np.transpose(out, (1, 2, 0))
+    if mirror_x:
+        out = out[..., ::-1]
+    return np.ascontiguousarray(out)
+
+
+def test_P11_lattice_symmetry(lbo):
+    """One step commutes with a rotation of the axes and a mirror (index order N4, S2, S9)."""
+    nx, ny, nz = 6, 5, 4
+    rng = np.random.default_rng(11)
+    solid = np.zeros((nz, ny, nx), bool)
+    solid[:, 0, :] = True
+    solid[2, 3, 4] = True
+    fr = tw.equilibrium(rng.uniform(0.1, 0.9, (nz, ny, nx)), 0.02 * rng.normal(size=(3, nz, ny, nx)))
+    fb = tw.equilibrium(rng.uniform(0.1, 0.9, (nz, ny, nx)), 0.02 * rng.normal(size=(3, nz, ny, nx)))
+    fr *= ~solid
+    fb *= ~solid
+    g = np.array([1e-4, -2e-4, 3e-4])
+
+    def run(fr_, fb_, solid_, g_):
+        sz, sy, sx = solid_.shape
+        o = lbo.Oracle(sx, sy, sz, 0.8, 1.1, 0.01, 0.7, 0.02)
+        o.set_geometry(solid_)
+        o.set_body_force(*g_)
+        o.init(np.ones(solid_.shape), np.ones(solid_.shape), np.zeros((3,) + solid_.shape))
+        o.set_populations(0, fr_)
+        o.set_populations(1, fb_)
+        o.step(1)
+        return o.get_populations(0), o.get_populations(1)
+
+    a_r, a_b = run(fr, fb, solid, g)
+    g_t = g[[2, 0, 1]] * np.array([-1, 1, 1])
+    b_r, b_b = run(_transform(fr, True, True), _transform(fb, True, True),
+                   _transform_scalar(solid, True, True), g_t)
+    assert np.abs(_transform(a_r, True, True) - b_r).max() < 1e-13
+    assert np.abs(_transform(a_b, True, True) - b_b).max() < 1e-13
+    assert np.abs(a_r - fr).max() > 1e-4
+
+
+# ---------------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("shape,walls", [((4, 4, 4), False), ((6, 5, 4), True)])
+def test_P12_brute_force_numpy_twin(lbo, shape, walls):
+    """All of S1-S9 (both taus, force, near-contact probe, bounce-back) against the numpy
+    restatement in tests/np_twin.py, 10 steps, every population, 1e-13."""
+    nx, ny, nz = shape
+    rng = np.random.default_rng(12 + nx)
+    solid = np.zeros((nz, ny, nx), bool)
+    if walls:
+        solid[:, 0, :] = True
+        solid[1, 2, 3] = True
+    par = dict(tau_r=0.8, tau_b=1.2, A=0.01, beta=0.7, A_nc=0.02)
+    g = (1e-4, -5e-5, 2e-5)
+    rho_r = rng.uniform(0.2, 0.8, (nz, ny, nx))
+    rho_b = rng.uniform(0.2, 0.8, (nz, ny, nx))
+    u = 0.02 * rng.normal(size=(3, nz, ny, nx))
+    o = lbo.Oracle(nx, ny, nz, **par)
+    o.set_geometry(solid)
+    o.set_body_force(*g)
+    o.init(rho_r, rho_b, u)
+    fr = tw.equilibrium(rho_r, u) * ~solid
+    fb = tw.equilibrium(rho_b, u) * ~solid
+    assert np.abs(o.get_populations(0) - fr).max() < 1e-16
+    contacts = 0
+    for _ in range(10):
+        contacts += int((o.get_fields()["h"] > 0).sum())
+        fr, fb = tw.step(fr, fb, solid, g=g, **par)
+        o.step(1)
+        assert np.abs(o.get_populations(0) - fr).max() < 1e-13
+        assert np.abs(o.get_populations(1) - fb).max() < 1e-13
+    assert contacts > 0                                        # the probe did fire
+
+
+# ---------------------------------------------------------------------------------- P13
+def test_P13_taylor_green_decay(lbo):
+    """Config C2 at 64^3 (viscous regime): kinetic energy at t = 200 is
+    E0 exp(-6 nu k0^2 t) = 0.680 E0 with nu = 1/30 (Eq. 4 with tau = 0.6), within 5 %."""
+    n = 64
+    z, y, x = np.meshgrid(*(2 * np.pi * np.arange(n) / n,) * 3, indexing="ij")
+    u = np.zeros((3, n, n, n))
+    u[0] = 0.02 * np.sin(x) * np.cos(y) * np.cos(z)
+    u[1] = -0.02 * np.cos(x) * np.sin(y) * np.cos(z)
+    o = lbo.Oracle(n, n, n, 0.6, 0.6)
+    o.init(np.ones((n, n, n)), None, u)
+    rho, _, uu = o.get_macros()
+    e0 = (rho * (uu ** 2).sum(0)).sum()
+    o.step(200)
+    rho, _, uu = o.get_macros()
+    e1 = (rho * (uu ** 2).sum(0)).sum()
+    expect = np.exp(-6 * (1 / 30) * (2 * np.pi / n) ** 2 * 200)
+    assert abs(expect - 0.680) < 1e-3
+    assert abs(e1 / e0 - expect) / expect < 0.05
