@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- GLUPS of the two-component colour-gradient D3Q19 hot path on B200.
+
+One "step" is one LB time step of the whole box: the phase-field kernel K1 plus the fused
+stream-collide kernel K2 (every row A0-A10 of the hot path).  Prints ONE JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c5|c4|c2|c1] [--storage ab|aa]
+  python bench.py --impl reference ...     # the fp64 CPU oracle on this box's host cores
+
+N > 1 (torchrun): the path does not shard in this build ("replicas only"): every
+rank advances its own box; value = N * sites * K / max-over-ranks time; no collective is on
+the data path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "GLUPS (two-component D3Q19 site updates/s)"
+BYTES_PER_UPDATE = {True: 2 * 2 * 19 * 4, False: 2 * 19 * 4}   # two-component 304 B, single 152 B
+FALLBACK_HBM_GBS = 6650.0
+
+
+# ------------------------------------------------------------------------------ helpers
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def max_over_ranks(value, world, device=None):
+    """MAX of a python float over all ranks (torch.distributed, any backend)."""
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def glups(sites_per_rank, steps, seconds, world):
+    """Whole-job throughput: all ranks' site updates over the max-over-ranks time."""
+    return world * sites_per_rank * steps / seconds / 1e9
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def stored_traffic(kernel="k_fused"):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc = index, None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+        return self
+
+    def __exit__(self, *a):
+        self.result = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if not self.proc:
+            return
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            out = self.proc.communicate(timeout=5)[0]
+        except Exception:
+            return
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            p = [s.strip() for s in line.split(",")]
+            if len(p) < 6:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, p[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if sm:
+            self.result = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons)}
+
+
+def config_of(w, storage, extra=None):
+    c = {"workload": w.name, "box": [w.nx, w.ny, w.nz], "sites": w.sites, "fluid_sites": w.fluid_sites,
+         "components": 2 if w.rho_b is not None else 1, "near_contact": bool(w.A_nc != 0.0),
+         "walls": w.solid is not None, "storage": storage,
+         "params": dict(tau_r=w.tau_r, tau_b=w.tau_b, A=w.A, beta=w.beta, A_nc=w.A_nc, g=list(w.g)),
+         "l2": "state (%.2f GB) is larger than L2, no flush needed" % (w.sites * 4 * (38 if w.rho_b is not None else 19) * (2 if storage == "ab" else 1) / 1e9)}
+    c.update(w.info)
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ------------------------------------------------------------------------------ oracle legs
+def oracle_sample_workload(name, budget_updates):
+    """The same recipe as the timed workload at the largest cubic size whose (steps x sites)
+    fits the CPU budget."""
+    from paper_2005_12764_b200 import workloads as W
+    def make(n):
+        if name == "c2":
+            return W.c2_taylor_green(n)
+        if name == "c4":
+            return W.c4_channel(4 * n, n, n, R=10.0 if n >= 64 else 6.0)
+        if name == "c5":
+            return W.c5_emulsion(n, max(1, int(3000 * (n / 640.0) ** 3)))
+        if name == "c1":
+            return W.c1_droplet()
+        return W.c3_spinodal(n)
+    best = 32
+    for n in (32, 48, 64, 96, 128, 160):
+        sites = n ** 3 * (4 if name == "c4" else 1)
+        if sites <= budget_updates:
+            best = n
+    return make(best)
+
+
+def time_oracle(w, steps, warmup):
+    from oracle import lbo
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    if w.solid is not None:
+        o.set_geometry(w.solid)
+    o.set_body_force(*w.g)
+    o.set_nc_cutoff(w.phi_c)
+    o.init(w.rho_r, w.rho_b, w.u)
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    return time.perf_counter() - t0
+
+
+def omp_threads():
+    try:
+        return int(os.environ.get("OMP_NUM_THREADS", "")) 
+    except ValueError:
+        return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+def cpu_baseline(name, seconds_budget=15.0):
+    """The oracle as it stands on this box's host cores, on a bounded sample of the workload."""
+    w = oracle_sample_workload(name, budget_updates=2.2e6)
+    steps = 4
+    dt = time_oracle(w, steps, 1)
+    rate = w.fluid_sites * steps / dt
+    more = int(max(0, min(60, (seconds_budget - dt) * rate / w.fluid_sites)))
+    if more >= 4:
+        dt = time_oracle(w, more, 1)
+        steps = more
+    return {"value": w.fluid_sites * steps / dt / 1e9, "unit": "GLUPS", "cores": omp_threads(), "kind": "oracle",
+            "sample": "%s at %dx%dx%d (same recipe, smaller box), %d steps, fp64, OpenMP" % (w.name, w.nx, w.ny, w.nz, steps)}
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    total = max(1, args.steps + args.warmup)
+    w = oracle_sample_workload(args.workload, budget_updates=4.0e6 * 120.0 / total)
+    dt = time_oracle(w, args.steps, args.warmup)
+    val = w.fluid_sites * args.steps / dt / 1e9
+    sample = "%s at %dx%dx%d (same recipe, smaller box), %d steps, fp64, OpenMP" % (w.name, w.nx, w.ny, w.nz, args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GLUPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_of(w, "oracle", {"note": "bounded sample of workload %s" % args.workload}),
+            "cpu_baseline": {"value": val, "unit": "GLUPS", "cores": omp_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "GLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------ GPU arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1 and not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2005_12764_b200 import lb, workloads as W
+
+    w = W.get(args.workload)
+    two = w.rho_b is not None
+    K, Wu = args.steps, args.warmup
+
+    # inputs resident in HBM before the timed region
+    d_rr = torch.from_numpy(w.rho_r).to(dev)
+    d_rb = torch.from_numpy(w.rho_b).to(dev) if two else None
+    d_u = torch.from_numpy(w.u).to(dev)
+    sim = lb.from_workload(w, storage=args.storage)
+    sim.init(d_rr, d_rb, d_u)
+    sim.set_profiling(True)
+    sim.step(Wu)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    l0 = sim.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        torch.cuda.synchronize()
+        ev0.record()
+        sim.step(K)
+        ev1.record()
+        torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = sim.launch_count() - l0
+    ms = ev0.elapsed_time(ev1)
+    ms_k2 = sim.last_step_ms(1)
+    ms_k1 = sim.last_step_ms(2) if two else 0.0
+    ms_max = max_over_ranks(ms, world, dev)
+    value = glups(w.fluid_sites, K, ms_max * 1e-3, world)
+
+    # sanity: the state is finite and mass is where it was
+    rr, rb, u = sim.get_macros()
+    mass = float(np.sum(rr, dtype=np.float64))
+    mass0 = float(np.sum(w.rho_r if w.solid is None else w.rho_r * (w.solid == 0), dtype=np.float64))
+    finite = bool(np.isfinite(u).all())
+
+    # end to end through the C-ABI with HOST buffers: init (H2D) + K steps + get_macros (D2H)
+    h_rr = torch.from_numpy(w.rho_r).pin_memory()
+    h_rb = torch.from_numpy(w.rho_b).pin_memory() if two else None
+    h_u = torch.from_numpy(w.u).pin_memory()
+    o_rr, o_u = torch.empty_like(h_rr).pin_memory(), torch.empty_like(h_u).pin_memory()
+    o_rb = torch.empty_like(h_rb).pin_memory() if two else None
+    sim.set_profiling(False)
+    e2e_ms = []
+    for _ in range(2):          # first pass warms the staging allocations
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        sim.init(h_rr, h_rb, h_u)
+        sim.step(K)
+        sim.get_macros(o_rr, o_rb, o_u)
+        torch.cuda.synchronize()
+        e2e_ms.append((time.perf_counter() - t0) * 1e3)
+    e2e_max = max_over_ranks(e2e_ms[-1], world, dev)
+    nfield = (5 if two else 4) * w.sites * 4
+    e2e = {"value": glups(w.fluid_sites, K, e2e_max * 1e-3, world), "unit": "GLUPS",
+           "h2d_bytes_per_step": nfield / K, "d2h_bytes_per_step": nfield / K,
+           "note": "lb_init(host) + lb_step(%d) + lb_get_macros(host) per timed region; bytes are totals / K" % K}
+
+    if rank != 0:
+        return 0
+    peak, peak_src = measured_peak()
+    upd_bytes = BYTES_PER_UPDATE[two]
+    k2_s = ms_k2 * 1e-3 / K
+    achieved = upd_bytes * w.fluid_sites / k2_s / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_fused" if two else "k_single", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic("k_fused" if two else "k_single"),
+                "peak_source": peak_src, "algorithmic_bytes_per_update": upd_bytes,
+                "kernel_ms": ms_k2 / K, "kernel_share_of_step": ms_k2 / ms,
+                "phase_kernel_ms": ms_k1 / K,
+                "whole_step_effective_gbs": upd_bytes * w.fluid_sites * K / (ms * 1e-3) / 1e9,
+                "whole_step_frac": upd_bytes * w.fluid_sites * K / (ms * 1e-3) / 1e9 / peak}
+    line = {"metric": METRIC, "value": value, "unit": "GLUPS", "n_gpus": world, "steps": K, "warmup": Wu,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": config_of(w, args.storage, {"parallelism": "replicas x%d" % world}),
+            "clocks": clk.result, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "checks": {"finite": finite, "red_mass_rel_drift": abs(mass - mass0) / mass0}}
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(args.workload)
+    elif world > 1:
+        line["cpu_baseline"] = None
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini"])
+    ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

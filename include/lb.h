@@ -1,0 +1,137 @@
+/* lb.h -- C-ABI boundary of the B200-native two-component colour-gradient D3Q19 lattice
+ * Boltzmann hot path (arxiv 2005.12764, "Towards Exascale Design of Soft Mesoscale Materials").
+ *
+ * Citations are to /root/reference/PAPER.md (line, equation).  Where the paper is silent the
+ * reading is one of G1-G24 in DESIGN.md.
+ *
+ * The problem, as the paper states it: two sets of populations f^r_i, f^b_i on a D3Q19 lattice
+ * advance by collide-and-stream (Eq. 1; Eq. 5-6)
+ * with a common velocity and a mixture relaxation rate (Eq. 7-8), under a
+ * source term S_i carrying body and near-contact forces (Eq. 11),
+ * between bounce-back walls with one periodic axis.
+ *
+ * Conventions for every call
+ *   layout      scalar fields are [z][y][x], x fastest: index x + nx*(y + ny*z).  u is three such
+ *               planes [3][z][y][x].  Populations are [19][z][y][x] in the velocity order below.
+ *   pointers    every array argument may be a HOST or a DEVICE pointer (detected with
+ *               cudaPointerGetAttributes); host arrays are staged through a temporary device
+ *               buffer.  The caller owns every array it passes; the handle owns all device state.
+ *   stream      all work is enqueued on the handle's stream (lb_set_stream; default stream 0).
+ *               lb_step is asynchronous.  Calls that write to host memory synchronise the
+ *               stream before returning.
+ *   time        after lb_init the state is t = 0, after lb_step(n) it is t = n.  "The state at t"
+ *               is the set of pre-collision populations f^k_i(x, t) (those that have arrived at x).
+ *   errors      0 on success, negative LB_E* otherwise; text via lb_last_error.  Nothing throws,
+ *               nothing aborts.  There is no CPU fallback: without a CUDA device every call that
+ *               touches the device returns LB_ECUDA.
+ *
+ * Velocity order (free in the paper, which numbers i = 1..19):
+ *   0:(0,0,0) 1:(+1,0,0) 2:(-1,0,0) 3:(0,+1,0) 4:(0,-1,0) 5:(0,0,+1) 6:(0,0,-1)
+ *   7:(+1,+1,0) 8:(-1,-1,0) 9:(+1,-1,0) 10:(-1,+1,0) 11:(+1,0,+1) 12:(-1,0,-1)
+ *   13:(+1,0,-1) 14:(-1,0,+1) 15:(0,+1,+1) 16:(0,-1,-1) 17:(0,+1,-1) 18:(0,-1,+1)
+ */
+#ifndef LB_B200_H
+#define LB_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LB_OK 0
+#define LB_EINVAL (-1) /* bad size, NULL where not allowed, tau <= 0.5, nx not a multiple of 4 */
+#define LB_ENOMEM (-2) /* device allocation failed */
+#define LB_ECUDA (-3)  /* a CUDA call failed (or there is no device) */
+#define LB_ESTATE (-4) /* call out of order: step before init, set_geometry after init, ... */
+
+/* tau_k: relaxation times, omega_k = 1/tau_k, nu_k = (tau_k - 1/2)/3 (Eq. 4).
+ * A: strength of the colour-gradient surface-tension perturbation (sigma ~ 4/9 A tau).
+ * beta: Latva-Kokko recolouring strength.  A_nc: near-contact strength, the constant "A" of
+ * A_h[h] in Eq. 11; 0 switches the near-contact force off. */
+typedef struct {
+  float tau_r, tau_b, A, beta, A_nc;
+} lb_params;
+
+typedef struct lb_handle_s* lb_handle;
+
+/* Device-memory hooks.  PyTorch is the allocator in production: the Python binding passes
+ * wrappers of torch's CUDA caching allocator.  alloc returns a device pointer or NULL.
+ * Process-wide; set before lb_create.  NULL, NULL restores cudaMalloc / cudaFree. */
+typedef void* (*lb_alloc_fn)(size_t bytes, void* user);
+typedef void (*lb_free_fn)(void* ptr, void* user);
+int lb_set_allocator(lb_alloc_fn alloc, lb_free_fn free_fn, void* user);
+
+/* Create a simulation on an nx x ny x nz box (all axes periodic in topology; walls are solid
+ * sites, see lb_set_geometry).  Requires nx % 4 == 0 and every extent >= 4; tau_k > 0.5.
+ * Allocates nothing large: population buffers are allocated by lb_init. */
+int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out);
+
+/* Frees all device state.  lb_destroy(NULL) is a no-op. */
+void lb_destroy(lb_handle h);
+
+/* CUDA stream (a cudaStream_t passed as void*) that all later work of this handle uses. */
+int lb_set_stream(lb_handle h, void* cuda_stream);
+
+/* Solid mask, S = nx*ny*nz bytes, 1 = solid, 0 = fluid; NULL = all fluid.  Stored bit-packed.
+ * Solid sites hold no populations; links into them bounce back half-way (G21).
+ * Must precede lb_init. */
+int lb_set_geometry(lb_handle h, const uint8_t* solid_mask);
+
+/* Uniform acceleration g: body force F = rho g enters through the source term. */
+int lb_set_body_force(lb_handle h, float gx, float gy, float gz);
+
+/* Near-contact force acts where |phi| < phi_c (default 0.9). */
+int lb_set_nc_cutoff(lb_handle h, float phi_c);
+
+/* Storage of the populations.  0 = A/B double buffer (default), 1 = AA-pattern, one buffer
+ * updated in place.  Must precede lb_init. */
+int lb_set_storage(lb_handle h, int mode);
+
+/* Initial state (t = 0): f^k_i = w_i rho_k [1 + 3 c.u + 4.5 (c.u)^2 - 1.5 u.u] with the common u
+ * (Eq. 2, per component as in Eq. 5-6).  rho_b == NULL selects
+ * the single-component BGK mode (config C2).  Input on solid sites is ignored.  Allocates the
+ * population buffers: 2 (A/B) or 1 (AA) x 38 (or 19) x S floats, plus the padded phi array. */
+int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u);
+
+/* Advance nsteps time steps: per step the phase-field kernel (rho_r, rho_b, phi; Eq. 3,
+ * PAPER.md:96) and the fused pull-stream + collide kernel (Eq. 1-2, 5-8, 11).  Asynchronous. */
+int lb_step(lb_handle h, int nsteps);
+
+/* rho_r, rho_b and the velocity u = (sum_i c_i f_i + F/2)/rho of the current state (Eq. 3,
+ * PAPER.md:96, with the half-force shift of Guo forcing; G16).  Zeros on solid sites.  Any
+ * output pointer may be NULL; rho_b is ignored in single-component mode.  Does not disturb
+ * the state. */
+int lb_get_macros(lb_handle h, float* rho_r, float* rho_b, float* u);
+
+/* Debug / checkpoint accessors: the full pre-collision populations f^comp_i(x, t), comp 0 = red,
+ * 1 = blue, 19*S floats.  Internally the state is stored as deviations;
+ * these calls convert.  lb_set_populations must be called for both components (red first)
+ * before the next lb_step; values on solid sites are ignored. */
+int lb_get_populations(lb_handle h, int comp, float* f);
+int lb_set_populations(lb_handle h, int comp, const float* f);
+
+/* phi = (rho_r - rho_b)/(rho_r + rho_b) of the current state, S floats (0 on solid sites). */
+int lb_get_phi(lb_handle h, float* phi);
+
+/* Number of kernel launches this handle has made so far (for the harness' gpu_launches). */
+long long lb_launch_count(lb_handle h);
+
+/* Bytes of device memory the handle currently owns. */
+size_t lb_device_bytes(lb_handle h);
+
+/* Last error text of this handle (or of the failed lb_create when h == NULL). */
+const char* lb_last_error(lb_handle h);
+
+/* Timing hook: an event pair recorded around the kernels of the LAST lb_step call, on the
+ * handle's stream; returns the elapsed milliseconds (synchronises on the end event).
+ * which: 0 = whole lb_step, 1 = sum over the fused stream-collide launches, 2 = sum over the
+ * phase-field launches.  which = 1, 2 are recorded only after lb_set_profiling(h, 1). */
+int lb_set_profiling(lb_handle h, int on);
+int lb_last_step_ms(lb_handle h, int which, float* ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LB_B200_H */

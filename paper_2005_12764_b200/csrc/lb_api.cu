@@ -1,0 +1,622 @@
+// C-ABI of the B200 colour-gradient LB hot path (include/lb.h).  Host logic only: argument
+// checks, device memory through the allocator hooks (PyTorch's caching allocator in
+// production), kernel launches on the handle's stream.  No CPU fallback of any step.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/lb.h"
+#include "lb_kernels.cuh"
+
+using namespace lb;
+
+namespace {
+
+lb_alloc_fn g_alloc = nullptr;
+lb_free_fn g_free = nullptr;
+void* g_user = nullptr;
+std::string g_create_error;
+
+void* dev_alloc(size_t bytes) {
+  if (g_alloc) return g_alloc(bytes, g_user);
+  void* p = nullptr;
+  if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return p;
+}
+void dev_free(void* p) {
+  if (!p) return;
+  if (g_free) g_free(p, g_user);
+  else cudaFree(p);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+}  // namespace
+
+struct lb_handle_s {
+  int nx = 0, ny = 0, nz = 0;
+  long long S = 0;
+  lb_params par{};
+  float g[3] = {0, 0, 0};
+  float phi_c = 0.9f;
+  int storage = 0;          // 0 A/B, 1 AA
+  bool two = true;
+  bool inited = false;
+  bool has_solid = false;
+  int aa_odd = 0;           // AA: is the next step the odd one?
+  int cur = 0;              // A/B: buffer holding the current state
+  float* buf[2] = {nullptr, nullptr};
+  float* phi = nullptr;
+  uint32_t* mask = nullptr;
+  size_t bytes = 0;
+  cudaStream_t stream = 0;
+  long long launches = 0;
+  CUtensorMap tmap{};
+  bool tmap_ok = false;
+  bool phi_current = false;  // phi array matches the current populations
+  int profiling = 0;
+  cudaEvent_t ev_step[2] = {nullptr, nullptr};
+  std::vector<cudaEvent_t> ev_k;   // 4 per step when profiling: K1 begin/end, K2 begin/end
+  int ev_steps = 0;
+  std::string err;
+
+  Box box() const {
+    Box b;
+    b.nx = nx; b.ny = ny; b.nz = nz;
+    b.nxw = (nx + 31) / 32;
+    b.S = S;
+    b.mask = has_solid ? mask : nullptr;
+    return b;
+  }
+  int planes() const { return two ? 2 * Q : Q; }
+  int mode() const { return storage == 0 ? MODE_AB : (aa_odd ? MODE_AA_ODD : MODE_AA_EVEN); }
+  float* cur_buf() const { return storage == 0 ? buf[cur] : buf[0]; }
+};
+
+namespace {
+
+int fail(lb_handle h, int code, const std::string& msg) {
+  if (h) h->err = msg;
+  else g_create_error = msg;
+  return code;
+}
+
+int cuda_fail(lb_handle h, cudaError_t e, const char* what) {
+  cudaGetLastError();
+  return fail(h, LB_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// A device view of a caller array: the pointer itself, or a staged copy of a host array.
+struct Staged {
+  void* dev = nullptr;
+  bool owned = false;
+  ~Staged() { if (owned) dev_free(dev); }
+};
+
+int stage_in(lb_handle h, const void* src, size_t bytes, Staged& s) {
+  if (is_device_ptr(src)) { s.dev = const_cast<void*>(src); return LB_OK; }
+  s.dev = dev_alloc(bytes);
+  if (!s.dev) return fail(h, LB_ENOMEM, "staging buffer allocation failed");
+  s.owned = true;
+  cudaError_t e = cudaMemcpyAsync(s.dev, src, bytes, cudaMemcpyHostToDevice, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "H2D copy");
+  return LB_OK;
+}
+
+// Output staging: device pointer as is, else a device temporary copied back by finish_out.
+int stage_out(lb_handle h, void* dst, size_t bytes, Staged& s) {
+  if (!dst) return LB_OK;
+  if (is_device_ptr(dst)) { s.dev = dst; return LB_OK; }
+  s.dev = dev_alloc(bytes);
+  if (!s.dev) return fail(h, LB_ENOMEM, "staging buffer allocation failed");
+  s.owned = true;
+  return LB_OK;
+}
+int finish_out(lb_handle h, void* dst, size_t bytes, Staged& s) {
+  if (!dst || !s.owned) return LB_OK;
+  cudaError_t e = cudaMemcpyAsync(dst, s.dev, bytes, cudaMemcpyDeviceToHost, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "D2H copy");
+  return LB_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------ launches
+namespace {
+
+StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
+  StepParams p;
+  p.src = src; p.dst = dst; p.phi = h->phi;
+  p.box = h->box();
+  p.zc = zc;
+  p.halo = h->par.A_nc != 0.f ? H_MAX_NC : 1;
+  p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
+  p.A_nc = h->par.A_nc; p.phi_c = h->phi_c;
+  p.gx = h->g[0]; p.gy = h->g[1]; p.gz = h->g[2];
+  p.two_tau = h->par.tau_r != h->par.tau_b;
+  p.has_g = (h->g[0] != 0.f || h->g[1] != 0.f || h->g[2] != 0.f);
+  return p;
+}
+
+// z planes per CTA: enough CTAs for ~8 waves of 148 SMs x 4 resident CTAs, at least 8 planes
+// so that the phi-ring prologue (2H+1 planes) is amortised.
+int pick_zc(lb_handle h) {
+  const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
+  const long long want = 148LL * 4 * 8;
+  long long zsplit = (want + cols - 1) / cols;
+  if (zsplit < 1) zsplit = 1;
+  int zc = (int)((h->nz + zsplit - 1) / zsplit);
+  const int zmin = h->par.A_nc != 0.f ? 16 : 8;
+  if (zc < zmin) zc = zmin;
+  if (zc > h->nz) zc = h->nz;
+  return zc;
+}
+
+dim3 tile_grid(lb_handle h, int zc) {
+  return dim3((h->nx + TX - 1) / TX, (h->ny + TY - 1) / TY, (h->nz + zc - 1) / zc);
+}
+
+template <int MODE>
+void launch_phase(lb_handle h, const StepParams& p, dim3 grid) {
+  if (h->has_solid) k_phase<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+  else k_phase<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+}
+template <int MODE>
+void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
+  const bool nc = h->par.A_nc != 0.f;
+  const dim3 blk(TX, TY);
+  if (h->has_solid) {
+    if (nc) k_fused<MODE, true, true><<<grid, blk, 0, h->stream>>>(p, h->tmap);
+    else k_fused<MODE, true, false><<<grid, blk, 0, h->stream>>>(p, h->tmap);
+  } else {
+    if (nc) k_fused<MODE, false, true><<<grid, blk, 0, h->stream>>>(p, h->tmap);
+    else k_fused<MODE, false, false><<<grid, blk, 0, h->stream>>>(p, h->tmap);
+  }
+}
+template <int MODE>
+void launch_single(lb_handle h, const StepParams& p, dim3 grid) {
+  if (h->has_solid) k_single<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+  else k_single<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+}
+
+// K1 on the current state (no-op if phi is already current or in single-component mode)
+void run_phase(lb_handle h) {
+  if (!h->two || h->phi_current) return;
+  const int zc = pick_zc(h);
+  const StepParams p = make_step_params(h, h->cur_buf(), nullptr, zc);
+  const dim3 grid = tile_grid(h, zc);
+  switch (h->mode()) {
+    case MODE_AB: launch_phase<MODE_AB>(h, p, grid); break;
+    case MODE_AA_EVEN: launch_phase<MODE_AA_EVEN>(h, p, grid); break;
+    default: launch_phase<MODE_AA_ODD>(h, p, grid); break;
+  }
+  h->launches++;
+  h->phi_current = true;
+}
+
+// K2 / K2s: advance one step and flip the buffer / parity
+void run_collide(lb_handle h) {
+  const int zc = pick_zc(h);
+  const dim3 grid = tile_grid(h, zc);
+  float* src = h->cur_buf();
+  float* dst = h->storage == 0 ? h->buf[h->cur ^ 1] : h->buf[0];
+  const StepParams p = make_step_params(h, src, dst, zc);
+  const int mode = h->mode();
+  if (h->two) {
+    if (mode == MODE_AB) launch_fused<MODE_AB>(h, p, grid);
+    else if (mode == MODE_AA_EVEN) launch_fused<MODE_AA_EVEN>(h, p, grid);
+    else launch_fused<MODE_AA_ODD>(h, p, grid);
+  } else {
+    if (mode == MODE_AB) launch_single<MODE_AB>(h, p, grid);
+    else if (mode == MODE_AA_EVEN) launch_single<MODE_AA_EVEN>(h, p, grid);
+    else launch_single<MODE_AA_ODD>(h, p, grid);
+  }
+  h->launches++;
+  if (h->storage == 0) h->cur ^= 1;
+  else h->aa_odd ^= 1;
+  h->phi_current = false;
+}
+
+IoParams make_io_params(lb_handle h) {
+  IoParams p;
+  memset(&p, 0, sizeof(p));
+  p.buf = h->cur_buf();
+  p.box = h->box();
+  p.two = h->two;
+  p.phi = h->phi;
+  p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
+  p.A_nc = h->par.A_nc; p.phi_c = h->phi_c;
+  p.gx = h->g[0]; p.gy = h->g[1]; p.gz = h->g[2];
+  return p;
+}
+
+void launch_scatter(lb_handle h, const IoParams& p) {
+  const int tb = 256;
+  const unsigned nb = (unsigned)((h->S + tb - 1) / tb);
+  switch (h->mode()) {
+    case MODE_AB: k_scatter<MODE_AB><<<nb, tb, 0, h->stream>>>(p); break;
+    case MODE_AA_EVEN: k_scatter<MODE_AA_EVEN><<<nb, tb, 0, h->stream>>>(p); break;
+    default: k_scatter<MODE_AA_ODD><<<nb, tb, 0, h->stream>>>(p); break;
+  }
+  h->launches++;
+}
+void launch_gatherf(lb_handle h, const IoParams& p) {
+  const int tb = 256;
+  const unsigned nb = (unsigned)((h->S + tb - 1) / tb);
+  switch (h->mode()) {
+    case MODE_AB: k_gatherf<MODE_AB><<<nb, tb, 0, h->stream>>>(p); break;
+    case MODE_AA_EVEN: k_gatherf<MODE_AA_EVEN><<<nb, tb, 0, h->stream>>>(p); break;
+    default: k_gatherf<MODE_AA_ODD><<<nb, tb, 0, h->stream>>>(p); break;
+  }
+  h->launches++;
+}
+void launch_macros(lb_handle h, const IoParams& p) {
+  const int tb = 256;
+  const unsigned nb = (unsigned)((h->S + tb - 1) / tb);
+  switch (h->mode()) {
+    case MODE_AB: k_macros<MODE_AB><<<nb, tb, 0, h->stream>>>(p); break;
+    case MODE_AA_EVEN: k_macros<MODE_AA_EVEN><<<nb, tb, 0, h->stream>>>(p); break;
+    default: k_macros<MODE_AA_ODD><<<nb, tb, 0, h->stream>>>(p); break;
+  }
+  h->launches++;
+}
+
+int check_launch(lb_handle h, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, LB_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  return LB_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------ C-ABI
+extern "C" {
+
+int lb_set_allocator(lb_alloc_fn alloc, lb_free_fn free_fn, void* user) {
+  if ((alloc == nullptr) != (free_fn == nullptr)) return LB_EINVAL;
+  g_alloc = alloc; g_free = free_fn; g_user = user;
+  return LB_OK;
+}
+
+int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
+  if (!out) return fail(nullptr, LB_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!p) return fail(nullptr, LB_EINVAL, "params is NULL");
+  if (nx < 4 || ny < 4 || nz < 4) return fail(nullptr, LB_EINVAL, "every extent must be >= 4");
+  if (nx % 4 != 0) return fail(nullptr, LB_EINVAL, "nx must be a multiple of 4");
+  if ((long long)nx * ny * nz >= (1LL << 31)) return fail(nullptr, LB_EINVAL, "box too large (>= 2^31 sites)");
+  if (!(p->tau_r > 0.5f) || !(p->tau_b > 0.5f)) return fail(nullptr, LB_EINVAL, "tau must exceed 0.5");
+  lb_handle h = new (std::nothrow) lb_handle_s();
+  if (!h) return fail(nullptr, LB_ENOMEM, "host allocation failed");
+  h->nx = nx; h->ny = ny; h->nz = nz;
+  h->S = (long long)nx * ny * nz;
+  h->par = *p;
+  *out = h;
+  return LB_OK;
+}
+
+void lb_destroy(lb_handle h) {
+  if (!h) return;
+  if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
+  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->mask);
+  for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
+  for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
+  cudaGetLastError();
+  delete h;
+}
+
+int lb_set_stream(lb_handle h, void* cuda_stream) {
+  if (!h) return LB_EINVAL;
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  return LB_OK;
+}
+
+int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
+  if (!h) return LB_EINVAL;
+  if (h->inited) return fail(h, LB_ESTATE, "lb_set_geometry after lb_init");
+  if (!solid_mask) { h->has_solid = false; return LB_OK; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(h, LB_ECUDA, "no CUDA device (there is no CPU fallback)");
+  }
+  Box b = h->box();
+  const size_t nwords = (size_t)b.nxw * h->ny * h->nz;
+  if (!h->mask) {
+    h->mask = static_cast<uint32_t*>(dev_alloc(nwords * 4));
+    if (!h->mask) return fail(h, LB_ENOMEM, "mask allocation failed");
+    h->bytes += nwords * 4;
+  }
+  Staged in;
+  int rc = stage_in(h, solid_mask, (size_t)h->S, in);
+  if (rc) return rc;
+  const int tb = 256;
+  k_pack_mask<<<(unsigned)((nwords + tb - 1) / tb), tb, 0, h->stream>>>(static_cast<const uint8_t*>(in.dev), h->mask, b);
+  h->launches++;
+  rc = check_launch(h, "k_pack_mask");
+  if (rc) return rc;
+  cudaError_t e = cudaStreamSynchronize(h->stream);   // the staged copy dies with `in`
+  if (e != cudaSuccess) return cuda_fail(h, e, "lb_set_geometry");
+  h->has_solid = true;
+  return LB_OK;
+}
+
+int lb_set_body_force(lb_handle h, float gx, float gy, float gz) {
+  if (!h) return LB_EINVAL;
+  h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
+  return LB_OK;
+}
+
+int lb_set_nc_cutoff(lb_handle h, float phi_c) {
+  if (!h) return LB_EINVAL;
+  h->phi_c = phi_c;
+  return LB_OK;
+}
+
+int lb_set_storage(lb_handle h, int mode) {
+  if (!h || (mode != 0 && mode != 1)) return fail(h, LB_EINVAL, "storage mode must be 0 (A/B) or 1 (AA)");
+  if (h->inited) return fail(h, LB_ESTATE, "lb_set_storage after lb_init");
+  h->storage = mode;
+  return LB_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// (Re)allocate population buffers, the padded phi array and its TMA descriptor.
+int allocate_state(lb_handle h, bool two) {
+  const int nbuf = h->storage == 0 ? 2 : 1;
+  const int planes = two ? 2 * Q : Q;
+  const size_t pbytes = (size_t)planes * (size_t)h->S * sizeof(float);
+  if (h->inited && two != h->two) {   // component count changed: start over
+    for (int i = 0; i < 2; ++i) { if (h->buf[i]) h->bytes -= (size_t)h->planes() * h->S * 4; dev_free(h->buf[i]); h->buf[i] = nullptr; }
+  }
+  h->two = two;
+  for (int i = 0; i < nbuf; ++i) {
+    if (!h->buf[i]) {
+      h->buf[i] = static_cast<float*>(dev_alloc(pbytes));
+      if (!h->buf[i]) return fail(h, LB_ENOMEM, "population buffer allocation failed");
+      h->bytes += pbytes;
+    }
+  }
+  if (two && !h->phi) {
+    const size_t px = h->nx + 2 * HALO, py = h->ny + 2 * HALO, pz = h->nz + 2 * HALO;
+    const size_t phib = px * py * pz * sizeof(float);
+    h->phi = static_cast<float*>(dev_alloc(phib));
+    if (!h->phi) return fail(h, LB_ENOMEM, "phi allocation failed");
+    h->bytes += phib;
+    cudaError_t e = cudaMemsetAsync(h->phi, 0, phib, h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "phi memset");
+    // TMA descriptor of the padded phi array: dims (x, y, z), box (BX, BY, 1)
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return fail(h, LB_ECUDA, "cuTensorMapEncodeTiled entry point not found");
+    const bool nc = h->par.A_nc != 0.f;
+    cuuint64_t dims[3] = {px, py, pz};
+    cuuint64_t strides[2] = {px * sizeof(float), px * py * sizeof(float)};
+    cuuint32_t box[3] = {(cuuint32_t)(nc ? Ring<H_MAX_NC>::BX : Ring<1>::BX),
+                         (cuuint32_t)(nc ? Ring<H_MAX_NC>::BY : Ring<1>::BY), 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(&h->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, h->phi, dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(h, LB_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
+    h->tmap_ok = true;
+  }
+  return LB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u) {
+  if (!h) return LB_EINVAL;
+  if (!rho_r || !u) return fail(h, LB_EINVAL, "rho_r and u must not be NULL");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(h, LB_ECUDA, "no CUDA device (there is no CPU fallback)");
+  }
+  int rc = allocate_state(h, rho_b != nullptr);
+  if (rc) return rc;
+  const size_t fb = (size_t)h->S * sizeof(float);
+  Staged srr, srb, su;
+  if ((rc = stage_in(h, rho_r, fb, srr))) return rc;
+  if (rho_b && (rc = stage_in(h, rho_b, fb, srb))) return rc;
+  if ((rc = stage_in(h, u, 3 * fb, su))) return rc;
+  h->cur = 0;
+  h->aa_odd = 0;
+  IoParams p = make_io_params(h);
+  p.comp = -1;
+  p.rho_r = static_cast<const float*>(srr.dev);
+  p.rho_b = static_cast<const float*>(srb.dev);
+  p.u = static_cast<const float*>(su.dev);
+  // solid sites keep zeros so that stray reads are harmless
+  cudaError_t e = cudaMemsetAsync(h->cur_buf(), 0, (size_t)h->planes() * fb, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "population memset");
+  launch_scatter(h, p);
+  if ((rc = check_launch(h, "k_scatter"))) return rc;
+  h->inited = true;
+  h->phi_current = false;
+  if (srr.owned || srb.owned || su.owned) {
+    e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_init");
+  }
+  return LB_OK;
+}
+
+int lb_step(lb_handle h, int nsteps) {
+  if (!h || nsteps < 0) return fail(h, LB_EINVAL, "nsteps must be >= 0");
+  if (!h->inited) return fail(h, LB_ESTATE, "lb_step before lb_init");
+  for (int i = 0; i < 2; ++i)
+    if (!h->ev_step[i] && cudaEventCreate(&h->ev_step[i]) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
+  const bool prof = h->profiling != 0;
+  if (prof) {
+    while ((int)h->ev_k.size() < 4 * nsteps) {
+      cudaEvent_t e;
+      if (cudaEventCreate(&e) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
+      h->ev_k.push_back(e);
+    }
+  }
+  h->ev_steps = prof ? nsteps : 0;
+  cudaEventRecord(h->ev_step[0], h->stream);
+  for (int t = 0; t < nsteps; ++t) {
+    if (prof) cudaEventRecord(h->ev_k[4 * t + 0], h->stream);
+    run_phase(h);
+    if (prof) { cudaEventRecord(h->ev_k[4 * t + 1], h->stream); cudaEventRecord(h->ev_k[4 * t + 2], h->stream); }
+    run_collide(h);
+    if (prof) cudaEventRecord(h->ev_k[4 * t + 3], h->stream);
+  }
+  cudaEventRecord(h->ev_step[1], h->stream);
+  return check_launch(h, "lb_step");
+}
+
+int lb_get_macros(lb_handle h, float* rho_r, float* rho_b, float* u) {
+  if (!h) return LB_EINVAL;
+  if (!h->inited) return fail(h, LB_ESTATE, "lb_get_macros before lb_init");
+  const size_t fb = (size_t)h->S * sizeof(float);
+  Staged o0, o1, o2;
+  int rc;
+  if ((rc = stage_out(h, rho_r, fb, o0))) return rc;
+  if (h->two && (rc = stage_out(h, rho_b, fb, o1))) return rc;
+  if ((rc = stage_out(h, u, 3 * fb, o2))) return rc;
+  run_phase(h);
+  IoParams p = make_io_params(h);
+  p.out0 = static_cast<float*>(o0.dev);
+  p.out1 = static_cast<float*>(o1.dev);
+  p.out2 = static_cast<float*>(o2.dev);
+  launch_macros(h, p);
+  if ((rc = check_launch(h, "k_macros"))) return rc;
+  if ((rc = finish_out(h, rho_r, fb, o0))) return rc;
+  if (h->two && (rc = finish_out(h, rho_b, fb, o1))) return rc;
+  if ((rc = finish_out(h, u, 3 * fb, o2))) return rc;
+  if (o0.owned || o1.owned || o2.owned) {
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_get_macros");
+  }
+  return LB_OK;
+}
+
+int lb_get_populations(lb_handle h, int comp, float* f) {
+  if (!h || !f) return fail(h, LB_EINVAL, "f is NULL");
+  if (!h->inited) return fail(h, LB_ESTATE, "lb_get_populations before lb_init");
+  if (comp < 0 || comp > (h->two ? 1 : 0)) return fail(h, LB_EINVAL, "bad component");
+  const size_t fb = (size_t)Q * h->S * sizeof(float);
+  Staged o;
+  int rc;
+  if ((rc = stage_out(h, f, fb, o))) return rc;
+  IoParams p = make_io_params(h);
+  p.comp = comp;
+  p.out0 = static_cast<float*>(o.dev);
+  launch_gatherf(h, p);
+  if ((rc = check_launch(h, "k_gatherf"))) return rc;
+  if ((rc = finish_out(h, f, fb, o))) return rc;
+  if (o.owned) {
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_get_populations");
+  }
+  return LB_OK;
+}
+
+int lb_set_populations(lb_handle h, int comp, const float* f) {
+  if (!h || !f) return fail(h, LB_EINVAL, "f is NULL");
+  if (!h->inited) return fail(h, LB_ESTATE, "lb_set_populations before lb_init");
+  if (comp < 0 || comp > (h->two ? 1 : 0)) return fail(h, LB_EINVAL, "bad component");
+  const size_t fb = (size_t)Q * h->S * sizeof(float);
+  Staged in;
+  int rc;
+  if ((rc = stage_in(h, f, fb, in))) return rc;
+  if (comp == 0 && h->storage == 1) h->aa_odd = 0;   // AA: a full rewrite restores the natural layout
+  IoParams p = make_io_params(h);
+  p.comp = comp;
+  p.in0 = static_cast<const float*>(in.dev);
+  launch_scatter(h, p);
+  if ((rc = check_launch(h, "k_scatter"))) return rc;
+  h->phi_current = false;
+  if (in.owned) {
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_set_populations");
+  }
+  return LB_OK;
+}
+
+int lb_get_phi(lb_handle h, float* phi) {
+  if (!h || !phi) return fail(h, LB_EINVAL, "phi is NULL");
+  if (!h->inited || !h->two) return fail(h, LB_ESTATE, "lb_get_phi needs an initialised two-component state");
+  const size_t fb = (size_t)h->S * sizeof(float);
+  Staged o;
+  int rc;
+  if ((rc = stage_out(h, phi, fb, o))) return rc;
+  run_phase(h);
+  const int tb = 256;
+  k_unpad_phi<<<(unsigned)((h->S + tb - 1) / tb), tb, 0, h->stream>>>(h->phi, static_cast<float*>(o.dev), h->box());
+  h->launches++;
+  if ((rc = check_launch(h, "k_unpad_phi"))) return rc;
+  if ((rc = finish_out(h, phi, fb, o))) return rc;
+  if (o.owned) {
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_get_phi");
+  }
+  return LB_OK;
+}
+
+long long lb_launch_count(lb_handle h) { return h ? h->launches : 0; }
+size_t lb_device_bytes(lb_handle h) { return h ? h->bytes : 0; }
+const char* lb_last_error(lb_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int lb_set_profiling(lb_handle h, int on) {
+  if (!h) return LB_EINVAL;
+  h->profiling = on ? 1 : 0;
+  return LB_OK;
+}
+
+int lb_last_step_ms(lb_handle h, int which, float* ms) {
+  if (!h || !ms || which < 0 || which > 2) return fail(h, LB_EINVAL, "bad argument");
+  if (!h->ev_step[1]) return fail(h, LB_ESTATE, "no lb_step recorded yet");
+  cudaError_t e = cudaEventSynchronize(h->ev_step[1]);
+  if (e != cudaSuccess) return cuda_fail(h, e, "event sync");
+  if (which == 0) {
+    e = cudaEventElapsedTime(ms, h->ev_step[0], h->ev_step[1]);
+    if (e != cudaSuccess) return cuda_fail(h, e, "event elapsed");
+    return LB_OK;
+  }
+  if (h->ev_steps == 0) return fail(h, LB_ESTATE, "profiling was off during the last lb_step");
+  float total = 0.f;
+  for (int t = 0; t < h->ev_steps; ++t) {
+    float v = 0.f;
+    const int a = which == 1 ? 4 * t + 2 : 4 * t + 0;
+    e = cudaEventElapsedTime(&v, h->ev_k[a], h->ev_k[a + 1]);
+    if (e != cudaSuccess) return cuda_fail(h, e, "event elapsed");
+    total += v;
+  }
+  *ms = total;
+  return LB_OK;
+}
+
+}  // extern "C"

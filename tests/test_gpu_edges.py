@@ -1,0 +1,216 @@
+"""GPU edge cases, accessors, error behaviour and full-size checks of the CUDA path."""
+import numpy as np
+import pytest
+
+import parity_util as pu
+from paper_2005_12764_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lbmod():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2005_12764_b200 import lb
+    return lb
+
+
+def _random_workload(nx, ny, nz, seed, walls=False, A_nc=0.02, tau=(0.8, 1.2), g=(1e-4, -5e-5, 2e-5)):
+    rng = np.random.default_rng(seed)
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    # smooth random phase field so that interfaces, probes and bulk all occur
+    phi = np.zeros((nz, ny, nx))
+    for _ in range(6):
+        k = rng.integers(1, 3, 3)
+        ph = rng.uniform(0, 2 * np.pi, 3)
+        phi += rng.normal() * np.cos(2 * np.pi * k[0] * x / nx + ph[0]) * np.cos(2 * np.pi * k[1] * y / ny + ph[1]) \
+            * np.cos(2 * np.pi * k[2] * z / nz + ph[2])
+    phi = np.tanh(1.5 * phi)
+    rho = 1.0 + 0.02 * rng.uniform(-1, 1, phi.shape)
+    solid = None
+    if walls:
+        solid = np.zeros((nz, ny, nx), np.uint8)
+        solid[:, 0, :] = 1
+        solid[0, :, :] = 1
+        solid[nz // 2, ny // 2, nx // 3] = 1
+        solid[1:3, 2:4, nx - 1] = 1
+    return W.Workload("random", nx, ny, nz, tau[0], tau[1], 0.01, 0.7, A_nc,
+                      (rho * (1 + phi) / 2).astype(np.float32), (rho * (1 - phi) / 2).astype(np.float32),
+                      (0.02 * rng.normal(size=(3, nz, ny, nx))).astype(np.float32), solid=solid, g=g)
+
+
+@pytest.mark.parametrize("shape", [(4, 4, 4), (36, 13, 7), (68, 9, 21), (32, 8, 16)])
+@pytest.mark.parametrize("walls", [False, True])
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_ragged_boxes_all_features(lbmod, lbo, shape, walls, storage):
+    """Smallest box, extents that are not multiples of the 32 x 8 tile or of the z chunk, two
+    taus, body force, walls, near contact: populations after 1, 2 and 5 steps."""
+    w = _random_workload(*shape, seed=sum(shape) + walls, walls=walls)
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
+    fluid = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
+    assert pu.pop_error(sim, o).max() < pu.POP_TOL
+    phi_g = sim.get_phi()
+    assert np.abs(phi_g - o.get_fields()["phi"])[fluid].max() < 1e-5
+    risky = np.zeros(w.shape, bool)
+    done = 0
+    for n in (1, 2, 5):
+        for _ in range(n - done):
+            risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+            o.step(1); sim.step(1)
+        done = n
+        e = pu.pop_error(sim, o)
+        ok = ~risky
+        if ok.any():
+            assert e[ok].max() < pu.POP_TOL, (n, e[ok].max())
+        assert risky.mean() < 0.2 or w.sites < 5000     # tiny boxes: the dilated set covers them
+    errs, _, _ = pu.macro_errors(sim, o)
+    if not risky.any():
+        assert max(errs.values()) < pu.MACRO_TOL
+
+
+def test_no_near_contact_no_force_paths(lbmod, lbo):
+    """A_nc = 0 (H = 1 ring), equal taus, g = 0, with and without walls."""
+    for walls in (False, True):
+        w = _random_workload(40, 12, 10, seed=77, walls=walls, A_nc=0.0, tau=(1.0, 1.0), g=(0, 0, 0))
+        o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w)
+        o.step(3); sim.step(3)
+        assert pu.pop_error(sim, o).max() < pu.POP_TOL
+
+
+def test_poiseuille_single_component_walls(lbmod, lbo):
+    """Single-component kernel with the bit-packed mask and a body force (pin P7's setup)."""
+    nx, ny, nz = 4, 34, 4
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = solid[:, -1, :] = 1
+    w = W.Workload("poiseuille", nx, ny, nz, 1.0, 1.0, 0, 0, 0, np.ones((nz, ny, nx), np.float32), None,
+                   np.zeros((3, nz, ny, nx), np.float32), solid=solid, g=(1e-6, 0, 0))
+    for storage in ("ab", "aa"):
+        o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
+        o.step(2001); sim.step(2001)
+        errs, (rr, _, u), (orr, _, ou) = pu.macro_errors(sim, o)
+        assert errs["u"] < 1e-7 and errs["rho_r"] < 1e-5, errs
+        assert u[0].max() > 1e-4
+
+
+def test_set_get_populations_roundtrip(lbmod, lbo):
+    w = _random_workload(36, 9, 6, seed=5, walls=True)
+    o = pu.make_oracle(lbo, w)
+    o.step(2)
+    for storage in ("ab", "aa"):
+        sim = pu.make_gpu(lbmod, w, storage)
+        sim.step(1)          # AA: leave the buffer in the swapped state first
+        fr, fb = o.get_populations(0).astype(np.float32), o.get_populations(1).astype(np.float32)
+        sim.set_populations(0, fr)
+        sim.set_populations(1, fb)
+        fluid = w.solid == 0
+        assert np.abs(sim.get_populations(0) - fr)[:, fluid].max() < 1e-7
+        assert np.abs(sim.get_populations(1) - fb)[:, fluid].max() < 1e-7
+        o2 = pu.make_oracle(lbo, w)
+        o2.set_populations(0, fr); o2.set_populations(1, fb)
+        o2.step(1); sim.step(1)
+        assert pu.pop_error(sim, o2).max() < pu.POP_TOL
+
+
+def test_device_pointers_and_stream(lbmod, lbo):
+    """Device-resident inputs/outputs (torch tensors) and a non-default torch stream."""
+    import torch
+    w = W.get("c1")
+    o = pu.make_oracle(lbo, w)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        rr = torch.from_numpy(w.rho_r).cuda()
+        rb = torch.from_numpy(w.rho_b).cuda()
+        u = torch.from_numpy(w.u).cuda()
+        sim = lbmod.from_workload(w)
+        sim.init(rr, rb, u)
+        sim.step(10)
+        out_r, out_b, out_u = torch.empty_like(rr), torch.empty_like(rb), torch.empty_like(u)
+        sim.get_macros(out_r, out_b, out_u)
+    s.synchronize()
+    o.step(10)
+    orr, orb, ou = o.get_macros()
+    assert np.abs(out_r.cpu().numpy() - orr).max() < pu.MACRO_TOL
+    assert np.abs(out_u.cpu().numpy() - ou).max() < pu.MACRO_TOL
+    assert sim.launch_count() >= 21 and sim.device_bytes() > 2 * 38 * w.sites * 4
+
+
+def test_error_codes(lbmod):
+    lb = lbmod
+    for bad in [(30, 8, 8), (2, 8, 8), (8, 3, 8)]:
+        with pytest.raises(lb.LBError) as ei:
+            lb.LB(*bad)
+        assert ei.value.code == lb.LB_EINVAL
+    with pytest.raises(lb.LBError) as ei:
+        lb.LB(8, 8, 8, tau_r=0.5)
+    assert ei.value.code == lb.LB_EINVAL
+    sim = lb.LB(8, 8, 8)
+    with pytest.raises(lb.LBError) as ei:
+        sim.step(1)
+    assert ei.value.code == lb.LB_ESTATE
+    sim.init(np.ones((8, 8, 8), np.float32), np.ones((8, 8, 8), np.float32), np.zeros((3, 8, 8, 8), np.float32))
+    with pytest.raises(lb.LBError) as ei:
+        sim.set_geometry(np.zeros((8, 8, 8), np.uint8))
+    assert ei.value.code == lb.LB_ESTATE
+    with pytest.raises(lb.LBError) as ei:
+        sim.set_storage("aa")
+    assert ei.value.code == lb.LB_ESTATE
+    sim.step(0)
+    sim.destroy()
+    sim.destroy()
+
+
+# ------------------------------------------------------------------------------- full size
+def _block_oracle_check(lbmod, lbo, w, sim, centres, half=14, margin=7):
+    """Sampled outputs at full size: around each centre cut a (2*half)^3 block of the INPUT,
+    run the oracle on it as a periodic box for one step and compare the block's interior, whose
+    domain of dependence (1 stream + 1 gradient + 4 probe + 1 slack) lies inside the block."""
+    f = [sim.get_populations(k) for k in (0, 1)]
+    worst = 0.0
+    for (cx, cy, cz) in centres:
+        ix = np.arange(cx - half, cx + half) % w.nx
+        iy = np.arange(cy - half, cy + half) % w.ny
+        iz = np.arange(cz - half, cz + half) % w.nz
+        sel = np.ix_(iz, iy, ix)
+        n = 2 * half
+        o = lbo.Oracle(n, n, n, *w.params)
+        if w.solid is not None:
+            o.set_geometry(w.solid[sel])
+        o.set_body_force(*w.g)
+        o.set_nc_cutoff(w.phi_c)
+        o.init(w.rho_r[sel], w.rho_b[sel], w.u[(slice(None),) + sel])
+        marg = o.get_fields()["margin"]
+        o.step(1)
+        inner = np.zeros((n, n, n), bool)
+        inner[margin:-margin, margin:-margin, margin:-margin] = True
+        if w.solid is not None:
+            inner &= w.solid[sel] == 0
+        inner &= ~pu.dilate(marg < 1e-5, 1)
+        for k in (0, 1):
+            e = np.abs(f[k][(slice(None),) + sel].astype(np.float64) - o.get_populations(k)) / pu.W19[:, None, None, None]
+            worst = max(worst, e[:, inner].max())
+    return worst
+
+
+@pytest.mark.parametrize("name", ["c3", "c4"])
+def test_full_size_sampled_blocks_and_conservation(lbmod, lbo, name):
+    """Full-size configs in the launch configuration bench.py times: one step checked on
+    sampled blocks against the oracle, then conservation over more steps."""
+    w = W.get(name)
+    sim = pu.make_gpu(lbmod, w)
+    rr0, rb0, _ = sim.get_macros()
+    m0 = pu.masses(rr0, rb0)
+    sim.step(1)
+    rng = np.random.default_rng(9)
+    centres = [(0, 0, 0), (w.nx - 1, w.ny // 2, w.nz - 1)] + \
+        [tuple(int(v) for v in rng.integers(0, [w.nx, w.ny, w.nz])) for _ in range(4)]
+    worst = _block_oracle_check(lbmod, lbo, w, sim, centres)
+    assert worst < pu.POP_TOL, worst
+    sim.step(199)
+    rr, rb, u = sim.get_macros()
+    assert np.isfinite(u).all()
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
+    if name == "c3":
+        mom = np.abs([(u[a].astype(np.float64) * (rr + rb)).sum() for a in range(3)]).max() / w.sites
+        assert mom < 1e-5

@@ -1,0 +1,145 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by
+element, on the same seeded inputs.  Tolerances are north_star's (tests/parity_util.py)."""
+import numpy as np
+import pytest
+
+import parity_util as pu
+from paper_2005_12764_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lbmod():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2005_12764_b200 import lb
+    return lb
+
+
+# ------------------------------------------------------------------------------- C1
+def test_C1_droplet_full(lbmod, lbo):
+    """Config C1 in full: populations after 1 step, macros after 100 and 1000 steps, mass."""
+    w = W.get("c1")
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w)
+    assert pu.pop_error(sim, o).max() < pu.POP_TOL          # t = 0: init parity
+    rr0, rb0, _ = sim.get_macros()
+    m0 = pu.masses(rr0, rb0)
+    o.step(1); sim.step(1)
+    e = pu.pop_error(sim, o)
+    assert e.max() < pu.POP_TOL, e.max()
+    o.step(99); sim.step(99)
+    errs, (rr, rb, u), _ = pu.macro_errors(sim, o)
+    assert max(errs.values()) < pu.MACRO_TOL, errs
+    o.step(900); sim.step(900)
+    errs, (rr, rb, u), _ = pu.macro_errors(sim, o)
+    assert max(errs.values()) < pu.MACRO_TOL, errs
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
+
+
+# ------------------------------------------------------------------------------- C2 mini
+def test_C2_mini_single_component(lbmod, lbo):
+    w = W.get("c2-mini")
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w)
+    o.step(1); sim.step(1)
+    assert pu.pop_error(sim, o, two=False).max() < pu.POP_TOL
+    o.step(199); sim.step(199)
+    errs, (rr, _, u), _ = pu.macro_errors(sim, o)
+    assert max(errs.values()) < pu.MACRO_TOL, errs
+    assert abs(float(rr.sum(dtype=np.float64)) - w.sites) / w.sites < pu.DRIFT_TOL
+
+
+# ------------------------------------------------------------------------------- C3 mini
+def test_C3_mini_spinodal(lbmod, lbo):
+    """Linearly unstable mixture: 1, 10, 100 steps; the GPU error must stay within 3x the
+    divergence of an oracle run whose input was perturbed by 1e-7 (sensitivity control)."""
+    w = W.get("c3-mini")
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w)
+    rng = np.random.default_rng(5)
+    pert = 1e-7 * rng.uniform(-1, 1, w.shape)
+    o2 = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    o2.init(w.rho_r.astype(np.float64) + pert, w.rho_b.astype(np.float64) - pert, w.u)
+    o.step(1); sim.step(1); o2.step(1)
+    assert pu.pop_error(sim, o).max() < pu.POP_TOL
+    done = 1
+    for target in (10, 100):
+        o.step(target - done); sim.step(target - done); o2.step(target - done)
+        done = target
+        errs, (rr, rb, u), (orr, orb, ou) = pu.macro_errors(sim, o)
+        c_rr, c_rb, c_u = o2.get_macros()
+        control = max(np.abs(c_rr - orr).max(), np.abs(c_rb - orb).max(), np.abs(c_u - ou).max())
+        assert max(errs.values()) < max(3 * control, pu.MACRO_TOL), (target, errs, control)
+    m0 = pu.masses(w.rho_r, w.rho_b)
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
+    # zero-force momentum stays zero per site on average
+    mom = np.abs([(u[a].astype(np.float64) * (rr + rb)).sum() for a in range(3)]).max() / w.sites
+    assert mom < 1e-5
+
+
+def _nc_parity_one_step(lbmod, lbo, w, storage="ab"):
+    """1-step population parity with the near-contact force on: sites whose discrete decisions
+    (|phi| < phi_c, probe rounding, phi(p_k) >= phi(x)) have a margin below 1e-5 in the oracle,
+    and their neighbours, are excluded (G12); the excluded set must be small."""
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
+    fl = o.get_fields()
+    fluid = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
+    risky = (fl["margin"] < 1e-5) & fluid
+    interface = (np.abs(fl["phi"]) < w.phi_c) & fluid
+    assert risky.sum() <= max(2, 1e-3 * interface.sum()), (risky.sum(), interface.sum())
+    assert (fl["h"] > 0).sum() > 0, "workload has no near-contact sites"
+    o.step(1); sim.step(1)
+    e = pu.pop_error(sim, o)
+    ok = ~pu.dilate(risky, 1)
+    assert e[ok].max() < pu.POP_TOL, e[ok].max()
+    return o, sim, risky
+
+
+# ------------------------------------------------------------------------------- C4 mini
+def test_C4_mini_channel(lbmod, lbo):
+    """Walls (bit-packed mask, bounce-back), body force, near-contact probe: 1 and 100 steps."""
+    w = W.get("c4-mini")
+    o, sim, risky = _nc_parity_one_step(lbmod, lbo, w)
+    rr0, rb0, _ = pu.make_gpu(lbmod, w).get_macros()
+    m0 = pu.masses(rr0, rb0)
+    o.step(99); sim.step(99)
+    errs, (rr, rb, u), (orr, orb, ou) = pu.macro_errors(sim, o)
+    # a flipped contact decision changes the local force by up to A_nc |G|/2 for a step, so the
+    # max norm gets a looser bound here; the bulk of the sites must meet the 1e-4 bar
+    frac_bad = (np.abs(u - ou).max(0) > pu.MACRO_TOL).mean()
+    assert frac_bad < 1e-3, frac_bad
+    assert errs["u"] < 5e-3 and errs["rho_r"] < 5e-2, errs
+    solid = w.solid != 0
+    assert rr[solid].max() == 0 and np.abs(u[:, solid]).max() == 0
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
+    assert u[0][~solid].mean() > 0        # the body force drives the flow along +x
+
+
+# ------------------------------------------------------------------------------- C5 mini
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_C5_mini_emulsion(lbmod, lbo, storage):
+    """Dense emulsion with near contact, A/B and AA storage: 1, 2, 3 steps (both AA parities)."""
+    w = W.get("c5-mini")
+    o, sim, risky = _nc_parity_one_step(lbmod, lbo, w, storage)
+    for n in (2, 3):
+        o.step(1); sim.step(1)
+        e = pu.pop_error(sim, o)
+        ok = ~pu.dilate(risky, n + 1)
+        # later steps may meet new marginal decisions: allow a handful of outliers
+        assert (e[ok] > pu.POP_TOL).sum() <= 50 and np.quantile(e[ok], 0.9999) < pu.POP_TOL, (n, e[ok].max())
+
+
+def test_AA_equals_AB_bitwise(lbmod):
+    """AA and A/B share the arithmetic, so they must agree bit for bit (3 and 4 steps)."""
+    w = W.get("c5-mini")
+    a, b = pu.make_gpu(lbmod, w, "ab"), pu.make_gpu(lbmod, w, "aa")
+    for n in (3, 1):
+        a.step(n); b.step(n)
+        for k in (0, 1):
+            assert np.array_equal(a.get_populations(k), b.get_populations(k))
+    ra, _, ua = a.get_macros()
+    rb_, _, ub = b.get_macros()
+    assert np.array_equal(ra, rb_) and np.array_equal(ua, ub)
+    assert b.device_bytes() < 0.6 * a.device_bytes()
