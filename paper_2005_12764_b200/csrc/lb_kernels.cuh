@@ -113,6 +113,14 @@ __device__ __forceinline__ void make_ctx(Ctx& c, const Box& b, int x, int y, int
   c.dzo[2] = (z == b.nz - 1 ? -(b.nz - 1) : 1) * pl;
 }
 
+// s + e <- s + e + x with the rounding error of the addition kept in e (Knuth two-sum).
+__device__ __forceinline__ void two_sum_acc(float& s, float& e, float x) {
+  const float t = __fadd_rn(s, x);
+  const float bp = __fsub_rn(t, s);
+  e = __fadd_rn(e, __fadd_rn(__fsub_rn(s, __fsub_rn(t, bp)), __fsub_rn(x, bp)));
+  s = t;
+}
+
 // ----------------------------------------------------------------------------- K1 phase field
 // One thread per site of a TX x TY tile, marching over zc planes.  152 B read, 4 B written.
 template <int MODE, bool HAS_SOLID>
@@ -145,11 +153,19 @@ __global__ void __launch_bounds__(TX* TY) k_phase(const StepParams p) {
         t[q] = ld_pop<MODE>(p.src + s);
         r[q] = ld_pop<MODE>(p.src + (size_t)Q * c.S + s);
       });
-      // fixed-order pairwise sums (same order in K2/K3)
-      float dr = 0.f, rr = 0.f;
-      static_for<0, Q>([&](auto qc) { constexpr int q = decltype(qc)::value; dr += t[q]; rr += r[q]; });
-      const float rho = 1.0f + dr;
-      phi = (2.0f * rr - rho) / rho;   // (rho_r - rho_b)/rho with rho_b = rho - rho_r
+      // Compensated (two-sum) accumulation: the direction of grad phi, which the perturbation and
+      // the recolouring use, is ill-conditioned where |grad phi| is small, so phi is formed to
+      // ~1e-8 instead of the ~1e-7 that a plain fp32 sum of 19 terms gives.
+      float dr = 0.f, de = 0.f, rr = 0.f, re = 0.f;
+      static_for<0, Q>([&](auto qc) {
+        constexpr int q = decltype(qc)::value;
+        two_sum_acc(dr, de, t[q]);
+        two_sum_acc(rr, re, r[q]);
+      });
+      // rho_r - rho_b = 2 rho_r - rho = (2 rr - 1 - dr) + (2 re - de); rho = 1 + dr + de
+      const float num = ((2.0f * rr - 1.0f) - dr) + (2.0f * re - de);
+      const float rho = (1.0f + dr) + de;
+      phi = num / rho;
     }
     // home location plus the periodic images that fall into the ghost layers
     const int sx[3] = {0, x < H ? b.nx : 0, x >= b.nx - H ? -b.nx : 0};
@@ -203,7 +219,10 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 
 template <int H>
 struct Ring {
-  static constexpr int BX = (H == 1) ? 36 : 40;       // box extent in x: 16-byte multiple >= TX + 2H
+  // Box extent in x is TX + 2 HALO for every H and the box starts at padded x = x0: the TMA unit
+  // faults (illegal instruction, measured on B200) when the innermost start
+  // coordinate is not a multiple of 16 bytes, so the box cannot start at x0 + HALO - H for H = 1.
+  static constexpr int BX = TX + 2 * HALO;
   static constexpr int BY = TY + 2 * H;
   static constexpr int PF = 2;                         // planes prefetched ahead
   static constexpr int NS = 2 * H + 1 + PF;            // ring slots
@@ -242,7 +261,7 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
   auto issue = [&](int j) {
     const int s = j % R_::NS;
     mbar_expect_tx(&bars[s], R_::BYTES);
-    tma_load_3d(&ring[s * R_::SLOT], &tmap, &bars[s], x0 + HALO - H, y0 + HALO - H, zb - H + j + HALO);
+    tma_load_3d(&ring[s * R_::SLOT], &tmap, &bars[s], x0, y0 + HALO - H, zb - H + j + HALO);
   };
   if (tid == 0) {
     const int n0 = min(npl, R_::NS - 1);
@@ -251,7 +270,7 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
 
   const float omega_same = 1.0f / p.tau_r;
   const float nu_r = (p.tau_r - 0.5f) * (1.0f / 3.0f), nu_b = (p.tau_b - 0.5f) * (1.0f / 3.0f);
-  const int lx = threadIdx.x + H, ly = threadIdx.y + H;
+  const int lx = threadIdx.x + HALO, ly = threadIdx.y + H;
 
   for (int jz = 0; jz < ze - zb; ++jz) {
     const int z = zb + jz;
@@ -357,8 +376,13 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
       // ---- collide on the total (deviation form), perturb, recolour, store
       float* dT = p.dst;
       float* dR = p.dst + (size_t)Q * c.S;
-      static_for<0, Q>([&](auto qc) {
-        constexpr int q = decltype(qc)::value;
+      // Directions 1..18 first; the rest populations then take what is left of rho - 1 and of
+      // rho_r (collision conserves both at every site), so that the per-site masses are conserved
+      // to the rounding of one sum instead of carrying the relative error of rho_r/rho or of
+      // w_q * drho (a systematic drift in uniform regions).
+      float racc = 0.f, tacc = 0.f;
+      static_for<1, Q + 1>([&](auto qc) {
+        constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
         constexpr float w = wq(q);
         const float cu = cx(q) * ux + cy(q) * uy + cz(q) * uz;
         const float cG = cx(q) * Gx + cy(q) * Gy + cz(q) * Gz;
@@ -369,8 +393,15 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
           ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
         }
         ts += p.A * (w * cG * cG * invG - bq(q) * Gne);
-        float rs = fr_r * (ts + w);
-        if constexpr (q > 0) rs += kcol * (w * inv_cnorm(q)) * cG;
+        float rs;
+        if constexpr (q > 0) {
+          rs = fr_r * (ts + w) + kcol * (w * inv_cnorm(q)) * cG;
+          racc += rs;
+          tacc += ts;
+        } else {
+          ts = dr - tacc;
+          rs = rr - racc;
+        }
         const size_t s = write_slot<MODE, HAS_SOLID, q>(c, smask);
         dT[s] = ts;
         dR[s] = rs;
@@ -418,8 +449,9 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
     const float ux = (mx + 0.5f * Fx) * inv_rho, uy = (my + 0.5f * Fy) * inv_rho, uz = (mz + 0.5f * Fz) * inv_rho;
     const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
     const float uF = ux * Fx + uy * Fy + uz * Fz;
-    static_for<0, Q>([&](auto qc) {
-      constexpr int q = decltype(qc)::value;
+    float tacc = 0.f;   // the rest population takes what is left of rho - 1 (see k_fused)
+    static_for<1, Q + 1>([&](auto qc) {
+      constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
       constexpr float w = wq(q);
       const float cu = cx(q) * ux + cy(q) * uy + cz(q) * uz;
       const float teq = w * (dr + rho * (3.0f * cu + 4.5f * cu * cu - uu15));
@@ -428,6 +460,8 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
         const float cF = cx(q) * Fx + cy(q) * Fy + cz(q) * Fz;
         ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
       }
+      if constexpr (q > 0) tacc += ts;
+      else ts = dr - tacc;
       p.dst[write_slot<MODE, HAS_SOLID, q>(c, smask)] = ts;
     });
   }

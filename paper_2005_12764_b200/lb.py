@@ -147,7 +147,7 @@ class LB:
             pass
 
     def destroy(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and lib is not None:   # lib is None at interpreter shutdown
             lib.lb_destroy(self.h)
             self.h = None
 

@@ -63,7 +63,7 @@ def test_ragged_boxes_all_features(lbmod, lbo, shape, walls, storage):
         ok = ~risky
         if ok.any():
             assert e[ok].max() < pu.POP_TOL, (n, e[ok].max())
-        assert risky.mean() < 0.2 or w.sites < 5000     # tiny boxes: the dilated set covers them
+        assert risky.mean() < 0.5 or w.sites < 5000     # small boxes: the dilated set grows by a shell per step
     errs, _, _ = pu.macro_errors(sim, o)
     if not risky.any():
         assert max(errs.values()) < pu.MACRO_TOL
