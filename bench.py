@@ -60,13 +60,18 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def stored_traffic(kernel="k_fused"):
-    """dram bytes per launch of the dominant kernel from the committed ncu summary, if any."""
+def stored_traffic(kernel, workload, storage):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary
+    (profiles/traffic.csv: kernel,workload,storage,bytes,source), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(kernel)
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                p = line.strip().split(",")
+                if len(p) >= 4 and not line.startswith("#") and (p[0], p[1], p[2]) == (kernel, workload, storage):
+                    return float(p[3])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
@@ -286,7 +291,7 @@ def run_ours(args):
     k2_s = ms_k2 * 1e-3 / K
     achieved = upd_bytes * w.fluid_sites / k2_s / 1e9
     roofline = {"bound": "hbm", "kernel": "k_fused" if two else "k_single", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic("k_fused" if two else "k_single"),
+                "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic("k_fused" if two else "k_single", args.workload, args.storage),
                 "peak_source": peak_src, "algorithmic_bytes_per_update": upd_bytes,
                 "kernel_ms": ms_k2 / K, "kernel_share_of_step": ms_k2 / ms,
                 "phase_kernel_ms": ms_k1 / K,
