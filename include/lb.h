@@ -115,6 +115,14 @@ int lb_set_populations(lb_handle h, int comp, const float* f);
 /* phi = (rho_r - rho_b)/(rho_r + rho_b) of the current state, S floats (0 on solid sites). */
 int lb_get_phi(lb_handle h, float* phi);
 
+/* Tuning of lb_step (never changes results).  key = "pipeline": 1 = one launch per step (experimental),
+ * the phase-field and fused passes interleaved slab by slab so that each population is fetched
+ * from HBM once; 0 (default) = two launches per step.  "zs": z planes per work item;
+ * "slack": extra slabs by which the phase-field pass leads; "ys": rows per pencil; "ctas_per_sm":
+ * cap on resident CTAs.  value 0 (-1 for "slack") restores the automatic choice.
+ * Returns LB_EINVAL for an unknown key. */
+int lb_set_tuning(lb_handle h, const char* key, int value);
+
 /* Number of kernel launches this handle has made so far (for the harness' gpu_launches). */
 long long lb_launch_count(lb_handle h);
 

@@ -73,6 +73,12 @@ struct lb_handle_s {
   CUtensorMap tmap{};
   bool tmap_ok = false;
   bool phi_current = false;  // phi array matches the current populations
+  // pipelined single-launch step (k_step): tuning knobs (0 = choose automatically) and scratch
+  int pipeline = 0;          // 1 = k_step (experimental, slower so far), 0 = two launches per step
+  int tune_zs = 0, tune_slack = -1, tune_ys = 0, tune_ctas = 0, tune_prefetch = 1;
+  int* sched_buf = nullptr;  // [ticket, pdone[NP * nzs]]
+  size_t sched_ints = 0;
+  int num_sm = 0;
   int profiling = 0;
   cudaEvent_t ev_step[2] = {nullptr, nullptr};
   std::vector<cudaEvent_t> ev_k;   // 4 per step when profiling: K1 begin/end, K2 begin/end
@@ -242,6 +248,118 @@ void run_collide(lb_handle h) {
   h->phi_current = false;
 }
 
+// Schedule of the pipelined step (see k_step).  Returns false if the box is too small for it.
+bool make_sched(lb_handle h, Sched& sc, int resident_ctas) {
+  const bool nc = h->par.A_nc != 0.f;
+  const int H = nc ? H_MAX_NC : 1;
+  sc.H = H;
+  sc.ntx = (h->nx + TX - 1) / TX;
+  sc.ZS = h->tune_zs > 0 ? h->tune_zs : 2;
+  if (sc.ZS > h->nz) sc.ZS = h->nz;
+  sc.nzs = (h->nz + sc.ZS - 1) / sc.ZS;
+  sc.HS = (H + sc.ZS - 1) / sc.ZS;
+  if (sc.HS > sc.nzs) sc.HS = sc.nzs;
+  // pencils: y strips sized so that the H planes by which F trails P stay L2-resident
+  int ys = h->tune_ys;
+  if (ys <= 0) {
+    const double budget = 16.0e6;   // bytes of populations (read + written) per H planes of a pencil
+    ys = (int)(budget / ((double)H * h->nx * 304.0));
+  }
+  ys = (ys / TY) * TY;
+  if (ys < 2 * TY) ys = 2 * TY;
+  int np = (h->ny + ys - 1) / ys;
+  if (np < 1) np = 1;
+  ys = (((h->ny + np - 1) / np) + TY - 1) / TY * TY;      // balance the strips
+  np = (h->ny + ys - 1) / ys;
+  if (np > 1 && h->ny - (np - 1) * ys < H) np -= 1;       // the last strip must hold the halo of its neighbour
+  if (np > 1 && ys < H) return false;
+  sc.NP = np;
+  sc.YS = ys;
+  const int last_rows = h->ny - (np - 1) * ys;
+  for (int c = 0; c < 3; ++c) {
+    int rows, hb, hf;
+    if (np == 1) { rows = h->ny; hb = 0; hf = 0; }
+    else if (c == 0) { rows = ys; hb = H; hf = H; }
+    else if (c == 1) { rows = ys; hb = 0; hf = H; }
+    else { rows = last_rows; hb = 0; hf = 0; }
+    sc.hb[c] = hb;
+    sc.frow[c] = rows;
+    sc.prow[c] = rows + hb + hf;
+    sc.nFt[c] = sc.ntx * ((rows + TY - 1) / TY);
+    sc.nPt[c] = sc.ntx * ((sc.prow[c] + TY - 1) / TY);
+    sc.tk[c] = (long long)sc.nzs * (sc.nPt[c] + sc.nFt[c]);
+  }
+  sc.total = sc.tk[0] + (np > 2 ? (long long)(np - 2) * sc.tk[1] : 0) + (np > 1 ? sc.tk[2] : 0);
+  if (sc.total >= (1LL << 31)) return false;
+  // lead of P over F: 2 HS + 1 slabs are the data dependence; the slack keeps the polling thread
+  // from ever waiting: the P items F needs were issued >= ~1.5 x resident CTAs tickets earlier
+  int slack = h->tune_slack;
+  if (slack < 0) {
+    const int per_slab = sc.nPt[1] + sc.nFt[1];
+    slack = (int)((1.5 * resident_ctas + per_slab - 1) / per_slab);
+    if (slack < 1) slack = 1;
+  }
+  sc.LEAD = 2 * sc.HS + 1 + slack;
+  if (sc.LEAD > sc.nzs) sc.LEAD = sc.nzs;
+  const size_t ints = 1 + (size_t)np * sc.nzs;
+  if (ints > h->sched_ints) {
+    dev_free(h->sched_buf);
+    h->sched_buf = static_cast<int*>(dev_alloc(ints * sizeof(int)));
+    if (!h->sched_buf) { h->sched_ints = 0; return false; }
+    h->sched_ints = ints;
+  }
+  sc.ticket = h->sched_buf;
+  sc.prefetch = h->tune_prefetch;
+  sc.pdone = h->sched_buf + 1;
+  return true;
+}
+
+template <int MODE, bool HAS_SOLID, bool HAS_NC>
+bool launch_step_t(lb_handle h, const StepParams& p) {
+  auto kern = k_step<MODE, HAS_SOLID, HAS_NC>;
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, TX * TY, 0) != cudaSuccess || occ < 1) { cudaGetLastError(); return false; }
+  if (h->tune_ctas > 0 && occ > h->tune_ctas) occ = h->tune_ctas;
+  if (!h->num_sm) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&h->num_sm, cudaDevAttrMultiProcessorCount, dev);
+  }
+  const int resident = occ * h->num_sm;
+  Sched sc;
+  if (!make_sched(h, sc, resident)) return false;
+  if (cudaMemsetAsync(h->sched_buf, 0, (1 + (size_t)sc.NP * sc.nzs) * sizeof(int), h->stream) != cudaSuccess) { cudaGetLastError(); return false; }
+  const long long grid = sc.total < resident ? sc.total : resident;
+  kern<<<(unsigned)grid, dim3(TX, TY), 0, h->stream>>>(p, h->tmap, sc);
+  return true;
+}
+
+template <int MODE>
+bool launch_step(lb_handle h, const StepParams& p) {
+  const bool nc = h->par.A_nc != 0.f;
+  if (h->has_solid) return nc ? launch_step_t<MODE, true, true>(h, p) : launch_step_t<MODE, true, false>(h, p);
+  return nc ? launch_step_t<MODE, false, true>(h, p) : launch_step_t<MODE, false, false>(h, p);
+}
+
+// K12: one launch per step (two-component runs).  Returns false if the pipelined schedule cannot be
+// used (then the caller falls back to the two-launch form, which is the same arithmetic).
+bool run_step_pipelined(lb_handle h) {
+  float* src = h->cur_buf();
+  float* dst = h->storage == 0 ? h->buf[h->cur ^ 1] : h->buf[0];
+  const StepParams p = make_step_params(h, src, dst, 1);
+  const int mode = h->mode();
+  bool ok;
+  if (mode == MODE_AB) ok = launch_step<MODE_AB>(h, p);
+  else if (mode == MODE_AA_EVEN) ok = launch_step<MODE_AA_EVEN>(h, p);
+  else ok = launch_step<MODE_AA_ODD>(h, p);
+  if (!ok) return false;
+  h->launches++;
+  if (h->storage == 0) h->cur ^= 1;
+  else h->aa_odd ^= 1;
+  h->phi_current = false;
+  return true;
+}
+
 IoParams make_io_params(lb_handle h) {
   IoParams p;
   memset(&p, 0, sizeof(p));
@@ -323,7 +441,7 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
 void lb_destroy(lb_handle h) {
   if (!h) return;
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
-  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->mask);
+  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->mask); dev_free(h->sched_buf);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
   for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
   cudaGetLastError();
@@ -488,9 +606,13 @@ int lb_step(lb_handle h, int nsteps) {
   cudaEventRecord(h->ev_step[0], h->stream);
   for (int t = 0; t < nsteps; ++t) {
     if (prof) cudaEventRecord(h->ev_k[4 * t + 0], h->stream);
-    run_phase(h);
+    const bool piped = h->two && h->pipeline;
+    if (!piped) run_phase(h);
     if (prof) { cudaEventRecord(h->ev_k[4 * t + 1], h->stream); cudaEventRecord(h->ev_k[4 * t + 2], h->stream); }
-    run_collide(h);
+    if (!piped || !run_step_pipelined(h)) {
+      if (piped) run_phase(h);     // schedule not applicable to this box: two-launch form
+      run_collide(h);
+    }
     if (prof) cudaEventRecord(h->ev_k[4 * t + 3], h->stream);
   }
   cudaEventRecord(h->ev_step[1], h->stream);
@@ -589,6 +711,19 @@ int lb_get_phi(lb_handle h, float* phi) {
 long long lb_launch_count(lb_handle h) { return h ? h->launches : 0; }
 size_t lb_device_bytes(lb_handle h) { return h ? h->bytes : 0; }
 const char* lb_last_error(lb_handle h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int lb_set_tuning(lb_handle h, const char* key, int value) {
+  if (!h || !key) return LB_EINVAL;
+  const std::string k(key);
+  if (k == "pipeline") h->pipeline = value ? 1 : 0;
+  else if (k == "zs") h->tune_zs = value;
+  else if (k == "slack") h->tune_slack = value;
+  else if (k == "ys") h->tune_ys = value;
+  else if (k == "ctas_per_sm") h->tune_ctas = value;
+  else if (k == "prefetch") h->tune_prefetch = value;
+  else return fail(h, LB_EINVAL, "unknown tuning key: " + k);
+  return LB_OK;
+}
 
 int lb_set_profiling(lb_handle h, int on) {
   if (!h) return LB_EINVAL;

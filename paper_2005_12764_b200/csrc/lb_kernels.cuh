@@ -124,13 +124,8 @@ __device__ __forceinline__ void two_sum_acc(float& s, float& e, float x) {
 // ----------------------------------------------------------------------------- K1 phase field
 // One thread per site of a TX x TY tile, marching over zc planes.  152 B read, 4 B written.
 template <int MODE, bool HAS_SOLID>
-__global__ void __launch_bounds__(TX* TY) k_phase(const StepParams p) {
+__device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, int zb, int ze) {
   const Box& b = p.box;
-  const int x = blockIdx.x * TX + threadIdx.x;
-  const int y = blockIdx.y * TY + threadIdx.y;
-  if (x >= b.nx || y >= b.ny) return;
-  const int zb = blockIdx.z * p.zc;
-  const int ze = min(b.nz, zb + p.zc);
   const int H = p.halo;
   const int px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
   for (int z = zb; z < ze; ++z) {
@@ -187,6 +182,15 @@ __global__ void __launch_bounds__(TX* TY) k_phase(const StepParams p) {
   }
 }
 
+template <int MODE, bool HAS_SOLID>
+__global__ void __launch_bounds__(TX* TY) k_phase(const StepParams p) {
+  const int x = blockIdx.x * TX + threadIdx.x;
+  const int y = blockIdx.y * TY + threadIdx.y;
+  if (x >= p.box.nx || y >= p.box.ny) return;
+  const int zb = blockIdx.z * p.zc;
+  phase_column<MODE, HAS_SOLID>(p, x, y, zb, min(p.box.nz, zb + p.zc));
+}
+
 // ----------------------------------------------------------------------------- TMA / mbarrier
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -235,34 +239,28 @@ struct Ring {
 // planes z-H..z+H (+2 prefetched) of the tile with an H-wide halo live in a shared-memory ring
 // filled by TMA from the padded phi array (ghost layers make every box in-bounds, so periodic
 // wrap never reaches the TMA unit).  H = 1 without near contact, 4 with it.
+// One TX x TY tile starting at (x0, y0), planes [zb, ze).  `ring`/`bars` are the CTA's phi ring and
+// its mbarriers (initialised once per CTA); `jbase` counts the planes this CTA has pushed through the
+// ring so far, so that slot numbers and mbarrier phase parities carry over from one call to the next.
 template <int MODE, bool HAS_SOLID, bool HAS_NC>
-__global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
+__device__ __forceinline__ void fused_column(const StepParams& p, const CUtensorMap& tmap, float* ring, uint64_t* bars,
+                                             int x0, int y0, int ylim, int zb, int ze, uint32_t& jbase) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
   using R_ = Ring<H>;
-  __shared__ __align__(128) float ring[R_::NS * R_::SLOT];
-  __shared__ __align__(8) uint64_t bars[R_::NS];
-
   const Box& b = p.box;
   const int tid = threadIdx.y * TX + threadIdx.x;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int x = x0 + threadIdx.x, y = y0 + threadIdx.y;
-  const bool active = x < b.nx && y < b.ny;
-  const int zb = blockIdx.z * p.zc;
-  const int ze = min(b.nz, zb + p.zc);
+  const bool active = x < b.nx && y < ylim;
   const int npl = (ze - zb) + 2 * H;
+  const uint32_t jb = jbase;
+  jbase += npl;
 
-  if (tid == 0) {
-#pragma unroll
-    for (int s = 0; s < R_::NS; ++s) mbar_init(&bars[s], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  }
-  __syncthreads();
   auto issue = [&](int j) {
-    const int s = j % R_::NS;
+    const int s = (jb + j) % R_::NS;
     mbar_expect_tx(&bars[s], R_::BYTES);
     tma_load_3d(&ring[s * R_::SLOT], &tmap, &bars[s], x0, y0 + HALO - H, zb - H + j + HALO);
   };
+  auto wait = [&](int j) { mbar_wait(&bars[(jb + j) % R_::NS], ((jb + j) / R_::NS) & 1); };
   if (tid == 0) {
     const int n0 = min(npl, R_::NS - 1);
     for (int j = 0; j < n0; ++j) issue(j);
@@ -280,13 +278,12 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
     }
     if (jz == 0) {
 #pragma unroll
-      for (int j = 0; j <= 2 * H; ++j) mbar_wait(&bars[j % R_::NS], (j / R_::NS) & 1);
+      for (int j = 0; j <= 2 * H; ++j) wait(j);
     } else {
-      const int j = jz + 2 * H;
-      mbar_wait(&bars[j % R_::NS], (j / R_::NS) & 1);
+      wait(jz + 2 * H);
     }
     // plane dz of the ring
-    auto plane = [&](int dz) -> const float* { return &ring[((jz + H + dz) % R_::NS) * R_::SLOT]; };
+    auto plane = [&](int dz) -> const float* { return &ring[((jb + jz + H + dz) % R_::NS) * R_::SLOT]; };
     const float* pl0 = plane(0);
     const float phi0 = pl0[ly * R_::BX + lx];
     const bool fluid = active && !(HAS_SOLID && phi0 > PHI_SOLID_TEST);
@@ -408,6 +405,224 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
       });
     }
     __syncthreads();   // everyone is done with plane jz before its slot is refilled
+  }
+}
+
+template <int H>
+__device__ __forceinline__ void ring_init(uint64_t* bars) {
+  if (threadIdx.y * TX + threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < Ring<H>::NS; ++s) mbar_init(&bars[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+}
+
+template <int MODE, bool HAS_SOLID, bool HAS_NC>
+__global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
+  constexpr int H = HAS_NC ? H_MAX_NC : 1;
+  __shared__ __align__(128) float ring[Ring<H>::NS * Ring<H>::SLOT];
+  __shared__ __align__(8) uint64_t bars[Ring<H>::NS];
+  ring_init<H>(bars);
+  uint32_t jbase = 0;
+  const int zb = blockIdx.z * p.zc;
+  fused_column<MODE, HAS_SOLID, HAS_NC>(p, tmap, ring, bars, blockIdx.x * TX, blockIdx.y * TY, p.box.ny, zb, min(p.box.nz, zb + p.zc), jbase);
+}
+
+// ----------------------------------------------------------------------------- K12 pipelined step
+// One launch per LB step doing the work of K1 and K2 in an order that lets K2's gather hit in L2.
+// The box is cut into pencils (y strips of YS rows, full x extent, all z) that are processed one
+// after another; inside a pencil the work is cut into items of one TX x TY tile x ZS planes and
+// ordered z-slab by z-slab: the phase-field items P(k) of slab k run LEAD slabs ahead of the fused
+// items F(s).  P(k) pulls the 38 planes of slab k from HBM; F(k) gathers the same lines a few
+// hundred items later, while they are still in the 126 MB L2, so HBM sees each population once.
+// Persistent CTAs draw items from a global ticket counter in schedule order.  F(s) needs phi on
+// planes [s ZS - H, (s+1) ZS + H) of its tile and halo, i.e. completed P items with SMALLER ticket
+// numbers only; P items never wait.  The CTA holding the smallest unfinished ticket can therefore
+// always proceed: no deadlock, whether or not all CTAs are co-resident.  Completion is published
+// per (pencil, slab) with a release (fence + atomic add) and observed by one polling thread with an
+// acquire followed by fence.proxy.async, because the consumer of phi is the TMA unit.
+struct Sched {
+  int ZS, nzs, HS, LEAD;     // planes per slab, slabs, halo in slabs, lead of P over F in slabs
+  int H;                     // phi halo (1 or 4)
+  int ntx;                   // tiles along x
+  int NP, YS;                // pencils, rows per pencil (multiple of TY; the last pencil takes the rest)
+  // pencil classes: 0 = first, 1 = middle, 2 = last (a single pencil is class 0 with no halo)
+  int hb[3], prow[3], frow[3];   // backward halo rows, P rows (interior + halos), F rows
+  int nPt[3], nFt[3];            // P tiles and F tiles per slab
+  long long tk[3];               // tickets per pencil of this class
+  long long total;               // tickets per step
+  int* ticket;                   // global ticket counter (zeroed before the launch)
+  int* pdone;                    // [NP][nzs] completed P items (zeroed before the launch)
+  int prefetch;                  // hint the next P item's lines into L2 while the current item runs
+};
+
+struct Item {
+  int type;      // 0 = P, 1 = F, -1 = none
+  int pencil, cls, slab, tx, ty;
+};
+
+__device__ __forceinline__ Item decode_ticket(const Sched& sc, long long t) {
+  Item it;
+  it.type = -1;
+  if (t >= sc.total) return it;
+  int pencil = 0, cls = 0;
+  if (t >= sc.tk[0]) {
+    t -= sc.tk[0];
+    const long long nmid = sc.NP - 2;
+    if (nmid > 0 && t < nmid * sc.tk[1]) {
+      pencil = 1 + (int)(t / sc.tk[1]);
+      t -= (long long)(pencil - 1) * sc.tk[1];
+      cls = 1;
+    } else {
+      if (nmid > 0) t -= nmid * sc.tk[1];
+      pencil = sc.NP - 1;
+      cls = 2;
+    }
+  }
+  it.pencil = pencil;
+  it.cls = cls;
+  const int nP = sc.nPt[cls], nF = sc.nFt[cls];
+  int u = (int)t, tile;
+  const int A = sc.LEAD * nP;
+  if (u < A) {
+    it.type = 0; it.slab = u / nP; tile = u - it.slab * nP;
+  } else {
+    u -= A;
+    const int pair = nP + nF, npairs = sc.nzs - sc.LEAD;
+    if (u < npairs * pair) {
+      const int i = u / pair, r = u - i * pair;
+      if (r < nF) { it.type = 1; it.slab = i; tile = r; }
+      else { it.type = 0; it.slab = sc.LEAD + i; tile = r - nF; }
+    } else {
+      u -= npairs * pair;
+      const int i = u / nF;
+      it.type = 1; it.slab = npairs + i; tile = u - i * nF;
+    }
+  }
+  if (it.type == 0) {   // P slabs start HS slabs below the top so that F(0) finds its lower halo
+    it.slab = it.slab + sc.nzs - sc.HS;
+    if (it.slab >= sc.nzs) it.slab -= sc.nzs;
+  }
+  it.ty = tile / sc.ntx;
+  it.tx = tile - it.ty * sc.ntx;
+  return it;
+}
+
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+__device__ __forceinline__ int ld_relaxed(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
+// Block until every P item that F(pencil, slab) depends on has been published (one thread calls).
+// All counters are read with independent relaxed loads (their latencies overlap), then one fence
+// gives the acquire; fence.proxy.async orders the phi data before the TMA reads that follow.
+__device__ __forceinline__ void wait_phi_ready(const Sched& sc, const Box& b, int pencil, int slab) {
+  const int zb = slab * sc.ZS, ze = min(b.nz, zb + sc.ZS);
+  // own pencil, the pencil behind (its interior holds our backward halo rows) and, for the last
+  // pencil, pencil 0 (our forward halo rows wrap onto it)
+  int who[3] = {pencil, pencil, pencil};
+  if (sc.NP > 1) {
+    if (pencil > 0) who[1] = pencil - 1;
+    if (pencil == sc.NP - 1) who[2] = 0;
+  }
+  int need[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) need[i] = sc.nPt[who[i] == 0 ? 0 : (who[i] == sc.NP - 1 ? 2 : 1)];
+  bool ok;
+  do {
+    ok = true;
+    for (int pl = zb - sc.H; pl < ze + sc.H; ++pl) {
+      int w = pl;
+      while (w < 0) w += b.nz;
+      while (w >= b.nz) w -= b.nz;
+      const int k = w / sc.ZS;
+#pragma unroll
+      for (int i = 0; i < 3; ++i) ok &= ld_relaxed(sc.pdone + (size_t)who[i] * sc.nzs + k) >= need[i];
+    }
+    if (!ok) __nanosleep(100);
+  } while (!ok);
+  __threadfence();
+  asm volatile("fence.proxy.async;" ::: "memory");
+}
+
+// Hint the lines that P item `it` will gather into L2 (one line per component, direction, row, plane).
+template <int MODE>
+__device__ __forceinline__ void prefetch_p_item(const StepParams& p, const Sched& sc, const Item& it, int tid) {
+  const Box& b = p.box;
+  const int zb = it.slab * sc.ZS, ze = min(b.nz, zb + sc.ZS);
+  const int rows = min(TY, sc.prow[it.cls] - it.ty * TY);
+  const int x0 = it.tx * TX;
+  const int n = 2 * Q * rows * (ze - zb);
+  for (int i = tid; i < n; i += TX * TY) {
+    const int pq = i % (2 * Q);
+    const int rz = i / (2 * Q);
+    const int r = rz % rows, z = zb + rz / rows;
+    const int q = pq % Q;
+    int y = it.pencil * sc.YS - sc.hb[it.cls] + it.ty * TY + r;
+    int dx = 0, dy = 0, dz = 0, plane = q;
+    if (MODE != MODE_AA_EVEN) { dx = c_cx[q]; dy = c_cy[q]; dz = c_cz[q]; }
+    if (MODE == MODE_AA_ODD) plane = opp(q);
+    y -= dy;
+    while (y < 0) y += b.ny;
+    while (y >= b.ny) y -= b.ny;
+    int zz = z - dz;
+    if (zz < 0) zz += b.nz;
+    if (zz >= b.nz) zz -= b.nz;
+    int xx = x0 + (dx < 0 ? TX - 1 : 0);          // the line that holds all but one element of the row
+    if (xx >= b.nx) xx = b.nx - 1;
+    const float* a = p.src + (size_t)(plane + (pq >= Q ? Q : 0)) * b.S + ((size_t)xx + (size_t)b.nx * ((size_t)y + (size_t)b.ny * zz));
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+  }
+}
+
+template <int MODE, bool HAS_SOLID, bool HAS_NC>
+__global__ void __launch_bounds__(TX* TY, 3) k_step(const StepParams p, const __grid_constant__ CUtensorMap tmap, const Sched sc) {
+  constexpr int H = HAS_NC ? H_MAX_NC : 1;
+  __shared__ __align__(128) float ring[Ring<H>::NS * Ring<H>::SLOT];
+  __shared__ __align__(8) uint64_t bars[Ring<H>::NS];
+  __shared__ int tq[4];          // ticket queue: current, next (prefetched into L2), two in flight
+  const int tid = threadIdx.y * TX + threadIdx.x;
+  const Box& b = p.box;
+  if (tid < 3) tq[tid] = atomicAdd(sc.ticket, 1);
+  ring_init<H>(bars);          // ends with __syncthreads: the queue is visible
+  uint32_t jbase = 0;
+  for (int i = 0;; ++i) {
+    const Item it = decode_ticket(sc, tq[i & 3]);
+    if (it.type < 0) break;
+    const Item nx = decode_ticket(sc, tq[(i + 1) & 3]);
+    if (tid == 0) tq[(i + 3) & 3] = atomicAdd(sc.ticket, 1);
+    if (sc.prefetch && nx.type == 0) prefetch_p_item<MODE>(p, sc, nx, tid);
+    const int y0p = (it.pencil * sc.YS);                           // first interior row of the pencil
+    const int zb = it.slab * sc.ZS, ze = min(b.nz, zb + sc.ZS);
+    if (it.type == 0) {
+      const int r = it.ty * TY + threadIdx.y;                        // row inside the pencil's P range
+      const int x = it.tx * TX + threadIdx.x;
+      if (r < sc.prow[it.cls] && x < b.nx) {
+        int y = y0p - sc.hb[it.cls] + r;
+        if (y < 0) y += b.ny;
+        if (y >= b.ny) y -= b.ny;
+        phase_column<MODE, HAS_SOLID>(p, x, y, zb, ze);
+      }
+      __syncthreads();
+      if (tid == 0) {
+        __threadfence();
+        atomicAdd(sc.pdone + (size_t)it.pencil * sc.nzs + it.slab, 1);
+      }
+    } else {
+      if (tid == 0) wait_phi_ready(sc, b, it.pencil, it.slab);
+      fused_column<MODE, HAS_SOLID, HAS_NC>(p, tmap, ring, bars, it.tx * TX, y0p + it.ty * TY,
+                                            min(b.ny, y0p + sc.frow[it.cls]), zb, ze, jbase);
+      // fused_column ends with __syncthreads
+    }
   }
 }
 

@@ -20,7 +20,7 @@ SYMBOLS = [
     "lb_set_allocator", "lb_create", "lb_destroy", "lb_set_stream", "lb_set_geometry",
     "lb_set_body_force", "lb_set_nc_cutoff", "lb_set_storage", "lb_init", "lb_step",
     "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
-    "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms",
+    "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
 ]
 
 
@@ -62,6 +62,7 @@ def _load():
     lib.lb_device_bytes.restype = C.c_size_t
     lib.lb_last_error.argtypes = [vp]
     lib.lb_last_error.restype = C.c_char_p
+    lib.lb_set_tuning.argtypes = [vp, C.c_char_p, C.c_int]
     lib.lb_set_profiling.argtypes = [vp, C.c_int]
     lib.lb_last_step_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
     return lib
@@ -208,6 +209,10 @@ class LB:
 
     def device_bytes(self):
         return int(lib.lb_device_bytes(self.h))
+
+    def set_tuning(self, **kw):
+        for k, v in kw.items():
+            self._ck(lib.lb_set_tuning(self.h, k.encode(), int(v)))
 
     def set_profiling(self, on):
         self._ck(lib.lb_set_profiling(self.h, int(bool(on))))
