@@ -115,12 +115,10 @@ int lb_set_populations(lb_handle h, int comp, const float* f);
 /* phi = (rho_r - rho_b)/(rho_r + rho_b) of the current state, S floats (0 on solid sites). */
 int lb_get_phi(lb_handle h, float* phi);
 
-/* Tuning of lb_step (never changes results).  key = "pipeline": 1 = one launch per step (experimental),
- * the phase-field and fused passes interleaved slab by slab so that each population is fetched
- * from HBM once; 0 (default) = two launches per step.  "zs": z planes per work item;
- * "slack": extra slabs by which the phase-field pass leads; "ys": rows per pencil; "ctas_per_sm":
- * cap on resident CTAs.  value 0 (-1 for "slack") restores the automatic choice.
- * Returns LB_EINVAL for an unknown key. */
+/* Tuning of lb_step.  key = "forward": 1 (default) = the fused kernel forwards the moments of the
+ * next state and a light kernel turns them into phi; 0 = a full
+ * phase-field sweep over the populations before every step (same phi to ~1e-8).  "zc": z planes
+ * per CTA, 0 = automatic.  Returns LB_EINVAL for an unknown key. */
 int lb_set_tuning(lb_handle h, const char* key, int value);
 
 /* Number of kernel launches this handle has made so far (for the harness' gpu_launches). */
@@ -134,8 +132,8 @@ const char* lb_last_error(lb_handle h);
 
 /* Timing hook: an event pair recorded around the kernels of the LAST lb_step call, on the
  * handle's stream; returns the elapsed milliseconds (synchronises on the end event).
- * which: 0 = whole lb_step, 1 = sum over the fused stream-collide launches, 2 = sum over the
- * phase-field launches.  which = 1, 2 are recorded only after lb_set_profiling(h, 1). */
+ * which: 0 = whole lb_step, 1 = sum over the fused stream-collide launches (k_fused / k_single),
+ * 2 = sum over the phase-field launches (k_phase_fwd, or k_phase).  which = 1, 2 are recorded only after lb_set_profiling(h, 1). */
 int lb_set_profiling(lb_handle h, int on);
 int lb_last_step_ms(lb_handle h, int which, float* ms);
 

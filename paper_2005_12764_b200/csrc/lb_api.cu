@@ -73,12 +73,9 @@ struct lb_handle_s {
   CUtensorMap tmap{};
   bool tmap_ok = false;
   bool phi_current = false;  // phi array matches the current populations
-  // pipelined single-launch step (k_step): tuning knobs (0 = choose automatically) and scratch
-  int pipeline = 0;          // 1 = k_step (experimental, slower so far), 0 = two launches per step
-  int tune_zs = 0, tune_slack = -1, tune_ys = 0, tune_ctas = 0, tune_prefetch = 1;
-  int* sched_buf = nullptr;  // [ticket, pdone[NP * nzs]]
-  size_t sched_ints = 0;
-  int num_sm = 0;
+  float* mom = nullptr;      // forwarded moments Md, Mt (2 x S floats), written by k_fused
+  int forward = 1;           // 1 = phi(t+1) from forwarded moments (k_phase_fwd), 0 = full k_phase sweep
+  int tune_zc = 0;           // z planes per CTA (0 = automatic)
   int profiling = 0;
   cudaEvent_t ev_step[2] = {nullptr, nullptr};
   std::vector<cudaEvent_t> ev_k;   // 4 per step when profiling: K1 begin/end, K2 begin/end
@@ -158,6 +155,7 @@ namespace {
 StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   StepParams p;
   p.src = src; p.dst = dst; p.phi = h->phi;
+  p.Md = h->mom; p.Mt = h->mom ? h->mom + h->S : nullptr; p.EX = h->mom ? h->mom + 2 * h->S : nullptr;
   p.box = h->box();
   p.zc = zc;
   p.halo = h->par.A_nc != 0.f ? H_MAX_NC : 1;
@@ -172,6 +170,7 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
 // z planes per CTA: enough CTAs for ~8 waves of 148 SMs x 4 resident CTAs, at least 8 planes
 // so that the phi-ring prologue (2H+1 planes) is amortised.
 int pick_zc(lb_handle h) {
+  if (h->tune_zc > 0) return h->tune_zc < h->nz ? h->tune_zc : h->nz;
   const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
   const long long want = 148LL * 4 * 8;
   long long zsplit = (want + cols - 1) / cols;
@@ -192,17 +191,31 @@ void launch_phase(lb_handle h, const StepParams& p, dim3 grid) {
   if (h->has_solid) k_phase<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
   else k_phase<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
 }
+template <int MODE, bool HAS_SOLID, bool HAS_NC>
+void launch_fused_t(lb_handle h, const StepParams& p, dim3 grid) {
+  constexpr size_t smem = FusedSmem<HAS_NC ? H_MAX_NC : 1>::BYTES;
+  static bool attr_set = false;   // per instantiation
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, HAS_NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  k_fused<MODE, HAS_SOLID, HAS_NC><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap);
+}
 template <int MODE>
 void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
   const bool nc = h->par.A_nc != 0.f;
-  const dim3 blk(TX, TY);
   if (h->has_solid) {
-    if (nc) k_fused<MODE, true, true><<<grid, blk, 0, h->stream>>>(p, h->tmap);
-    else k_fused<MODE, true, false><<<grid, blk, 0, h->stream>>>(p, h->tmap);
+    if (nc) launch_fused_t<MODE, true, true>(h, p, grid);
+    else launch_fused_t<MODE, true, false>(h, p, grid);
   } else {
-    if (nc) k_fused<MODE, false, true><<<grid, blk, 0, h->stream>>>(p, h->tmap);
-    else k_fused<MODE, false, false><<<grid, blk, 0, h->stream>>>(p, h->tmap);
+    if (nc) launch_fused_t<MODE, false, true>(h, p, grid);
+    else launch_fused_t<MODE, false, false>(h, p, grid);
   }
+}
+template <int MODE>
+void launch_phase_fwd(lb_handle h, const StepParams& p, dim3 grid) {
+  if (h->has_solid) k_phase_fwd<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+  else k_phase_fwd<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
 }
 template <int MODE>
 void launch_single(lb_handle h, const StepParams& p, dim3 grid) {
@@ -226,7 +239,7 @@ void run_phase(lb_handle h) {
 }
 
 // K2 / K2s: advance one step and flip the buffer / parity
-void run_collide(lb_handle h) {
+void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
   const int zc = pick_zc(h);
   const dim3 grid = tile_grid(h, zc);
   float* src = h->cur_buf();
@@ -246,118 +259,19 @@ void run_collide(lb_handle h) {
   if (h->storage == 0) h->cur ^= 1;
   else h->aa_odd ^= 1;
   h->phi_current = false;
-}
-
-// Schedule of the pipelined step (see k_step).  Returns false if the box is too small for it.
-bool make_sched(lb_handle h, Sched& sc, int resident_ctas) {
-  const bool nc = h->par.A_nc != 0.f;
-  const int H = nc ? H_MAX_NC : 1;
-  sc.H = H;
-  sc.ntx = (h->nx + TX - 1) / TX;
-  sc.ZS = h->tune_zs > 0 ? h->tune_zs : 2;
-  if (sc.ZS > h->nz) sc.ZS = h->nz;
-  sc.nzs = (h->nz + sc.ZS - 1) / sc.ZS;
-  sc.HS = (H + sc.ZS - 1) / sc.ZS;
-  if (sc.HS > sc.nzs) sc.HS = sc.nzs;
-  // pencils: y strips sized so that the H planes by which F trails P stay L2-resident
-  int ys = h->tune_ys;
-  if (ys <= 0) {
-    const double budget = 16.0e6;   // bytes of populations (read + written) per H planes of a pencil
-    ys = (int)(budget / ((double)H * h->nx * 304.0));
+  if (after_k2) cudaEventRecord(after_k2, h->stream);
+  if (h->two && h->forward) {
+    // K1f: phi of the new state from the moments k_fused forwarded (same z chunks: the bricks must match)
+    const StepParams q = make_step_params(h, h->cur_buf(), nullptr, zc);
+    const dim3 gridf(grid.x, grid.y, h->nz);   // one plane per CTA
+    switch (h->mode()) {
+      case MODE_AB: launch_phase_fwd<MODE_AB>(h, q, gridf); break;
+      case MODE_AA_EVEN: launch_phase_fwd<MODE_AA_EVEN>(h, q, gridf); break;
+      default: launch_phase_fwd<MODE_AA_ODD>(h, q, gridf); break;
+    }
+    h->launches++;
+    h->phi_current = true;
   }
-  ys = (ys / TY) * TY;
-  if (ys < 2 * TY) ys = 2 * TY;
-  int np = (h->ny + ys - 1) / ys;
-  if (np < 1) np = 1;
-  ys = (((h->ny + np - 1) / np) + TY - 1) / TY * TY;      // balance the strips
-  np = (h->ny + ys - 1) / ys;
-  if (np > 1 && h->ny - (np - 1) * ys < H) np -= 1;       // the last strip must hold the halo of its neighbour
-  if (np > 1 && ys < H) return false;
-  sc.NP = np;
-  sc.YS = ys;
-  const int last_rows = h->ny - (np - 1) * ys;
-  for (int c = 0; c < 3; ++c) {
-    int rows, hb, hf;
-    if (np == 1) { rows = h->ny; hb = 0; hf = 0; }
-    else if (c == 0) { rows = ys; hb = H; hf = H; }
-    else if (c == 1) { rows = ys; hb = 0; hf = H; }
-    else { rows = last_rows; hb = 0; hf = 0; }
-    sc.hb[c] = hb;
-    sc.frow[c] = rows;
-    sc.prow[c] = rows + hb + hf;
-    sc.nFt[c] = sc.ntx * ((rows + TY - 1) / TY);
-    sc.nPt[c] = sc.ntx * ((sc.prow[c] + TY - 1) / TY);
-    sc.tk[c] = (long long)sc.nzs * (sc.nPt[c] + sc.nFt[c]);
-  }
-  sc.total = sc.tk[0] + (np > 2 ? (long long)(np - 2) * sc.tk[1] : 0) + (np > 1 ? sc.tk[2] : 0);
-  if (sc.total >= (1LL << 31)) return false;
-  // lead of P over F: 2 HS + 1 slabs are the data dependence; the slack keeps the polling thread
-  // from ever waiting: the P items F needs were issued >= ~1.5 x resident CTAs tickets earlier
-  int slack = h->tune_slack;
-  if (slack < 0) {
-    const int per_slab = sc.nPt[1] + sc.nFt[1];
-    slack = (int)((1.5 * resident_ctas + per_slab - 1) / per_slab);
-    if (slack < 1) slack = 1;
-  }
-  sc.LEAD = 2 * sc.HS + 1 + slack;
-  if (sc.LEAD > sc.nzs) sc.LEAD = sc.nzs;
-  const size_t ints = 1 + (size_t)np * sc.nzs;
-  if (ints > h->sched_ints) {
-    dev_free(h->sched_buf);
-    h->sched_buf = static_cast<int*>(dev_alloc(ints * sizeof(int)));
-    if (!h->sched_buf) { h->sched_ints = 0; return false; }
-    h->sched_ints = ints;
-  }
-  sc.ticket = h->sched_buf;
-  sc.prefetch = h->tune_prefetch;
-  sc.pdone = h->sched_buf + 1;
-  return true;
-}
-
-template <int MODE, bool HAS_SOLID, bool HAS_NC>
-bool launch_step_t(lb_handle h, const StepParams& p) {
-  auto kern = k_step<MODE, HAS_SOLID, HAS_NC>;
-  int occ = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, TX * TY, 0) != cudaSuccess || occ < 1) { cudaGetLastError(); return false; }
-  if (h->tune_ctas > 0 && occ > h->tune_ctas) occ = h->tune_ctas;
-  if (!h->num_sm) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&h->num_sm, cudaDevAttrMultiProcessorCount, dev);
-  }
-  const int resident = occ * h->num_sm;
-  Sched sc;
-  if (!make_sched(h, sc, resident)) return false;
-  if (cudaMemsetAsync(h->sched_buf, 0, (1 + (size_t)sc.NP * sc.nzs) * sizeof(int), h->stream) != cudaSuccess) { cudaGetLastError(); return false; }
-  const long long grid = sc.total < resident ? sc.total : resident;
-  kern<<<(unsigned)grid, dim3(TX, TY), 0, h->stream>>>(p, h->tmap, sc);
-  return true;
-}
-
-template <int MODE>
-bool launch_step(lb_handle h, const StepParams& p) {
-  const bool nc = h->par.A_nc != 0.f;
-  if (h->has_solid) return nc ? launch_step_t<MODE, true, true>(h, p) : launch_step_t<MODE, true, false>(h, p);
-  return nc ? launch_step_t<MODE, false, true>(h, p) : launch_step_t<MODE, false, false>(h, p);
-}
-
-// K12: one launch per step (two-component runs).  Returns false if the pipelined schedule cannot be
-// used (then the caller falls back to the two-launch form, which is the same arithmetic).
-bool run_step_pipelined(lb_handle h) {
-  float* src = h->cur_buf();
-  float* dst = h->storage == 0 ? h->buf[h->cur ^ 1] : h->buf[0];
-  const StepParams p = make_step_params(h, src, dst, 1);
-  const int mode = h->mode();
-  bool ok;
-  if (mode == MODE_AB) ok = launch_step<MODE_AB>(h, p);
-  else if (mode == MODE_AA_EVEN) ok = launch_step<MODE_AA_EVEN>(h, p);
-  else ok = launch_step<MODE_AA_ODD>(h, p);
-  if (!ok) return false;
-  h->launches++;
-  if (h->storage == 0) h->cur ^= 1;
-  else h->aa_odd ^= 1;
-  h->phi_current = false;
-  return true;
 }
 
 IoParams make_io_params(lb_handle h) {
@@ -427,7 +341,7 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
   if (!p) return fail(nullptr, LB_EINVAL, "params is NULL");
   if (nx < 4 || ny < 4 || nz < 4) return fail(nullptr, LB_EINVAL, "every extent must be >= 4");
   if (nx % 4 != 0) return fail(nullptr, LB_EINVAL, "nx must be a multiple of 4");
-  if ((long long)nx * ny * nz >= (1LL << 31)) return fail(nullptr, LB_EINVAL, "box too large (>= 2^31 sites)");
+  if ((long long)nx * ny * nz >= (1LL << 30)) return fail(nullptr, LB_EINVAL, "box too large (>= 2^30 sites)");
   if (!(p->tau_r > 0.5f) || !(p->tau_b > 0.5f)) return fail(nullptr, LB_EINVAL, "tau must exceed 0.5");
   lb_handle h = new (std::nothrow) lb_handle_s();
   if (!h) return fail(nullptr, LB_ENOMEM, "host allocation failed");
@@ -441,7 +355,7 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
 void lb_destroy(lb_handle h) {
   if (!h) return;
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
-  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->mask); dev_free(h->sched_buf);
+  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->mask); dev_free(h->mom);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
   for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
   cudaGetLastError();
@@ -522,6 +436,13 @@ int allocate_state(lb_handle h, bool two) {
       if (!h->buf[i]) return fail(h, LB_ENOMEM, "population buffer allocation failed");
       h->bytes += pbytes;
     }
+  }
+  if (two && !h->mom) {
+    const size_t ex = (size_t)h->nz * h->ny * ((h->nx + TX - 1) / TX) * 4;   // x-face sums: 2 sides x {D, Tm}
+    const size_t mb = (2 * (size_t)h->S + ex) * sizeof(float);
+    h->mom = static_cast<float*>(dev_alloc(mb));
+    if (!h->mom) return fail(h, LB_ENOMEM, "moment buffer allocation failed");
+    h->bytes += mb;
   }
   if (two && !h->phi) {
     const size_t px = h->nx + 2 * HALO, py = h->ny + 2 * HALO, pz = h->nz + 2 * HALO;
@@ -606,13 +527,9 @@ int lb_step(lb_handle h, int nsteps) {
   cudaEventRecord(h->ev_step[0], h->stream);
   for (int t = 0; t < nsteps; ++t) {
     if (prof) cudaEventRecord(h->ev_k[4 * t + 0], h->stream);
-    const bool piped = h->two && h->pipeline;
-    if (!piped) run_phase(h);
-    if (prof) { cudaEventRecord(h->ev_k[4 * t + 1], h->stream); cudaEventRecord(h->ev_k[4 * t + 2], h->stream); }
-    if (!piped || !run_step_pipelined(h)) {
-      if (piped) run_phase(h);     // schedule not applicable to this box: two-launch form
-      run_collide(h);
-    }
+    run_phase(h);                 // K1: no-op unless phi is stale (first step, or forwarding off)
+    if (prof) cudaEventRecord(h->ev_k[4 * t + 1], h->stream);
+    run_collide(h, prof ? h->ev_k[4 * t + 2] : nullptr);   // K2 (+ K1f) or K2s
     if (prof) cudaEventRecord(h->ev_k[4 * t + 3], h->stream);
   }
   cudaEventRecord(h->ev_step[1], h->stream);
@@ -715,12 +632,8 @@ const char* lb_last_error(lb_handle h) { return h ? h->err.c_str() : g_create_er
 int lb_set_tuning(lb_handle h, const char* key, int value) {
   if (!h || !key) return LB_EINVAL;
   const std::string k(key);
-  if (k == "pipeline") h->pipeline = value ? 1 : 0;
-  else if (k == "zs") h->tune_zs = value;
-  else if (k == "slack") h->tune_slack = value;
-  else if (k == "ys") h->tune_ys = value;
-  else if (k == "ctas_per_sm") h->tune_ctas = value;
-  else if (k == "prefetch") h->tune_prefetch = value;
+  if (k == "forward") h->forward = value ? 1 : 0;
+  else if (k == "zc") h->tune_zc = value;
   else return fail(h, LB_EINVAL, "unknown tuning key: " + k);
   return LB_OK;
 }
@@ -745,8 +658,14 @@ int lb_last_step_ms(lb_handle h, int which, float* ms) {
   float total = 0.f;
   for (int t = 0; t < h->ev_steps; ++t) {
     float v = 0.f;
-    const int a = which == 1 ? 4 * t + 2 : 4 * t + 0;
-    e = cudaEventElapsedTime(&v, h->ev_k[a], h->ev_k[a + 1]);
+    if (which == 1) {
+      e = cudaEventElapsedTime(&v, h->ev_k[4 * t + 1], h->ev_k[4 * t + 2]);
+    } else {
+      float v2 = 0.f;
+      e = cudaEventElapsedTime(&v, h->ev_k[4 * t + 0], h->ev_k[4 * t + 1]);
+      if (e == cudaSuccess) e = cudaEventElapsedTime(&v2, h->ev_k[4 * t + 2], h->ev_k[4 * t + 3]);
+      v += v2;
+    }
     if (e != cudaSuccess) return cuda_fail(h, e, "event elapsed");
     total += v;
   }

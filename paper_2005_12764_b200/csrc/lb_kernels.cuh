@@ -26,7 +26,10 @@ namespace lb {
 struct StepParams {
   const float* src;   // population buffer read by this step
   float* dst;         // buffer written (== src in AA modes)
-  float* phi;         // padded phi array (written by K1, read by K2/K3)
+  float* phi;         // padded phi array (written by K1 / K1f, read by K2 / K3)
+  float* Md;          // forwarded moments of the next state (written by K2, read by K1f):
+  float* Mt;          //   Md = sum (f^r - f^b), Mt = sum (f - w) over what arrives from inside the brick
+  float* EX;          // the same sums for what crosses the x faces of the bricks: [z][y][tile][side]{D, Tm}
   Box box;
   int zc;             // z planes per CTA
   int halo;           // ghost depth K1 must fill (1 without near contact, 4 with)
@@ -37,52 +40,83 @@ struct StepParams {
 constexpr int TX = 32, TY = 8;   // CTA tile in x-y; one warp per x row segment
 
 // ----------------------------------------------------------------------------- addressing
-struct Ctx {
-  int idx;            // own site
-  int dxo[3];         // index deltas to x-1, x, x+1 (wrapped)
-  int dyo[3];         // to y-1, y, y+1
-  int dzo[3];         // to z-1, z, z+1
-  long long S;
+// A population lives in plane `plane` (0..18, + 19 for the red set) at byte offset `off` inside
+// the plane.  Offsets are 32-bit (a plane is < 4 GB: S < 2^30), plane bases are uniform across
+// the warp, so one access costs one integer add instead of a 64-bit index computation.
+struct Slot {
+  int plane;
+  uint32_t off;
 };
 
-// Index delta from the own site to x - c_q.
+struct Ctx {
+  int idx;            // own site (elements)
+  uint32_t ob;        // own site (bytes)
+  int dxo[3];         // byte deltas to x-1, x, x+1 (wrapped)
+  int dyo[3];         // to y-1, y, y+1
+  int dzo[3];         // to z-1, z, z+1
+  size_t Sb;          // bytes per plane
+};
+
+// Byte delta from the own site to x - c_q.
 template <int q>
 __device__ __forceinline__ int delta_src(const Ctx& c) {
   return c.dxo[1 - cx(q)] + c.dyo[1 - cy(q)] + c.dzo[1 - cz(q)];
 }
 
-// Flattened (plane * S + site) location that holds f_q(x) of the current state.
-// smask bit i set <=> x + c_i is solid.
+// Where f_q(x) of the current state is stored.  smask bit i set <=> x + c_i is solid.
 template <int MODE, bool HAS_SOLID, int q>
-__device__ __forceinline__ size_t read_slot(const Ctx& c, uint32_t smask) {
+__device__ __forceinline__ Slot read_slot(const Ctx& c, uint32_t smask) {
   if constexpr (MODE == MODE_AA_EVEN || q == 0) {
-    return (size_t)q * c.S + c.idx;
+    return Slot{q, c.ob};
   } else {
-    const bool bounce = HAS_SOLID && ((smask >> opp(q)) & 1u);
-    if constexpr (MODE == MODE_AB) {
-      return bounce ? (size_t)opp(q) * c.S + c.idx : (size_t)q * c.S + (c.idx + delta_src<q>(c));
-    } else {  // AA_ODD
-      return bounce ? (size_t)q * c.S + c.idx : (size_t)opp(q) * c.S + (c.idx + delta_src<q>(c));
+    const uint32_t nb = c.ob + (uint32_t)delta_src<q>(c);
+    if constexpr (!HAS_SOLID) {
+      return MODE == MODE_AB ? Slot{q, nb} : Slot{opp(q), nb};
+    } else {
+      const bool bounce = (smask >> opp(q)) & 1u;
+      if constexpr (MODE == MODE_AB) return bounce ? Slot{opp(q), c.ob} : Slot{q, nb};
+      else return bounce ? Slot{q, c.ob} : Slot{opp(q), nb};   // AA_ODD
     }
   }
 }
 
 // Where the post-collision value f*_q goes.
 template <int MODE, bool HAS_SOLID, int q>
-__device__ __forceinline__ size_t write_slot(const Ctx& c, uint32_t smask) {
+__device__ __forceinline__ Slot write_slot(const Ctx& c, uint32_t smask) {
   if constexpr (MODE == MODE_AB) {
-    return (size_t)q * c.S + c.idx;
+    return Slot{q, c.ob};
   } else if constexpr (MODE == MODE_AA_EVEN) {
-    return (size_t)opp(q) * c.S + c.idx;
+    return Slot{opp(q), c.ob};
   } else {
     return read_slot<MODE, HAS_SOLID, opp(q)>(c, smask);
   }
+}
+
+// comp = 0: total-deviation planes, 1: red planes
+__device__ __forceinline__ const float* slot_ptr(const float* base, const Ctx& c, Slot s, int comp) {
+  return reinterpret_cast<const float*>(reinterpret_cast<const char*>(base) + (size_t)(s.plane + comp * Q) * c.Sb + s.off);
+}
+__device__ __forceinline__ float* slot_ptr(float* base, const Ctx& c, Slot s, int comp) {
+  return reinterpret_cast<float*>(reinterpret_cast<char*>(base) + (size_t)(s.plane + comp * Q) * c.Sb + s.off);
 }
 
 template <int MODE>
 __device__ __forceinline__ float ld_pop(const float* p) {
   if constexpr (MODE == MODE_AB) return __ldg(p);   // source buffer is read-only in A/B mode
   else return *p;
+}
+
+// c_q . a without the multiplications by 0 and +-1 that IEEE arithmetic would not let the compiler drop
+template <int q>
+__device__ __forceinline__ float cdot(float ax, float ay, float az) {
+  constexpr int X = cx(q), Y = cy(q), Z = cz(q);
+  if constexpr (X != 0 && Y != 0) return (X > 0 ? ax : -ax) + (Y > 0 ? ay : -ay);
+  else if constexpr (X != 0 && Z != 0) return (X > 0 ? ax : -ax) + (Z > 0 ? az : -az);
+  else if constexpr (Y != 0 && Z != 0) return (Y > 0 ? ay : -ay) + (Z > 0 ? az : -az);
+  else if constexpr (X != 0) return X > 0 ? ax : -ax;
+  else if constexpr (Y != 0) return Y > 0 ? ay : -ay;
+  else if constexpr (Z != 0) return Z > 0 ? az : -az;
+  else return 0.0f;
 }
 
 // Solid flags of the 18 neighbours from the bit-packed mask (bit i <=> x + c_i solid).
@@ -99,15 +133,17 @@ __device__ __forceinline__ uint32_t neighbour_mask(const Box& b, int x, int y, i
 }
 
 __device__ __forceinline__ void make_ctx(Ctx& c, const Box& b, int x, int y, int z) {
-  c.S = b.S;
+  c.Sb = (size_t)b.S * sizeof(float);
   c.idx = x + b.nx * (y + b.ny * z);
-  c.dxo[0] = (x == 0 ? b.nx - 1 : -1);
+  c.ob = (uint32_t)c.idx * 4u;
+  c.dxo[0] = (x == 0 ? b.nx - 1 : -1) * 4;
   c.dxo[1] = 0;
-  c.dxo[2] = (x == b.nx - 1 ? -(b.nx - 1) : 1);
-  c.dyo[0] = (y == 0 ? b.ny - 1 : -1) * b.nx;
+  c.dxo[2] = (x == b.nx - 1 ? -(b.nx - 1) : 1) * 4;
+  const int row = b.nx * 4;
+  c.dyo[0] = (y == 0 ? b.ny - 1 : -1) * row;
   c.dyo[1] = 0;
-  c.dyo[2] = (y == b.ny - 1 ? -(b.ny - 1) : 1) * b.nx;
-  const int pl = b.nx * b.ny;
+  c.dyo[2] = (y == b.ny - 1 ? -(b.ny - 1) : 1) * row;
+  const int pl = b.nx * b.ny * 4;
   c.dzo[0] = (z == 0 ? b.nz - 1 : -1) * pl;
   c.dzo[1] = 0;
   c.dzo[2] = (z == b.nz - 1 ? -(b.nz - 1) : 1) * pl;
@@ -121,13 +157,35 @@ __device__ __forceinline__ void two_sum_acc(float& s, float& e, float x) {
   s = t;
 }
 
+// phi of site (x, y, z) to its home in the padded array and to every periodic image that falls
+// into the ghost layers (depth H).
+__device__ __forceinline__ void store_phi_with_images(const StepParams& p, int x, int y, int z, int H, float phi) {
+  const Box& b = p.box;
+  const int px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
+  const int sx[3] = {0, x < H ? b.nx : 0, x >= b.nx - H ? -b.nx : 0};
+  const int sy[3] = {0, y < H ? b.ny : 0, y >= b.ny - H ? -b.ny : 0};
+  const int sz[3] = {0, z < H ? b.nz : 0, z >= b.nz - H ? -b.nz : 0};
+#pragma unroll
+  for (int iz = 0; iz < 3; ++iz) {
+    if (iz && !sz[iz]) continue;
+#pragma unroll
+    for (int iy = 0; iy < 3; ++iy) {
+      if (iy && !sy[iy]) continue;
+#pragma unroll
+      for (int ix = 0; ix < 3; ++ix) {
+        if (ix && !sx[ix]) continue;
+        p.phi[(size_t)(x + sx[ix] + HALO) + (size_t)px * ((size_t)(y + sy[iy] + HALO) + (size_t)py * (size_t)(z + sz[iz] + HALO))] = phi;
+      }
+    }
+  }
+}
+
 // ----------------------------------------------------------------------------- K1 phase field
 // One thread per site of a TX x TY tile, marching over zc planes.  152 B read, 4 B written.
 template <int MODE, bool HAS_SOLID>
 __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, int zb, int ze) {
   const Box& b = p.box;
   const int H = p.halo;
-  const int px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
   for (int z = zb; z < ze; ++z) {
     Ctx c;
     make_ctx(c, b, x, y, z);
@@ -144,9 +202,9 @@ __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, 
       float t[Q], r[Q];
       static_for<0, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
-        const size_t s = read_slot<MODE, HAS_SOLID, q>(c, smask);
-        t[q] = ld_pop<MODE>(p.src + s);
-        r[q] = ld_pop<MODE>(p.src + (size_t)Q * c.S + s);
+        const Slot s = read_slot<MODE, HAS_SOLID, q>(c, smask);
+        t[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 0));
+        r[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 1));
       });
       // Compensated (two-sum) accumulation: the direction of grad phi, which the perturbation and
       // the recolouring use, is ill-conditioned where |grad phi| is small, so phi is formed to
@@ -162,23 +220,7 @@ __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, 
       const float rho = (1.0f + dr) + de;
       phi = num / rho;
     }
-    // home location plus the periodic images that fall into the ghost layers
-    const int sx[3] = {0, x < H ? b.nx : 0, x >= b.nx - H ? -b.nx : 0};
-    const int sy[3] = {0, y < H ? b.ny : 0, y >= b.ny - H ? -b.ny : 0};
-    const int sz[3] = {0, z < H ? b.nz : 0, z >= b.nz - H ? -b.nz : 0};
-#pragma unroll
-    for (int iz = 0; iz < 3; ++iz) {
-      if (iz && !sz[iz]) continue;
-#pragma unroll
-      for (int iy = 0; iy < 3; ++iy) {
-        if (iy && !sy[iy]) continue;
-#pragma unroll
-        for (int ix = 0; ix < 3; ++ix) {
-          if (ix && !sx[ix]) continue;
-          p.phi[(size_t)(x + sx[ix] + HALO) + (size_t)px * ((size_t)(y + sy[iy] + HALO) + (size_t)py * (size_t)(z + sz[iz] + HALO))] = phi;
-        }
-      }
-    }
+    store_phi_with_images(p, x, y, z, H, phi);
   }
 }
 
@@ -235,58 +277,101 @@ struct Ring {
 };
 
 // ----------------------------------------------------------------------------- K2 fused
-// Per thread: one site per plane, marching over zc planes; per CTA a TX x TY tile.  The phi
-// planes z-H..z+H (+2 prefetched) of the tile with an H-wide halo live in a shared-memory ring
-// filled by TMA from the padded phi array (ghost layers make every box in-bounds, so periodic
-// wrap never reaches the TMA unit).  H = 1 without near contact, 4 with it.
-// One TX x TY tile starting at (x0, y0), planes [zb, ze).  `ring`/`bars` are the CTA's phi ring and
-// its mbarriers (initialised once per CTA); `jbase` counts the planes this CTA has pushed through the
-// ring so far, so that slot numbers and mbarrier phase parities carry over from one call to the next.
+// Per thread: one site per plane, marching over zc planes; per CTA a TX x TY tile ("brick" =
+// tile x z range of the CTA).  The phi planes z-H..z+H (+ 2 prefetched) of the tile with an H-wide
+// halo live in a shared-memory ring filled by TMA from the padded phi array (ghost layers make
+// every box in-bounds, so periodic wrap never reaches the TMA unit).  H = 1 without near
+// contact, 4 with it.
+//
+// Moment forwarding.  The next step needs phi(t+1) = (rho_r - rho_b)/rho of the populations that
+// will ARRIVE at each site, i.e. sums over the neighbours' post-collision values.  Instead of a
+// second sweep over the 38 planes (k_phase), this kernel adds up, for every site of its brick,
+// the contributions that come from inside the brick while the post-collision values are still in
+// registers:  D(y) = sum_q (f^r*_q - f^b*_q)(y - c_q),  Tm(y) = sum_q (f*_q - w_q)(y - c_q).
+// x: warp shuffles (a row of 32 sites is one warp); y: one shared-memory exchange per plane;
+// z: carried in registers from one plane to the next (plane z-1 is complete once plane z is done).
+// A population that would enter a solid site returns to its own site (bounce-back) and is added
+// there.  What enters a brick through its faces is added by k_phase_fwd from the stored values.
+template <int H>
+struct FusedSmem {
+  static constexpr int NEX = 12;   // exchanged values: 6 (cy = +-1) x {D, Tm}
+  static constexpr size_t RING = (size_t)Ring<H>::NS * Ring<H>::SLOT * sizeof(float);
+  static constexpr size_t YEX = (size_t)2 * NEX * TX * TY * sizeof(float);
+  static constexpr size_t XEX = (size_t)2 * 2 * 4 * TY * sizeof(float);   // [buffer][side][(+1,-1) x {D, Tm}][row]
+  static constexpr size_t BYTES = RING + YEX + XEX + Ring<H>::NS * sizeof(uint64_t);
+};
+
 template <int MODE, bool HAS_SOLID, bool HAS_NC>
-__device__ __forceinline__ void fused_column(const StepParams& p, const CUtensorMap& tmap, float* ring, uint64_t* bars,
-                                             int x0, int y0, int ylim, int zb, int ze, uint32_t& jbase) {
+__global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
   using R_ = Ring<H>;
+  using SM_ = FusedSmem<H>;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float* ring = reinterpret_cast<float*>(smem_raw);
+  float* yex = reinterpret_cast<float*>(smem_raw + SM_::RING);                 // [2][NEX][TY][TX]
+  float* xex = reinterpret_cast<float*>(smem_raw + SM_::RING + SM_::YEX);     // [2][2][4][TY]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + SM_::RING + SM_::YEX + SM_::XEX);
+
   const Box& b = p.box;
   const int tid = threadIdx.y * TX + threadIdx.x;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int x = x0 + threadIdx.x, y = y0 + threadIdx.y;
-  const bool active = x < b.nx && y < ylim;
+  const bool active = x < b.nx && y < b.ny;
+  const int zb = blockIdx.z * p.zc;
+  const int ze = min(b.nz, zb + p.zc);
   const int npl = (ze - zb) + 2 * H;
-  const uint32_t jb = jbase;
-  jbase += npl;
 
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < R_::NS; ++s) mbar_init(&bars[s], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
   auto issue = [&](int j) {
-    const int s = (jb + j) % R_::NS;
+    const int s = j % R_::NS;
     mbar_expect_tx(&bars[s], R_::BYTES);
     tma_load_3d(&ring[s * R_::SLOT], &tmap, &bars[s], x0, y0 + HALO - H, zb - H + j + HALO);
   };
-  auto wait = [&](int j) { mbar_wait(&bars[(jb + j) % R_::NS], ((jb + j) / R_::NS) & 1); };
   if (tid == 0) {
-    const int n0 = min(npl, R_::NS - 1);
+    const int n0 = min(npl, R_::NS);
     for (int j = 0; j < n0; ++j) issue(j);
   }
 
   const float omega_same = 1.0f / p.tau_r;
   const float nu_r = (p.tau_r - 0.5f) * (1.0f / 3.0f), nu_b = (p.tau_b - 0.5f) * (1.0f / 3.0f);
   const int lx = threadIdx.x + HALO, ly = threadIdx.y + H;
+  const size_t plane_sites = (size_t)b.nx * b.ny;
+  const size_t col = (size_t)x + (size_t)b.nx * y;
+  // carried between planes: pend = b0(z-1) + b+(z-2) (plane z-1 still misses b-(z)), bpc = b+(z-1)
+  float pend_d = 0.f, pend_t = 0.f, bpc_d = 0.f, bpc_t = 0.f;
+  // the same for what leaves the brick through its x faces (kept by the first and the last active
+  // lane of each row): the sums land in p.EX, indexed by target row and plane, and k_phase_fwd adds
+  // them to the first / last column of the neighbouring brick
+  const int lastx = min(TX, b.nx - x0) - 1;
+  const bool lL = threadIdx.x == 0, lR = (int)threadIdx.x == lastx;
+  const int side = lR ? 1 : 0;
+  float pe_d = 0.f, pe_t = 0.f, bpe_d = 0.f, bpe_t = 0.f;
+  const int ntx = gridDim.x;
 
   for (int jz = 0; jz < ze - zb; ++jz) {
     const int z = zb + jz;
-    if (tid == 0) {
-      const int j = jz + R_::NS - 1;
-      if (j < npl) issue(j);
-    }
     if (jz == 0) {
 #pragma unroll
-      for (int j = 0; j <= 2 * H; ++j) wait(j);
+      for (int j = 0; j <= 2 * H; ++j) mbar_wait(&bars[j % R_::NS], (j / R_::NS) & 1);
     } else {
-      wait(jz + 2 * H);
+      const int j = jz + 2 * H;
+      mbar_wait(&bars[j % R_::NS], (j / R_::NS) & 1);
     }
     // plane dz of the ring
-    auto plane = [&](int dz) -> const float* { return &ring[((jb + jz + H + dz) % R_::NS) * R_::SLOT]; };
+    auto plane = [&](int dz) -> const float* { return &ring[((jz + H + dz) % R_::NS) * R_::SLOT]; };
     const float* pl0 = plane(0);
     const float phi0 = pl0[ly * R_::BX + lx];
     const bool fluid = active && !(HAS_SOLID && phi0 > PHI_SOLID_TEST);
+    // what this site sends along each direction: vd = f^r* - f^b*, vt = f* - w (zero if not fluid)
+    float vd[Q], vt[Q];
+#pragma unroll
+    for (int q = 0; q < Q; ++q) { vd[q] = 0.f; vt[q] = 0.f; }
     if (fluid) {
       Ctx c;
       make_ctx(c, b, x, y, z);
@@ -311,9 +396,9 @@ __device__ __forceinline__ void fused_column(const StepParams& p, const CUtensor
       float T[Q], R[Q];
       static_for<0, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
-        const size_t s = read_slot<MODE, HAS_SOLID, q>(c, smask);
-        T[q] = ld_pop<MODE>(p.src + s);
-        R[q] = ld_pop<MODE>(p.src + (size_t)Q * c.S + s);
+        const Slot s = read_slot<MODE, HAS_SOLID, q>(c, smask);
+        T[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 0));
+        R[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 1));
       });
       // ---- moments (Eq. 3)
       float dr = 0.f, rr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
@@ -371,8 +456,6 @@ __device__ __forceinline__ void fused_column(const StepParams& p, const CUtensor
       const float kcol = p.beta * rr * rb * inv_rho * invG;   // recolouring amplitude / |G|
       const float om1 = 1.0f - omega;
       // ---- collide on the total (deviation form), perturb, recolour, store
-      float* dT = p.dst;
-      float* dR = p.dst + (size_t)Q * c.S;
       // Directions 1..18 first; the rest populations then take what is left of rho - 1 and of
       // rho_r (collision conserves both at every site), so that the per-site masses are conserved
       // to the rounding of one sum instead of carrying the relative error of rho_r/rho or of
@@ -381,12 +464,12 @@ __device__ __forceinline__ void fused_column(const StepParams& p, const CUtensor
       static_for<1, Q + 1>([&](auto qc) {
         constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
         constexpr float w = wq(q);
-        const float cu = cx(q) * ux + cy(q) * uy + cz(q) * uz;
-        const float cG = cx(q) * Gx + cy(q) * Gy + cz(q) * Gz;
+        const float cu = cdot<q>(ux, uy, uz);
+        const float cG = cdot<q>(Gx, Gy, Gz);
         const float teq = w * (dr + rho * (3.0f * cu + 4.5f * cu * cu - uu15));
         float ts = om1 * T[q] + omega * teq;
         if (forced) {
-          const float cF = cx(q) * Fx + cy(q) * Fy + cz(q) * Fz;
+          const float cF = cdot<q>(Fx, Fy, Fz);
           ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
         }
         ts += p.A * (w * cG * cG * invG - bq(q) * Gne);
@@ -399,230 +482,153 @@ __device__ __forceinline__ void fused_column(const StepParams& p, const CUtensor
           ts = dr - tacc;
           rs = rr - racc;
         }
-        const size_t s = write_slot<MODE, HAS_SOLID, q>(c, smask);
-        dT[s] = ts;
-        dR[s] = rs;
+        const Slot s = write_slot<MODE, HAS_SOLID, q>(c, smask);
+        *slot_ptr(p.dst, c, s, 0) = ts;
+        *slot_ptr(p.dst, c, s, 1) = rs;
+        // f^r* - f^b* = 2 f^r* - f* = (2 rs - w) - ts: the first difference is exact in the mixed
+        // regions where phi matters, so the forwarded sum keeps ~1e-8 there
+        vd[q] = (2.0f * rs - w) - ts;
+        vt[q] = ts;
       });
-    }
-    __syncthreads();   // everyone is done with plane jz before its slot is refilled
-  }
-}
-
-template <int H>
-__device__ __forceinline__ void ring_init(uint64_t* bars) {
-  if (threadIdx.y * TX + threadIdx.x == 0) {
-#pragma unroll
-    for (int s = 0; s < Ring<H>::NS; ++s) mbar_init(&bars[s], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  }
-  __syncthreads();
-}
-
-template <int MODE, bool HAS_SOLID, bool HAS_NC>
-__global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
-  constexpr int H = HAS_NC ? H_MAX_NC : 1;
-  __shared__ __align__(128) float ring[Ring<H>::NS * Ring<H>::SLOT];
-  __shared__ __align__(8) uint64_t bars[Ring<H>::NS];
-  ring_init<H>(bars);
-  uint32_t jbase = 0;
-  const int zb = blockIdx.z * p.zc;
-  fused_column<MODE, HAS_SOLID, HAS_NC>(p, tmap, ring, bars, blockIdx.x * TX, blockIdx.y * TY, p.box.ny, zb, min(p.box.nz, zb + p.zc), jbase);
-}
-
-// ----------------------------------------------------------------------------- K12 pipelined step
-// One launch per LB step doing the work of K1 and K2 in an order that lets K2's gather hit in L2.
-// The box is cut into pencils (y strips of YS rows, full x extent, all z) that are processed one
-// after another; inside a pencil the work is cut into items of one TX x TY tile x ZS planes and
-// ordered z-slab by z-slab: the phase-field items P(k) of slab k run LEAD slabs ahead of the fused
-// items F(s).  P(k) pulls the 38 planes of slab k from HBM; F(k) gathers the same lines a few
-// hundred items later, while they are still in the 126 MB L2, so HBM sees each population once.
-// Persistent CTAs draw items from a global ticket counter in schedule order.  F(s) needs phi on
-// planes [s ZS - H, (s+1) ZS + H) of its tile and halo, i.e. completed P items with SMALLER ticket
-// numbers only; P items never wait.  The CTA holding the smallest unfinished ticket can therefore
-// always proceed: no deadlock, whether or not all CTAs are co-resident.  Completion is published
-// per (pencil, slab) with a release (fence + atomic add) and observed by one polling thread with an
-// acquire followed by fence.proxy.async, because the consumer of phi is the TMA unit.
-struct Sched {
-  int ZS, nzs, HS, LEAD;     // planes per slab, slabs, halo in slabs, lead of P over F in slabs
-  int H;                     // phi halo (1 or 4)
-  int ntx;                   // tiles along x
-  int NP, YS;                // pencils, rows per pencil (multiple of TY; the last pencil takes the rest)
-  // pencil classes: 0 = first, 1 = middle, 2 = last (a single pencil is class 0 with no halo)
-  int hb[3], prow[3], frow[3];   // backward halo rows, P rows (interior + halos), F rows
-  int nPt[3], nFt[3];            // P tiles and F tiles per slab
-  long long tk[3];               // tickets per pencil of this class
-  long long total;               // tickets per step
-  int* ticket;                   // global ticket counter (zeroed before the launch)
-  int* pdone;                    // [NP][nzs] completed P items (zeroed before the launch)
-  int prefetch;                  // hint the next P item's lines into L2 while the current item runs
-};
-
-struct Item {
-  int type;      // 0 = P, 1 = F, -1 = none
-  int pencil, cls, slab, tx, ty;
-};
-
-__device__ __forceinline__ Item decode_ticket(const Sched& sc, long long t) {
-  Item it;
-  it.type = -1;
-  if (t >= sc.total) return it;
-  int pencil = 0, cls = 0;
-  if (t >= sc.tk[0]) {
-    t -= sc.tk[0];
-    const long long nmid = sc.NP - 2;
-    if (nmid > 0 && t < nmid * sc.tk[1]) {
-      pencil = 1 + (int)(t / sc.tk[1]);
-      t -= (long long)(pencil - 1) * sc.tk[1];
-      cls = 1;
-    } else {
-      if (nmid > 0) t -= nmid * sc.tk[1];
-      pencil = sc.NP - 1;
-      cls = 2;
-    }
-  }
-  it.pencil = pencil;
-  it.cls = cls;
-  const int nP = sc.nPt[cls], nF = sc.nFt[cls];
-  int u = (int)t, tile;
-  const int A = sc.LEAD * nP;
-  if (u < A) {
-    it.type = 0; it.slab = u / nP; tile = u - it.slab * nP;
-  } else {
-    u -= A;
-    const int pair = nP + nF, npairs = sc.nzs - sc.LEAD;
-    if (u < npairs * pair) {
-      const int i = u / pair, r = u - i * pair;
-      if (r < nF) { it.type = 1; it.slab = i; tile = r; }
-      else { it.type = 0; it.slab = sc.LEAD + i; tile = r - nF; }
-    } else {
-      u -= npairs * pair;
-      const int i = u / nF;
-      it.type = 1; it.slab = npairs + i; tile = u - i * nF;
-    }
-  }
-  if (it.type == 0) {   // P slabs start HS slabs below the top so that F(0) finds its lower halo
-    it.slab = it.slab + sc.nzs - sc.HS;
-    if (it.slab >= sc.nzs) it.slab -= sc.nzs;
-  }
-  it.ty = tile / sc.ntx;
-  it.tx = tile - it.ty * sc.ntx;
-  return it;
-}
-
-__device__ __forceinline__ int ld_acquire(const int* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-
-__device__ __forceinline__ int ld_relaxed(const int* p) {
-  int v;
-  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-
-// Block until every P item that F(pencil, slab) depends on has been published (one thread calls).
-// All counters are read with independent relaxed loads (their latencies overlap), then one fence
-// gives the acquire; fence.proxy.async orders the phi data before the TMA reads that follow.
-__device__ __forceinline__ void wait_phi_ready(const Sched& sc, const Box& b, int pencil, int slab) {
-  const int zb = slab * sc.ZS, ze = min(b.nz, zb + sc.ZS);
-  // own pencil, the pencil behind (its interior holds our backward halo rows) and, for the last
-  // pencil, pencil 0 (our forward halo rows wrap onto it)
-  int who[3] = {pencil, pencil, pencil};
-  if (sc.NP > 1) {
-    if (pencil > 0) who[1] = pencil - 1;
-    if (pencil == sc.NP - 1) who[2] = 0;
-  }
-  int need[3];
-#pragma unroll
-  for (int i = 0; i < 3; ++i) need[i] = sc.nPt[who[i] == 0 ? 0 : (who[i] == sc.NP - 1 ? 2 : 1)];
-  bool ok;
-  do {
-    ok = true;
-    for (int pl = zb - sc.H; pl < ze + sc.H; ++pl) {
-      int w = pl;
-      while (w < 0) w += b.nz;
-      while (w >= b.nz) w -= b.nz;
-      const int k = w / sc.ZS;
-#pragma unroll
-      for (int i = 0; i < 3; ++i) ok &= ld_relaxed(sc.pdone + (size_t)who[i] * sc.nzs + k) >= need[i];
-    }
-    if (!ok) __nanosleep(100);
-  } while (!ok);
-  __threadfence();
-  asm volatile("fence.proxy.async;" ::: "memory");
-}
-
-// Hint the lines that P item `it` will gather into L2 (one line per component, direction, row, plane).
-template <int MODE>
-__device__ __forceinline__ void prefetch_p_item(const StepParams& p, const Sched& sc, const Item& it, int tid) {
-  const Box& b = p.box;
-  const int zb = it.slab * sc.ZS, ze = min(b.nz, zb + sc.ZS);
-  const int rows = min(TY, sc.prow[it.cls] - it.ty * TY);
-  const int x0 = it.tx * TX;
-  const int n = 2 * Q * rows * (ze - zb);
-  for (int i = tid; i < n; i += TX * TY) {
-    const int pq = i % (2 * Q);
-    const int rz = i / (2 * Q);
-    const int r = rz % rows, z = zb + rz / rows;
-    const int q = pq % Q;
-    int y = it.pencil * sc.YS - sc.hb[it.cls] + it.ty * TY + r;
-    int dx = 0, dy = 0, dz = 0, plane = q;
-    if (MODE != MODE_AA_EVEN) { dx = c_cx[q]; dy = c_cy[q]; dz = c_cz[q]; }
-    if (MODE == MODE_AA_ODD) plane = opp(q);
-    y -= dy;
-    while (y < 0) y += b.ny;
-    while (y >= b.ny) y -= b.ny;
-    int zz = z - dz;
-    if (zz < 0) zz += b.nz;
-    if (zz >= b.nz) zz -= b.nz;
-    int xx = x0 + (dx < 0 ? TX - 1 : 0);          // the line that holds all but one element of the row
-    if (xx >= b.nx) xx = b.nx - 1;
-    const float* a = p.src + (size_t)(plane + (pq >= Q ? Q : 0)) * b.S + ((size_t)xx + (size_t)b.nx * ((size_t)y + (size_t)b.ny * zz));
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
-  }
-}
-
-template <int MODE, bool HAS_SOLID, bool HAS_NC>
-__global__ void __launch_bounds__(TX* TY, 3) k_step(const StepParams p, const __grid_constant__ CUtensorMap tmap, const Sched sc) {
-  constexpr int H = HAS_NC ? H_MAX_NC : 1;
-  __shared__ __align__(128) float ring[Ring<H>::NS * Ring<H>::SLOT];
-  __shared__ __align__(8) uint64_t bars[Ring<H>::NS];
-  __shared__ int tq[4];          // ticket queue: current, next (prefetched into L2), two in flight
-  const int tid = threadIdx.y * TX + threadIdx.x;
-  const Box& b = p.box;
-  if (tid < 3) tq[tid] = atomicAdd(sc.ticket, 1);
-  ring_init<H>(bars);          // ends with __syncthreads: the queue is visible
-  uint32_t jbase = 0;
-  for (int i = 0;; ++i) {
-    const Item it = decode_ticket(sc, tq[i & 3]);
-    if (it.type < 0) break;
-    const Item nx = decode_ticket(sc, tq[(i + 1) & 3]);
-    if (tid == 0) tq[(i + 3) & 3] = atomicAdd(sc.ticket, 1);
-    if (sc.prefetch && nx.type == 0) prefetch_p_item<MODE>(p, sc, nx, tid);
-    const int y0p = (it.pencil * sc.YS);                           // first interior row of the pencil
-    const int zb = it.slab * sc.ZS, ze = min(b.nz, zb + sc.ZS);
-    if (it.type == 0) {
-      const int r = it.ty * TY + threadIdx.y;                        // row inside the pencil's P range
-      const int x = it.tx * TX + threadIdx.x;
-      if (r < sc.prow[it.cls] && x < b.nx) {
-        int y = y0p - sc.hb[it.cls] + r;
-        if (y < 0) y += b.ny;
-        if (y >= b.ny) y -= b.ny;
-        phase_column<MODE, HAS_SOLID>(p, x, y, zb, ze);
+      if constexpr (HAS_SOLID) {   // link bounce-back: what would enter a solid site comes back here
+        float sd = 0.f, st = 0.f;
+        static_for<1, Q>([&](auto qc) {
+          constexpr int q = decltype(qc)::value;
+          if ((smask >> q) & 1u) { sd += vd[q]; st += vt[q]; vd[q] = 0.f; vt[q] = 0.f; }
+        });
+        vd[0] += sd;
+        vt[0] += st;
       }
-      __syncthreads();
-      if (tid == 0) {
-        __threadfence();
-        atomicAdd(sc.pdone + (size_t)it.pencil * sc.nzs + it.slab, 1);
-      }
-    } else {
-      if (tid == 0) wait_phi_ready(sc, b, it.pencil, it.slab);
-      fused_column<MODE, HAS_SOLID, HAS_NC>(p, tmap, ring, bars, it.tx * TX, y0p + it.ty * TY,
-                                            min(b.ny, y0p + sc.frow[it.cls]), zb, ze, jbase);
-      // fused_column ends with __syncthreads
     }
+    // ---- forward the moments.  x: target lane L receives c_x = +1 values from lane L-1 and
+    // c_x = -1 values from lane L+1; nothing crosses the ends of the warp row (brick faces).
+    const unsigned full = 0xffffffffu;
+    const bool l0 = threadIdx.x == 0, l31 = threadIdx.x == TX - 1;
+    auto up = [&](float v) { const float t = __shfl_up_sync(full, v, 1); return l0 ? 0.f : t; };
+    auto down = [&](float v) { const float t = __shfl_down_sync(full, v, 1); return l31 ? 0.f : t; };
+    // a[cy][cz] after the x step (velocity order: include/lb.h)
+    const float a00_d = vd[0] + up(vd[1]) + down(vd[2]),  a00_t = vt[0] + up(vt[1]) + down(vt[2]);
+    const float ap0_d = vd[3] + up(vd[7]) + down(vd[10]), ap0_t = vt[3] + up(vt[7]) + down(vt[10]);
+    const float am0_d = vd[4] + up(vd[9]) + down(vd[8]),  am0_t = vt[4] + up(vt[9]) + down(vt[8]);
+    const float a0p_d = vd[5] + up(vd[11]) + down(vd[14]), a0p_t = vt[5] + up(vt[11]) + down(vt[14]);
+    const float a0m_d = vd[6] + up(vd[13]) + down(vd[12]), a0m_t = vt[6] + up(vt[13]) + down(vt[12]);
+    // what crosses the x faces: c_x = -1 values of lane 0 (left), c_x = +1 values of the last lane (right)
+    const float e00_d = lL ? vd[2] : vd[1],   e00_t = lL ? vt[2] : vt[1];      // (0, 0)
+    const float ep0_d = lL ? vd[10] : vd[7],  ep0_t = lL ? vt[10] : vt[7];     // (+1, 0)
+    const float em0_d = lL ? vd[8] : vd[9],   em0_t = lL ? vt[8] : vt[9];      // (-1, 0)
+    const float e0p_d = lL ? vd[14] : vd[11], e0p_t = lL ? vt[14] : vt[11];    // (0, +1)
+    const float e0m_d = lL ? vd[12] : vd[13], e0m_t = lL ? vt[12] : vt[13];    // (0, -1)
+    float* xe = xex + (size_t)((jz & 1) * 2 + side) * 4 * TY;
+    if (lL || lR) {
+      xe[0 * TY + threadIdx.y] = ep0_d; xe[1 * TY + threadIdx.y] = ep0_t;
+      xe[2 * TY + threadIdx.y] = em0_d; xe[3 * TY + threadIdx.y] = em0_t;
+    }
+    // y: rows exchange their c_y = +-1 sums through shared memory (double-buffered by plane parity)
+    float* ex = yex + (size_t)(jz & 1) * SM_::NEX * TX * TY;
+    const int eo = threadIdx.y * TX + threadIdx.x;
+    ex[0 * TX * TY + eo] = ap0_d;   ex[1 * TX * TY + eo] = ap0_t;      // (+1, 0)
+    ex[2 * TX * TY + eo] = am0_d;   ex[3 * TX * TY + eo] = am0_t;      // (-1, 0)
+    ex[4 * TX * TY + eo] = vd[15];  ex[5 * TX * TY + eo] = vt[15];     // (+1, +1)
+    ex[6 * TX * TY + eo] = vd[18];  ex[7 * TX * TY + eo] = vt[18];     // (-1, +1)
+    ex[8 * TX * TY + eo] = vd[17];  ex[9 * TX * TY + eo] = vt[17];     // (+1, -1)
+    ex[10 * TX * TY + eo] = vd[16]; ex[11 * TX * TY + eo] = vt[16];    // (-1, -1)
+    __syncthreads();   // exchange visible; also: every thread is done with ring plane j = jz
+    if (tid == 0) {
+      const int j = jz + R_::NS;
+      if (j < npl) issue(j);
+    }
+    const bool has_below = threadIdx.y > 0, has_above = threadIdx.y < TY - 1;
+    auto below = [&](int slot) { return has_below ? ex[slot * TX * TY + eo - TX] : 0.f; };   // c_y = +1 from row - 1
+    auto above = [&](int slot) { return has_above ? ex[slot * TX * TY + eo + TX] : 0.f; };   // c_y = -1 from row + 1
+    const float b0_d = a00_d + below(0) + above(2), b0_t = a00_t + below(1) + above(3);
+    const float bp_d = a0p_d + below(4) + above(6), bp_t = a0p_t + below(5) + above(7);      // goes to plane z + 1
+    const float bm_d = a0m_d + below(8) + above(10), bm_t = a0m_t + below(9) + above(11);    // goes to plane z - 1
+    // z: plane z-1 is complete now
+    if (jz > 0 && active) {
+      const size_t s = col + plane_sites * (size_t)(z - 1);
+      p.Md[s] = pend_d + bm_d;
+      p.Mt[s] = pend_t + bm_t;
+    }
+    pend_d = b0_d + bpc_d; pend_t = b0_t + bpc_t;
+    bpc_d = bp_d; bpc_t = bp_t;
+    if ((lL || lR) && y < b.ny) {
+      const float eb_d = e00_d + (has_below ? xe[0 * TY + threadIdx.y - 1] : 0.f) + (has_above ? xe[2 * TY + threadIdx.y + 1] : 0.f);
+      const float eb_t = e00_t + (has_below ? xe[1 * TY + threadIdx.y - 1] : 0.f) + (has_above ? xe[3 * TY + threadIdx.y + 1] : 0.f);
+      if (jz > 0) {
+        float2* o = reinterpret_cast<float2*>(p.EX) + (((size_t)(z - 1) * b.ny + y) * ntx + blockIdx.x) * 2 + side;
+        *o = make_float2(pe_d + e0m_d, pe_t + e0m_t);
+      }
+      pe_d = eb_d + bpe_d; pe_t = eb_t + bpe_t;
+      bpe_d = e0p_d; bpe_t = e0p_t;
+    }
+  }
+  if (active) {
+    const size_t s = col + plane_sites * (size_t)(ze - 1);
+    p.Md[s] = pend_d;
+    p.Mt[s] = pend_t;
+  }
+  if ((lL || lR) && y < b.ny) {
+    float2* o = reinterpret_cast<float2*>(p.EX) + (((size_t)(ze - 1) * b.ny + y) * ntx + blockIdx.x) * 2 + side;
+    *o = make_float2(pe_d, pe_t);
+  }
+}
+
+// ----------------------------------------------------------------------------- K1f phase field, forwarded
+// phi(t+1) from the moments that k_fused forwarded plus what enters each brick through its faces:
+// for a site on a face of its brick (tile-local x = 0 / TX-1, y = 0 / TY-1, z = first / last plane
+// of the z chunk, or the last row / column / plane of the box) the directions whose source lies in
+// another brick are gathered from the populations k_fused stored, with the read rule of the NEXT
+// step (template MODE).  A solid source contributes nothing here: its link bounced back inside
+// k_fused.  Interior sites read 8 bytes.  Writes phi with its periodic ghost images like k_phase.
+template <int MODE, bool HAS_SOLID>
+__global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
+  const Box& b = p.box;
+  const int x = blockIdx.x * TX + threadIdx.x;
+  const int y = blockIdx.y * TY + threadIdx.y;
+  if (x >= b.nx || y >= b.ny) return;
+  // one plane per CTA (nothing is reused along z here, so the parallelism is worth more than a
+  // march); zb, ze are the z range of the k_fused brick this plane belongs to
+  const int z = blockIdx.z;
+  const int zb = (z / p.zc) * p.zc;
+  const int ze = min(b.nz, zb + p.zc);
+  const int H = p.halo;
+  const bool xm = threadIdx.x == 0, xp = threadIdx.x == TX - 1 || x == b.nx - 1;
+  const bool ym = threadIdx.y == 0, yp = threadIdx.y == TY - 1 || y == b.ny - 1;
+  const int ntx = gridDim.x;
+  {
+    float phi;
+    bool self_solid = false;
+    uint32_t smask = 0;
+    if constexpr (HAS_SOLID) {
+      self_solid = solid_at(b, x, y, z);
+      if (!self_solid) smask = neighbour_mask(b, x, y, z);
+    }
+    if (self_solid) {
+      phi = PHI_SOLID;
+    } else {
+      Ctx c;
+      make_ctx(c, b, x, y, z);
+      float d = __ldg(p.Md + c.idx), t = __ldg(p.Mt + c.idx);
+      const bool zm = z == zb, zp = z == ze - 1;
+      // what the neighbouring bricks sent through the x faces (rows and planes of this brick only)
+      const float2* ex = reinterpret_cast<const float2*>(p.EX) + ((size_t)z * b.ny + y) * ntx * 2;
+      if (xm) { const float2 v = __ldg(ex + (blockIdx.x == 0 ? ntx - 1 : blockIdx.x - 1) * 2 + 1); d += v.x; t += v.y; }
+      if (xp) { const float2 v = __ldg(ex + (blockIdx.x == ntx - 1 ? 0 : blockIdx.x + 1) * 2 + 0); d += v.x; t += v.y; }
+      static_for<1, Q>([&](auto qc) {
+        constexpr int q = decltype(qc)::value;
+        // sources in another row range or z chunk are gathered; x-only crossings came through EX
+        const bool crosses = (cy(q) > 0 && ym) || (cy(q) < 0 && yp) || (cz(q) > 0 && zm) || (cz(q) < 0 && zp);
+        if (crosses && !(HAS_SOLID && ((smask >> opp(q)) & 1u))) {
+          const Slot s = read_slot<MODE, false, q>(c, 0u);
+          const float tq = __ldg(slot_ptr(p.src, c, s, 0));
+          const float rq = __ldg(slot_ptr(p.src, c, s, 1));
+          d += (2.0f * rq - wq(q)) - tq;
+          t += tq;
+        }
+      });
+      phi = d / (1.0f + t);
+    }
+    store_phi_with_images(p, x, y, z, H, phi);
   }
 }
 
@@ -648,7 +654,7 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
     float T[Q];
     static_for<0, Q>([&](auto qc) {
       constexpr int q = decltype(qc)::value;
-      T[q] = ld_pop<MODE>(p.src + read_slot<MODE, HAS_SOLID, q>(c, smask));
+      T[q] = ld_pop<MODE>(slot_ptr(p.src, c, read_slot<MODE, HAS_SOLID, q>(c, smask), 0));
     });
     float dr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
     static_for<0, Q>([&](auto qc) {
@@ -668,16 +674,16 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
     static_for<1, Q + 1>([&](auto qc) {
       constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
       constexpr float w = wq(q);
-      const float cu = cx(q) * ux + cy(q) * uy + cz(q) * uz;
+      const float cu = cdot<q>(ux, uy, uz);
       const float teq = w * (dr + rho * (3.0f * cu + 4.5f * cu * cu - uu15));
       float ts = om1 * T[q] + omega * teq;
       if (p.has_g) {
-        const float cF = cx(q) * Fx + cy(q) * Fy + cz(q) * Fz;
+        const float cF = cdot<q>(Fx, Fy, Fz);
         ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
       }
       if constexpr (q > 0) tacc += ts;
       else ts = dr - tacc;
-      p.dst[write_slot<MODE, HAS_SOLID, q>(c, smask)] = ts;
+      *slot_ptr(p.dst, c, write_slot<MODE, HAS_SOLID, q>(c, smask), 0) = ts;
     });
   }
 }
