@@ -155,6 +155,10 @@ namespace {
 StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   StepParams p;
   p.src = src; p.dst = dst; p.phi = h->phi;
+  for (int q = 0; q < 2 * Q; ++q) {
+    p.ps[q] = src ? src + (size_t)q * h->S : nullptr;
+    p.pd[q] = dst ? dst + (size_t)q * h->S : nullptr;
+  }
   p.Md = h->mom; p.Mt = h->mom ? h->mom + h->S : nullptr; p.EX = h->mom ? h->mom + 2 * h->S : nullptr;
   p.box = h->box();
   p.zc = zc;
@@ -191,25 +195,30 @@ void launch_phase(lb_handle h, const StepParams& p, dim3 grid) {
   if (h->has_solid) k_phase<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
   else k_phase<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
 }
-template <int MODE, bool HAS_SOLID, bool HAS_NC>
+template <int MODE, bool HAS_SOLID, bool HAS_NC, bool HAS_G>
 void launch_fused_t(lb_handle h, const StepParams& p, dim3 grid) {
   constexpr size_t smem = FusedSmem<HAS_NC ? H_MAX_NC : 1>::BYTES;
   static bool attr_set = false;   // per instantiation
   if (!attr_set) {
-    cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, HAS_NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, HAS_NC, HAS_G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
-  k_fused<MODE, HAS_SOLID, HAS_NC><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap);
+  k_fused<MODE, HAS_SOLID, HAS_NC, HAS_G><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap);
+}
+template <int MODE, bool HAS_SOLID, bool HAS_NC>
+void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
+  if (p.has_g) launch_fused_t<MODE, HAS_SOLID, HAS_NC, true>(h, p, grid);
+  else launch_fused_t<MODE, HAS_SOLID, HAS_NC, false>(h, p, grid);
 }
 template <int MODE>
 void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
   const bool nc = h->par.A_nc != 0.f;
   if (h->has_solid) {
-    if (nc) launch_fused_t<MODE, true, true>(h, p, grid);
-    else launch_fused_t<MODE, true, false>(h, p, grid);
+    if (nc) launch_fused_g<MODE, true, true>(h, p, grid);
+    else launch_fused_g<MODE, true, false>(h, p, grid);
   } else {
-    if (nc) launch_fused_t<MODE, false, true>(h, p, grid);
-    else launch_fused_t<MODE, false, false>(h, p, grid);
+    if (nc) launch_fused_g<MODE, false, true>(h, p, grid);
+    else launch_fused_g<MODE, false, false>(h, p, grid);
   }
 }
 template <int MODE>

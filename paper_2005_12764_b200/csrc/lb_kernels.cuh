@@ -25,6 +25,8 @@ namespace lb {
 
 struct StepParams {
   const float* src;   // population buffer read by this step
+  const float* ps[2 * Q];   // src + plane * S for every plane: host-computed so that an access is
+  float* pd[2 * Q];         // one 64-bit add of a constant-bank operand and a 32-bit byte offset
   float* dst;         // buffer written (== src in AA modes)
   float* phi;         // padded phi array (written by K1 / K1f, read by K2 / K3)
   float* Md;          // forwarded moments of the next state (written by K2, read by K1f):
@@ -93,11 +95,13 @@ __device__ __forceinline__ Slot write_slot(const Ctx& c, uint32_t smask) {
 }
 
 // comp = 0: total-deviation planes, 1: red planes
-__device__ __forceinline__ const float* slot_ptr(const float* base, const Ctx& c, Slot s, int comp) {
-  return reinterpret_cast<const float*>(reinterpret_cast<const char*>(base) + (size_t)(s.plane + comp * Q) * c.Sb + s.off);
+template <class P>
+__device__ __forceinline__ const float* src_ptr(const P& p, Slot s, int comp) {
+  return reinterpret_cast<const float*>(reinterpret_cast<const char*>(p.ps[s.plane + comp * Q]) + s.off);
 }
-__device__ __forceinline__ float* slot_ptr(float* base, const Ctx& c, Slot s, int comp) {
-  return reinterpret_cast<float*>(reinterpret_cast<char*>(base) + (size_t)(s.plane + comp * Q) * c.Sb + s.off);
+template <class P>
+__device__ __forceinline__ float* dst_ptr(const P& p, Slot s, int comp) {
+  return reinterpret_cast<float*>(reinterpret_cast<char*>(p.pd[s.plane + comp * Q]) + s.off);
 }
 
 template <int MODE>
@@ -162,6 +166,10 @@ __device__ __forceinline__ void two_sum_acc(float& s, float& e, float x) {
 __device__ __forceinline__ void store_phi_with_images(const StepParams& p, int x, int y, int z, int H, float phi) {
   const Box& b = p.box;
   const int px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
+  if (x >= H && x < b.nx - H && y >= H && y < b.ny - H && z >= H && z < b.nz - H) {   // no image
+    p.phi[(size_t)(x + HALO) + (size_t)px * ((size_t)(y + HALO) + (size_t)py * (size_t)(z + HALO))] = phi;
+    return;
+  }
   const int sx[3] = {0, x < H ? b.nx : 0, x >= b.nx - H ? -b.nx : 0};
   const int sy[3] = {0, y < H ? b.ny : 0, y >= b.ny - H ? -b.ny : 0};
   const int sz[3] = {0, z < H ? b.nz : 0, z >= b.nz - H ? -b.nz : 0};
@@ -203,8 +211,8 @@ __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, 
       static_for<0, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
         const Slot s = read_slot<MODE, HAS_SOLID, q>(c, smask);
-        t[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 0));
-        r[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 1));
+        t[q] = ld_pop<MODE>(src_ptr(p, s, 0));
+        r[q] = ld_pop<MODE>(src_ptr(p, s, 1));
       });
       // Compensated (two-sum) accumulation: the direction of grad phi, which the perturbation and
       // the recolouring use, is ill-conditioned where |grad phi| is small, so phi is formed to
@@ -301,7 +309,7 @@ struct FusedSmem {
   static constexpr size_t BYTES = RING + YEX + XEX + Ring<H>::NS * sizeof(uint64_t);
 };
 
-template <int MODE, bool HAS_SOLID, bool HAS_NC>
+template <int MODE, bool HAS_SOLID, bool HAS_NC, bool HAS_G>
 __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
   using R_ = Ring<H>;
@@ -397,8 +405,8 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
       static_for<0, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
         const Slot s = read_slot<MODE, HAS_SOLID, q>(c, smask);
-        T[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 0));
-        R[q] = ld_pop<MODE>(slot_ptr(p.src, c, s, 1));
+        T[q] = ld_pop<MODE>(src_ptr(p, s, 0));
+        R[q] = ld_pop<MODE>(src_ptr(p, s, 1));
       });
       // ---- moments (Eq. 3)
       float dr = 0.f, rr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
@@ -440,8 +448,8 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
           }
         }
       }
-      const bool forced = HAS_NC || p.has_g;
-      if (p.has_g) { Fx += rho * p.gx; Fy += rho * p.gy; Fz += rho * p.gz; }
+      constexpr bool forced = HAS_NC || HAS_G;
+      if constexpr (HAS_G) { Fx += rho * p.gx; Fy += rho * p.gy; Fz += rho * p.gz; }
       // ---- velocity with the half-force shift, relaxation rate (Eq. 7-8)
       const float ux = (mx + 0.5f * Fx) * inv_rho, uy = (my + 0.5f * Fy) * inv_rho, uz = (mz + 0.5f * Fz) * inv_rho;
       float omega = omega_same;
@@ -468,7 +476,7 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
         const float cG = cdot<q>(Gx, Gy, Gz);
         const float teq = w * (dr + rho * (3.0f * cu + 4.5f * cu * cu - uu15));
         float ts = om1 * T[q] + omega * teq;
-        if (forced) {
+        if constexpr (forced) {
           const float cF = cdot<q>(Fx, Fy, Fz);
           ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
         }
@@ -483,8 +491,8 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
           rs = rr - racc;
         }
         const Slot s = write_slot<MODE, HAS_SOLID, q>(c, smask);
-        *slot_ptr(p.dst, c, s, 0) = ts;
-        *slot_ptr(p.dst, c, s, 1) = rs;
+        *dst_ptr(p, s, 0) = ts;
+        *dst_ptr(p, s, 1) = rs;
         // f^r* - f^b* = 2 f^r* - f* = (2 rs - w) - ts: the first difference is exact in the mixed
         // regions where phi matters, so the forwarded sum keeps ~1e-8 there
         vd[q] = (2.0f * rs - w) - ts;
@@ -614,14 +622,14 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
       const float2* ex = reinterpret_cast<const float2*>(p.EX) + ((size_t)z * b.ny + y) * ntx * 2;
       if (xm) { const float2 v = __ldg(ex + (blockIdx.x == 0 ? ntx - 1 : blockIdx.x - 1) * 2 + 1); d += v.x; t += v.y; }
       if (xp) { const float2 v = __ldg(ex + (blockIdx.x == ntx - 1 ? 0 : blockIdx.x + 1) * 2 + 0); d += v.x; t += v.y; }
-      static_for<1, Q>([&](auto qc) {
+      if (ym || yp || zm || zp) static_for<1, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
         // sources in another row range or z chunk are gathered; x-only crossings came through EX
         const bool crosses = (cy(q) > 0 && ym) || (cy(q) < 0 && yp) || (cz(q) > 0 && zm) || (cz(q) < 0 && zp);
         if (crosses && !(HAS_SOLID && ((smask >> opp(q)) & 1u))) {
           const Slot s = read_slot<MODE, false, q>(c, 0u);
-          const float tq = __ldg(slot_ptr(p.src, c, s, 0));
-          const float rq = __ldg(slot_ptr(p.src, c, s, 1));
+          const float tq = __ldg(src_ptr(p, s, 0));
+          const float rq = __ldg(src_ptr(p, s, 1));
           d += (2.0f * rq - wq(q)) - tq;
           t += tq;
         }
@@ -654,7 +662,7 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
     float T[Q];
     static_for<0, Q>([&](auto qc) {
       constexpr int q = decltype(qc)::value;
-      T[q] = ld_pop<MODE>(slot_ptr(p.src, c, read_slot<MODE, HAS_SOLID, q>(c, smask), 0));
+      T[q] = ld_pop<MODE>(src_ptr(p, read_slot<MODE, HAS_SOLID, q>(c, smask), 0));
     });
     float dr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
     static_for<0, Q>([&](auto qc) {
@@ -683,7 +691,7 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
       }
       if constexpr (q > 0) tacc += ts;
       else ts = dr - tacc;
-      *slot_ptr(p.dst, c, write_slot<MODE, HAS_SOLID, q>(c, smask), 0) = ts;
+      *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask), 0) = ts;
     });
   }
 }
