@@ -310,7 +310,7 @@ struct FusedSmem {
 };
 
 template <int MODE, bool HAS_SOLID, bool HAS_NC, bool HAS_G>
-__global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
+__global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
   using R_ = Ring<H>;
   using SM_ = FusedSmem<H>;
@@ -459,10 +459,24 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
       }
       const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
       const float uF = ux * Fx + uy * Fy + uz * Fz;
-      const float g0 = 1.0f - 0.5f * omega;
       const float fr_r = rr * inv_rho;                       // rho_r / rho
       const float kcol = p.beta * rr * rb * inv_rho * invG;   // recolouring amplitude / |G|
       const float om1 = 1.0f - omega;
+      // Per-site constants of the three weight classes (rest, axis, diagonal), so that the loop
+      // over directions is a handful of fused multiply-adds:
+      //   omega f^eq_q - A B_q |G| = ob[c] + orw[c] cu (3 + 4.5 cu)
+      //   A w_q (c.G)^2 / |G|      = (pa[c] cG) cG
+      //   Guo source               = gw[c] (cF (1 + 3 cu) - u.F)
+      //   red share                = fr_r (f*_q + w_q) + kc[c] cG
+      const float eq0 = dr - rho * uu15;
+      const float orw[3] = {omega * rho * wq(0), omega * rho * wq(1), omega * rho * wq(7)};
+      const float ob[3] = {omega * wq(0) * eq0 - p.A * bq(0) * Gne, omega * wq(1) * eq0 - p.A * bq(1) * Gne,
+                           omega * wq(7) * eq0 - p.A * bq(7) * Gne};
+      const float pa[3] = {0.f, p.A * wq(1) * invG, p.A * wq(7) * invG};
+      const float g3 = 3.0f * (1.0f - 0.5f * omega);
+      const float gw[3] = {g3 * wq(0), g3 * wq(1), g3 * wq(7)};
+      const float kc[3] = {0.f, kcol * wq(1), kcol * (wq(7) * inv_cnorm(7))};
+      const float frw[3] = {fr_r * wq(0), fr_r * wq(1), fr_r * wq(7)};
       // ---- collide on the total (deviation form), perturb, recolour, store
       // Directions 1..18 first; the rest populations then take what is left of rho - 1 and of
       // rho_r (collision conserves both at every site), so that the per-site masses are conserved
@@ -471,19 +485,19 @@ __global__ void __launch_bounds__(TX* TY) k_fused(const StepParams p, const __gr
       float racc = 0.f, tacc = 0.f;
       static_for<1, Q + 1>([&](auto qc) {
         constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
+        constexpr int k = q == 0 ? 0 : (q < 7 ? 1 : 2);
         constexpr float w = wq(q);
-        const float cu = cdot<q>(ux, uy, uz);
-        const float cG = cdot<q>(Gx, Gy, Gz);
-        const float teq = w * (dr + rho * (3.0f * cu + 4.5f * cu * cu - uu15));
-        float ts = om1 * T[q] + omega * teq;
-        if constexpr (forced) {
-          const float cF = cdot<q>(Fx, Fy, Fz);
-          ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
-        }
-        ts += p.A * (w * cG * cG * invG - bq(q) * Gne);
-        float rs;
+        float ts, rs;
         if constexpr (q > 0) {
-          rs = fr_r * (ts + w) + kcol * (w * inv_cnorm(q)) * cG;
+          const float cu = cdot<q>(ux, uy, uz);
+          const float cG = cdot<q>(Gx, Gy, Gz);
+          ts = fmaf(om1, T[q], fmaf(orw[k], cu * fmaf(4.5f, cu, 3.0f), ob[k]));
+          if constexpr (forced) {
+            const float cF = cdot<q>(Fx, Fy, Fz);
+            ts = fmaf(gw[k], fmaf(cF, fmaf(3.0f, cu, 1.0f), -uF), ts);
+          }
+          ts = fmaf(pa[k] * cG, cG, ts);
+          rs = fmaf(fr_r, ts, fmaf(kc[k], cG, frw[k]));
           racc += rs;
           tacc += ts;
         } else {
