@@ -173,17 +173,31 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
 
 // z planes per CTA: enough CTAs for ~8 waves of 148 SMs x 4 resident CTAs, at least 8 planes
 // so that the phi-ring prologue (2H+1 planes) is amortised.
+// z planes per CTA.  Measured on B200: short columns win (256^3: 0.91 ms at 8
+// planes, 0.95 at 16, 1.11 at 64; 640^3: 16.2 ms at 16, 18.9 at 214), but every brick face costs
+// k_phase_fwd a gather, so: 10..20 planes, and among those the count whose number of CTAs fills
+// whole waves of (SMs x 3 resident CTAs) best.
 int pick_zc(lb_handle h) {
   if (h->tune_zc > 0) return h->tune_zc < h->nz ? h->tune_zc : h->nz;
+  if (h->nz <= 10) return h->nz;
+  static int slots = 0;
+  if (!slots) {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaGetLastError();
+    slots = 3 * sms;
+  }
   const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
-  const long long want = 148LL * 4 * 8;
-  long long zsplit = (want + cols - 1) / cols;
-  if (zsplit < 1) zsplit = 1;
-  int zc = (int)((h->nz + zsplit - 1) / zsplit);
-  const int zmin = h->par.A_nc != 0.f ? 16 : 8;
-  if (zc < zmin) zc = zmin;
-  if (zc > h->nz) zc = h->nz;
-  return zc;
+  int best = 16;
+  double best_eff = -1.0;
+  for (int zc = 10; zc <= 20 && zc <= h->nz; ++zc) {
+    const long long ctas = cols * ((h->nz + zc - 1) / zc);
+    const long long waves = (ctas + slots - 1) / slots;
+    // planes actually computed per slot-wave (the last chunk may be short)
+    const double eff = (double)cols * h->nz / ((double)waves * slots * zc);
+    if (eff > best_eff + 1e-9) { best_eff = eff; best = zc; }
+  }
+  return best;
 }
 
 dim3 tile_grid(lb_handle h, int zc) {
