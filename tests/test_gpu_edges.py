@@ -214,3 +214,45 @@ def test_full_size_sampled_blocks_and_conservation(lbmod, lbo, name):
     if name == "c3":
         mom = np.abs([(u[a].astype(np.float64) * (rr + rb)).sum() for a in range(3)]).max() / w.sites
         assert mom < 1e-5
+
+
+# ------------------------------------------------------------------------------- moment forwarding
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+@pytest.mark.parametrize("walls", [False, True])
+def test_forwarded_phi_matches_oracle_and_full_sweep(lbmod, lbo, storage, walls):
+    """phi(t+1) that k_fused forwards (+ k_phase_fwd for the brick faces) against the oracle's phi
+    and against the full phase-field sweep (forward = 0), over several steps, on a box whose
+    extents are not multiples of the 32 x 8 tile and with bricks of 3 planes so that every kind
+    of brick face, edge and box wrap occurs many times."""
+    w = _random_workload(68, 21, 13, seed=11 + walls, walls=walls)
+    fluid = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
+    o = pu.make_oracle(lbo, w)
+    a, b = pu.make_gpu(lbmod, w, storage), pu.make_gpu(lbmod, w, storage)
+    a.set_tuning(forward=1, zc=3)
+    b.set_tuning(forward=0)
+    risky = np.zeros(w.shape, bool)
+    for n in range(1, 5):
+        risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+        o.step(1); a.step(1); b.step(1)
+        pa, pb, po = a.get_phi(), b.get_phi(), o.get_fields()["phi"]
+        ok = fluid & ~risky
+        assert np.abs(pa - po)[ok].max() < 2e-6, (n, np.abs(pa - po)[ok].max())
+        # the two phi paths differ only in summation order
+        assert np.abs(pa - pb)[ok].max() < 2e-6, (n, np.abs(pa - pb)[ok].max())
+        e = pu.pop_error(a, o)
+        assert e[ok].max() < pu.POP_TOL, (n, e[ok].max())
+
+
+def test_forwarding_brick_sizes_agree(lbmod):
+    """The forwarded sums may not depend on how the box is cut into bricks beyond rounding."""
+    w = W.get("c5-mini")
+    ref = None
+    for zc in (0, 1, 5, 96):
+        sim = pu.make_gpu(lbmod, w)
+        sim.set_tuning(zc=zc)
+        sim.step(3)
+        phi = sim.get_phi()
+        if ref is None:
+            ref = phi
+        else:
+            assert np.abs(phi - ref).max() < 1e-6, (zc, np.abs(phi - ref).max())
