@@ -602,55 +602,97 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
 // another brick are gathered from the populations k_fused stored, with the read rule of the NEXT
 // step (template MODE).  A solid source contributes nothing here: its link bounced back inside
 // k_fused.  Interior sites read 8 bytes.  Writes phi with its periodic ghost images like k_phase.
+constexpr int FZ = 4;   // planes per CTA of k_phase_fwd
 template <int MODE, bool HAS_SOLID>
 __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
+  // Four consecutive x sites per thread (128-bit loads and stores); CTA = 8 quads x TY rows x FZ
+  // planes = one k_fused tile over FZ planes.  nx % 4 == 0, so a quad is inside the box or not.
   const Box& b = p.box;
-  const int x = blockIdx.x * TX + threadIdx.x;
+  const int qx = threadIdx.x;                        // quad inside the tile row
+  const int x = blockIdx.x * TX + qx * 4;
   const int y = blockIdx.y * TY + threadIdx.y;
-  if (x >= b.nx || y >= b.ny) return;
-  // one plane per CTA (nothing is reused along z here, so the parallelism is worth more than a
-  // march); zb, ze are the z range of the k_fused brick this plane belongs to
-  const int z = blockIdx.z;
+  const int z = blockIdx.z * FZ + threadIdx.z;
+  if (x >= b.nx || y >= b.ny || z >= b.nz) return;
+  // z range of the k_fused brick this plane belongs to
   const int zb = (z / p.zc) * p.zc;
   const int ze = min(b.nz, zb + p.zc);
   const int H = p.halo;
-  const bool xm = threadIdx.x == 0, xp = threadIdx.x == TX - 1 || x == b.nx - 1;
+  const bool xm = qx == 0;                            // element 0 is the first column of its brick
+  const bool xp = qx == TX / 4 - 1 || x + 4 == b.nx;  // element 3 is the last column of its brick
   const bool ym = threadIdx.y == 0, yp = threadIdx.y == TY - 1 || y == b.ny - 1;
+  const bool zm = z == zb, zp = z == ze - 1;
   const int ntx = gridDim.x;
-  {
-    float phi;
-    bool self_solid = false;
-    uint32_t smask = 0;
-    if constexpr (HAS_SOLID) {
-      self_solid = solid_at(b, x, y, z);
-      if (!self_solid) smask = neighbour_mask(b, x, y, z);
-    }
-    if (self_solid) {
-      phi = PHI_SOLID;
-    } else {
-      Ctx c;
-      make_ctx(c, b, x, y, z);
-      float d = __ldg(p.Md + c.idx), t = __ldg(p.Mt + c.idx);
-      const bool zm = z == zb, zp = z == ze - 1;
-      // what the neighbouring bricks sent through the x faces (rows and planes of this brick only)
-      const float2* ex = reinterpret_cast<const float2*>(p.EX) + ((size_t)z * b.ny + y) * ntx * 2;
-      if (xm) { const float2 v = __ldg(ex + (blockIdx.x == 0 ? ntx - 1 : blockIdx.x - 1) * 2 + 1); d += v.x; t += v.y; }
-      if (xp) { const float2 v = __ldg(ex + (blockIdx.x == ntx - 1 ? 0 : blockIdx.x + 1) * 2 + 0); d += v.x; t += v.y; }
-      if (ym || yp || zm || zp) static_for<1, Q>([&](auto qc) {
-        constexpr int q = decltype(qc)::value;
-        // sources in another row range or z chunk are gathered; x-only crossings came through EX
-        const bool crosses = (cy(q) > 0 && ym) || (cy(q) < 0 && yp) || (cz(q) > 0 && zm) || (cz(q) < 0 && zp);
-        if (crosses && !(HAS_SOLID && ((smask >> opp(q)) & 1u))) {
-          const Slot s = read_slot<MODE, false, q>(c, 0u);
-          const float tq = __ldg(src_ptr(p, s, 0));
-          const float rq = __ldg(src_ptr(p, s, 1));
-          d += (2.0f * rq - wq(q)) - tq;
-          t += tq;
+  const size_t row = (size_t)b.nx * ((size_t)y + (size_t)b.ny * z);
+  const size_t idx = row + x;
+  const float4 d4 = __ldg(reinterpret_cast<const float4*>(p.Md + idx));
+  const float4 t4 = __ldg(reinterpret_cast<const float4*>(p.Mt + idx));
+  float d[4] = {d4.x, d4.y, d4.z, d4.w}, t[4] = {t4.x, t4.y, t4.z, t4.w};
+  // what the neighbouring bricks sent through the x faces (rows and planes of this brick only)
+  const float2* ex = reinterpret_cast<const float2*>(p.EX) + ((size_t)z * b.ny + y) * ntx * 2;
+  if (xm) { const float2 v = __ldg(ex + (blockIdx.x == 0 ? ntx - 1 : blockIdx.x - 1) * 2 + 1); d[0] += v.x; t[0] += v.y; }
+  if (xp) { const float2 v = __ldg(ex + (blockIdx.x == ntx - 1 ? 0 : blockIdx.x + 1) * 2 + 0); d[3] += v.x; t[3] += v.y; }
+  bool solid[4] = {false, false, false, false};
+  if constexpr (HAS_SOLID) {
+#pragma unroll
+    for (int e = 0; e < 4; ++e) solid[e] = solid_at(b, x + e, y, z);
+  }
+  if (ym || yp || zm || zp) {
+    // sources in another row range or z chunk are gathered from the stored populations with the
+    // read rule of the next step; x-only crossings came through EX; a solid source bounced back
+    // inside k_fused
+    static_for<1, Q>([&](auto qc) {
+      constexpr int q = decltype(qc)::value;
+      const bool crosses = (cy(q) > 0 && ym) || (cy(q) < 0 && yp) || (cz(q) > 0 && zm) || (cz(q) < 0 && zp);
+      if (crosses) {
+        constexpr bool own = MODE == MODE_AA_EVEN;          // AA-even reads its own site
+        constexpr int plane = MODE == MODE_AA_ODD ? opp(q) : q;
+        constexpr int sx = own ? 0 : cx(q);
+        const int ys = own ? y : (cy(q) > 0 ? wrap_m(y, b.ny) : (cy(q) < 0 ? wrap_p(y, b.ny) : y));
+        const int zs = own ? z : (cz(q) > 0 ? wrap_m(z, b.nz) : (cz(q) < 0 ? wrap_p(z, b.nz) : z));
+        const size_t srow = (size_t)b.nx * ((size_t)ys + (size_t)b.ny * zs);
+        float tq[4], rq[4];
+        if constexpr (sx == 0) {
+          const float4 a = __ldg(reinterpret_cast<const float4*>(p.ps[plane] + srow + x));
+          const float4 r = __ldg(reinterpret_cast<const float4*>(p.ps[plane + Q] + srow + x));
+          tq[0] = a.x; tq[1] = a.y; tq[2] = a.z; tq[3] = a.w;
+          rq[0] = r.x; rq[1] = r.y; rq[2] = r.z; rq[3] = r.w;
+        } else {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            int xs = x + e - sx;
+            xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
+            tq[e] = __ldg(p.ps[plane] + srow + xs);
+            rq[e] = __ldg(p.ps[plane + Q] + srow + xs);
+          }
         }
-      });
-      phi = d / (1.0f + t);
-    }
-    store_phi_with_images(p, x, y, z, H, phi);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          bool use = true;
+          if constexpr (HAS_SOLID) {     // is the site this population comes from solid?
+            int xs = x + e - cx(q);
+            xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
+            const int yq = cy(q) > 0 ? wrap_m(y, b.ny) : (cy(q) < 0 ? wrap_p(y, b.ny) : y);
+            const int zq = cz(q) > 0 ? wrap_m(z, b.nz) : (cz(q) < 0 ? wrap_p(z, b.nz) : z);
+            use = !solid_at(b, xs, yq, zq);
+          }
+          if (use) {
+            d[e] += (2.0f * rq[e] - wq(q)) - tq[e];
+            t[e] += tq[e];
+          }
+        }
+      }
+    });
+  }
+  float phi[4];
+#pragma unroll
+  for (int e = 0; e < 4; ++e) phi[e] = solid[e] ? PHI_SOLID : d[e] / (1.0f + t[e]);
+  if (x >= H && x + 4 <= b.nx - H && y >= H && y < b.ny - H && z >= H && z < b.nz - H) {   // no ghost image
+    const size_t px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
+    *reinterpret_cast<float4*>(p.phi + (size_t)(x + HALO) + px * ((size_t)(y + HALO) + py * (size_t)(z + HALO))) =
+        make_float4(phi[0], phi[1], phi[2], phi[3]);
+  } else {
+#pragma unroll
+    for (int e = 0; e < 4; ++e) store_phi_with_images(p, x + e, y, z, H, phi[e]);
   }
 }
 
