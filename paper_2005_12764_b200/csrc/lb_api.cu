@@ -237,8 +237,8 @@ void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
 }
 template <int MODE>
 void launch_phase_fwd(lb_handle h, const StepParams& p, dim3 grid) {
-  if (h->has_solid) k_phase_fwd<MODE, true><<<grid, dim3(TX / 4, TY, FZ), 0, h->stream>>>(p);
-  else k_phase_fwd<MODE, false><<<grid, dim3(TX / 4, TY, FZ), 0, h->stream>>>(p);
+  if (h->has_solid) k_phase_fwd<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+  else k_phase_fwd<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
 }
 template <int MODE>
 void launch_single(lb_handle h, const StepParams& p, dim3 grid) {
@@ -286,7 +286,7 @@ void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
   if (h->two && h->forward) {
     // K1f: phi of the new state from the moments k_fused forwarded (same z chunks: the bricks must match)
     const StepParams q = make_step_params(h, h->cur_buf(), nullptr, zc);
-    const dim3 gridf(grid.x, grid.y, (h->nz + FZ - 1) / FZ);   // FZ planes per CTA, 4 sites per thread
+    const dim3 gridf((h->nx / 4 + TX - 1) / TX, grid.y, h->nz);   // 4 sites per thread, one plane per CTA
     switch (h->mode()) {
       case MODE_AB: launch_phase_fwd<MODE_AB>(h, q, gridf); break;
       case MODE_AA_EVEN: launch_phase_fwd<MODE_AA_EVEN>(h, q, gridf); break;

@@ -602,17 +602,19 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
 // another brick are gathered from the populations k_fused stored, with the read rule of the NEXT
 // step (template MODE).  A solid source contributes nothing here: its link bounced back inside
 // k_fused.  Interior sites read 8 bytes.  Writes phi with its periodic ghost images like k_phase.
-constexpr int FZ = 4;   // planes per CTA of k_phase_fwd
 template <int MODE, bool HAS_SOLID>
 __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
-  // Four consecutive x sites per thread (128-bit loads and stores); CTA = 8 quads x TY rows x FZ
-  // planes = one k_fused tile over FZ planes.  nx % 4 == 0, so a quad is inside the box or not.
+  // Four consecutive x sites per thread (128-bit loads and stores).  CTA = 32 quads x TY rows of
+  // one plane (four k_fused tiles side by side), so that a warp is one row: the rows on a brick
+  // face gather as whole warps and the others skip that code.  nx % 4 == 0: a quad is inside the
+  // box or outside.
   const Box& b = p.box;
-  const int qx = threadIdx.x;                        // quad inside the tile row
-  const int x = blockIdx.x * TX + qx * 4;
+  const int x = (blockIdx.x * TX + threadIdx.x) * 4;
   const int y = blockIdx.y * TY + threadIdx.y;
-  const int z = blockIdx.z * FZ + threadIdx.z;
-  if (x >= b.nx || y >= b.ny || z >= b.nz) return;
+  const int z = blockIdx.z;
+  if (x >= b.nx || y >= b.ny) return;
+  const int tile = x / TX;                            // k_fused tile (brick column) of this quad
+  const int qx = threadIdx.x & (TX / 4 - 1);          // quad inside the tile row
   // z range of the k_fused brick this plane belongs to
   const int zb = (z / p.zc) * p.zc;
   const int ze = min(b.nz, zb + p.zc);
@@ -621,7 +623,7 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
   const bool xp = qx == TX / 4 - 1 || x + 4 == b.nx;  // element 3 is the last column of its brick
   const bool ym = threadIdx.y == 0, yp = threadIdx.y == TY - 1 || y == b.ny - 1;
   const bool zm = z == zb, zp = z == ze - 1;
-  const int ntx = gridDim.x;
+  const int ntx = (b.nx + TX - 1) / TX;
   const size_t row = (size_t)b.nx * ((size_t)y + (size_t)b.ny * z);
   const size_t idx = row + x;
   const float4 d4 = __ldg(reinterpret_cast<const float4*>(p.Md + idx));
@@ -629,8 +631,8 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
   float d[4] = {d4.x, d4.y, d4.z, d4.w}, t[4] = {t4.x, t4.y, t4.z, t4.w};
   // what the neighbouring bricks sent through the x faces (rows and planes of this brick only)
   const float2* ex = reinterpret_cast<const float2*>(p.EX) + ((size_t)z * b.ny + y) * ntx * 2;
-  if (xm) { const float2 v = __ldg(ex + (blockIdx.x == 0 ? ntx - 1 : blockIdx.x - 1) * 2 + 1); d[0] += v.x; t[0] += v.y; }
-  if (xp) { const float2 v = __ldg(ex + (blockIdx.x == ntx - 1 ? 0 : blockIdx.x + 1) * 2 + 0); d[3] += v.x; t[3] += v.y; }
+  if (xm) { const float2 v = __ldg(ex + (tile == 0 ? ntx - 1 : tile - 1) * 2 + 1); d[0] += v.x; t[0] += v.y; }
+  if (xp) { const float2 v = __ldg(ex + (tile == ntx - 1 ? 0 : tile + 1) * 2 + 0); d[3] += v.x; t[3] += v.y; }
   bool solid[4] = {false, false, false, false};
   if constexpr (HAS_SOLID) {
 #pragma unroll
