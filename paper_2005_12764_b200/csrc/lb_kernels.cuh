@@ -400,14 +400,21 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
         if constexpr (cy(q) != 0) Gy += (k * cy(q)) * v;
         if constexpr (cz(q) != 0) Gz += (k * cz(q)) * v;
       });
-      // ---- gather
+      // ---- gather.  Walls are rare: a warp none of whose sites has a solid neighbour takes the
+      // addressing of the wall-free variant (no per-direction select between the two slots).
+      bool near_wall = false;
+      if constexpr (HAS_SOLID) near_wall = __any_sync(__activemask(), smask != 0u);
       float T[Q], R[Q];
-      static_for<0, Q>([&](auto qc) {
-        constexpr int q = decltype(qc)::value;
-        const Slot s = read_slot<MODE, HAS_SOLID, q>(c, smask);
-        T[q] = ld_pop<MODE>(src_ptr(p, s, 0));
-        R[q] = ld_pop<MODE>(src_ptr(p, s, 1));
-      });
+      auto gather = [&](auto bounce) {
+        static_for<0, Q>([&](auto qc) {
+          constexpr int q = decltype(qc)::value;
+          const Slot s = read_slot<MODE, decltype(bounce)::value, q>(c, smask);
+          T[q] = ld_pop<MODE>(src_ptr(p, s, 0));
+          R[q] = ld_pop<MODE>(src_ptr(p, s, 1));
+        });
+      };
+      if (HAS_SOLID && near_wall) gather(std::integral_constant<bool, HAS_SOLID>{});
+      else gather(std::false_type{});
       // ---- moments (Eq. 3)
       float dr = 0.f, rr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
       static_for<0, Q>([&](auto qc) {
@@ -512,7 +519,7 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
         vd[q] = (2.0f * rs - w) - ts;
         vt[q] = ts;
       });
-      if constexpr (HAS_SOLID) {   // link bounce-back: what would enter a solid site comes back here
+      if (HAS_SOLID && near_wall) {   // link bounce-back: what would enter a solid site comes back here
         float sd = 0.f, st = 0.f;
         static_for<1, Q>([&](auto qc) {
           constexpr int q = decltype(qc)::value;
