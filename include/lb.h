@@ -130,10 +130,12 @@ size_t lb_device_bytes(lb_handle h);
 /* Last error text of this handle (or of the failed lb_create when h == NULL). */
 const char* lb_last_error(lb_handle h);
 
-/* Timing hook: an event pair recorded around the kernels of the LAST lb_step call, on the
- * handle's stream; returns the elapsed milliseconds (synchronises on the end event).
- * which: 0 = whole lb_step, 1 = sum over the fused stream-collide launches (k_fused / k_single),
- * 2 = sum over the phase-field launches (k_phase_fwd, or k_phase).  which = 1, 2 are recorded only after lb_set_profiling(h, 1). */
+/* Timing hooks, on the handle's stream.  lb_last_step_ms(h, 0, &ms): milliseconds of the whole LAST
+ * lb_step call (an event pair around all its launches; synchronises on the end event).
+ * lb_set_profiling(h, n), n > 0: in later lb_step calls every n-th step is bracketed kernel by
+ * kernel; lb_last_step_ms then returns the MEAN per sampled step of which = 1: the fused
+ * stream-collide launch (k_fused / k_single), which = 2: the phase-field launches (k_phase_fwd,
+ * or k_phase).  n = 0 switches the sampling off (the events cost ~3 % when taken every step). */
 int lb_set_profiling(lb_handle h, int on);
 int lb_last_step_ms(lb_handle h, int which, float* ms);
 

@@ -538,22 +538,24 @@ int lb_step(lb_handle h, int nsteps) {
   if (!h->inited) return fail(h, LB_ESTATE, "lb_step before lb_init");
   for (int i = 0; i < 2; ++i)
     if (!h->ev_step[i] && cudaEventCreate(&h->ev_step[i]) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
-  const bool prof = h->profiling != 0;
-  if (prof) {
-    while ((int)h->ev_k.size() < 4 * nsteps) {
-      cudaEvent_t e;
-      if (cudaEventCreate(&e) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
-      h->ev_k.push_back(e);
-    }
+  // profiling = n > 0: every n-th step of this call is bracketed by events (kernel by kernel)
+  const int stride = h->profiling;
+  const int nprof = stride > 0 ? (nsteps + stride - 1) / stride : 0;
+  while ((int)h->ev_k.size() < 4 * nprof) {
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
+    h->ev_k.push_back(e);
   }
-  h->ev_steps = prof ? nsteps : 0;
+  h->ev_steps = nprof;
   cudaEventRecord(h->ev_step[0], h->stream);
   for (int t = 0; t < nsteps; ++t) {
-    if (prof) cudaEventRecord(h->ev_k[4 * t + 0], h->stream);
+    const bool prof = stride > 0 && t % stride == 0;
+    const int k = prof ? 4 * (t / stride) : 0;
+    if (prof) cudaEventRecord(h->ev_k[k + 0], h->stream);
     run_phase(h);                 // K1: no-op unless phi is stale (first step, or forwarding off)
-    if (prof) cudaEventRecord(h->ev_k[4 * t + 1], h->stream);
-    run_collide(h, prof ? h->ev_k[4 * t + 2] : nullptr);   // K2 (+ K1f) or K2s
-    if (prof) cudaEventRecord(h->ev_k[4 * t + 3], h->stream);
+    if (prof) cudaEventRecord(h->ev_k[k + 1], h->stream);
+    run_collide(h, prof ? h->ev_k[k + 2] : nullptr);   // K2 (+ K1f) or K2s
+    if (prof) cudaEventRecord(h->ev_k[k + 3], h->stream);
   }
   cudaEventRecord(h->ev_step[1], h->stream);
   return check_launch(h, "lb_step");
@@ -663,7 +665,7 @@ int lb_set_tuning(lb_handle h, const char* key, int value) {
 
 int lb_set_profiling(lb_handle h, int on) {
   if (!h) return LB_EINVAL;
-  h->profiling = on ? 1 : 0;
+  h->profiling = on > 0 ? on : 0;
   return LB_OK;
 }
 
@@ -692,7 +694,7 @@ int lb_last_step_ms(lb_handle h, int which, float* ms) {
     if (e != cudaSuccess) return cuda_fail(h, e, "event elapsed");
     total += v;
   }
-  *ms = total;
+  *ms = total / (float)h->ev_steps;   // mean per sampled step
   return LB_OK;
 }
 

@@ -781,12 +781,9 @@ struct IoParams {
 template <int MODE>
 __device__ __forceinline__ size_t read_slot_rt(const Box& b, int q, int x, int y, int z) {
   // run-time-q version of read_slot for the cold kernels
-  const int cxs[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
-  const int cys[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
-  const int czs[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
   const size_t own = (size_t)x + (size_t)b.nx * ((size_t)y + (size_t)b.ny * z);
   if (MODE == MODE_AA_EVEN || q == 0) return (size_t)q * b.S + own;
-  int xs = x - cxs[q], ys = y - cys[q], zs = z - czs[q];
+  int xs = x - c_cx[q], ys = y - c_cy[q], zs = z - c_cz[q];
   xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
   ys = ys < 0 ? b.ny - 1 : (ys >= b.ny ? 0 : ys);
   zs = zs < 0 ? b.nz - 1 : (zs >= b.nz ? 0 : zs);
@@ -815,14 +812,11 @@ __global__ void k_scatter(const IoParams p) {
     ux = p.u[s]; uy = p.u[b.S + s]; uz = p.u[2 * b.S + s];
   }
   const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
-  const int cxs[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
-  const int cys[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
-  const int czs[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
   for (int q = 0; q < Q; ++q) {
     const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
     const float w = wq(q);
     if (p.comp < 0) {
-      const float cu = cxs[q] * ux + cys[q] * uy + czs[q] * uz;
+      const float cu = c_cx[q] * ux + c_cy[q] * uy + c_cz[q] * uz;
       const float e = 3.0f * cu + 4.5f * cu * cu - uu15;       // feq/(w rho) - 1
       const float drho = (rr + rb) - 1.0f;
       p.buf[slot] = w * (drho + (rr + rb) * e);                 // total as deviation
@@ -871,15 +865,12 @@ __global__ void k_macros(const IoParams p) {
   const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
   float rr = 0.f, rb = 0.f, ux = 0.f, uy = 0.f, uz = 0.f;
   if (!(b.mask && solid_at(b, x, y, z))) {
-    const int cxs[Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
-    const int cys[Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
-    const int czs[Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
     float dr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
     for (int q = 0; q < Q; ++q) {
       const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
       const float t = p.buf[slot];
       dr += t;
-      mx += cxs[q] * t; my += cys[q] * t; mz += czs[q] * t;
+      mx += c_cx[q] * t; my += c_cy[q] * t; mz += c_cz[q] * t;
       if (p.two) rr += p.buf[(size_t)Q * b.S + slot];
     }
     const float rho = 1.0f + dr;
@@ -892,10 +883,10 @@ __global__ void k_macros(const IoParams p) {
       const float phi0 = ph[0];
       float Gx = 0.f, Gy = 0.f, Gz = 0.f;
       for (int q = 1; q < Q; ++q) {
-        float v = ph[cxs[q] + px * cys[q] + pxy * czs[q]];
+        float v = ph[c_cx[q] + px * c_cy[q] + pxy * c_cz[q]];
         if (v > PHI_SOLID_TEST) v = phi0;
         const float k = 3.0f * wq(q);
-        Gx += k * cxs[q] * v; Gy += k * cys[q] * v; Gz += k * czs[q] * v;
+        Gx += k * c_cx[q] * v; Gy += k * c_cy[q] * v; Gz += k * c_cz[q] * v;
       }
       const float Gn = sqrtf(Gx * Gx + Gy * Gy + Gz * Gz);
       if (fabsf(phi0) < p.phi_c && Gn > EPS_G) {

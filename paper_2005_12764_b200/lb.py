@@ -215,7 +215,7 @@ class LB:
             self._ck(lib.lb_set_tuning(self.h, k.encode(), int(v)))
 
     def set_profiling(self, on):
-        self._ck(lib.lb_set_profiling(self.h, int(bool(on))))
+        self._ck(lib.lb_set_profiling(self.h, int(on)))
 
     def last_step_ms(self, which=0):
         ms = C.c_float()

@@ -256,3 +256,49 @@ def test_forwarding_brick_sizes_agree(lbmod):
             ref = phi
         else:
             assert np.abs(phi - ref).max() < 1e-6, (zc, np.abs(phi - ref).max())
+
+
+def test_full_size_c5_sampled_macros_and_conservation(lbmod, lbo):
+    """Config C5 at its full 640^3 (near contact, periodic, A/B, the launch configuration that
+    bench.py times): rho_r, rho_b, u after one step on sampled blocks against the oracle run on
+    a cut-out of the input (the populations of 2.6e8 sites are too many to bring back), then
+    mass conservation and finiteness over 50 steps."""
+    w = W.get("c5")
+    sim = pu.make_gpu(lbmod, w)
+    m0 = pu.masses(w.rho_r, w.rho_b)
+    sim.step(1)
+    rr, rb, u = sim.get_macros()
+    rng = np.random.default_rng(17)
+    centres = [(0, 0, 0), (w.nx - 1, w.ny // 2, w.nz - 1)] + \
+        [tuple(int(v) for v in rng.integers(0, [w.nx, w.ny, w.nz])) for _ in range(4)]
+    # two centres on droplet surfaces so that the probe and the recolouring are exercised
+    zz, yy, xx = np.nonzero(np.abs(w.rho_r[::40, ::40, ::40] - 0.5) < 0.3)
+    centres += [(int(xx[i]) * 40, int(yy[i]) * 40, int(zz[i]) * 40) for i in (0, len(xx) // 2)] if len(xx) else []
+    half, margin = 14, 7
+    n = 2 * half
+    worst = 0.0
+    for (cx, cy, cz) in centres:
+        ix = np.arange(cx - half, cx + half) % w.nx
+        iy = np.arange(cy - half, cy + half) % w.ny
+        iz = np.arange(cz - half, cz + half) % w.nz
+        sel = np.ix_(iz, iy, ix)
+        o = lbo.Oracle(n, n, n, *w.params)
+        o.set_nc_cutoff(w.phi_c)
+        o.init(w.rho_r[sel], w.rho_b[sel], w.u[(slice(None),) + sel])
+        risky = o.get_fields()["margin"] < 1e-5
+        o.step(1)
+        risky |= o.get_fields()["margin"] < 1e-5       # get_macros evaluates the force again
+        orr, orb, ou = o.get_macros()
+        inner = np.zeros((n, n, n), bool)
+        inner[margin:-margin, margin:-margin, margin:-margin] = True
+        inner &= ~pu.dilate(risky, 2)
+        worst = max(worst, np.abs(rr[sel] - orr)[inner].max(), np.abs(rb[sel] - orb)[inner].max(),
+                    np.abs(u[(slice(None),) + sel] - ou)[:, inner].max())
+    assert worst < 5e-6, worst
+    sim.step(49)
+    rr, rb, u = sim.get_macros()
+    assert np.isfinite(u).all()
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
+    mom = np.abs([(u[a].astype(np.float64) * (rr + rb)).sum() for a in range(3)]).max() / w.sites
+    assert mom < 1e-5
