@@ -155,9 +155,10 @@ namespace {
 StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   StepParams p;
   p.src = src; p.dst = dst; p.phi = h->phi;
-  for (int q = 0; q < 2 * Q; ++q) {
-    p.ps[q] = src ? src + (size_t)q * h->S : nullptr;
-    p.pd[q] = dst ? dst + (size_t)q * h->S : nullptr;
+  const size_t plane = (h->two ? 2 : 1) * (size_t)h->S;   // floats per direction plane ({T, R} pairs or T)
+  for (int q = 0; q < Q; ++q) {
+    p.ps[q] = src ? src + (size_t)q * plane : nullptr;
+    p.pd[q] = dst ? dst + (size_t)q * plane : nullptr;
   }
   p.Md = h->mom; p.Mt = h->mom ? h->mom + h->S : nullptr; p.EX = h->mom ? h->mom + 2 * h->S : nullptr;
   p.box = h->box();
@@ -364,7 +365,7 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
   if (!p) return fail(nullptr, LB_EINVAL, "params is NULL");
   if (nx < 4 || ny < 4 || nz < 4) return fail(nullptr, LB_EINVAL, "every extent must be >= 4");
   if (nx % 4 != 0) return fail(nullptr, LB_EINVAL, "nx must be a multiple of 4");
-  if ((long long)nx * ny * nz >= (1LL << 30)) return fail(nullptr, LB_EINVAL, "box too large (>= 2^30 sites)");
+  if ((long long)nx * ny * nz >= (1LL << 29)) return fail(nullptr, LB_EINVAL, "box too large (>= 2^29 sites)");
   if (!(p->tau_r > 0.5f) || !(p->tau_b > 0.5f)) return fail(nullptr, LB_EINVAL, "tau must exceed 0.5");
   lb_handle h = new (std::nothrow) lb_handle_s();
   if (!h) return fail(nullptr, LB_ENOMEM, "host allocation failed");

@@ -25,8 +25,8 @@ namespace lb {
 
 struct StepParams {
   const float* src;   // population buffer read by this step
-  const float* ps[2 * Q];   // src + plane * S for every plane: host-computed so that an access is
-  float* pd[2 * Q];         // one 64-bit add of a constant-bank operand and a 32-bit byte offset
+  const float* ps[Q];   // base of every direction plane of src / dst: host-computed so that an access
+  float* pd[Q];         // is one 64-bit add of a constant-bank operand and a 32-bit byte offset
   float* dst;         // buffer written (== src in AA modes)
   float* phi;         // padded phi array (written by K1 / K1f, read by K2 / K3)
   float* Md;          // forwarded moments of the next state (written by K2, read by K1f):
@@ -56,7 +56,6 @@ struct Ctx {
   int dxo[3];         // byte deltas to x-1, x, x+1 (wrapped)
   int dyo[3];         // to y-1, y, y+1
   int dzo[3];         // to z-1, z, z+1
-  size_t Sb;          // bytes per plane
 };
 
 // Byte delta from the own site to x - c_q.
@@ -94,14 +93,20 @@ __device__ __forceinline__ Slot write_slot(const Ctx& c, uint32_t smask) {
   }
 }
 
-// comp = 0: total-deviation planes, 1: red planes
+// Two-component buffers hold, per direction plane, one float2 {T_q, R_q} per site (T = total as a
+// deviation, R = red), so a direction costs one 64-bit access.  Single-component buffers hold T_q.
 template <class P>
-__device__ __forceinline__ const float* src_ptr(const P& p, Slot s, int comp) {
-  return reinterpret_cast<const float*>(reinterpret_cast<const char*>(p.ps[s.plane + comp * Q]) + s.off);
+__device__ __forceinline__ const float* src_ptr(const P& p, Slot s) {
+  return reinterpret_cast<const float*>(reinterpret_cast<const char*>(p.ps[s.plane]) + s.off);
 }
 template <class P>
-__device__ __forceinline__ float* dst_ptr(const P& p, Slot s, int comp) {
-  return reinterpret_cast<float*>(reinterpret_cast<char*>(p.pd[s.plane + comp * Q]) + s.off);
+__device__ __forceinline__ float* dst_ptr(const P& p, Slot s) {
+  return reinterpret_cast<float*>(reinterpret_cast<char*>(p.pd[s.plane]) + s.off);
+}
+template <int MODE>
+__device__ __forceinline__ float2 ld_pair(const float* p) {
+  if constexpr (MODE == MODE_AB) return __ldg(reinterpret_cast<const float2*>(p));   // read-only in A/B mode
+  else return *reinterpret_cast<const float2*>(p);
 }
 
 template <int MODE>
@@ -136,18 +141,19 @@ __device__ __forceinline__ uint32_t neighbour_mask(const Box& b, int x, int y, i
   return m;
 }
 
+// ESZ: bytes per site in a plane (8 for the {T, R} pairs of a two-component run, 4 for one component)
+template <int ESZ>
 __device__ __forceinline__ void make_ctx(Ctx& c, const Box& b, int x, int y, int z) {
-  c.Sb = (size_t)b.S * sizeof(float);
   c.idx = x + b.nx * (y + b.ny * z);
-  c.ob = (uint32_t)c.idx * 4u;
-  c.dxo[0] = (x == 0 ? b.nx - 1 : -1) * 4;
+  c.ob = (uint32_t)c.idx * (uint32_t)ESZ;
+  c.dxo[0] = (x == 0 ? b.nx - 1 : -1) * ESZ;
   c.dxo[1] = 0;
-  c.dxo[2] = (x == b.nx - 1 ? -(b.nx - 1) : 1) * 4;
-  const int row = b.nx * 4;
+  c.dxo[2] = (x == b.nx - 1 ? -(b.nx - 1) : 1) * ESZ;
+  const int row = b.nx * ESZ;
   c.dyo[0] = (y == 0 ? b.ny - 1 : -1) * row;
   c.dyo[1] = 0;
   c.dyo[2] = (y == b.ny - 1 ? -(b.ny - 1) : 1) * row;
-  const int pl = b.nx * b.ny * 4;
+  const int pl = b.nx * b.ny * ESZ;
   c.dzo[0] = (z == 0 ? b.nz - 1 : -1) * pl;
   c.dzo[1] = 0;
   c.dzo[2] = (z == b.nz - 1 ? -(b.nz - 1) : 1) * pl;
@@ -196,7 +202,7 @@ __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, 
   const int H = p.halo;
   for (int z = zb; z < ze; ++z) {
     Ctx c;
-    make_ctx(c, b, x, y, z);
+    make_ctx<8>(c, b, x, y, z);
     float phi;
     bool self_solid = false;
     uint32_t smask = 0;
@@ -211,8 +217,9 @@ __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, 
       static_for<0, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
         const Slot s = read_slot<MODE, HAS_SOLID, q>(c, smask);
-        t[q] = ld_pop<MODE>(src_ptr(p, s, 0));
-        r[q] = ld_pop<MODE>(src_ptr(p, s, 1));
+        const float2 v = ld_pair<MODE>(src_ptr(p, s));
+        t[q] = v.x;
+        r[q] = v.y;
       });
       // Compensated (two-sum) accumulation: the direction of grad phi, which the perturbation and
       // the recolouring use, is ill-conditioned where |grad phi| is small, so phi is formed to
@@ -382,7 +389,7 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
     for (int q = 0; q < Q; ++q) { vd[q] = 0.f; vt[q] = 0.f; }
     if (fluid) {
       Ctx c;
-      make_ctx(c, b, x, y, z);
+      make_ctx<8>(c, b, x, y, z);
       // ---- grad phi (stencil of Eq. 10) and solid flags from the phi tile
       const float* plm = plane(-1);
       const float* plp = plane(+1);
@@ -409,8 +416,9 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
         static_for<0, Q>([&](auto qc) {
           constexpr int q = decltype(qc)::value;
           const Slot s = read_slot<MODE, decltype(bounce)::value, q>(c, smask);
-          T[q] = ld_pop<MODE>(src_ptr(p, s, 0));
-          R[q] = ld_pop<MODE>(src_ptr(p, s, 1));
+          const float2 v = ld_pair<MODE>(src_ptr(p, s));
+          T[q] = v.x;
+          R[q] = v.y;
         });
       };
       if (HAS_SOLID && near_wall) gather(std::integral_constant<bool, HAS_SOLID>{});
@@ -512,8 +520,7 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
           rs = rr - racc;
         }
         const Slot s = write_slot<MODE, HAS_SOLID, q>(c, smask);
-        *dst_ptr(p, s, 0) = ts;
-        *dst_ptr(p, s, 1) = rs;
+        *reinterpret_cast<float2*>(dst_ptr(p, s)) = make_float2(ts, rs);
         // f^r* - f^b* = 2 f^r* - f* = (2 rs - w) - ts: the first difference is exact in the mixed
         // regions where phi matters, so the forwarded sum keeps ~1e-8 there
         vd[q] = (2.0f * rs - w) - ts;
@@ -660,18 +667,20 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
         const int zs = own ? z : (cz(q) > 0 ? wrap_m(z, b.nz) : (cz(q) < 0 ? wrap_p(z, b.nz) : z));
         const size_t srow = (size_t)b.nx * ((size_t)ys + (size_t)b.ny * zs);
         float tq[4], rq[4];
+        const float2* pl = reinterpret_cast<const float2*>(p.ps[plane]) + srow;   // {T, R} pairs of the source row
         if constexpr (sx == 0) {
-          const float4 a = __ldg(reinterpret_cast<const float4*>(p.ps[plane] + srow + x));
-          const float4 r = __ldg(reinterpret_cast<const float4*>(p.ps[plane + Q] + srow + x));
-          tq[0] = a.x; tq[1] = a.y; tq[2] = a.z; tq[3] = a.w;
-          rq[0] = r.x; rq[1] = r.y; rq[2] = r.z; rq[3] = r.w;
+          const float4 a = __ldg(reinterpret_cast<const float4*>(pl + x));
+          const float4 r = __ldg(reinterpret_cast<const float4*>(pl + x + 2));
+          tq[0] = a.x; rq[0] = a.y; tq[1] = a.z; rq[1] = a.w;
+          tq[2] = r.x; rq[2] = r.y; tq[3] = r.z; rq[3] = r.w;
         } else {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             int xs = x + e - sx;
             xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
-            tq[e] = __ldg(p.ps[plane] + srow + xs);
-            rq[e] = __ldg(p.ps[plane + Q] + srow + xs);
+            const float2 v = __ldg(pl + xs);
+            tq[e] = v.x;
+            rq[e] = v.y;
           }
         }
 #pragma unroll
@@ -723,11 +732,11 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
       smask = neighbour_mask(b, x, y, z);
     }
     Ctx c;
-    make_ctx(c, b, x, y, z);
+    make_ctx<4>(c, b, x, y, z);
     float T[Q];
     static_for<0, Q>([&](auto qc) {
       constexpr int q = decltype(qc)::value;
-      T[q] = ld_pop<MODE>(src_ptr(p, read_slot<MODE, HAS_SOLID, q>(c, smask), 0));
+      T[q] = ld_pop<MODE>(src_ptr(p, read_slot<MODE, HAS_SOLID, q>(c, smask)));
     });
     float dr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
     static_for<0, Q>([&](auto qc) {
@@ -756,7 +765,7 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
       }
       if constexpr (q > 0) tacc += ts;
       else ts = dr - tacc;
-      *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask), 0) = ts;
+      *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask)) = ts;
     });
   }
 }
@@ -819,14 +828,15 @@ __global__ void k_scatter(const IoParams p) {
       const float cu = c_cx[q] * ux + c_cy[q] * uy + c_cz[q] * uz;
       const float e = 3.0f * cu + 4.5f * cu * cu - uu15;       // feq/(w rho) - 1
       const float drho = (rr + rb) - 1.0f;
-      p.buf[slot] = w * (drho + (rr + rb) * e);                 // total as deviation
-      if (p.two) p.buf[(size_t)Q * b.S + slot] = w * rr * (1.0f + e);
+      const float tv = w * (drho + (rr + rb) * e);                 // total as deviation
+      if (p.two) { p.buf[2 * slot] = tv; p.buf[2 * slot + 1] = w * rr * (1.0f + e); }
+      else p.buf[slot] = tv;
     } else if (p.comp == 0) {
       const float f = p.in0[(size_t)q * b.S + s];
-      p.buf[slot] = f - w;
-      if (p.two) p.buf[(size_t)Q * b.S + slot] = f;
+      if (p.two) { p.buf[2 * slot] = f - w; p.buf[2 * slot + 1] = f; }
+      else p.buf[slot] = f - w;
     } else {
-      p.buf[slot] += p.in0[(size_t)q * b.S + s];
+      p.buf[2 * slot] += p.in0[(size_t)q * b.S + s];
     }
   }
 }
@@ -843,10 +853,10 @@ __global__ void k_gatherf(const IoParams p) {
     float v = 0.f;
     if (!sol) {
       const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
-      const float t = p.buf[slot] + wq(q);
+      const float t = p.buf[p.two ? 2 * slot : slot] + wq(q);
       if (!p.two) v = t;
       else {
-        const float r = p.buf[(size_t)Q * b.S + slot];
+        const float r = p.buf[2 * slot + 1];
         v = p.comp == 0 ? r : t - r;
       }
     }
@@ -868,10 +878,10 @@ __global__ void k_macros(const IoParams p) {
     float dr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
     for (int q = 0; q < Q; ++q) {
       const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
-      const float t = p.buf[slot];
+      const float t = p.buf[p.two ? 2 * slot : slot];
       dr += t;
       mx += c_cx[q] * t; my += c_cy[q] * t; mz += c_cz[q] * t;
-      if (p.two) rr += p.buf[(size_t)Q * b.S + slot];
+      if (p.two) rr += p.buf[2 * slot + 1];
     }
     const float rho = 1.0f + dr;
     if (!p.two) rr = rho;
