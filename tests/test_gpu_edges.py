@@ -302,3 +302,35 @@ def test_full_size_c5_sampled_macros_and_conservation(lbmod, lbo):
     assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
     mom = np.abs([(u[a].astype(np.float64) * (rr + rb)).sum() for a in range(3)]).max() / w.sites
     assert mom < 1e-5
+
+
+@pytest.mark.parametrize("name,steps", [("c2", 1000), ("c3", 5000), ("c4", 10000)])
+def test_whole_run_conservation(lbmod, name, steps):
+    """The run lengths BASELINE.json asks for, at full size: no NaN, per-component mass drift
+    below 1e-6 relative over the whole run, momentum per site constant where no force acts."""
+    w = W.get(name)
+    sim = pu.make_gpu(lbmod, w)
+    rr0, rb0, u0 = sim.get_macros()
+    m0 = pu.masses(rr0, rb0)
+    sim.step(steps)
+    rr, rb, u = sim.get_macros()
+    assert np.isfinite(u).all() and np.isfinite(rr).all()
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL, (m0, m1)
+    if rb is not None:
+        assert abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL, (m0, m1)
+    rho = rr if rb is None else rr + rb
+    mom = np.array([(u[a].astype(np.float64) * rho).sum() for a in range(3)]) / w.sites
+    if name == "c3":
+        assert np.abs(mom).max() < 1e-5, mom
+        # the mixture has separated: phi is bimodal now, it was +-0.1 noise at t = 0
+        phi = (rr - rb) / rho
+        assert np.mean(np.abs(phi) > 0.5) > 0.5
+    if name == "c2":
+        assert np.abs(mom).max() < 1e-5, mom
+        ke0 = float((u0.astype(np.float64) ** 2).sum())
+        ke = float((u.astype(np.float64) ** 2).sum())
+        assert 0.5 < ke / ke0 < 1.0, ke / ke0       # decays (0.886 for pure viscous decay, G19/P13)
+    if name == "c4":
+        fluid = w.solid == 0
+        assert u[0][fluid].mean() > 0 and np.abs(u[:, ~fluid]).max() == 0
