@@ -284,6 +284,27 @@ def run_ours(args):
            "h2d_bytes_per_step": nfield / K, "d2h_bytes_per_step": nfield / K,
            "note": "lb_init(host) + lb_step(%d) + lb_get_macros(host) per timed region; bytes are totals / K" % K}
 
+    # optional: throughput over the course of the run (the interface fraction changes as domains
+    # coarsen or droplets move): --windows N times N windows of K steps spread over w.steps
+    windows = None
+    if args.windows > 0 and world == 1:
+        sim.init(d_rr, d_rb, d_u)
+        gap = max(0, (w.steps - args.windows * K) // max(1, args.windows - 1)) if args.windows > 1 else 0
+        windows, done = [], 0
+        for i in range(args.windows):
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); sim.step(K); e1.record(); torch.cuda.synchronize()
+            done += K
+            entry = {"steps": [done - K, done], "glups": glups(w.fluid_sites, K, e0.elapsed_time(e1) * 1e-3, 1)}
+            if two:
+                phi = sim.get_phi()
+                fl = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
+                entry["interface_fraction"] = float((np.abs(phi[fl]) < 0.9).mean())
+            windows.append(entry)
+            if i + 1 < args.windows and gap:
+                sim.step(gap); done += gap
+
     if rank != 0:
         return 0
     peak, peak_src = measured_peak()
@@ -302,6 +323,8 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic", "config": config_of(w, args.storage, {"parallelism": "replicas x%d" % world}),
             "clocks": clk.result, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "checks": {"finite": finite, "red_mass_rel_drift": abs(mass - mass0) / mass0}}
+    if windows is not None:
+        line["windows"] = windows
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload)
     elif world > 1:
@@ -321,6 +344,7 @@ def main(argv=None):
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--windows", type=int, default=0, help="also time N windows of K steps spread over the config's run length")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -92,11 +92,13 @@ int lb_set_storage(lb_handle h, int mode);
 /* Initial state (t = 0): f^k_i = w_i rho_k [1 + 3 c.u + 4.5 (c.u)^2 - 1.5 u.u] with the common u
  * (Eq. 2, per component as in Eq. 5-6).  rho_b == NULL selects
  * the single-component BGK mode (config C2).  Input on solid sites is ignored.  Allocates the
- * population buffers: 2 (A/B) or 1 (AA) x 38 (or 19) x S floats, plus the padded phi array. */
+ * population buffers: 2 (A/B) or 1 (AA) x 38 (or 19) x S floats, plus the padded phi array and
+ * 2.125 x S floats of forwarded moments.  Requires S = nx*ny*nz < 2^29. */
 int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u);
 
-/* Advance nsteps time steps: per step the phase-field kernel (rho_r, rho_b, phi; Eq. 3,
- * PAPER.md:96) and the fused pull-stream + collide kernel (Eq. 1-2, 5-8, 11).  Asynchronous. */
+/* Advance nsteps time steps: per step the fused pull-stream + collide kernel (Eq. 1-2, 5-8, 11),
+ * which also forwards the moments of the next state, and the phase-field kernel that turns them
+ * into phi = (rho_r - rho_b)/rho (Eq. 3).  Asynchronous. */
 int lb_step(lb_handle h, int nsteps);
 
 /* rho_r, rho_b and the velocity u = (sum_i c_i f_i + F/2)/rho of the current state (Eq. 3,

@@ -1,20 +1,24 @@
 // CUDA kernels of the colour-gradient D3Q19 hot path, written for sm_100a (B200).
 //
-//   k_phase   K1  gather both components' populations, rho_r, rho_b, phi (Eq. 3),
-//                 write phi (+ periodic ghost images, + sentinel at solid sites)
-//   k_fused   K2  pull-stream + moments + grad phi from a TMA-staged shared-memory phi ring +
-//                 near-contact probe (Eq. 11) + Guo force + BGK on the total
-//                 (Eq. 1-2, 5-8) + perturbation + recolouring + store
-//   k_single  K2s single-component BGK (Eq. 1-4), the pure-bandwidth baseline (config C2)
-//   k_scatter K0  place given pre-collision populations where the next gather finds them
-//   k_gatherf     debug accessor: full pre-collision populations
-//   k_macros  K3  rho_r, rho_b, u with the half-force shift
+// One LB step of a two-component run = k_fused + k_phase_fwd:
+//   k_fused     K2  pull-stream + moments + grad phi from a TMA-staged shared-memory phi ring +
+//                   near-contact probe (Eq. 11) + Guo force + BGK on the total
+//                   (Eq. 1-2, 5-8) + perturbation + recolouring + store, and the
+//                   moments of the NEXT state (Eq. 3) forwarded from registers
+//   k_phase_fwd K1f phi of the next state from the forwarded moments + the brick-face terms
+// Others:
+//   k_phase     K1  full phase-field sweep: gather both components' populations, rho_r, rho_b, phi;
+//                   runs after lb_init / lb_set_populations (phi is not forwarded yet)
+//   k_single    K2s single-component BGK (Eq. 1-4), the pure-bandwidth baseline (config C2)
+//   k_scatter   K0  place given pre-collision populations where the next gather finds them
+//   k_gatherf       debug accessor: full pre-collision populations
+//   k_macros    K3  rho_r, rho_b, u with the half-force shift
 //
-// Storage: SoA planes, x fastest.  Two components: planes 0..18 hold
-// T_q = f^r_q + f^b_q - w_q (the total as a deviation from the lattice weights, so that the
-// hydrodynamic part keeps ~1e-9 absolute precision in fp32), planes 19..37 hold R_q = f^r_q.
-// Single component: planes 0..18 hold f_q - w_q.  The collision is carried out on the
-// deviations directly (T^eq_q = w_q [drho + rho (3 cu + 4.5 cu^2 - 1.5 uu)]).
+// Storage: SoA over the 19 directions, x fastest.  Two components: plane q holds
+// one float2 {T_q, R_q} per site, T_q = f^r_q + f^b_q - w_q (the total as a deviation from the lattice
+// weight, so that the hydrodynamic part keeps ~1e-9 absolute precision in fp32), R_q = f^r_q.
+// Single component: plane q holds f_q - w_q.  The collision is carried out on the deviations
+// directly (T^eq_q = w_q [drho + rho (3 cu + 4.5 cu^2 - 1.5 uu)]).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -106,7 +110,7 @@ __device__ __forceinline__ float* dst_ptr(const P& p, Slot s) {
 template <int MODE>
 __device__ __forceinline__ float2 ld_pair(const float* p) {
   if constexpr (MODE == MODE_AB) return __ldg(reinterpret_cast<const float2*>(p));   // read-only in A/B mode
-  else return *reinterpret_cast<const float2*>(p);
+  else return __ldcg(reinterpret_cast<const float2*>(p));   // in place: read through L2, not through a stale or thrashing L1
 }
 
 template <int MODE>
