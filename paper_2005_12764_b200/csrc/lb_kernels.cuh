@@ -502,6 +502,7 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
       // to the rounding of one sum instead of carrying the relative error of rho_r/rho or of
       // w_q * drho (a systematic drift in uniform regions).
       float racc = 0.f, tacc = 0.f;
+      auto collide = [&](auto bounce) {
       static_for<1, Q + 1>([&](auto qc) {
         constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
         constexpr int k = q == 0 ? 0 : (q < 7 ? 1 : 2);
@@ -523,13 +524,18 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
           ts = dr - tacc;
           rs = rr - racc;
         }
-        const Slot s = write_slot<MODE, HAS_SOLID, q>(c, smask);
+        const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
         *reinterpret_cast<float2*>(dst_ptr(p, s)) = make_float2(ts, rs);
         // f^r* - f^b* = 2 f^r* - f* = (2 rs - w) - ts: the first difference is exact in the mixed
         // regions where phi matters, so the forwarded sum keeps ~1e-8 there
         vd[q] = (2.0f * rs - w) - ts;
         vt[q] = ts;
       });
+      };
+      // only the in-place odd step writes to neighbouring sites, so only there the store slots
+      // depend on the walls; everywhere else one copy of the loop serves both cases
+      if (MODE == MODE_AA_ODD && HAS_SOLID && near_wall) collide(std::integral_constant<bool, HAS_SOLID>{});
+      else collide(std::false_type{});
       if (HAS_SOLID && near_wall) {   // link bounce-back: what would enter a solid site comes back here
         float sd = 0.f, st = 0.f;
         static_for<1, Q>([&](auto qc) {
