@@ -11,7 +11,8 @@
 //   S1 moments      rho_k = sum_i f^k_i, m = sum_i c_i f_i         PAPER.md:96 (Eq. 3)
 //   S2 gradient     G = 3 sum_i w_i c_i phi(x+c_i)                 stencil of Eq. 10
 //   S3 near contact F_rep = -A_h[h] n delta_I                      PAPER.md:221-223 (Eq. 11)
-//   S4 force, u     Guo half-force shift (north_star; S_i role PAPER.md:92)
+//   S4 force, u     Guo half-force shift (north_star; S_i role PAPER.md:92); variant: exact
+//                   difference, the paper's own Eq. 9, lbo_set_forcing(h, 1)
 //   S5 omega_eff    Eq. 7-8, sign of Eq. 7 fixed by Eq. 4
 //   S6 BGK + source Eq. 1 on the total f = f^r + f^b
 //   S7 perturbation colour-gradient surface tension (north_star; not in the paper's text)
@@ -63,6 +64,7 @@ struct Oracle {
   double g[3] = {0, 0, 0};
   double phi_c = 0.9;
   int nc_mode = 0;  // 0 = probe (S3), 1 = test hook: every |phi|<phi_c site in contact with A_h = A_nc
+  int forcing = 0;  // 0 = Guo (north_star; S4, S6), 1 = exact difference, the paper's own Eq. 9
   bool two = true;
   bool inited = false;
   bool any_solid = false;
@@ -203,10 +205,14 @@ void collide_at(Oracle& o, int x, int y, int z) {
   force_at(o, x, y, z, Gx, Gy, Gz, Fx, Fy, Fz);
   const double rr = o.rho_r[s], rb = o.rho_b[s];
   const double rho = rr + rb;
-  // S4: u = (m + F/2)/rho
-  const double ux = (o.mx[s] + 0.5 * Fx) / rho;
-  const double uy = (o.my[s] + 0.5 * Fy) / rho;
-  const double uz = (o.mz[s] + 0.5 * Fz) / rho;
+  // S4: u = (m + F/2)/rho with Guo forcing.  With exact-difference forcing (Eq. 9)
+  // the equilibrium is taken at the bare velocity m/rho (Eq. 3) and the source is
+  // f^eq(rho, u + F dt/rho) - f^eq(rho, u), dt = 1.
+  const bool edm = o.forcing == 1;
+  const double hs = edm ? 0.0 : 0.5;
+  const double ux = (o.mx[s] + hs * Fx) / rho;
+  const double uy = (o.my[s] + hs * Fy) / rho;
+  const double uz = (o.mz[s] + hs * Fz) / rho;
   // S5: relaxation rate. Eq. 8, then omega = 1/(3 nu + 1/2) which is Eq. 4
   // PAPER.md:102 inverted (the minus sign printed in Eq. 7 contradicts Eq. 4: G1).
   double omega;
@@ -230,6 +236,7 @@ void collide_at(Oracle& o, int x, int y, int z) {
     double sy = 3.0 * (CY[i] - uy) + 9.0 * cu * CY[i];
     double sz = 3.0 * (CZ[i] - uz) + 9.0 * cu * CZ[i];
     double guo = (1.0 - 0.5 * omega) * W[i] * (sx * Fx + sy * Fy + sz * Fz);
+    if (edm) guo = feq(i, rho, ux + Fx / rho, uy + Fy / rho, uz + Fz / rho) - fe;   // Eq. 9
     double v = fi - omega * (fi - fe) + guo;
     // S7: colour-gradient perturbation (G5).
     if (aniso) {
@@ -356,6 +363,14 @@ int lbo_set_nc_cutoff(void* h, double phi_c) {
   Oracle* o = static_cast<Oracle*>(h);
   if (!o) return LBO_EINVAL;
   o->phi_c = phi_c;
+  return LBO_OK;
+}
+
+// 0 = Guo forcing (default), 1 = exact-difference forcing (Eq. 9)
+int lbo_set_forcing(void* h, int mode) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (mode != 0 && mode != 1)) return LBO_EINVAL;
+  o->forcing = mode;
   return LBO_OK;
 }
 

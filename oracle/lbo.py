@@ -39,6 +39,7 @@ def _load():
         lib.lbo_set_body_force.argtypes = [vp, C.c_double, C.c_double, C.c_double]
         lib.lbo_set_nc_cutoff.argtypes = [vp, C.c_double]
         lib.lbo_set_nc_mode.argtypes = [vp, C.c_int]
+        lib.lbo_set_forcing.argtypes = [vp, C.c_int]
         lib.lbo_init.argtypes = [vp, dp, dp, dp]
         lib.lbo_step.argtypes = [vp, C.c_int]
         lib.lbo_get_macros.argtypes = [vp, dp, dp, dp]
@@ -109,6 +110,10 @@ class Oracle:
 
     def set_nc_cutoff(self, phi_c):
         self._ck(self.lib.lbo_set_nc_cutoff(self.h, phi_c), "lbo_set_nc_cutoff")
+
+    def set_forcing(self, mode):
+        """0 / 'guo' = Guo forcing, 1 / 'edm' = exact-difference forcing (Eq. 9)."""
+        self._ck(self.lib.lbo_set_forcing(self.h, {'guo': 0, 'edm': 1}.get(mode, mode)), "lbo_set_forcing")
 
     def set_nc_mode(self, mode):
         self._ck(self.lib.lbo_set_nc_mode(self.h, mode), "lbo_set_nc_mode")

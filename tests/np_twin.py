@@ -28,7 +28,7 @@ def half_away(v):
 
 
 def step(fr, fb, solid, tau_r, tau_b, A, beta, A_nc=0.0, g=(0.0, 0.0, 0.0), phi_c=0.9,
-         h_min=3, h_max=4, eps=1e-12):
+         h_min=3, h_max=4, eps=1e-12, forcing="guo"):
     """One time step. fr, fb: [19, nz, ny, nx] pre-collision; solid: bool [nz, ny, nx]."""
     nz, ny, nx = solid.shape
     fluid = ~solid
@@ -66,7 +66,8 @@ def step(fr, fb, solid, tau_r, tau_b, A, beta, A_nc=0.0, g=(0.0, 0.0, 0.0), phi_
                         Ah = A_nc if h <= h_min else A_nc * (h_min / h) ** 3
                         Fnc[:, z, y, x] = 0.5 * Ah * G[:, z, y, x]
     F = np.stack([rho * g[a] + Fnc[a] for a in range(3)])
-    u = (m + 0.5 * F) / rho
+    edm = forcing == "edm"       # exact difference, Eq. 9: bare velocity in f^eq
+    u = m / rho if edm else (m + 0.5 * F) / rho
     if tau_r == tau_b:
         omega = np.full(rho.shape, 1.0 / tau_r)
     else:
@@ -82,6 +83,10 @@ def step(fr, fb, solid, tau_r, tau_b, A, beta, A_nc=0.0, g=(0.0, 0.0, 0.0), phi_
         cu = sum(C[i, a] * u[a] for a in range(3))
         feq = WT[i] * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * uu)
         guo = (1 - 0.5 * omega) * WT[i] * sum((3 * (C[i, a] - u[a]) + 9 * cu * C[i, a]) * F[a] for a in range(3))
+        if edm:
+            v = u + F / rho
+            cv = sum(C[i, a] * v[a] for a in range(3))
+            guo = WT[i] * rho * (1 + 3 * cv + 4.5 * cv ** 2 - 1.5 * (v ** 2).sum(0)) - feq
         fs = ftot[i] - omega * (ftot[i] - feq) + guo
         cg = sum(C[i, a] * G[a] for a in range(3))
         fs = fs + np.where(aniso, A * (WT[i] * cg ** 2 / Gs - BB[i] * Gn), 0.0)

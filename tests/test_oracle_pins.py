@@ -149,8 +149,10 @@ def test_P6_mixture_viscosity(lbo):
 
 
 # ---------------------------------------------------------------------------------- P7
-def test_P7_poiseuille(lbo):
-    """Body-force driven channel between half-way bounce-back walls:
+@pytest.mark.parametrize("forcing", ["guo", "edm"])
+def test_P7_poiseuille(lbo, forcing):
+    """Guo forcing and the paper's exact-difference forcing (Eq. 9) must give the
+    same steady profile.  Body-force driven channel between half-way bounce-back walls:
     u_x(y) = g/(2 nu) (y - 1/2)(32.5 - y), nu = 1/6, peak 7.68e-4; 1 % of peak everywhere."""
     nx, ny, nz = 4, 34, 4
     g = 1e-6
@@ -159,6 +161,7 @@ def test_P7_poiseuille(lbo):
     solid[:, 0, :] = solid[:, -1, :] = True
     o.set_geometry(solid)
     o.set_body_force(g, 0, 0)
+    o.set_forcing(forcing)
     o.init(np.ones((nz, ny, nx)), None, np.zeros((3, nz, ny, nx)))
     o.step(20000)
     _, _, u = o.get_macros()
@@ -332,8 +335,9 @@ def test_P11_lattice_symmetry(lbo):
 
 
 # ---------------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("forcing", ["guo", "edm"])
 @pytest.mark.parametrize("shape,walls", [((4, 4, 4), False), ((6, 5, 4), True)])
-def test_P12_brute_force_numpy_twin(lbo, shape, walls):
+def test_P12_brute_force_numpy_twin(lbo, shape, walls, forcing):
     """All of S1-S9 (both taus, force, near-contact probe, bounce-back) against the numpy
     restatement in tests/np_twin.py, 10 steps, every population, 1e-13."""
     nx, ny, nz = shape
@@ -350,6 +354,7 @@ def test_P12_brute_force_numpy_twin(lbo, shape, walls):
     o = lbo.Oracle(nx, ny, nz, **par)
     o.set_geometry(solid)
     o.set_body_force(*g)
+    o.set_forcing(forcing)
     o.init(rho_r, rho_b, u)
     fr = tw.equilibrium(rho_r, u) * ~solid
     fb = tw.equilibrium(rho_b, u) * ~solid
@@ -357,7 +362,7 @@ def test_P12_brute_force_numpy_twin(lbo, shape, walls):
     contacts = 0
     for _ in range(10):
         contacts += int((o.get_fields()["h"] > 0).sum())
-        fr, fb = tw.step(fr, fb, solid, g=g, **par)
+        fr, fb = tw.step(fr, fb, solid, g=g, forcing=forcing, **par)
         o.step(1)
         assert np.abs(o.get_populations(0) - fr).max() < 1e-13
         assert np.abs(o.get_populations(1) - fb).max() < 1e-13
@@ -383,3 +388,25 @@ def test_P13_taylor_green_decay(lbo):
     expect = np.exp(-6 * (1 / 30) * (2 * np.pi / n) ** 2 * 200)
     assert abs(expect - 0.680) < 1e-3
     assert abs(e1 / e0 - expect) / expect < 0.05
+
+
+# ---------------------------------------------------------------------------------- P14
+def test_P14_exact_difference_source_moments(lbo):
+    """Eq. 9: S_i = f^eq(rho, u + F/rho) - f^eq(rho, u) carries no mass and exactly
+    the momentum F; one collision of a uniform fluid at rest under a uniform force therefore
+    changes the momentum per site by F and nothing else (A = beta = 0, periodic)."""
+    n = 4
+    F = np.array([3e-4, -2e-4, 1e-4])
+    o = lbo.Oracle(n, n, n, 0.9, 0.9, 0.0, 0.0, 0.0)
+    o.set_body_force(*F)                 # rho = 1: force per site = g
+    o.set_forcing("edm")
+    o.init(0.4 * np.ones((n, n, n)), 0.6 * np.ones((n, n, n)), np.zeros((3, n, n, n)))
+    c = np.array(lbo.constants()[0], float)
+    for t in range(1, 4):
+        o.step(1)
+        f = o.get_populations(0) + o.get_populations(1)
+        assert np.abs(f.sum(0) - 1.0).max() < 1e-15                       # no mass
+        mom = np.einsum("ia,izyx->azyx", c, f)
+        assert np.abs(mom - (t * F)[:, None, None, None]).max() < 1e-15   # momentum grows by F per step
+        _, _, u = o.get_macros()
+        assert np.abs(u - ((t + 0.5) * F)[:, None, None, None]).max() < 1e-15   # half-step velocity
