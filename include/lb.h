@@ -82,6 +82,12 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask);
 /* Uniform acceleration g: body force F = rho g enters through the source term. */
 int lb_set_body_force(lb_handle h, float gx, float gy, float gz);
 
+/* How the force enters the collision.  0 (default) = Guo forcing (north_star): source term
+ * (1 - omega/2) w_i [3 (c_i - u) + 9 (c_i.u) c_i].F with u = (m + F/2)/rho.  1 = exact-difference
+ * forcing, the paper's own Eq. 9: S_i = f^eq_i(rho, u + F/rho) - f^eq_i(rho, u)
+ * with the bare u = m/rho.  lb_get_macros returns (m + F/2)/rho in both cases. */
+int lb_set_forcing(lb_handle h, int mode);
+
 /* Near-contact force acts where |phi| < phi_c (default 0.9). */
 int lb_set_nc_cutoff(lb_handle h, float phi_c);
 

@@ -41,6 +41,7 @@ struct StepParams {
   int halo;           // ghost depth K1 must fill (1 without near contact, 4 with)
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
   int two_tau, has_g;
+  int edm;            // exact-difference forcing (Eq. 9) instead of Guo
 };
 
 constexpr int TX = 32, TY = 8;   // CTA tile in x-y; one warp per x row segment
@@ -320,9 +321,12 @@ struct FusedSmem {
   static constexpr size_t BYTES = RING + YEX + XEX + Ring<H>::NS * sizeof(uint64_t);
 };
 
-template <int MODE, bool HAS_SOLID, bool HAS_NC, bool HAS_G>
+// FMODE: bit 0 = a body force rho g acts, bit 1 = the force enters by the exact-difference source
+// (Eq. 9) instead of the Guo term
+template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE>
 __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
+  constexpr bool HAS_G = (FMODE & 1) != 0, EDM = (FMODE & 2) != 0;
   using R_ = Ring<H>;
   using SM_ = FusedSmem<H>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -470,7 +474,9 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
       constexpr bool forced = HAS_NC || HAS_G;
       if constexpr (HAS_G) { Fx += rho * p.gx; Fy += rho * p.gy; Fz += rho * p.gz; }
       // ---- velocity with the half-force shift, relaxation rate (Eq. 7-8)
-      const float ux = (mx + 0.5f * Fx) * inv_rho, uy = (my + 0.5f * Fy) * inv_rho, uz = (mz + 0.5f * Fz) * inv_rho;
+      // (exact difference: f^eq at the bare velocity m/rho, source f^eq(u + F/rho) - f^eq(u))
+      constexpr float hs = EDM ? 0.0f : 0.5f;
+      const float ux = (mx + hs * Fx) * inv_rho, uy = (my + hs * Fy) * inv_rho, uz = (mz + hs * Fz) * inv_rho;
       float omega = omega_same;
       if (p.two_tau) {
         const float inv_nu = (rr * inv_rho) / nu_r + (rb * inv_rho) / nu_b;
@@ -492,6 +498,10 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
       const float ob[3] = {omega * wq(0) * eq0 - p.A * bq(0) * Gne, omega * wq(1) * eq0 - p.A * bq(1) * Gne,
                            omega * wq(7) * eq0 - p.A * bq(7) * Gne};
       const float pa[3] = {0.f, p.A * wq(1) * invG, p.A * wq(7) * invG};
+      //   exact difference         = rw[c] ((cv - cu)(3 + 4.5 (cv + cu)) - 1.5 (v.v - u.u)),  v = u + F/rho
+      const float vx = ux + Fx * inv_rho, vy = uy + Fy * inv_rho, vz = uz + Fz * inv_rho;
+      const float dvv15 = 1.5f * (vx * vx + vy * vy + vz * vz) - uu15;
+      const float rw[3] = {rho * wq(0), rho * wq(1), rho * wq(7)};
       const float g3 = 3.0f * (1.0f - 0.5f * omega);
       const float gw[3] = {g3 * wq(0), g3 * wq(1), g3 * wq(7)};
       const float kc[3] = {0.f, kcol * wq(1), kcol * (wq(7) * inv_cnorm(7))};
@@ -512,9 +522,13 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
           const float cu = cdot<q>(ux, uy, uz);
           const float cG = cdot<q>(Gx, Gy, Gz);
           ts = fmaf(om1, T[q], fmaf(orw[k], cu * fmaf(4.5f, cu, 3.0f), ob[k]));
-          if constexpr (forced) {
+          if constexpr (forced && !EDM) {
             const float cF = cdot<q>(Fx, Fy, Fz);
             ts = fmaf(gw[k], fmaf(cF, fmaf(3.0f, cu, 1.0f), -uF), ts);
+          }
+          if constexpr (forced && EDM) {
+            const float cv = cdot<q>(vx, vy, vz);
+            ts = fmaf(rw[k], fmaf(cv - cu, fmaf(4.5f, cv + cu, 3.0f), -dvv15), ts);
           }
           ts = fmaf(pa[k] * cG, cG, ts);
           rs = fmaf(fr_r, ts, fmaf(kc[k], cG, frw[k]));
@@ -759,9 +773,12 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
     const float rho = 1.0f + dr, inv_rho = 1.0f / rho;
     float Fx = 0.f, Fy = 0.f, Fz = 0.f;
     if (p.has_g) { Fx = rho * p.gx; Fy = rho * p.gy; Fz = rho * p.gz; }
-    const float ux = (mx + 0.5f * Fx) * inv_rho, uy = (my + 0.5f * Fy) * inv_rho, uz = (mz + 0.5f * Fz) * inv_rho;
+    const float hs = p.edm ? 0.0f : 0.5f;
+    const float ux = (mx + hs * Fx) * inv_rho, uy = (my + hs * Fy) * inv_rho, uz = (mz + hs * Fz) * inv_rho;
     const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
     const float uF = ux * Fx + uy * Fy + uz * Fz;
+    const float vx = ux + Fx * inv_rho, vy = uy + Fy * inv_rho, vz = uz + Fz * inv_rho;
+    const float dvv15 = 1.5f * (vx * vx + vy * vy + vz * vz) - uu15;
     float tacc = 0.f;   // the rest population takes what is left of rho - 1 (see k_fused)
     static_for<1, Q + 1>([&](auto qc) {
       constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
@@ -770,8 +787,13 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
       const float teq = w * (dr + rho * (3.0f * cu + 4.5f * cu * cu - uu15));
       float ts = om1 * T[q] + omega * teq;
       if (p.has_g) {
-        const float cF = cdot<q>(Fx, Fy, Fz);
-        ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
+        if (p.edm) {      // exact difference (Eq. 9)
+          const float cv = cdot<q>(vx, vy, vz);
+          ts += (rho * w) * ((cv - cu) * (3.0f + 4.5f * (cv + cu)) - dvv15);
+        } else {
+          const float cF = cdot<q>(Fx, Fy, Fz);
+          ts += g0 * w * (3.0f * (cF - uF) + 9.0f * cu * cF);
+        }
       }
       if constexpr (q > 0) tacc += ts;
       else ts = dr - tacc;

@@ -335,3 +335,44 @@ def test_whole_run_conservation(lbmod, name, steps):
     if name == "c4":
         fluid = w.solid == 0
         assert u[0][fluid].mean() > 0 and np.abs(u[:, ~fluid]).max() == 0
+
+
+# ------------------------------------------------------------------------------- exact-difference forcing
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+@pytest.mark.parametrize("walls", [False, True])
+def test_exact_difference_forcing_parity(lbmod, lbo, storage, walls):
+    """The paper's own forcing (Eq. 9) on the CUDA path against the oracle: body
+    force, near contact, two taus, with and without walls; populations after 1, 2 and 5 steps."""
+    w = _random_workload(36, 13, 10, seed=31 + walls, walls=walls)
+    fluid = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
+    o.set_forcing("edm"); sim.set_forcing("edm")
+    risky = np.zeros(w.shape, bool)
+    done = 0
+    for n in (1, 2, 5):
+        for _ in range(n - done):
+            risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+            o.step(1); sim.step(1)
+        done = n
+        e = pu.pop_error(sim, o)
+        assert e[~risky].max() < pu.POP_TOL, (n, e[~risky].max())
+    # the two forcings are different schemes: the Guo run must differ from this one
+    g = pu.make_gpu(lbmod, w, storage)
+    g.step(5)
+    assert np.abs(g.get_populations(0) - sim.get_populations(0)).max() > 1e-7
+    errs, _, _ = pu.macro_errors(sim, o)
+    assert errs["u"] < 5e-3
+
+
+def test_exact_difference_poiseuille_single_component(lbmod, lbo):
+    nx, ny, nz = 4, 34, 4
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = solid[:, -1, :] = 1
+    w = W.Workload("poiseuille", nx, ny, nz, 1.0, 1.0, 0, 0, 0, np.ones((nz, ny, nx), np.float32), None,
+                   np.zeros((3, nz, ny, nx), np.float32), solid=solid, g=(1e-6, 0, 0))
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w)
+    o.set_forcing("edm"); sim.set_forcing("edm")
+    o.step(2001); sim.step(2001)
+    errs, (rr, _, u), _ = pu.macro_errors(sim, o)
+    assert errs["u"] < 1e-7 and errs["rho_r"] < 1e-5, errs
+    assert u[0].max() > 1e-4
