@@ -18,6 +18,8 @@
 //   S7 perturbation colour-gradient surface tension (north_star; not in the paper's text)
 //   S8 recolouring  Latva-Kokko (north_star; not in the paper's text)
 //   S9 streaming    exact shift + link-wise bounce-back
+// Second model (lbo_set_model(h, 1, G_C)): the paper's section 3.1 as printed, Shan-Chen force
+// (Eq. 10) with exact-difference forcing (Eq. 9) in Eq. 5-6; S1, S5, S9 are shared.
 // Readings of everything the paper leaves open are G1-G24 of SURVEY.md section 8(c), restated
 // in DESIGN.md.
 //
@@ -64,6 +66,8 @@ struct Oracle {
   double g[3] = {0, 0, 0};
   double phi_c = 0.9;
   int nc_mode = 0;  // 0 = probe (S3), 1 = test hook: every |phi|<phi_c site in contact with A_h = A_nc
+  int model = 0;    // 0 = colour gradient (north_star), 1 = Shan-Chen, the paper's own Eq. 5-10
+  double G_C = 0.0; // strength of the inter-component force of Eq. 10, positive = repulsive
   int forcing = 0;  // 0 = Guo (north_star; S4, S6), 1 = exact difference, the paper's own Eq. 9
   bool two = true;
   bool inited = false;
@@ -280,8 +284,68 @@ void stream(Oracle& o) {
       }
 }
 
+// ---- Shan-Chen model, the paper's section 3.1 as printed (model = 1) --------------------------
+// Eq. 10: F^r(x) = rho^r(x) G_C sum_i w_i rho^b(x + c_i) c_i, and the same with r, b
+// swapped.  "G_C ... takes positive values for repulsive interactions", which needs a
+// minus sign in front (reading G27 in DESIGN.md): a^k = F^k / rho^k = -G_C sum_i w_i rho^kbar(x + c_i) c_i.
+// A solid neighbour contributes the centre value (neutral wall, as G8).  The body acceleration g is
+// added to both.  Returns the accelerations a^r, a^b.
+void sc_accel_at(const Oracle& o, int x, int y, int z, double ar[3], double ab[3]) {
+  const size_t s = o.idx(x, y, z);
+  for (int a = 0; a < 3; ++a) ar[a] = ab[a] = 0.0;
+  for (int i = 1; i < Q; ++i) {
+    size_t n = o.nbr(x, y, z, CX[i], CY[i], CZ[i]);
+    const double pb = o.solid[n] ? o.rho_b[s] : o.rho_b[n];
+    const double pr = o.solid[n] ? o.rho_r[s] : o.rho_r[n];
+    const int c[3] = {CX[i], CY[i], CZ[i]};
+    for (int a = 0; a < 3; ++a) {
+      ar[a] += -o.G_C * W[i] * pb * c[a];
+      ab[a] += -o.G_C * W[i] * pr * c[a];
+    }
+  }
+  for (int a = 0; a < 3; ++a) { ar[a] += o.g[a]; ab[a] += o.g[a]; }
+}
+
+// Eq. 5-9 at one fluid site: each component relaxes to f^eq(rho^k, u) with the
+// common bare velocity u = m / rho (Eq. 3) and the common omega_eff (Eq. 7-8, sign G1), plus the
+// exact-difference source S^k_i = f^eq_i(rho^k, u + F^k dt / rho^k) - f^eq_i(rho^k, u), dt = 1.
+void collide_sc_at(Oracle& o, int x, int y, int z) {
+  const size_t s = o.idx(x, y, z);
+  double ar[3], ab[3];
+  sc_accel_at(o, x, y, z, ar, ab);
+  const double rr = o.rho_r[s], rb = o.rho_b[s], rho = rr + rb;
+  o.Fx[s] = rr * ar[0] + rb * ab[0];   // total force, for the velocity that get_macros returns
+  o.Fy[s] = rr * ar[1] + rb * ab[1];
+  o.Fz[s] = rr * ar[2] + rb * ab[2];
+  const double ux = o.mx[s] / rho, uy = o.my[s] / rho, uz = o.mz[s] / rho;
+  double omega;
+  if (o.tau_r == o.tau_b) {
+    omega = 1.0 / o.tau_r;
+  } else {
+    double nu_r = (o.tau_r - 0.5) / 3.0, nu_b = (o.tau_b - 0.5) / 3.0;
+    double nu = 1.0 / ((rr / rho) / nu_r + (rb / rho) / nu_b);
+    omega = 1.0 / (3.0 * nu + 0.5);
+  }
+  for (int i = 0; i < Q; ++i) {
+    const double fer = feq(i, rr, ux, uy, uz), feb = feq(i, rb, ux, uy, uz);
+    const double Sr = feq(i, rr, ux + ar[0], uy + ar[1], uz + ar[2]) - fer;
+    const double Sb = feq(i, rb, ux + ab[0], uy + ab[1], uz + ab[2]) - feb;
+    o.fpost[0][s * Q + i] = (1.0 - omega) * o.f[0][s * Q + i] + omega * fer + Sr;
+    o.fpost[1][s * Q + i] = (1.0 - omega) * o.f[1][s * Q + i] + omega * feb + Sb;
+  }
+}
+
 void one_step(Oracle& o) {
   moments(o);
+  if (o.model == 1) {
+#pragma omp parallel for schedule(static)
+    for (int z = 0; z < o.nz; ++z)
+      for (int y = 0; y < o.ny; ++y)
+        for (int x = 0; x < o.nx; ++x)
+          if (!o.solid[o.idx(x, y, z)]) collide_sc_at(o, x, y, z);
+    stream(o);
+    return;
+  }
 #pragma omp parallel for schedule(static)
   for (int z = 0; z < o.nz; ++z)
     for (int y = 0; y < o.ny; ++y)
@@ -299,6 +363,17 @@ void eval_forces(Oracle& o) {
         size_t s = o.idx(x, y, z);
         if (o.solid[s]) {
           o.Fx[s] = o.Fy[s] = o.Fz[s] = 0;
+          o.Gx[s] = o.Gy[s] = o.Gz[s] = 0;
+          o.hcontact[s] = 0;
+          o.margin[s] = 1e300;
+          continue;
+        }
+        if (o.model == 1) {
+          double ar[3], ab[3];
+          sc_accel_at(o, x, y, z, ar, ab);
+          o.Fx[s] = o.rho_r[s] * ar[0] + o.rho_b[s] * ab[0];
+          o.Fy[s] = o.rho_r[s] * ar[1] + o.rho_b[s] * ab[1];
+          o.Fz[s] = o.rho_r[s] * ar[2] + o.rho_b[s] * ab[2];
           o.Gx[s] = o.Gy[s] = o.Gz[s] = 0;
           o.hcontact[s] = 0;
           o.margin[s] = 1e300;
@@ -366,6 +441,17 @@ int lbo_set_nc_cutoff(void* h, double phi_c) {
   return LBO_OK;
 }
 
+// model 0 = colour gradient (A, beta, A_nc of lbo_create apply), 1 = Shan-Chen with exact-difference
+// forcing, Eq. 5-10 of the paper (G_C applies; A, beta, A_nc are ignored; needs two components)
+int lbo_set_model(void* h, int model, double G_C) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (model != 0 && model != 1)) return LBO_EINVAL;
+  if (o->inited) return LBO_ESTATE;
+  o->model = model;
+  o->G_C = G_C;
+  return LBO_OK;
+}
+
 // 0 = Guo forcing (default), 1 = exact-difference forcing (Eq. 9)
 int lbo_set_forcing(void* h, int mode) {
   Oracle* o = static_cast<Oracle*>(h);
@@ -385,6 +471,7 @@ int lbo_set_nc_mode(void* h, int mode) {
 int lbo_init(void* h, const double* rho_r, const double* rho_b, const double* u) {
   Oracle* o = static_cast<Oracle*>(h);
   if (!o || !rho_r || !u) return LBO_EINVAL;
+  if (o->model == 1 && !rho_b) return LBO_EINVAL;   // the Shan-Chen model couples two components
   const size_t S = o->S;
   o->two = rho_b != nullptr;
   const int nk = o->two ? 2 : 1;

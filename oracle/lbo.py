@@ -40,6 +40,7 @@ def _load():
         lib.lbo_set_nc_cutoff.argtypes = [vp, C.c_double]
         lib.lbo_set_nc_mode.argtypes = [vp, C.c_int]
         lib.lbo_set_forcing.argtypes = [vp, C.c_int]
+        lib.lbo_set_model.argtypes = [vp, C.c_int, C.c_double]
         lib.lbo_init.argtypes = [vp, dp, dp, dp]
         lib.lbo_step.argtypes = [vp, C.c_int]
         lib.lbo_get_macros.argtypes = [vp, dp, dp, dp]
@@ -110,6 +111,10 @@ class Oracle:
 
     def set_nc_cutoff(self, phi_c):
         self._ck(self.lib.lbo_set_nc_cutoff(self.h, phi_c), "lbo_set_nc_cutoff")
+
+    def set_model(self, model, G_C=0.0):
+        """0 / 'cg' = colour gradient, 1 / 'sc' = Shan-Chen + exact difference (Eq. 5-10 of the paper)."""
+        self._ck(self.lib.lbo_set_model(self.h, {'cg': 0, 'sc': 1}.get(model, model), float(G_C)), "lbo_set_model")
 
     def set_forcing(self, mode):
         """0 / 'guo' = Guo forcing, 1 / 'edm' = exact-difference forcing (Eq. 9)."""
