@@ -29,6 +29,7 @@ sys.path.insert(0, ROOT)
 METRIC = "GLUPS (two-component D3Q19 site updates/s)"
 BYTES_PER_UPDATE = {True: 2 * 2 * 19 * 4, False: 2 * 19 * 4}   # two-component 304 B, single 152 B
 FALLBACK_HBM_GBS = 6650.0
+MODEL = ["cg", 0.0]      # --model: colour gradient (north_star) or the paper's Shan-Chen coupling, and its G_C
 
 
 # ------------------------------------------------------------------------------ helpers
@@ -121,7 +122,7 @@ class ClockSampler:
 def config_of(w, storage, extra=None):
     c = {"workload": w.name, "box": [w.nx, w.ny, w.nz], "sites": w.sites, "fluid_sites": w.fluid_sites,
          "components": 2 if w.rho_b is not None else 1, "near_contact": bool(w.A_nc != 0.0),
-         "walls": w.solid is not None, "storage": storage,
+         "walls": w.solid is not None, "storage": storage, "model": "colour-gradient" if MODEL[0] == "cg" else "shan-chen G_C=%g" % MODEL[1],
          "params": dict(tau_r=w.tau_r, tau_b=w.tau_b, A=w.A, beta=w.beta, A_nc=w.A_nc, g=list(w.g)),
          "l2": "state (%.2f GB) is larger than L2, no flush needed" % (w.sites * 4 * (38 if w.rho_b is not None else 19) * (2 if storage == "ab" else 1) / 1e9)}
     c.update(w.info)
@@ -156,6 +157,8 @@ def oracle_sample_workload(name, budget_updates):
 def time_oracle(w, steps, warmup):
     from oracle import lbo
     o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    if MODEL[0] == "sc":
+        o.set_model("sc", MODEL[1])
     if w.solid is not None:
         o.set_geometry(w.solid)
     o.set_body_force(*w.g)
@@ -231,6 +234,8 @@ def run_ours(args):
     d_rb = torch.from_numpy(w.rho_b).to(dev) if two else None
     d_u = torch.from_numpy(w.u).to(dev)
     sim = lb.from_workload(w, storage=args.storage)
+    if MODEL[0] == "sc":
+        sim.set_model("sc", MODEL[1])
     sim.init(d_rr, d_rb, d_u)
     sim.set_profiling(7)      # every 7th step (odd, so that both AA parities are sampled) is timed kernel by kernel (CUDA events on the stream)
     sim.step(Wu)
@@ -344,9 +349,12 @@ def main(argv=None):
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--model", default="cg", choices=["cg", "sc"], help="cg = colour gradient (north_star), sc = Shan-Chen + exact difference (Eq. 5-10 of the paper)")
+    ap.add_argument("--gc", type=float, default=3.0, help="G_C of the Shan-Chen model")
     ap.add_argument("--windows", type=int, default=0, help="also time N windows of K steps spread over the config's run length")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    MODEL[0], MODEL[1] = args.model, args.gc
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

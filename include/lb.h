@@ -82,6 +82,14 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask);
 /* Uniform acceleration g: body force F = rho g enters through the source term. */
 int lb_set_body_force(lb_handle h, float gx, float gy, float gz);
 
+/* Which two-component model lb_step advances.  0 (default) = colour gradient + Latva-Kokko
+ * recolouring + near contact (north_star; A, beta, A_nc of lb_params).  1 = the paper's section
+ * 3.1 as printed: each component relaxes to f^eq(rho^k, u) (Eq. 5-6) and
+ * receives the exact-difference source (Eq. 9) of the Shan-Chen force
+ * F^r = -G_C rho^r sum_i w_i rho^b(x + c_i) c_i, and r, b swapped (Eq. 10; positive
+ * G_C repels); A, beta, A_nc do not act.  Must precede lb_init; needs rho_b. */
+int lb_set_model(lb_handle h, int model, float G_C);
+
 /* How the force enters the collision.  0 (default) = Guo forcing (north_star): source term
  * (1 - omega/2) w_i [3 (c_i - u) + 9 (c_i.u) c_i].F with u = (m + F/2)/rho.  1 = exact-difference
  * forcing, the paper's own Eq. 9: S_i = f^eq_i(rho, u + F/rho) - f^eq_i(rho, u)

@@ -72,6 +72,10 @@ struct lb_handle_s {
   cudaStream_t stream = 0;
   long long launches = 0;
   CUtensorMap tmap{};
+  CUtensorMap tmap2{};       // Shan-Chen model: the rho_b array
+  float* phi2 = nullptr;
+  int model = 0;            // 0 colour gradient, 1 Shan-Chen + exact difference (Eq. 5-10 of the paper)
+  float G_C = 0.f;
   bool tmap_ok = false;
   bool phi_current = false;  // phi array matches the current populations
   float* mom = nullptr;      // forwarded moments Md, Mt (2 x S floats), written by k_fused
@@ -156,6 +160,7 @@ namespace {
 StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   StepParams p;
   p.src = src; p.dst = dst; p.phi = h->phi;
+  p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
   const size_t plane = (h->two ? 2 : 1) * (size_t)h->S;   // floats per direction plane ({T, R} pairs or T)
   for (int q = 0; q < Q; ++q) {
     p.ps[q] = src ? src + (size_t)q * plane : nullptr;
@@ -164,7 +169,7 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   p.Md = h->mom; p.Mt = h->mom ? h->mom + h->S : nullptr; p.EX = h->mom ? h->mom + 2 * h->S : nullptr;
   p.box = h->box();
   p.zc = zc;
-  p.halo = h->par.A_nc != 0.f ? H_MAX_NC : 1;
+  p.halo = (h->model == 0 && h->par.A_nc != 0.f) ? H_MAX_NC : 1;
   p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
   p.A_nc = h->par.A_nc; p.phi_c = h->phi_c;
   p.gx = h->g[0]; p.gy = h->g[1]; p.gz = h->g[2];
@@ -209,8 +214,14 @@ dim3 tile_grid(lb_handle h, int zc) {
 
 template <int MODE>
 void launch_phase(lb_handle h, const StepParams& p, dim3 grid) {
-  if (h->has_solid) k_phase<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
-  else k_phase<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+  const dim3 blk(TX, TY);
+  if (h->model == 1) {
+    if (h->has_solid) k_phase<MODE, true, true><<<grid, blk, 0, h->stream>>>(p);
+    else k_phase<MODE, false, true><<<grid, blk, 0, h->stream>>>(p);
+  } else {
+    if (h->has_solid) k_phase<MODE, true, false><<<grid, blk, 0, h->stream>>>(p);
+    else k_phase<MODE, false, false><<<grid, blk, 0, h->stream>>>(p);
+  }
 }
 template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE>
 void launch_fused_t(lb_handle h, const StepParams& p, dim3 grid) {
@@ -220,7 +231,7 @@ void launch_fused_t(lb_handle h, const StepParams& p, dim3 grid) {
     cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, HAS_NC, FMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
-  k_fused<MODE, HAS_SOLID, HAS_NC, FMODE><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap);
+  k_fused<MODE, HAS_SOLID, HAS_NC, FMODE><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap);
 }
 template <int MODE, bool HAS_SOLID, bool HAS_NC>
 void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
@@ -237,8 +248,24 @@ void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
     else launch_fused_t<MODE, HAS_SOLID, HAS_NC, 0>(h, p, grid);
   }
 }
+template <int MODE, bool HAS_SOLID, int FMODE>
+void launch_fused_sc(lb_handle h, const StepParams& p, dim3 grid) {
+  constexpr size_t smem = FusedSmem<1, true>::BYTES;
+  static bool attr_set = false;   // per instantiation
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, false, FMODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  k_fused<MODE, HAS_SOLID, false, FMODE, true><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap2);
+}
 template <int MODE>
 void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
+  if (h->model == 1) {      // Shan-Chen: no near contact; the only force flag is the body force
+    const bool g = p.has_g || MODE != MODE_AB;    // AA: the body-force instantiation, as in launch_fused_g
+    if (h->has_solid) { if (g) launch_fused_sc<MODE, true, 1>(h, p, grid); else launch_fused_sc<MODE, true, 0>(h, p, grid); }
+    else { if (g) launch_fused_sc<MODE, false, 1>(h, p, grid); else launch_fused_sc<MODE, false, 0>(h, p, grid); }
+    return;
+  }
   const bool nc = h->par.A_nc != 0.f;
   if (h->has_solid) {
     if (nc) launch_fused_g<MODE, true, true>(h, p, grid);
@@ -250,8 +277,14 @@ void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
 }
 template <int MODE>
 void launch_phase_fwd(lb_handle h, const StepParams& p, dim3 grid) {
-  if (h->has_solid) k_phase_fwd<MODE, true><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
-  else k_phase_fwd<MODE, false><<<grid, dim3(TX, TY), 0, h->stream>>>(p);
+  const dim3 blk(TX, TY);
+  if (h->model == 1) {
+    if (h->has_solid) k_phase_fwd<MODE, true, true><<<grid, blk, 0, h->stream>>>(p);
+    else k_phase_fwd<MODE, false, true><<<grid, blk, 0, h->stream>>>(p);
+  } else {
+    if (h->has_solid) k_phase_fwd<MODE, true, false><<<grid, blk, 0, h->stream>>>(p);
+    else k_phase_fwd<MODE, false, false><<<grid, blk, 0, h->stream>>>(p);
+  }
 }
 template <int MODE>
 void launch_single(lb_handle h, const StepParams& p, dim3 grid) {
@@ -317,6 +350,7 @@ IoParams make_io_params(lb_handle h) {
   p.box = h->box();
   p.two = h->two;
   p.phi = h->phi;
+  p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
   p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
   p.A_nc = h->par.A_nc; p.phi_c = h->phi_c;
   p.gx = h->g[0]; p.gy = h->g[1]; p.gz = h->g[2];
@@ -391,7 +425,7 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
 void lb_destroy(lb_handle h) {
   if (!h) return;
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
-  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->mask); dev_free(h->mom);
+  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->phi2); dev_free(h->mask); dev_free(h->mom);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
   for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
   cudaGetLastError();
@@ -437,6 +471,14 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
 int lb_set_body_force(lb_handle h, float gx, float gy, float gz) {
   if (!h) return LB_EINVAL;
   h->g[0] = gx; h->g[1] = gy; h->g[2] = gz;
+  return LB_OK;
+}
+
+int lb_set_model(lb_handle h, int model, float G_C) {
+  if (!h || (model != 0 && model != 1)) return fail(h, LB_EINVAL, "model must be 0 (colour gradient) or 1 (Shan-Chen)");
+  if (h->inited) return fail(h, LB_ESTATE, "lb_set_model after lb_init");
+  h->model = model;
+  h->G_C = G_C;
   return LB_OK;
 }
 
@@ -486,24 +528,26 @@ int allocate_state(lb_handle h, bool two) {
     if (!h->mom) return fail(h, LB_ENOMEM, "moment buffer allocation failed");
     h->bytes += mb;
   }
-  if (two && !h->phi) {
+  const bool nc = h->model == 0 && h->par.A_nc != 0.f;
+  for (int f = 0; f < (h->model == 1 ? 2 : 1); ++f) {
+    float*& field = f == 0 ? h->phi : h->phi2;
+    if (!two || field) continue;
     const size_t px = h->nx + 2 * HALO, py = h->ny + 2 * HALO, pz = h->nz + 2 * HALO;
     const size_t phib = px * py * pz * sizeof(float);
-    h->phi = static_cast<float*>(dev_alloc(phib));
-    if (!h->phi) return fail(h, LB_ENOMEM, "phi allocation failed");
+    field = static_cast<float*>(dev_alloc(phib));
+    if (!field) return fail(h, LB_ENOMEM, "phi allocation failed");
     h->bytes += phib;
-    cudaError_t e = cudaMemsetAsync(h->phi, 0, phib, h->stream);
+    cudaError_t e = cudaMemsetAsync(field, 0, phib, h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "phi memset");
-    // TMA descriptor of the padded phi array: dims (x, y, z), box (BX, BY, 1)
+    // TMA descriptor of the padded array: dims (x, y, z), box (BX, BY, 1)
     EncodeTiledFn enc = get_encode();
     if (!enc) return fail(h, LB_ECUDA, "cuTensorMapEncodeTiled entry point not found");
-    const bool nc = h->par.A_nc != 0.f;
     cuuint64_t dims[3] = {px, py, pz};
     cuuint64_t strides[2] = {px * sizeof(float), px * py * sizeof(float)};
     cuuint32_t box[3] = {(cuuint32_t)(nc ? Ring<H_MAX_NC>::BX : Ring<1>::BX),
                          (cuuint32_t)(nc ? Ring<H_MAX_NC>::BY : Ring<1>::BY), 1};
     cuuint32_t estr[3] = {1, 1, 1};
-    CUresult r = enc(&h->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, h->phi, dims, strides, box, estr,
+    CUresult r = enc(f == 0 ? &h->tmap : &h->tmap2, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, field, dims, strides, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(h, LB_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
@@ -519,6 +563,7 @@ extern "C" {
 int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u) {
   if (!h) return LB_EINVAL;
   if (!rho_r || !u) return fail(h, LB_EINVAL, "rho_r and u must not be NULL");
+  if (h->model == 1 && !rho_b) return fail(h, LB_EINVAL, "the Shan-Chen model couples two components: rho_b must not be NULL");
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
     cudaGetLastError();
@@ -658,7 +703,7 @@ int lb_get_phi(lb_handle h, float* phi) {
   if ((rc = stage_out(h, phi, fb, o))) return rc;
   run_phase(h);
   const int tb = 256;
-  k_unpad_phi<<<(unsigned)((h->S + tb - 1) / tb), tb, 0, h->stream>>>(h->phi, static_cast<float*>(o.dev), h->box());
+  k_unpad_phi<<<(unsigned)((h->S + tb - 1) / tb), tb, 0, h->stream>>>(h->phi, h->model == 1 ? h->phi2 : nullptr, static_cast<float*>(o.dev), h->box());
   h->launches++;
   if ((rc = check_launch(h, "k_unpad_phi"))) return rc;
   if ((rc = finish_out(h, phi, fb, o))) return rc;

@@ -33,6 +33,7 @@ struct StepParams {
   float* pd[Q];         // is one 64-bit add of a constant-bank operand and a 32-bit byte offset
   float* dst;         // buffer written (== src in AA modes)
   float* phi;         // padded phi array (written by K1 / K1f, read by K2 / K3)
+  float* phi2;        // Shan-Chen model only: the padded array of rho_b (phi then holds rho_r)
   float* Md;          // forwarded moments of the next state (written by K2, read by K1f):
   float* Mt;          //   Md = sum (f^r - f^b), Mt = sum (f - w) over what arrives from inside the brick
   float* EX;          // the same sums for what crosses the x faces of the bricks: [z][y][tile][side]{D, Tm}
@@ -42,6 +43,8 @@ struct StepParams {
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
   int two_tau, has_g;
   int edm;            // exact-difference forcing (Eq. 9) instead of Guo
+  int sc;             // Shan-Chen model (Eq. 5-10 of the paper): the fields are rho_r, rho_b instead of phi
+  float G_C;          // its coupling strength, positive = repulsive
 };
 
 constexpr int TX = 32, TY = 8;   // CTA tile in x-y; one warp per x row segment
@@ -174,11 +177,10 @@ __device__ __forceinline__ void two_sum_acc(float& s, float& e, float x) {
 
 // phi of site (x, y, z) to its home in the padded array and to every periodic image that falls
 // into the ghost layers (depth H).
-__device__ __forceinline__ void store_phi_with_images(const StepParams& p, int x, int y, int z, int H, float phi) {
-  const Box& b = p.box;
+__device__ __forceinline__ void store_field_with_images(float* field, const Box& b, int x, int y, int z, int H, float phi) {
   const int px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
   if (x >= H && x < b.nx - H && y >= H && y < b.ny - H && z >= H && z < b.nz - H) {   // no image
-    p.phi[(size_t)(x + HALO) + (size_t)px * ((size_t)(y + HALO) + (size_t)py * (size_t)(z + HALO))] = phi;
+    field[(size_t)(x + HALO) + (size_t)px * ((size_t)(y + HALO) + (size_t)py * (size_t)(z + HALO))] = phi;
     return;
   }
   const int sx[3] = {0, x < H ? b.nx : 0, x >= b.nx - H ? -b.nx : 0};
@@ -193,31 +195,42 @@ __device__ __forceinline__ void store_phi_with_images(const StepParams& p, int x
 #pragma unroll
       for (int ix = 0; ix < 3; ++ix) {
         if (ix && !sx[ix]) continue;
-        p.phi[(size_t)(x + sx[ix] + HALO) + (size_t)px * ((size_t)(y + sy[iy] + HALO) + (size_t)py * (size_t)(z + sz[iz] + HALO))] = phi;
+        field[(size_t)(x + sx[ix] + HALO) + (size_t)px * ((size_t)(y + sy[iy] + HALO) + (size_t)py * (size_t)(z + sz[iz] + HALO))] = phi;
       }
     }
   }
 }
 
+// What the fused kernel needs of its neighbours at site (x, y, z), from d = rho_r - rho_b and rho:
+// phi = d / rho for the colour-gradient model, the pair rho_r, rho_b for the Shan-Chen model.
+// Solid sites carry the sentinel in the first field.
+template <bool SC>
+__device__ __forceinline__ void store_fields(const StepParams& p, int x, int y, int z, int H, bool solid, float d, float rho) {
+  if constexpr (!SC) {
+    store_field_with_images(p.phi, p.box, x, y, z, H, solid ? PHI_SOLID : d / rho);
+  } else {
+    store_field_with_images(p.phi, p.box, x, y, z, H, solid ? PHI_SOLID : 0.5f * (rho + d));
+    store_field_with_images(p.phi2, p.box, x, y, z, H, solid ? 0.f : 0.5f * (rho - d));
+  }
+}
+
 // ----------------------------------------------------------------------------- K1 phase field
 // One thread per site of a TX x TY tile, marching over zc planes.  152 B read, 4 B written.
-template <int MODE, bool HAS_SOLID>
+template <int MODE, bool HAS_SOLID, bool SC>
 __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, int zb, int ze) {
   const Box& b = p.box;
   const int H = p.halo;
   for (int z = zb; z < ze; ++z) {
     Ctx c;
     make_ctx<8>(c, b, x, y, z);
-    float phi;
+    float num = 0.f, rho = 1.f;
     bool self_solid = false;
     uint32_t smask = 0;
     if constexpr (HAS_SOLID) {
       self_solid = solid_at(b, x, y, z);
       if (!self_solid) smask = neighbour_mask(b, x, y, z);
     }
-    if (self_solid) {
-      phi = PHI_SOLID;
-    } else {
+    if (!self_solid) {
       float t[Q], r[Q];
       static_for<0, Q>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
@@ -236,21 +249,20 @@ __device__ __forceinline__ void phase_column(const StepParams& p, int x, int y, 
         two_sum_acc(rr, re, r[q]);
       });
       // rho_r - rho_b = 2 rho_r - rho = (2 rr - 1 - dr) + (2 re - de); rho = 1 + dr + de
-      const float num = ((2.0f * rr - 1.0f) - dr) + (2.0f * re - de);
-      const float rho = (1.0f + dr) + de;
-      phi = num / rho;
+      num = ((2.0f * rr - 1.0f) - dr) + (2.0f * re - de);
+      rho = (1.0f + dr) + de;
     }
-    store_phi_with_images(p, x, y, z, H, phi);
+    store_fields<SC>(p, x, y, z, H, self_solid, num, rho);
   }
 }
 
-template <int MODE, bool HAS_SOLID>
+template <int MODE, bool HAS_SOLID, bool SC>
 __global__ void __launch_bounds__(TX* TY) k_phase(const StepParams p) {
   const int x = blockIdx.x * TX + threadIdx.x;
   const int y = blockIdx.y * TY + threadIdx.y;
   if (x >= p.box.nx || y >= p.box.ny) return;
   const int zb = blockIdx.z * p.zc;
-  phase_column<MODE, HAS_SOLID>(p, x, y, zb, min(p.box.nz, zb + p.zc));
+  phase_column<MODE, HAS_SOLID, SC>(p, x, y, zb, min(p.box.nz, zb + p.zc));
 }
 
 // ----------------------------------------------------------------------------- TMA / mbarrier
@@ -312,10 +324,11 @@ struct Ring {
 // z: carried in registers from one plane to the next (plane z-1 is complete once plane z is done).
 // A population that would enter a solid site returns to its own site (bounce-back) and is added
 // there.  What enters a brick through its faces is added by k_phase_fwd from the stored values.
-template <int H>
+template <int H, bool SC = false>
 struct FusedSmem {
   static constexpr int NEX = 12;   // exchanged values: 6 (cy = +-1) x {D, Tm}
-  static constexpr size_t RING = (size_t)Ring<H>::NS * Ring<H>::SLOT * sizeof(float);
+  static constexpr size_t RING1 = (size_t)Ring<H>::NS * Ring<H>::SLOT * sizeof(float);
+  static constexpr size_t RING = (SC ? 2 : 1) * RING1;   // Shan-Chen: a second ring for rho_b
   static constexpr size_t YEX = (size_t)2 * NEX * TX * TY * sizeof(float);
   static constexpr size_t XEX = (size_t)2 * 2 * 4 * TY * sizeof(float);   // [buffer][side][(+1,-1) x {D, Tm}][row]
   static constexpr size_t BYTES = RING + YEX + XEX + Ring<H>::NS * sizeof(uint64_t);
@@ -323,14 +336,21 @@ struct FusedSmem {
 
 // FMODE: bit 0 = a body force rho g acts, bit 1 = the force enters by the exact-difference source
 // (Eq. 9) instead of the Guo term
-template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE>
-__global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap) {
+// SC: the paper's section 3.1 as printed instead of the colour-gradient model: the two rings hold
+// rho_r and rho_b, the Shan-Chen accelerations (Eq. 10; sign: DESIGN.md G27) replace
+// grad phi, each component gets the exact-difference source of Eq. 9, and there is no perturbation,
+// recolouring or near-contact force (HAS_NC = false; FMODE bit 0 only).
+template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE, bool SC = false>
+__global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap,
+                                                     const __grid_constant__ CUtensorMap tmap2) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
   constexpr bool HAS_G = (FMODE & 1) != 0, EDM = (FMODE & 2) != 0;
+  static_assert(!SC || !HAS_NC, "the Shan-Chen model has no near-contact force");
   using R_ = Ring<H>;
-  using SM_ = FusedSmem<H>;
+  using SM_ = FusedSmem<H, SC>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float* ring = reinterpret_cast<float*>(smem_raw);
+  float* ring2 = reinterpret_cast<float*>(smem_raw + SM_::RING1);     // used only if SC
   float* yex = reinterpret_cast<float*>(smem_raw + SM_::RING);                 // [2][NEX][TY][TX]
   float* xex = reinterpret_cast<float*>(smem_raw + SM_::RING + SM_::YEX);     // [2][2][4][TY]
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + SM_::RING + SM_::YEX + SM_::XEX);
@@ -353,8 +373,9 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
   __syncthreads();
   auto issue = [&](int j) {
     const int s = j % R_::NS;
-    mbar_expect_tx(&bars[s], R_::BYTES);
+    mbar_expect_tx(&bars[s], (SC ? 2u : 1u) * R_::BYTES);
     tma_load_3d(&ring[s * R_::SLOT], &tmap, &bars[s], x0, y0 + HALO - H, zb - H + j + HALO);
+    if constexpr (SC) tma_load_3d(&ring2[s * R_::SLOT], &tmap2, &bars[s], x0, y0 + HALO - H, zb - H + j + HALO);
   };
   if (tid == 0) {
     const int n0 = min(npl, R_::NS);
@@ -401,20 +422,39 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
       // ---- grad phi (stencil of Eq. 10) and solid flags from the phi tile
       const float* plm = plane(-1);
       const float* plp = plane(+1);
-      float Gx = 0.f, Gy = 0.f, Gz = 0.f;
+      float Gx = 0.f, Gy = 0.f, Gz = 0.f;       // SC: sum_i w_i c_i rho_b(x + c_i)
+      float Hx = 0.f, Hy = 0.f, Hz = 0.f;       // SC: sum_i w_i c_i rho_r(x + c_i)
       uint32_t smask = 0;
-      static_for<1, Q>([&](auto qc) {
-        constexpr int q = decltype(qc)::value;
-        const float* pl = cz(q) == 0 ? pl0 : (cz(q) > 0 ? plp : plm);
-        float v = pl[(ly + cy(q)) * R_::BX + lx + cx(q)];
-        if constexpr (HAS_SOLID) {
-          if (v > PHI_SOLID_TEST) { smask |= 1u << q; v = phi0; }
-        }
-        constexpr float k = 3.0f * wq(q);
-        if constexpr (cx(q) != 0) Gx += (k * cx(q)) * v;
-        if constexpr (cy(q) != 0) Gy += (k * cy(q)) * v;
-        if constexpr (cz(q) != 0) Gz += (k * cz(q)) * v;
-      });
+      if constexpr (!SC) {
+        static_for<1, Q>([&](auto qc) {
+          constexpr int q = decltype(qc)::value;
+          const float* pl = cz(q) == 0 ? pl0 : (cz(q) > 0 ? plp : plm);
+          float v = pl[(ly + cy(q)) * R_::BX + lx + cx(q)];
+          if constexpr (HAS_SOLID) {
+            if (v > PHI_SOLID_TEST) { smask |= 1u << q; v = phi0; }
+          }
+          constexpr float k = 3.0f * wq(q);
+          if constexpr (cx(q) != 0) Gx += (k * cx(q)) * v;
+          if constexpr (cy(q) != 0) Gy += (k * cy(q)) * v;
+          if constexpr (cz(q) != 0) Gz += (k * cz(q)) * v;
+        });
+      } else {
+        const int ro = (int)(ring2 - ring);     // the rho_b tile sits at the same place in the second ring
+        const float rb0 = pl0[ro + ly * R_::BX + lx];
+        static_for<1, Q>([&](auto qc) {
+          constexpr int q = decltype(qc)::value;
+          const float* pl = cz(q) == 0 ? pl0 : (cz(q) > 0 ? plp : plm);
+          const int o = (ly + cy(q)) * R_::BX + lx + cx(q);
+          float vr = pl[o], vb = pl[ro + o];
+          if constexpr (HAS_SOLID) {
+            if (vr > PHI_SOLID_TEST) { smask |= 1u << q; vr = phi0; vb = rb0; }   // neutral wall
+          }
+          constexpr float k = wq(q);
+          if constexpr (cx(q) != 0) { Gx += (k * cx(q)) * vb; Hx += (k * cx(q)) * vr; }
+          if constexpr (cy(q) != 0) { Gy += (k * cy(q)) * vb; Hy += (k * cy(q)) * vr; }
+          if constexpr (cz(q) != 0) { Gz += (k * cz(q)) * vb; Hz += (k * cz(q)) * vr; }
+        });
+      }
       // ---- gather.  Walls are rare: a warp none of whose sites has a solid neighbour takes the
       // addressing of the wall-free variant (no per-direction select between the two slots).
       bool near_wall = false;
@@ -444,6 +484,7 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
       const float rho = 1.0f + dr;
       const float rb = rho - rr;
       const float inv_rho = 1.0f / rho;
+      if constexpr (!SC) {
       const float Gn2 = Gx * Gx + Gy * Gy + Gz * Gz;
       const float Gn = sqrtf(Gn2);
       const bool aniso = Gn > EPS_G;
@@ -550,6 +591,61 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
       // depend on the walls; everywhere else one copy of the loop serves both cases
       if (MODE == MODE_AA_ODD && HAS_SOLID && near_wall) collide(std::integral_constant<bool, HAS_SOLID>{});
       else collide(std::false_type{});
+      } else {
+        // ---- Shan-Chen model: Eq. 5-10 of the paper.  Accelerations
+        // a^k = F^k / rho^k = -G_C sum_i w_i rho^kbar(x + c_i) c_i + g (never divides by rho^k),
+        // common bare velocity u = m / rho, each component relaxes to f^eq(rho^k, u) and receives
+        // S^k_q = f^eq_q(rho^k, u + a^k) - f^eq_q(rho^k, u)
+        //       = w_q rho^k [(cv - cu)(3 + 4.5 (cv + cu)) - 1.5 (v.v - u.u)],  v = u + a^k.
+        float arx = -p.G_C * Gx, ary = -p.G_C * Gy, arz = -p.G_C * Gz;
+        float abx = -p.G_C * Hx, aby = -p.G_C * Hy, abz = -p.G_C * Hz;
+        if constexpr (HAS_G) { arx += p.gx; ary += p.gy; arz += p.gz; abx += p.gx; aby += p.gy; abz += p.gz; }
+        const float ux = mx * inv_rho, uy = my * inv_rho, uz = mz * inv_rho;
+        float omega = omega_same;
+        if (p.two_tau) {
+          const float inv_nu = (rr * inv_rho) / nu_r + (rb * inv_rho) / nu_b;
+          omega = 1.0f / (3.0f / inv_nu + 0.5f);
+        }
+        const float om1 = 1.0f - omega;
+        const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
+        const float vrx = ux + arx, vry = uy + ary, vrz = uz + arz;
+        const float vbx = ux + abx, vby = uy + aby, vbz = uz + abz;
+        const float dr15 = 1.5f * (vrx * vrx + vry * vry + vrz * vrz) - uu15;
+        const float db15 = 1.5f * (vbx * vbx + vby * vby + vbz * vbz) - uu15;
+        const float wr[3] = {wq(0) * rr, wq(1) * rr, wq(7) * rr};
+        const float wb[3] = {wq(0) * rb, wq(1) * rb, wq(7) * rb};
+        const float owd[3] = {omega * wq(0) * dr, omega * wq(1) * dr, omega * wq(7) * dr};
+        const float owr[3] = {omega * wq(0) * rho, omega * wq(1) * rho, omega * wq(7) * rho};
+        float racc = 0.f, tacc = 0.f;
+        auto collide = [&](auto bounce) {
+        static_for<1, Q + 1>([&](auto qc) {
+          constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
+          constexpr int k = q == 0 ? 0 : (q < 7 ? 1 : 2);
+          constexpr float w = wq(q);
+          float ts, rs;
+          if constexpr (q > 0) {
+            const float cu = cdot<q>(ux, uy, uz);
+            const float e = fmaf(cu, fmaf(4.5f, cu, 3.0f), -uu15);          // f^eq / (w rho) - 1
+            const float cvr = cdot<q>(vrx, vry, vrz), cvb = cdot<q>(vbx, vby, vbz);
+            const float sr = fmaf(cvr - cu, fmaf(4.5f, cvr + cu, 3.0f), -dr15);
+            const float sb = fmaf(cvb - cu, fmaf(4.5f, cvb + cu, 3.0f), -db15);
+            rs = fmaf(om1, R[q], wr[k] * fmaf(omega, 1.0f + e, sr));
+            ts = fmaf(om1, T[q], fmaf(owr[k], e, owd[k])) + fmaf(wr[k], sr, wb[k] * sb);
+            racc += rs;
+            tacc += ts;
+          } else {                       // the rest populations take what is left (mass is conserved)
+            ts = dr - tacc;
+            rs = rr - racc;
+          }
+          const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
+          *reinterpret_cast<float2*>(dst_ptr(p, s)) = make_float2(ts, rs);
+          vd[q] = (2.0f * rs - w) - ts;
+          vt[q] = ts;
+        });
+        };
+        if (MODE == MODE_AA_ODD && HAS_SOLID && near_wall) collide(std::integral_constant<bool, HAS_SOLID>{});
+        else collide(std::false_type{});
+      }
       if (HAS_SOLID && near_wall) {   // link bounce-back: what would enter a solid site comes back here
         float sd = 0.f, st = 0.f;
         static_for<1, Q>([&](auto qc) {
@@ -640,7 +736,7 @@ __global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const _
 // another brick are gathered from the populations k_fused stored, with the read rule of the NEXT
 // step (template MODE).  A solid source contributes nothing here: its link bounced back inside
 // k_fused.  Interior sites read 8 bytes.  Writes phi with its periodic ghost images like k_phase.
-template <int MODE, bool HAS_SOLID>
+template <int MODE, bool HAS_SOLID, bool SC>
 __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
   // Four consecutive x sites per thread (128-bit loads and stores).  CTA = 32 quads x TY rows of
   // one plane (four k_fused tiles side by side), so that a warp is one row: the rows on a brick
@@ -725,16 +821,25 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
       }
     });
   }
-  float phi[4];
-#pragma unroll
-  for (int e = 0; e < 4; ++e) phi[e] = solid[e] ? PHI_SOLID : d[e] / (1.0f + t[e]);
   if (x >= H && x + 4 <= b.nx - H && y >= H && y < b.ny - H && z >= H && z < b.nz - H) {   // no ghost image
+    float f0[4], f1[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const float rho = 1.0f + t[e];
+      if constexpr (!SC) {
+        f0[e] = solid[e] ? PHI_SOLID : d[e] / rho;
+      } else {
+        f0[e] = solid[e] ? PHI_SOLID : 0.5f * (rho + d[e]);
+        f1[e] = solid[e] ? 0.f : 0.5f * (rho - d[e]);
+      }
+    }
     const size_t px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
-    *reinterpret_cast<float4*>(p.phi + (size_t)(x + HALO) + px * ((size_t)(y + HALO) + py * (size_t)(z + HALO))) =
-        make_float4(phi[0], phi[1], phi[2], phi[3]);
+    const size_t o = (size_t)(x + HALO) + px * ((size_t)(y + HALO) + py * (size_t)(z + HALO));
+    *reinterpret_cast<float4*>(p.phi + o) = make_float4(f0[0], f0[1], f0[2], f0[3]);
+    if constexpr (SC) *reinterpret_cast<float4*>(p.phi2 + o) = make_float4(f1[0], f1[1], f1[2], f1[3]);
   } else {
 #pragma unroll
-    for (int e = 0; e < 4; ++e) store_phi_with_images(p, x + e, y, z, H, phi[e]);
+    for (int e = 0; e < 4; ++e) store_fields<SC>(p, x + e, y, z, H, solid[e], d[e], 1.0f + t[e]);
   }
 }
 
@@ -815,7 +920,10 @@ struct IoParams {
   float* out0;           // k_gatherf / k_macros outputs
   float* out1;
   float* out2;
-  const float* phi;      // padded phi (k_macros)
+  const float* phi;      // padded phi (k_macros); rho_r in the Shan-Chen model
+  const float* phi2;     // Shan-Chen model: padded rho_b
+  int sc;                // Shan-Chen model
+  float G_C;
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
 };
 
@@ -919,7 +1027,22 @@ __global__ void k_macros(const IoParams p) {
     if (!p.two) rr = rho;
     rb = p.two ? rho - rr : 0.f;
     float Fx = rho * p.gx, Fy = rho * p.gy, Fz = rho * p.gz;
-    if (p.two && p.A_nc != 0.f) {
+    if (p.sc) {
+      // Shan-Chen (Eq. 10; G27): F = rho_r a^r + rho_b a^b, g included
+      const size_t o0 = phi_index(b, x, y, z);
+      const long long px = b.nx + 2 * HALO, pxy = px * (b.ny + 2 * HALO);
+      const float r0 = p.phi[o0], b0 = p.phi2[o0];
+      float Sbx = 0.f, Sby = 0.f, Sbz = 0.f, Srx = 0.f, Sry = 0.f, Srz = 0.f;
+      for (int q = 1; q < Q; ++q) {
+        const long long d = c_cx[q] + px * c_cy[q] + pxy * c_cz[q];
+        float vr = p.phi[o0 + d], vb = p.phi2[o0 + d];
+        if (vr > PHI_SOLID_TEST) { vr = r0; vb = b0; }
+        const float k = wq(q);
+        Sbx += k * c_cx[q] * vb; Sby += k * c_cy[q] * vb; Sbz += k * c_cz[q] * vb;
+        Srx += k * c_cx[q] * vr; Sry += k * c_cy[q] * vr; Srz += k * c_cz[q] * vr;
+      }
+      Fx += -p.G_C * (rr * Sbx + rb * Srx); Fy += -p.G_C * (rr * Sby + rb * Sry); Fz += -p.G_C * (rr * Sbz + rb * Srz);
+    } else if (p.two && p.A_nc != 0.f) {
       const float* ph = p.phi + phi_index(b, x, y, z);
       const long long px = b.nx + 2 * HALO, pxy = px * (b.ny + 2 * HALO);
       const float phi0 = ph[0];
@@ -955,13 +1078,19 @@ __global__ void k_macros(const IoParams p) {
   if (p.out2) { p.out2[s] = ux; p.out2[b.S + s] = uy; p.out2[2 * b.S + s] = uz; }
 }
 
-// phi without ghost layers or sentinels, for lb_get_phi
-__global__ void k_unpad_phi(const float* phi, float* out, Box b) {
+// phi without ghost layers or sentinels, for lb_get_phi (Shan-Chen: from the rho_r, rho_b arrays)
+__global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box b) {
   const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= b.S) return;
   const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
   const float v = phi[phi_index(b, x, y, z)];
-  out[s] = v > PHI_SOLID_TEST ? 0.f : v;
+  if (v > PHI_SOLID_TEST) { out[s] = 0.f; return; }
+  if (phi2) {
+    const float w = phi2[phi_index(b, x, y, z)];
+    out[s] = (v - w) / (v + w);
+  } else {
+    out[s] = v;
+  }
 }
 
 // bytes [S] -> bit-packed words

@@ -18,7 +18,7 @@ LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 
 SYMBOLS = [
     "lb_set_allocator", "lb_create", "lb_destroy", "lb_set_stream", "lb_set_geometry",
-    "lb_set_body_force", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_storage", "lb_init", "lb_step",
+    "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_storage", "lb_init", "lb_step",
     "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
 ]
@@ -48,6 +48,7 @@ def _load():
     lib.lb_set_stream.argtypes = [vp, vp]
     lib.lb_set_geometry.argtypes = [vp, fp]
     lib.lb_set_body_force.argtypes = [vp, C.c_float, C.c_float, C.c_float]
+    lib.lb_set_model.argtypes = [vp, C.c_int, C.c_float]
     lib.lb_set_forcing.argtypes = [vp, C.c_int]
     lib.lb_set_nc_cutoff.argtypes = [vp, C.c_float]
     lib.lb_set_storage.argtypes = [vp, C.c_int]
@@ -161,6 +162,9 @@ class LB:
 
     def set_body_force(self, gx, gy, gz):
         self._ck(lib.lb_set_body_force(self.h, gx, gy, gz))
+
+    def set_model(self, model, G_C=0.0):
+        self._ck(lib.lb_set_model(self.h, {"cg": 0, "sc": 1}.get(model, model), float(G_C)))
 
     def set_forcing(self, mode):
         self._ck(lib.lb_set_forcing(self.h, {"guo": 0, "edm": 1}.get(mode, mode)))
