@@ -341,7 +341,7 @@ struct FusedSmem {
 // grad phi, each component gets the exact-difference source of Eq. 9, and there is no perturbation,
 // recolouring or near-contact force (HAS_NC = false; FMODE bit 0 only).
 template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE, bool SC = false>
-__global__ void __launch_bounds__(TX* TY, 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap,
+__global__ void __launch_bounds__(TX* TY, (MODE == MODE_AA_ODD && SC) ? 2 : 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap,
                                                      const __grid_constant__ CUtensorMap tmap2) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
   constexpr bool HAS_G = (FMODE & 1) != 0, EDM = (FMODE & 2) != 0;
