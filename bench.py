@@ -317,7 +317,7 @@ def run_ours(args):
     k2_s = ms_k2 * 1e-3            # mean k_fused / k_single launch over the sampled steps of the timed region
     achieved = upd_bytes * w.fluid_sites / k2_s / 1e9
     roofline = {"bound": "hbm", "kernel": "k_fused" if two else "k_single", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic("k_fused" if two else "k_single", args.workload, args.storage),
+                "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic(("k_fused(sc)" if MODEL[0] == "sc" else "k_fused") if two else "k_single", args.workload, args.storage),
                 "peak_source": peak_src, "algorithmic_bytes_per_update": upd_bytes,
                 "kernel_ms": ms_k2, "kernel_share_of_step": ms_k2 * K / ms,
                 "phase_kernel_ms": ms_k1, "kernel_timing": "CUDA events around every 7th step of the timed region",
