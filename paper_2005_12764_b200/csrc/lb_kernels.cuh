@@ -768,9 +768,14 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
   if (xm) { const float2 v = __ldg(ex + (tile == 0 ? ntx - 1 : tile - 1) * 2 + 1); d[0] += v.x; t[0] += v.y; }
   if (xp) { const float2 v = __ldg(ex + (tile == ntx - 1 ? 0 : tile + 1) * 2 + 0); d[3] += v.x; t[3] += v.y; }
   bool solid[4] = {false, false, false, false};
+  // solid bits of the quad's own sites: x % 4 == 0, so the four bits sit in one mask word
+  auto quad_bits = [&](int yy, int zz) -> uint32_t {
+    return (b.mask[(size_t)(zz * b.ny + yy) * b.nxw + (x >> 5)] >> (x & 31)) & 0xfu;
+  };
   if constexpr (HAS_SOLID) {
+    const uint32_t m = quad_bits(y, z);
 #pragma unroll
-    for (int e = 0; e < 4; ++e) solid[e] = solid_at(b, x + e, y, z);
+    for (int e = 0; e < 4; ++e) solid[e] = (m >> e) & 1u;
   }
   if (ym || yp || zm || zp) {
     // sources in another row range or z chunk are gathered from the stored populations with the
@@ -803,16 +808,20 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
             rq[e] = v.y;
           }
         }
+        // is the site a population comes from (x + e - c_q) solid?  One mask word for the quad of
+        // the source row, plus the one site beyond its end when c_x != 0
+        uint32_t sm = 0;
+        if constexpr (HAS_SOLID) {
+          const int yq = cy(q) > 0 ? wrap_m(y, b.ny) : (cy(q) < 0 ? wrap_p(y, b.ny) : y);
+          const int zq = cz(q) > 0 ? wrap_m(z, b.nz) : (cz(q) < 0 ? wrap_p(z, b.nz) : z);
+          const uint32_t m = quad_bits(yq, zq);
+          if constexpr (cx(q) == 0) sm = m;
+          else if constexpr (cx(q) > 0) sm = (m << 1) | (solid_at(b, x == 0 ? b.nx - 1 : x - 1, yq, zq) ? 1u : 0u);
+          else sm = (m >> 1) | (solid_at(b, x + 4 >= b.nx ? 0 : x + 4, yq, zq) ? 8u : 0u);
+        }
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-          bool use = true;
-          if constexpr (HAS_SOLID) {     // is the site this population comes from solid?
-            int xs = x + e - cx(q);
-            xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
-            const int yq = cy(q) > 0 ? wrap_m(y, b.ny) : (cy(q) < 0 ? wrap_p(y, b.ny) : y);
-            const int zq = cz(q) > 0 ? wrap_m(z, b.nz) : (cz(q) < 0 ? wrap_p(z, b.nz) : z);
-            use = !solid_at(b, xs, yq, zq);
-          }
+          const bool use = !((sm >> e) & 1u);
           if (use) {
             d[e] += (2.0f * rq[e] - wq(q)) - tq[e];
             t[e] += tq[e];
