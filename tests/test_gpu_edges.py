@@ -376,3 +376,69 @@ def test_exact_difference_poiseuille_single_component(lbmod, lbo):
     errs, (rr, _, u), _ = pu.macro_errors(sim, o)
     assert errs["u"] < 1e-7 and errs["rho_r"] < 1e-5, errs
     assert u[0].max() > 1e-4
+
+
+# ------------------------------------------------------------------------------- handle life cycle
+def test_handles_are_independent_and_reusable(lbmod, lbo):
+    """Two handles of different boxes and models stepping alternately; re-init of a handle (also
+    with a different component count); create/destroy cycles return the device memory."""
+    import torch
+    lb = lbmod
+    w1 = _random_workload(36, 13, 7, seed=3, walls=True)
+    w2 = _random_workload(40, 12, 10, seed=4, walls=False, A_nc=0.0)
+    o1, s1 = pu.make_oracle(lbo, w1), pu.make_gpu(lb, w1, "aa")
+    o2 = lbo.Oracle(w2.nx, w2.ny, w2.nz, *w2.params); o2.set_model("sc", 1.5); o2.set_body_force(*w2.g); o2.init(w2.rho_r, w2.rho_b, w2.u)
+    s2 = lb.LB(w2.nx, w2.ny, w2.nz, *w2.params); s2.set_model("sc", 1.5); s2.set_body_force(*w2.g)
+    s2.init(w2.rho_r, w2.rho_b, w2.u)
+    risky = np.zeros(w1.shape, bool)
+    fluid = w1.solid == 0
+    for _ in range(3):
+        risky = pu.dilate(risky, 1) | pu.dilate((o1.get_fields()["margin"] < 1e-5) & fluid, 1)
+        s1.step(1); s2.step(1); o1.step(1); o2.step(1)
+    assert pu.pop_error(s1, o1)[~risky].max() < pu.POP_TOL
+    assert pu.pop_error(s2, o2).max() < pu.POP_TOL
+    # re-init the same handle: two components again, then a single component, then two again
+    s2.init(w2.rho_r, w2.rho_b, w2.u)
+    o2.init(w2.rho_r, w2.rho_b, w2.u)
+    s2.step(2); o2.step(2)
+    assert pu.pop_error(s2, o2).max() < pu.POP_TOL
+    s3 = lb.LB(w2.nx, w2.ny, w2.nz, 0.8, 0.8)
+    s3.init(w2.rho_r + w2.rho_b, None, w2.u)
+    s3.step(2)
+    s3.init(w2.rho_r, w2.rho_b, w2.u)
+    o3 = lbo.Oracle(w2.nx, w2.ny, w2.nz, 0.8, 0.8); o3.init(w2.rho_r, w2.rho_b, w2.u)
+    s3.step(2); o3.step(2)
+    assert pu.pop_error(s3, o3).max() < pu.POP_TOL
+    # memory comes back
+    torch.cuda.synchronize()
+    for s in (s1, s2, s3):
+        s.destroy()
+    base = torch.cuda.memory_allocated()
+    for _ in range(5):
+        s = pu.make_gpu(lb, w1)
+        s.step(1)
+        s.destroy()
+    torch.cuda.synchronize()
+    assert torch.cuda.memory_allocated() == base
+
+
+def test_set_populations_then_forwarded_steps(lbmod, lbo):
+    """After lb_set_populations the forwarded phi is stale: the next step must take the full
+    phase-field sweep, the ones after it the forwarded path, in both models."""
+    w = _random_workload(36, 9, 6, seed=9, walls=True)
+    for model in ("cg", "sc"):
+        o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params); o.set_model(model, 1.4); o.set_geometry(w.solid); o.init(w.rho_r, w.rho_b, w.u)
+        o.step(3)
+        fr, fb = o.get_populations(0).astype(np.float32), o.get_populations(1).astype(np.float32)
+        o2 = lbo.Oracle(w.nx, w.ny, w.nz, *w.params); o2.set_model(model, 1.4); o2.set_geometry(w.solid); o2.init(w.rho_r, w.rho_b, w.u)
+        o2.set_populations(0, fr); o2.set_populations(1, fb)
+        sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params); sim.set_model(model, 1.4)
+        sim.set_geometry(np.ascontiguousarray(w.solid, dtype=np.uint8))
+        sim.init(w.rho_r, w.rho_b, w.u)
+        sim.step(2)
+        sim.set_populations(0, fr); sim.set_populations(1, fb)
+        risky = np.zeros(w.shape, bool)
+        for n in range(3):
+            risky = pu.dilate(risky, 1) | pu.dilate((o2.get_fields()["margin"] < 1e-5) & (w.solid == 0), 1)
+            sim.step(1); o2.step(1)
+            assert pu.pop_error(sim, o2)[~risky].max() < pu.POP_TOL, (model, n)
