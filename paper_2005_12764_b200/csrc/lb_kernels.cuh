@@ -798,14 +798,14 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
           const float4 r = __ldg(reinterpret_cast<const float4*>(pl + x + 2));
           tq[0] = a.x; rq[0] = a.y; tq[1] = a.z; rq[1] = a.w;
           tq[2] = r.x; rq[2] = r.y; tq[3] = r.z; rq[3] = r.w;
-        } else {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            int xs = x + e - sx;
-            xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
-            const float2 v = __ldg(pl + xs);
-            tq[e] = v.x;
-            rq[e] = v.y;
+        } else {      // sources x - 1 .. x + 2 or x + 1 .. x + 4: the aligned quad plus one site beyond its end
+          const float4 a = __ldg(reinterpret_cast<const float4*>(pl + x));
+          const float4 r = __ldg(reinterpret_cast<const float4*>(pl + x + 2));
+          const float2 ext = __ldg(pl + (sx > 0 ? (x == 0 ? b.nx - 1 : x - 1) : (x + 4 >= b.nx ? 0 : x + 4)));
+          if constexpr (sx > 0) {
+            tq[0] = ext.x; rq[0] = ext.y; tq[1] = a.x; rq[1] = a.y; tq[2] = a.z; rq[2] = a.w; tq[3] = r.x; rq[3] = r.y;
+          } else {
+            tq[0] = a.z; rq[0] = a.w; tq[1] = r.x; rq[1] = r.y; tq[2] = r.z; rq[2] = r.w; tq[3] = ext.x; rq[3] = ext.y;
           }
         }
         // is the site a population comes from (x + e - c_q) solid?  One mask word for the quad of
