@@ -442,3 +442,54 @@ def test_set_populations_then_forwarded_steps(lbmod, lbo):
             risky = pu.dilate(risky, 1) | pu.dilate((o2.get_fields()["margin"] < 1e-5) & (w.solid == 0), 1)
             sim.step(1); o2.step(1)
             assert pu.pop_error(sim, o2)[~risky].max() < pu.POP_TOL, (model, n)
+
+
+# ------------------------------------------------------------------------------- randomised configurations
+@pytest.mark.parametrize("seed", list(range(12)))
+def test_randomised_configurations(lbmod, lbo, seed):
+    """Random box shapes (incl. extents of 4 and long thin boxes) with random combinations of walls,
+    near contact, body force, equal / unequal taus, forcing, model, storage and brick size:
+    populations after 1 and 4 steps against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    nx = int(rng.choice([4, 8, 12, 36, 64, 100, 132]))
+    ny = int(rng.choice([4, 5, 8, 9, 16, 23]))
+    nz = int(rng.choice([4, 6, 11, 16, 33]))
+    if nx * ny * nz > 60000:
+        nz = 4
+    walls = bool(rng.integers(2))
+    model = "sc" if rng.integers(3) == 0 else "cg"
+    A_nc = 0.0 if (model == "sc" or rng.integers(2)) else 0.02
+    tau = (0.8, 1.2) if rng.integers(2) else (1.0, 1.0)
+    g = (1e-4, -5e-5, 2e-5) if rng.integers(2) else (0.0, 0.0, 0.0)
+    forcing = "edm" if rng.integers(2) else "guo"
+    storage = "aa" if rng.integers(2) else "ab"
+    zc = int(rng.choice([0, 1, 2, 5]))
+    w = _random_workload(nx, ny, nz, seed=2000 + seed, walls=walls, A_nc=A_nc, tau=tau, g=g)
+    if walls and (ny < 5 or nz < 5 or nx < 8):
+        w.solid[:] = 0
+        w.solid[0, :, :] = 1                    # one wall plane is all a tiny box has room for
+    fluid = w.solid == 0 if w.solid is not None else np.ones(w.shape, bool)
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    sim.set_storage(storage)
+    if model == "sc":
+        o.set_model("sc", 1.5); sim.set_model("sc", 1.5)
+    else:
+        o.set_forcing(forcing); sim.set_forcing(forcing)
+    if w.solid is not None:
+        o.set_geometry(w.solid); sim.set_geometry(np.ascontiguousarray(w.solid, dtype=np.uint8))
+    o.set_body_force(*g); sim.set_body_force(*g)
+    o.init(w.rho_r, w.rho_b, w.u); sim.init(w.rho_r, w.rho_b, w.u)
+    sim.set_tuning(zc=zc)
+    tag = dict(shape=(nx, ny, nz), walls=walls, model=model, A_nc=A_nc, tau=tau, g=g, forcing=forcing, storage=storage, zc=zc)
+    risky = np.zeros(w.shape, bool)
+    for n in range(1, 5):
+        risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+        o.step(1); sim.step(1)
+        if n in (1, 4):
+            e = pu.pop_error(sim, o)
+            ok = ~risky & fluid
+            if ok.any():
+                assert e[ok].max() < pu.POP_TOL, (tag, n, e[ok].max())
+    rr, rb, u = sim.get_macros()
+    assert np.isfinite(u).all(), tag
