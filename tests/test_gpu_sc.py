@@ -106,3 +106,45 @@ def test_sc_errors(lbmod):
     with pytest.raises(lb.LBError) as ei:
         sim.set_model("cg")
     assert ei.value.code == lb.LB_ESTATE
+
+
+def test_sc_full_size_sampled_blocks_and_conservation(lbmod, lbo):
+    """The configuration bench.py --model sc times (C3 at 256^3, G_C = 3): one step checked on
+    sampled 28^3 blocks against the oracle run on a cut-out of the input, then 200 more steps:
+    finite, masses conserved, zero net momentum, the mixture has started to separate."""
+    w = W.get("c3")
+    _, sim = None, lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    sim.set_model("sc", 3.0)
+    sim.init(np.ascontiguousarray(w.rho_r), np.ascontiguousarray(w.rho_b), np.ascontiguousarray(w.u))
+    sim.step(1)
+    f = [sim.get_populations(k) for k in (0, 1)]
+    rng = np.random.default_rng(19)
+    centres = [(0, 0, 0), (w.nx - 1, w.ny // 2, w.nz - 1)] + \
+        [tuple(int(v) for v in rng.integers(0, [w.nx, w.ny, w.nz])) for _ in range(4)]
+    half, margin = 14, 3
+    n = 2 * half
+    worst = 0.0
+    for (cx, cy, cz) in centres:
+        ix = np.arange(cx - half, cx + half) % w.nx
+        iy = np.arange(cy - half, cy + half) % w.ny
+        iz = np.arange(cz - half, cz + half) % w.nz
+        sel = np.ix_(iz, iy, ix)
+        o = lbo.Oracle(n, n, n, *w.params)
+        o.set_model("sc", 3.0)
+        o.init(w.rho_r[sel], w.rho_b[sel], w.u[(slice(None),) + sel])
+        o.step(1)
+        inner = np.zeros((n, n, n), bool)
+        inner[margin:-margin, margin:-margin, margin:-margin] = True
+        for k in (0, 1):
+            e = np.abs(f[k][(slice(None),) + sel].astype(np.float64) - o.get_populations(k)) / pu.W19[:, None, None, None]
+            worst = max(worst, e[:, inner].max())
+    assert worst < pu.POP_TOL, worst
+    del f
+    sim.step(200)
+    rr, rb, u = sim.get_macros()
+    assert np.isfinite(u).all()
+    m0, m1 = pu.masses(w.rho_r, w.rho_b), pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
+    mom = np.abs([(u[a].astype(np.float64) * (rr + rb)).sum() for a in range(3)]).max() / w.sites
+    assert mom < 1e-5
+    assert np.std((rr - rb) / (rr + rb)) > 3 * np.std((w.rho_r - w.rho_b) / (w.rho_r + w.rho_b))
