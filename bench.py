@@ -125,6 +125,9 @@ def config_of(w, storage, extra=None):
          "walls": w.solid is not None, "storage": storage, "model": "colour-gradient" if MODEL[0] == "cg" else "shan-chen G_C=%g" % MODEL[1],
          "params": dict(tau_r=w.tau_r, tau_b=w.tau_b, A=w.A, beta=w.beta, A_nc=w.A_nc, g=list(w.g)),
          "l2": "state (%.2f GB) is larger than L2, no flush needed" % (w.sites * 4 * (38 if w.rho_b is not None else 19) * (2 if storage == "ab" else 1) / 1e9)}
+    if w.rho_b is not None and w.A_nc != 0.0 and w.A > 0.0:
+        # N_c = A dx / sigma with sigma = (4/9) A tau of the colour-gradient perturbation (G5)
+        c["N_c"] = w.A_nc / ((4.0 / 9.0) * w.A * w.tau_r)
     c.update(w.info)
     if extra:
         c.update(extra)
