@@ -1,10 +1,12 @@
 #!/usr/bin/env python
 """bench.py -- GLUPS of the two-component colour-gradient D3Q19 hot path on B200.
 
-One "step" is one LB time step of the whole box: the phase-field kernel K1 plus the fused
-stream-collide kernel K2 (every row A0-A10 of the hot path).  Prints ONE JSON line.
+One "step" is one LB time step of the whole box: the fused stream-collide kernel k_fused (which
+also forwards the moments of the next state) plus the phase-field kernel k_phase_fwd, i.e. every
+row A0-A10 of the hot path.  Prints ONE JSON line.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c5|c4|c2|c1] [--storage ab|aa]
+                  [--model cg|sc] [--windows N]
   python bench.py --impl reference ...     # the fp64 CPU oracle on this box's host cores
 
 N > 1 (torchrun): the path does not shard in this build ("replicas only"): every
@@ -245,17 +247,25 @@ def run_ours(args):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    l0 = sim.launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
-        torch.cuda.synchronize()
-        ev0.record()
-        sim.step(K)
-        ev1.record()
-        torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    launches = sim.launch_count() - l0
+    # a run that saw a hardware or thermal slowdown is rejected and measured again, once
+    BAD = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+    remeasured = False
+    for attempt in range(2):
+        l0 = sim.launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(local_rank) as clk:
+            torch.cuda.synchronize()
+            ev0.record()
+            sim.step(K)
+            ev1.record()
+            torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        launches = sim.launch_count() - l0
+        if world > 1 or not (BAD & set(clk.result.get("reasons", []))):
+            break
+        remeasured = True
+        time.sleep(5.0)
     ms = ev0.elapsed_time(ev1)
     ms_k2 = sim.last_step_ms(1)
     ms_k1 = sim.last_step_ms(2) if two else 0.0
@@ -329,7 +339,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": "GLUPS", "n_gpus": world, "steps": K, "warmup": Wu,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": config_of(w, args.storage, {"parallelism": "replicas x%d" % world}),
-            "clocks": clk.result, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "clocks": dict(clk.result, remeasured=remeasured), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "checks": {"finite": finite, "red_mass_rel_drift": abs(mass - mass0) / mass0}}
     if windows is not None:
         line["windows"] = windows
