@@ -72,7 +72,8 @@ struct Oracle {
   bool two = true;
   bool inited = false;
   bool any_solid = false;
-  std::vector<uint8_t> solid;            // S, 1 = solid
+  std::vector<uint8_t> solid;            // S, 0 = fluid, 1 = wall at rest, 2 / 3 = walls moving with uw[2] / uw[3]
+  double uw[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // wall velocities by group (G28)
   std::vector<double> f[2], fpost[2];    // [k][site*19 + i], pre- and post-collision
   std::vector<double> rho_r, rho_b, phi; // per site (S1)
   std::vector<double> mx, my, mz;        // bare momentum (S1)
@@ -278,8 +279,19 @@ void stream(Oracle& o) {
         if (o.solid[s]) continue;
         for (int i = 0; i < Q; ++i) {
           size_t n = o.nbr(x, y, z, -CX[i], -CY[i], -CZ[i]);
-          for (int k = 0; k < nk; ++k)
-            o.f[k][s * Q + i] = o.solid[n] ? o.fpost[k][s * Q + OPP[i]] : o.fpost[k][n * Q + i];
+          for (int k = 0; k < nk; ++k) {
+            if (!o.solid[n]) {
+              o.f[k][s * Q + i] = o.fpost[k][n * Q + i];
+            } else {
+              // half-way bounce-back at a wall moving with u_w ("solid walls with opposite speeds
+              // +-U"; rule: reading G28): the reflected population gains
+              // 2 w_i rho^k (c_i . u_w) / c_s^2 = 6 w_i rho^k (c_i . u_w), rho^k the site's density
+              const double* uw = o.uw[o.solid[n]];
+              const double cu = CX[i] * uw[0] + CY[i] * uw[1] + CZ[i] * uw[2];
+              const double rk = k == 0 ? o.rho_r[s] : o.rho_b[s];
+              o.f[k][s * Q + i] = o.fpost[k][s * Q + OPP[i]] + 6.0 * W[i] * rk * cu;
+            }
+          }
         }
       }
 }
@@ -421,9 +433,17 @@ int lbo_set_geometry(void* h, const uint8_t* mask) {
   if (o->inited) return LBO_ESTATE;
   o->any_solid = false;
   for (size_t s = 0; s < o->S; ++s) {
-    o->solid[s] = mask ? (mask[s] != 0) : 0;
+    o->solid[s] = mask ? (mask[s] > 3 ? 1 : mask[s]) : 0;   // 0 fluid, 1 wall at rest, 2 / 3 moving wall groups
     o->any_solid |= o->solid[s] != 0;
   }
+  return LBO_OK;
+}
+
+// velocity of the walls whose mask value is `group` (2 or 3); walls with mask value 1 are at rest
+int lbo_set_wall_velocity(void* h, int group, double ux, double uy, double uz) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (group != 2 && group != 3)) return LBO_EINVAL;
+  o->uw[group][0] = ux; o->uw[group][1] = uy; o->uw[group][2] = uz;
   return LBO_OK;
 }
 

@@ -37,6 +37,7 @@ def _load():
         lib.lbo_destroy.restype = None
         lib.lbo_set_geometry.argtypes = [vp, u8p]
         lib.lbo_set_body_force.argtypes = [vp, C.c_double, C.c_double, C.c_double]
+        lib.lbo_set_wall_velocity.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double]
         lib.lbo_set_nc_cutoff.argtypes = [vp, C.c_double]
         lib.lbo_set_nc_mode.argtypes = [vp, C.c_int]
         lib.lbo_set_forcing.argtypes = [vp, C.c_int]
@@ -105,6 +106,10 @@ class Oracle:
             return
         m = np.ascontiguousarray(mask, dtype=np.uint8).reshape(self.shape)
         self._ck(self.lib.lbo_set_geometry(self.h, m.ctypes.data_as(C.POINTER(C.c_uint8))), "lbo_set_geometry")
+
+    def set_wall_velocity(self, group, ux, uy, uz):
+        """Velocity of the walls whose mask value is `group` (2 or 3)."""
+        self._ck(self.lib.lbo_set_wall_velocity(self.h, group, ux, uy, uz), "lbo_set_wall_velocity")
 
     def set_body_force(self, gx, gy, gz):
         self._ck(self.lib.lbo_set_body_force(self.h, gx, gy, gz), "lbo_set_body_force")

@@ -28,7 +28,7 @@ def half_away(v):
 
 
 def step(fr, fb, solid, tau_r, tau_b, A, beta, A_nc=0.0, g=(0.0, 0.0, 0.0), phi_c=0.9,
-         h_min=3, h_max=4, eps=1e-12, forcing="guo"):
+         h_min=3, h_max=4, eps=1e-12, forcing="guo", wall_group=None, wall_u=None):
     """One time step. fr, fb: [19, nz, ny, nx] pre-collision; solid: bool [nz, ny, nx]."""
     nz, ny, nx = solid.shape
     fluid = ~solid
@@ -101,10 +101,16 @@ def step(fr, fb, solid, tau_r, tau_b, A, beta, A_nc=0.0, g=(0.0, 0.0, 0.0), phi_
     for i in range(19):
         o = opposite(i)
         dest_solid = shift(solid, -C[i])          # is x + c_i solid?
-        for post, new in ((post_r, new_r), (post_b, new_b)):
+        for post, new, rk in ((post_r, new_r, rr), (post_b, new_b, rb)):
             go = np.where(fluid & ~dest_solid, post[i], 0.0)
             new[i] += shift(go, C[i])
-            new[o] += np.where(fluid & dest_solid, post[i], 0.0)
+            back = post[i]
+            if wall_group is not None:
+                # moving wall (G28): the reflected population loses 6 w_i rho^k (c_i . u_w)
+                grp = shift(wall_group, -C[i])            # group of the site x + c_i
+                cuw = sum(C[i, a] * np.asarray(wall_u)[grp, a] for a in range(3))
+                back = back - 6.0 * WT[i] * rk * cuw
+            new[o] += np.where(fluid & dest_solid, back, 0.0)
     new_r *= fluid
     new_b *= fluid
     return new_r, new_b
@@ -120,7 +126,7 @@ def equilibrium(rho, u):
     return np.stack(out)
 
 
-def step_sc(fr, fb, solid, tau_r, tau_b, G_C, g=(0.0, 0.0, 0.0)):
+def step_sc(fr, fb, solid, tau_r, tau_b, G_C, g=(0.0, 0.0, 0.0), wall_group=None, wall_u=None):
     """One time step of the paper's section 3.1 as printed: Eq. 5-6 with the exact-difference
     source of Eq. 9 and the Shan-Chen force of Eq. 10, repulsive for G_C > 0
     (G27).  Whole-array form, push streaming."""
@@ -157,10 +163,16 @@ def step_sc(fr, fb, solid, tau_r, tau_b, G_C, g=(0.0, 0.0, 0.0)):
     for i in range(19):
         o = opposite(i)
         dest_solid = shift(solid, -C[i])
-        for post, new in ((post_r, new_r), (post_b, new_b)):
+        for post, new, rk in ((post_r, new_r, rr), (post_b, new_b, rb)):
             go = np.where(fluid & ~dest_solid, post[i], 0.0)
             new[i] += shift(go, C[i])
-            new[o] += np.where(fluid & dest_solid, post[i], 0.0)
+            back = post[i]
+            if wall_group is not None:
+                # moving wall (G28): the reflected population loses 6 w_i rho^k (c_i . u_w)
+                grp = shift(wall_group, -C[i])            # group of the site x + c_i
+                cuw = sum(C[i, a] * np.asarray(wall_u)[grp, a] for a in range(3))
+                back = back - 6.0 * WT[i] * rk * cuw
+            new[o] += np.where(fluid & dest_solid, back, 0.0)
     new_r *= fluid
     new_b *= fluid
     return new_r, new_b

@@ -355,6 +355,15 @@ def test_P12_brute_force_numpy_twin(lbo, shape, walls, forcing):
     o.set_geometry(solid)
     o.set_body_force(*g)
     o.set_forcing(forcing)
+    wall_group, wall_u = None, None
+    if walls:       # the wall plane slides and pushes, the single solid node moves the other way
+        wall_group = np.zeros((nz, ny, nx), int)
+        wall_group[:, 0, :] = 2
+        wall_group[1, 2, 3] = 3
+        wall_u = np.array([[0, 0, 0], [0, 0, 0], [0.01, 0.002, -0.003], [-0.004, 0.0, 0.006]])
+        o.set_geometry(wall_group.astype(np.uint8))
+        o.set_wall_velocity(2, *wall_u[2])
+        o.set_wall_velocity(3, *wall_u[3])
     o.init(rho_r, rho_b, u)
     fr = tw.equilibrium(rho_r, u) * ~solid
     fb = tw.equilibrium(rho_b, u) * ~solid
@@ -362,7 +371,7 @@ def test_P12_brute_force_numpy_twin(lbo, shape, walls, forcing):
     contacts = 0
     for _ in range(10):
         contacts += int((o.get_fields()["h"] > 0).sum())
-        fr, fb = tw.step(fr, fb, solid, g=g, forcing=forcing, **par)
+        fr, fb = tw.step(fr, fb, solid, g=g, forcing=forcing, wall_group=wall_group, wall_u=wall_u, **par)
         o.step(1)
         assert np.abs(o.get_populations(0) - fr).max() < 1e-13
         assert np.abs(o.get_populations(1) - fb).max() < 1e-13
@@ -410,3 +419,37 @@ def test_P14_exact_difference_source_moments(lbo):
         assert np.abs(mom - (t * F)[:, None, None, None]).max() < 1e-15   # momentum grows by F per step
         _, _, u = o.get_macros()
         assert np.abs(u - ((t + 0.5) * F)[:, None, None, None]).max() < 1e-15   # half-step velocity
+
+
+# ---------------------------------------------------------------------------------- P15
+def _couette(o_factory, ny=34, steps=30000, U=0.01):
+    nx, nz = 4, 4
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 2
+    solid[:, -1, :] = 3
+    return o_factory(nx, ny, nz, solid, (-U, 0.0, 0.0), (U, 0.0, 0.0), steps)
+
+
+def test_P15_couette_between_sliding_walls(lbo):
+    """"solid walls with opposite speeds +-U = 0.01": half-way bounce-back
+    at moving walls (G28) gives the linear Couette profile u_x(y) = U (2 (y - 1/2)/H - 1) between
+    walls half a link outside the first and last fluid nodes (H = 32), exactly in the steady
+    state; single component and a uniform two-component mixture with unequal taus."""
+    def run(nx, ny, nz, solid, ulo, uhi, steps, two=False):
+        o = lbo.Oracle(nx, ny, nz, 0.9, 1.3 if two else 0.9, 0.0, 0.0, 0.0)
+        o.set_geometry(solid)
+        o.set_wall_velocity(2, *ulo)
+        o.set_wall_velocity(3, *uhi)
+        ones = np.ones((nz, ny, nx))
+        o.init(0.4 * ones if two else ones, 0.6 * ones if two else None, np.zeros((3, nz, ny, nx)))
+        o.step(steps)
+        return o.get_macros()
+    for two in (False, True):
+        rr, rb, u = _couette(lambda *a: run(*a, two=two))
+        y = np.arange(34)
+        exact = 0.01 * (2 * (y - 0.5) / 32.0 - 1.0)
+        prof = u[0][2, :, 1]
+        assert np.abs(prof[1:-1] - exact[1:-1]).max() < 2e-6, np.abs(prof[1:-1] - exact[1:-1]).max()
+        assert np.abs(u[1]).max() < 1e-12 and np.abs(u[2]).max() < 1e-12
+        rho = rr if rb is None else rr + rb
+        assert abs(rho[:, 1:-1, :].mean() - 1.0) < 1e-12          # tangential walls exchange no mass
