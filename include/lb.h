@@ -74,10 +74,15 @@ void lb_destroy(lb_handle h);
 /* CUDA stream (a cudaStream_t passed as void*) that all later work of this handle uses. */
 int lb_set_stream(lb_handle h, void* cuda_stream);
 
-/* Solid mask, S = nx*ny*nz bytes, 1 = solid, 0 = fluid; NULL = all fluid.  Stored bit-packed.
- * Solid sites hold no populations; links into them bounce back half-way (G21).
- * Must precede lb_init. */
+/* Solid mask, S = nx*ny*nz bytes: 0 = fluid, 1 = wall at rest, 2 and 3 = walls moving with the
+ * velocities of lb_set_wall_velocity (any other value counts as 1); NULL = all fluid.  Stored
+ * bit-packed.  Solid sites hold no populations; links into them bounce back half-way
+ * (G21).  Must precede lb_init. */
 int lb_set_geometry(lb_handle h, const uint8_t* solid_mask);
+
+/* Velocity u_w of the walls of group 2 or 3 ("solid walls with opposite speeds +-U", PAPER.md:341,
+ * :367; G28): a population reflected at such a wall along link i loses 6 w_i rho^k (c_i . u_w). */
+int lb_set_wall_velocity(lb_handle h, int group, float ux, float uy, float uz);
 
 /* Uniform acceleration g: body force F = rho g enters through the source term. */
 int lb_set_body_force(lb_handle h, float gx, float gy, float gz);

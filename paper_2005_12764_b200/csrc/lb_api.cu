@@ -63,6 +63,8 @@ struct lb_handle_s {
   bool two = true;
   bool inited = false;
   bool has_solid = false;
+  bool has_moving = false;   // the mask holds wall groups 2 / 3 (moving walls)
+  float uw[2][3] = {{0, 0, 0}, {0, 0, 0}};   // their velocities
   int aa_odd = 0;           // AA: is the next step the odd one?
   int cur = 0;              // A/B: buffer holding the current state
   float* buf[2] = {nullptr, nullptr};
@@ -93,6 +95,7 @@ struct lb_handle_s {
     b.nxw = (nx + 31) / 32;
     b.S = S;
     b.mask = has_solid ? mask : nullptr;
+    b.gmask = (has_solid && has_moving) ? mask + (size_t)b.nxw * ny * nz : nullptr;
     return b;
   }
   int planes() const { return two ? 2 * Q : Q; }
@@ -176,6 +179,8 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   p.two_tau = h->par.tau_r != h->par.tau_b;
   p.has_g = (h->g[0] != 0.f || h->g[1] != 0.f || h->g[2] != 0.f);
   p.edm = h->forcing;
+  p.has_moving = h->has_solid && h->has_moving;
+  for (int a = 0; a < 3; ++a) { p.uw2[a] = h->uw[0][a]; p.uw3[a] = h->uw[1][a]; }
   return p;
 }
 
@@ -223,56 +228,61 @@ void launch_phase(lb_handle h, const StepParams& p, dim3 grid) {
     else k_phase<MODE, false, false><<<grid, blk, 0, h->stream>>>(p);
   }
 }
-template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE>
+template <int MODE, int WALLS, bool HAS_NC, int FMODE>
 void launch_fused_t(lb_handle h, const StepParams& p, dim3 grid) {
   constexpr size_t smem = FusedSmem<HAS_NC ? H_MAX_NC : 1>::BYTES;
   static bool attr_set = false;   // per instantiation
   if (!attr_set) {
-    cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, HAS_NC, FMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_fused<MODE, WALLS, HAS_NC, FMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
-  k_fused<MODE, HAS_SOLID, HAS_NC, FMODE><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap);
+  k_fused<MODE, WALLS, HAS_NC, FMODE><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap);
 }
-template <int MODE, bool HAS_SOLID, bool HAS_NC>
+template <int MODE, int WALLS, bool HAS_NC>
 void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
   // The in-place (AA) instantiations without any force run 25 % slower than those that carry the
   // Guo term (measured at 256^3: 1.16 against 0.87 ms; the extra arithmetic spaces out the shifted
   // stores), and with g = 0 the term adds exactly zero, so AA always takes the force variant.
-  const bool g = p.has_g || (MODE != MODE_AB && !HAS_NC);
+  // moving walls (WALLS == 2, a rare configuration) are built for the force variants only
+  const bool g = p.has_g || (MODE != MODE_AB && !HAS_NC) || WALLS == 2;
   const bool edm = p.edm && (HAS_NC || p.has_g);    // no force, no source: nothing to choose
   if (edm) {
-    if (g) launch_fused_t<MODE, HAS_SOLID, HAS_NC, 3>(h, p, grid);
-    else if constexpr (HAS_NC) launch_fused_t<MODE, HAS_SOLID, HAS_NC, 2>(h, p, grid);
+    if (g) launch_fused_t<MODE, WALLS, HAS_NC, 3>(h, p, grid);
+    else if constexpr (HAS_NC && WALLS != 2) launch_fused_t<MODE, WALLS, HAS_NC, 2>(h, p, grid);
   } else {
-    if (g) launch_fused_t<MODE, HAS_SOLID, HAS_NC, 1>(h, p, grid);
-    else launch_fused_t<MODE, HAS_SOLID, HAS_NC, 0>(h, p, grid);
+    if (g) launch_fused_t<MODE, WALLS, HAS_NC, 1>(h, p, grid);
+    else if constexpr (WALLS != 2) launch_fused_t<MODE, WALLS, HAS_NC, 0>(h, p, grid);
   }
 }
-template <int MODE, bool HAS_SOLID, int FMODE>
+template <int MODE, int WALLS, int FMODE>
 void launch_fused_sc(lb_handle h, const StepParams& p, dim3 grid) {
   constexpr size_t smem = FusedSmem<1, true>::BYTES;
   static bool attr_set = false;   // per instantiation
   if (!attr_set) {
-    cudaFuncSetAttribute(k_fused<MODE, HAS_SOLID, false, FMODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_fused<MODE, WALLS, false, FMODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
-  k_fused<MODE, HAS_SOLID, false, FMODE, true><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap2);
+  k_fused<MODE, WALLS, false, FMODE, true><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap2);
 }
 template <int MODE>
 void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
   if (h->model == 1) {      // Shan-Chen: no near contact; the only force flag is the body force
     const bool g = p.has_g || MODE != MODE_AB;    // AA: the body-force instantiation, as in launch_fused_g
-    if (h->has_solid) { if (g) launch_fused_sc<MODE, true, 1>(h, p, grid); else launch_fused_sc<MODE, true, 0>(h, p, grid); }
-    else { if (g) launch_fused_sc<MODE, false, 1>(h, p, grid); else launch_fused_sc<MODE, false, 0>(h, p, grid); }
+    if (p.has_moving) launch_fused_sc<MODE, 2, 1>(h, p, grid);
+    else if (h->has_solid) { if (g) launch_fused_sc<MODE, 1, 1>(h, p, grid); else launch_fused_sc<MODE, 1, 0>(h, p, grid); }
+    else { if (g) launch_fused_sc<MODE, 0, 1>(h, p, grid); else launch_fused_sc<MODE, 0, 0>(h, p, grid); }
     return;
   }
   const bool nc = h->par.A_nc != 0.f;
-  if (h->has_solid) {
-    if (nc) launch_fused_g<MODE, true, true>(h, p, grid);
-    else launch_fused_g<MODE, true, false>(h, p, grid);
+  if (p.has_moving) {
+    if (nc) launch_fused_g<MODE, 2, true>(h, p, grid);
+    else launch_fused_g<MODE, 2, false>(h, p, grid);
+  } else if (h->has_solid) {
+    if (nc) launch_fused_g<MODE, 1, true>(h, p, grid);
+    else launch_fused_g<MODE, 1, false>(h, p, grid);
   } else {
-    if (nc) launch_fused_g<MODE, false, true>(h, p, grid);
-    else launch_fused_g<MODE, false, false>(h, p, grid);
+    if (nc) launch_fused_g<MODE, 0, true>(h, p, grid);
+    else launch_fused_g<MODE, 0, false>(h, p, grid);
   }
 }
 template <int MODE>
@@ -449,22 +459,35 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
   }
   Box b = h->box();
   const size_t nwords = (size_t)b.nxw * h->ny * h->nz;
+  // three bit masks behind each other (solid, wall group 2, wall group 3) and one flag word
   if (!h->mask) {
-    h->mask = static_cast<uint32_t*>(dev_alloc(nwords * 4));
+    h->mask = static_cast<uint32_t*>(dev_alloc((3 * nwords + 1) * 4));
     if (!h->mask) return fail(h, LB_ENOMEM, "mask allocation failed");
-    h->bytes += nwords * 4;
+    h->bytes += (3 * nwords + 1) * 4;
   }
   Staged in;
   int rc = stage_in(h, solid_mask, (size_t)h->S, in);
   if (rc) return rc;
   const int tb = 256;
-  k_pack_mask<<<(unsigned)((nwords + tb - 1) / tb), tb, 0, h->stream>>>(static_cast<const uint8_t*>(in.dev), h->mask, b);
-  h->launches++;
+  int* flag = reinterpret_cast<int*>(h->mask + 3 * nwords);
+  cudaMemsetAsync(flag, 0, sizeof(int), h->stream);
+  k_pack_mask<<<(unsigned)((nwords + tb - 1) / tb), tb, 0, h->stream>>>(static_cast<const uint8_t*>(in.dev), h->mask, h->mask + nwords, b);
+  k_any_moving<<<(unsigned)((h->S + tb - 1) / tb), tb, 0, h->stream>>>(static_cast<const uint8_t*>(in.dev), h->S, flag);
+  h->launches += 2;
   rc = check_launch(h, "k_pack_mask");
   if (rc) return rc;
-  cudaError_t e = cudaStreamSynchronize(h->stream);   // the staged copy dies with `in`
+  int moving = 0;
+  cudaError_t e = cudaMemcpyAsync(&moving, flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);   // also: the staged copy dies with `in`
   if (e != cudaSuccess) return cuda_fail(h, e, "lb_set_geometry");
+  h->has_moving = moving != 0;
   h->has_solid = true;
+  return LB_OK;
+}
+
+int lb_set_wall_velocity(lb_handle h, int group, float ux, float uy, float uz) {
+  if (!h || (group != 2 && group != 3)) return fail(h, LB_EINVAL, "wall group must be 2 or 3");
+  h->uw[group - 2][0] = ux; h->uw[group - 2][1] = uy; h->uw[group - 2][2] = uz;
   return LB_OK;
 }
 

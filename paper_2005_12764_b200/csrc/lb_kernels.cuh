@@ -43,6 +43,8 @@ struct StepParams {
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
   int two_tau, has_g;
   int edm;            // exact-difference forcing (Eq. 9) instead of Guo
+  int has_moving;     // some walls move (mask groups 2, 3): half-way bounce-back with the wall velocity (G28)
+  float uw2[3], uw3[3];
   int sc;             // Shan-Chen model (Eq. 5-10 of the paper): the fields are rho_r, rho_b instead of phi
   float G_C;          // its coupling strength, positive = repulsive
 };
@@ -149,6 +151,20 @@ __device__ __forceinline__ uint32_t neighbour_mask(const Box& b, int x, int y, i
   return m;
 }
 
+// The same for the moving wall groups: bit i of g2 / g3 <=> x + c_i is a wall of group 2 / 3.
+__device__ __forceinline__ void neighbour_groups(const Box& b, int x, int y, int z, uint32_t& g2, uint32_t& g3) {
+  const int xs[3] = {wrap_m(x, b.nx), x, wrap_p(x, b.nx)};
+  const int ys[3] = {wrap_m(y, b.ny), y, wrap_p(y, b.ny)};
+  const int zs[3] = {wrap_m(z, b.nz), z, wrap_p(z, b.nz)};
+  g2 = g3 = 0;
+  static_for<1, Q>([&](auto qc) {
+    constexpr int q = decltype(qc)::value;
+    const int g = wall_group_at(b, xs[1 + cx(q)], ys[1 + cy(q)], zs[1 + cz(q)]);
+    if (g == 2) g2 |= 1u << q;
+    if (g == 3) g3 |= 1u << q;
+  });
+}
+
 // ESZ: bytes per site in a plane (8 for the {T, R} pairs of a two-component run, 4 for one component)
 template <int ESZ>
 __device__ __forceinline__ void make_ctx(Ctx& c, const Box& b, int x, int y, int z) {
@@ -206,10 +222,12 @@ __device__ __forceinline__ void store_field_with_images(float* field, const Box&
 // Solid sites carry the sentinel in the first field.
 template <bool SC>
 __device__ __forceinline__ void store_fields(const StepParams& p, int x, int y, int z, int H, bool solid, float d, float rho) {
+  // the sentinel of a solid site also carries its wall group (1e30, 2e30, 3e30)
+  const float sent = solid ? PHI_SOLID * (float)wall_group_at(p.box, x, y, z) : 0.f;
   if constexpr (!SC) {
-    store_field_with_images(p.phi, p.box, x, y, z, H, solid ? PHI_SOLID : d / rho);
+    store_field_with_images(p.phi, p.box, x, y, z, H, solid ? sent : d / rho);
   } else {
-    store_field_with_images(p.phi, p.box, x, y, z, H, solid ? PHI_SOLID : 0.5f * (rho + d));
+    store_field_with_images(p.phi, p.box, x, y, z, H, solid ? sent : 0.5f * (rho + d));
     store_field_with_images(p.phi2, p.box, x, y, z, H, solid ? 0.f : 0.5f * (rho - d));
   }
 }
@@ -340,10 +358,13 @@ struct FusedSmem {
 // rho_r and rho_b, the Shan-Chen accelerations (Eq. 10; sign: DESIGN.md G27) replace
 // grad phi, each component gets the exact-difference source of Eq. 9, and there is no perturbation,
 // recolouring or near-contact force (HAS_NC = false; FMODE bit 0 only).
-template <int MODE, bool HAS_SOLID, bool HAS_NC, int FMODE, bool SC = false>
-__global__ void __launch_bounds__(TX* TY, (MODE == MODE_AA_ODD && SC) ? 2 : 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap,
+// WALLS: 0 = no solid sites, 1 = walls at rest, 2 = some walls move (G28; two CTAs per SM: the
+// extra live values of the wall correction would spill at 80 registers)
+template <int MODE, int WALLS, bool HAS_NC, int FMODE, bool SC = false>
+__global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS == 2) ? 2 : 3) k_fused(const StepParams p, const __grid_constant__ CUtensorMap tmap,
                                                      const __grid_constant__ CUtensorMap tmap2) {
   constexpr int H = HAS_NC ? H_MAX_NC : 1;
+  constexpr bool HAS_SOLID = WALLS > 0, MOVING = WALLS == 2;
   constexpr bool HAS_G = (FMODE & 1) != 0, EDM = (FMODE & 2) != 0;
   static_assert(!SC || !HAS_NC, "the Shan-Chen model has no near-contact force");
   using R_ = Ring<H>;
@@ -579,6 +600,18 @@ __global__ void __launch_bounds__(TX* TY, (MODE == MODE_AA_ODD && SC) ? 2 : 3) k
           ts = dr - tacc;
           rs = rr - racc;
         }
+        if constexpr (MOVING && q > 0) {
+          // half-way bounce-back at a moving wall (G28): what this link reflects loses
+          // 6 w_q rho^k (c_q . u_w); the wall group sits in the neighbour's sentinel (1e30 x group).
+          // The mass sums above keep the uncorrected values: a wall pushing on the fluid adds mass.
+          if ((smask >> q) & 1u) {
+            const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
+            const float cw = sv > 2.5f * PHI_SOLID ? cdot<q>(p.uw3[0], p.uw3[1], p.uw3[2])
+                                                   : (sv > 1.5f * PHI_SOLID ? cdot<q>(p.uw2[0], p.uw2[1], p.uw2[2]) : 0.f);
+            ts = fmaf(-6.0f * w * rho, cw, ts);
+            rs = fmaf(-6.0f * w * rr, cw, rs);
+          }
+        }
         const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
         *reinterpret_cast<float2*>(dst_ptr(p, s)) = make_float2(ts, rs);
         // f^r* - f^b* = 2 f^r* - f* = (2 rs - w) - ts: the first difference is exact in the mixed
@@ -637,6 +670,18 @@ __global__ void __launch_bounds__(TX* TY, (MODE == MODE_AA_ODD && SC) ? 2 : 3) k
             ts = dr - tacc;
             rs = rr - racc;
           }
+          if constexpr (MOVING && q > 0) {
+            // half-way bounce-back at a moving wall (G28): what this link reflects loses
+            // 6 w_q rho^k (c_q . u_w); the wall group sits in the neighbour's sentinel (1e30 x group).
+            // The mass sums above keep the uncorrected values: a wall pushing on the fluid adds mass.
+            if ((smask >> q) & 1u) {
+              const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
+              const float cw = sv > 2.5f * PHI_SOLID ? cdot<q>(p.uw3[0], p.uw3[1], p.uw3[2])
+                                                     : (sv > 1.5f * PHI_SOLID ? cdot<q>(p.uw2[0], p.uw2[1], p.uw2[2]) : 0.f);
+              ts = fmaf(-6.0f * w * rho, cw, ts);
+              rs = fmaf(-6.0f * w * rr, cw, rs);
+            }
+          }
           const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
           *reinterpret_cast<float2*>(dst_ptr(p, s)) = make_float2(ts, rs);
           vd[q] = (2.0f * rs - w) - ts;
@@ -644,7 +689,7 @@ __global__ void __launch_bounds__(TX* TY, (MODE == MODE_AA_ODD && SC) ? 2 : 3) k
         });
         };
         if (MODE == MODE_AA_ODD && HAS_SOLID && near_wall) collide(std::integral_constant<bool, HAS_SOLID>{});
-        else collide(std::false_type{});
+      else collide(std::false_type{});
       }
       if (HAS_SOLID && near_wall) {   // link bounce-back: what would enter a solid site comes back here
         float sd = 0.f, st = 0.f;
@@ -836,9 +881,9 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
     for (int e = 0; e < 4; ++e) {
       const float rho = 1.0f + t[e];
       if constexpr (!SC) {
-        f0[e] = solid[e] ? PHI_SOLID : d[e] / rho;
+        f0[e] = solid[e] ? PHI_SOLID * (float)wall_group_at(b, x + e, y, z) : d[e] / rho;
       } else {
-        f0[e] = solid[e] ? PHI_SOLID : 0.5f * (rho + d[e]);
+        f0[e] = solid[e] ? PHI_SOLID * (float)wall_group_at(b, x + e, y, z) : 0.5f * (rho + d[e]);
         f1[e] = solid[e] ? 0.f : 0.5f * (rho - d[e]);
       }
     }
@@ -864,10 +909,11 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
   const float omega = 1.0f / p.tau_r;
   const float om1 = 1.0f - omega, g0 = 1.0f - 0.5f * omega;
   for (int z = zb; z < ze; ++z) {
-    uint32_t smask = 0;
+    uint32_t smask = 0, g2m = 0, g3m = 0;
     if constexpr (HAS_SOLID) {
       if (solid_at(b, x, y, z)) continue;
       smask = neighbour_mask(b, x, y, z);
+      if (p.has_moving && smask) { neighbour_groups(b, x, y, z, g2m, g3m); g2m &= smask; g3m &= smask; }
     }
     Ctx c;
     make_ctx<4>(c, b, x, y, z);
@@ -911,6 +957,12 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
       }
       if constexpr (q > 0) tacc += ts;
       else ts = dr - tacc;
+      if constexpr (HAS_SOLID && q > 0) {      // moving wall (G28): the reflected value loses 6 w rho (c . u_w)
+        if ((g2m | g3m) >> q & 1u) {
+          const float cw = ((g2m >> q) & 1u) ? cdot<q>(p.uw2[0], p.uw2[1], p.uw2[2]) : cdot<q>(p.uw3[0], p.uw3[1], p.uw3[2]);
+          ts = fmaf(-6.0f * w * rho, cw, ts);
+        }
+      }
       *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask)) = ts;
     });
   }
@@ -1102,19 +1154,32 @@ __global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box
   }
 }
 
-// bytes [S] -> bit-packed words
-__global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, Box b) {
+// bytes [S] (0 fluid, 1 wall at rest, 2 / 3 moving wall groups) -> bit-packed words: solid, and
+// (if groups != nullptr) the two group masks behind each other
+__global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* groups, Box b) {
   const long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nw = (long long)b.nxw * b.ny * b.nz;
   if (wi >= nw) return;
   const long long row = wi / b.nxw;
   const int xw = (int)(wi % b.nxw);
-  uint32_t m = 0;
+  uint32_t m = 0, g2 = 0, g3 = 0;
   for (int i = 0; i < 32; ++i) {
     const int x = xw * 32 + i;
-    if (x < b.nx && bytes[row * b.nx + x]) m |= 1u << i;
+    if (x < b.nx) {
+      const uint8_t v = bytes[row * b.nx + x];
+      if (v) m |= 1u << i;
+      if (v == 2) g2 |= 1u << i;
+      if (v == 3) g3 |= 1u << i;
+    }
   }
   words[wi] = m;
+  if (groups) { groups[wi] = g2; groups[nw + wi] = g3; }
+}
+
+// does the byte mask hold a moving wall group?  out[0] |= 1
+__global__ void k_any_moving(const uint8_t* bytes, long long S, int* out) {
+  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s < S && (bytes[s] == 2 || bytes[s] == 3)) atomicOr(out, 1);
 }
 
 }  // namespace lb

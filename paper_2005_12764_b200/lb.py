@@ -18,7 +18,7 @@ LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 
 SYMBOLS = [
     "lb_set_allocator", "lb_create", "lb_destroy", "lb_set_stream", "lb_set_geometry",
-    "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_storage", "lb_init", "lb_step",
+    "lb_set_wall_velocity", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_storage", "lb_init", "lb_step",
     "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
 ]
@@ -47,6 +47,7 @@ def _load():
     lib.lb_destroy.restype = None
     lib.lb_set_stream.argtypes = [vp, vp]
     lib.lb_set_geometry.argtypes = [vp, fp]
+    lib.lb_set_wall_velocity.argtypes = [vp, C.c_int, C.c_float, C.c_float, C.c_float]
     lib.lb_set_body_force.argtypes = [vp, C.c_float, C.c_float, C.c_float]
     lib.lb_set_model.argtypes = [vp, C.c_int, C.c_float]
     lib.lb_set_forcing.argtypes = [vp, C.c_int]
@@ -159,6 +160,9 @@ class LB:
     def set_geometry(self, solid_mask):
         self._sync_stream()
         self._ck(lib.lb_set_geometry(self.h, _addr(solid_mask)))
+
+    def set_wall_velocity(self, group, ux, uy, uz):
+        self._ck(lib.lb_set_wall_velocity(self.h, int(group), ux, uy, uz))
 
     def set_body_force(self, gx, gy, gz):
         self._ck(lib.lb_set_body_force(self.h, gx, gy, gz))

@@ -493,3 +493,75 @@ def test_randomised_configurations(lbmod, lbo, seed):
                 assert e[ok].max() < pu.POP_TOL, (tag, n, e[ok].max())
     rr, rb, u = sim.get_macros()
     assert np.isfinite(u).all(), tag
+
+
+# ------------------------------------------------------------------------------- moving walls
+def _couette_workload(two, ny=34, nx=8, nz=4):
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 2
+    solid[:, -1, :] = 3
+    ones = np.ones((nz, ny, nx), np.float32)
+    return W.Workload("couette", nx, ny, nz, 0.9, 1.3 if two else 0.9, 0.0, 0.0, 0.0,
+                      0.4 * ones if two else ones, 0.6 * ones if two else None,
+                      np.zeros((3, nz, ny, nx), np.float32), solid=solid)
+
+
+@pytest.mark.parametrize("two", [False, True])
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_couette_between_sliding_walls(lbmod, two, storage):
+    """"solid walls with opposite speeds +-U = 0.01" (G28): the steady profile
+    between half-way moving walls is the straight line u_x = U (2 (y - 1/2)/H - 1), on the CUDA
+    path itself (closed form, no oracle), one and two components."""
+    w = _couette_workload(two)
+    sim = lbmod.from_workload(w, storage=storage)
+    sim.set_wall_velocity(2, -0.01, 0.0, 0.0)
+    sim.set_wall_velocity(3, 0.01, 0.0, 0.0)
+    sim.init(w.rho_r, w.rho_b, w.u)
+    sim.step(30000)
+    rr, rb, u = sim.get_macros()
+    y = np.arange(w.ny)
+    exact = 0.01 * (2 * (y - 0.5) / (w.ny - 2.0) - 1.0)
+    prof = u[0][2, :, 3]
+    assert np.abs(prof[1:-1] - exact[1:-1]).max() < 1e-5, np.abs(prof[1:-1] - exact[1:-1]).max()
+    rho = rr if rb is None else rr + rb
+    assert abs(float(rho[:, 1:-1, :].mean()) - 1.0) < 1e-5
+
+
+@pytest.mark.parametrize("model", ["cg", "sc"])
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_moving_walls_parity(lbmod, lbo, model, storage):
+    """Sliding and pushing walls of both groups (and a wall at rest) against the oracle:
+    populations after 1, 2 and 5 steps, both models, near contact and body force on."""
+    w = _random_workload(36, 13, 10, seed=51, walls=True, A_nc=0.0 if model == "sc" else 0.02)
+    w.solid[:, 0, :] = 2                  # the y = 0 plane slides and pushes
+    w.solid[0, :, :] = 1                  # the z = 0 plane is at rest
+    w.solid[w.nz // 2, w.ny // 2, w.nx // 3] = 3
+    fluid = w.solid == 0
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    sim.set_storage(storage)
+    if model == "sc":
+        o.set_model("sc", 1.5); sim.set_model("sc", 1.5)
+    for obj in (o, sim):
+        obj.set_geometry(w.solid)
+        obj.set_body_force(*w.g)
+        obj.set_wall_velocity(2, 0.01, 0.002, -0.003)
+        obj.set_wall_velocity(3, -0.004, 0.0, 0.006)
+        obj.init(w.rho_r, w.rho_b, w.u)
+    risky = np.zeros(w.shape, bool)
+    done = 0
+    for n in (1, 2, 5):
+        for _ in range(n - done):
+            risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+            o.step(1); sim.step(1)
+        done = n
+        e = pu.pop_error(sim, o)
+        assert e[~risky & fluid].max() < pu.POP_TOL, (n, e[~risky & fluid].max())
+    # the moving walls do change the result
+    ref = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    ref.set_storage(storage)
+    if model == "sc":
+        ref.set_model("sc", 1.5)
+    ref.set_geometry(w.solid); ref.set_body_force(*w.g); ref.init(w.rho_r, w.rho_b, w.u)
+    ref.step(5)
+    assert np.abs(ref.get_populations(0) - sim.get_populations(0)).max() > 1e-6
