@@ -27,8 +27,11 @@
 // P5 shear-wave viscosity (Eq. 4), P6 mixture viscosity (Eq. 8), P7 Poiseuille, P8 Laplace,
 // P9 near-contact sign/size, P10 film table A_h(h), P11 lattice symmetry, P12 brute-force numpy
 // twin, P13 Taylor-Green decay.
+// P14 exact-difference forcing, P15 Couette flow between sliding walls (G28), P16 colour-exchange
+// symmetry of the symmetric probe (G29), P17 wetting: symmetry, neutrality and monotone contact
+// angle (G30); SC1-SC5 for the second model.
 // PARITY UNPINNED against the paper (pinned only against DESIGN.md's reading): the discrete
-// contact search (G10), H_MAX, the wall rule for phi (G8), the guard eps (G7).
+// contact search (G10), H_MAX, the wall rule for phi (G8, G30), the guard eps (G7).
 //
 // Deliberately nothing clever: loops over sites and over the 19 directions, two full
 // population arrays, OpenMP on the outermost site loop only.
@@ -66,6 +69,9 @@ struct Oracle {
   double g[3] = {0, 0, 0};
   double phi_c = 0.9;
   int nc_mode = 0;  // 0 = probe (S3), 1 = test hook: every |phi|<phi_c site in contact with A_h = A_nc
+  int nc_sym = 0;   // 1 = colour-symmetric probe (G29): the rule plus its image under r <-> b
+  int wet = 0;      // 1 = prescribed phi at solid nodes (G30): a solid neighbour contributes phi_wall
+  double phi_wall = 0.0;
   int model = 0;    // 0 = colour gradient (north_star), 1 = Shan-Chen, the paper's own Eq. 5-10
   double G_C = 0.0; // strength of the inter-component force of Eq. 10, positive = repulsive
   int forcing = 0;  // 0 = Guo (north_star; S4, S6), 1 = exact difference, the paper's own Eq. 9
@@ -142,10 +148,11 @@ void force_at(Oracle& o, int x, int y, int z, double& Gx, double& Gy, double& Gz
   double marg = 1e300;
   if (o.two) {
     const double phi0 = o.phi[s];
-    // S2: G = 3 sum_{i>=1} w_i c_i phi~(x+c_i); a solid neighbour contributes phi(x) (G8).
+    // S2: G = 3 sum_{i>=1} w_i c_i phi~(x+c_i); a solid neighbour contributes phi(x) (G8), or
+    // the prescribed wall value phi_wall when wetting is on (G30).
     for (int i = 1; i < Q; ++i) {
       size_t n = o.nbr(x, y, z, CX[i], CY[i], CZ[i]);
-      double p = o.solid[n] ? phi0 : o.phi[n];
+      double p = o.solid[n] ? (o.wet ? o.phi_wall : phi0) : o.phi[n];
       Gx += 3.0 * W[i] * CX[i] * p;
       Gy += 3.0 * W[i] * CY[i] * p;
       Gz += 3.0 * W[i] * CZ[i] * p;
@@ -183,6 +190,33 @@ void force_at(Oracle& o, int x, int y, int z, double& Gx, double& Gy, double& Gz
             // A_h = A for h <= h_min, decays as h^-3 beyond.
             Ah = hfound <= H_MIN ? o.A_nc
                                  : o.A_nc * std::pow((double)H_MIN / (double)hfound, 3.0);
+          }
+          if (o.nc_sym) {
+            // G29: Fig. 5 is symmetric in the two fluids.  The image of the rule
+            // above under r <-> b (phi -> -phi, G -> -G): march along +G/|G| and stop at the first
+            // k >= 2 with phi(probe) <= phi(x) (two blue interfaces across a red film); its force
+            // is -A_h(h+) G / 2.  Both are applied: F = (A_h(h-) - A_h(h+)) G / 2.
+            int hplus = 0;
+            for (int k = 1; k <= H_MAX; ++k) {
+              int d[3];
+              for (int a = 0; a < 3; ++a) {
+                double v = -k * n[a];
+                d[a] = (int)std::lround(v);
+              }
+              size_t p = o.nbr(x, y, z, d[0], d[1], d[2]);
+              if (o.solid[p]) break;
+              if (k >= 2) {
+                marg = std::fmin(marg, std::fabs(o.phi[p] - phi0));
+                if (o.phi[p] <= phi0) {
+                  hplus = k;
+                  break;
+                }
+              }
+            }
+            if (hplus > 0) {
+              Ah -= hplus <= H_MIN ? o.A_nc : o.A_nc * std::pow((double)H_MIN / (double)hplus, 3.0);
+              hfound |= hplus << 4;   // reported as h- + 16 h+
+            }
           }
         }
         // -A_h n delta_I = -A_h (-G/|G|) (|G|/2) = +A_h G / 2
@@ -477,6 +511,24 @@ int lbo_set_forcing(void* h, int mode) {
   Oracle* o = static_cast<Oracle*>(h);
   if (!o || (mode != 0 && mode != 1)) return LBO_EINVAL;
   o->forcing = mode;
+  return LBO_OK;
+}
+
+// 1 = colour-symmetric near-contact probe (G29); 0 = the probe toward decreasing phi only (default)
+int lbo_set_nc_symmetric(void* h, int on) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (on != 0 && on != 1)) return LBO_EINVAL;
+  o->nc_sym = on;
+  return LBO_OK;
+}
+
+// on = 1: solid nodes carry the prescribed value phi_wall in the colour-gradient stencil (G30);
+// on = 0: a solid neighbour contributes the centre value (G8, default)
+int lbo_set_wall_phi(void* h, int on, double phi_wall) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (on != 0 && on != 1) || !(std::fabs(phi_wall) <= 1.0)) return LBO_EINVAL;
+  o->wet = on;
+  o->phi_wall = phi_wall;
   return LBO_OK;
 }
 

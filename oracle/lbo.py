@@ -40,6 +40,8 @@ def _load():
         lib.lbo_set_wall_velocity.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double]
         lib.lbo_set_nc_cutoff.argtypes = [vp, C.c_double]
         lib.lbo_set_nc_mode.argtypes = [vp, C.c_int]
+        lib.lbo_set_nc_symmetric.argtypes = [vp, C.c_int]
+        lib.lbo_set_wall_phi.argtypes = [vp, C.c_int, C.c_double]
         lib.lbo_set_forcing.argtypes = [vp, C.c_int]
         lib.lbo_set_model.argtypes = [vp, C.c_int, C.c_double]
         lib.lbo_init.argtypes = [vp, dp, dp, dp]
@@ -124,6 +126,15 @@ class Oracle:
     def set_forcing(self, mode):
         """0 / 'guo' = Guo forcing, 1 / 'edm' = exact-difference forcing (Eq. 9)."""
         self._ck(self.lib.lbo_set_forcing(self.h, {'guo': 0, 'edm': 1}.get(mode, mode)), "lbo_set_forcing")
+
+    def set_nc_symmetric(self, on):
+        """Colour-symmetric near-contact probe (G29)."""
+        self._ck(self.lib.lbo_set_nc_symmetric(self.h, int(bool(on))), "lbo_set_nc_symmetric")
+
+    def set_wall_phi(self, phi_wall):
+        """Prescribed phi at solid nodes (wetting, G30); None = neutral rule G8."""
+        self._ck(self.lib.lbo_set_wall_phi(self.h, 0 if phi_wall is None else 1,
+                                           0.0 if phi_wall is None else float(phi_wall)), "lbo_set_wall_phi")
 
     def set_nc_mode(self, mode):
         self._ck(self.lib.lbo_set_nc_mode(self.h, mode), "lbo_set_nc_mode")

@@ -453,3 +453,169 @@ def test_P15_couette_between_sliding_walls(lbo):
         assert np.abs(u[1]).max() < 1e-12 and np.abs(u[2]).max() < 1e-12
         rho = rr if rb is None else rr + rb
         assert abs(rho[:, 1:-1, :].mean() - 1.0) < 1e-12          # tangential walls exchange no mass
+
+
+# ---------------------------------------------------------------------------------- P16
+def _film(h, sign):
+    nx, x0 = 64, 20
+    phi = np.ones(nx)
+    phi[x0] = 0.5
+    phi[x0 + 1:x0 + h] = -0.8
+    phi[x0 + h] = 0.5
+    return sign * phi, x0
+
+
+@pytest.mark.parametrize("h", [2, 3, 4, 5])
+def test_P16_symmetric_probe_film_table(lbo, h):
+    """Fig. 5 is symmetric in the two fluids (G24); the colour-symmetric probe
+    (G29) applies the rule and its image under r <-> b.  On the film of P10: a blue film
+    between red slabs gives the table of P10 unchanged (the + probe finds nothing); a red film
+    between blue slabs, invisible to the one-sided probe, gives the same force field (the force
+    acts on the total momentum and pushes the interfaces apart in both cases)."""
+    A_nc = 0.02
+    table = {2: A_nc, 3: A_nc, 4: A_nc * 0.421875, 5: 0.0}
+    out = {}
+    for sign in (+1.0, -1.0):
+        for sym in (0, 1):
+            phi, x0 = _film(h, sign)
+            o = lbo.Oracle(phi.size, 1, 1, 1.0, 1.0, 0.01, 0.7, A_nc)
+            o.set_nc_symmetric(sym)
+            p3 = phi.reshape(1, 1, -1)
+            o.init((1 + p3) / 2, (1 - p3) / 2, np.zeros((3, 1, 1, phi.size)))
+            fl = o.get_fields()
+            out[sign, sym] = (fl["F"][0].ravel().copy(), fl["h"].ravel().copy(), fl["G"][0].ravel().copy())
+    F_ref, h_ref, G_ref = out[+1.0, 0]
+    hh = h if h <= 4 else 0
+    assert h_ref[x0] == hh and abs(F_ref[x0] - 0.5 * table[h] * G_ref[x0]) < 1e-17
+    # blue film, symmetric probe: unchanged
+    assert np.array_equal(out[+1.0, 1][0], F_ref) and np.array_equal(out[+1.0, 1][1], h_ref)
+    # red film: nothing for the one-sided probe, the mirrored table for the symmetric one
+    assert np.abs(out[-1.0, 0][0]).max() == 0 and out[-1.0, 0][1].max() == 0
+    assert np.array_equal(out[-1.0, 1][0], F_ref)
+    assert np.array_equal(out[-1.0, 1][1], h_ref << 4)                      # reported as h- + 16 h+
+    assert np.array_equal(out[-1.0, 1][2], -G_ref)
+    if hh:
+        assert np.sign(F_ref[x0]) == -1.0 and np.sign(F_ref[x0 + h]) == +1.0    # away from the film
+
+
+def test_P16_colour_exchange_invariance(lbo):
+    """With the symmetric probe the whole model is invariant under the exchange of the two
+    fluids (rho_r <-> rho_b, tau_r <-> tau_b): 20 steps of a 16^3 mixture with thin films of
+    both colours agree to rounding; with the one-sided probe they do not (the pin would catch a
+    probe that marches the wrong way or applies the wrong sign)."""
+    n = 16
+    z, y, x = np.meshgrid(*(np.arange(n),) * 3, indexing="ij")
+    k = 2 * np.pi / n
+    s = (np.sin(2 * k * x + 0.3) * np.cos(k * y) + np.sin(2 * k * y + 1.1) * np.cos(2 * k * z + 0.5)
+         + 0.7 * np.sin(3 * k * z + k * x))
+    phi = 0.98 * np.tanh(2.0 * s)
+    u0 = 0.01 * np.stack([np.sin(k * y), np.sin(k * z), np.sin(k * x)])
+
+    def run(swap, sym):
+        tr, tb = (1.2, 0.8) if swap else (0.8, 1.2)
+        o = lbo.Oracle(n, n, n, tr, tb, 0.01, 0.7, 0.05)
+        o.set_nc_symmetric(sym)
+        p = -phi if swap else phi
+        o.init((1 + p) / 2, (1 - p) / 2, u0)
+        fl = o.get_fields()
+        o.step(20)
+        return o.get_macros(), fl
+
+    (a_r, a_b, a_u), fa = run(False, 1)
+    (b_r, b_b, b_u), fb = run(True, 1)
+    hm, hp = fa["h"] & 15, fa["h"] >> 4
+    assert (hm > 0).sum() > 500 and (hp > 0).sum() > 500                     # both probes fire
+    assert np.abs(fa["F"] - fb["F"]).max() < 1e-15 and np.abs(fa["F"]).max() > 1e-2
+    assert np.abs(a_r - b_b).max() < 1e-13 and np.abs(a_b - b_r).max() < 1e-13
+    assert np.abs(a_u - b_u).max() < 1e-13
+    (c_r, _, c_u), _ = run(False, 0)
+    (_, d_b, d_u), _ = run(True, 0)
+    assert np.abs(c_r - d_b).max() > 1e-3                                    # the one-sided rule is not symmetric
+
+
+# ---------------------------------------------------------------------------------- P17
+def test_P17_wall_phi_in_the_stencil(lbo):
+    """Wetting (G30): a solid node carries the prescribed phi_wall in the colour-gradient stencil.
+    Quasi-1-D, where the D3Q19 stencil is the central difference: next to the wall
+    G_x = (phi_wall - phi(x-1))/2 exactly; with wetting off, (phi(x) - phi(x-1))/2 (G8)."""
+    nx = 16
+    rng = np.random.default_rng(17)
+    phi = rng.uniform(-0.8, 0.8, nx)
+    solid = np.zeros(nx, np.uint8)
+    solid[0] = solid[-1] = 1
+    for pw in (None, -0.6, 0.0, 0.35):
+        o = lbo.Oracle(nx, 1, 1, 1.0, 1.0, 0.01, 0.7, 0.0)
+        o.set_geometry(solid.reshape(1, 1, nx))
+        o.set_wall_phi(pw)
+        p3 = phi.reshape(1, 1, nx)
+        o.init((1 + p3) / 2, (1 - p3) / 2, np.zeros((3, 1, 1, nx)))
+        fl = o.get_fields()
+        G = fl["G"][0].ravel()
+        ph = fl["phi"].ravel()
+        assert abs(G[nx - 2] - ((ph[nx - 2] if pw is None else pw) - ph[nx - 3]) / 2) < 1e-15
+        assert abs(G[1] - (ph[2] - (ph[1] if pw is None else pw)) / 2) < 1e-15
+        assert abs(G[5] - (ph[6] - ph[4]) / 2) < 1e-15
+
+
+def test_P17_wetting_colour_exchange(lbo):
+    """(rho_r, rho_b, phi_wall) -> (rho_b, rho_r, -phi_wall) exchanges the two fluids exactly."""
+    nx, ny, nz = 12, 10, 8
+    rng = np.random.default_rng(170)
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 1
+    solid[:, -1, :] = 1
+    solid[3:5, 4:6, 5:8] = 1
+    rr = rng.uniform(0.1, 0.9, (nz, ny, nx))
+    rb = rng.uniform(0.1, 0.9, (nz, ny, nx))
+    u0 = 0.01 * rng.normal(size=(3, nz, ny, nx))
+
+    def run(swap):
+        o = lbo.Oracle(nx, ny, nz, 0.9, 0.9, 0.01, 0.7, 0.0)
+        o.set_geometry(solid)
+        o.set_wall_phi(-0.4 if swap else 0.4)
+        o.init(rb if swap else rr, rr if swap else rb, u0)
+        o.step(10)
+        return o.get_macros()
+
+    a_r, a_b, a_u = run(False)
+    b_r, b_b, b_u = run(True)
+    assert np.abs(a_r - b_b).max() < 1e-13 and np.abs(a_b - b_r).max() < 1e-13 and np.abs(a_u - b_u).max() < 1e-14
+
+
+def _contact_angle(lbo, phi_w, nx=64, ny=26, R=10.0, steps=4000):
+    """Red half-disc on the lower wall of a quasi-2-D channel, relaxed; the angle of the circular
+    cap from its height H and base width B: tan(theta / 2) = 2 H / B."""
+    solid = np.zeros((1, ny, nx), np.uint8)
+    solid[:, 0, :] = 1
+    solid[:, -1, :] = 1
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    d = np.sqrt((x - nx / 2 + 0.5) ** 2 + (y - 0.5) ** 2)           # centred on the wall plane y = 1/2
+    phi = np.tanh((R - d) / 1.5).reshape(1, ny, nx)
+    o = lbo.Oracle(nx, ny, 1, 1.0, 1.0, 0.01, 0.7, 0.0)
+    o.set_geometry(solid)
+    o.set_wall_phi(phi_w)
+    o.init((1 + phi) / 2, (1 - phi) / 2, np.zeros((3, 1, ny, nx)))
+    o.step(steps)
+    rr, rb, _ = o.get_macros()
+    p = ((rr - rb) / np.where(rr + rb > 0, rr + rb, 1.0))[0]
+
+    def crossing(v):
+        i = int(np.where((v[:-1] > 0) & (v[1:] <= 0))[0][0])
+        return i + v[i] / (v[i] - v[i + 1])
+
+    H = crossing(0.5 * (p[1:-1, nx // 2 - 1] + p[1:-1, nx // 2])) + 0.5   # first fluid row: half a link above the wall
+    B = 2.0 * (crossing(p[1, nx // 2:]) + 0.5)
+    return 2.0 * np.arctan(2.0 * H / B)
+
+
+def test_P17_contact_angle(lbo):
+    """The static contact angle of the colour-gradient model with a prescribed wall value follows
+    cos(theta) ~= phi_wall (the known approximate law for this family of wall rules; the paper has
+    no wetting model, PAPER.md is silent: G30).  Checked to 0.2 in cos(theta), with the spacing
+    between phi_wall = -0.5, 0, 0.5 within 0.1 of 0.5, theta decreasing as the wall turns red."""
+    from threadpoolctl import threadpool_limits
+    with threadpool_limits(limits=1, user_api="openmp"):     # nz = 1: nothing to share out
+        cos = {pw: float(np.cos(_contact_angle(lbo, pw))) for pw in (-0.5, 0.0, 0.5)}
+    for pw, c in cos.items():
+        assert abs(c - pw) < 0.2, cos
+    assert abs((cos[0.0] - cos[-0.5]) - 0.5) < 0.1 and abs((cos[0.5] - cos[0.0]) - 0.5) < 0.1, cos
