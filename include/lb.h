@@ -104,6 +104,19 @@ int lb_set_forcing(lb_handle h, int mode);
 /* Near-contact force acts where |phi| < phi_c (default 0.9). */
 int lb_set_nc_cutoff(lb_handle h, float phi_c);
 
+/* Colour-symmetric near-contact probe (G29; Fig. 5, is symmetric in the
+ * two fluids).  on = 0 (default): the probe marches along -G/|G| and finds h- = the first k >= 2
+ * with phi(probe) >= phi(x): F_nc = A_h(h-) G / 2 (two red interfaces across a blue film).
+ * on = 1: its image under r <-> b is applied as well (along +G/|G|, h+ = first k >= 2 with
+ * phi(probe) <= phi(x)): F_nc = (A_h(h-) - A_h(h+)) G / 2.  May be changed between steps. */
+int lb_set_nc_symmetric(lb_handle h, int on);
+
+/* Wetting (G30; the paper has no wetting model).  on = 0 (default): a solid neighbour
+ * contributes the centre value phi(x) to the colour-gradient stencil (neutral wall).  on = 1: it
+ * contributes the prescribed phi_wall in [-1, 1], one value for all walls (static contact angle
+ * cos(theta) ~= phi_wall).  Colour-gradient model only.  May be changed between steps. */
+int lb_set_wall_phi(lb_handle h, int on, float phi_wall);
+
 /* Storage of the populations.  0 = A/B double buffer (default), 1 = AA-pattern, one buffer
  * updated in place.  Must precede lb_init. */
 int lb_set_storage(lb_handle h, int mode);

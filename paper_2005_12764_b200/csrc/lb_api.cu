@@ -58,6 +58,9 @@ struct lb_handle_s {
   lb_params par{};
   float g[3] = {0, 0, 0};
   float phi_c = 0.9f;
+  int nc_sym = 0;            // colour-symmetric near-contact probe (G29)
+  int wet = 0;               // prescribed phi at solid nodes (G30)
+  float phi_wall = 0.f;
   int forcing = 0;          // 0 Guo, 1 exact difference (Eq. 9)
   int storage = 0;          // 0 A/B, 1 AA
   bool two = true;
@@ -175,6 +178,7 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   p.halo = (h->model == 0 && h->par.A_nc != 0.f) ? H_MAX_NC : 1;
   p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
   p.A_nc = h->par.A_nc; p.phi_c = h->phi_c;
+  p.nc_sym = h->nc_sym; p.wet = h->wet; p.phi_wall = h->phi_wall;
   p.gx = h->g[0]; p.gy = h->g[1]; p.gz = h->g[2];
   p.two_tau = h->par.tau_r != h->par.tau_b;
   p.has_g = (h->g[0] != 0.f || h->g[1] != 0.f || h->g[2] != 0.f);
@@ -363,6 +367,7 @@ IoParams make_io_params(lb_handle h) {
   p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
   p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
   p.A_nc = h->par.A_nc; p.phi_c = h->phi_c;
+  p.nc_sym = h->nc_sym; p.wet = h->wet; p.phi_wall = h->phi_wall;
   p.gx = h->g[0]; p.gy = h->g[1]; p.gz = h->g[2];
   return p;
 }
@@ -514,6 +519,21 @@ int lb_set_forcing(lb_handle h, int mode) {
 int lb_set_nc_cutoff(lb_handle h, float phi_c) {
   if (!h) return LB_EINVAL;
   h->phi_c = phi_c;
+  return LB_OK;
+}
+
+int lb_set_nc_symmetric(lb_handle h, int on) {
+  if (!h) return LB_EINVAL;
+  if (on != 0 && on != 1) return fail(h, LB_EINVAL, "lb_set_nc_symmetric: on must be 0 or 1");
+  h->nc_sym = on;
+  return LB_OK;
+}
+
+int lb_set_wall_phi(lb_handle h, int on, float phi_wall) {
+  if (!h) return LB_EINVAL;
+  if ((on != 0 && on != 1) || !(fabsf(phi_wall) <= 1.0f)) return fail(h, LB_EINVAL, "lb_set_wall_phi: on must be 0 or 1 and |phi_wall| <= 1");
+  h->wet = on;
+  h->phi_wall = phi_wall;
   return LB_OK;
 }
 

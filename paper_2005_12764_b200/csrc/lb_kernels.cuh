@@ -43,6 +43,9 @@ struct StepParams {
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
   int two_tau, has_g;
   int edm;            // exact-difference forcing (Eq. 9) instead of Guo
+  int nc_sym;         // colour-symmetric near-contact probe (G29)
+  int wet;            // solid nodes carry phi_wall in the colour-gradient stencil (G30)
+  float phi_wall;
   int has_moving;     // some walls move (mask groups 2, 3): half-way bounce-back with the wall velocity (G28)
   float uw2[3], uw3[3];
   int sc;             // Shan-Chen model (Eq. 5-10 of the paper): the fields are rho_r, rho_b instead of phi
@@ -447,12 +450,14 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
       float Hx = 0.f, Hy = 0.f, Hz = 0.f;       // SC: sum_i w_i c_i rho_r(x + c_i)
       uint32_t smask = 0;
       if constexpr (!SC) {
+        // a solid neighbour contributes the centre value (G8) or the prescribed wall value (G30)
+        const float wallv = (HAS_SOLID && p.wet) ? p.phi_wall : phi0;
         static_for<1, Q>([&](auto qc) {
           constexpr int q = decltype(qc)::value;
           const float* pl = cz(q) == 0 ? pl0 : (cz(q) > 0 ? plp : plm);
           float v = pl[(ly + cy(q)) * R_::BX + lx + cx(q)];
           if constexpr (HAS_SOLID) {
-            if (v > PHI_SOLID_TEST) { smask |= 1u << q; v = phi0; }
+            if (v > PHI_SOLID_TEST) { smask |= 1u << q; v = wallv; }
           }
           constexpr float k = 3.0f * wq(q);
           if constexpr (cx(q) != 0) Gx += (k * cx(q)) * v;
@@ -516,19 +521,31 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
       if constexpr (HAS_NC) {
         if (fabsf(phi0) < p.phi_c && aniso) {
           const float nx_ = -Gx * invG, ny_ = -Gy * invG, nz_ = -Gz * invG;
-          int h = 0;
-          bool alive = true;
+          // h: first k >= 2 along -G with phi(probe) >= phi(x); hp (symmetric probe, G29): first
+          // k >= 2 along +G (the mirrored offsets) with phi(probe) <= phi(x)
+          int h = 0, hp = 0;
+          bool alive = true, alive2 = p.nc_sym != 0;
 #pragma unroll
           for (int k = 1; k <= H_MAX_NC; ++k) {
-            if (alive) {
+            if (alive || alive2) {
               const int dx = (int)roundf(k * nx_), dy = (int)roundf(k * ny_), dz = (int)roundf(k * nz_);
-              const float v = plane(dz)[(ly + dy) * R_::BX + lx + dx];
-              if (HAS_SOLID && v > PHI_SOLID_TEST) alive = false;
-              else if (k >= 2 && v >= phi0) { h = k; alive = false; }
+              if (alive) {
+                const float v = plane(dz)[(ly + dy) * R_::BX + lx + dx];
+                if (HAS_SOLID && v > PHI_SOLID_TEST) alive = false;
+                else if (k >= 2 && v >= phi0) { h = k; alive = false; }
+              }
+              if (alive2) {
+                const float v = plane(-dz)[(ly - dy) * R_::BX + lx - dx];
+                if (HAS_SOLID && v > PHI_SOLID_TEST) alive2 = false;
+                else if (k >= 2 && v <= phi0) { hp = k; alive2 = false; }
+              }
             }
           }
-          if (h > 0) {
-            const float Ah = h <= H_MIN_NC ? p.A_nc : p.A_nc * ((float)(H_MIN_NC * H_MIN_NC * H_MIN_NC) / (float)(h * h * h));
+          auto A_h = [&](int hh) {
+            return hh == 0 ? 0.f : (hh <= H_MIN_NC ? p.A_nc : p.A_nc * ((float)(H_MIN_NC * H_MIN_NC * H_MIN_NC) / (float)(hh * hh * hh)));
+          };
+          if (h > 0 || hp > 0) {
+            const float Ah = A_h(h) - A_h(hp);
             Fx = 0.5f * Ah * Gx; Fy = 0.5f * Ah * Gy; Fz = 0.5f * Ah * Gz;
           }
         }
@@ -986,6 +1003,8 @@ struct IoParams {
   int sc;                // Shan-Chen model
   float G_C;
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
+  int nc_sym, wet;       // as in StepParams
+  float phi_wall;
 };
 
 template <int MODE>
@@ -1110,7 +1129,7 @@ __global__ void k_macros(const IoParams p) {
       float Gx = 0.f, Gy = 0.f, Gz = 0.f;
       for (int q = 1; q < Q; ++q) {
         float v = ph[c_cx[q] + px * c_cy[q] + pxy * c_cz[q]];
-        if (v > PHI_SOLID_TEST) v = phi0;
+        if (v > PHI_SOLID_TEST) v = p.wet ? p.phi_wall : phi0;
         const float k = 3.0f * wq(q);
         Gx += k * c_cx[q] * v; Gy += k * c_cy[q] * v; Gz += k * c_cz[q] * v;
       }
@@ -1118,17 +1137,18 @@ __global__ void k_macros(const IoParams p) {
       if (fabsf(phi0) < p.phi_c && Gn > EPS_G) {
         const float invG = 1.0f / Gn;
         const float nx_ = -Gx * invG, ny_ = -Gy * invG, nz_ = -Gz * invG;
-        int h = 0;
-        for (int k = 1; k <= H_MAX_NC; ++k) {
-          const int dx = (int)roundf(k * nx_), dy = (int)roundf(k * ny_), dz = (int)roundf(k * nz_);
-          const float v = ph[dx + px * dy + pxy * dz];
-          if (v > PHI_SOLID_TEST) break;
-          if (k >= 2 && v >= phi0) { h = k; break; }
+        float Ah = 0.f;
+        for (int sgn = 1; sgn >= (p.nc_sym ? -1 : 1); sgn -= 2) {     // +1: along -G; -1: the mirrored probe (G29)
+          int h = 0;
+          for (int k = 1; k <= H_MAX_NC; ++k) {
+            const int dx = sgn * (int)roundf(k * nx_), dy = sgn * (int)roundf(k * ny_), dz = sgn * (int)roundf(k * nz_);
+            const float v = ph[dx + px * dy + pxy * dz];
+            if (v > PHI_SOLID_TEST) break;
+            if (k >= 2 && (sgn > 0 ? v >= phi0 : v <= phi0)) { h = k; break; }
+          }
+          if (h > 0) Ah += sgn * (h <= H_MIN_NC ? p.A_nc : p.A_nc * ((float)(H_MIN_NC * H_MIN_NC * H_MIN_NC) / (float)(h * h * h)));
         }
-        if (h > 0) {
-          const float Ah = h <= H_MIN_NC ? p.A_nc : p.A_nc * ((float)(H_MIN_NC * H_MIN_NC * H_MIN_NC) / (float)(h * h * h));
-          Fx += 0.5f * Ah * Gx; Fy += 0.5f * Ah * Gy; Fz += 0.5f * Ah * Gz;
-        }
+        Fx += 0.5f * Ah * Gx; Fy += 0.5f * Ah * Gy; Fz += 0.5f * Ah * Gz;
       }
     }
     const float inv_rho = 1.0f / rho;

@@ -18,7 +18,7 @@ LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 
 SYMBOLS = [
     "lb_set_allocator", "lb_create", "lb_destroy", "lb_set_stream", "lb_set_geometry",
-    "lb_set_wall_velocity", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_storage", "lb_init", "lb_step",
+    "lb_set_wall_velocity", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_nc_symmetric", "lb_set_wall_phi", "lb_set_storage", "lb_init", "lb_step",
     "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
 ]
@@ -52,6 +52,8 @@ def _load():
     lib.lb_set_model.argtypes = [vp, C.c_int, C.c_float]
     lib.lb_set_forcing.argtypes = [vp, C.c_int]
     lib.lb_set_nc_cutoff.argtypes = [vp, C.c_float]
+    lib.lb_set_nc_symmetric.argtypes = [vp, C.c_int]
+    lib.lb_set_wall_phi.argtypes = [vp, C.c_int, C.c_float]
     lib.lb_set_storage.argtypes = [vp, C.c_int]
     lib.lb_init.argtypes = [vp, fp, fp, fp]
     lib.lb_step.argtypes = [vp, C.c_int]
@@ -175,6 +177,13 @@ class LB:
 
     def set_nc_cutoff(self, phi_c):
         self._ck(lib.lb_set_nc_cutoff(self.h, phi_c))
+
+    def set_nc_symmetric(self, on):
+        self._ck(lib.lb_set_nc_symmetric(self.h, int(bool(on))))
+
+    def set_wall_phi(self, phi_wall):
+        """Prescribed phi at solid nodes; None switches back to the neutral wall."""
+        self._ck(lib.lb_set_wall_phi(self.h, 0 if phi_wall is None else 1, 0.0 if phi_wall is None else float(phi_wall)))
 
     def set_storage(self, mode):
         self._ck(lib.lb_set_storage(self.h, {"ab": 0, "aa": 1}.get(mode, mode)))

@@ -565,3 +565,85 @@ def test_moving_walls_parity(lbmod, lbo, model, storage):
     ref.set_geometry(w.solid); ref.set_body_force(*w.g); ref.init(w.rho_r, w.rho_b, w.u)
     ref.step(5)
     assert np.abs(ref.get_populations(0) - sim.get_populations(0)).max() > 1e-6
+
+
+@pytest.mark.parametrize("forcing", ["guo", "edm"])
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_symmetric_probe_and_wetting_parity(lbmod, lbo, storage, forcing):
+    """Colour-symmetric near-contact probe (G29) and prescribed phi at solid nodes (G30) against the
+    oracle: populations after 1, 2 and 5 steps and the velocity of lb_get_macros (which repeats
+    the probe), walls, body force and two taus on; both options change the result."""
+    w = _random_workload(36, 13, 10, seed=61, walls=True, A_nc=0.05)
+    fluid = w.solid == 0
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    sim.set_storage(storage)
+    for obj in (o, sim):
+        obj.set_geometry(w.solid)
+        obj.set_body_force(*w.g)
+        obj.set_forcing(forcing)
+        obj.set_nc_symmetric(True)
+        obj.set_wall_phi(0.4)
+        obj.init(w.rho_r, w.rho_b, w.u)
+    h = o.get_fields()["h"]
+    assert ((h & 15) > 0).sum() > 20 and ((h >> 4) > 0).sum() > 20          # both probes fire
+    risky = np.zeros(w.shape, bool)
+    done = 0
+    for n in (1, 2, 5):
+        for _ in range(n - done):
+            risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+            o.step(1); sim.step(1)
+        done = n
+        e = pu.pop_error(sim, o)
+        assert e[~risky & fluid].max() < pu.POP_TOL, (n, e[~risky & fluid].max())
+    now_risky = pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1) | risky
+    _, _, u_o = o.get_macros()
+    _, _, u_g = sim.get_macros()
+    assert np.abs(u_g - u_o)[:, ~now_risky & fluid].max() < 1e-5
+    assert risky[fluid].mean() < 0.5
+    # each option alone changes the result
+    for kw in ({"sym": False, "wet": 0.4}, {"sym": True, "wet": None}):
+        ref = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+        ref.set_storage(storage)
+        ref.set_geometry(w.solid); ref.set_body_force(*w.g); ref.set_forcing(forcing)
+        ref.set_nc_symmetric(kw["sym"]); ref.set_wall_phi(kw["wet"])
+        ref.init(w.rho_r, w.rho_b, w.u)
+        ref.step(5)
+        assert np.abs(ref.get_populations(0) - sim.get_populations(0)).max() > 1e-6, kw
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_colour_exchange_invariance_on_gpu(lbmod, storage):
+    """With the symmetric probe and phi_wall -> -phi_wall the CUDA path is invariant under the
+    exchange of the two fluids up to fp32 rounding (the stored pair {f - w, f^r} is not symmetric
+    in r and b); with the one-sided probe it is not."""
+    n = 16
+    z, y, x = np.meshgrid(*(np.arange(n),) * 3, indexing="ij")
+    k = 2 * np.pi / n
+    s = (np.sin(2 * k * x + 0.3) * np.cos(k * y) + np.sin(2 * k * y + 1.1) * np.cos(2 * k * z + 0.5)
+         + 0.7 * np.sin(3 * k * z + k * x))
+    phi = 0.98 * np.tanh(2.0 * s)
+    u0 = (0.01 * np.stack([np.sin(k * y), np.sin(k * z), np.sin(k * x)])).astype(np.float32)
+    solid = np.zeros((n, n, n), np.uint8)
+    solid[:, 0, :] = 1
+    fluid = solid == 0
+
+    def run(swap, sym):
+        tr, tb = (1.2, 0.8) if swap else (0.8, 1.2)
+        sim = lbmod.LB(n, n, n, tr, tb, 0.01, 0.7, 0.05)
+        sim.set_storage(storage)
+        sim.set_geometry(solid)
+        sim.set_nc_symmetric(sym)
+        sim.set_wall_phi(-0.3 if swap else 0.3)
+        p = -phi if swap else phi
+        sim.init(((1 + p) / 2).astype(np.float32), ((1 - p) / 2).astype(np.float32), u0)
+        sim.step(20)
+        return sim.get_macros()
+
+    a_r, a_b, a_u = run(False, True)
+    b_r, b_b, b_u = run(True, True)
+    assert np.abs(a_r - b_b)[fluid].max() < 2e-5 and np.abs(a_b - b_r)[fluid].max() < 2e-5
+    assert np.abs(a_u - b_u)[:, fluid].max() < 2e-5
+    c_r, _, _ = run(False, False)
+    _, d_b, _ = run(True, False)
+    assert np.abs(c_r - d_b)[fluid].max() > 1e-3

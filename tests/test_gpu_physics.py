@@ -141,3 +141,37 @@ def test_taylor_green_decay_on_gpu(lbmod):
     _, _, u = sim.get_macros()
     ratio = float((u.astype(np.float64) ** 2).sum() / (w.u.astype(np.float64) ** 2).sum())
     assert 0.5 < ratio <= 0.886 * 1.02, ratio
+
+
+def test_contact_angle_follows_wall_phi(lbmod):
+    """Wetting (G30) on the CUDA path itself: a red half-cylinder on the lower wall relaxes to the
+    static angle cos(theta) ~= phi_wall (within 0.2, spacing within 0.1 of 0.5, as pin P17 of the
+    oracle)."""
+    nx, ny, nz, R = 64, 26, 4, 10.0
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 1
+    solid[:, -1, :] = 1
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    d = np.sqrt((x - nx / 2 + 0.5) ** 2 + (y - 0.5) ** 2)
+    phi = np.broadcast_to(np.tanh((R - d) / 1.5), (nz, ny, nx))
+
+    def crossing(v):
+        i = int(np.where((v[:-1] > 0) & (v[1:] <= 0))[0][0])
+        return i + v[i] / (v[i] - v[i + 1])
+
+    cos = {}
+    for pw in (-0.5, 0.0, 0.5):
+        sim = lbmod.LB(nx, ny, nz, 1.0, 1.0, 0.01, 0.7, 0.0)
+        sim.set_geometry(solid)
+        sim.set_wall_phi(pw)
+        sim.init(((1 + phi) / 2).astype(np.float32), ((1 - phi) / 2).astype(np.float32),
+                 np.zeros((3, nz, ny, nx), np.float32))
+        sim.step(4000)
+        rr, rb, _ = sim.get_macros()
+        p = ((rr - rb) / np.where(rr + rb > 0, rr + rb, 1.0))[1]
+        H = crossing(0.5 * (p[1:-1, nx // 2 - 1] + p[1:-1, nx // 2])) + 0.5
+        B = 2.0 * (crossing(p[1, nx // 2:]) + 0.5)
+        cos[pw] = float(np.cos(2.0 * np.arctan(2.0 * H / B)))
+    for pw, c in cos.items():
+        assert abs(c - pw) < 0.2, cos
+    assert abs((cos[0.0] - cos[-0.5]) - 0.5) < 0.1 and abs((cos[0.5] - cos[0.0]) - 0.5) < 0.1, cos
