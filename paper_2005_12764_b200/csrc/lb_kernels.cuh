@@ -799,7 +799,7 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
 // step (template MODE).  A solid source contributes nothing here: its link bounced back inside
 // k_fused.  Interior sites read 8 bytes.  Writes phi with its periodic ghost images like k_phase.
 template <int MODE, bool HAS_SOLID, bool SC>
-__global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
+__global__ void __launch_bounds__(TX* TY, 8) k_phase_fwd(const StepParams p) {
   // Four consecutive x sites per thread (128-bit loads and stores).  CTA = 32 quads x TY rows of
   // one plane (four k_fused tiles side by side), so that a warp is one row: the rows on a brick
   // face gather as whole warps and the others skip that code.  nx % 4 == 0: a quad is inside the
@@ -830,6 +830,7 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
   if (xm) { const float2 v = __ldg(ex + (tile == 0 ? ntx - 1 : tile - 1) * 2 + 1); d[0] += v.x; t[0] += v.y; }
   if (xp) { const float2 v = __ldg(ex + (tile == ntx - 1 ? 0 : tile + 1) * 2 + 0); d[3] += v.x; t[3] += v.y; }
   bool solid[4] = {false, false, false, false};
+  float sent[4] = {PHI_SOLID, PHI_SOLID, PHI_SOLID, PHI_SOLID};   // sentinel of a solid site: 1e30 x wall group
   // solid bits of the quad's own sites: x % 4 == 0, so the four bits sit in one mask word
   auto quad_bits = [&](int yy, int zz) -> uint32_t {
     return (b.mask[(size_t)(zz * b.ny + yy) * b.nxw + (x >> 5)] >> (x & 31)) & 0xfu;
@@ -838,6 +839,10 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
     const uint32_t m = quad_bits(y, z);
 #pragma unroll
     for (int e = 0; e < 4; ++e) solid[e] = (m >> e) & 1u;
+    if (b.gmask != nullptr && m != 0u) {     // moving walls somewhere in the box, and a solid site here
+#pragma unroll
+      for (int e = 0; e < 4; ++e) sent[e] = PHI_SOLID * (float)wall_group_at(b, x + e, y, z);
+    }
   }
   if (ym || yp || zm || zp) {
     // sources in another row range or z chunk are gathered from the stored populations with the
@@ -898,9 +903,9 @@ __global__ void __launch_bounds__(TX* TY) k_phase_fwd(const StepParams p) {
     for (int e = 0; e < 4; ++e) {
       const float rho = 1.0f + t[e];
       if constexpr (!SC) {
-        f0[e] = solid[e] ? PHI_SOLID * (float)wall_group_at(b, x + e, y, z) : d[e] / rho;
+        f0[e] = solid[e] ? sent[e] : d[e] / rho;
       } else {
-        f0[e] = solid[e] ? PHI_SOLID * (float)wall_group_at(b, x + e, y, z) : 0.5f * (rho + d[e]);
+        f0[e] = solid[e] ? sent[e] : 0.5f * (rho + d[e]);
         f1[e] = solid[e] ? 0.f : 0.5f * (rho - d[e]);
       }
     }
