@@ -29,7 +29,8 @@
 // twin, P13 Taylor-Green decay.
 // P14 exact-difference forcing, P15 Couette flow between sliding walls (G28), P16 colour-exchange
 // symmetry of the symmetric probe (G29), P17 wetting: symmetry, neutrality and monotone contact
-// angle (G30); SC1-SC5 for the second model.
+// angle (G30), P18 open boundaries: plug flow fixed point, pressure-driven Poiseuille, mass balance
+// (G31); SC1-SC5 for the second model.
 // PARITY UNPINNED against the paper (pinned only against DESIGN.md's reading): the discrete
 // contact search (G10), H_MAX, the wall rule for phi (G8, G30), the guard eps (G7).
 //
@@ -80,6 +81,9 @@ struct Oracle {
   bool any_solid = false;
   std::vector<uint8_t> solid;            // S, 0 = fluid, 1 = wall at rest, 2 / 3 = walls moving with uw[2] / uw[3]
   double uw[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // wall velocities by group (G28)
+  int wtype[4] = {0, 0, 0, 0};           // group 2 / 3: 0 = moving wall, 1 = velocity inlet, 2 = reservoir, 3 = pressure outlet (G31)
+  double wrho[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};             // prescribed rho_r, rho_b of an inlet / outlet
+  std::vector<double> uex, uey, uez;     // velocity that entered f^eq in the last collision (outlet rule, G31)
   std::vector<double> f[2], fpost[2];    // [k][site*19 + i], pre- and post-collision
   std::vector<double> rho_r, rho_b, phi; // per site (S1)
   std::vector<double> mx, my, mz;        // bare momentum (S1)
@@ -252,6 +256,7 @@ void collide_at(Oracle& o, int x, int y, int z) {
   const double ux = (o.mx[s] + hs * Fx) / rho;
   const double uy = (o.my[s] + hs * Fy) / rho;
   const double uz = (o.mz[s] + hs * Fz) / rho;
+  o.uex[s] = ux; o.uey[s] = uy; o.uez[s] = uz;
   // S5: relaxation rate. Eq. 8, then omega = 1/(3 nu + 1/2) which is Eq. 4
   // PAPER.md:102 inverted (the minus sign printed in Eq. 7 contradicts Eq. 4: G1).
   double omega;
@@ -320,10 +325,33 @@ void stream(Oracle& o) {
               // half-way bounce-back at a wall moving with u_w ("solid walls with opposite speeds
               // +-U"; rule: reading G28): the reflected population gains
               // 2 w_i rho^k (c_i . u_w) / c_s^2 = 6 w_i rho^k (c_i . u_w), rho^k the site's density
-              const double* uw = o.uw[o.solid[n]];
+              const int g = o.solid[n];
+              const double* uw = o.uw[g];
               const double cu = CX[i] * uw[0] + CY[i] * uw[1] + CZ[i] * uw[2];
-              const double rk = k == 0 ? o.rho_r[s] : o.rho_b[s];
-              o.f[k][s * Q + i] = o.fpost[k][s * Q + OPP[i]] + 6.0 * W[i] * rk * cu;
+              if (o.wtype[g] >= 2) {
+                // open boundaries (G31; the flow focuser's outlet, rule not given):
+                // pressure outlet by anti-bounce-back,
+                // f^k_i(x, t+1) = -f^k*_opp(i)(x, t) + 2 w_i rho^k_out [1 + 4.5 (c_i.u)^2 - 1.5 u.u],
+                // u = the velocity that entered f^eq at x in this step
+                const double vx = o.uex[s], vy = o.uey[s], vz = o.uez[s];
+                const double cv = CX[i] * vx + CY[i] * vy + CZ[i] * vz;
+                const double E = 1.0 + 4.5 * cv * cv - 1.5 * (vx * vx + vy * vy + vz * vz);
+                // type 2 (reservoir): rho^k_out as prescribed.  Type 3 (outflow): only the total is
+                // prescribed, the composition is the boundary node's own,
+                // rho^k_out = (rho_r + rho_b)_prescribed rho^k(x) / rho(x)
+                double rk_out = o.wrho[g][k];
+                if (o.wtype[g] == 3) {
+                  const double rk = k == 0 ? o.rho_r[s] : o.rho_b[s];
+                  const double rho = o.two ? o.rho_r[s] + o.rho_b[s] : o.rho_r[s];
+                  rk_out = (o.wrho[g][0] + o.wrho[g][1]) * rk / rho;
+                }
+                o.f[k][s * Q + i] = -o.fpost[k][s * Q + OPP[i]] + 2.0 * W[i] * rk_out * E;
+              } else {
+                // type 1, velocity inlet: the same rule with the prescribed densities of the
+                // incoming fluid in place of the site's own (G31)
+                const double rk = o.wtype[g] == 1 ? o.wrho[g][k] : (k == 0 ? o.rho_r[s] : o.rho_b[s]);
+                o.f[k][s * Q + i] = o.fpost[k][s * Q + OPP[i]] + 6.0 * W[i] * rk * cu;
+              }
             }
           }
         }
@@ -364,6 +392,7 @@ void collide_sc_at(Oracle& o, int x, int y, int z) {
   o.Fy[s] = rr * ar[1] + rb * ab[1];
   o.Fz[s] = rr * ar[2] + rb * ab[2];
   const double ux = o.mx[s] / rho, uy = o.my[s] / rho, uz = o.mz[s] / rho;
+  o.uex[s] = ux; o.uey[s] = uy; o.uez[s] = uz;
   double omega;
   if (o.tau_r == o.tau_b) {
     omega = 1.0 / o.tau_r;
@@ -448,7 +477,7 @@ int lbo_create(int nx, int ny, int nz, const double* params, void** out) {
   try {
     o->solid.assign(o->S, 0);
     for (auto* v : {&o->rho_r, &o->rho_b, &o->phi, &o->mx, &o->my, &o->mz, &o->Fx, &o->Fy, &o->Fz,
-                    &o->Gx, &o->Gy, &o->Gz, &o->margin})
+                    &o->Gx, &o->Gy, &o->Gz, &o->margin, &o->uex, &o->uey, &o->uez})
       v->assign(o->S, 0.0);
     o->hcontact.assign(o->S, 0);
   } catch (...) {
@@ -478,6 +507,20 @@ int lbo_set_wall_velocity(void* h, int group, double ux, double uy, double uz) {
   Oracle* o = static_cast<Oracle*>(h);
   if (!o || (group != 2 && group != 3)) return LBO_EINVAL;
   o->uw[group][0] = ux; o->uw[group][1] = uy; o->uw[group][2] = uz;
+  return LBO_OK;
+}
+
+// What a wall group (2 or 3) is (G31): 0 = moving wall (default; lbo_set_wall_velocity), 1 =
+// velocity inlet (wall velocity = inflow velocity, prescribed densities rho_r, rho_b of the
+// incoming fluid), 2 = pressure boundary with both densities prescribed (a reservoir), 3 = pressure
+// outlet: rho_r + rho_b prescribes the total density, the composition is that of the outgoing
+// fluid.  The wall velocity is not used by types 2 and 3.
+int lbo_set_wall_type(void* h, int group, int type, double rho_r, double rho_b) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || (group != 2 && group != 3) || type < 0 || type > 3) return LBO_EINVAL;
+  if (type != 0 && (!(rho_r >= 0.0) || !(rho_b >= 0.0))) return LBO_EINVAL;
+  o->wtype[group] = type;
+  o->wrho[group][0] = rho_r; o->wrho[group][1] = rho_b;
   return LBO_OK;
 }
 

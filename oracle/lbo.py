@@ -41,6 +41,7 @@ def _load():
         lib.lbo_set_nc_cutoff.argtypes = [vp, C.c_double]
         lib.lbo_set_nc_mode.argtypes = [vp, C.c_int]
         lib.lbo_set_nc_symmetric.argtypes = [vp, C.c_int]
+        lib.lbo_set_wall_type.argtypes = [vp, C.c_int, C.c_int, C.c_double, C.c_double]
         lib.lbo_set_wall_phi.argtypes = [vp, C.c_int, C.c_double]
         lib.lbo_set_forcing.argtypes = [vp, C.c_int]
         lib.lbo_set_model.argtypes = [vp, C.c_int, C.c_double]
@@ -112,6 +113,12 @@ class Oracle:
     def set_wall_velocity(self, group, ux, uy, uz):
         """Velocity of the walls whose mask value is `group` (2 or 3)."""
         self._ck(self.lib.lbo_set_wall_velocity(self.h, group, ux, uy, uz), "lbo_set_wall_velocity")
+
+    def set_wall_type(self, group, kind, rho_r=0.0, rho_b=0.0):
+        """'wall' (moving wall), 'inlet' (velocity inlet), 'reservoir' (pressure boundary, both densities
+        prescribed) or 'outlet' (pressure outlet, total density prescribed), G31."""
+        t = {'wall': 0, 'inlet': 1, 'reservoir': 2, 'outlet': 3}.get(kind, kind)
+        self._ck(self.lib.lbo_set_wall_type(self.h, group, t, float(rho_r), float(rho_b)), "lbo_set_wall_type")
 
     def set_body_force(self, gx, gy, gz):
         self._ck(self.lib.lbo_set_body_force(self.h, gx, gy, gz), "lbo_set_body_force")

@@ -619,3 +619,116 @@ def test_P17_contact_angle(lbo):
     for pw, c in cos.items():
         assert abs(c - pw) < 0.2, cos
     assert abs((cos[0.0] - cos[-0.5]) - 0.5) < 0.1 and abs((cos[0.5] - cos[0.0]) - 0.5) < 0.1, cos
+
+
+# ---------------------------------------------------------------------------------- P18
+def _open_channel_mask(nx, ny, nz, walls):
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    if walls:
+        solid[:, 1:-1, 0] = 2
+        solid[:, 1:-1, -1] = 3
+        solid[:, 0, :] = 1
+        solid[:, -1, :] = 1
+    else:
+        solid[:, :, 0] = 2
+        solid[:, :, -1] = 3
+    return solid
+
+
+@pytest.mark.parametrize("exit_kind", ["reservoir", "outlet"])
+@pytest.mark.parametrize("two", [False, True])
+def test_P18_plug_flow_is_a_fixed_point(lbo, two, exit_kind):
+    """Open boundaries (G31).  A uniform flow u = (U, 0, 0) at the prescribed densities is an exact
+    fixed point of velocity inlet + pressure boundary: f^eq_i - f^eq_opp(i) = 6 w_i rho (c_i.u) and
+    f^eq_i + f^eq_opp(i) = 2 w_i rho [1 + 4.5 (c_i.u)^2 - 1.5 u.u] (Eq. 2).  A wrong
+    sign, factor or direction index in either rule breaks it."""
+    nx, ny, nz, U = 12, 5, 4, 0.03
+    solid = _open_channel_mask(nx, ny, nz, walls=False)
+    o = lbo.Oracle(nx, ny, nz, 0.8, 1.1 if two else 0.8, 0.0, 0.0, 0.0)
+    o.set_geometry(solid)
+    o.set_wall_velocity(2, U, 0.0, 0.0)
+    rr0, rb0 = (0.7, 0.4) if two else (1.1, 0.0)
+    o.set_wall_type(2, "inlet", rr0, rb0)
+    o.set_wall_type(3, exit_kind, rr0, rb0)
+    ones = np.ones((nz, ny, nx))
+    u0 = np.zeros((3, nz, ny, nx))
+    u0[0] = U
+    o.init(rr0 * ones, rb0 * ones if two else None, u0)
+    o.step(50)
+    rr, rb, u = o.get_macros()
+    fl = solid == 0
+    assert np.abs(rr[fl] - rr0).max() < 1e-13 and np.abs(u[0][fl] - U).max() < 1e-13
+    assert np.abs(u[1:]).max() < 1e-14
+    if two:
+        assert np.abs(rb[fl] - rb0).max() < 1e-13
+
+
+def test_P18_pressure_driven_poiseuille(lbo):
+    """Two reservoirs at rho_hi and rho_lo (p = rho / 3) drive plane Poiseuille flow between walls:
+    u_x(y) = -(dp/dx) y' (H - y') / (2 rho nu).  With the nominal gradient (rho_hi - rho_lo)/(3 L),
+    L = nx - 2, the peak is met within 8 % (the end effect of the two boundary columns is about two
+    lattice units in 32; 1.5 % at L = 128); with the density gradient measured mid-channel within
+    1 %.  The flow runs from high to low pressure and the mass flux is the same through every
+    cross-section."""
+    from threadpoolctl import threadpool_limits
+    nx, ny, nz, tau = 34, 18, 1, 1.0
+    nu = (tau - 0.5) / 3.0
+    solid = _open_channel_mask(nx, ny, nz, walls=True)
+    rhi, rlo = 1.002, 0.998
+    o = lbo.Oracle(nx, ny, nz, tau, tau, 0.0, 0.0, 0.0)
+    o.set_geometry(solid)
+    o.set_wall_type(2, "reservoir", 0.6 * rhi, 0.4 * rhi)
+    o.set_wall_type(3, "reservoir", 0.6 * rlo, 0.4 * rlo)
+    ones = np.ones((nz, ny, nx))
+    with threadpool_limits(limits=1, user_api="openmp"):
+        o.init(0.6 * ones, 0.4 * ones, np.zeros((3, nz, ny, nx)))
+        o.step(8000)
+    rr, rb, u = o.get_macros()
+    rho = rr + rb
+    L, H = nx - 2, ny - 2
+    y = np.arange(ny) - 0.5
+    shape = y * (H - y) / (2.0 * nu)
+    xm = nx // 2
+    prof = u[0][0, 1:-1, xm]
+    nominal = (rhi - rlo) / 3.0 / L * shape[1:-1]
+    assert prof.min() > 0                                                   # from high to low pressure
+    assert abs(prof.max() / nominal.max() - 1.0) < 0.08
+    grad = (rho[0, 1:-1, xm - 4].mean() - rho[0, 1:-1, xm + 4].mean()) / 8.0 / 3.0
+    local = grad / rho[0, 1:-1, xm].mean() * shape[1:-1]
+    assert np.abs(prof - local).max() / local.max() < 0.01
+    flux = (rho * u[0])[0, 1:-1, 1:-1].sum(axis=0)
+    assert np.abs(flux / flux.mean() - 1.0).max() < 1e-9
+    assert np.abs(rr / np.where(rho > 0, rho, 1.0) - 0.6)[solid == 0].max() < 1e-12   # uniform composition stays
+
+
+def test_P18_inlet_outlet_mass_balance(lbo):
+    """Velocity inlet (red-rich fluid, plug profile U) and pressure outlet in a walled channel.  In
+    the steady state the mass flux through every cross-section equals what the inlet links inject,
+    rho_in U (H - 1/3) exactly (each inlet link adds 6 w_i rho_in U; the two corner nodes lack one
+    diagonal link each: 2 x 6/36); the outlet lets the composition of the incoming fluid through
+    (red flux = 0.7 of the total), the profile develops into the parabola."""
+    from threadpoolctl import threadpool_limits
+    nx, ny, nz, U = 50, 14, 1, 0.02
+    solid = _open_channel_mask(nx, ny, nz, walls=True)
+    o = lbo.Oracle(nx, ny, nz, 0.9, 0.9, 0.0, 0.0, 0.0)
+    o.set_geometry(solid)
+    o.set_wall_velocity(2, U, 0.0, 0.0)
+    o.set_wall_type(2, "inlet", 0.7, 0.3)
+    o.set_wall_type(3, "outlet", 0.5, 0.5)
+    ones = np.ones((nz, ny, nx))
+    with threadpool_limits(limits=1, user_api="openmp"):
+        o.init(0.5 * ones, 0.5 * ones, np.zeros((3, nz, ny, nx)))
+        o.step(12000)
+    rr, rb, u = o.get_macros()
+    rho = rr + rb
+    H = ny - 2
+    flux = (rho * u[0])[0, 1:-1, 1:-1].sum(axis=0)
+    assert np.abs(flux - 1.0 * U * (H - 1.0 / 3.0)).max() < 1e-10
+    red = (rr * u[0])[0, 1:-1, 1:-1].sum(axis=0)
+    assert np.abs(red - 0.7 * U * (H - 1.0 / 3.0)).max() < 1e-4
+    assert abs(rr[0, 6, -2] / rho[0, 6, -2] - 0.7) < 1e-3                    # still converging (4e-5 at 12000 steps)
+    y = np.arange(ny) - 0.5
+    x = nx - 8
+    umean = flux[x - 1] / H / rho[0, 1:-1, x].mean()
+    para = 6.0 * umean * y[1:-1] * (H - y[1:-1]) / H ** 2
+    assert np.abs(u[0][0, 1:-1, x] / para - 1.0).max() < 0.025
