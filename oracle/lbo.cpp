@@ -79,10 +79,10 @@ struct Oracle {
   bool two = true;
   bool inited = false;
   bool any_solid = false;
-  std::vector<uint8_t> solid;            // S, 0 = fluid, 1 = wall at rest, 2 / 3 = walls moving with uw[2] / uw[3]
-  double uw[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // wall velocities by group (G28)
-  int wtype[4] = {0, 0, 0, 0};           // group 2 / 3: 0 = moving wall, 1 = velocity inlet, 2 = reservoir, 3 = pressure outlet (G31)
-  double wrho[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};             // prescribed rho_r, rho_b of an inlet / outlet
+  std::vector<uint8_t> solid;            // S, 0 = fluid, 1 = wall at rest, 2 / 3 / 4 = walls moving with uw[2] / uw[3] / uw[4]
+  double uw[5][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // wall velocities by group (G28)
+  int wtype[5] = {0, 0, 0, 0, 0};        // group 2 / 3 / 4: 0 = moving wall, 1 = velocity inlet, 2 = reservoir, 3 = pressure outlet (G31)
+  double wrho[5][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}};             // prescribed rho_r, rho_b of an inlet / outlet
   std::vector<double> uex, uey, uez;     // velocity that entered f^eq in the last collision (outlet rule, G31)
   std::vector<double> f[2], fpost[2];    // [k][site*19 + i], pre- and post-collision
   std::vector<double> rho_r, rho_b, phi; // per site (S1)
@@ -496,28 +496,29 @@ int lbo_set_geometry(void* h, const uint8_t* mask) {
   if (o->inited) return LBO_ESTATE;
   o->any_solid = false;
   for (size_t s = 0; s < o->S; ++s) {
-    o->solid[s] = mask ? (mask[s] > 3 ? 1 : mask[s]) : 0;   // 0 fluid, 1 wall at rest, 2 / 3 moving wall groups
+    o->solid[s] = mask ? (mask[s] > 4 ? 1 : mask[s]) : 0;   // 0 fluid, 1 wall at rest, 2 / 3 / 4 wall groups (three: the flow
+                                                            // focuser has two kinds of inlet and an outlet; G31)
     o->any_solid |= o->solid[s] != 0;
   }
   return LBO_OK;
 }
 
-// velocity of the walls whose mask value is `group` (2 or 3); walls with mask value 1 are at rest
+// velocity of the walls whose mask value is `group` (2, 3 or 4); walls with mask value 1 are at rest
 int lbo_set_wall_velocity(void* h, int group, double ux, double uy, double uz) {
   Oracle* o = static_cast<Oracle*>(h);
-  if (!o || (group != 2 && group != 3)) return LBO_EINVAL;
+  if (!o || group < 2 || group > 4) return LBO_EINVAL;
   o->uw[group][0] = ux; o->uw[group][1] = uy; o->uw[group][2] = uz;
   return LBO_OK;
 }
 
-// What a wall group (2 or 3) is (G31): 0 = moving wall (default; lbo_set_wall_velocity), 1 =
+// What a wall group (2, 3 or 4) is (G31): 0 = moving wall (default; lbo_set_wall_velocity), 1 =
 // velocity inlet (wall velocity = inflow velocity, prescribed densities rho_r, rho_b of the
 // incoming fluid), 2 = pressure boundary with both densities prescribed (a reservoir), 3 = pressure
 // outlet: rho_r + rho_b prescribes the total density, the composition is that of the outgoing
 // fluid.  The wall velocity is not used by types 2 and 3.
 int lbo_set_wall_type(void* h, int group, int type, double rho_r, double rho_b) {
   Oracle* o = static_cast<Oracle*>(h);
-  if (!o || (group != 2 && group != 3) || type < 0 || type > 3) return LBO_EINVAL;
+  if (!o || group < 2 || group > 4 || type < 0 || type > 3) return LBO_EINVAL;
   if (type != 0 && (!(rho_r >= 0.0) || !(rho_b >= 0.0))) return LBO_EINVAL;
   o->wtype[group] = type;
   o->wrho[group][0] = rho_r; o->wrho[group][1] = rho_b;

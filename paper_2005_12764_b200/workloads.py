@@ -223,6 +223,59 @@ def c5_emulsion(n=640, ndrops=3000, rmin=8.0, rmax=14.0, gap=3.0, steps=1000, in
                     info=dict(droplets=int(len(radii)), red_fraction=frac))
 
 
+def focuser(nx=96, ny=48, nz=1, wd=10, wc=12, t=4, li=24, wo=10, lo=8, u_d=0.01, u_c=0.01,
+            tau=1.0, A=0.01, beta=0.7, A_nc=0.0, walls_z=False, steps=2000):
+    """Flow-focusing device (Fig. 4): a dispersed (red) inlet of width wd between
+    two continuous (blue) inlets of width wc, all on the x = 0 plane and kept apart by dividers of
+    thickness t and length li, an orifice of width wo and length lo behind the junction, and an
+    outlet chamber that ends in a pressure outlet on the x = nx-1 plane.  alpha = u_d / (2 u_c) as
+    in the paper.  The device dimensions are NOT in the paper: these are stand-ins.
+
+    Mask values: 1 wall at rest, 2 dispersed inlet, 3 continuous inlets, 4 outlet; what the groups
+    are is in info["wall_groups"] and set on an Oracle or an LB by configure_walls()."""
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 1
+    solid[:, -1, :] = 1
+    if walls_z:
+        solid[0] = 1
+        solid[-1] = 1
+    y0d = (ny - wd) // 2
+    y1d = y0d + wd
+    solid[:, y0d - t:y0d, :li] = 1
+    solid[:, y1d:y1d + t, :li] = 1
+    # the continuous inlets reach from the dividers wc sites outwards, the rest of the face is wall
+    lo_c, hi_c = max(1, y0d - t - wc), min(ny - 1, y1d + t + wc)
+    solid[:, 1:lo_c, :li] = 1
+    solid[:, hi_c:ny - 1, :li] = 1
+    xo = li + max(wd, wc)
+    y0o = (ny - wo) // 2
+    solid[:, 1:y0o, xo:xo + lo] = 1
+    solid[:, y0o + wo:ny - 1, xo:xo + lo] = 1
+    face = solid[:, :, 0] == 0
+    yy = np.broadcast_to(np.arange(ny)[None, :], (nz, ny))
+    solid[:, :, 0] = np.where(face, np.where((yy >= y0d) & (yy < y1d), 2, 3), solid[:, :, 0])
+    solid[:, :, -1] = np.where(solid[:, :, -1] == 0, 4, solid[:, :, -1])
+    # red fills the dispersed channel up to the junction, blue everything else
+    x = np.arange(nx, dtype=np.float64)[None, None, :]
+    y = np.arange(ny, dtype=np.float64)[None, :, None]
+    phi = np.tanh((li - 2.0 - x) / 2.0) * np.ones((nz, 1, 1))
+    phi = np.where((y >= y0d) & (y < y1d), phi, -1.0)
+    rr, rb = _from_phi(phi.astype(np.float32))
+    walls = {2: dict(kind="inlet", u=(u_d, 0.0, 0.0), rho=(1.0, 0.0)),
+             3: dict(kind="inlet", u=(u_c, 0.0, 0.0), rho=(0.0, 1.0)),
+             4: dict(kind="outlet", u=(0.0, 0.0, 0.0), rho=(0.5, 0.5))}
+    return Workload("focuser", nx, ny, nz, tau, tau, A, beta, A_nc, rr, rb,
+                    np.zeros((3, nz, ny, nx), np.float32), solid=solid, steps=steps,
+                    info=dict(alpha=u_d / (2.0 * u_c), wall_groups=walls, li=li, xo=xo, wd=wd, wc=wc))
+
+
+def configure_walls(obj, w):
+    """Apply info["wall_groups"] of a workload to an oracle or an LB (same method names on both)."""
+    for group, d in sorted(w.info.get("wall_groups", {}).items()):
+        obj.set_wall_velocity(group, *d["u"])
+        obj.set_wall_type(group, d["kind"], *d["rho"])
+
+
 def get(name):
     """Workloads by name: full configs c1..c5 and the parity minis."""
     table = {
@@ -235,5 +288,8 @@ def get(name):
         "c3-mini": lambda: c3_spinodal(64, steps=100),
         "c4-mini": lambda: c4_channel(128, 32, 32, R=6.0, steps=100),
         "c5-mini": lambda: c5_emulsion(96, 8, steps=100),
+        "focuser": focuser,
+        "focuser-3d": lambda: focuser(256, 96, 48, wd=20, wc=24, t=6, li=48, wo=20, lo=16, walls_z=True,
+                                      A_nc=0.02, steps=20000),
     }
     return table[name]()

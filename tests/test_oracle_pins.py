@@ -732,3 +732,66 @@ def test_P18_inlet_outlet_mass_balance(lbo):
     umean = flux[x - 1] / H / rho[0, 1:-1, x].mean()
     para = 6.0 * umean * y[1:-1] * (H - y[1:-1]) / H ** 2
     assert np.abs(u[0][0, 1:-1, x] / para - 1.0).max() < 0.025
+
+
+# ---------------------------------------------------------------------------------- P19
+def _inlet_link_rate(solid, group, u_in, rho_in):
+    """Mass a velocity inlet injects per step, counted link by link from the mask alone: every link
+    i that arrives at a fluid site from a node of `group` gains 6 w_i rho_in (c_i . u_in) (G31)."""
+    total = 0.0
+    nz, ny, nx = solid.shape
+    for i in range(1, 19):
+        c = tw.C[i]
+        src = np.roll(solid, shift=(c[2], c[1], c[0]), axis=(0, 1, 2))     # src[s] = solid[s - c_i]
+        n = np.count_nonzero((solid == 0) & (src == group))
+        total += n * 6.0 * tw.WT[i] * rho_in * float(np.dot(c, u_in))
+    return total
+
+
+def test_P19_focuser_three_groups_and_exact_injection(lbo):
+    """Flow focuser: dispersed inlet, continuous inlets and outlet are three wall
+    groups (2, 3, 4; G31).  (a) Relabelling the groups together with their settings changes nothing,
+    bit for bit.  (b) While no red fluid has reached the outlet, the red mass grows per step by
+    exactly what the links out of the dispersed inlet inject, counted from the mask alone,
+    = u_d (w_d - 1/3) per plane; the blue inlets inject no red.  (c) The red front advances and
+    the total mass stays bounded (the outlet lets out what the inlets push in)."""
+    from paper_2005_12764_b200 import workloads as W
+    w = W.focuser()
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    o.set_geometry(w.solid)
+    W.configure_walls(o, w)
+    o.init(w.rho_r, w.rho_b, w.u)
+    # (a) the same device with the labels permuted 2 -> 4 -> 3 -> 2
+    perm = {2: 4, 4: 3, 3: 2}
+    solid2 = w.solid.copy()
+    for a, b in perm.items():
+        solid2[w.solid == a] = b
+    o2 = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    o2.set_geometry(solid2)
+    for g, d in w.info["wall_groups"].items():
+        o2.set_wall_velocity(perm[g], *d["u"])
+        o2.set_wall_type(perm[g], d["kind"], *d["rho"])
+    o2.init(w.rho_r, w.rho_b, w.u)
+    fl = w.solid == 0
+    rr0, rb0, _ = o.get_macros()
+    m0r, m0 = rr0[fl].sum(), (rr0 + rb0)[fl].sum()
+    o.step(40); o2.step(40)
+    for a, b in zip(o.get_macros(), o2.get_macros()):
+        assert np.array_equal(a, b)
+    # (b)
+    d = w.info["wall_groups"][2]
+    rate = _inlet_link_rate(w.solid, 2, d["u"], d["rho"][0])
+    assert abs(rate - d["u"][0] * (w.info["wd"] - 1.0 / 3.0) * w.nz) < 1e-15
+    rr, rb, u = o.get_macros()
+    assert rr[:, :, -8:].max() == 0.0                        # no red near the outlet yet
+    assert abs((rr[fl].sum() - m0r) - 40 * rate) < 1e-11
+    o.step(1460)
+    rr, rb, u = o.get_macros()
+    assert rr[:, :, -8:].max() < 1e-12
+    assert abs((rr[fl].sum() - m0r) - 1500 * rate) < 1e-9
+    # (c)
+    front0 = np.where((rr0 > rb0) & fl)[2].max()
+    front = np.where((rr > rb) & fl)[2].max()
+    assert front > front0 + 8
+    assert abs((rr + rb)[fl].sum() / m0 - 1.0) < 0.02
+    assert u[0][fl].min() > -5e-3 and np.isfinite(u).all()
