@@ -150,6 +150,8 @@ def oracle_sample_workload(name, budget_updates):
             return W.c5_emulsion(n, max(1, int(3000 * (n / 640.0) ** 3)))
         if name == "c1":
             return W.c1_droplet()
+        if name.startswith("focuser"):
+            return W.focuser(128, 48, 24, wd=10, wc=12, t=3, li=24, wo=10, lo=8, walls_z=True, A_nc=0.02)
         return W.c3_spinodal(n)
     best = 32
     for n in (32, 48, 64, 96, 128, 160):
@@ -168,6 +170,8 @@ def time_oracle(w, steps, warmup):
         o.set_geometry(w.solid)
     o.set_body_force(*w.g)
     o.set_nc_cutoff(w.phi_c)
+    from paper_2005_12764_b200 import workloads as W
+    W.configure_walls(o, w)
     o.init(w.rho_r, w.rho_b, w.u)
     if warmup:
         o.step(warmup)
@@ -359,7 +363,7 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--model", default="cg", choices=["cg", "sc"], help="cg = colour gradient (north_star), sc = Shan-Chen + exact difference (Eq. 5-10 of the paper)")

@@ -74,15 +74,29 @@ void lb_destroy(lb_handle h);
 /* CUDA stream (a cudaStream_t passed as void*) that all later work of this handle uses. */
 int lb_set_stream(lb_handle h, void* cuda_stream);
 
-/* Solid mask, S = nx*ny*nz bytes: 0 = fluid, 1 = wall at rest, 2 and 3 = walls moving with the
- * velocities of lb_set_wall_velocity (any other value counts as 1); NULL = all fluid.  Stored
+/* Solid mask, S = nx*ny*nz bytes: 0 = fluid, 1 = wall at rest, 2, 3 and 4 = wall groups: walls
+ * moving with the velocities of lb_set_wall_velocity or the open boundaries of lb_set_wall_type
+ * (any other value counts as 1); NULL = all fluid.  Stored
  * bit-packed.  Solid sites hold no populations; links into them bounce back half-way
  * (G21).  Must precede lb_init. */
 int lb_set_geometry(lb_handle h, const uint8_t* solid_mask);
 
-/* Velocity u_w of the walls of group 2 or 3 ("solid walls with opposite speeds +-U", PAPER.md:341,
+/* Velocity u_w of the walls of group 2, 3 or 4 ("solid walls with opposite speeds +-U", PAPER.md:341,
  * :367; G28): a population reflected at such a wall along link i loses 6 w_i rho^k (c_i . u_w). */
 int lb_set_wall_velocity(lb_handle h, int group, float ux, float uy, float uz);
+
+/* What the wall group 2, 3 or 4 is (G31; the two kinds of inlet and the outlet of the
+ * flow focuser, whose boundary rules the paper does not give).  type 0 (default) = moving
+ * wall.  1 = velocity inlet: the moving-wall rule with u_w = the inflow velocity
+ * (lb_set_wall_velocity) and the prescribed densities rho_r, rho_b of the incoming fluid in place
+ * of the site's own.  2 = reservoir (pressure boundary, both densities prescribed) by
+ * anti-bounce-back: f^k_opp(i)(x, t+1) = -f^k*_i(x, t) + 2 w_i rho^k_out [1 + 4.5 (c_i.u)^2 -
+ * 1.5 u.u], u = the velocity that entered f^eq at x in this step.  3 = pressure outlet: the same
+ * with rho^k_out = (rho_r + rho_b) rho^k(x) / rho(x), so that the composition of the outgoing
+ * fluid passes.  One component: rho_r is the density (type 3: rho_r + rho_b).  May be called at
+ * any time; acts from the next lb_step.  LB_EINVAL: group not 2..4, type not 0..3, a negative or
+ * NaN density. */
+int lb_set_wall_type(lb_handle h, int group, int type, float rho_r, float rho_b);
 
 /* Uniform acceleration g: body force F = rho g enters through the source term. */
 int lb_set_body_force(lb_handle h, float gx, float gy, float gz);

@@ -66,8 +66,10 @@ struct lb_handle_s {
   bool two = true;
   bool inited = false;
   bool has_solid = false;
-  bool has_moving = false;   // the mask holds wall groups 2 / 3 (moving walls)
-  float uw[2][3] = {{0, 0, 0}, {0, 0, 0}};   // their velocities
+  bool has_moving = false;   // the mask holds wall groups 2 / 3 / 4 (moving walls, open boundaries)
+  float uw[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // their velocities
+  int wtype[3] = {0, 0, 0};  // what they are (G31): 0 moving wall, 1 velocity inlet, 2 reservoir, 3 pressure outlet
+  float wrho[3][2] = {{0, 0}, {0, 0}, {0, 0}};       // prescribed rho_r, rho_b of an inlet / reservoir / outlet
   int aa_odd = 0;           // AA: is the next step the odd one?
   int cur = 0;              // A/B: buffer holding the current state
   float* buf[2] = {nullptr, nullptr};
@@ -184,7 +186,11 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
   p.has_g = (h->g[0] != 0.f || h->g[1] != 0.f || h->g[2] != 0.f);
   p.edm = h->forcing;
   p.has_moving = h->has_solid && h->has_moving;
-  for (int a = 0; a < 3; ++a) { p.uw2[a] = h->uw[0][a]; p.uw3[a] = h->uw[1][a]; }
+  for (int g = 0; g < 3; ++g) {
+    for (int a = 0; a < 3; ++a) p.uw[g][a] = h->uw[g][a];
+    p.wtype[g] = h->wtype[g];
+    p.wrho[g][0] = h->wrho[g][0]; p.wrho[g][1] = h->wrho[g][1];
+  }
   return p;
 }
 
@@ -491,8 +497,17 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
 }
 
 int lb_set_wall_velocity(lb_handle h, int group, float ux, float uy, float uz) {
-  if (!h || (group != 2 && group != 3)) return fail(h, LB_EINVAL, "wall group must be 2 or 3");
+  if (!h || group < 2 || group > 4) return fail(h, LB_EINVAL, "wall group must be 2, 3 or 4");
   h->uw[group - 2][0] = ux; h->uw[group - 2][1] = uy; h->uw[group - 2][2] = uz;
+  return LB_OK;
+}
+
+int lb_set_wall_type(lb_handle h, int group, int type, float rho_r, float rho_b) {
+  if (!h || group < 2 || group > 4) return fail(h, LB_EINVAL, "wall group must be 2, 3 or 4");
+  if (type < 0 || type > 3) return fail(h, LB_EINVAL, "wall type must be 0 (wall), 1 (inlet), 2 (reservoir) or 3 (outlet)");
+  if (type != 0 && (!(rho_r >= 0.f) || !(rho_b >= 0.f))) return fail(h, LB_EINVAL, "prescribed densities must be >= 0");
+  h->wtype[group - 2] = type;
+  h->wrho[group - 2][0] = rho_r; h->wrho[group - 2][1] = rho_b;
   return LB_OK;
 }
 

@@ -46,8 +46,10 @@ struct StepParams {
   int nc_sym;         // colour-symmetric near-contact probe (G29)
   int wet;            // solid nodes carry phi_wall in the colour-gradient stencil (G30)
   float phi_wall;
-  int has_moving;     // some walls move (mask groups 2, 3): half-way bounce-back with the wall velocity (G28)
-  float uw2[3], uw3[3];
+  int has_moving;     // some walls move (mask groups 2, 3, 4): half-way bounce-back with the wall velocity (G28)
+  float uw[3][3];     // velocities of groups 2, 3, 4
+  int wtype[3];       // what these groups are (G31): 0 moving wall, 1 velocity inlet, 2 reservoir, 3 pressure outlet
+  float wrho[3][2];   // prescribed rho_r, rho_b of an inlet / reservoir / outlet
   int sc;             // Shan-Chen model (Eq. 5-10 of the paper): the fields are rho_r, rho_b instead of phi
   float G_C;          // its coupling strength, positive = repulsive
 };
@@ -141,6 +143,37 @@ __device__ __forceinline__ float cdot(float ax, float ay, float az) {
   else return 0.0f;
 }
 
+// What a link q into a wall of group 2 + gi (gi = 0, 1, 2) sends back: the stored
+// post-collision pair {ts = f* - w, rs = f^r*} is replaced by what the site reads along opp(q) in
+// the next step.  Moving wall (G28): the reflected population loses 6 w_q rho^k (c_q . u_w), rho^k
+// the site's own densities; velocity inlet (G31, type 1): the same with the prescribed densities.
+// Reservoir / pressure outlet (G31, types 2 / 3; the flow focuser's open ends):
+// anti-bounce-back, f^k <- -f^k* + 2 w_q rho^k_out [1 + 4.5 (c_q.u)^2 - 1.5 u.u] with u the
+// velocity that entered f^eq; the outlet keeps the site's composition,
+// rho^k_out = (rho_r + rho_b)_prescribed rho^k / rho.  In deviation form the total becomes
+// -ts + 2 w_q [(rho_out - 1) + rho_out (4.5 (c.u)^2 - 1.5 u.u)].
+// ONE: single component, whose density is the prescribed rho_r (the outlet's: rho_r + rho_b).
+template <int q, bool ONE = false>
+__device__ __forceinline__ void open_link(const StepParams& p, int gi, float rho, float rr, float inv_rho,
+                                          float ux, float uy, float uz, float uu15, float& ts, float& rs) {
+  constexpr float w = wq(q);
+  const int wt = p.wtype[gi];
+  const float pr = p.wrho[gi][0], pb = p.wrho[gi][1];
+  if (wt >= 2) {
+    const float cu = cdot<q>(ux, uy, uz);
+    const float e1 = fmaf(4.5f * cu, cu, -uu15);
+    const float ro = (ONE && wt == 2) ? pr : pr + pb;
+    const float rro = wt == 3 ? ro * (rr * inv_rho) : pr;
+    ts = fmaf(2.0f * w, fmaf(ro, e1, ro - 1.0f), -ts);
+    rs = fmaf(2.0f * w * rro, 1.0f + e1, -rs);
+  } else {
+    const float cw = cdot<q>(p.uw[gi][0], p.uw[gi][1], p.uw[gi][2]);
+    const float rt = wt == 1 ? (ONE ? pr : pr + pb) : rho, r1 = wt == 1 ? pr : rr;
+    ts = fmaf(-6.0f * w * rt, cw, ts);
+    rs = fmaf(-6.0f * w * r1, cw, rs);
+  }
+}
+
 // Solid flags of the 18 neighbours from the bit-packed mask (bit i <=> x + c_i solid).
 __device__ __forceinline__ uint32_t neighbour_mask(const Box& b, int x, int y, int z) {
   const int xs[3] = {wrap_m(x, b.nx), x, wrap_p(x, b.nx)};
@@ -154,7 +187,8 @@ __device__ __forceinline__ uint32_t neighbour_mask(const Box& b, int x, int y, i
   return m;
 }
 
-// The same for the moving wall groups: bit i of g2 / g3 <=> x + c_i is a wall of group 2 / 3.
+// The same for the wall groups 2, 3, 4: bit i of g2 <=> x + c_i is a wall of group 2 or 4, of g3 <=>
+// of group 3 or 4 (the two bit planes of Box::gmask).
 __device__ __forceinline__ void neighbour_groups(const Box& b, int x, int y, int z, uint32_t& g2, uint32_t& g3) {
   const int xs[3] = {wrap_m(x, b.nx), x, wrap_p(x, b.nx)};
   const int ys[3] = {wrap_m(y, b.ny), y, wrap_p(y, b.ny)};
@@ -163,8 +197,8 @@ __device__ __forceinline__ void neighbour_groups(const Box& b, int x, int y, int
   static_for<1, Q>([&](auto qc) {
     constexpr int q = decltype(qc)::value;
     const int g = wall_group_at(b, xs[1 + cx(q)], ys[1 + cy(q)], zs[1 + cz(q)]);
-    if (g == 2) g2 |= 1u << q;
-    if (g == 3) g3 |= 1u << q;
+    if (g == 2 || g == 4) g2 |= 1u << q;
+    if (g == 3 || g == 4) g3 |= 1u << q;
   });
 }
 
@@ -618,15 +652,12 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
           rs = rr - racc;
         }
         if constexpr (MOVING && q > 0) {
-          // half-way bounce-back at a moving wall (G28): what this link reflects loses
-          // 6 w_q rho^k (c_q . u_w); the wall group sits in the neighbour's sentinel (1e30 x group).
-          // The mass sums above keep the uncorrected values: a wall pushing on the fluid adds mass.
+          // moving wall (G28) or open boundary (G31), see open_link; the wall group sits in the
+          // neighbour's sentinel (1e30 x group).  The mass sums above keep the uncorrected values:
+          // a wall pushing on the fluid, an inlet or an outlet changes the mass.
           if ((smask >> q) & 1u) {
             const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
-            const float cw = sv > 2.5f * PHI_SOLID ? cdot<q>(p.uw3[0], p.uw3[1], p.uw3[2])
-                                                   : (sv > 1.5f * PHI_SOLID ? cdot<q>(p.uw2[0], p.uw2[1], p.uw2[2]) : 0.f);
-            ts = fmaf(-6.0f * w * rho, cw, ts);
-            rs = fmaf(-6.0f * w * rr, cw, rs);
+            if (sv > 1.5f * PHI_SOLID) open_link<q>(p, (int)(sv > 2.5f * PHI_SOLID) + (int)(sv > 3.5f * PHI_SOLID), rho, rr, inv_rho, ux, uy, uz, uu15, ts, rs);
           }
         }
         const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
@@ -688,15 +719,10 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
             rs = rr - racc;
           }
           if constexpr (MOVING && q > 0) {
-            // half-way bounce-back at a moving wall (G28): what this link reflects loses
-            // 6 w_q rho^k (c_q . u_w); the wall group sits in the neighbour's sentinel (1e30 x group).
-            // The mass sums above keep the uncorrected values: a wall pushing on the fluid adds mass.
+            // moving wall (G28) or open boundary (G31), see open_link
             if ((smask >> q) & 1u) {
               const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
-              const float cw = sv > 2.5f * PHI_SOLID ? cdot<q>(p.uw3[0], p.uw3[1], p.uw3[2])
-                                                     : (sv > 1.5f * PHI_SOLID ? cdot<q>(p.uw2[0], p.uw2[1], p.uw2[2]) : 0.f);
-              ts = fmaf(-6.0f * w * rho, cw, ts);
-              rs = fmaf(-6.0f * w * rr, cw, rs);
+              if (sv > 1.5f * PHI_SOLID) open_link<q>(p, (int)(sv > 2.5f * PHI_SOLID) + (int)(sv > 3.5f * PHI_SOLID), rho, rr, inv_rho, ux, uy, uz, uu15, ts, rs);
             }
           }
           const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
@@ -979,10 +1005,10 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
       }
       if constexpr (q > 0) tacc += ts;
       else ts = dr - tacc;
-      if constexpr (HAS_SOLID && q > 0) {      // moving wall (G28): the reflected value loses 6 w rho (c . u_w)
+      if constexpr (HAS_SOLID && q > 0) {      // moving wall (G28) or open boundary (G31), see open_link
         if ((g2m | g3m) >> q & 1u) {
-          const float cw = ((g2m >> q) & 1u) ? cdot<q>(p.uw2[0], p.uw2[1], p.uw2[2]) : cdot<q>(p.uw3[0], p.uw3[1], p.uw3[2]);
-          ts = fmaf(-6.0f * w * rho, cw, ts);
+          float rs = 0.f;                      // one component: rho_r is the density
+          open_link<q, true>(p, (int)((g2m >> q) & 1u) + 2 * (int)((g3m >> q) & 1u) - 1, rho, rho, inv_rho, ux, uy, uz, uu15, ts, rs);
         }
       }
       *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask)) = ts;
@@ -1179,8 +1205,8 @@ __global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box
   }
 }
 
-// bytes [S] (0 fluid, 1 wall at rest, 2 / 3 moving wall groups) -> bit-packed words: solid, and
-// (if groups != nullptr) the two group masks behind each other
+// bytes [S] (0 fluid, 1 wall at rest, 2 / 3 / 4 wall groups) -> bit-packed words: solid, and
+// (if groups != nullptr) two bit planes behind each other that hold group - 1 in binary
 __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* groups, Box b) {
   const long long wi = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long nw = (long long)b.nxw * b.ny * b.nz;
@@ -1193,8 +1219,8 @@ __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* gro
     if (x < b.nx) {
       const uint8_t v = bytes[row * b.nx + x];
       if (v) m |= 1u << i;
-      if (v == 2) g2 |= 1u << i;
-      if (v == 3) g3 |= 1u << i;
+      if (v == 2 || v == 4) g2 |= 1u << i;
+      if (v == 3 || v == 4) g3 |= 1u << i;
     }
   }
   words[wi] = m;
@@ -1204,7 +1230,7 @@ __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* gro
 // does the byte mask hold a moving wall group?  out[0] |= 1
 __global__ void k_any_moving(const uint8_t* bytes, long long S, int* out) {
   const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s < S && (bytes[s] == 2 || bytes[s] == 3)) atomicOr(out, 1);
+  if (s < S && bytes[s] >= 2 && bytes[s] <= 4) atomicOr(out, 1);
 }
 
 }  // namespace lb

@@ -69,14 +69,14 @@ struct Box {
   int nxw;               // 32-bit mask words per x row
   long long S;           // sites
   const uint32_t* mask;  // bit-packed solid mask (bit x&31 of word row*nxw + x>>5), or nullptr
-  const uint32_t* gmask; // moving walls: two more masks of the same shape behind each other (group 2, group 3), or nullptr
+  const uint32_t* gmask; // wall groups: two more bit planes of the same shape behind each other (group - 1 in binary), or nullptr
 };
 
 __device__ __forceinline__ bool solid_at(const Box& b, int x, int y, int z) {
   return (b.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)] >> (x & 31)) & 1u;
 }
 
-// Wall group of a solid site: 1 = at rest, 2 / 3 = moving with StepParams::uw2 / uw3.
+// Wall group of a solid site: 1 = at rest, 2 / 3 / 4 = moving or open, StepParams::uw, wtype, wrho.
 __device__ __forceinline__ int wall_group_at(const Box& b, int x, int y, int z) {
   if (!b.gmask) return 1;
   const size_t w = (size_t)(z * b.ny + y) * b.nxw + (x >> 5);

@@ -18,7 +18,7 @@ LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 
 SYMBOLS = [
     "lb_set_allocator", "lb_create", "lb_destroy", "lb_set_stream", "lb_set_geometry",
-    "lb_set_wall_velocity", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_nc_symmetric", "lb_set_wall_phi", "lb_set_storage", "lb_init", "lb_step",
+    "lb_set_wall_velocity", "lb_set_wall_type", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_nc_symmetric", "lb_set_wall_phi", "lb_set_storage", "lb_init", "lb_step",
     "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
 ]
@@ -48,6 +48,7 @@ def _load():
     lib.lb_set_stream.argtypes = [vp, vp]
     lib.lb_set_geometry.argtypes = [vp, fp]
     lib.lb_set_wall_velocity.argtypes = [vp, C.c_int, C.c_float, C.c_float, C.c_float]
+    lib.lb_set_wall_type.argtypes = [vp, C.c_int, C.c_int, C.c_float, C.c_float]
     lib.lb_set_body_force.argtypes = [vp, C.c_float, C.c_float, C.c_float]
     lib.lb_set_model.argtypes = [vp, C.c_int, C.c_float]
     lib.lb_set_forcing.argtypes = [vp, C.c_int]
@@ -93,7 +94,10 @@ def use_torch_allocator():
             return None
 
     def _free(ptr, _user):
-        torch.cuda.caching_allocator_delete(ptr)
+        try:
+            torch.cuda.caching_allocator_delete(ptr)
+        except AttributeError:      # interpreter shutdown: torch is already torn down, the context frees the memory
+            pass
 
     a, f = ALLOC_FN(_alloc), FREE_FN(_free)
     _keepalive.extend([a, f])
@@ -165,6 +169,10 @@ class LB:
 
     def set_wall_velocity(self, group, ux, uy, uz):
         self._ck(lib.lb_set_wall_velocity(self.h, int(group), ux, uy, uz))
+
+    def set_wall_type(self, group, kind, rho_r=0.0, rho_b=0.0):
+        t = {"wall": 0, "inlet": 1, "reservoir": 2, "outlet": 3}.get(kind, kind)
+        self._ck(lib.lb_set_wall_type(self.h, int(group), int(t), float(rho_r), float(rho_b)))
 
     def set_body_force(self, gx, gy, gz):
         self._ck(lib.lb_set_body_force(self.h, gx, gy, gz))
@@ -252,4 +260,6 @@ def from_workload(w, storage="ab", torch_allocator=True):
         sim.set_geometry(np.ascontiguousarray(w.solid, dtype=np.uint8))
     sim.set_body_force(*w.g)
     sim.set_nc_cutoff(w.phi_c)
+    from . import workloads
+    workloads.configure_walls(sim, w)      # wall groups of the workload (velocities, open boundaries)
     return sim

@@ -647,3 +647,279 @@ def test_colour_exchange_invariance_on_gpu(lbmod, storage):
     c_r, _, _ = run(False, False)
     _, d_b, _ = run(True, False)
     assert np.abs(c_r - d_b)[fluid].max() > 1e-3
+
+
+# ---------------------------------------------------------------------------------- open boundaries (G31)
+def _open_mask(nx, ny, nz, walls):
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    if walls:
+        solid[:, 1:-1, 0] = 2
+        solid[:, 1:-1, -1] = 3
+        solid[:, 0, :] = 1
+        solid[:, -1, :] = 1
+    else:
+        solid[:, :, 0] = 2
+        solid[:, :, -1] = 3
+    return solid
+
+
+@pytest.mark.parametrize("model", ["cg", "sc", "single"])
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+@pytest.mark.parametrize("kinds", [("inlet", "outlet"), ("reservoir", "reservoir"), ("outlet", "inlet")])
+def test_open_boundaries_parity(lbmod, lbo, model, storage, kinds):
+    """Velocity inlet, reservoir and pressure outlet (G31; the flow focuser's open ends,
+    PAPER.md:207-219) on wall groups 2 and 3 against the oracle: populations after 1, 2 and 5
+    steps on a random state with a wall at rest, body force and (colour gradient) near contact."""
+    two = model != "single"
+    w = _random_workload(36, 13, 10, seed=77, walls=True, A_nc=0.02 if model == "cg" else 0.0)
+    w.solid[:, :, 0] = 2                  # the x = 0 plane is open (group 2)
+    w.solid[:, :, -1] = 3                 # so is x = nx-1 (group 3)
+    w.solid[0, :, 1:-1] = 1               # the z = 0 plane is at rest
+    w.solid[w.nz // 2, w.ny // 2, w.nx // 3] = 3
+    fluid = w.solid == 0
+    params = list(w.params)
+    if not two:
+        params[1] = params[0]
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *params)
+    sim = lbmod.LB(w.nx, w.ny, w.nz, *params)
+    sim.set_storage(storage)
+    if model == "sc":
+        o.set_model("sc", 1.5); sim.set_model("sc", 1.5)
+    rho_r = w.rho_r + (0 if two else w.rho_b)
+
+    def dens(kind, a, b):
+        # one component: the density of an inlet / reservoir is rho_r alone (rho_b is ignored), that
+        # of an outlet rho_r + rho_b; keep either near the fluid's (a 40 % jump is a shock whose
+        # fp32 rounding differences grow by orders of magnitude within a few steps)
+        return (a, b) if two or kind == "outlet" else (a + b, 0.5)
+    for obj in (o, sim):
+        obj.set_geometry(w.solid)
+        obj.set_body_force(*w.g)
+        obj.set_wall_velocity(2, 0.012, 0.002, -0.003)
+        obj.set_wall_velocity(3, -0.008, 0.001, 0.002)
+        obj.set_wall_type(2, kinds[0], *dens(kinds[0], 0.62, 0.41))
+        obj.set_wall_type(3, kinds[1], *dens(kinds[1], 0.35, 0.63))
+        obj.init(rho_r, w.rho_b if two else None, w.u)
+    risky = np.zeros(w.shape, bool)
+    done = 0
+    for n in (1, 2, 5):
+        for _ in range(n - done):
+            if model == "cg":
+                risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+            o.step(1); sim.step(1)
+        done = n
+        e = pu.pop_error(sim, o, two=two)
+        assert e[~risky & fluid].max() < pu.POP_TOL, (n, e[~risky & fluid].max())
+    errs, _, _ = pu.macro_errors(sim, o)
+    assert max(errs.values()) < pu.MACRO_TOL, errs
+    # the open boundaries do change the result (against the same groups as moving walls)
+    ref = lbmod.LB(w.nx, w.ny, w.nz, *params)
+    ref.set_storage(storage)
+    if model == "sc":
+        ref.set_model("sc", 1.5)
+    ref.set_geometry(w.solid); ref.set_body_force(*w.g)
+    ref.set_wall_velocity(2, 0.012, 0.002, -0.003); ref.set_wall_velocity(3, -0.008, 0.001, 0.002)
+    ref.init(rho_r, w.rho_b if two else None, w.u)
+    ref.step(5)
+    assert np.abs(ref.get_populations(0) - sim.get_populations(0)).max() > 1e-4
+
+
+@pytest.mark.parametrize("exit_kind", ["reservoir", "outlet"])
+@pytest.mark.parametrize("two", [False, True])
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_open_plug_flow_is_a_fixed_point_on_gpu(lbmod, two, exit_kind, storage):
+    """A uniform flow at the prescribed densities is an exact fixed point of velocity inlet +
+    pressure boundary (f^eq_i -+ f^eq_opp(i) of Eq. 2): closed form on the CUDA
+    path itself, no oracle.  fp32: the state stays within rounding of the plug flow."""
+    nx, ny, nz, U = 36, 9, 12, 0.03
+    solid = _open_mask(nx, ny, nz, walls=False)
+    rr0, rb0 = (0.7, 0.4) if two else (1.1, 0.0)
+    sim = lbmod.LB(nx, ny, nz, 0.8, 1.1 if two else 0.8, 0.0, 0.0, 0.0)
+    sim.set_storage(storage)
+    sim.set_geometry(solid)
+    sim.set_wall_velocity(2, U, 0.0, 0.0)
+    sim.set_wall_type(2, "inlet", rr0, rb0)
+    sim.set_wall_type(3, exit_kind, rr0, rb0)
+    ones = np.ones((nz, ny, nx), np.float32)
+    u0 = np.zeros((3, nz, ny, nx), np.float32)
+    u0[0] = U
+    sim.init(rr0 * ones, rb0 * ones if two else None, u0)
+    sim.step(500)
+    rr, rb, u = sim.get_macros()
+    fl = solid == 0
+    assert np.abs(rr[fl] - rr0).max() < 2e-5 and np.abs(u[0][fl] - U).max() < 2e-5
+    assert np.abs(u[1:]).max() < 2e-5
+    if two:
+        assert np.abs(rb[fl] - rb0).max() < 2e-5
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_open_inlet_outlet_mass_balance_on_gpu(lbmod, storage):
+    """Velocity inlet (red-rich plug U) and pressure outlet in a walled channel, on the CUDA path
+    itself: the steady mass flux through every cross-section is what the inlet links inject,
+    rho_in U (H - 1/3) (each inlet link adds 6 w_i rho_in U; the two corner nodes lack one diagonal
+    each); the red share of the flux tends to the inlet's 0.7; the profile develops into the
+    parabola (the oracle's pin P18, here in fp32)."""
+    nx, ny, nz, U = 52, 14, 4, 0.02
+    solid = _open_mask(nx, ny, nz, walls=True)
+    sim = lbmod.LB(nx, ny, nz, 0.9, 0.9, 0.0, 0.0, 0.0)
+    sim.set_storage(storage)
+    sim.set_geometry(solid)
+    sim.set_wall_velocity(2, U, 0.0, 0.0)
+    sim.set_wall_type(2, "inlet", 0.7, 0.3)
+    sim.set_wall_type(3, "outlet", 0.5, 0.5)
+    sim.set_wall_type(4, "reservoir", 0.5, 0.5)
+    sim.set_wall_velocity(4, 0.01, 0.0, 0.0)
+    with pytest.raises(RuntimeError):
+        sim.set_wall_velocity(5, 0.01, 0.0, 0.0)
+    ones = np.ones((nz, ny, nx), np.float32)
+    sim.init(0.5 * ones, 0.5 * ones, np.zeros((3, nz, ny, nx), np.float32))
+    sim.step(12000)
+    rr, rb, u = sim.get_macros()
+    rr, rb, u = rr.astype(np.float64), rb.astype(np.float64), u.astype(np.float64)
+    rho = rr + rb
+    H = ny - 2
+    flux = (rho * u[0])[1, 1:-1, 1:-1].sum(axis=0)
+    assert np.abs(flux / (U * (H - 1.0 / 3.0)) - 1.0).max() < 1e-4, np.abs(flux / (U * (H - 1.0 / 3.0)) - 1.0).max()
+    red = (rr * u[0])[1, 1:-1, 1:-1].sum(axis=0)
+    assert np.abs(red / (0.7 * U * (H - 1.0 / 3.0)) - 1.0).max() < 5e-3
+    y = np.arange(ny) - 0.5
+    x = nx - 8
+    umean = flux[x - 1] / H / rho[1, 1:-1, x].mean()
+    para = 6.0 * umean * y[1:-1] * (H - y[1:-1]) / H ** 2
+    assert np.abs(u[0][1, 1:-1, x] / para - 1.0).max() < 0.025
+
+
+def test_open_boundary_error_codes(lbmod):
+    sim = lbmod.LB(8, 8, 8, 1.0, 1.0, 0.0, 0.0, 0.0)
+    for args in ((1, 1, 1.0, 0.0), (5, 1, 1.0, 0.0), (2, 4, 1.0, 0.0), (2, -1, 1.0, 0.0), (2, 1, -0.5, 0.0),
+                 (3, 2, 0.5, float("nan"))):
+        with pytest.raises(RuntimeError):
+            sim.set_wall_type(*args)
+    sim.set_wall_type(2, 0)
+    sim.set_wall_type(3, "outlet", 0.5, 0.5)
+    sim.set_wall_type(4, "reservoir", 0.5, 0.5)
+    sim.set_wall_velocity(4, 0.01, 0.0, 0.0)
+    with pytest.raises(RuntimeError):
+        sim.set_wall_velocity(5, 0.01, 0.0, 0.0)
+
+
+# ---------------------------------------------------------------------------------- flow focuser (three wall groups)
+def _focuser_pair(lbmod, lbo, w, storage):
+    o = lbo.Oracle(w.nx, w.ny, w.nz, *w.params)
+    sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    sim.set_storage(storage)
+    for obj in (o, sim):
+        obj.set_geometry(w.solid)
+        W.configure_walls(obj, w)
+        obj.init(w.rho_r, w.rho_b, w.u)
+    return o, sim
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_focuser_parity(lbmod, lbo, storage):
+    """The flow-focusing device (stand-in dimensions, G31) with its
+    dispersed inlet, continuous inlets and outlet on wall groups 2, 3, 4, in 3-D with walls in z
+    and the near-contact force on: populations after 1, 2 and 5 steps and macroscopic fields after
+    300 steps against the oracle."""
+    w = W.focuser(72, 40, 12, wd=8, wc=8, t=3, li=16, wo=8, lo=6, u_d=0.02, u_c=0.015, A_nc=0.02, walls_z=True)
+    o, sim = _focuser_pair(lbmod, lbo, w, storage)
+    fluid = w.solid == 0
+    risky = np.zeros(w.shape, bool)
+    done = 0
+    for n in (1, 2, 5):
+        for _ in range(n - done):
+            risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+            o.step(1); sim.step(1)
+        done = n
+        e = pu.pop_error(sim, o)
+        assert e[~risky & fluid].max() < pu.POP_TOL, (n, e[~risky & fluid].max())
+    o.step(295); sim.step(295)
+    errs, (rr, rb, u), _ = pu.macro_errors(sim, o)
+    assert max(errs.values()) < pu.MACRO_TOL, errs
+    assert np.abs(u).max() > 5e-3                       # the inlets do drive a flow
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_focuser_relabelled_groups_and_exact_injection_on_gpu(lbmod, storage):
+    """On the CUDA path itself (no oracle): (a) permuting the labels of the three wall groups
+    together with their settings changes nothing, bit for bit; (b) while no red fluid has reached
+    the outlet the red mass grows per step by what the links out of the dispersed inlet inject,
+    u_d (w_d - 1/3) per plane (oracle pin P19, here to fp32 rounding)."""
+    w = W.focuser(96, 48, 4)
+    sims = []
+    for perm in ({2: 2, 3: 3, 4: 4}, {2: 4, 4: 3, 3: 2}):
+        solid = w.solid.copy()
+        for a, b in perm.items():
+            solid[w.solid == a] = b
+        sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+        sim.set_storage(storage)
+        sim.set_geometry(solid)
+        for g, d in w.info["wall_groups"].items():
+            sim.set_wall_velocity(perm[g], *d["u"])
+            sim.set_wall_type(perm[g], d["kind"], *d["rho"])
+        sim.init(w.rho_r, w.rho_b, w.u)
+        sims.append(sim)
+    fl = w.solid == 0
+    m0 = float(sims[0].get_macros()[0][fl].sum(dtype=np.float64))
+    for s in sims:
+        s.step(1500)
+    a, b = sims[0].get_macros(), sims[1].get_macros()
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    rr = a[0]
+    assert rr[:, :, -8:].max() < 1e-7
+    rate = w.info["wall_groups"][2]["u"][0] * (w.info["wd"] - 1.0 / 3.0) * w.nz
+    gain = float(rr[fl].sum(dtype=np.float64)) - m0
+    assert abs(gain / (1500 * rate) - 1.0) < 1e-4, gain / (1500 * rate)
+
+
+def test_focuser_3d_run(lbmod):
+    """The 3-D device (256 x 96 x 48, walls in z, near contact on) for 6000 steps: the dispersed
+    phase is pushed through the orifice, everything stays finite and within the lattice's Mach
+    range, the total mass stays bounded (the outlet passes what the inlets inject) and the wall
+    groups reach the kernel (the inlet columns move at the prescribed speeds)."""
+    w = W.get("focuser-3d")
+    sim = lbmod.LB(w.nx, w.ny, w.nz, *w.params)
+    sim.set_geometry(w.solid)
+    W.configure_walls(sim, w)
+    sim.init(w.rho_r, w.rho_b, w.u)
+    fl = w.solid == 0
+    rr0, rb0, _ = sim.get_macros()
+    m0 = float((rr0 + rb0)[fl].sum(dtype=np.float64))
+    front0 = np.where((rr0 > rb0) & fl)[2].max()
+    sim.step(6000)
+    rr, rb, u = sim.get_macros()
+    assert np.isfinite(u).all() and np.abs(u).max() < 0.15
+    front = np.where((rr > rb) & fl)[2].max()
+    assert front > front0 + 20, (front0, front)
+    assert abs(float((rr + rb)[fl].sum(dtype=np.float64)) / m0 - 1.0) < 0.03
+    zc, yc = w.nz // 2, w.ny // 2
+    ud = w.info["wall_groups"][2]["u"][0]
+    assert 0.5 * ud < u[0][zc, yc, 4] < 2.5 * ud           # between the plug speed and the developed peak
+    assert u[0][zc, 6 + 12, 4] > 0
+
+
+def test_focuser_pinches_off_a_droplet(lbmod):
+    """The device in the dripping regime (Ca = rho nu u_c / sigma = 0.125, alpha = u_d / 2 u_c = 0.15;
+    "focuser-drip"): behind the orifice the continuous phase squeezes the dispersed thread until a
+    droplet pinches off, the mechanism of the paper's Fig. 4.  After 12000 steps
+    the red phase consists of the thread and at least one separate droplet of more than 5000
+    sites; the thread was one piece at 3000 steps."""
+    from scipy import ndimage
+    w = W.get("focuser-drip")
+    sim = lbmod.from_workload(w)
+    sim.init(w.rho_r, w.rho_b, w.u)
+    fl = w.solid == 0
+
+    def pieces():
+        rr, rb, u = sim.get_macros()
+        assert np.isfinite(u).all()
+        lab, n = ndimage.label((rr > rb) & fl)
+        return sorted(np.bincount(lab.ravel())[1:].tolist(), reverse=True)
+
+    sim.step(3000)
+    assert len([s for s in pieces() if s > 1000]) == 1
+    sim.step(9000)
+    big = [s for s in pieces() if s > 5000]
+    assert len(big) >= 2, big
