@@ -199,17 +199,19 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
 // z planes per CTA.  Measured on B200: short columns win (256^3: 0.91 ms at 8
 // planes, 0.95 at 16, 1.11 at 64; 640^3: 16.2 ms at 16, 18.9 at 214), but every brick face costs
 // k_phase_fwd a gather, so: 10..20 planes, and among those the count whose number of CTAs fills
-// whole waves of (SMs x 3 resident CTAs) best.
+// whole waves of (SMs x resident CTAs) best.
 int pick_zc(lb_handle h) {
   if (h->tune_zc > 0) return h->tune_zc < h->nz ? h->tune_zc : h->nz;
   if (h->nz <= 10) return h->nz;
-  static int slots = 0;
-  if (!slots) {
+  static int sm_count = 0;
+  if (!sm_count) {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cudaGetLastError();
-    slots = 3 * sms;
+    sm_count = sms;
   }
+  // resident CTAs per SM: 3, but 2 for the instantiations with wall groups (WALLS = 2)
+  const int slots = ((h->has_solid && h->has_moving) ? 2 : 3) * sm_count;
   const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
   int best = 16;
   double best_eff = -1.0;

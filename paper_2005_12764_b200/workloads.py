@@ -291,6 +291,8 @@ def get(name):
         "focuser": focuser,
         "focuser-3d": lambda: focuser(256, 96, 48, wd=20, wc=24, t=6, li=48, wo=20, lo=16, walls_z=True,
                                       A_nc=0.02, steps=20000),
+        "focuser-large": lambda: focuser(1024, 256, 128, wd=56, wc=64, t=16, li=128, wo=40, lo=48, walls_z=True,
+                                         A_nc=0.02, steps=20000),
         # dripping regime (Ca = rho nu u_c / sigma = 0.125 with sigma = 4 A tau / 9): droplets pinch off behind the orifice
         "focuser-drip": lambda: focuser(256, 96, 48, wd=20, wc=24, t=6, li=48, wo=14, lo=16, u_d=0.006, u_c=0.02,
                                         A=0.06, A_nc=0.02, walls_z=True, steps=36000),
