@@ -604,7 +604,7 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
       // over directions is a handful of fused multiply-adds:
       //   omega f^eq_q - A B_q |G| = ob[c] + orw[c] cu (3 + 4.5 cu)
       //   A w_q (c.G)^2 / |G|      = (pa[c] cG) cG
-      //   Guo source               = gw[c] (cF (1 + 3 cu) - u.F)
+      //   Guo source               = gw[c] (cF (1 + 3 cu) - u.F)   (-gw[c] u.F is folded into obf[c])
       //   red share                = fr_r (f*_q + w_q) + kc[c] cG
       const float eq0 = dr - rho * uu15;
       const float orw[3] = {omega * rho * wq(0), omega * rho * wq(1), omega * rho * wq(7)};
@@ -625,35 +625,21 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
       // to the rounding of one sum instead of carrying the relative error of rho_r/rho or of
       // w_q * drho (a systematic drift in uniform regions).
       float racc = 0.f, tacc = 0.f;
+      // Guo forcing: opposite directions q, q+1 = opp(q) share (c.u)^2, (c.G)^2, (c.F)(c.u) and differ
+      // in the sign of the odd terms, so a pair costs one even part s and one odd part a:
+      //   f*_q, f*_opp = (1 - omega) T + s +- a,   red share = fr_r f* + frw +- kc cG
+      const float orw45[3] = {0.f, 4.5f * orw[1], 4.5f * orw[2]};
+      const float orw3[3] = {0.f, 3.0f * orw[1], 3.0f * orw[2]};
+      const float gw3[3] = {0.f, 3.0f * gw[1], 3.0f * gw[2]};
+      const float obf[3] = {0.f, forced ? fmaf(-gw[1], uF, ob[1]) : ob[1], forced ? fmaf(-gw[2], uF, ob[2]) : ob[2]};
       auto collide = [&](auto bounce) {
-      static_for<1, Q + 1>([&](auto qc) {
-        constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
-        constexpr int k = q == 0 ? 0 : (q < 7 ? 1 : 2);
+      // what happens to every direction once its post-collision pair {ts, rs} is known
+      auto finish = [&](auto qc, float ts, float rs) {
+        constexpr int q = decltype(qc)::value;
         constexpr float w = wq(q);
-        float ts, rs;
-        if constexpr (q > 0) {
-          const float cu = cdot<q>(ux, uy, uz);
-          const float cG = cdot<q>(Gx, Gy, Gz);
-          ts = fmaf(om1, T[q], fmaf(orw[k], cu * fmaf(4.5f, cu, 3.0f), ob[k]));
-          if constexpr (forced && !EDM) {
-            const float cF = cdot<q>(Fx, Fy, Fz);
-            ts = fmaf(gw[k], fmaf(cF, fmaf(3.0f, cu, 1.0f), -uF), ts);
-          }
-          if constexpr (forced && EDM) {
-            const float cv = cdot<q>(vx, vy, vz);
-            ts = fmaf(rw[k], fmaf(cv - cu, fmaf(4.5f, cv + cu, 3.0f), -dvv15), ts);
-          }
-          ts = fmaf(pa[k] * cG, cG, ts);
-          rs = fmaf(fr_r, ts, fmaf(kc[k], cG, frw[k]));
-          racc += rs;
-          tacc += ts;
-        } else {
-          ts = dr - tacc;
-          rs = rr - racc;
-        }
         if constexpr (MOVING && q > 0) {
           // moving wall (G28) or open boundary (G31), see open_link; the wall group sits in the
-          // neighbour's sentinel (1e30 x group).  The mass sums above keep the uncorrected values:
+          // neighbour's sentinel (1e30 x group).  The mass sums keep the uncorrected values:
           // a wall pushing on the fluid, an inlet or an outlet changes the mass.
           if ((smask >> q) & 1u) {
             const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
@@ -666,7 +652,57 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
         // regions where phi matters, so the forwarded sum keeps ~1e-8 there
         vd[q] = (2.0f * rs - w) - ts;
         vt[q] = ts;
-      });
+      };
+      // (not in the in-place odd step with near contact: there the pair form spills, and a spill
+      // reload queued behind the shifted stores is expensive: C4 AA 15.2 -> 13.1 GLUPS)
+      constexpr bool PAIRED = !EDM && !(MODE == MODE_AA_ODD && HAS_NC);
+      if constexpr (PAIRED) {
+        static_for<0, (Q - 1) / 2>([&](auto pc) {
+          constexpr int q = 2 * decltype(pc)::value + 1;   // 1, 3, ..., 17; opp(q) = q + 1
+          constexpr int k = q < 7 ? 1 : 2;
+          const float cu = cdot<q>(ux, uy, uz);
+          const float cG = cdot<q>(Gx, Gy, Gz);
+          float s = fmaf(orw45[k], cu * cu, obf[k]);
+          // (explicitly rounded product: a force-free run must give the same bits in the forced
+          // instantiation, which the in-place modes use, and in the unforced one, where the
+          // compiler would otherwise contract this product into the two sums below)
+          float a = __fmul_rn(orw3[k], cu);
+          if constexpr (forced) {
+            const float cF = cdot<q>(Fx, Fy, Fz);
+            s = fmaf(gw3[k] * cF, cu, s);
+            a = fmaf(gw[k], cF, a);
+          }
+          s = fmaf(pa[k] * cG, cG, s);
+          const float ts0 = __fadd_rn(fmaf(om1, T[q], s), a), ts1 = __fsub_rn(fmaf(om1, T[q + 1], s), a);
+          const float rs0 = fmaf(fr_r, ts0, fmaf(kc[k], cG, frw[k])), rs1 = fmaf(fr_r, ts1, fmaf(-kc[k], cG, frw[k]));
+          racc += rs0 + rs1;
+          tacc += ts0 + ts1;
+          finish(std::integral_constant<int, q>{}, ts0, rs0);
+          finish(std::integral_constant<int, q + 1>{}, ts1, rs1);
+        });
+      } else {
+        static_for<1, Q>([&](auto qc) {
+          constexpr int q = decltype(qc)::value;
+          constexpr int k = q < 7 ? 1 : 2;
+          const float cu = cdot<q>(ux, uy, uz);
+          const float cG = cdot<q>(Gx, Gy, Gz);
+          float ts = fmaf(om1, T[q], fmaf(orw[k], cu * fmaf(4.5f, cu, 3.0f), ob[k]));
+          if constexpr (forced && !EDM) {
+            const float cF = cdot<q>(Fx, Fy, Fz);
+            ts = fmaf(gw[k], fmaf(cF, fmaf(3.0f, cu, 1.0f), -uF), ts);
+          }
+          if constexpr (forced && EDM) {
+            const float cv = cdot<q>(vx, vy, vz);
+            ts = fmaf(rw[k], fmaf(cv - cu, fmaf(4.5f, cv + cu, 3.0f), -dvv15), ts);
+          }
+          ts = fmaf(pa[k] * cG, cG, ts);
+          const float rs = fmaf(fr_r, ts, fmaf(kc[k], cG, frw[k]));
+          racc += rs;
+          tacc += ts;
+          finish(qc, ts, rs);
+        });
+      }
+      finish(std::integral_constant<int, 0>{}, dr - tacc, rr - racc);
       };
       // only the in-place odd step writes to neighbouring sites, so only there the store slots
       // depend on the walls; everywhere else one copy of the loop serves both cases

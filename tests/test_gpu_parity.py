@@ -148,15 +148,27 @@ def test_C5_mini_100_steps_macros(lbmod, lbo, storage):
     assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
 
 
-def test_AA_equals_AB_bitwise(lbmod):
-    """AA and A/B share the arithmetic, so they must agree bit for bit (3 and 4 steps)."""
-    w = W.get("c5-mini")
+@pytest.mark.parametrize("name", ["c3-mini", "c5-mini"])
+def test_AA_equals_AB_bitwise(lbmod, name):
+    """AA and A/B share the arithmetic, so they must agree bit for bit (3 and 4 steps).  With the
+    near-contact force (c5-mini) the in-place odd step keeps the direction-by-direction form of the
+    collision where the others use the pair form (register pressure): there the two
+    agree to rounding, a few ulp of w_i, which still rules out any addressing error."""
+    w = W.get(name)
+    exact = w.A_nc == 0.0
     a, b = pu.make_gpu(lbmod, w, "ab"), pu.make_gpu(lbmod, w, "aa")
     for n in (3, 1):
         a.step(n); b.step(n)
         for k in (0, 1):
-            assert np.array_equal(a.get_populations(k), b.get_populations(k))
+            fa, fb = a.get_populations(k), b.get_populations(k)
+            if exact:
+                assert np.array_equal(fa, fb)
+            else:
+                assert (np.abs(fa.astype(np.float64) - fb) / pu.W19[:, None, None, None]).max() < 2e-6
     ra, _, ua = a.get_macros()
     rb_, _, ub = b.get_macros()
-    assert np.array_equal(ra, rb_) and np.array_equal(ua, ub)
+    if exact:
+        assert np.array_equal(ra, rb_) and np.array_equal(ua, ub)
+    else:
+        assert np.abs(ra - rb_).max() < 1e-6 and np.abs(ua - ub).max() < 1e-6
     assert b.device_bytes() < 0.6 * a.device_bytes()
