@@ -733,27 +733,19 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
         const float wb[3] = {wq(0) * rb, wq(1) * rb, wq(7) * rb};
         const float owd[3] = {omega * wq(0) * dr, omega * wq(1) * dr, omega * wq(7) * dr};
         const float owr[3] = {omega * wq(0) * rho, omega * wq(1) * rho, omega * wq(7) * rho};
+        // Pair form (as in the colour-gradient branch): for opposite directions q, opp(q) = q + 1,
+        // with cu = c.u and ca = c.a^k,
+        //   f^eq_q / (w rho) - 1 = [4.5 cu^2 - 1.5 u.u] +- 3 cu
+        //   S^k_q / (w rho^k)    = [ca (4.5 ca + 9 cu) - 1.5 (v.v - u.u)] +- 3 ca
+        // so each pair costs one even part and one odd part per component.
+        const float wr3[3] = {0.f, 3.0f * wr[1], 3.0f * wr[2]};
+        const float wb3[3] = {0.f, 3.0f * wb[1], 3.0f * wb[2]};
+        const float owr3[3] = {0.f, 3.0f * owr[1], 3.0f * owr[2]};
         float racc = 0.f, tacc = 0.f;
         auto collide = [&](auto bounce) {
-        static_for<1, Q + 1>([&](auto qc) {
-          constexpr int q = decltype(qc)::value % Q;   // 1, 2, ..., 18, 0
-          constexpr int k = q == 0 ? 0 : (q < 7 ? 1 : 2);
+        auto finish = [&](auto qc, float ts, float rs) {
+          constexpr int q = decltype(qc)::value;
           constexpr float w = wq(q);
-          float ts, rs;
-          if constexpr (q > 0) {
-            const float cu = cdot<q>(ux, uy, uz);
-            const float e = fmaf(cu, fmaf(4.5f, cu, 3.0f), -uu15);          // f^eq / (w rho) - 1
-            const float cvr = cdot<q>(vrx, vry, vrz), cvb = cdot<q>(vbx, vby, vbz);
-            const float sr = fmaf(cvr - cu, fmaf(4.5f, cvr + cu, 3.0f), -dr15);
-            const float sb = fmaf(cvb - cu, fmaf(4.5f, cvb + cu, 3.0f), -db15);
-            rs = fmaf(om1, R[q], wr[k] * fmaf(omega, 1.0f + e, sr));
-            ts = fmaf(om1, T[q], fmaf(owr[k], e, owd[k])) + fmaf(wr[k], sr, wb[k] * sb);
-            racc += rs;
-            tacc += ts;
-          } else {                       // the rest populations take what is left (mass is conserved)
-            ts = dr - tacc;
-            rs = rr - racc;
-          }
           if constexpr (MOVING && q > 0) {
             // moving wall (G28) or open boundary (G31), see open_link
             if ((smask >> q) & 1u) {
@@ -765,7 +757,32 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
           *reinterpret_cast<float2*>(dst_ptr(p, s)) = make_float2(ts, rs);
           vd[q] = (2.0f * rs - w) - ts;
           vt[q] = ts;
+        };
+        static_for<0, (Q - 1) / 2>([&](auto pc) {
+          constexpr int q = 2 * decltype(pc)::value + 1;   // 1, 3, ..., 17; opp(q) = q + 1
+          constexpr int k = q < 7 ? 1 : 2;
+          const float cu = cdot<q>(ux, uy, uz);
+          const float car = cdot<q>(arx, ary, arz), cab = cdot<q>(abx, aby, abz);
+          const float cu9 = 9.0f * cu;
+          const float ee = fmaf(4.5f * cu, cu, -uu15);                      // even part of f^eq / (w rho) - 1
+          const float sre = fmaf(car, fmaf(4.5f, car, cu9), -dr15);          // even parts of S^k / (w rho^k)
+          const float sbe = fmaf(cab, fmaf(4.5f, cab, cu9), -db15);
+          // red: even and odd part (explicitly rounded products: no contraction into the sums, so
+          // that every instantiation computes the same bits)
+          const float re = __fmul_rn(wr[k], fmaf(omega, 1.0f + ee, sre));
+          const float ro = __fmul_rn(wr3[k], fmaf(omega, cu, car));
+          const float rs0 = __fadd_rn(fmaf(om1, R[q], re), ro), rs1 = __fsub_rn(fmaf(om1, R[q + 1], re), ro);
+          // total
+          const float te = fmaf(wb[k], sbe, fmaf(wr[k], sre, fmaf(owr[k], ee, owd[k])));
+          const float to = fmaf(wb3[k], cab, fmaf(wr3[k], car, __fmul_rn(owr3[k], cu)));
+          const float ts0 = __fadd_rn(fmaf(om1, T[q], te), to), ts1 = __fsub_rn(fmaf(om1, T[q + 1], te), to);
+          racc += rs0 + rs1;
+          tacc += ts0 + ts1;
+          finish(std::integral_constant<int, q>{}, ts0, rs0);
+          finish(std::integral_constant<int, q + 1>{}, ts1, rs1);
         });
+        // the rest populations take what is left (mass is conserved)
+        finish(std::integral_constant<int, 0>{}, dr - tacc, rr - racc);
         };
         if (MODE == MODE_AA_ODD && HAS_SOLID && near_wall) collide(std::integral_constant<bool, HAS_SOLID>{});
       else collide(std::false_type{});
