@@ -612,7 +612,8 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
                            omega * wq(7) * eq0 - p.A * bq(7) * Gne};
       const float pa[3] = {0.f, p.A * wq(1) * invG, p.A * wq(7) * invG};
       //   exact difference         = rw[c] ((cv - cu)(3 + 4.5 (cv + cu)) - 1.5 (v.v - u.u)),  v = u + F/rho
-      const float vx = ux + Fx * inv_rho, vy = uy + Fy * inv_rho, vz = uz + Fz * inv_rho;
+      const float fax = Fx * inv_rho, fay = Fy * inv_rho, faz = Fz * inv_rho;   // v - u
+      const float vx = ux + fax, vy = uy + fay, vz = uz + faz;
       const float dvv15 = 1.5f * (vx * vx + vy * vy + vz * vz) - uu15;
       const float rw[3] = {rho * wq(0), rho * wq(1), rho * wq(7)};
       const float g3 = 3.0f * (1.0f - 0.5f * omega);
@@ -631,7 +632,8 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
       const float orw45[3] = {0.f, 4.5f * orw[1], 4.5f * orw[2]};
       const float orw3[3] = {0.f, 3.0f * orw[1], 3.0f * orw[2]};
       const float gw3[3] = {0.f, 3.0f * gw[1], 3.0f * gw[2]};
-      const float obf[3] = {0.f, forced ? fmaf(-gw[1], uF, ob[1]) : ob[1], forced ? fmaf(-gw[2], uF, ob[2]) : ob[2]};
+      const float obf[3] = {0.f, (forced && !EDM) ? fmaf(-gw[1], uF, ob[1]) : ob[1], (forced && !EDM) ? fmaf(-gw[2], uF, ob[2]) : ob[2]};
+      const float rw3[3] = {0.f, 3.0f * rw[1], 3.0f * rw[2]};
       auto collide = [&](auto bounce) {
       // what happens to every direction once its post-collision pair {ts, rs} is known
       auto finish = [&](auto qc, float ts, float rs) {
@@ -653,9 +655,9 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
         vd[q] = (2.0f * rs - w) - ts;
         vt[q] = ts;
       };
-      // (not in the in-place odd step with near contact: there the pair form spills, and a spill
+      // (not in the in-place odd step with near contact or exact-difference forcing: there the pair form spills, and a spill
       // reload queued behind the shifted stores is expensive: C4 AA 15.2 -> 13.1 GLUPS)
-      constexpr bool PAIRED = !EDM && !(MODE == MODE_AA_ODD && HAS_NC);
+      constexpr bool PAIRED = !(MODE == MODE_AA_ODD && (HAS_NC || EDM));
       if constexpr (PAIRED) {
         static_for<0, (Q - 1) / 2>([&](auto pc) {
           constexpr int q = 2 * decltype(pc)::value + 1;   // 1, 3, ..., 17; opp(q) = q + 1
@@ -667,10 +669,17 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
           // instantiation, which the in-place modes use, and in the unforced one, where the
           // compiler would otherwise contract this product into the two sums below)
           float a = __fmul_rn(orw3[k], cu);
-          if constexpr (forced) {
+          if constexpr (forced && !EDM) {
             const float cF = cdot<q>(Fx, Fy, Fz);
             s = fmaf(gw3[k] * cF, cu, s);
             a = fmaf(gw[k], cF, a);
+          }
+          if constexpr (forced && EDM) {
+            // exact difference, ca = c.(v - u) = c.F / rho:
+            // S_q / (w rho) = [ca (4.5 ca + 9 cu) - 1.5 (v.v - u.u)] +- 3 ca
+            const float ca = cdot<q>(fax, fay, faz);
+            s = fmaf(rw[k], fmaf(ca, fmaf(4.5f, ca, 9.0f * cu), -dvv15), s);
+            a = fmaf(rw3[k], ca, a);
           }
           s = fmaf(pa[k] * cG, cG, s);
           const float ts0 = __fadd_rn(fmaf(om1, T[q], s), a), ts1 = __fsub_rn(fmaf(om1, T[q + 1], s), a);
