@@ -689,6 +689,29 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
           finish(std::integral_constant<int, q>{}, ts0, rs0);
           finish(std::integral_constant<int, q + 1>{}, ts1, rs1);
         });
+      } else if constexpr (!EDM && WALLS != 1) {
+        // the same pairs with the constants of the direction loop only (no orw45, orw3, gw3, obf:
+        // four live values fewer, two instructions more per pair), for the in-place odd step
+        // (C5 AA 16.45 -> 16.58 GLUPS; not with walls at rest: one spilled value there, whose
+        // reload behind the shifted stores took C4 AA from 15.3 to 12.6 GLUPS)
+        static_for<0, (Q - 1) / 2>([&](auto pc) {
+          constexpr int q = 2 * decltype(pc)::value + 1;
+          constexpr int k = q < 7 ? 1 : 2;
+          const float cu = cdot<q>(ux, uy, uz);
+          const float cG = cdot<q>(Gx, Gy, Gz);
+          const float cF = cdot<q>(Fx, Fy, Fz);
+          const float cu3 = 3.0f * cu;
+          float s = fmaf(orw[k], (1.5f * cu3) * cu, ob[k]);
+          s = fmaf(gw[k], fmaf(cF, cu3, -uF), s);
+          s = fmaf(pa[k] * cG, cG, s);
+          const float a = fmaf(gw[k], cF, __fmul_rn(orw[k], cu3));
+          const float ts0 = __fadd_rn(fmaf(om1, T[q], s), a), ts1 = __fsub_rn(fmaf(om1, T[q + 1], s), a);
+          const float rs0 = fmaf(fr_r, ts0, fmaf(kc[k], cG, frw[k])), rs1 = fmaf(fr_r, ts1, fmaf(-kc[k], cG, frw[k]));
+          racc += rs0 + rs1;
+          tacc += ts0 + ts1;
+          finish(std::integral_constant<int, q>{}, ts0, rs0);
+          finish(std::integral_constant<int, q + 1>{}, ts1, rs1);
+        });
       } else {
         static_for<1, Q>([&](auto qc) {
           constexpr int q = decltype(qc)::value;
