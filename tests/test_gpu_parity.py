@@ -151,9 +151,9 @@ def test_C5_mini_100_steps_macros(lbmod, lbo, storage):
 @pytest.mark.parametrize("name", ["c3-mini", "c5-mini"])
 def test_AA_equals_AB_bitwise(lbmod, name):
     """AA and A/B share the arithmetic, so they must agree bit for bit (3 and 4 steps).  With the
-    near-contact force (c5-mini) the in-place odd step keeps the direction-by-direction form of the
-    collision where the others use the pair form (register pressure): there the two
-    agree to rounding, a few ulp of w_i, which still rules out any addressing error."""
+    near-contact force (c5-mini) the in-place odd step uses a leaner form of the collision than the
+    others (register pressure): there the two agree to rounding,
+    a few ulp of w_i, which still rules out any addressing error."""
     w = W.get(name)
     exact = w.A_nc == 0.0
     a, b = pu.make_gpu(lbmod, w, "ab"), pu.make_gpu(lbmod, w, "aa")
