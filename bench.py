@@ -31,6 +31,7 @@ sys.path.insert(0, ROOT)
 METRIC = "GLUPS (two-component D3Q19 site updates/s)"
 BYTES_PER_UPDATE = {True: 2 * 2 * 19 * 4, False: 2 * 19 * 4}   # two-component 304 B, single 152 B
 FALLBACK_HBM_GBS = 6650.0
+NOMINAL_HBM_GBS = 8000.0     # north_star's "~8 TB/s"; every fraction is reported against the measured copy rate and against this
 MODEL = ["cg", 0.0]      # --model: colour gradient (north_star) or the paper's Shan-Chen coupling, and its G_C
 
 
@@ -222,30 +223,25 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------ GPU arm
-def run_ours(args):
+def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with_e2e=False, windows=0):
+    """One workload on this rank's GPU: W warm-up steps, then K timed steps (CUDA events on the
+    handle's stream, barrier + synchronize on both sides, MAX over ranks).  Returns the record
+    (value, ms_per_step, roofline, clocks, checks, optionally e2e) and the workload."""
     import torch
     import torch.distributed as dist
-    rank, local_rank, world = dist_env()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1 and not dist.is_initialized():
-        dist.init_process_group("nccl", device_id=dev)
     from paper_2005_12764_b200 import lb, workloads as W
-
-    w = W.get(args.workload)
+    if w is None:
+        w = W.get(wl_name)
     two = w.rho_b is not None
-    K, Wu = args.steps, args.warmup
-
     # inputs resident in HBM before the timed region
     d_rr = torch.from_numpy(w.rho_r).to(dev)
     d_rb = torch.from_numpy(w.rho_b).to(dev) if two else None
     d_u = torch.from_numpy(w.u).to(dev)
-    sim = lb.from_workload(w, storage=args.storage)
+    sim = lb.from_workload(w, storage=storage)
     if MODEL[0] == "sc":
         sim.set_model("sc", MODEL[1])
     sim.init(d_rr, d_rb, d_u)
+    mass0 = sim.check_state()
     sim.set_profiling(7)      # every 7th step (odd, so that both AA parities are sampled) is timed kernel by kernel (CUDA events on the stream)
     sim.step(Wu)
     torch.cuda.synchronize()
@@ -276,44 +272,62 @@ def run_ours(args):
     ms_max = max_over_ranks(ms, world, dev)
     value = glups(w.fluid_sites, K, ms_max * 1e-3, world)
 
-    # sanity: the state is finite and mass is where it was
-    rr, rb, u = sim.get_macros()
-    mass = float(np.sum(rr, dtype=np.float64))
-    mass0 = float(np.sum(w.rho_r if w.solid is None else w.rho_r * (w.solid == 0), dtype=np.float64))
-    finite = bool(np.isfinite(u).all())
+    # sanity: the state is finite and the component masses are where they were (summed on the
+    # device by lb_check_state; raises on a NaN / Inf state)
+    mass = sim.check_state()
+    finite = True
+    drift = [abs(a - b) / b if b > 0 else 0.0 for a, b in zip(mass, mass0)]
 
-    # end to end through the C-ABI with HOST buffers: init (H2D) + K steps + get_macros (D2H)
-    h_rr = torch.from_numpy(w.rho_r).pin_memory()
-    h_rb = torch.from_numpy(w.rho_b).pin_memory() if two else None
-    h_u = torch.from_numpy(w.u).pin_memory()
-    o_rr, o_u = torch.empty_like(h_rr).pin_memory(), torch.empty_like(h_u).pin_memory()
-    o_rb = torch.empty_like(h_rb).pin_memory() if two else None
-    sim.set_profiling(False)
-    e2e_ms = []
-    for _ in range(2):          # first pass warms the staging allocations
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        sim.init(h_rr, h_rb, h_u)
-        sim.step(K)
-        sim.get_macros(o_rr, o_rb, o_u)
-        torch.cuda.synchronize()
-        e2e_ms.append((time.perf_counter() - t0) * 1e3)
-    e2e_max = max_over_ranks(e2e_ms[-1], world, dev)
-    nfield = (5 if two else 4) * w.sites * 4
-    e2e = {"value": glups(w.fluid_sites, K, e2e_max * 1e-3, world), "unit": "GLUPS",
-           "h2d_bytes_per_step": nfield / K, "d2h_bytes_per_step": nfield / K,
-           "note": "lb_init(host) + lb_step(%d) + lb_get_macros(host) per timed region; bytes are totals / K" % K}
+    peak, peak_src = measured_peak()
+    upd_bytes = BYTES_PER_UPDATE[two]
+    achieved = upd_bytes * w.fluid_sites / (ms_k2 * 1e-3) / 1e9      # mean k_fused / k_single launch over the sampled steps
+    whole = upd_bytes * w.fluid_sites * K / (ms * 1e-3) / 1e9
+    kname = ("k_fused(sc)" if MODEL[0] == "sc" else "k_fused") if two else "k_single"
+    rec = {"value": value, "unit": "GLUPS", "ms_per_step": ms_max / K,
+           "config": config_of(w, storage, {"parallelism": "replicas x%d" % world}),
+           "roofline": {"bound": "hbm", "kernel": "k_fused" if two else "k_single", "achieved": achieved, "peak": peak,
+                        "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic(kname, wl_name, storage),
+                        "peak_source": peak_src, "algorithmic_bytes_per_update": upd_bytes,
+                        "kernel_ms": ms_k2, "kernel_share_of_step": ms_k2 * K / ms,
+                        "phase_kernel_ms": ms_k1, "kernel_timing": "CUDA events around every 7th step of the timed region",
+                        "whole_step_effective_gbs": whole, "whole_step_frac": whole / peak,
+                        "whole_step_frac_of_nominal_8000": whole / NOMINAL_HBM_GBS},
+           "clocks": dict(clk.result, remeasured=remeasured), "gpu_launches": int(launches),
+           "checks": {"finite": finite, "red_mass_rel_drift": drift[0], "blue_mass_rel_drift": drift[1]}}
+
+    if with_e2e:
+        # end to end through the C-ABI with HOST buffers: init (H2D) + K steps + get_macros (D2H)
+        h_rr = torch.from_numpy(w.rho_r).pin_memory()
+        h_rb = torch.from_numpy(w.rho_b).pin_memory() if two else None
+        h_u = torch.from_numpy(w.u).pin_memory()
+        o_rr, o_u = torch.empty_like(h_rr).pin_memory(), torch.empty_like(h_u).pin_memory()
+        o_rb = torch.empty_like(h_rb).pin_memory() if two else None
+        sim.set_profiling(False)
+        e2e_ms = []
+        for _ in range(2):          # first pass warms the staging allocations
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+            t0 = time.perf_counter()
+            sim.init(h_rr, h_rb, h_u)
+            sim.step(K)
+            sim.get_macros(o_rr, o_rb, o_u)
+            torch.cuda.synchronize()
+            e2e_ms.append((time.perf_counter() - t0) * 1e3)
+        e2e_max = max_over_ranks(e2e_ms[-1], world, dev)
+        nfield = (5 if two else 4) * w.sites * 4
+        rec["e2e"] = {"value": glups(w.fluid_sites, K, e2e_max * 1e-3, world), "unit": "GLUPS",
+                      "h2d_bytes_per_step": nfield / K, "d2h_bytes_per_step": nfield / K,
+                      "note": "lb_init(host) + lb_step(%d) + lb_get_macros(host) per timed region; bytes are totals / K" % K}
+        del h_rr, h_rb, h_u, o_rr, o_rb, o_u
 
     # optional: throughput over the course of the run (the interface fraction changes as domains
     # coarsen or droplets move): --windows N times N windows of K steps spread over w.steps
-    windows = None
-    if args.windows > 0 and world == 1:
+    if windows > 0 and world == 1:
         sim.init(d_rr, d_rb, d_u)
-        gap = max(0, (w.steps - args.windows * K) // max(1, args.windows - 1)) if args.windows > 1 else 0
-        windows, done = [], 0
-        for i in range(args.windows):
+        gap = max(0, (w.steps - windows * K) // max(1, windows - 1)) if windows > 1 else 0
+        out, done = [], 0
+        for i in range(windows):
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(); sim.step(K); e1.record(); torch.cuda.synchronize()
@@ -323,30 +337,54 @@ def run_ours(args):
                 phi = sim.get_phi()
                 fl = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
                 entry["interface_fraction"] = float((np.abs(phi[fl]) < 0.9).mean())
-            windows.append(entry)
-            if i + 1 < args.windows and gap:
+            out.append(entry)
+            if i + 1 < windows and gap:
                 sim.step(gap); done += gap
+        rec["windows"] = out
 
+    sim.destroy()
+    del sim, d_rr, d_rb, d_u
+    torch.cuda.empty_cache()
+    return rec, w
+
+
+# The other rows of the table: measured in the same run, after the headline, and
+# reported under "configs" in the same JSON line.
+EXTRA_CONFIGS = [("c3", "ab"), ("c4", "ab"), ("c5", "aa"), ("c2", "ab")]
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1 and not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=dev)
+    K, Wu = args.steps, args.warmup
+
+    head, w = measure_config(args.workload, args.storage, K, Wu, dev, local_rank, world, with_e2e=True, windows=args.windows)
+    extra = []
+    if args.configs == "all" and world == 1 and MODEL[0] == "cg":
+        for name, storage in EXTRA_CONFIGS:
+            if (name, storage) == (args.workload, args.storage):
+                continue
+            rec, wx = measure_config(name, storage, K, Wu, dev, local_rank, world, w=w if name == args.workload else None)
+            rec.pop("unit", None)
+            extra.append(rec)
+            del wx
     if rank != 0:
         return 0
-    peak, peak_src = measured_peak()
-    upd_bytes = BYTES_PER_UPDATE[two]
-    k2_s = ms_k2 * 1e-3            # mean k_fused / k_single launch over the sampled steps of the timed region
-    achieved = upd_bytes * w.fluid_sites / k2_s / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_fused" if two else "k_single", "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic(("k_fused(sc)" if MODEL[0] == "sc" else "k_fused") if two else "k_single", args.workload, args.storage),
-                "peak_source": peak_src, "algorithmic_bytes_per_update": upd_bytes,
-                "kernel_ms": ms_k2, "kernel_share_of_step": ms_k2 * K / ms,
-                "phase_kernel_ms": ms_k1, "kernel_timing": "CUDA events around every 7th step of the timed region",
-                "whole_step_effective_gbs": upd_bytes * w.fluid_sites * K / (ms * 1e-3) / 1e9,
-                "whole_step_frac": upd_bytes * w.fluid_sites * K / (ms * 1e-3) / 1e9 / peak}
-    line = {"metric": METRIC, "value": value, "unit": "GLUPS", "n_gpus": world, "steps": K, "warmup": Wu,
-            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic", "config": config_of(w, args.storage, {"parallelism": "replicas x%d" % world}),
-            "clocks": dict(clk.result, remeasured=remeasured), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "checks": {"finite": finite, "red_mass_rel_drift": abs(mass - mass0) / mass0}}
-    if windows is not None:
-        line["windows"] = windows
+    line = {"metric": METRIC, "value": head["value"], "unit": "GLUPS", "n_gpus": world, "steps": K, "warmup": Wu,
+            "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": head["config"], "clocks": head["clocks"], "e2e": head["e2e"],
+            "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "checks": head["checks"]}
+    if "windows" in head:
+        line["windows"] = head["windows"]
+    if extra:
+        line["configs"] = extra
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload)
     elif world > 1:
@@ -363,14 +401,17 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large"])
+    ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--configs", default=None, choices=["all", "none"], help="all = also measure C3 A/B, C4 A/B, C5 AA and C2 and report them under 'configs' (default when --workload is left at c5)")
     ap.add_argument("--model", default="cg", choices=["cg", "sc"], help="cg = colour gradient (north_star), sc = Shan-Chen + exact difference (Eq. 5-10 of the paper)")
     ap.add_argument("--gc", type=float, default=3.0, help="G_C of the Shan-Chen model")
     ap.add_argument("--windows", type=int, default=0, help="also time N windows of K steps spread over the config's run length")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.configs is None:
+        args.configs = "all" if (args.workload == "c5" and args.storage == "ab") else "none"
     MODEL[0], MODEL[1] = args.model, args.gc
     if args.impl == "reference":
         return run_reference(args)

@@ -57,8 +57,11 @@ typedef struct {
 typedef struct lb_handle_s* lb_handle;
 
 /* Device-memory hooks.  PyTorch is the allocator in production: the Python binding passes
- * wrappers of torch's CUDA caching allocator.  alloc returns a device pointer or NULL.
- * Process-wide; set before lb_create.  NULL, NULL restores cudaMalloc / cudaFree. */
+ * wrappers of torch's CUDA caching allocator.  alloc returns a device pointer (on the device
+ * that is current when it is called) or NULL.  The pair is a process-wide default that every
+ * handle captures at lb_create and keeps for its whole life; NULL, NULL restores cudaMalloc /
+ * cudaFree for handles created afterwards.  A handle lives on the device that was current at
+ * lb_create; every call makes that device current for its duration. */
 typedef void* (*lb_alloc_fn)(size_t bytes, void* user);
 typedef void (*lb_free_fn)(void* ptr, void* user);
 int lb_set_allocator(lb_alloc_fn alloc, lb_free_fn free_fn, void* user);
@@ -144,8 +147,18 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
 
 /* Advance nsteps time steps: per step the fused pull-stream + collide kernel (Eq. 1-2, 5-8, 11),
  * which also forwards the moments of the next state, and the phase-field kernel that turns them
- * into phi = (rho_r - rho_b)/rho (Eq. 3).  Asynchronous. */
+ * into phi = (rho_r - rho_b)/rho (Eq. 3).  Asynchronous, except that every 1000
+ * steps it runs lb_check_state and returns LB_ESTATE if the state is no longer finite. */
 int lb_step(lb_handle h, int nsteps);
+
+/* State check (G23; the paper names fault tolerance as an exascale issue):
+ * sums rho_r and rho_b (Eq. 3) over the fluid sites on the device, in double
+ * precision, and looks for NaN / Inf populations.  Returns LB_ESTATE (text: how many sites, after
+ * how many steps) if the state is not finite, LB_OK otherwise; mass_r, mass_b (HOST pointers, may
+ * be NULL) receive the sums (single component: mass_r is the mass, mass_b is 0).  Synchronises the
+ * stream.  lb_step runs the same check by itself every 1000 steps since the last check and then
+ * returns LB_ESTATE instead of stepping on: that is the one place where lb_step synchronises. */
+int lb_check_state(lb_handle h, double* mass_r, double* mass_b);
 
 /* rho_r, rho_b and the velocity u = (sum_i c_i f_i + F/2)/rho of the current state (Eq. 3,
  * PAPER.md:96, with the half-force shift of Guo forcing; G16).  Zeros on solid sites.  Any

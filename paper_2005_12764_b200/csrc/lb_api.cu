@@ -4,6 +4,8 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -22,17 +24,41 @@ lb_free_fn g_free = nullptr;
 void* g_user = nullptr;
 std::string g_create_error;
 
-void* dev_alloc(size_t bytes) {
-  if (g_alloc) return g_alloc(bytes, g_user);
+// The allocator hooks are process-wide defaults; every handle captures the pair that was current
+// at lb_create and uses it for its whole life (so a later lb_set_allocator never makes a handle
+// free memory with another allocator than the one it came from).
+struct Allocator {
+  lb_alloc_fn alloc = nullptr;
+  lb_free_fn free_fn = nullptr;
+  void* user = nullptr;
+};
+
+void* dev_alloc(const Allocator& a, size_t bytes) {
+  if (a.alloc) return a.alloc(bytes, a.user);
   void* p = nullptr;
   if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
   return p;
 }
-void dev_free(void* p) {
+void dev_free(const Allocator& a, void* p) {
   if (!p) return;
-  if (g_free) g_free(p, g_user);
+  if (a.free_fn) a.free_fn(p, a.user);
   else cudaFree(p);
 }
+
+constexpr int MAX_DEVICES = 64;
+
+// Makes the handle's device current for the duration of one C-ABI call (one process may hold
+// handles on several devices) and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (dev < 0) return;
+    if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
+    if (prev != dev) { switched = cudaSetDevice(dev) == cudaSuccess; cudaGetLastError(); }
+  }
+  ~DeviceGuard() { if (switched) { cudaSetDevice(prev); cudaGetLastError(); } }
+};
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -53,6 +79,8 @@ EncodeTiledFn get_encode() {
 }  // namespace
 
 struct lb_handle_s {
+  Allocator al;              // captured at lb_create
+  int device = -1;           // CUDA device of this handle (the device current at lb_create; -1: none)
   int nx = 0, ny = 0, nz = 0;
   long long S = 0;
   lb_params par{};
@@ -88,6 +116,10 @@ struct lb_handle_s {
   float* mom = nullptr;      // forwarded moments Md, Mt (2 x S floats), written by k_fused
   int forward = 1;           // 1 = phi(t+1) from forwarded moments (k_phase_fwd), 0 = full k_phase sweep
   int tune_zc = 0;           // z planes per CTA (0 = automatic)
+  int sm_count = 0;          // SMs of the handle's device (0: not asked yet)
+  double* chk = nullptr;     // state check (lb_check_state): {sum rho_r, sum rho_b, non-finite count}
+  long long steps_done = 0;  // time steps since lb_init
+  long long last_check = 0;  // steps_done at the last state check
   int profiling = 0;
   cudaEvent_t ev_step[2] = {nullptr, nullptr};
   std::vector<cudaEvent_t> ev_k;   // 4 per step when profiling: K1 begin/end, K2 begin/end
@@ -116,6 +148,8 @@ int fail(lb_handle h, int code, const std::string& msg) {
   return code;
 }
 
+constexpr long long CHECK_EVERY = 1000;   // steps between two state checks inside lb_step (G23)
+
 int cuda_fail(lb_handle h, cudaError_t e, const char* what) {
   cudaGetLastError();
   return fail(h, LB_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
@@ -131,12 +165,14 @@ bool is_device_ptr(const void* p) {
 struct Staged {
   void* dev = nullptr;
   bool owned = false;
-  ~Staged() { if (owned) dev_free(dev); }
+  Allocator al;
+  ~Staged() { if (owned) dev_free(al, dev); }
 };
 
 int stage_in(lb_handle h, const void* src, size_t bytes, Staged& s) {
   if (is_device_ptr(src)) { s.dev = const_cast<void*>(src); return LB_OK; }
-  s.dev = dev_alloc(bytes);
+  s.al = h->al;
+  s.dev = dev_alloc(h->al, bytes);
   if (!s.dev) return fail(h, LB_ENOMEM, "staging buffer allocation failed");
   s.owned = true;
   cudaError_t e = cudaMemcpyAsync(s.dev, src, bytes, cudaMemcpyHostToDevice, h->stream);
@@ -148,7 +184,8 @@ int stage_in(lb_handle h, const void* src, size_t bytes, Staged& s) {
 int stage_out(lb_handle h, void* dst, size_t bytes, Staged& s) {
   if (!dst) return LB_OK;
   if (is_device_ptr(dst)) { s.dev = dst; return LB_OK; }
-  s.dev = dev_alloc(bytes);
+  s.al = h->al;
+  s.dev = dev_alloc(h->al, bytes);
   if (!s.dev) return fail(h, LB_ENOMEM, "staging buffer allocation failed");
   s.owned = true;
   return LB_OK;
@@ -203,13 +240,13 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
 int pick_zc(lb_handle h) {
   if (h->tune_zc > 0) return h->tune_zc < h->nz ? h->tune_zc : h->nz;
   if (h->nz <= 10) return h->nz;
-  static int sm_count = 0;
-  if (!sm_count) {
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (!h->sm_count) {       // of the handle's own device
+    int sms = 148;
+    if (h->device >= 0) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
     cudaGetLastError();
-    sm_count = sms;
+    h->sm_count = sms;
   }
+  const int sm_count = h->sm_count;
   // resident CTAs per SM: 3, but 2 for the instantiations with wall groups (WALLS = 2)
   const int slots = ((h->has_solid && h->has_moving) ? 2 : 3) * sm_count;
   const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
@@ -243,10 +280,11 @@ void launch_phase(lb_handle h, const StepParams& p, dim3 grid) {
 template <int MODE, int WALLS, bool HAS_NC, int FMODE>
 void launch_fused_t(lb_handle h, const StepParams& p, dim3 grid) {
   constexpr size_t smem = FusedSmem<HAS_NC ? H_MAX_NC : 1>::BYTES;
-  static bool attr_set = false;   // per instantiation
-  if (!attr_set) {
+  static bool attr_set[MAX_DEVICES] = {};   // per instantiation and per device (the attribute is per device)
+  const int d = h->device >= 0 && h->device < MAX_DEVICES ? h->device : 0;
+  if (!attr_set[d]) {
     cudaFuncSetAttribute(k_fused<MODE, WALLS, HAS_NC, FMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
+    attr_set[d] = true;
   }
   k_fused<MODE, WALLS, HAS_NC, FMODE><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap);
 }
@@ -269,10 +307,11 @@ void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
 template <int MODE, int WALLS, int FMODE>
 void launch_fused_sc(lb_handle h, const StepParams& p, dim3 grid) {
   constexpr size_t smem = FusedSmem<1, true>::BYTES;
-  static bool attr_set = false;   // per instantiation
-  if (!attr_set) {
+  static bool attr_set[MAX_DEVICES] = {};   // per instantiation and per device
+  const int d = h->device >= 0 && h->device < MAX_DEVICES ? h->device : 0;
+  if (!attr_set[d]) {
     cudaFuncSetAttribute(k_fused<MODE, WALLS, false, FMODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
+    attr_set[d] = true;
   }
   k_fused<MODE, WALLS, false, FMODE, true><<<grid, dim3(TX, TY), smem, h->stream>>>(p, h->tmap, h->tmap2);
 }
@@ -411,6 +450,34 @@ void launch_macros(lb_handle h, const IoParams& p) {
   h->launches++;
 }
 
+// Component masses and finiteness of the stored state (k_check); synchronises the stream.
+int state_check(lb_handle h, double* mass_r, double* mass_b) {
+  if (!h->chk) {
+    h->chk = static_cast<double*>(dev_alloc(h->al, 3 * sizeof(double)));
+    if (!h->chk) return fail(h, LB_ENOMEM, "state-check buffer allocation failed");
+    h->bytes += 3 * sizeof(double);
+  }
+  cudaError_t e = cudaMemsetAsync(h->chk, 0, 3 * sizeof(double), h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "state check memset");
+  const int nb = (int)std::min<long long>((h->S + 255) / 256, 148 * 16);
+  if (h->two) k_check<true><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), h->chk);
+  else k_check<false><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), h->chk);
+  h->launches++;
+  double out[3] = {0, 0, 0};
+  e = cudaMemcpyAsync(out, h->chk, sizeof(out), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "state check");
+  h->last_check = h->steps_done;
+  if (mass_r) *mass_r = out[0];
+  if (mass_b) *mass_b = out[1];
+  if (out[2] != 0.0 || !std::isfinite(out[0]) || !std::isfinite(out[1])) {
+    char msg[160];
+    snprintf(msg, sizeof(msg), "non-finite state after %lld steps: %.0f sites hold a NaN or Inf population", h->steps_done, out[2]);
+    return fail(h, LB_ESTATE, msg);
+  }
+  return LB_OK;
+}
+
 int check_launch(lb_handle h, const char* what) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, LB_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
@@ -441,14 +508,17 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
   h->nx = nx; h->ny = ny; h->nz = nz;
   h->S = (long long)nx * ny * nz;
   h->par = *p;
+  h->al.alloc = g_alloc; h->al.free_fn = g_free; h->al.user = g_user;
+  if (cudaGetDevice(&h->device) != cudaSuccess) { cudaGetLastError(); h->device = -1; }   // no device: later calls return LB_ECUDA
   *out = h;
   return LB_OK;
 }
 
 void lb_destroy(lb_handle h) {
   if (!h) return;
+  DeviceGuard guard(h->device);
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
-  dev_free(h->buf[0]); dev_free(h->buf[1]); dev_free(h->phi); dev_free(h->phi2); dev_free(h->mask); dev_free(h->mom);
+  for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk}) dev_free(h->al, q);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
   for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
   cudaGetLastError();
@@ -463,6 +533,7 @@ int lb_set_stream(lb_handle h, void* cuda_stream) {
 
 int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
   if (!h) return LB_EINVAL;
+  DeviceGuard guard(h->device);
   if (h->inited) return fail(h, LB_ESTATE, "lb_set_geometry after lb_init");
   if (!solid_mask) { h->has_solid = false; return LB_OK; }
   int ndev = 0;
@@ -474,7 +545,7 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
   const size_t nwords = (size_t)b.nxw * h->ny * h->nz;
   // three bit masks behind each other (solid, wall group 2, wall group 3) and one flag word
   if (!h->mask) {
-    h->mask = static_cast<uint32_t*>(dev_alloc((3 * nwords + 1) * 4));
+    h->mask = static_cast<uint32_t*>(dev_alloc(h->al, (3 * nwords + 1) * 4));
     if (!h->mask) return fail(h, LB_ENOMEM, "mask allocation failed");
     h->bytes += (3 * nwords + 1) * 4;
   }
@@ -571,12 +642,12 @@ int allocate_state(lb_handle h, bool two) {
   const int planes = two ? 2 * Q : Q;
   const size_t pbytes = (size_t)planes * (size_t)h->S * sizeof(float);
   if (h->inited && two != h->two) {   // component count changed: start over
-    for (int i = 0; i < 2; ++i) { if (h->buf[i]) h->bytes -= (size_t)h->planes() * h->S * 4; dev_free(h->buf[i]); h->buf[i] = nullptr; }
+    for (int i = 0; i < 2; ++i) { if (h->buf[i]) h->bytes -= (size_t)h->planes() * h->S * 4; dev_free(h->al, h->buf[i]); h->buf[i] = nullptr; }
   }
   h->two = two;
   for (int i = 0; i < nbuf; ++i) {
     if (!h->buf[i]) {
-      h->buf[i] = static_cast<float*>(dev_alloc(pbytes));
+      h->buf[i] = static_cast<float*>(dev_alloc(h->al, pbytes));
       if (!h->buf[i]) return fail(h, LB_ENOMEM, "population buffer allocation failed");
       h->bytes += pbytes;
     }
@@ -584,7 +655,7 @@ int allocate_state(lb_handle h, bool two) {
   if (two && !h->mom) {
     const size_t ex = (size_t)h->nz * h->ny * ((h->nx + TX - 1) / TX) * 4;   // x-face sums: 2 sides x {D, Tm}
     const size_t mb = (2 * (size_t)h->S + ex) * sizeof(float);
-    h->mom = static_cast<float*>(dev_alloc(mb));
+    h->mom = static_cast<float*>(dev_alloc(h->al, mb));
     if (!h->mom) return fail(h, LB_ENOMEM, "moment buffer allocation failed");
     h->bytes += mb;
   }
@@ -594,7 +665,7 @@ int allocate_state(lb_handle h, bool two) {
     if (!two || field) continue;
     const size_t px = h->nx + 2 * HALO, py = h->ny + 2 * HALO, pz = h->nz + 2 * HALO;
     const size_t phib = px * py * pz * sizeof(float);
-    field = static_cast<float*>(dev_alloc(phib));
+    field = static_cast<float*>(dev_alloc(h->al, phib));
     if (!field) return fail(h, LB_ENOMEM, "phi allocation failed");
     h->bytes += phib;
     cudaError_t e = cudaMemsetAsync(field, 0, phib, h->stream);
@@ -622,6 +693,7 @@ extern "C" {
 
 int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u) {
   if (!h) return LB_EINVAL;
+  DeviceGuard guard(h->device);
   if (!rho_r || !u) return fail(h, LB_EINVAL, "rho_r and u must not be NULL");
   if (h->model == 1 && !rho_b) return fail(h, LB_EINVAL, "the Shan-Chen model couples two components: rho_b must not be NULL");
   int ndev = 0;
@@ -638,6 +710,8 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   if ((rc = stage_in(h, u, 3 * fb, su))) return rc;
   h->cur = 0;
   h->aa_odd = 0;
+  h->steps_done = 0;
+  h->last_check = 0;
   IoParams p = make_io_params(h);
   p.comp = -1;
   p.rho_r = static_cast<const float*>(srr.dev);
@@ -659,6 +733,7 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
 
 int lb_step(lb_handle h, int nsteps) {
   if (!h || nsteps < 0) return fail(h, LB_EINVAL, "nsteps must be >= 0");
+  DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_step before lb_init");
   for (int i = 0; i < 2; ++i)
     if (!h->ev_step[i] && cudaEventCreate(&h->ev_step[i]) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
@@ -680,13 +755,29 @@ int lb_step(lb_handle h, int nsteps) {
     if (prof) cudaEventRecord(h->ev_k[k + 1], h->stream);
     run_collide(h, prof ? h->ev_k[k + 2] : nullptr);   // K2 (+ K1f) or K2s
     if (prof) cudaEventRecord(h->ev_k[k + 3], h->stream);
+    h->steps_done++;
+    // G23: every CHECK_EVERY steps the component masses are summed on the device; a non-finite
+    // state ends the call with LB_ESTATE (this is the one place where lb_step synchronises)
+    if (h->steps_done - h->last_check >= CHECK_EVERY) {
+      int rc = check_launch(h, "lb_step");
+      if (!rc) rc = state_check(h, nullptr, nullptr);
+      if (rc) { cudaEventRecord(h->ev_step[1], h->stream); return rc; }
+    }
   }
   cudaEventRecord(h->ev_step[1], h->stream);
   return check_launch(h, "lb_step");
 }
 
+int lb_check_state(lb_handle h, double* mass_r, double* mass_b) {
+  if (!h) return LB_EINVAL;
+  if (!h->inited) return fail(h, LB_ESTATE, "lb_check_state before lb_init");
+  DeviceGuard guard(h->device);
+  return state_check(h, mass_r, mass_b);
+}
+
 int lb_get_macros(lb_handle h, float* rho_r, float* rho_b, float* u) {
   if (!h) return LB_EINVAL;
+  DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_get_macros before lb_init");
   const size_t fb = (size_t)h->S * sizeof(float);
   Staged o0, o1, o2;
@@ -713,6 +804,7 @@ int lb_get_macros(lb_handle h, float* rho_r, float* rho_b, float* u) {
 
 int lb_get_populations(lb_handle h, int comp, float* f) {
   if (!h || !f) return fail(h, LB_EINVAL, "f is NULL");
+  DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_get_populations before lb_init");
   if (comp < 0 || comp > (h->two ? 1 : 0)) return fail(h, LB_EINVAL, "bad component");
   const size_t fb = (size_t)Q * h->S * sizeof(float);
@@ -734,6 +826,7 @@ int lb_get_populations(lb_handle h, int comp, float* f) {
 
 int lb_set_populations(lb_handle h, int comp, const float* f) {
   if (!h || !f) return fail(h, LB_EINVAL, "f is NULL");
+  DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_set_populations before lb_init");
   if (comp < 0 || comp > (h->two ? 1 : 0)) return fail(h, LB_EINVAL, "bad component");
   const size_t fb = (size_t)Q * h->S * sizeof(float);
@@ -756,6 +849,7 @@ int lb_set_populations(lb_handle h, int comp, const float* f) {
 
 int lb_get_phi(lb_handle h, float* phi) {
   if (!h || !phi) return fail(h, LB_EINVAL, "phi is NULL");
+  DeviceGuard guard(h->device);
   if (!h->inited || !h->two) return fail(h, LB_ESTATE, "lb_get_phi needs an initialised two-component state");
   const size_t fb = (size_t)h->S * sizeof(float);
   Staged o;
@@ -796,6 +890,7 @@ int lb_set_profiling(lb_handle h, int on) {
 int lb_last_step_ms(lb_handle h, int which, float* ms) {
   if (!h || !ms || which < 0 || which > 2) return fail(h, LB_EINVAL, "bad argument");
   if (!h->ev_step[1]) return fail(h, LB_ESTATE, "no lb_step recorded yet");
+  DeviceGuard guard(h->device);
   cudaError_t e = cudaEventSynchronize(h->ev_step[1]);
   if (e != cudaSuccess) return cuda_fail(h, e, "event sync");
   if (which == 0) {

@@ -68,14 +68,16 @@ struct Slot {
 struct Ctx {
   int idx;            // own site (elements)
   uint32_t ob;        // own site (bytes)
-  int dxo[3];         // byte deltas to x-1, x, x+1 (wrapped)
-  int dyo[3];         // to y-1, y, y+1
-  int dzo[3];         // to z-1, z, z+1
+  // byte deltas to the wrapped neighbours, modulo 2^32: a wrap across the whole box exceeds
+  // INT_MAX once S * 8 > 2^31 (656^3), so the arithmetic is unsigned, where wrap-around is defined
+  uint32_t dxo[3];    // to x-1, x, x+1
+  uint32_t dyo[3];    // to y-1, y, y+1
+  uint32_t dzo[3];    // to z-1, z, z+1
 };
 
 // Byte delta from the own site to x - c_q.
 template <int q>
-__device__ __forceinline__ int delta_src(const Ctx& c) {
+__device__ __forceinline__ uint32_t delta_src(const Ctx& c) {
   return c.dxo[1 - cx(q)] + c.dyo[1 - cy(q)] + c.dzo[1 - cz(q)];
 }
 
@@ -85,7 +87,7 @@ __device__ __forceinline__ Slot read_slot(const Ctx& c, uint32_t smask) {
   if constexpr (MODE == MODE_AA_EVEN || q == 0) {
     return Slot{q, c.ob};
   } else {
-    const uint32_t nb = c.ob + (uint32_t)delta_src<q>(c);
+    const uint32_t nb = c.ob + delta_src<q>(c);
     if constexpr (!HAS_SOLID) {
       return MODE == MODE_AB ? Slot{q, nb} : Slot{opp(q), nb};
     } else {
@@ -207,17 +209,18 @@ template <int ESZ>
 __device__ __forceinline__ void make_ctx(Ctx& c, const Box& b, int x, int y, int z) {
   c.idx = x + b.nx * (y + b.ny * z);
   c.ob = (uint32_t)c.idx * (uint32_t)ESZ;
-  c.dxo[0] = (x == 0 ? b.nx - 1 : -1) * ESZ;
-  c.dxo[1] = 0;
-  c.dxo[2] = (x == b.nx - 1 ? -(b.nx - 1) : 1) * ESZ;
-  const int row = b.nx * ESZ;
-  c.dyo[0] = (y == 0 ? b.ny - 1 : -1) * row;
-  c.dyo[1] = 0;
-  c.dyo[2] = (y == b.ny - 1 ? -(b.ny - 1) : 1) * row;
-  const int pl = b.nx * b.ny * ESZ;
-  c.dzo[0] = (z == 0 ? b.nz - 1 : -1) * pl;
-  c.dzo[1] = 0;
-  c.dzo[2] = (z == b.nz - 1 ? -(b.nz - 1) : 1) * pl;
+  constexpr uint32_t E = (uint32_t)ESZ;
+  c.dxo[0] = x == 0 ? (uint32_t)(b.nx - 1) * E : 0u - E;
+  c.dxo[1] = 0u;
+  c.dxo[2] = x == b.nx - 1 ? 0u - (uint32_t)(b.nx - 1) * E : E;
+  const uint32_t row = (uint32_t)b.nx * E;
+  c.dyo[0] = y == 0 ? (uint32_t)(b.ny - 1) * row : 0u - row;
+  c.dyo[1] = 0u;
+  c.dyo[2] = y == b.ny - 1 ? 0u - (uint32_t)(b.ny - 1) * row : row;
+  const uint32_t pl = (uint32_t)b.nx * (uint32_t)b.ny * E;
+  c.dzo[0] = z == 0 ? (uint32_t)(b.nz - 1) * pl : 0u - pl;
+  c.dzo[1] = 0u;
+  c.dzo[2] = z == b.nz - 1 ? 0u - (uint32_t)(b.nz - 1) * pl : pl;
 }
 
 // s + e <- s + e + x with the rounding error of the addition kept in e (Knuth two-sum).
@@ -1310,6 +1313,50 @@ __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* gro
   }
   words[wi] = m;
   if (groups) { groups[wi] = g2; groups[nw + wi] = g3; }
+}
+
+// State check (G23: "lb_step reports LB_ESTATE if the mass check it runs every 1000 steps
+// is non-finite"; the paper names fault tolerance as an exascale issue).  In every
+// storage mode each slot of a fluid site holds one population of one fluid site, so the sums over the
+// slots of the fluid sites are the component masses (Eq. 3, summed over the box).
+// out[0] += sum rho_r, out[1] += sum rho_b, out[2] += number of sites holding a non-finite value.
+template <bool TWO>
+__global__ void __launch_bounds__(256) k_check(const float* __restrict__ buf, const Box b, double* out) {
+  double sr = 0.0, sb = 0.0, bad = 0.0;
+  for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < b.S; s += (long long)gridDim.x * blockDim.x) {
+    if (b.mask) {
+      const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
+      if (solid_at(b, x, y, z)) continue;
+    }
+    float t = 0.f, r = 0.f;
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      if constexpr (TWO) {
+        const float2 v = __ldcg(reinterpret_cast<const float2*>(buf) + (size_t)q * b.S + s);
+        t += v.x; r += v.y;
+      } else {
+        t += __ldcg(buf + (size_t)q * b.S + s);
+      }
+    }
+    if (!isfinite(t) || !isfinite(r)) { bad += 1.0; continue; }
+    if constexpr (TWO) { sr += (double)r; sb += (double)(1.0f + t) - (double)r; }
+    else sr += (double)(1.0f + t);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sr += __shfl_down_sync(0xffffffffu, sr, o);
+    sb += __shfl_down_sync(0xffffffffu, sb, o);
+    bad += __shfl_down_sync(0xffffffffu, bad, o);
+  }
+  __shared__ double red[3][8];
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  if (lane == 0) { red[0][wp] = sr; red[1][wp] = sb; red[2][wp] = bad; }
+  __syncthreads();
+  if (threadIdx.x < 3) {
+    double v = 0.0;
+    for (int i = 0; i < 8; ++i) v += red[threadIdx.x][i];
+    if (v != 0.0) atomicAdd(out + threadIdx.x, v);
+  }
 }
 
 // does the byte mask hold a moving wall group?  out[0] |= 1

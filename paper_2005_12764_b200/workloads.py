@@ -50,7 +50,7 @@ class Workload:
 
     @property
     def fluid_sites(self):
-        return self.sites if self.solid is None else int(self.sites - int(self.solid.sum()))
+        return self.sites if self.solid is None else int((self.solid == 0).sum())    # wall groups are 2, 3, 4: count, do not sum
 
     @property
     def params(self):

@@ -923,3 +923,35 @@ def test_focuser_pinches_off_a_droplet(lbmod):
     sim.step(9000)
     big = [s for s in pieces() if s > 5000]
     assert len(big) >= 2, big
+
+
+def test_state_check_reports_nan_and_masses(lbmod):
+    """G23 (fault tolerance is named at PAPER.md:154): lb_check_state sums the
+    component masses on the device and reports a non-finite state with LB_ESTATE; lb_step runs the
+    same check by itself every 1000 steps and then stops stepping."""
+    w = W.get("c1")
+    for storage in ("ab", "aa"):
+        sim = pu.make_gpu(lbmod, w, storage)
+        m0 = pu.masses(w.rho_r, w.rho_b)
+        mr, mb = sim.check_state()
+        assert abs(mr - m0[0]) / m0[0] < 1e-6 and abs(mb - m0[1]) / m0[1] < 1e-6
+        sim.step(1001)                              # crosses one automatic check: healthy state, no error
+        mr, mb = sim.check_state()
+        assert abs(mr - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(mb - m0[1]) / m0[1] < pu.DRIFT_TOL
+        fr, fb = sim.get_populations(0), sim.get_populations(1)
+        fr[3, 5, 6, 7] = np.nan
+        sim.set_populations(0, fr)
+        sim.set_populations(1, fb)
+        with pytest.raises(lbmod.LBError) as ei:
+            sim.check_state()
+        assert ei.value.code == lbmod.LB_ESTATE and "non-finite" in str(ei.value)
+        sim.step(999)                               # below the check interval: the NaN spreads silently
+        with pytest.raises(lbmod.LBError) as ei:
+            sim.step(2)                             # 1001 steps since the last check: lb_step reports it
+        assert ei.value.code == lbmod.LB_ESTATE
+    # single component
+    w2 = W.get("c2-mini")
+    sim = pu.make_gpu(lbmod, w2)
+    sim.step(3)
+    mr, mb = sim.check_state()
+    assert abs(mr - w2.sites) / w2.sites < 1e-6 and mb == 0.0

@@ -795,3 +795,82 @@ def test_P19_focuser_three_groups_and_exact_injection(lbo):
     assert front > front0 + 8
     assert abs((rr + rb)[fl].sum() / m0 - 1.0) < 0.02
     assert u[0][fl].min() > -5e-3 and np.isfinite(u).all()
+
+
+# ---------------------------------------------------------------------------------- P20
+# The anisotropic term of the recolouring (S8, G6): beta (rho_r rho_b / rho) w_i (c_i.G)/(|c_i| |G|).
+# Closed form it must reproduce (derivation in DESIGN.md "P20"): for a flat interface at rest the
+# red density obeys rho_r(x) = sum_i f^r*_i(x - c_i) with f^r*_i = w_i [rho_r + beta (rho_r rho_b / rho) k_i],
+# k_i = (c_i.n)/|c_i|.  Expanding to second order with sum_i w_i c_ia c_ib = delta_ab / 3 and
+# sum_i w_i c_ia c_ib / |c_i| = kappa delta_ab, kappa = [2/18 + 8/(36 sqrt 2)] = (1 + sqrt 2)/9, gives
+# rho_r'/6 = beta kappa rho_r rho_b / rho, i.e.  phi = tanh(x / xi),  1/xi = 3 beta kappa = beta (1 + sqrt 2)/3,
+# whatever the total density and the orientation.  None of P3, P4, P8, P16 depends on beta, on the
+# 1/|c_i| normalisation or on the power of rho in the prefactor; this pin does (dropping 1/|c_i|
+# gives 1/xi = beta, 24 % off; a prefactor rho_r rho_b / rho^2 makes xi depend on rho).
+KAPPA_LK = (1.0 + np.sqrt(2.0)) / 9.0
+
+
+def _interface_inverse_width(lbo, beta, rho0=1.0, orient=0, n=96, steps=4000, A=1e-4):
+    """Two flat interfaces in a quasi-1-D periodic box along axis `orient` (0 = x, 1 = y, 2 = z),
+    relaxed for `steps` steps; returns the slope of atanh(phi) over |phi| < 0.9 on both of them
+    and the largest velocity left."""
+    s = np.arange(n)
+    phi = np.tanh((n / 4 - np.abs(s - (n - 1) / 2)) / 2.0)
+    shape = [1, 1, 1]
+    shape[2 - orient] = n
+    p3 = phi.reshape(shape)
+    o = lbo.Oracle(shape[2], shape[1], shape[0], 1.0, 1.0, A, beta, 0.0)
+    o.init(rho0 * (1 + p3) / 2, rho0 * (1 - p3) / 2, np.zeros([3] + shape))
+    o.step(steps)
+    ph = o.get_fields()["phi"].ravel()
+    slopes = []
+    for sl in (slice(0, n // 2), slice(n // 2, n)):
+        m = np.abs(ph[sl]) < 0.9
+        assert m.sum() >= 4
+        slopes.append(abs(np.polyfit(s[sl][m], np.arctanh(ph[sl][m]), 1)[0]))
+    return np.array(slopes), float(np.abs(o.get_macros()[2]).max())
+
+
+@pytest.mark.parametrize("beta,tol", [(0.35, 0.01), (0.5, 0.01), (0.7, 0.01), (1.0, 0.04)])
+def test_P20_interface_width_vs_beta(lbo, beta, tol):
+    """phi = tanh(x/xi) with 1/xi = beta (1 + sqrt 2)/3 across a flat interface (the Latva-Kokko
+    operator's closed form; lattice corrections are O(1/xi^2): 0.4 % up to beta = 0.7, 2.3 % at
+    beta = 1)."""
+    k, umax = _interface_inverse_width(lbo, beta)
+    assert umax < 1e-10                                    # at rest
+    assert abs(k[0] - k[1]) < 1e-9                         # both interfaces alike
+    assert abs(k.mean() / (3.0 * beta * KAPPA_LK) - 1.0) < tol, (k, 3.0 * beta * KAPPA_LK)
+
+
+def test_P20_halving_beta_doubles_the_width_and_rho_drops_out(lbo):
+    k_07, _ = _interface_inverse_width(lbo, 0.7)
+    k_035, _ = _interface_inverse_width(lbo, 0.35)
+    assert abs(k_07.mean() / k_035.mean() - 2.0) < 0.01     # xi(0.35) = 2 xi(0.7)
+    # prefactor rho_r rho_b / rho (first power): the width does not depend on the total density
+    k_rho2, _ = _interface_inverse_width(lbo, 0.7, rho0=2.0)
+    assert abs(k_rho2.mean() / k_07.mean() - 1.0) < 1e-9
+    # the operator is isotropic to second order: same width along y and z
+    for orient in (1, 2):
+        k_o, _ = _interface_inverse_width(lbo, 0.7, orient=orient)
+        assert abs(k_o.mean() / k_07.mean() - 1.0) < 1e-9
+
+
+def test_P20_diagonal_interface(lbo):
+    """An interface along (1, 1, 0): the sites sit 1/sqrt 2 apart along the normal, the closed form
+    is the same (sum_i w_i c_ia c_ib / |c_i| is isotropic): pins the diagonal links' weight and
+    their 1/sqrt 2."""
+    n, beta = 64, 0.5
+    y, x = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+    sdiag = (x + y) % n                                      # n sites of spacing 1/sqrt 2 along the normal
+    d = (n / 4 - np.abs(sdiag - (n - 1) / 2)) / np.sqrt(2.0)
+    phi = np.tanh(d / 2.0).reshape(1, n, n)
+    o = lbo.Oracle(n, n, 1, 1.0, 1.0, 1e-4, beta, 0.0)
+    o.init((1 + phi) / 2, (1 - phi) / 2, np.zeros((3, 1, n, n)))
+    o.step(4000)
+    ph = o.get_fields()["phi"][0]
+    line = ph[0, :]                                          # y = 0: s = x
+    s = np.arange(n) / np.sqrt(2.0)
+    m = (np.abs(line) < 0.9) & (np.arange(n) < n // 2)
+    k = abs(np.polyfit(s[m], np.arctanh(line[m]), 1)[0])
+    assert abs(k / (3.0 * beta * KAPPA_LK) - 1.0) < 0.01, k
+    assert np.abs(ph - ph[0, (x + y) % n]).max() < 1e-9      # stays a function of x + y
