@@ -176,6 +176,54 @@ int lb_set_populations(lb_handle h, int comp, const float* f);
 /* phi = (rho_r - rho_b)/(rho_r + rho_b) of the current state, S floats (0 on solid sites). */
 int lb_get_phi(lb_handle h, float* phi);
 
+/* ---- z-slab decomposition over several handles / GPUs -----------------
+ * The paper splits the fluid box equally over the ranks, "according to a either 1D, or 2D or 3D
+ * domain decomposition"; the collision is local ("zero communication",
+ * PAPER.md:161) and streaming reaches first neighbours only.  Here: slabs along z
+ * (x stays contiguous).  A slab handle owns the planes [z0, z0 + nz) of a box of nz_global planes
+ * that is periodic over nz_global; nz is the nz of lb_create.  Internally it holds one ghost
+ * plane below and one above its own planes.  What crosses a z face per step and per direction of
+ * travel: the 5 populations per component with c_z = +1 (or -1), i.e. 5 * nx * ny * 8 bytes (4 for
+ * one component), and H planes of the padded phase field, H = 4 with the near-contact force (its
+ * probe reaches 4 sites), else 1: H * (nx + 8) * (ny + 8) * 4 bytes (twice that in the Shan-Chen
+ * model, whose fields are rho_r and rho_b).  The library packs and unpacks these messages; MOVING
+ * them is the caller's job (ncclSend / ncclRecv through torch.distributed in
+ * paper_2005_12764_b200/slab.py, peer copies, or plain copies between two handles of one process),
+ * so the boundary carries no communicator type.  Message buffers are DEVICE memory, 16-byte
+ * aligned, owned by the caller.  "lo" = the face towards smaller z (the rank below), "hi" = above.
+ *
+ * lb_set_slab(h, z0, nz_global): declares the handle a slab; before lb_set_geometry and lb_init;
+ * nz >= 8; nz_global <= 0 undoes it.  For a slab, lb_set_geometry takes (nz + 2) * ny * nx bytes:
+ * the planes z0 - 1 .. z0 + nz of the global mask (periodic), i.e. including the two ghost planes;
+ * every other array argument (lb_init, lb_get_macros, ...) holds the slab's own nz planes only.
+ * lb_step returns LB_ESTATE for a slab; one time step is, in this order:
+ *   lb_slab_begin(h, send_lo, send_hi)    fused stream-collide on the first and the last brick of
+ *                                         the slab; packs the populations the neighbours need
+ *   [caller: send_hi -> rank above's recv_lo, send_lo -> rank below's recv_hi; may overlap with:]
+ *   lb_slab_interior(h)                   fused kernel on the bricks in between, and the phase
+ *                                         field of the planes that do not wait for the halo
+ *   lb_slab_end(h, recv_lo, recv_hi)      unpacks the received populations into the ghost planes
+ *                                         (after an in-place odd step: into the own boundary
+ *                                         planes), phase field of the H planes next to each face;
+ *                                         the state is then t + 1 (runs the 1000-step state check
+ *                                         like lb_step)
+ *   lb_slab_pack_phi(h, send_lo, send_hi) the H phi planes next to each face
+ *   [caller: exchange as above]
+ *   lb_slab_unpack_phi(h, recv_lo, recv_hi)   into the z ghost planes of the padded phi array
+ * After lb_init (and after lb_set_populations) the last three calls must run once before the first
+ * lb_slab_begin or lb_get_macros (phi of the initial state is computed by lb_slab_pack_phi).
+ * All calls are asynchronous on the handle's stream at the time of the call (lb_set_stream may
+ * switch streams between phases; ordering across streams is the caller's, by events).  Errors:
+ * LB_ESTATE for a call out of order or on a handle that is not a slab, LB_EINVAL for NULL,
+ * misaligned or host message buffers.  One component: the phi calls do nothing. */
+int lb_set_slab(lb_handle h, int z0, int nz_global);
+int lb_slab_halo_bytes(lb_handle h, size_t* pop_bytes, size_t* phi_bytes);   /* per face and direction of travel; after lb_init */
+int lb_slab_begin(lb_handle h, void* send_lo, void* send_hi);
+int lb_slab_interior(lb_handle h);
+int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi);
+int lb_slab_pack_phi(lb_handle h, void* send_lo, void* send_hi);
+int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi);
+
 /* Tuning of lb_step.  key = "forward": 1 (default) = the fused kernel forwards the moments of the
  * next state and a light kernel turns them into phi; 0 = a full
  * phase-field sweep over the populations before every step (same phi to ~1e-8).  "zc": z planes

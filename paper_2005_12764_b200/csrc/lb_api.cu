@@ -81,8 +81,13 @@ EncodeTiledFn get_encode() {
 struct lb_handle_s {
   Allocator al;              // captured at lb_create
   int device = -1;           // CUDA device of this handle (the device current at lb_create; -1: none)
-  int nx = 0, ny = 0, nz = 0;
-  long long S = 0;
+  int nx = 0, ny = 0, nz = 0;   // the caller's box: nz planes (of a slab: its own planes)
+  int gz = 0;                // ghost planes below and above (1 for a z slab, lb_set_slab)
+  int slab_z0 = 0, slab_nzg = 0;   // slab: first global plane, global extent
+  int slab_phase = 0;        // slab: 0 = between steps, 1 = after lb_slab_begin, 2 = after lb_slab_interior
+  bool phi_ghost_ok = false; // slab: the z ghost planes of phi match the current state (lb_slab_unpack_phi)
+  long long S = 0;           // allocated sites nx * ny * (nz + 2 gz): what the kernels index
+  long long Sx = 0;          // sites of the caller's arrays nx * ny * nz
   lb_params par{};
   float g[3] = {0, 0, 0};
   float phi_c = 0.9f;
@@ -126,13 +131,17 @@ struct lb_handle_s {
   int ev_steps = 0;
   std::string err;
 
+  int nza() const { return nz + 2 * gz; }   // allocated planes
+  int zlo() const { return gz; }
+  int zhi() const { return gz + nz; }
   Box box() const {
     Box b;
-    b.nx = nx; b.ny = ny; b.nz = nz;
+    b.nx = nx; b.ny = ny; b.nz = nza();
+    b.zlo = zlo(); b.zhi = zhi(); b.zper = gz == 0;
     b.nxw = (nx + 31) / 32;
     b.S = S;
     b.mask = has_solid ? mask : nullptr;
-    b.gmask = (has_solid && has_moving) ? mask + (size_t)b.nxw * ny * nz : nullptr;
+    b.gmask = (has_solid && has_moving) ? mask + (size_t)b.nxw * ny * nza() : nullptr;
     return b;
   }
   int planes() const { return two ? 2 * Q : Q; }
@@ -202,8 +211,10 @@ int finish_out(lb_handle h, void* dst, size_t bytes, Staged& s) {
 // ------------------------------------------------------------------------------ launches
 namespace {
 
-StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
+StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc, int z0 = -1, int z1 = -1) {
   StepParams p;
+  p.z0 = z0 < 0 ? h->zlo() : z0;
+  p.z1 = z1 < 0 ? h->zhi() : z1;
   p.src = src; p.dst = dst; p.phi = h->phi;
   p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
   const size_t plane = (h->two ? 2 : 1) * (size_t)h->S;   // floats per direction plane ({T, R} pairs or T)
@@ -238,32 +249,37 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc) {
 // k_phase_fwd a gather, so: 10..20 planes, and among those the count whose number of CTAs fills
 // whole waves of (SMs x resident CTAs) best.
 int pick_zc(lb_handle h) {
-  if (h->tune_zc > 0) return h->tune_zc < h->nz ? h->tune_zc : h->nz;
-  if (h->nz <= 10) return h->nz;
-  if (!h->sm_count) {       // of the handle's own device
-    int sms = 148;
-    if (h->device >= 0) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
-    cudaGetLastError();
-    h->sm_count = sms;
+  int zc = 16;
+  if (h->tune_zc > 0) zc = h->tune_zc < h->nz ? h->tune_zc : h->nz;
+  else if (h->nz <= 10) zc = h->nz;
+  else {
+    if (!h->sm_count) {       // of the handle's own device
+      int sms = 148;
+      if (h->device >= 0) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
+      cudaGetLastError();
+      h->sm_count = sms;
+    }
+    // resident CTAs per SM: 3, but 2 for the instantiations with wall groups (WALLS = 2)
+    const int slots = ((h->has_solid && h->has_moving) ? 2 : 3) * h->sm_count;
+    const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
+    double best_eff = -1.0;
+    for (int c = 10; c <= 20 && c <= h->nz; ++c) {
+      const long long ctas = cols * ((h->nz + c - 1) / c);
+      const long long waves = (ctas + slots - 1) / slots;
+      // planes actually computed per slot-wave (the last chunk may be short)
+      const double eff = (double)cols * h->nz / ((double)waves * slots * c);
+      if (eff > best_eff + 1e-9) { best_eff = eff; zc = c; }
+    }
   }
-  const int sm_count = h->sm_count;
-  // resident CTAs per SM: 3, but 2 for the instantiations with wall groups (WALLS = 2)
-  const int slots = ((h->has_solid && h->has_moving) ? 2 : 3) * sm_count;
-  const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
-  int best = 16;
-  double best_eff = -1.0;
-  for (int zc = 10; zc <= 20 && zc <= h->nz; ++zc) {
-    const long long ctas = cols * ((h->nz + zc - 1) / zc);
-    const long long waves = (ctas + slots - 1) / slots;
-    // planes actually computed per slot-wave (the last chunk may be short)
-    const double eff = (double)cols * h->nz / ((double)waves * slots * zc);
-    if (eff > best_eff + 1e-9) { best_eff = eff; best = zc; }
-  }
-  return best;
+  // A slab's phi planes that wait for the halo, [zlo, zlo + H) and [zhi - H, zhi), must not touch an
+  // inner brick face (lb_slab_end): bricks deeper than the phi halo, or one brick for the whole slab.
+  if (h->gz && zc <= H_MAX_NC) zc = h->nz;
+  return zc;
 }
 
-dim3 tile_grid(lb_handle h, int zc) {
-  return dim3((h->nx + TX - 1) / TX, (h->ny + TY - 1) / TY, (h->nz + zc - 1) / zc);
+dim3 tile_grid(lb_handle h, int zc, int nplanes = -1) {
+  if (nplanes < 0) nplanes = h->nz;
+  return dim3((h->nx + TX - 1) / TX, (h->ny + TY - 1) / TY, (nplanes + zc - 1) / zc);
 }
 
 template <int MODE>
@@ -366,15 +382,19 @@ void run_phase(lb_handle h) {
   }
   h->launches++;
   h->phi_current = true;
+  h->phi_ghost_ok = false;
 }
 
-// K2 / K2s: advance one step and flip the buffer / parity
-void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
+float* next_buf(lb_handle h) { return h->storage == 0 ? h->buf[h->cur ^ 1] : h->buf[0]; }
+int next_mode(lb_handle h) { return h->storage == 0 ? MODE_AB : (h->aa_odd ? MODE_AA_EVEN : MODE_AA_ODD); }
+
+// K2 / K2s on the bricks that cover the planes [z0, z1) (whole bricks, counted from zlo): reads the
+// current buffer, writes the next one.  Does not flip.
+void launch_collide(lb_handle h, int z0, int z1) {
+  if (z1 <= z0) return;
   const int zc = pick_zc(h);
-  const dim3 grid = tile_grid(h, zc);
-  float* src = h->cur_buf();
-  float* dst = h->storage == 0 ? h->buf[h->cur ^ 1] : h->buf[0];
-  const StepParams p = make_step_params(h, src, dst, zc);
+  const dim3 grid = tile_grid(h, zc, z1 - z0);
+  const StepParams p = make_step_params(h, h->cur_buf(), next_buf(h), zc, z0, z1);
   const int mode = h->mode();
   if (h->two) {
     if (mode == MODE_AB) launch_fused<MODE_AB>(h, p, grid);
@@ -386,21 +406,41 @@ void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
     else launch_single<MODE_AA_ODD>(h, p, grid);
   }
   h->launches++;
+}
+
+// K1f on the planes [z0, z1): phi of the state that launch_collide has just written (buffer
+// next_buf, read rule next_mode) from the moments k_fused forwarded.  Call before flip().
+void launch_phase_forward(lb_handle h, int z0, int z1) {
+  if (z1 <= z0 || !h->two) return;
+  const int zc = pick_zc(h);      // the same z chunks as k_fused: the bricks must match
+  const StepParams q = make_step_params(h, next_buf(h), nullptr, zc, z0, z1);
+  const dim3 gridf((h->nx / 4 + TX - 1) / TX, (h->ny + TY - 1) / TY, z1 - z0);   // 4 sites per thread, one plane per CTA
+  switch (next_mode(h)) {
+    case MODE_AB: launch_phase_fwd<MODE_AB>(h, q, gridf); break;
+    case MODE_AA_EVEN: launch_phase_fwd<MODE_AA_EVEN>(h, q, gridf); break;
+    default: launch_phase_fwd<MODE_AA_ODD>(h, q, gridf); break;
+  }
+  h->launches++;
+}
+
+// the next buffer / parity becomes the current state
+void flip(lb_handle h) {
   if (h->storage == 0) h->cur ^= 1;
   else h->aa_odd ^= 1;
-  h->phi_current = false;
+  h->steps_done++;
+}
+
+// One whole step of a box that is periodic in z: K2 (+ K1f) or K2s
+void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
+  launch_collide(h, h->zlo(), h->zhi());
   if (after_k2) cudaEventRecord(after_k2, h->stream);
   if (h->two && h->forward) {
-    // K1f: phi of the new state from the moments k_fused forwarded (same z chunks: the bricks must match)
-    const StepParams q = make_step_params(h, h->cur_buf(), nullptr, zc);
-    const dim3 gridf((h->nx / 4 + TX - 1) / TX, grid.y, h->nz);   // 4 sites per thread, one plane per CTA
-    switch (h->mode()) {
-      case MODE_AB: launch_phase_fwd<MODE_AB>(h, q, gridf); break;
-      case MODE_AA_EVEN: launch_phase_fwd<MODE_AA_EVEN>(h, q, gridf); break;
-      default: launch_phase_fwd<MODE_AA_ODD>(h, q, gridf); break;
-    }
-    h->launches++;
+    launch_phase_forward(h, h->zlo(), h->zhi());
+    flip(h);
     h->phi_current = true;
+  } else {
+    flip(h);
+    h->phi_current = false;
   }
 }
 
@@ -408,8 +448,11 @@ IoParams make_io_params(lb_handle h) {
   IoParams p;
   memset(&p, 0, sizeof(p));
   p.buf = h->cur_buf();
+  const size_t plane = (h->two ? 2 : 1) * (size_t)h->S;   // floats per direction plane
+  for (int q = 0; q < Q; ++q) { p.ps[q] = p.buf + (size_t)q * plane; p.pd[q] = p.buf + (size_t)q * plane; }
   p.box = h->box();
-  p.two = h->two;
+  p.s0 = (long long)h->zlo() * h->nx * h->ny;      // the caller's arrays hold the handle's own planes
+  p.s1 = (long long)h->zhi() * h->nx * h->ny;
   p.phi = h->phi;
   p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
   p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
@@ -419,36 +462,34 @@ IoParams make_io_params(lb_handle h) {
   return p;
 }
 
-void launch_scatter(lb_handle h, const IoParams& p) {
-  const int tb = 256;
-  const unsigned nb = (unsigned)((h->S + tb - 1) / tb);
-  switch (h->mode()) {
-    case MODE_AB: k_scatter<MODE_AB><<<nb, tb, 0, h->stream>>>(p); break;
-    case MODE_AA_EVEN: k_scatter<MODE_AA_EVEN><<<nb, tb, 0, h->stream>>>(p); break;
-    default: k_scatter<MODE_AA_ODD><<<nb, tb, 0, h->stream>>>(p); break;
+// the cold kernels are instantiated for (storage mode) x (one / two components) x (walls)
+#define LB_IO_DISPATCH(KERNEL)                                                                       \
+  template <int MODE, bool TWO>                                                                      \
+  void launch_##KERNEL##_t(lb_handle h, const IoParams& p, unsigned nb) {                            \
+    if (h->has_solid) KERNEL<MODE, TWO, true><<<nb, 256, 0, h->stream>>>(p);                         \
+    else KERNEL<MODE, TWO, false><<<nb, 256, 0, h->stream>>>(p);                                     \
+  }                                                                                                  \
+  void launch_##KERNEL(lb_handle h, const IoParams& p) {                                             \
+    const unsigned nb = (unsigned)((p.s1 - p.s0 + 255) / 256);                                       \
+    const int mode = h->mode();                                                                      \
+    if (h->two) {                                                                                    \
+      if (mode == MODE_AB) launch_##KERNEL##_t<MODE_AB, true>(h, p, nb);                             \
+      else if (mode == MODE_AA_EVEN) launch_##KERNEL##_t<MODE_AA_EVEN, true>(h, p, nb);              \
+      else launch_##KERNEL##_t<MODE_AA_ODD, true>(h, p, nb);                                         \
+    } else {                                                                                         \
+      if (mode == MODE_AB) launch_##KERNEL##_t<MODE_AB, false>(h, p, nb);                            \
+      else if (mode == MODE_AA_EVEN) launch_##KERNEL##_t<MODE_AA_EVEN, false>(h, p, nb);             \
+      else launch_##KERNEL##_t<MODE_AA_ODD, false>(h, p, nb);                                        \
+    }                                                                                                \
+    h->launches++;                                                                                   \
   }
-  h->launches++;
-}
-void launch_gatherf(lb_handle h, const IoParams& p) {
-  const int tb = 256;
-  const unsigned nb = (unsigned)((h->S + tb - 1) / tb);
-  switch (h->mode()) {
-    case MODE_AB: k_gatherf<MODE_AB><<<nb, tb, 0, h->stream>>>(p); break;
-    case MODE_AA_EVEN: k_gatherf<MODE_AA_EVEN><<<nb, tb, 0, h->stream>>>(p); break;
-    default: k_gatherf<MODE_AA_ODD><<<nb, tb, 0, h->stream>>>(p); break;
-  }
-  h->launches++;
-}
-void launch_macros(lb_handle h, const IoParams& p) {
-  const int tb = 256;
-  const unsigned nb = (unsigned)((h->S + tb - 1) / tb);
-  switch (h->mode()) {
-    case MODE_AB: k_macros<MODE_AB><<<nb, tb, 0, h->stream>>>(p); break;
-    case MODE_AA_EVEN: k_macros<MODE_AA_EVEN><<<nb, tb, 0, h->stream>>>(p); break;
-    default: k_macros<MODE_AA_ODD><<<nb, tb, 0, h->stream>>>(p); break;
-  }
-  h->launches++;
-}
+LB_IO_DISPATCH(k_scatter)
+LB_IO_DISPATCH(k_gatherf)
+LB_IO_DISPATCH(k_macros)
+#undef LB_IO_DISPATCH
+void launch_scatter(lb_handle h, const IoParams& p) { launch_k_scatter(h, p); }
+void launch_gatherf(lb_handle h, const IoParams& p) { launch_k_gatherf(h, p); }
+void launch_macros(lb_handle h, const IoParams& p) { launch_k_macros(h, p); }
 
 // Component masses and finiteness of the stored state (k_check); synchronises the stream.
 int state_check(lb_handle h, double* mass_r, double* mass_b) {
@@ -459,9 +500,10 @@ int state_check(lb_handle h, double* mass_r, double* mass_b) {
   }
   cudaError_t e = cudaMemsetAsync(h->chk, 0, 3 * sizeof(double), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "state check memset");
-  const int nb = (int)std::min<long long>((h->S + 255) / 256, 148 * 16);
-  if (h->two) k_check<true><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), h->chk);
-  else k_check<false><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), h->chk);
+  const long long s0 = (long long)h->zlo() * h->nx * h->ny, s1 = (long long)h->zhi() * h->nx * h->ny;
+  const int nb = (int)std::min<long long>((s1 - s0 + 255) / 256, 148 * 16);
+  if (h->two) k_check<true><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), s0, s1, h->chk);
+  else k_check<false><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), s0, s1, h->chk);
   h->launches++;
   double out[3] = {0, 0, 0};
   e = cudaMemcpyAsync(out, h->chk, sizeof(out), cudaMemcpyDeviceToHost, h->stream);
@@ -506,7 +548,7 @@ int lb_create(int nx, int ny, int nz, const lb_params* p, lb_handle* out) {
   lb_handle h = new (std::nothrow) lb_handle_s();
   if (!h) return fail(nullptr, LB_ENOMEM, "host allocation failed");
   h->nx = nx; h->ny = ny; h->nz = nz;
-  h->S = (long long)nx * ny * nz;
+  h->S = h->Sx = (long long)nx * ny * nz;
   h->par = *p;
   h->al.alloc = g_alloc; h->al.free_fn = g_free; h->al.user = g_user;
   if (cudaGetDevice(&h->device) != cudaSuccess) { cudaGetLastError(); h->device = -1; }   // no device: later calls return LB_ECUDA
@@ -542,7 +584,7 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
     return fail(h, LB_ECUDA, "no CUDA device (there is no CPU fallback)");
   }
   Box b = h->box();
-  const size_t nwords = (size_t)b.nxw * h->ny * h->nz;
+  const size_t nwords = (size_t)b.nxw * h->ny * h->nza();   // a slab's mask covers its ghost planes too
   // three bit masks behind each other (solid, wall group 2, wall group 3) and one flag word
   if (!h->mask) {
     h->mask = static_cast<uint32_t*>(dev_alloc(h->al, (3 * nwords + 1) * 4));
@@ -632,6 +674,23 @@ int lb_set_storage(lb_handle h, int mode) {
   return LB_OK;
 }
 
+int lb_set_slab(lb_handle h, int z0, int nz_global) {
+  if (!h) return LB_EINVAL;
+  if (h->inited || h->mask) return fail(h, LB_ESTATE, "lb_set_slab must precede lb_set_geometry and lb_init");
+  if (nz_global <= 0) {      // back to a box that is periodic in z
+    h->gz = 0; h->slab_z0 = 0; h->slab_nzg = 0;
+    h->S = h->Sx;
+    return LB_OK;
+  }
+  if (z0 < 0 || z0 + h->nz > nz_global) return fail(h, LB_EINVAL, "slab [z0, z0 + nz) does not fit the global extent");
+  if (h->nz < 2 * H_MAX_NC) return fail(h, LB_EINVAL, "a slab needs at least 8 planes (twice the phi halo)");
+  const long long Sa = (long long)h->nx * h->ny * (h->nz + 2);
+  if (Sa >= (1LL << 29)) return fail(h, LB_EINVAL, "slab too large (>= 2^29 sites with its ghost planes)");
+  h->gz = 1; h->slab_z0 = z0; h->slab_nzg = nz_global;
+  h->S = Sa;
+  return LB_OK;
+}
+
 }  // extern "C"
 
 namespace {
@@ -653,7 +712,7 @@ int allocate_state(lb_handle h, bool two) {
     }
   }
   if (two && !h->mom) {
-    const size_t ex = (size_t)h->nz * h->ny * ((h->nx + TX - 1) / TX) * 4;   // x-face sums: 2 sides x {D, Tm}
+    const size_t ex = (size_t)h->nza() * h->ny * ((h->nx + TX - 1) / TX) * 4;   // x-face sums: 2 sides x {D, Tm}
     const size_t mb = (2 * (size_t)h->S + ex) * sizeof(float);
     h->mom = static_cast<float*>(dev_alloc(h->al, mb));
     if (!h->mom) return fail(h, LB_ENOMEM, "moment buffer allocation failed");
@@ -663,7 +722,7 @@ int allocate_state(lb_handle h, bool two) {
   for (int f = 0; f < (h->model == 1 ? 2 : 1); ++f) {
     float*& field = f == 0 ? h->phi : h->phi2;
     if (!two || field) continue;
-    const size_t px = h->nx + 2 * HALO, py = h->ny + 2 * HALO, pz = h->nz + 2 * HALO;
+    const size_t px = h->nx + 2 * HALO, py = h->ny + 2 * HALO, pz = h->nza() + 2 * HALO;
     const size_t phib = px * py * pz * sizeof(float);
     field = static_cast<float*>(dev_alloc(h->al, phib));
     if (!field) return fail(h, LB_ENOMEM, "phi allocation failed");
@@ -703,7 +762,7 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   }
   int rc = allocate_state(h, rho_b != nullptr);
   if (rc) return rc;
-  const size_t fb = (size_t)h->S * sizeof(float);
+  const size_t fb = (size_t)h->Sx * sizeof(float);
   Staged srr, srb, su;
   if ((rc = stage_in(h, rho_r, fb, srr))) return rc;
   if (rho_b && (rc = stage_in(h, rho_b, fb, srb))) return rc;
@@ -718,7 +777,7 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   p.rho_b = static_cast<const float*>(srb.dev);
   p.u = static_cast<const float*>(su.dev);
   // solid sites keep zeros so that stray reads are harmless
-  cudaError_t e = cudaMemsetAsync(h->cur_buf(), 0, (size_t)h->planes() * fb, h->stream);
+  cudaError_t e = cudaMemsetAsync(h->cur_buf(), 0, (size_t)h->planes() * h->S * sizeof(float), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "population memset");
   launch_scatter(h, p);
   if ((rc = check_launch(h, "k_scatter"))) return rc;
@@ -735,6 +794,7 @@ int lb_step(lb_handle h, int nsteps) {
   if (!h || nsteps < 0) return fail(h, LB_EINVAL, "nsteps must be >= 0");
   DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_step before lb_init");
+  if (h->gz) return fail(h, LB_ESTATE, "a slab is stepped by lb_slab_begin / _interior / _end and the phi exchange, not by lb_step");
   for (int i = 0; i < 2; ++i)
     if (!h->ev_step[i] && cudaEventCreate(&h->ev_step[i]) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "event create");
   // profiling = n > 0: every n-th step of this call is bracketed by events (kernel by kernel)
@@ -755,7 +815,6 @@ int lb_step(lb_handle h, int nsteps) {
     if (prof) cudaEventRecord(h->ev_k[k + 1], h->stream);
     run_collide(h, prof ? h->ev_k[k + 2] : nullptr);   // K2 (+ K1f) or K2s
     if (prof) cudaEventRecord(h->ev_k[k + 3], h->stream);
-    h->steps_done++;
     // G23: every CHECK_EVERY steps the component masses are summed on the device; a non-finite
     // state ends the call with LB_ESTATE (this is the one place where lb_step synchronises)
     if (h->steps_done - h->last_check >= CHECK_EVERY) {
@@ -779,7 +838,7 @@ int lb_get_macros(lb_handle h, float* rho_r, float* rho_b, float* u) {
   if (!h) return LB_EINVAL;
   DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_get_macros before lb_init");
-  const size_t fb = (size_t)h->S * sizeof(float);
+  const size_t fb = (size_t)h->Sx * sizeof(float);
   Staged o0, o1, o2;
   int rc;
   if ((rc = stage_out(h, rho_r, fb, o0))) return rc;
@@ -807,7 +866,7 @@ int lb_get_populations(lb_handle h, int comp, float* f) {
   DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_get_populations before lb_init");
   if (comp < 0 || comp > (h->two ? 1 : 0)) return fail(h, LB_EINVAL, "bad component");
-  const size_t fb = (size_t)Q * h->S * sizeof(float);
+  const size_t fb = (size_t)Q * h->Sx * sizeof(float);
   Staged o;
   int rc;
   if ((rc = stage_out(h, f, fb, o))) return rc;
@@ -829,7 +888,7 @@ int lb_set_populations(lb_handle h, int comp, const float* f) {
   DeviceGuard guard(h->device);
   if (!h->inited) return fail(h, LB_ESTATE, "lb_set_populations before lb_init");
   if (comp < 0 || comp > (h->two ? 1 : 0)) return fail(h, LB_EINVAL, "bad component");
-  const size_t fb = (size_t)Q * h->S * sizeof(float);
+  const size_t fb = (size_t)Q * h->Sx * sizeof(float);
   Staged in;
   int rc;
   if ((rc = stage_in(h, f, fb, in))) return rc;
@@ -851,13 +910,14 @@ int lb_get_phi(lb_handle h, float* phi) {
   if (!h || !phi) return fail(h, LB_EINVAL, "phi is NULL");
   DeviceGuard guard(h->device);
   if (!h->inited || !h->two) return fail(h, LB_ESTATE, "lb_get_phi needs an initialised two-component state");
-  const size_t fb = (size_t)h->S * sizeof(float);
+  const size_t fb = (size_t)h->Sx * sizeof(float);
   Staged o;
   int rc;
   if ((rc = stage_out(h, phi, fb, o))) return rc;
   run_phase(h);
   const int tb = 256;
-  k_unpad_phi<<<(unsigned)((h->S + tb - 1) / tb), tb, 0, h->stream>>>(h->phi, h->model == 1 ? h->phi2 : nullptr, static_cast<float*>(o.dev), h->box());
+  const long long s0 = (long long)h->zlo() * h->nx * h->ny, s1 = (long long)h->zhi() * h->nx * h->ny;
+  k_unpad_phi<<<(unsigned)((h->Sx + tb - 1) / tb), tb, 0, h->stream>>>(h->phi, h->model == 1 ? h->phi2 : nullptr, static_cast<float*>(o.dev), h->box(), s0, s1);
   h->launches++;
   if ((rc = check_launch(h, "k_unpad_phi"))) return rc;
   if ((rc = finish_out(h, phi, fb, o))) return rc;
@@ -865,6 +925,180 @@ int lb_get_phi(lb_handle h, float* phi) {
     cudaError_t e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "lb_get_phi");
   }
+  return LB_OK;
+}
+
+// ------------------------------------------------------------------------------ z slabs
+}  // extern "C"
+
+namespace {
+
+const int DIRS_UP[5] = {5, 11, 14, 15, 18};   // c_z = +1 (velocity order: include/lb.h)
+const int DIRS_DN[5] = {6, 12, 13, 16, 17};   // c_z = -1
+
+// The five (direction, plane) blocks of a face's message.  [0]: the message that travels to / came
+// from the rank BELOW, [1]: ABOVE.  Which blocks depends on the storage mode of the step that has
+// just collided:
+//   A/B       pull: the neighbour reads F_q(x - c_q) out of its ghost plane        real plane -> ghost
+//   AA even   the odd step reads slot (opp q, x - c_q) out of the ghost plane     real plane -> ghost
+//   AA odd    the step pushed f*_q into slot (q, x + c_q) of the ghost plane      ghost -> real plane
+struct SlabBlocks { const int* dirs[2]; int plane[2]; };
+
+SlabBlocks slab_send_blocks(lb_handle h, int mode) {
+  SlabBlocks b;
+  if (mode == MODE_AB) { b.dirs[0] = DIRS_DN; b.plane[0] = h->zlo(); b.dirs[1] = DIRS_UP; b.plane[1] = h->zhi() - 1; }
+  else if (mode == MODE_AA_EVEN) { b.dirs[0] = DIRS_UP; b.plane[0] = h->zlo(); b.dirs[1] = DIRS_DN; b.plane[1] = h->zhi() - 1; }
+  else { b.dirs[0] = DIRS_DN; b.plane[0] = h->zlo() - 1; b.dirs[1] = DIRS_UP; b.plane[1] = h->zhi(); }
+  return b;
+}
+SlabBlocks slab_recv_blocks(lb_handle h, int mode) {
+  SlabBlocks b;
+  if (mode == MODE_AB) { b.dirs[0] = DIRS_UP; b.plane[0] = h->zlo() - 1; b.dirs[1] = DIRS_DN; b.plane[1] = h->zhi(); }
+  else if (mode == MODE_AA_EVEN) { b.dirs[0] = DIRS_DN; b.plane[0] = h->zlo() - 1; b.dirs[1] = DIRS_UP; b.plane[1] = h->zhi(); }
+  else { b.dirs[0] = DIRS_UP; b.plane[0] = h->zlo(); b.dirs[1] = DIRS_DN; b.plane[1] = h->zhi() - 1; }
+  return b;
+}
+
+int slab_msg_check(lb_handle h, const void* lo, const void* hi) {
+  if (!lo || !hi) return fail(h, LB_EINVAL, "halo message buffers must not be NULL");
+  if (((uintptr_t)lo | (uintptr_t)hi) & 15u) return fail(h, LB_EINVAL, "halo message buffers must be 16-byte aligned");
+  if (!is_device_ptr(lo) || !is_device_ptr(hi)) return fail(h, LB_EINVAL, "halo message buffers must be device memory");
+  return LB_OK;
+}
+
+// pack (blocks of `buf` -> messages) or unpack (messages -> blocks of `buf`)
+void slab_copy_populations(lb_handle h, float* buf, const SlabBlocks& b, void* msg_lo, void* msg_hi, bool pack) {
+  const size_t esz = h->two ? 2 : 1;                       // floats per site in a plane
+  const size_t blockf = (size_t)h->nx * h->ny * esz;       // floats per (direction, plane) block
+  HaloCopy c;
+  c.n4 = (long long)(blockf / 4);
+  void* msg[2] = {msg_lo, msg_hi};
+  for (int f = 0; f < 2; ++f)
+    for (int k = 0; k < 5; ++k) {
+      float* blk = buf + (size_t)b.dirs[f][k] * h->S * esz + (size_t)b.plane[f] * blockf;
+      float* m = static_cast<float*>(msg[f]) + (size_t)k * blockf;
+      c.src[f][k] = reinterpret_cast<const float4*>(pack ? blk : m);
+      c.dst[f][k] = reinterpret_cast<float4*>(pack ? m : blk);
+    }
+  k_halo_copy<<<dim3((unsigned)((c.n4 + 255) / 256), 5, 2), 256, 0, h->stream>>>(c);
+  h->launches++;
+}
+
+int slab_phi_halo(lb_handle h) { return (h->model == 0 && h->par.A_nc != 0.f) ? H_MAX_NC : 1; }
+size_t slab_phi_plane_floats(lb_handle h) { return (size_t)(h->nx + 2 * HALO) * (h->ny + 2 * HALO); }
+
+int slab_ready(lb_handle h, int phase, const char* what) {
+  if (!h) return LB_EINVAL;
+  if (!h->gz) return fail(h, LB_ESTATE, std::string(what) + ": not a slab (lb_set_slab)");
+  if (!h->inited) return fail(h, LB_ESTATE, std::string(what) + " before lb_init");
+  if (h->slab_phase != phase) return fail(h, LB_ESTATE, std::string(what) + " out of order (lb_slab_begin, lb_slab_interior, lb_slab_end, then the phi exchange)");
+  return LB_OK;
+}
+
+// first and last brick of the slab, and what lies between
+struct SlabBricks { int first0, first1, last0, last1, mid0, mid1; };
+SlabBricks slab_bricks(lb_handle h) {
+  const int zc = pick_zc(h), zlo = h->zlo(), zhi = h->zhi();
+  const int nb = (h->nz + zc - 1) / zc;
+  SlabBricks b;
+  b.first0 = zlo; b.first1 = std::min(zhi, zlo + zc);
+  b.last0 = nb > 1 ? zlo + (nb - 1) * zc : zhi; b.last1 = zhi;
+  b.mid0 = b.first1; b.mid1 = nb > 2 ? b.last0 : b.first1;
+  return b;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lb_slab_halo_bytes(lb_handle h, size_t* pop_bytes, size_t* phi_bytes) {
+  if (!h) return LB_EINVAL;
+  if (!h->gz || !h->inited) return fail(h, LB_ESTATE, "lb_slab_halo_bytes needs an initialised slab");
+  if (pop_bytes) *pop_bytes = (size_t)5 * h->nx * h->ny * (h->two ? 2 : 1) * sizeof(float);
+  if (phi_bytes) *phi_bytes = h->two ? (size_t)(h->model == 1 ? 2 : 1) * slab_phi_halo(h) * slab_phi_plane_floats(h) * sizeof(float) : 0;
+  return LB_OK;
+}
+
+int lb_slab_begin(lb_handle h, void* send_lo, void* send_hi) {
+  int rc = slab_ready(h, 0, "lb_slab_begin");
+  if (rc) return rc;
+  if ((rc = slab_msg_check(h, send_lo, send_hi))) return rc;
+  if (h->two && !(h->phi_current && h->phi_ghost_ok))
+    return fail(h, LB_ESTATE, "lb_slab_begin: the phi ghost planes are stale (lb_slab_pack_phi, exchange, lb_slab_unpack_phi first)");
+  if (h->two && !h->forward) return fail(h, LB_ESTATE, "slabs need moment forwarding (lb_set_tuning forward = 1)");
+  DeviceGuard guard(h->device);
+  const SlabBricks b = slab_bricks(h);
+  launch_collide(h, b.first0, b.first1);
+  launch_collide(h, b.last0, b.last1);
+  slab_copy_populations(h, next_buf(h), slab_send_blocks(h, h->mode()), send_lo, send_hi, true);
+  h->slab_phase = 1;
+  return check_launch(h, "lb_slab_begin");
+}
+
+int lb_slab_interior(lb_handle h) {
+  int rc = slab_ready(h, 1, "lb_slab_interior");
+  if (rc) return rc;
+  DeviceGuard guard(h->device);
+  const SlabBricks b = slab_bricks(h);
+  launch_collide(h, b.mid0, b.mid1);
+  const int H = slab_phi_halo(h);
+  launch_phase_forward(h, h->zlo() + H, h->zhi() - H);     // the planes whose phi does not wait for the halo
+  h->slab_phase = 2;
+  return check_launch(h, "lb_slab_interior");
+}
+
+int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi) {
+  int rc = slab_ready(h, 2, "lb_slab_end");
+  if (rc) return rc;
+  if ((rc = slab_msg_check(h, recv_lo, recv_hi))) return rc;
+  DeviceGuard guard(h->device);
+  slab_copy_populations(h, next_buf(h), slab_recv_blocks(h, h->mode()), const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false);
+  const int H = slab_phi_halo(h);
+  launch_phase_forward(h, h->zlo(), std::min(h->zlo() + H, h->zhi()));
+  launch_phase_forward(h, std::max(h->zhi() - H, h->zlo() + H), h->zhi());
+  flip(h);
+  h->phi_current = h->two;
+  h->phi_ghost_ok = false;
+  h->slab_phase = 0;
+  if ((rc = check_launch(h, "lb_slab_end"))) return rc;
+  if (h->steps_done - h->last_check >= CHECK_EVERY) return state_check(h, nullptr, nullptr);   // G23, as in lb_step
+  return LB_OK;
+}
+
+int lb_slab_pack_phi(lb_handle h, void* send_lo, void* send_hi) {
+  int rc = slab_ready(h, 0, "lb_slab_pack_phi");
+  if (rc) return rc;
+  if (!h->two) return LB_OK;                       // one component: no phase field
+  if ((rc = slab_msg_check(h, send_lo, send_hi))) return rc;
+  DeviceGuard guard(h->device);
+  run_phase(h);                                    // after lb_init / lb_set_populations: the full sweep
+  const int H = slab_phi_halo(h);
+  const size_t pf = slab_phi_plane_floats(h), nb = (size_t)H * pf * sizeof(float);
+  const float* fields[2] = {h->phi, h->phi2};
+  for (int f = 0; f < (h->model == 1 ? 2 : 1); ++f) {
+    cudaError_t e = cudaMemcpyAsync(static_cast<char*>(send_lo) + f * nb, fields[f] + (size_t)(h->zlo() + HALO) * pf, nb, cudaMemcpyDeviceToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(static_cast<char*>(send_hi) + f * nb, fields[f] + (size_t)(h->zhi() - H + HALO) * pf, nb, cudaMemcpyDeviceToDevice, h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_slab_pack_phi");
+  }
+  return check_launch(h, "lb_slab_pack_phi");
+}
+
+int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi) {
+  int rc = slab_ready(h, 0, "lb_slab_unpack_phi");
+  if (rc) return rc;
+  if (!h->two) return LB_OK;
+  if ((rc = slab_msg_check(h, recv_lo, recv_hi))) return rc;
+  if (!h->phi_current) return fail(h, LB_ESTATE, "lb_slab_unpack_phi before lb_slab_pack_phi");
+  DeviceGuard guard(h->device);
+  const int H = slab_phi_halo(h);
+  const size_t pf = slab_phi_plane_floats(h), nb = (size_t)H * pf * sizeof(float);
+  float* fields[2] = {h->phi, h->phi2};
+  for (int f = 0; f < (h->model == 1 ? 2 : 1); ++f) {
+    cudaError_t e = cudaMemcpyAsync(fields[f] + (size_t)(h->zlo() - H + HALO) * pf, static_cast<const char*>(recv_lo) + f * nb, nb, cudaMemcpyDeviceToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(fields[f] + (size_t)(h->zhi() + HALO) * pf, static_cast<const char*>(recv_hi) + f * nb, nb, cudaMemcpyDeviceToDevice, h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_slab_unpack_phi");
+  }
+  h->phi_ghost_ok = true;
   return LB_OK;
 }
 

@@ -38,6 +38,7 @@ struct StepParams {
   float* Mt;          //   Md = sum (f^r - f^b), Mt = sum (f - w) over what arrives from inside the brick
   float* EX;          // the same sums for what crosses the x faces of the bricks: [z][y][tile][side]{D, Tm}
   Box box;
+  int z0, z1;         // planes this launch covers: whole bricks, counted from box.zlo
   int zc;             // z planes per CTA
   int halo;           // ghost depth K1 must fill (1 without near contact, 4 with)
   float tau_r, tau_b, A, beta, A_nc, phi_c, gx, gy, gz;
@@ -235,13 +236,14 @@ __device__ __forceinline__ void two_sum_acc(float& s, float& e, float x) {
 // into the ghost layers (depth H).
 __device__ __forceinline__ void store_field_with_images(float* field, const Box& b, int x, int y, int z, int H, float phi) {
   const int px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
-  if (x >= H && x < b.nx - H && y >= H && y < b.ny - H && z >= H && z < b.nz - H) {   // no image
+  const bool zin = !b.zper || (z >= H && z < b.nz - H);      // a slab's z ghost planes come from its neighbours
+  if (x >= H && x < b.nx - H && y >= H && y < b.ny - H && zin) {   // no image
     field[(size_t)(x + HALO) + (size_t)px * ((size_t)(y + HALO) + (size_t)py * (size_t)(z + HALO))] = phi;
     return;
   }
   const int sx[3] = {0, x < H ? b.nx : 0, x >= b.nx - H ? -b.nx : 0};
   const int sy[3] = {0, y < H ? b.ny : 0, y >= b.ny - H ? -b.ny : 0};
-  const int sz[3] = {0, z < H ? b.nz : 0, z >= b.nz - H ? -b.nz : 0};
+  const int sz[3] = {0, (b.zper && z < H) ? b.nz : 0, (b.zper && z >= b.nz - H) ? -b.nz : 0};
 #pragma unroll
   for (int iz = 0; iz < 3; ++iz) {
     if (iz && !sz[iz]) continue;
@@ -319,8 +321,8 @@ __global__ void __launch_bounds__(TX* TY) k_phase(const StepParams p) {
   const int x = blockIdx.x * TX + threadIdx.x;
   const int y = blockIdx.y * TY + threadIdx.y;
   if (x >= p.box.nx || y >= p.box.ny) return;
-  const int zb = blockIdx.z * p.zc;
-  phase_column<MODE, HAS_SOLID, SC>(p, x, y, zb, min(p.box.nz, zb + p.zc));
+  const int zb = p.z0 + blockIdx.z * p.zc;
+  phase_column<MODE, HAS_SOLID, SC>(p, x, y, zb, min(p.z1, zb + p.zc));
 }
 
 // ----------------------------------------------------------------------------- TMA / mbarrier
@@ -421,8 +423,8 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
   const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
   const int x = x0 + threadIdx.x, y = y0 + threadIdx.y;
   const bool active = x < b.nx && y < b.ny;
-  const int zb = blockIdx.z * p.zc;
-  const int ze = min(b.nz, zb + p.zc);
+  const int zb = p.z0 + blockIdx.z * p.zc;
+  const int ze = min(p.z1, zb + p.zc);
   const int npl = (ze - zb) + 2 * H;
 
   if (tid == 0) {
@@ -921,13 +923,13 @@ __global__ void __launch_bounds__(TX* TY, 8) k_phase_fwd(const StepParams p) {
   const Box& b = p.box;
   const int x = (blockIdx.x * TX + threadIdx.x) * 4;
   const int y = blockIdx.y * TY + threadIdx.y;
-  const int z = blockIdx.z;
+  const int z = p.z0 + blockIdx.z;
   if (x >= b.nx || y >= b.ny) return;
   const int tile = x / TX;                            // k_fused tile (brick column) of this quad
   const int qx = threadIdx.x & (TX / 4 - 1);          // quad inside the tile row
-  // z range of the k_fused brick this plane belongs to
-  const int zb = (z / p.zc) * p.zc;
-  const int ze = min(b.nz, zb + p.zc);
+  // z range of the k_fused brick this plane belongs to (bricks are counted from the first plane the handle updates)
+  const int zb = b.zlo + ((z - b.zlo) / p.zc) * p.zc;
+  const int ze = min(b.zhi, zb + p.zc);
   const int H = p.halo;
   const bool xm = qx == 0;                            // element 0 is the first column of its brick
   const bool xp = qx == TX / 4 - 1 || x + 4 == b.nx;  // element 3 is the last column of its brick
@@ -1011,7 +1013,7 @@ __global__ void __launch_bounds__(TX* TY, 8) k_phase_fwd(const StepParams p) {
       }
     });
   }
-  if (x >= H && x + 4 <= b.nx - H && y >= H && y < b.ny - H && z >= H && z < b.nz - H) {   // no ghost image
+  if (x >= H && x + 4 <= b.nx - H && y >= H && y < b.ny - H && (!b.zper || (z >= H && z < b.nz - H))) {   // no ghost image
     float f0[4], f1[4];
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
@@ -1040,8 +1042,8 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
   const int x = blockIdx.x * TX + threadIdx.x;
   const int y = blockIdx.y * TY + threadIdx.y;
   if (x >= b.nx || y >= b.ny) return;
-  const int zb = blockIdx.z * p.zc;
-  const int ze = min(b.nz, zb + p.zc);
+  const int zb = p.z0 + blockIdx.z * p.zc;
+  const int ze = min(p.z1, zb + p.zc);
   const float omega = 1.0f / p.tau_r;
   const float om1 = 1.0f - omega, g0 = 1.0f - 0.5f * omega;
   for (int z = zb; z < ze; ++z) {
@@ -1105,12 +1107,18 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
 }
 
 // ----------------------------------------------------------------------------- cold kernels
+// One thread per site of the planes [box.zlo, box.zhi) the handle owns.  The caller's arrays hold
+// those planes only (a slab's ghost planes are internal): element e = s - s0 of a field, plane
+// stride Sx = s1 - s0 between the 19 directions of a population array.  Addressing is that of the
+// hot kernels (compile-time direction, Ctx byte deltas, one 64-bit access per {T, R} pair).
 struct IoParams {
   float* buf;            // population buffer
+  const float* ps[Q];    // its direction planes, as in StepParams
+  float* pd[Q];
   Box box;
-  int two;               // two components?
+  long long s0, s1;      // allocated site indices this launch covers: [zlo, zhi) x ny x nx
   int comp;              // component of k_scatter / k_gatherf
-  const float* in0;      // k_scatter: f[19][S] full populations (or nullptr: from rho,u)
+  const float* in0;      // k_scatter: f[19][Sx] full populations (or nullptr: from rho,u)
   const float* rho_r;    // init fields
   const float* rho_b;
   const float* u;
@@ -1126,107 +1134,128 @@ struct IoParams {
   float phi_wall;
 };
 
-template <int MODE>
-__device__ __forceinline__ size_t read_slot_rt(const Box& b, int q, int x, int y, int z) {
-  // run-time-q version of read_slot for the cold kernels
-  const size_t own = (size_t)x + (size_t)b.nx * ((size_t)y + (size_t)b.ny * z);
-  if (MODE == MODE_AA_EVEN || q == 0) return (size_t)q * b.S + own;
-  int xs = x - c_cx[q], ys = y - c_cy[q], zs = z - c_cz[q];
-  xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
-  ys = ys < 0 ? b.ny - 1 : (ys >= b.ny ? 0 : ys);
-  zs = zs < 0 ? b.nz - 1 : (zs >= b.nz ? 0 : zs);
-  const bool bounce = b.mask && solid_at(b, xs, ys, zs);
-  const size_t nb = (size_t)xs + (size_t)b.nx * ((size_t)ys + (size_t)b.ny * zs);
-  const int o = opp(q);
-  if (MODE == MODE_AB) return bounce ? (size_t)o * b.S + own : (size_t)q * b.S + nb;
-  return bounce ? (size_t)q * b.S + own : (size_t)o * b.S + nb;
+struct IoSite {
+  long long s, e, Sx;
+  int x, y, z;
+  bool inside, solid;
+  uint32_t smask;
+  Ctx c;
+};
+
+template <int ESZ, bool HAS_SOLID>
+__device__ __forceinline__ IoSite io_site(const IoParams& p) {
+  IoSite t;
+  const Box& b = p.box;
+  t.e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  t.s = p.s0 + t.e;
+  t.Sx = p.s1 - p.s0;
+  t.inside = t.s < p.s1;
+  t.solid = false;
+  t.smask = 0;
+  t.x = t.y = t.z = 0;
+  if (t.inside) {
+    t.x = (int)(t.s % b.nx); t.y = (int)((t.s / b.nx) % b.ny); t.z = (int)(t.s / ((long long)b.nx * b.ny));
+    if constexpr (HAS_SOLID) {
+      t.solid = solid_at(b, t.x, t.y, t.z);
+      if (!t.solid) t.smask = neighbour_mask(b, t.x, t.y, t.z);
+    }
+    make_ctx<ESZ>(t.c, b, t.x, t.y, t.z);
+  }
+  return t;
 }
 
 // K0: write the pre-collision state where the next gather will look for it.
 //   comp < 0 : equilibrium init from rho_r, rho_b, u (Eq. 2), both components
 //   comp = 0 : red populations from in0; the T planes receive f^r - w (blue must follow)
 //   comp = 1 : blue populations from in0 are ADDED to the T planes
-template <int MODE>
-__global__ void k_scatter(const IoParams p) {
-  const Box& b = p.box;
-  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= b.S) return;
-  const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
-  if (b.mask && solid_at(b, x, y, z)) return;
+template <int MODE, bool TWO, bool HAS_SOLID>
+__global__ void __launch_bounds__(256) k_scatter(const IoParams p) {
+  const IoSite t = io_site<TWO ? 8 : 4, HAS_SOLID>(p);
+  if (!t.inside || t.solid) return;
   float rr = 0.f, rb = 0.f, ux = 0.f, uy = 0.f, uz = 0.f;
   if (p.comp < 0) {
-    rr = p.rho_r[s];
-    rb = p.two ? p.rho_b[s] : 0.f;
-    ux = p.u[s]; uy = p.u[b.S + s]; uz = p.u[2 * b.S + s];
+    rr = __ldg(p.rho_r + t.e);
+    rb = TWO ? __ldg(p.rho_b + t.e) : 0.f;
+    ux = __ldg(p.u + t.e); uy = __ldg(p.u + t.Sx + t.e); uz = __ldg(p.u + 2 * t.Sx + t.e);
   }
   const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
-  for (int q = 0; q < Q; ++q) {
-    const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
-    const float w = wq(q);
+  const float drho = (rr + rb) - 1.0f;
+  static_for<0, Q>([&](auto qc) {
+    constexpr int q = decltype(qc)::value;
+    constexpr float w = wq(q);
+    float* dst = const_cast<float*>(src_ptr(p, read_slot<MODE, HAS_SOLID, q>(t.c, t.smask)));
     if (p.comp < 0) {
-      const float cu = c_cx[q] * ux + c_cy[q] * uy + c_cz[q] * uz;
+      const float cu = cdot<q>(ux, uy, uz);
       const float e = 3.0f * cu + 4.5f * cu * cu - uu15;       // feq/(w rho) - 1
-      const float drho = (rr + rb) - 1.0f;
-      const float tv = w * (drho + (rr + rb) * e);                 // total as deviation
-      if (p.two) { p.buf[2 * slot] = tv; p.buf[2 * slot + 1] = w * rr * (1.0f + e); }
-      else p.buf[slot] = tv;
-    } else if (p.comp == 0) {
-      const float f = p.in0[(size_t)q * b.S + s];
-      if (p.two) { p.buf[2 * slot] = f - w; p.buf[2 * slot + 1] = f; }
-      else p.buf[slot] = f - w;
+      const float tv = w * (drho + (rr + rb) * e);             // total as deviation
+      if constexpr (TWO) *reinterpret_cast<float2*>(dst) = make_float2(tv, w * rr * (1.0f + e));
+      else *dst = tv;
     } else {
-      p.buf[2 * slot] += p.in0[(size_t)q * b.S + s];
-    }
-  }
-}
-
-// Debug accessor: full pre-collision populations of one component, [19][S].
-template <int MODE>
-__global__ void k_gatherf(const IoParams p) {
-  const Box& b = p.box;
-  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= b.S) return;
-  const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
-  const bool sol = b.mask && solid_at(b, x, y, z);
-  for (int q = 0; q < Q; ++q) {
-    float v = 0.f;
-    if (!sol) {
-      const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
-      const float t = p.buf[p.two ? 2 * slot : slot] + wq(q);
-      if (!p.two) v = t;
-      else {
-        const float r = p.buf[2 * slot + 1];
-        v = p.comp == 0 ? r : t - r;
+      const float f = __ldg(p.in0 + (size_t)q * t.Sx + t.e);
+      if (p.comp == 0) {
+        if constexpr (TWO) *reinterpret_cast<float2*>(dst) = make_float2(f - w, f);
+        else *dst = f - w;
+      } else {
+        *dst += f;
       }
     }
-    p.out0[(size_t)q * b.S + s] = v;
-  }
+  });
+}
+
+// Debug accessor: full pre-collision populations of one component, [19][Sx].
+template <int MODE, bool TWO, bool HAS_SOLID>
+__global__ void __launch_bounds__(256) k_gatherf(const IoParams p) {
+  const IoSite t = io_site<TWO ? 8 : 4, HAS_SOLID>(p);
+  if (!t.inside) return;
+  static_for<0, Q>([&](auto qc) {
+    constexpr int q = decltype(qc)::value;
+    float v = 0.f;
+    if (!t.solid) {
+      const float* src = src_ptr(p, read_slot<MODE, HAS_SOLID, q>(t.c, t.smask));
+      if constexpr (TWO) {
+        const float2 tr = __ldcg(reinterpret_cast<const float2*>(src));
+        v = p.comp == 0 ? tr.y : (tr.x + wq(q)) - tr.y;
+      } else {
+        v = __ldcg(src) + wq(q);
+      }
+    }
+    p.out0[(size_t)q * t.Sx + t.e] = v;
+  });
 }
 
 // K3: rho_r, rho_b and u = (m + F/2)/rho (Eq. 3; half-force shift of Guo forcing).
 // Needs the phi array of the current state (K1 must have run).  out0 = rho_r, out1 = rho_b,
-// out2 = u[3][S]; any may be null.
-template <int MODE>
-__global__ void k_macros(const IoParams p) {
+// out2 = u[3][Sx]; any may be null.
+template <int MODE, bool TWO, bool HAS_SOLID>
+__global__ void __launch_bounds__(256) k_macros(const IoParams p) {
+  const IoSite t = io_site<TWO ? 8 : 4, HAS_SOLID>(p);
+  if (!t.inside) return;
   const Box& b = p.box;
-  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= b.S) return;
-  const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
+  const int x = t.x, y = t.y, z = t.z;
   float rr = 0.f, rb = 0.f, ux = 0.f, uy = 0.f, uz = 0.f;
-  if (!(b.mask && solid_at(b, x, y, z))) {
+  if (!t.solid) {
     float dr = 0.f, mx = 0.f, my = 0.f, mz = 0.f;
-    for (int q = 0; q < Q; ++q) {
-      const size_t slot = read_slot_rt<MODE>(b, q, x, y, z);
-      const float t = p.buf[p.two ? 2 * slot : slot];
-      dr += t;
-      mx += c_cx[q] * t; my += c_cy[q] * t; mz += c_cz[q] * t;
-      if (p.two) rr += p.buf[2 * slot + 1];
-    }
+    static_for<0, Q>([&](auto qc) {
+      constexpr int q = decltype(qc)::value;
+      const float* src = src_ptr(p, read_slot<MODE, HAS_SOLID, q>(t.c, t.smask));
+      float tv;
+      if constexpr (TWO) {
+        const float2 tr = __ldcg(reinterpret_cast<const float2*>(src));
+        tv = tr.x;
+        rr += tr.y;
+      } else {
+        tv = __ldcg(src);
+      }
+      dr += tv;
+      if constexpr (cx(q) != 0) mx += cx(q) * tv;
+      if constexpr (cy(q) != 0) my += cy(q) * tv;
+      if constexpr (cz(q) != 0) mz += cz(q) * tv;
+    });
     const float rho = 1.0f + dr;
-    if (!p.two) rr = rho;
-    rb = p.two ? rho - rr : 0.f;
+    if (!TWO) rr = rho;
+    rb = TWO ? rho - rr : 0.f;
     float Fx = rho * p.gx, Fy = rho * p.gy, Fz = rho * p.gz;
-    if (p.sc) {
+    if (TWO && p.sc) {
       // Shan-Chen (Eq. 10; G27): F = rho_r a^r + rho_b a^b, g included
       const size_t o0 = phi_index(b, x, y, z);
       const long long px = b.nx + 2 * HALO, pxy = px * (b.ny + 2 * HALO);
@@ -1241,7 +1270,7 @@ __global__ void k_macros(const IoParams p) {
         Srx += k * c_cx[q] * vr; Sry += k * c_cy[q] * vr; Srz += k * c_cz[q] * vr;
       }
       Fx += -p.G_C * (rr * Sbx + rb * Srx); Fy += -p.G_C * (rr * Sby + rb * Sry); Fz += -p.G_C * (rr * Sbz + rb * Srz);
-    } else if (p.two && p.A_nc != 0.f) {
+    } else if (TWO && p.A_nc != 0.f) {
       const float* ph = p.phi + phi_index(b, x, y, z);
       const long long px = b.nx + 2 * HALO, pxy = px * (b.ny + 2 * HALO);
       const float phi0 = ph[0];
@@ -1273,24 +1302,45 @@ __global__ void k_macros(const IoParams p) {
     const float inv_rho = 1.0f / rho;
     ux = (mx + 0.5f * Fx) * inv_rho; uy = (my + 0.5f * Fy) * inv_rho; uz = (mz + 0.5f * Fz) * inv_rho;
   }
-  if (p.out0) p.out0[s] = rr;
-  if (p.out1 && p.two) p.out1[s] = rb;
-  if (p.out2) { p.out2[s] = ux; p.out2[b.S + s] = uy; p.out2[2 * b.S + s] = uz; }
+  if (p.out0) p.out0[t.e] = rr;
+  if (p.out1 && TWO) p.out1[t.e] = rb;
+  if (p.out2) { p.out2[t.e] = ux; p.out2[t.Sx + t.e] = uy; p.out2[2 * t.Sx + t.e] = uz; }
 }
 
 // phi without ghost layers or sentinels, for lb_get_phi (Shan-Chen: from the rho_r, rho_b arrays)
-__global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box b) {
-  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= b.S) return;
+__global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box b, long long s0, long long s1) {
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long s = s0 + e;
+  if (s >= s1) return;
   const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
   const float v = phi[phi_index(b, x, y, z)];
-  if (v > PHI_SOLID_TEST) { out[s] = 0.f; return; }
+  if (v > PHI_SOLID_TEST) { out[e] = 0.f; return; }
   if (phi2) {
     const float w = phi2[phi_index(b, x, y, z)];
-    out[s] = (v - w) / (v + w);
+    out[e] = (v - w) / (v + w);
   } else {
-    out[s] = v;
+    out[e] = v;
   }
+}
+
+// ----------------------------------------------------------------------------- slab halo
+// z-slab decomposition ("the domain is equally distributed (according to a either 1D, or 2D or 3D
+// domain decomposition)"; streaming reaches first neighbours only): what
+// crosses a z face per step is the 5 populations per component with c_z = +1 (upwards) or -1
+// (downwards).  One (direction, plane) block is contiguous in the SoA layout; the message of a face
+// is the 5 blocks behind each other.  The same kernel packs (blocks -> message) and unpacks (message
+// -> blocks of the ghost plane, or of the own boundary plane after an in-place odd step); which
+// blocks is the host's choice (lb_api.cu, slab_blocks).  grid = (ceil(n4 / 256), 5, 2 faces).
+struct HaloCopy {
+  const float4* src[2][5];
+  float4* dst[2][5];
+  long long n4;          // float4 elements per block
+};
+__global__ void __launch_bounds__(256) k_halo_copy(const HaloCopy p) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= p.n4) return;
+  const int k = blockIdx.y, f = blockIdx.z;
+  p.dst[f][k][i] = __ldcg(p.src[f][k] + i);
 }
 
 // bytes [S] (0 fluid, 1 wall at rest, 2 / 3 / 4 wall groups) -> bit-packed words: solid, and
@@ -1321,9 +1371,9 @@ __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* gro
 // slots of the fluid sites are the component masses (Eq. 3, summed over the box).
 // out[0] += sum rho_r, out[1] += sum rho_b, out[2] += number of sites holding a non-finite value.
 template <bool TWO>
-__global__ void __launch_bounds__(256) k_check(const float* __restrict__ buf, const Box b, double* out) {
+__global__ void __launch_bounds__(256) k_check(const float* __restrict__ buf, const Box b, long long s0, long long s1, double* out) {
   double sr = 0.0, sb = 0.0, bad = 0.0;
-  for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < b.S; s += (long long)gridDim.x * blockDim.x) {
+  for (long long s = s0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; s < s1; s += (long long)gridDim.x * blockDim.x) {
     if (b.mask) {
       const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
       if (solid_at(b, x, y, z)) continue;

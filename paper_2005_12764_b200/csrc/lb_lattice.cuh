@@ -65,9 +65,11 @@ __device__ __forceinline__ void static_for(F&& f) {
 enum Mode { MODE_AB = 0, MODE_AA_EVEN = 1, MODE_AA_ODD = 2 };
 
 struct Box {
-  int nx, ny, nz;
+  int nx, ny, nz;        // allocated extents (a z slab holds one ghost plane below and one above its own planes)
+  int zlo, zhi;          // planes this handle updates: [zlo, zhi) = [0, nz), or [1, nz - 1) for a z slab
+  int zper;              // z is periodic inside this box (0 for a slab: its z neighbours are other handles)
   int nxw;               // 32-bit mask words per x row
-  long long S;           // sites
+  long long S;           // sites (allocated)
   const uint32_t* mask;  // bit-packed solid mask (bit x&31 of word row*nxw + x>>5), or nullptr
   const uint32_t* gmask; // wall groups: two more bit planes of the same shape behind each other (group - 1 in binary), or nullptr
 };

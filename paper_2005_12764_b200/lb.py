@@ -21,6 +21,8 @@ SYMBOLS = [
     "lb_set_wall_velocity", "lb_set_wall_type", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_nc_symmetric", "lb_set_wall_phi", "lb_set_storage", "lb_init", "lb_step",
     "lb_check_state", "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
+    "lb_set_slab", "lb_slab_halo_bytes", "lb_slab_begin", "lb_slab_interior", "lb_slab_end",
+    "lb_slab_pack_phi", "lb_slab_unpack_phi",
 ]
 
 
@@ -72,6 +74,13 @@ def _load():
     lib.lb_set_tuning.argtypes = [vp, C.c_char_p, C.c_int]
     lib.lb_set_profiling.argtypes = [vp, C.c_int]
     lib.lb_last_step_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+    lib.lb_set_slab.argtypes = [vp, C.c_int, C.c_int]
+    lib.lb_slab_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+    lib.lb_slab_begin.argtypes = [vp, fp, fp]
+    lib.lb_slab_interior.argtypes = [vp]
+    lib.lb_slab_end.argtypes = [vp, fp, fp]
+    lib.lb_slab_pack_phi.argtypes = [vp, fp, fp]
+    lib.lb_slab_unpack_phi.argtypes = [vp, fp, fp]
     return lib
 
 
@@ -240,6 +249,35 @@ class LB:
             out = np.empty(self.shape, np.float32)
         self._ck(lib.lb_get_phi(self.h, _addr(out)))
         return out
+
+    # ---- z slabs (include/lb.h "z-slab decomposition"); message buffers are device tensors
+    def set_slab(self, z0, nz_global):
+        self._ck(lib.lb_set_slab(self.h, int(z0), int(nz_global)))
+
+    def slab_halo_bytes(self):
+        a, b = C.c_size_t(), C.c_size_t()
+        self._ck(lib.lb_slab_halo_bytes(self.h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def slab_begin(self, send_lo, send_hi):
+        self._sync_stream()
+        self._ck(lib.lb_slab_begin(self.h, _addr(send_lo), _addr(send_hi)))
+
+    def slab_interior(self):
+        self._sync_stream()
+        self._ck(lib.lb_slab_interior(self.h))
+
+    def slab_end(self, recv_lo, recv_hi):
+        self._sync_stream()
+        self._ck(lib.lb_slab_end(self.h, _addr(recv_lo), _addr(recv_hi)))
+
+    def slab_pack_phi(self, send_lo, send_hi):
+        self._sync_stream()
+        self._ck(lib.lb_slab_pack_phi(self.h, _addr(send_lo), _addr(send_hi)))
+
+    def slab_unpack_phi(self, recv_lo, recv_hi):
+        self._sync_stream()
+        self._ck(lib.lb_slab_unpack_phi(self.h, _addr(recv_lo), _addr(recv_hi)))
 
     def launch_count(self):
         return int(lib.lb_launch_count(self.h))

@@ -45,8 +45,12 @@ def _random_workload(nx, ny, nz, seed, walls=False, A_nc=0.02, tau=(0.8, 1.2), g
 @pytest.mark.parametrize("storage", ["ab", "aa"])
 def test_ragged_boxes_all_features(lbmod, lbo, shape, walls, storage):
     """Smallest box, extents that are not multiples of the 32 x 8 tile or of the z chunk, two
-    taus, body force, walls, near contact: populations after 1, 2 and 5 steps."""
-    w = _random_workload(*shape, seed=sum(shape) + walls, walls=walls)
+    taus, body force, walls, near contact: populations after 1, 2 and 5 steps.  The 4 x 4 x 4 box runs
+    without the near-contact force (its probe of 4 sites wraps around the whole box and the G12
+    exclusion set would cover it), so that every one of its sites is checked at every step; on the
+    other boxes the set of checked sites may never be empty."""
+    tiny = shape == (4, 4, 4)
+    w = _random_workload(*shape, seed=sum(shape) + walls, walls=walls, A_nc=0.0 if tiny else 0.02)
     o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
     fluid = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
     assert pu.pop_error(sim, o).max() < pu.POP_TOL
@@ -60,10 +64,13 @@ def test_ragged_boxes_all_features(lbmod, lbo, shape, walls, storage):
             o.step(1); sim.step(1)
         done = n
         e = pu.pop_error(sim, o)
-        ok = ~risky
-        if ok.any():
-            assert e[ok].max() < pu.POP_TOL, (n, e[ok].max())
-        assert risky.mean() < 0.5 or w.sites < 5000     # small boxes: the dilated set grows by a shell per step
+        ok = ~risky & fluid
+        assert ok.any(), (n, risky.mean())
+        assert e[ok].max() < pu.POP_TOL, (n, e[ok].max())
+        if tiny:
+            assert not risky.any()
+        elif n == 1 or w.sites >= 5000:
+            assert risky.mean() < 0.5, (n, risky.mean())     # small boxes: the dilated set grows by a shell per step
     errs, _, _ = pu.macro_errors(sim, o)
     if not risky.any():
         assert max(errs.values()) < pu.MACRO_TOL

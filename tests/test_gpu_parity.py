@@ -98,52 +98,99 @@ def _nc_parity_one_step(lbmod, lbo, w, storage="ab"):
 
 # ------------------------------------------------------------------------------- C4 mini
 def test_C4_mini_channel(lbmod, lbo):
-    """Walls (bit-packed mask, bounce-back), body force, near-contact probe: 1 and 100 steps."""
+    """Walls (bit-packed mask, bounce-back), body force, near-contact probe: populations after 1 step
+    (G12 exclusion), macroscopic fields after 100 and 300 steps at north_star's 1e-4 on EVERY site."""
     w = W.get("c4-mini")
     o, sim, risky = _nc_parity_one_step(lbmod, lbo, w)
     rr0, rb0, _ = pu.make_gpu(lbmod, w).get_macros()
     m0 = pu.masses(rr0, rb0)
     o.step(99); sim.step(99)
     errs, (rr, rb, u), (orr, orb, ou) = pu.macro_errors(sim, o)
-    # a flipped contact decision changes the local force by up to A_nc |G|/2 for a step, so the
-    # max norm gets a looser bound here; the bulk of the sites must meet the 1e-4 bar
-    frac_bad = (np.abs(u - ou).max(0) > pu.MACRO_TOL).mean()
-    assert frac_bad < 1e-3, frac_bad
-    assert errs["u"] < 5e-3 and errs["rho_r"] < 5e-2, errs
+    assert max(errs.values()) < pu.MACRO_TOL, errs
     solid = w.solid != 0
     assert rr[solid].max() == 0 and np.abs(u[:, solid]).max() == 0
     m1 = pu.masses(rr, rb)
     assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
     assert u[0][~solid].mean() > 0        # the body force drives the flow along +x
+    o.step(200); sim.step(200)
+    errs, _, _ = pu.macro_errors(sim, o)
+    assert max(errs.values()) < pu.MACRO_TOL, errs
+
+
+def _long_run_with_tracked_decisions(lbmod, lbo, w, storage, steps):
+    """`steps` steps of both sides; every step the oracle's decision margins (G12) are read.  Returns
+    the per-site error of rho_r, rho_b, u at the end and the set of fluid sites where some discrete
+    decision (|phi| < phi_c, probe rounding, phi(p_k) >= phi(x)) had, at some step, a margin below
+    the tolerance that the fields themselves are held to (MACRO_TOL): a decision whose margin is
+    smaller than the error allowed in its inputs cannot be expected to come out the same in fp32 and
+    fp64."""
+    o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
+    fluid = np.ones(w.shape, bool) if w.solid is None else (w.solid == 0)
+    seeds = np.zeros(w.shape, bool)
+    per_step = []
+    for _ in range(steps):
+        f = o.get_fields()
+        m = (f["margin"] < pu.MACRO_TOL) & fluid
+        per_step.append(((f["margin"] < 1e-5) & fluid).sum() / max(1, ((np.abs(f["phi"]) < w.phi_c) & fluid).sum()))
+        seeds |= m
+        o.step(1); sim.step(1)
+    errs, (rr, rb, u), (orr, orb, ou) = pu.macro_errors(sim, o)
+    site_err = np.maximum(np.maximum(np.abs(rr - orr), np.abs(rb - orb)), np.abs(u - ou).max(0))
+    interface = (np.abs(o.get_fields()["phi"]) < w.phi_c) & fluid
+    return site_err, seeds, fluid, interface, max(per_step), (rr, rb)
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_C4_mini_1000_steps(lbmod, lbo, storage):
+    """north_star's horizon (1000 steps) with walls, body force and near contact.  Over such a run a
+    few contact decisions do flip between fp32 and fp64 (G12); each flip changes the local force by up
+    to A_nc |G| / 2 for a step.  Asserted: (a) outside the tracked set (sites within one shell of a
+    decision that was marginal at some step) every site meets north_star's 1e-4, with room: 1e-5;
+    (b) per step, marginal decisions (margin < 1e-5) stay below 0.1 % of the interface sites (G12's
+    own bound); (c) inside the tracked set the error stays within 10 x the bar and the sites above the
+    bar are fewer than 2 % of the interface sites; (d) the component masses do not drift."""
+    w = W.get("c4-mini")
+    site_err, seeds, fluid, interface, worst_step_frac, (rr, rb) = _long_run_with_tracked_decisions(lbmod, lbo, w, storage, 1000)
+    tracked = pu.dilate(seeds, 1) & fluid
+    assert (fluid & ~tracked).sum() > 0.1 * fluid.sum()
+    assert site_err[fluid & ~tracked].max() < 0.1 * pu.MACRO_TOL, site_err[fluid & ~tracked].max()
+    assert worst_step_frac < 1e-3, worst_step_frac
+    assert site_err.max() < 10 * pu.MACRO_TOL, site_err.max()
+    assert (site_err > pu.MACRO_TOL).sum() < 0.02 * interface.sum(), ((site_err > pu.MACRO_TOL).sum(), interface.sum())
+    m0 = pu.masses(w.rho_r * (w.solid == 0), w.rho_b * (w.solid == 0))
+    m1 = pu.masses(rr, rb)
+    assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
 
 
 # ------------------------------------------------------------------------------- C5 mini
 @pytest.mark.parametrize("storage", ["ab", "aa"])
 def test_C5_mini_emulsion(lbmod, lbo, storage):
-    """Dense emulsion with near contact, A/B and AA storage: 1, 2, 3 steps (both AA parities)."""
+    """Dense emulsion with near contact, A/B and AA storage: populations after 1, 2, 3 steps (both AA
+    parities).  The G12 exclusion set is carried along: every step adds the sites whose decisions are
+    marginal now, and what was excluded before spreads by one shell; everything else is held to 1e-5."""
     w = W.get("c5-mini")
     o, sim, risky = _nc_parity_one_step(lbmod, lbo, w, storage)
+    fluid = np.ones(w.shape, bool)
+    risky = pu.dilate(risky, 1)
     for n in (2, 3):
+        risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
         o.step(1); sim.step(1)
         e = pu.pop_error(sim, o)
-        ok = ~pu.dilate(risky, n + 1)
-        # later steps may meet new marginal decisions: allow a handful of outliers
-        assert (e[ok] > pu.POP_TOL).sum() <= 50 and np.quantile(e[ok], 0.9999) < pu.POP_TOL, (n, e[ok].max())
+        assert risky.mean() < 0.01, risky.mean()
+        assert e[~risky].max() < pu.POP_TOL, (n, e[~risky].max())
 
 
 @pytest.mark.parametrize("storage", ["ab", "aa"])
-def test_C5_mini_100_steps_macros(lbmod, lbo, storage):
-    """100 steps of the dense emulsion with near contact: macroscopic fields against the oracle.
-    A contact decision that flips between fp32 and fp64 changes the local force for a step, so the
-    bulk of the sites must meet the 1e-4 bar and the max norm gets a looser bound (as in C4-mini)."""
+def test_C5_mini_300_steps_macros(lbmod, lbo, storage):
+    """100 and 300 steps of the dense emulsion with near contact: rho_r, rho_b, u against the oracle at
+    north_star's 1e-4 on EVERY site, and the mass drift."""
     w = W.get("c5-mini")
     o, sim = pu.make_oracle(lbo, w), pu.make_gpu(lbmod, w, storage)
     m0 = pu.masses(w.rho_r, w.rho_b)
-    o.step(100); sim.step(100)
-    errs, (rr, rb, u), (orr, orb, ou) = pu.macro_errors(sim, o)
-    frac_bad = (np.abs(u - ou).max(0) > pu.MACRO_TOL).mean()
-    assert frac_bad < 1e-3, frac_bad
-    assert errs["u"] < 5e-3 and errs["rho_r"] < 5e-2, errs
+    for n in (100, 200):
+        o.step(n); sim.step(n)
+        errs, (rr, rb, u), _ = pu.macro_errors(sim, o)
+        assert max(errs.values()) < pu.MACRO_TOL, (n, errs)
     m1 = pu.masses(rr, rb)
     assert abs(m1[0] - m0[0]) / m0[0] < pu.DRIFT_TOL and abs(m1[1] - m0[1]) / m0[1] < pu.DRIFT_TOL
 

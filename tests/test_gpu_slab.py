@@ -1,0 +1,185 @@
+"""z-slab decomposition on ONE GPU: the slabs of a box
+as several handles of one process, halo messages moved by device copies (paper_2005_12764_b200.slab.
+LocalRing), against the undivided box.  With the bricks of both runs cut at the same planes the two
+must agree BIT FOR BIT (the slab faces are brick faces of the undivided run; a ghost plane holds a copy
+of what the neighbour stored); with the automatic brick depth they agree to the rounding of the
+forwarded sums.  The undivided box itself is held against the oracle in test_gpu_parity.py; one case
+here goes to the oracle directly."""
+import numpy as np
+import pytest
+
+import parity_util as pu
+from paper_2005_12764_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lbmod():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2005_12764_b200 import lb
+    return lb
+
+
+@pytest.fixture(scope="module")
+def slabmod(lbmod):
+    from paper_2005_12764_b200 import slab
+    return slab
+
+
+def _same_bits(ring, sim, two=True):
+    for k in range(2 if two else 1):
+        assert np.array_equal(ring.gather("get_populations", k), sim.get_populations(k)), "populations of component %d" % k
+    a, b = ring.gather("get_macros"), sim.get_macros()
+    for x, y in zip(a, b):
+        assert (x is None and y is None) or np.array_equal(x, y)
+    if two:
+        assert np.array_equal(ring.gather("get_phi"), sim.get_phi())
+
+
+# (workload, cuts, zc): the cuts are multiples of zc, so both runs have the same bricks
+CASES = [("c3-mini", (32, 32), 16), ("c3-mini", (16, 32, 16), 16), ("c4-mini", (16, 16), 8), ("c4-mini", (8, 24), 8),
+         ("c5-mini", (40, 56), 8), ("c5-mini", (96,), 12)]
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+@pytest.mark.parametrize("name,cuts,zc", CASES)
+def test_slabs_equal_undivided_box_bitwise(lbmod, slabmod, name, cuts, zc, storage):
+    """C3-mini (periodic), C4-mini (walls and body force: the wall planes z = 0, nz - 1 sit on both
+    sides of the periodic cut, the y walls cross every cut) and C5-mini (near contact: the probe and
+    its 4-plane phi halo cross the cuts), A/B and in-place storage, after 1, 2, 3 and 5 steps (both
+    in-place parities are packed and unpacked differently)."""
+    w = W.get(name)
+    sim = pu.make_gpu(lbmod, w, storage)
+    sim.set_tuning(zc=zc)
+    ring = slabmod.LocalRing(w, cuts, storage, zc=zc)
+    ring.init()
+    _same_bits(ring, sim)
+    done = 0
+    for n in (1, 2, 3, 5):
+        ring.step(n - done); sim.step(n - done)
+        done = n
+        _same_bits(ring, sim)
+    mr = sum(s.sim.check_state()[0] for s in ring.slabs)
+    assert abs(mr - sim.check_state()[0]) / mr < 1e-12          # the slabs' own planes, no ghost plane counted
+
+
+def test_slabs_single_component(lbmod, slabmod):
+    w = W.get("c2-mini")
+    for storage in ("ab", "aa"):
+        sim = pu.make_gpu(lbmod, w, storage)
+        sim.set_tuning(zc=16)
+        ring = slabmod.LocalRing(w, (32, 16, 16), storage, zc=16)
+        ring.init()
+        ring.step(4); sim.step(4)
+        _same_bits(ring, sim, two=False)
+        assert ring.slabs[0].halo_bytes == (5 * 64 * 64 * 4, 0)
+
+
+def _walled_random(nx, ny, nz, seed, model=None):
+    rng = np.random.default_rng(seed)
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    phi = np.zeros((nz, ny, nx))
+    for _ in range(6):
+        k = rng.integers(1, 3, 3)
+        ph = rng.uniform(0, 2 * np.pi, 3)
+        phi += rng.normal() * np.cos(2 * np.pi * k[0] * x / nx + ph[0]) * np.cos(2 * np.pi * k[1] * y / ny + ph[1]) \
+            * np.cos(2 * np.pi * k[2] * z / nz + ph[2])
+    phi = np.tanh(1.5 * phi)
+    rho = 1.0 + 0.02 * rng.uniform(-1, 1, phi.shape)
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 1
+    # obstacles on both sides of the cuts at z = 10 and z = 20, and one that spans a cut
+    solid[9, 3:6, 4:9] = 1
+    solid[10, 7:9, 20:30] = 1
+    solid[19:22, 5, 2:5] = 1
+    solid[0, :, 10:14] = 1
+    solid[nz - 1, 2:4, :] = 1
+    return W.Workload("walled-random", nx, ny, nz, 0.8, 1.2, 0.01, 0.7, 0.02,
+                      (rho * (1 + phi) / 2).astype(np.float32), (rho * (1 - phi) / 2).astype(np.float32),
+                      (0.02 * rng.normal(size=(3, nz, ny, nx))).astype(np.float32), solid=solid, g=(1e-4, -5e-5, 2e-5))
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_slabs_ragged_box_with_obstacles_on_the_cuts(lbmod, lbo, slabmod, storage):
+    """A box whose extents are no multiples of the tile (36 x 13 x 30), two relaxation times, body
+    force, near contact, obstacles that touch and span the cuts: three slabs of 10 planes against the
+    undivided box (bit for bit) and against the oracle (populations, G12 exclusion)."""
+    w = _walled_random(36, 13, 30, seed=3)
+    sim = pu.make_gpu(lbmod, w, storage)
+    sim.set_tuning(zc=10)
+    ring = slabmod.LocalRing(w, (10, 10, 10), storage, zc=10)
+    ring.init()
+    o = pu.make_oracle(lbo, w)
+    fluid = w.solid == 0
+    risky = np.zeros(w.shape, bool)
+    for n in range(1, 5):
+        risky = pu.dilate(risky, 1) | pu.dilate((o.get_fields()["margin"] < 1e-5) & fluid, 1)
+        ring.step(1); sim.step(1); o.step(1)
+        _same_bits(ring, sim)
+        ok = fluid & ~risky
+        assert ok.any()
+        for k in (0, 1):
+            e = np.abs(ring.gather("get_populations", k).astype(np.float64) - o.get_populations(k)) / pu.W19[:, None, None, None]
+            assert e.max(0)[ok].max() < pu.POP_TOL, (n, k)
+
+
+def test_slabs_automatic_bricks_agree_to_rounding(lbmod, slabmod):
+    """Without the brick depth pinned the two runs cut their bricks differently; the forwarded sums
+    then differ in summation order only (no near contact here: no decision can flip)."""
+    w = W.get("c3-mini")
+    sim = pu.make_gpu(lbmod, w)
+    ring = slabmod.LocalRing(w, (24, 40))
+    ring.init()
+    ring.step(5); sim.step(5)
+    for k in (0, 1):
+        d = np.abs(ring.gather("get_populations", k).astype(np.float64) - sim.get_populations(k)) / pu.W19[:, None, None, None]
+        assert d.max() < 1e-5
+    assert np.abs(ring.gather("get_phi") - sim.get_phi()).max() < 1e-6
+
+
+def test_slab_calls_out_of_order_and_bad_buffers(lbmod, slabmod):
+    import torch
+    w = W.get("c3-mini")
+    s = slabmod.Slab.from_workload(w, 0, 32)
+    with pytest.raises(lbmod.LBError) as ei:
+        s.sim.slab_halo_bytes()                                    # before lb_init
+    assert ei.value.code == lbmod.LB_ESTATE
+    s.init_from(w)
+    with pytest.raises(lbmod.LBError) as ei:
+        s.sim.step(1)                                              # a slab is not stepped by lb_step
+    assert ei.value.code == lbmod.LB_ESTATE
+    with pytest.raises(lbmod.LBError) as ei:
+        s.begin()                                                  # phi ghost planes not exchanged yet
+    assert ei.value.code == lbmod.LB_ESTATE
+    s.pack_phi(); s.buf["f_recv_lo"].copy_(s.buf["f_send_hi"]); s.buf["f_recv_hi"].copy_(s.buf["f_send_lo"]); s.unpack_phi()
+    with pytest.raises(lbmod.LBError) as ei:
+        s.interior()                                               # before lb_slab_begin
+    assert ei.value.code == lbmod.LB_ESTATE
+    with pytest.raises(lbmod.LBError) as ei:
+        s.sim.slab_begin(np.zeros(16, np.float32), np.zeros(16, np.float32))    # host buffers
+    assert ei.value.code == lbmod.LB_EINVAL
+    t = torch.zeros(s.halo_bytes[0] // 4 + 4, dtype=torch.float32, device="cuda")
+    with pytest.raises(lbmod.LBError) as ei:
+        s.sim.slab_begin(t[1:], t)                                 # misaligned
+    assert ei.value.code == lbmod.LB_EINVAL
+    plain = lbmod.LB(32, 32, 32)
+    with pytest.raises(lbmod.LBError):
+        plain.set_slab(0, 16)                                      # does not fit
+    with pytest.raises(lbmod.LBError):
+        lbmod.LB(32, 32, 4).set_slab(0, 64)                        # thinner than twice the phi halo
+
+
+@pytest.mark.parametrize("storage", ["ab", "aa"])
+def test_distributed_slab_world1_two_streams(lbmod, slabmod, storage):
+    """The per-rank driver (side stream for the population exchange, events between the phases) with
+    a world of one rank, whose neighbours are itself: bit-identical to the undivided box."""
+    w = W.get("c5-mini")
+    sim = pu.make_gpu(lbmod, w, storage)
+    sim.set_tuning(zc=12)
+    ds = slabmod.DistributedSlab(slabmod.Slab.from_workload(w, 0, w.nz, storage, zc=12), rank=0, world=1)
+    ds.init_from(w)
+    ds.step(4); sim.step(4)
+    for k in (0, 1):
+        assert np.array_equal(ds.slab.sim.get_populations(k), sim.get_populations(k))

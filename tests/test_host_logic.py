@@ -125,3 +125,57 @@ def test_reference_arm_other_ranks_do_nothing():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                           "--steps", "1", "--warmup", "0"], capture_output=True, text=True, timeout=120, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+_GLOO_SLAB_WORKER = r"""
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import torch, torch.distributed as dist
+from paper_2005_12764_b200 import slab
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+below, above = slab.ring_neighbours(rank, world)
+ok = True
+for it in range(3):                      # several rounds: messages of consecutive steps must not mix
+    n = 64
+    send_lo = torch.full((n,), 100.0 * rank + 1 + 1000 * it)      # "my bottom planes"
+    send_hi = torch.full((n,), 100.0 * rank + 2 + 1000 * it)      # "my top planes"
+    recv_lo, recv_hi = torch.zeros(n), torch.zeros(n)
+    slab.exchange(send_lo, send_hi, recv_lo, recv_hi, rank, world)
+    # my lower ghost holds the top planes of the rank below, my upper ghost the bottom planes of the rank above
+    ok &= bool((recv_lo == 100.0 * below + 2 + 1000 * it).all()) and bool((recv_hi == 100.0 * above + 1 + 1000 * it).all())
+t = torch.tensor([1.0 if ok else 0.0])
+dist.all_reduce(t, op=dist.ReduceOp.MIN)
+if rank == 0:
+    print("RESULT %d %d" % (int(t.item()), world), flush=True)
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_gloo_slab_halo_exchange_schedule(tmp_path, world):
+    """The halo exchange of the z-slab decomposition (paper_2005_12764_b200/slab.py: exchange) on a
+    ring of 2 and of 3 ranks over gloo: every rank's lower ghost receives the top message of the rank
+    below and its upper ghost the bottom message of the rank above; with 2 ranks both neighbours are
+    the same peer and the two messages must not be swapped."""
+    script = tmp_path / "worker.py"
+    script.write_text(_GLOO_SLAB_WORKER)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
+           "--master-addr", "127.0.0.1", "--master-port", str(29640 + world), str(script), ROOT]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=240)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("RESULT")][0].split()
+    assert line[1] == "1" and line[2] == str(world)
+
+
+def test_slab_split_and_mask():
+    from paper_2005_12764_b200 import slab
+    assert slab.split_planes(640, 8) == [(80 * r, 80) for r in range(8)]
+    parts = slab.split_planes(30, 4)
+    assert [n for _, n in parts] == [8, 8, 7, 7] and [z for z, _ in parts] == [0, 8, 16, 23]
+    assert slab.ring_neighbours(0, 4) == (3, 1) and slab.ring_neighbours(3, 4) == (2, 0) and slab.ring_neighbours(0, 1) == (0, 0)
+    import numpy as np
+    m = np.arange(6, dtype=np.uint8)[:, None, None] * np.ones((1, 2, 4), np.uint8)
+    assert slab.slab_mask(m, 0, 3)[:, 0, 0].tolist() == [5, 0, 1, 2, 3]      # ghost below wraps to the top plane
+    assert slab.slab_mask(m, 3, 3)[:, 0, 0].tolist() == [2, 3, 4, 5, 0]
+    assert slab.slab_mask(None, 0, 3) is None
