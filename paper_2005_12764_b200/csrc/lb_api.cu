@@ -966,10 +966,29 @@ int slab_msg_check(lb_handle h, const void* lo, const void* hi) {
   return LB_OK;
 }
 
-// pack (blocks of `buf` -> messages) or unpack (messages -> blocks of `buf`)
-void slab_copy_populations(lb_handle h, float* buf, const SlabBlocks& b, void* msg_lo, void* msg_hi, bool pack) {
+// pack (blocks of `buf` -> messages) or unpack (messages -> blocks of `buf`); merge: unpack after an
+// in-place odd step between walls (k_halo_merge: only the slots whose source site is fluid)
+void slab_copy_populations(lb_handle h, float* buf, const SlabBlocks& b, void* msg_lo, void* msg_hi, bool pack, bool merge = false) {
   const size_t esz = h->two ? 2 : 1;                       // floats per site in a plane
   const size_t blockf = (size_t)h->nx * h->ny * esz;       // floats per (direction, plane) block
+  if (merge) {
+    HaloMerge m;
+    void* msg[2] = {msg_lo, msg_hi};
+    for (int f = 0; f < 2; ++f)
+      for (int k = 0; k < 5; ++k) {
+        m.src[f][k] = static_cast<const float*>(msg[f]) + (size_t)k * blockf;
+        m.dst[f][k] = buf + (size_t)b.dirs[f][k] * h->S * esz + (size_t)b.plane[f] * blockf;
+        m.dirs[f][k] = b.dirs[f][k];
+      }
+    m.zsrc[0] = h->zlo() - 1;      // upward populations came out of the plane below the slab
+    m.zsrc[1] = h->zhi();          // downward ones out of the plane above
+    m.box = h->box();
+    const dim3 grid((unsigned)(((size_t)h->nx * h->ny + 255) / 256), 5, 2);
+    if (h->two) k_halo_merge<8><<<grid, 256, 0, h->stream>>>(m);
+    else k_halo_merge<4><<<grid, 256, 0, h->stream>>>(m);
+    h->launches++;
+    return;
+  }
   HaloCopy c;
   c.n4 = (long long)(blockf / 4);
   void* msg[2] = {msg_lo, msg_hi};
@@ -1052,7 +1071,8 @@ int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi) {
   if (rc) return rc;
   if ((rc = slab_msg_check(h, recv_lo, recv_hi))) return rc;
   DeviceGuard guard(h->device);
-  slab_copy_populations(h, next_buf(h), slab_recv_blocks(h, h->mode()), const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false);
+  slab_copy_populations(h, next_buf(h), slab_recv_blocks(h, h->mode()), const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), false,
+                        h->mode() == MODE_AA_ODD && h->has_solid);
   const int H = slab_phi_halo(h);
   launch_phase_forward(h, h->zlo(), std::min(h->zlo() + H, h->zhi()));
   launch_phase_forward(h, std::max(h->zhi() - H, h->zlo() + H), h->zhi());

@@ -1343,6 +1343,33 @@ __global__ void __launch_bounds__(256) k_halo_copy(const HaloCopy p) {
   p.dst[f][k][i] = __ldcg(p.src[f][k] + i);
 }
 
+// Unpacking after an in-place ODD step with walls.  That step pushed f*_q into slot (q, x + c_q); what
+// it pushed across a z face sits in the sender's ghost plane and belongs to the receiver's boundary
+// plane.  But a receiver site y whose source y - c_q is SOLID keeps the value it wrote itself (the
+// bounced-back population went to slot (q, y) at its own site), so the message may only overwrite
+// the slots whose source site, in the receiver's ghost plane zsrc[f], is fluid.
+struct HaloMerge {
+  const float* src[2][5];
+  float* dst[2][5];
+  int dirs[2][5];
+  int zsrc[2];
+  Box box;
+};
+template <int ESZ>       // bytes per site: 8 = {T, R} pair, 4 = one component
+__global__ void __launch_bounds__(256) k_halo_merge(const HaloMerge p) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const Box& b = p.box;
+  if (i >= (long long)b.nx * b.ny) return;
+  const int k = blockIdx.y, f = blockIdx.z, q = p.dirs[f][k];
+  const int x = (int)(i % b.nx), y = (int)(i / b.nx);
+  int xs = x - c_cx[q], ys = y - c_cy[q];
+  xs = xs < 0 ? b.nx - 1 : (xs >= b.nx ? 0 : xs);
+  ys = ys < 0 ? b.ny - 1 : (ys >= b.ny ? 0 : ys);
+  if (solid_at(b, xs, ys, p.zsrc[f])) return;
+  if constexpr (ESZ == 8) reinterpret_cast<float2*>(p.dst[f][k])[i] = __ldcg(reinterpret_cast<const float2*>(p.src[f][k]) + i);
+  else p.dst[f][k][i] = __ldcg(p.src[f][k] + i);
+}
+
 // bytes [S] (0 fluid, 1 wall at rest, 2 / 3 / 4 wall groups) -> bit-packed words: solid, and
 // (if groups != nullptr) two bit planes behind each other that hold group - 1 in binary
 __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* groups, Box b) {
