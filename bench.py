@@ -9,9 +9,10 @@ row A0-A10 of the hot path.  Prints ONE JSON line.
                   [--model cg|sc] [--windows N]
   python bench.py --impl reference ...     # the fp64 CPU oracle on this box's host cores
 
-N > 1 (torchrun): the path does not shard in this build ("replicas only"): every
-rank advances its own box; value = N * sites * K / max-over-ranks time; no collective is on
-the data path.
+N > 1 (torchrun): z-slab decomposition, weak scaling: every rank holds the workload's
+box as one slab of a box N times as tall and exchanges, per step and face, 5 populations per component
+and H planes of phi with its two neighbours (NCCL send/recv; paper_2005_12764_b200/slab.py);
+value = N * sites * K / max-over-ranks time.
 """
 from __future__ import annotations
 
@@ -223,7 +224,43 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------ GPU arm
-def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with_e2e=False, windows=0):
+class SlabRunner:
+    """N > 1 (or --slabs): this rank's box is one z slab of a box N times as tall (the workload
+    repeated along z, which is periodic), advanced by paper_2005_12764_b200/slab.py: halo exchange of 5
+    populations per component and H phi planes per face and step over NCCL send/recv, the population
+    exchange on a side stream under the interior bricks.  Same interface as lb.LB where bench uses it."""
+
+    def __init__(self, w, storage, rank, world):
+        from paper_2005_12764_b200 import slab
+        self.ds = slab.DistributedSlab(slab.Slab.from_workload(w, rank * w.nz, w.nz, storage, nz_global=world * w.nz), rank, world)
+        self.sim = self.ds.slab.sim
+
+    def init(self, rr, rb, u):
+        self.ds.init(rr, rb, u)
+
+    def step(self, n):
+        self.ds.step(n)
+
+    def check_state(self):
+        return self.sim.check_state()
+
+    def launch_count(self):
+        return self.sim.launch_count()
+
+    def get_macros(self, *a):
+        return self.sim.get_macros(*a)
+
+    def set_profiling(self, on):
+        pass
+
+    def last_step_ms(self, which):
+        return None           # the slab phases are not timed kernel by kernel
+
+    def destroy(self):
+        self.sim.destroy()
+
+
+def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with_e2e=False, windows=0, slabs=False):
     """One workload on this rank's GPU: W warm-up steps, then K timed steps (CUDA events on the
     handle's stream, barrier + synchronize on both sides, MAX over ranks).  Returns the record
     (value, ms_per_step, roofline, clocks, checks, optionally e2e) and the workload."""
@@ -237,9 +274,13 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
     d_rr = torch.from_numpy(w.rho_r).to(dev)
     d_rb = torch.from_numpy(w.rho_b).to(dev) if two else None
     d_u = torch.from_numpy(w.u).to(dev)
-    sim = lb.from_workload(w, storage=storage)
-    if MODEL[0] == "sc":
-        sim.set_model("sc", MODEL[1])
+    rank = dist.get_rank() if world > 1 else 0
+    if slabs:
+        sim = SlabRunner(w, storage, rank, world)
+    else:
+        sim = lb.from_workload(w, storage=storage)
+        if MODEL[0] == "sc":
+            sim.set_model("sc", MODEL[1])
     sim.init(d_rr, d_rb, d_u)
     mass0 = sim.check_state()
     sim.set_profiling(7)      # every 7th step (odd, so that both AA parities are sampled) is timed kernel by kernel (CUDA events on the stream)
@@ -269,6 +310,10 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
     ms = ev0.elapsed_time(ev1)
     ms_k2 = sim.last_step_ms(1)
     ms_k1 = sim.last_step_ms(2) if two else 0.0
+    kernel_timing = "CUDA events around every 7th step of the timed region"
+    if ms_k2 is None:        # slabs: the fused kernel runs as three launches per step; the whole step stands in
+        ms_k2, ms_k1 = ms / K, None
+        kernel_timing = "slab phases are not timed kernel by kernel: kernel_ms is the whole step (boundary + interior bricks, phase field, packing, exchange)"
     ms_max = max_over_ranks(ms, world, dev)
     value = glups(w.fluid_sites, K, ms_max * 1e-3, world)
 
@@ -284,12 +329,12 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
     whole = upd_bytes * w.fluid_sites * K / (ms * 1e-3) / 1e9
     kname = ("k_fused(sc)" if MODEL[0] == "sc" else "k_fused") if two else "k_single"
     rec = {"value": value, "unit": "GLUPS", "ms_per_step": ms_max / K,
-           "config": config_of(w, storage, {"parallelism": "replicas x%d" % world}),
+           "config": config_of(w, storage, {"parallelism": ("z-slabs x%d of a %dx%dx%d box, halo exchange by NCCL send/recv" % (world, w.nx, w.ny, world * w.nz)) if slabs else "single GPU"}),
            "roofline": {"bound": "hbm", "kernel": "k_fused" if two else "k_single", "achieved": achieved, "peak": peak,
                         "unit": "GB/s", "frac": achieved / peak, "traffic": stored_traffic(kname, wl_name, storage),
                         "peak_source": peak_src, "algorithmic_bytes_per_update": upd_bytes,
                         "kernel_ms": ms_k2, "kernel_share_of_step": ms_k2 * K / ms,
-                        "phase_kernel_ms": ms_k1, "kernel_timing": "CUDA events around every 7th step of the timed region",
+                        "phase_kernel_ms": ms_k1, "kernel_timing": kernel_timing,
                         "whole_step_effective_gbs": whole, "whole_step_frac": whole / peak,
                         "whole_step_frac_of_nominal_8000": whole / NOMINAL_HBM_GBS},
            "clocks": dict(clk.result, remeasured=remeasured), "gpu_launches": int(launches),
@@ -365,7 +410,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     K, Wu = args.steps, args.warmup
 
-    head, w = measure_config(args.workload, args.storage, K, Wu, dev, local_rank, world, with_e2e=True, windows=args.windows)
+    head, w = measure_config(args.workload, args.storage, K, Wu, dev, local_rank, world, with_e2e=True, windows=args.windows,
+                             slabs=world > 1 or args.slabs)
     extra = []
     if args.configs == "all" and world == 1 and MODEL[0] == "cg":
         for name, storage in EXTRA_CONFIGS:
@@ -404,6 +450,7 @@ def main(argv=None):
     ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slabs", action="store_true", help="run the z-slab driver also at N = 1 (the rank is then its own neighbour)")
     ap.add_argument("--configs", default=None, choices=["all", "none"], help="all = also measure C3 A/B, C4 A/B, C5 AA and C2 and report them under 'configs' (default when --workload is left at c5)")
     ap.add_argument("--model", default="cg", choices=["cg", "sc"], help="cg = colour gradient (north_star), sc = Shan-Chen + exact difference (Eq. 5-10 of the paper)")
     ap.add_argument("--gc", type=float, default=3.0, help="G_C of the Shan-Chen model")

@@ -152,8 +152,8 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
 int lb_step(lb_handle h, int nsteps);
 
 /* State check (G23; the paper names fault tolerance as an exascale issue):
- * sums rho_r and rho_b (Eq. 3) over the fluid sites on the device, in double
- * precision, and looks for NaN / Inf populations.  Returns LB_ESTATE (text: how many sites, after
+ * sums rho_r and rho_b (Eq. 3) over the handle's own fluid sites on the device, in
+ * double precision, and looks for NaN / Inf populations.  Returns LB_ESTATE (text: how many sites, after
  * how many steps) if the state is not finite, LB_OK otherwise; mass_r, mass_b (HOST pointers, may
  * be NULL) receive the sums (single component: mass_r is the mass, mass_b is 0).  Synchronises the
  * stream.  lb_step runs the same check by itself every 1000 steps since the last check and then

@@ -250,18 +250,23 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc, i
 // whole waves of (SMs x resident CTAs) best.
 int pick_zc(lb_handle h) {
   int zc = 16;
+  if (!h->sm_count) {       // of the handle's own device
+    int sms = 148;
+    if (h->device >= 0) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
+    cudaGetLastError();
+    h->sm_count = sms;
+  }
+  // resident CTAs per SM: 3, but 2 for the instantiations with wall groups (WALLS = 2)
+  const int slots = ((h->has_solid && h->has_moving) ? 2 : 3) * h->sm_count;
+  const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
   if (h->tune_zc > 0) zc = h->tune_zc < h->nz ? h->tune_zc : h->nz;
-  else if (h->nz <= 10) zc = h->nz;
-  else {
-    if (!h->sm_count) {       // of the handle's own device
-      int sms = 148;
-      if (h->device >= 0) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
-      cudaGetLastError();
-      h->sm_count = sms;
-    }
-    // resident CTAs per SM: 3, but 2 for the instantiations with wall groups (WALLS = 2)
-    const int slots = ((h->has_solid && h->has_moving) ? 2 : 3) * h->sm_count;
-    const long long cols = (long long)((h->nx + TX - 1) / TX) * ((h->ny + TY - 1) / TY);
+  else if (cols * ((h->nz + 9) / 10) < slots) {
+    // A box that does not fill one wave of CTAs even with 10-plane bricks (32^3: 8 bricks on 148 SMs):
+    // the step then lasts as long as ONE brick, so the bricks are made as shallow as one wave allows
+    // (C1: 27 -> 9 us per step).  Such a box lives in L2; the extra phi-ring prologues cost no HBM traffic.
+    zc = (int)((cols * h->nz + slots - 1) / slots);
+    if (zc < 1) zc = 1;
+  } else {
     double best_eff = -1.0;
     for (int c = 10; c <= 20 && c <= h->nz; ++c) {
       const long long ctas = cols * ((h->nz + c - 1) / c);
@@ -273,6 +278,7 @@ int pick_zc(lb_handle h) {
   }
   // A slab's phi planes that wait for the halo, [zlo, zlo + H) and [zhi - H, zhi), must not touch an
   // inner brick face (lb_slab_end): bricks deeper than the phi halo, or one brick for the whole slab.
+  if (zc > h->nz) zc = h->nz;
   if (h->gz && zc <= H_MAX_NC) zc = h->nz;
   return zc;
 }
@@ -487,6 +493,26 @@ LB_IO_DISPATCH(k_scatter)
 LB_IO_DISPATCH(k_gatherf)
 LB_IO_DISPATCH(k_macros)
 #undef LB_IO_DISPATCH
+template <int MODE, bool TWO>
+void launch_check_t(lb_handle h, const IoParams& p, int nb) {
+  if (h->has_solid) k_check<MODE, TWO, true><<<nb, 256, 0, h->stream>>>(p, h->chk);
+  else k_check<MODE, TWO, false><<<nb, 256, 0, h->stream>>>(p, h->chk);
+}
+void launch_check(lb_handle h) {
+  const IoParams p = make_io_params(h);
+  const int nb = (int)std::min<long long>((p.s1 - p.s0 + 255) / 256, 148 * 16);
+  const int mode = h->mode();
+  if (h->two) {
+    if (mode == MODE_AB) launch_check_t<MODE_AB, true>(h, p, nb);
+    else if (mode == MODE_AA_EVEN) launch_check_t<MODE_AA_EVEN, true>(h, p, nb);
+    else launch_check_t<MODE_AA_ODD, true>(h, p, nb);
+  } else {
+    if (mode == MODE_AB) launch_check_t<MODE_AB, false>(h, p, nb);
+    else if (mode == MODE_AA_EVEN) launch_check_t<MODE_AA_EVEN, false>(h, p, nb);
+    else launch_check_t<MODE_AA_ODD, false>(h, p, nb);
+  }
+  h->launches++;
+}
 void launch_scatter(lb_handle h, const IoParams& p) { launch_k_scatter(h, p); }
 void launch_gatherf(lb_handle h, const IoParams& p) { launch_k_gatherf(h, p); }
 void launch_macros(lb_handle h, const IoParams& p) { launch_k_macros(h, p); }
@@ -500,11 +526,7 @@ int state_check(lb_handle h, double* mass_r, double* mass_b) {
   }
   cudaError_t e = cudaMemsetAsync(h->chk, 0, 3 * sizeof(double), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "state check memset");
-  const long long s0 = (long long)h->zlo() * h->nx * h->ny, s1 = (long long)h->zhi() * h->nx * h->ny;
-  const int nb = (int)std::min<long long>((s1 - s0 + 255) / 256, 148 * 16);
-  if (h->two) k_check<true><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), s0, s1, h->chk);
-  else k_check<false><<<nb, 256, 0, h->stream>>>(h->cur_buf(), h->box(), s0, s1, h->chk);
-  h->launches++;
+  launch_check(h);
   double out[3] = {0, 0, 0};
   e = cudaMemcpyAsync(out, h->chk, sizeof(out), cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);

@@ -1307,6 +1307,56 @@ __global__ void __launch_bounds__(256) k_macros(const IoParams p) {
   if (p.out2) { p.out2[t.e] = ux; p.out2[t.Sx + t.e] = uy; p.out2[2 * t.Sx + t.e] = uz; }
 }
 
+// State check (DESIGN.md G23: "lb_step reports LB_ESTATE if the mass check it runs every 1000 steps
+// is non-finite"; the paper names fault tolerance as an exascale issue): the component
+// masses sum_x rho_k(x), rho_k = sum_q f^k_q (Eq. 3), over the handle's own fluid sites,
+// gathered with the read rule of the current storage mode like every other kernel.
+// out[0] += sum rho_r, out[1] += sum rho_b, out[2] += number of sites holding a non-finite value.
+template <int MODE, bool TWO, bool HAS_SOLID>
+__global__ void __launch_bounds__(256) k_check(const IoParams p, double* out) {
+  const Box& b = p.box;
+  double sr = 0.0, sb = 0.0, bad = 0.0;
+  for (long long s = p.s0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; s < p.s1; s += (long long)gridDim.x * blockDim.x) {
+    const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
+    uint32_t smask = 0;
+    if constexpr (HAS_SOLID) {
+      if (solid_at(b, x, y, z)) continue;
+      smask = neighbour_mask(b, x, y, z);
+    }
+    Ctx c;
+    make_ctx<TWO ? 8 : 4>(c, b, x, y, z);
+    float t = 0.f, r = 0.f;
+    static_for<0, Q>([&](auto qc) {
+      constexpr int q = decltype(qc)::value;
+      const float* src = src_ptr(p, read_slot<MODE, HAS_SOLID, q>(c, smask));
+      if constexpr (TWO) {
+        const float2 v = __ldcg(reinterpret_cast<const float2*>(src));
+        t += v.x; r += v.y;
+      } else {
+        t += __ldcg(src);
+      }
+    });
+    if (!isfinite(t) || !isfinite(r)) { bad += 1.0; continue; }
+    if constexpr (TWO) { sr += (double)r; sb += (double)(1.0f + t) - (double)r; }
+    else sr += (double)(1.0f + t);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sr += __shfl_down_sync(0xffffffffu, sr, o);
+    sb += __shfl_down_sync(0xffffffffu, sb, o);
+    bad += __shfl_down_sync(0xffffffffu, bad, o);
+  }
+  __shared__ double red[3][8];
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  if (lane == 0) { red[0][wp] = sr; red[1][wp] = sb; red[2][wp] = bad; }
+  __syncthreads();
+  if (threadIdx.x < 3) {
+    double v = 0.0;
+    for (int i = 0; i < 8; ++i) v += red[threadIdx.x][i];
+    if (v != 0.0) atomicAdd(out + threadIdx.x, v);
+  }
+}
+
 // phi without ghost layers or sentinels, for lb_get_phi (Shan-Chen: from the rho_r, rho_b arrays)
 __global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box b, long long s0, long long s1) {
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1390,50 +1440,6 @@ __global__ void k_pack_mask(const uint8_t* bytes, uint32_t* words, uint32_t* gro
   }
   words[wi] = m;
   if (groups) { groups[wi] = g2; groups[nw + wi] = g3; }
-}
-
-// State check (DESIGN.md G23: "lb_step reports LB_ESTATE if the mass check it runs every 1000 steps
-// is non-finite"; the paper names fault tolerance as an exascale issue).  In every
-// storage mode each slot of a fluid site holds one population of one fluid site, so the sums over the
-// slots of the fluid sites are the component masses (Eq. 3, summed over the box).
-// out[0] += sum rho_r, out[1] += sum rho_b, out[2] += number of sites holding a non-finite value.
-template <bool TWO>
-__global__ void __launch_bounds__(256) k_check(const float* __restrict__ buf, const Box b, long long s0, long long s1, double* out) {
-  double sr = 0.0, sb = 0.0, bad = 0.0;
-  for (long long s = s0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; s < s1; s += (long long)gridDim.x * blockDim.x) {
-    if (b.mask) {
-      const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
-      if (solid_at(b, x, y, z)) continue;
-    }
-    float t = 0.f, r = 0.f;
-#pragma unroll
-    for (int q = 0; q < Q; ++q) {
-      if constexpr (TWO) {
-        const float2 v = __ldcg(reinterpret_cast<const float2*>(buf) + (size_t)q * b.S + s);
-        t += v.x; r += v.y;
-      } else {
-        t += __ldcg(buf + (size_t)q * b.S + s);
-      }
-    }
-    if (!isfinite(t) || !isfinite(r)) { bad += 1.0; continue; }
-    if constexpr (TWO) { sr += (double)r; sb += (double)(1.0f + t) - (double)r; }
-    else sr += (double)(1.0f + t);
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    sr += __shfl_down_sync(0xffffffffu, sr, o);
-    sb += __shfl_down_sync(0xffffffffu, sb, o);
-    bad += __shfl_down_sync(0xffffffffu, bad, o);
-  }
-  __shared__ double red[3][8];
-  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
-  if (lane == 0) { red[0][wp] = sr; red[1][wp] = sb; red[2][wp] = bad; }
-  __syncthreads();
-  if (threadIdx.x < 3) {
-    double v = 0.0;
-    for (int i = 0; i < 8; ++i) v += red[threadIdx.x][i];
-    if (v != 0.0) atomicAdd(out + threadIdx.x, v);
-  }
 }
 
 // does the byte mask hold a moving wall group?  out[0] |= 1

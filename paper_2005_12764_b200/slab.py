@@ -89,10 +89,12 @@ class Slab:
         self.buf = None
 
     @classmethod
-    def from_workload(cls, w, z0, nz, storage="ab", zc=0):
-        """The slab [z0, z0 + nz) of a workloads.Workload (its fields are sliced by init_from)."""
+    def from_workload(cls, w, z0, nz, storage="ab", zc=0, nz_global=None):
+        """The slab [z0, z0 + nz) of a workloads.Workload (its fields are sliced by init_from).
+        nz_global > w.nz: the box is the workload repeated along z (weak scaling: every rank holds
+        one period; the mask and the fields wrap with period w.nz)."""
         from . import workloads
-        return cls(w.nx, w.ny, nz, z0, w.nz, *w.params, storage=storage, solid_global=w.solid, g=w.g,
+        return cls(w.nx, w.ny, nz, z0, nz_global or w.nz, *w.params, storage=storage, solid_global=w.solid, g=w.g,
                    phi_c=w.phi_c, configure=lambda sim: workloads.configure_walls(sim, w), zc=zc)
 
     def init(self, rho_r, rho_b, u):
@@ -107,7 +109,9 @@ class Slab:
         self.halo_bytes = (pop, phi)
 
     def init_from(self, w):
-        sl = slice(self.z0, self.z0 + self.nz)
+        z0 = self.z0 % w.nz                      # a box taller than the workload repeats it along z
+        assert z0 + self.nz <= w.nz
+        sl = slice(z0, z0 + self.nz)
         self.init(np.ascontiguousarray(w.rho_r[sl]), None if w.rho_b is None else np.ascontiguousarray(w.rho_b[sl]),
                   np.ascontiguousarray(w.u[:, sl]))
 

@@ -56,6 +56,9 @@ def test_slabs_equal_undivided_box_bitwise(lbmod, slabmod, name, cuts, zc, stora
     ring = slabmod.LocalRing(w, cuts, storage, zc=zc)
     ring.init()
     _same_bits(ring, sim)
+    m_ring = [sum(s.sim.check_state()[k] for s in ring.slabs) for k in (0, 1)]
+    m_box = sim.check_state()
+    assert abs(m_ring[0] - m_box[0]) / m_box[0] < 1e-12 and abs(m_ring[1] - m_box[1]) / m_box[1] < 1e-12    # at t = 0 too
     done = 0
     for n in (1, 2, 3, 5):
         ring.step(n - done); sim.step(n - done)
