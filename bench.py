@@ -33,6 +33,7 @@ METRIC = "GLUPS (two-component D3Q19 site updates/s)"
 BYTES_PER_UPDATE = {True: 2 * 2 * 19 * 4, False: 2 * 19 * 4}   # two-component 304 B, single 152 B
 FALLBACK_HBM_GBS = 6650.0
 NOMINAL_HBM_GBS = 8000.0     # north_star's "~8 TB/s"; every fraction is reported against the measured copy rate and against this
+TUNE = {}                # --tune
 MODEL = ["cg", 0.0]      # --model: colour gradient (north_star) or the paper's Shan-Chen coupling, and its G_C
 
 
@@ -281,6 +282,8 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
         sim = lb.from_workload(w, storage=storage)
         if MODEL[0] == "sc":
             sim.set_model("sc", MODEL[1])
+        if TUNE:
+            sim.set_tuning(**TUNE)
     sim.init(d_rr, d_rb, d_u)
     mass0 = sim.check_state()
     sim.set_profiling(7)      # every 7th step (odd, so that both AA parities are sampled) is timed kernel by kernel (CUDA events on the stream)
@@ -450,6 +453,7 @@ def main(argv=None):
     ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune", default="", help="lb_set_tuning settings for experiments, e.g. fixup=0,zc=12")
     ap.add_argument("--slabs", action="store_true", help="run the z-slab driver also at N = 1 (the rank is then its own neighbour)")
     ap.add_argument("--configs", default=None, choices=["all", "none"], help="all = also measure C3 A/B, C4 A/B, C5 AA and C2 and report them under 'configs' (default when --workload is left at c5)")
     ap.add_argument("--model", default="cg", choices=["cg", "sc"], help="cg = colour gradient (north_star), sc = Shan-Chen + exact difference (Eq. 5-10 of the paper)")
@@ -460,6 +464,7 @@ def main(argv=None):
     if args.configs is None:
         args.configs = "all" if (args.workload == "c5" and args.storage == "ab") else "none"
     MODEL[0], MODEL[1] = args.model, args.gc
+    TUNE.update({k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(",") if kv)})
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

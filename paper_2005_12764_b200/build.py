@@ -38,7 +38,9 @@ def stale():
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         tmp = LIB + ".tmp%d" % os.getpid()
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        # LB_BUILD_SUBSET=1: developer builds that compile a fifth of the k_fused instantiations (lb_api.cu)
+        subset = ["-DLB_BUILD_SUBSET"] if os.environ.get("LB_BUILD_SUBSET") == "1" else []
+        cmd = [_nvcc()] + NVCC_FLAGS + subset + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)

@@ -318,6 +318,13 @@ void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
   // moving walls (WALLS == 2, a rare configuration) are built for the force variants only
   const bool g = p.has_g || (MODE != MODE_AB && !HAS_NC) || WALLS == 2;
   const bool edm = p.edm && (HAS_NC || p.has_g);    // no force, no source: nothing to choose
+#ifdef LB_BUILD_SUBSET      // developer builds (LB_BUILD_SUBSET=1 python -m ...build): Guo forcing, walls at rest or none
+  if (edm || WALLS == 2) { h->err = "not in this developer build (LB_BUILD_SUBSET)"; return; }
+  if constexpr (WALLS != 2) {
+    if (g) launch_fused_t<MODE, WALLS, HAS_NC, 1>(h, p, grid);
+    else launch_fused_t<MODE, WALLS, HAS_NC, 0>(h, p, grid);
+  }
+#else
   if (edm) {
     if (g) launch_fused_t<MODE, WALLS, HAS_NC, 3>(h, p, grid);
     else if constexpr (HAS_NC && WALLS != 2) launch_fused_t<MODE, WALLS, HAS_NC, 2>(h, p, grid);
@@ -325,6 +332,7 @@ void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
     if (g) launch_fused_t<MODE, WALLS, HAS_NC, 1>(h, p, grid);
     else if constexpr (WALLS != 2) launch_fused_t<MODE, WALLS, HAS_NC, 0>(h, p, grid);
   }
+#endif
 }
 template <int MODE, int WALLS, int FMODE>
 void launch_fused_sc(lb_handle h, const StepParams& p, dim3 grid) {
@@ -339,6 +347,7 @@ void launch_fused_sc(lb_handle h, const StepParams& p, dim3 grid) {
 }
 template <int MODE>
 void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
+#ifndef LB_BUILD_SUBSET
   if (h->model == 1) {      // Shan-Chen: no near contact; the only force flag is the body force
     const bool g = p.has_g || MODE != MODE_AB;    // AA: the body-force instantiation, as in launch_fused_g
     if (p.has_moving) launch_fused_sc<MODE, 2, 1>(h, p, grid);
@@ -346,6 +355,7 @@ void launch_fused(lb_handle h, const StepParams& p, dim3 grid) {
     else { if (g) launch_fused_sc<MODE, 0, 1>(h, p, grid); else launch_fused_sc<MODE, 0, 0>(h, p, grid); }
     return;
   }
+#endif
   const bool nc = h->par.A_nc != 0.f;
   if (p.has_moving) {
     if (nc) launch_fused_g<MODE, 2, true>(h, p, grid);
