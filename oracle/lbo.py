@@ -13,7 +13,11 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lbo.cpp")
-_LIB = os.path.join(_HERE, "liblbo.so")
+# LBO_SANITIZE=1: the oracle is built with -fsanitize=address,undefined into its own library (run the CPU
+# tests as  LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 LBO_SANITIZE=1
+# python -m pytest tests -m "not gpu";  DESIGN.md section 7 records the outcome)
+_SAN = os.environ.get("LBO_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "liblbo_san.so" if _SAN else "liblbo.so")
 _lib = None
 
 
@@ -21,8 +25,9 @@ def build(force: bool = False) -> str:
     """Compile oracle/lbo.cpp to oracle/liblbo.so with g++ -O2 -fopenmp (no GPU needed)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp%d" % os.getpid()
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if _SAN else ["-O2"]
         subprocess.check_call(
-            ["g++", "-std=c++17", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC])
+            ["g++", "-std=c++17"] + flags + ["-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
 
