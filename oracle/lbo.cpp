@@ -30,7 +30,11 @@
 // P14 exact-difference forcing, P15 Couette flow between sliding walls (G28), P16 colour-exchange
 // symmetry of the symmetric probe (G29), P17 wetting: symmetry, neutrality and monotone contact
 // angle (G30), P18 open boundaries: plug flow fixed point, pressure-driven Poiseuille, mass balance
-// (G31); SC1-SC5 for the second model.
+// (G31); SC1-SC5 for the second model; P20 interface width of the recolouring operator (closed form).
+// Rigid particles (the paper's section 6; readings G32-G37 further down): PC1 exact
+// momentum of fluid + particles, PC2 no force in a fluid at rest, PC3 leapfrog / quaternion closed
+// forms, PC4 Stokes drag (Hasimoto), PC5 torque on a spinning sphere, PC6 pair force
+// (tests/test_oracle_colloids.py).
 // PARITY UNPINNED against the paper (pinned only against DESIGN.md's reading): the discrete
 // contact search (G10), H_MAX, the wall rule for phi (G8, G30), the guard eps (G7).
 //
@@ -79,10 +83,11 @@ struct Oracle {
   bool two = true;
   bool inited = false;
   bool any_solid = false;
-  std::vector<uint8_t> solid;            // S, 0 = fluid, 1 = wall at rest, 2 / 3 / 4 = walls moving with uw[2] / uw[3] / uw[4]
-  double uw[5][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // wall velocities by group (G28)
-  int wtype[5] = {0, 0, 0, 0, 0};        // group 2 / 3 / 4: 0 = moving wall, 1 = velocity inlet, 2 = reservoir, 3 = pressure outlet (G31)
-  double wrho[5][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}};             // prescribed rho_r, rho_b of an inlet / outlet
+  std::vector<uint8_t> solid;            // S, 0 = fluid, 1 = wall at rest, 2 / 3 / 4 = walls moving with uw[2] / uw[3] / uw[4],
+                                         // 5 = node inside a rigid particle (NEXT-4; pid[s] says which)
+  double uw[6][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // wall velocities by group (G28); [5] stays 0
+  int wtype[6] = {0, 0, 0, 0, 0, 0};     // group 2 / 3 / 4: 0 = moving wall, 1 = velocity inlet, 2 = reservoir, 3 = pressure outlet (G31)
+  double wrho[6][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}, {0, 0}};     // prescribed rho_r, rho_b of an inlet / outlet
   std::vector<double> uex, uey, uez;     // velocity that entered f^eq in the last collision (outlet rule, G31)
   std::vector<double> f[2], fpost[2];    // [k][site*19 + i], pre- and post-collision
   std::vector<double> rho_r, rho_b, phi; // per site (S1)
@@ -92,6 +97,19 @@ struct Oracle {
   std::vector<int> hcontact;             // contact distance found by the probe, 0 = none
   std::vector<double> margin;            // smallest margin of any discrete decision (G12)
   std::string err;
+  // ---- rigid spherical particles (the paper's section 6; readings G32-G37 below)
+  struct Particle {
+    double r[3], u[3], w[3], q[4];   // centre, velocity, angular velocity, orientation quaternion (w, x, y, z)
+    double R, mass, inertia;         // radius, m_p, I_p = 2/5 m_p R^2 (solid sphere)
+    double F[3], T[3];               // force and torque from the fluid links of the last step
+    double Fext[3], Text[3];         // constant external force / torque
+    double Fpp[3];                   // inter-particle force of the last step
+  };
+  std::vector<Particle> parts;
+  std::vector<int> pid;              // S, particle index of a particle node, else -1
+  int p_mobile = 1;                  // 0: particles are held (infinite inertia): links exchange momentum, nothing moves
+  double p_K = 0.0, p_hc = 0.0;      // soft repulsion K (h_c - h)^(3/2) for gaps h < h_c (G37)
+  int p_lub = 0;                     // 1: normal lubrication force for gaps h < h_c (G37)
 
   size_t idx(int x, int y, int z) const { return (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * (size_t)z); }
   static int wrap(int a, int n) {  // periodic image; loops so that boxes with n = 1 work (G22)
@@ -410,6 +428,288 @@ void collide_sc_at(Oracle& o, int x, int y, int z) {
   }
 }
 
+// ---- Rigid particles: the paper's section 6 ------------------------------
+// "colloidal particles are represented as rigid spheres of radius R, moving under the effect of a
+// total force F_p and torque T_p ... Newton's equations of motion (Eq. 15) ... solved by a leapfrog
+// approach, using quaternion algebra for the rotational component".  How the
+// fluid acts on a particle is only cited (refs [61, 62], Ladd).  Readings (G32-G37):
+//  G32 nodes: a lattice node x belongs to particle p if |x - r_p| < R_p (minimum image).  A link
+//      from a fluid node s along c_j into such a node meets the surface at its midpoint
+//      x_b = s + c_j / 2, which moves with u_b = u_p + w_p x (x_b - r_p).
+//  G33 link rule, applied right after the collision with the node map of time t: the population
+//      that leaves s towards the particle is stored as what comes back,
+//      g^k_j(s) = f^k*_j(s) - 6 w_j rho^k(s) (c_j . u_b)   (half-way bounce-back at a moving wall, as
+//      G28; rho^k the component's density at s), and the particle receives the momentum
+//      dP = sum_k (f^k*_j + g^k_j) c_j and the torque (x_b - r_p) x dP.
+//  G35 Eq. 15 by leapfrog: u_p += (F_p + F_pp + F_ext)/m_p, r_p += u_p, w_p += (T_p + T_ext)/I_p,
+//      q <- dq(w_p) q with dq the rotation by the angle |w_p| about w_p (unit time step).
+//  G36 node changes after the move.  A node that leaves the particle is filled with the equilibrium
+//      (Eq. 2) at the mean densities of its fluid neighbours and the surface velocity there; what it
+//      holds is taken from the particle's momentum.  A node that enters the particle gives its
+//      populations' momentum to the particle.  Links whose far end changed are put right so that
+//      momentum is conserved exactly: a link into a node that is fluid now gets its population
+//      f^k*_j back (the exchange of G33 is undone); a link into a node that is solid now is
+//      reflected by G33 with the particle's new state.  Streaming then uses the new node map.
+//  G37 particle-particle forces ("including the lubrication term", forms not given): for a
+//      gap h = |r_ij| - R_i - R_j < h_c a repulsion K (h_c - h)^(3/2) along the line of centres and,
+//      if switched on, the normal lubrication force -6 pi mu R_eff^2 (1/h - 1/h_c) (u_ij . n) n with
+//      R_eff = R_i R_j / (R_i + R_j), mu = rho_0 nu, rho_0 = 1, nu from tau_r; h is floored at 0.1.
+double min_image(double d, int n) { return d - n * std::floor(d / n + 0.5); }
+
+void cross(const double a[3], const double b[3], double c[3]) {
+  c[0] = a[1] * b[2] - a[2] * b[1];
+  c[1] = a[2] * b[0] - a[0] * b[2];
+  c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+bool inside_particle(const Oracle& o, const Oracle::Particle& P, int x, int y, int z) {
+  const double d[3] = {min_image(x - P.r[0], o.nx), min_image(y - P.r[1], o.ny), min_image(z - P.r[2], o.nz)};
+  return d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < P.R * P.R;
+}
+
+// loop over the lattice nodes of the box [r - R - m, r + R + m] (wrapped)
+template <class Fn>
+void for_box(const Oracle& o, const double r[3], double reach, Fn fn) {
+  int lo[3], hi[3];
+  const int n[3] = {o.nx, o.ny, o.nz};
+  for (int a = 0; a < 3; ++a) {
+    lo[a] = (int)std::floor(r[a] - reach);
+    hi[a] = (int)std::ceil(r[a] + reach);
+    if (hi[a] - lo[a] + 1 > n[a]) { lo[a] = 0; hi[a] = n[a] - 1; }   // never visit a node twice
+  }
+  for (int z = lo[2]; z <= hi[2]; ++z)
+    for (int y = lo[1]; y <= hi[1]; ++y)
+      for (int x = lo[0]; x <= hi[0]; ++x) fn(Oracle::wrap(x, o.nx), Oracle::wrap(y, o.ny), Oracle::wrap(z, o.nz));
+}
+
+// G32: mark the particle nodes (solid = 5, pid = p).  Walls keep their nodes.
+void rasterize(Oracle& o) {
+  for (size_t s = 0; s < o.S; ++s) {
+    if (o.solid[s] == 5) o.solid[s] = 0;
+    o.pid[s] = -1;
+  }
+  for (size_t p = 0; p < o.parts.size(); ++p)
+    for_box(o, o.parts[p].r, o.parts[p].R + 1.0, [&](int x, int y, int z) {
+      const size_t s = o.idx(x, y, z);
+      if (o.solid[s] == 0 && inside_particle(o, o.parts[p], x, y, z)) { o.solid[s] = 5; o.pid[s] = (int)p; }
+    });
+}
+
+// surface velocity of particle P at the point r_p + rel
+void surface_velocity(const Oracle::Particle& P, const double rel[3], double ub[3]) {
+  double wxr[3];
+  cross(P.w, rel, wxr);
+  for (int a = 0; a < 3; ++a) ub[a] = P.u[a] + wxr[a];
+}
+
+// G33 on one link: fluid node s = (x, y, z), direction j into a node of particle P (state P).
+// Replaces fpost_j(s) by the reflected value and returns the momentum dP given to the particle.
+void reflect_link(Oracle& o, const Oracle::Particle& P, int x, int y, int z, int j, double dP[3], double rel[3]) {
+  const size_t s = o.idx(x, y, z);
+  rel[0] = min_image(x - P.r[0], o.nx) + 0.5 * CX[j];
+  rel[1] = min_image(y - P.r[1], o.ny) + 0.5 * CY[j];
+  rel[2] = min_image(z - P.r[2], o.nz) + 0.5 * CZ[j];
+  double ub[3];
+  surface_velocity(P, rel, ub);
+  const double cu = CX[j] * ub[0] + CY[j] * ub[1] + CZ[j] * ub[2];
+  double tot = 0.0;
+  for (int k = 0; k < (o.two ? 2 : 1); ++k) {
+    const double rk = k == 0 ? o.rho_r[s] : o.rho_b[s];
+    const double fp = o.fpost[k][s * Q + j];
+    const double g = fp - 6.0 * W[j] * rk * cu;
+    o.fpost[k][s * Q + j] = g;
+    tot += fp + g;
+  }
+  dP[0] = tot * CX[j]; dP[1] = tot * CY[j]; dP[2] = tot * CZ[j];
+}
+
+// G33 for every link into a particle node, with the node map and the particle state of time t
+void particle_links(Oracle& o) {
+  for (size_t p = 0; p < o.parts.size(); ++p) {
+    Oracle::Particle& P = o.parts[p];
+    for (int a = 0; a < 3; ++a) P.F[a] = P.T[a] = 0.0;
+    for_box(o, P.r, P.R + 2.0, [&](int x, int y, int z) {
+      const size_t s = o.idx(x, y, z);
+      if (o.solid[s]) return;
+      for (int j = 1; j < Q; ++j) {
+        const size_t n = o.nbr(x, y, z, CX[j], CY[j], CZ[j]);
+        if (o.solid[n] != 5 || o.pid[n] != (int)p) continue;
+        double dP[3], rel[3], t[3];
+        reflect_link(o, P, x, y, z, j, dP, rel);
+        cross(rel, dP, t);
+        for (int a = 0; a < 3; ++a) { P.F[a] += dP[a]; P.T[a] += t[a]; }
+      }
+    });
+  }
+}
+
+// G37
+void interparticle(Oracle& o) {
+  const size_t N = o.parts.size();
+  for (size_t p = 0; p < N; ++p) for (int a = 0; a < 3; ++a) o.parts[p].Fpp[a] = 0.0;
+  if (o.p_hc <= 0.0) return;
+  const double mu = (o.tau_r - 0.5) / 3.0;   // rho_0 nu with rho_0 = 1
+  for (size_t p = 0; p < N; ++p)
+    for (size_t q = p + 1; q < N; ++q) {
+      Oracle::Particle &A = o.parts[p], &Bq = o.parts[q];
+      const double d[3] = {min_image(A.r[0] - Bq.r[0], o.nx), min_image(A.r[1] - Bq.r[1], o.ny), min_image(A.r[2] - Bq.r[2], o.nz)};
+      const double dist = std::sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+      double h = dist - A.R - Bq.R;
+      if (h >= o.p_hc) continue;
+      const double n[3] = {d[0] / dist, d[1] / dist, d[2] / dist};   // from q to p
+      double f = o.p_K * std::pow(o.p_hc - h, 1.5);
+      if (o.p_lub) {
+        const double hh = h < 0.1 ? 0.1 : h;
+        const double Reff = A.R * Bq.R / (A.R + Bq.R);
+        const double un = (A.u[0] - Bq.u[0]) * n[0] + (A.u[1] - Bq.u[1]) * n[1] + (A.u[2] - Bq.u[2]) * n[2];
+        f += -6.0 * M_PI * mu * Reff * Reff * (1.0 / hh - 1.0 / o.p_hc) * un;
+      }
+      for (int a = 0; a < 3; ++a) { A.Fpp[a] += f * n[a]; Bq.Fpp[a] -= f * n[a]; }
+    }
+}
+
+// G35
+void integrate(Oracle& o) {
+  const int n[3] = {o.nx, o.ny, o.nz};
+  for (auto& P : o.parts) {
+    for (int a = 0; a < 3; ++a) {
+      P.u[a] += (P.F[a] + P.Fpp[a] + P.Fext[a]) / P.mass;
+      P.w[a] += (P.T[a] + P.Text[a]) / P.inertia;
+      P.r[a] += P.u[a];
+      P.r[a] -= n[a] * std::floor(P.r[a] / n[a]);
+    }
+    const double th = std::sqrt(P.w[0] * P.w[0] + P.w[1] * P.w[1] + P.w[2] * P.w[2]);
+    if (th > 0.0) {
+      const double sh = std::sin(0.5 * th) / th, ch = std::cos(0.5 * th);
+      const double d[4] = {ch, sh * P.w[0], sh * P.w[1], sh * P.w[2]};
+      const double* q = P.q;
+      double r[4] = {d[0] * q[0] - d[1] * q[1] - d[2] * q[2] - d[3] * q[3],
+                     d[0] * q[1] + d[1] * q[0] + d[2] * q[3] - d[3] * q[2],
+                     d[0] * q[2] - d[1] * q[3] + d[2] * q[0] + d[3] * q[1],
+                     d[0] * q[3] + d[1] * q[2] - d[2] * q[1] + d[3] * q[0]};
+      const double nr = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + r[3] * r[3]);
+      for (int a = 0; a < 4; ++a) P.q[a] = r[a] / nr;
+    }
+  }
+}
+
+// G36: node changes of particle p after its move from `old` to the current state
+void remap_particle(Oracle& o, size_t p, const Oracle::Particle& old) {
+  Oracle::Particle& P = o.parts[p];
+  struct Node { int x, y, z; };
+  std::vector<Node> covered, uncovered;
+  for_box(o, P.r, P.R + 2.0, [&](int x, int y, int z) {
+    const size_t s = o.idx(x, y, z);
+    const bool was = o.solid[s] == 5 && o.pid[s] == (int)p;
+    const bool now = inside_particle(o, P, x, y, z) && (was || o.solid[s] == 0);
+    if (was && !now) uncovered.push_back({x, y, z});
+    if (!was && now) covered.push_back({x, y, z});
+  });
+  const int nk = o.two ? 2 : 1;
+  double dU[3] = {0, 0, 0}, dL[3] = {0, 0, 0};     // impulses: momentum and angular momentum
+  auto is_new_cover = [&](size_t s) {
+    for (const Node& c : covered) if (o.idx(c.x, c.y, c.z) == s) return true;
+    return false;
+  };
+  auto give = [&](const double mom[3], const double rel[3], double sign) {
+    double t[3];
+    cross(rel, mom, t);
+    for (int a = 0; a < 3; ++a) { dU[a] += sign * mom[a]; dL[a] += sign * t[a]; }
+  };
+  // nodes that leave the particle
+  for (const Node& c : uncovered) {
+    const size_t s = o.idx(c.x, c.y, c.z);
+    double rk[2] = {0, 0};
+    int cnt = 0;
+    for (int j = 1; j < Q; ++j) {
+      const size_t m = o.nbr(c.x, c.y, c.z, CX[j], CY[j], CZ[j]);
+      if (o.solid[m] || is_new_cover(m)) continue;
+      rk[0] += o.rho_r[m]; rk[1] += o.rho_b[m];
+      ++cnt;
+    }
+    if (cnt) { rk[0] /= cnt; rk[1] /= cnt; }
+    else { rk[0] = o.two ? 0.5 : 1.0; rk[1] = o.two ? 0.5 : 0.0; }
+    const double rel[3] = {min_image(c.x - P.r[0], o.nx), min_image(c.y - P.r[1], o.ny), min_image(c.z - P.r[2], o.nz)};
+    double ub[3];
+    surface_velocity(P, rel, ub);
+    for (int k = 0; k < nk; ++k)
+      for (int i = 0; i < Q; ++i) o.fpost[k][s * Q + i] = feq(i, rk[k], ub[0], ub[1], ub[2]);
+    const double rho = rk[0] + (o.two ? rk[1] : 0.0);
+    const double mom[3] = {rho * ub[0], rho * ub[1], rho * ub[2]};
+    give(mom, rel, -1.0);
+    o.rho_r[s] = rk[0]; o.rho_b[s] = o.two ? rk[1] : 0.0;      // the new node's densities, for the link rule
+    // the new node's own links into the particle (as it stands now) are reflected by G33
+    for (int j = 1; j < Q; ++j) {
+      const int mx = Oracle::wrap(c.x + CX[j], o.nx), my = Oracle::wrap(c.y + CY[j], o.ny), mz = Oracle::wrap(c.z + CZ[j], o.nz);
+      if (!inside_particle(o, P, mx, my, mz)) continue;
+      const size_t m = o.idx(mx, my, mz);
+      if (o.solid[m] != 0 && !(o.solid[m] == 5 && o.pid[m] == (int)p)) continue;   // a wall's or another particle's node
+      double dP[3], relb[3];
+      reflect_link(o, P, c.x, c.y, c.z, j, dP, relb);
+      give(dP, relb, +1.0);
+    }
+    // links of fluid neighbours into this node: the exchange of G33 is undone
+    for (int j = 1; j < Q; ++j) {
+      const int sx = Oracle::wrap(c.x - CX[j], o.nx), sy = Oracle::wrap(c.y - CY[j], o.ny), sz = Oracle::wrap(c.z - CZ[j], o.nz);
+      const size_t t = o.idx(sx, sy, sz);
+      if (o.solid[t] || is_new_cover(t)) continue;
+      double relb[3] = {min_image(sx - old.r[0], o.nx) + 0.5 * CX[j], min_image(sy - old.r[1], o.ny) + 0.5 * CY[j],
+                        min_image(sz - old.r[2], o.nz) + 0.5 * CZ[j]};
+      double ubo[3];
+      surface_velocity(old, relb, ubo);
+      const double cu = CX[j] * ubo[0] + CY[j] * ubo[1] + CZ[j] * ubo[2];
+      double tot = 0.0;
+      for (int k = 0; k < nk; ++k) {
+        const double rkk = k == 0 ? o.rho_r[t] : o.rho_b[t];
+        const double g = o.fpost[k][t * Q + j];
+        const double fp = g + 6.0 * W[j] * rkk * cu;
+        o.fpost[k][t * Q + j] = fp;
+        tot += fp + g;
+      }
+      const double dP[3] = {tot * CX[j], tot * CY[j], tot * CZ[j]};
+      give(dP, relb, -1.0);
+    }
+  }
+  // nodes that enter the particle
+  for (const Node& c : covered) {
+    const size_t s = o.idx(c.x, c.y, c.z);
+    // What the node holds: fpost_i is the population that would be at the neighbour along c_i after
+    // streaming, or, where that neighbour is solid, back at this node moving along -c_i (for a link
+    // into the particle the stored value is already the reflected one, G33).
+    double mom[3] = {0, 0, 0};
+    for (int i = 0; i < Q; ++i) {
+      const double sgn = o.solid[o.nbr(c.x, c.y, c.z, CX[i], CY[i], CZ[i])] ? -1.0 : 1.0;
+      for (int k = 0; k < nk; ++k) {
+        const double v = sgn * o.fpost[k][s * Q + i];
+        mom[0] += v * CX[i]; mom[1] += v * CY[i]; mom[2] += v * CZ[i];
+      }
+    }
+    const double rel[3] = {min_image(c.x - P.r[0], o.nx), min_image(c.y - P.r[1], o.ny), min_image(c.z - P.r[2], o.nz)};
+    give(mom, rel, +1.0);
+    for (int j = 1; j < Q; ++j) {
+      const int sx = Oracle::wrap(c.x - CX[j], o.nx), sy = Oracle::wrap(c.y - CY[j], o.ny), sz = Oracle::wrap(c.z - CZ[j], o.nz);
+      const size_t t = o.idx(sx, sy, sz);
+      if (o.solid[t] || is_new_cover(t)) continue;
+      double dP[3], relb[3];
+      reflect_link(o, P, sx, sy, sz, j, dP, relb);
+      give(dP, relb, +1.0);
+    }
+  }
+  for (int a = 0; a < 3; ++a) { P.u[a] += dU[a] / P.mass; P.w[a] += dL[a] / P.inertia; }
+  for (const Node& c : uncovered) { const size_t s = o.idx(c.x, c.y, c.z); o.solid[s] = 0; o.pid[s] = -1; }
+  for (const Node& c : covered) { const size_t s = o.idx(c.x, c.y, c.z); o.solid[s] = 5; o.pid[s] = (int)p; }
+}
+
+// the particle part of a step, between collision and streaming
+void particle_step(Oracle& o) {
+  particle_links(o);
+  if (!o.p_mobile) return;
+  interparticle(o);
+  std::vector<Oracle::Particle> old = o.parts;
+  integrate(o);
+  for (size_t p = 0; p < o.parts.size(); ++p) remap_particle(o, p, old[p]);
+}
+
 void one_step(Oracle& o) {
   moments(o);
   if (o.model == 1) {
@@ -426,6 +726,7 @@ void one_step(Oracle& o) {
     for (int y = 0; y < o.ny; ++y)
       for (int x = 0; x < o.nx; ++x)
         if (!o.solid[o.idx(x, y, z)]) collide_at(o, x, y, z);
+  if (!o.parts.empty()) particle_step(o);   // links (G33), Eq. 15 (G35), node changes (G36)
   stream(o);
 }
 
@@ -480,6 +781,7 @@ int lbo_create(int nx, int ny, int nz, const double* params, void** out) {
                     &o->Gx, &o->Gy, &o->Gz, &o->margin, &o->uex, &o->uey, &o->uez})
       v->assign(o->S, 0.0);
     o->hcontact.assign(o->S, 0);
+    o->pid.assign(o->S, -1);
   } catch (...) {
     delete o;
     return LBO_ENOMEM;
@@ -496,6 +798,7 @@ int lbo_set_geometry(void* h, const uint8_t* mask) {
   if (o->inited) return LBO_ESTATE;
   o->any_solid = false;
   for (size_t s = 0; s < o->S; ++s) {
+    o->pid[s] = -1;
     o->solid[s] = mask ? (mask[s] > 4 ? 1 : mask[s]) : 0;   // 0 fluid, 1 wall at rest, 2 / 3 / 4 wall groups (three: the flow
                                                             // focuser has two kinds of inlet and an outlet; G31)
     o->any_solid |= o->solid[s] != 0;
@@ -599,6 +902,7 @@ int lbo_init(void* h, const double* rho_r, const double* rho_b, const double* u)
   } catch (...) {
     return LBO_ENOMEM;
   }
+  if (!o->parts.empty()) rasterize(*o);
   for (size_t s = 0; s < S; ++s) {
     if (o->solid[s]) continue;
     for (int i = 0; i < Q; ++i) {
@@ -672,6 +976,73 @@ int lbo_get_fields(void* h, double* phi, double* G, double* F, int* hcontact, do
     if (F) { F[s] = o->Fx[s]; F[S + s] = o->Fy[s]; F[2 * S + s] = o->Fz[s]; }
     if (hcontact) hcontact[s] = o->hcontact[s];
     if (margin) margin[s] = o->margin[s];
+  }
+  return LBO_OK;
+}
+
+// ---- rigid particles.  state = n x 15 doubles: r[3], u[3], w[3], q[4], R, mass.
+// Must precede lbo_init (the particle nodes hold no fluid).  Colour-gradient or one component.
+int lbo_set_particles(void* h, int n, const double* state) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || n < 0 || (n > 0 && !state)) return LBO_EINVAL;
+  if (o->inited) return LBO_ESTATE;
+  if (o->model == 1) return LBO_EINVAL;
+  o->parts.clear();
+  for (int p = 0; p < n; ++p) {
+    const double* v = state + 15 * p;
+    Oracle::Particle P{};
+    for (int a = 0; a < 3; ++a) { P.r[a] = v[a]; P.u[a] = v[3 + a]; P.w[a] = v[6 + a]; }
+    for (int a = 0; a < 4; ++a) P.q[a] = v[9 + a];
+    P.R = v[13]; P.mass = v[14];
+    if (!(P.R > 0.0) || !(P.mass > 0.0)) return LBO_EINVAL;
+    P.inertia = 0.4 * P.mass * P.R * P.R;
+    o->parts.push_back(P);
+  }
+  return LBO_OK;
+}
+
+// state as in lbo_set_particles; force = n x 9 doubles: F[3], T[3] from the fluid links of the last
+// step, F_pp[3] from the other particles.  Either may be NULL.
+int lbo_get_particles(void* h, double* state, double* force) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  for (size_t p = 0; p < o->parts.size(); ++p) {
+    const Oracle::Particle& P = o->parts[p];
+    if (state) {
+      double* v = state + 15 * p;
+      for (int a = 0; a < 3; ++a) { v[a] = P.r[a]; v[3 + a] = P.u[a]; v[6 + a] = P.w[a]; }
+      for (int a = 0; a < 4; ++a) v[9 + a] = P.q[a];
+      v[13] = P.R; v[14] = P.mass;
+    }
+    if (force) for (int a = 0; a < 3; ++a) { force[9 * p + a] = P.F[a]; force[9 * p + 3 + a] = P.T[a]; force[9 * p + 6 + a] = P.Fpp[a]; }
+  }
+  return LBO_OK;
+}
+
+// mobile = 0 holds the particles in place (they still exchange momentum with the fluid);
+// K, h_c, lubrication: the particle-particle force of G37 (h_c <= 0: none)
+int lbo_set_particle_options(void* h, int mobile, double K, double h_c, int lubrication) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  o->p_mobile = mobile ? 1 : 0;
+  o->p_K = K; o->p_hc = h_c; o->p_lub = lubrication ? 1 : 0;
+  return LBO_OK;
+}
+
+int lbo_set_particle_force(void* h, int p, const double* F, const double* T) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o || p < 0 || p >= (int)o->parts.size()) return LBO_EINVAL;
+  for (int a = 0; a < 3; ++a) { o->parts[p].Fext[a] = F ? F[a] : 0.0; o->parts[p].Text[a] = T ? T[a] : 0.0; }
+  return LBO_OK;
+}
+
+// node map: 0 fluid, 1-4 walls, 5 particle; pid (may be NULL): particle index or -1
+int lbo_get_node_map(void* h, uint8_t* solid, int* pid) {
+  Oracle* o = static_cast<Oracle*>(h);
+  if (!o) return LBO_EINVAL;
+  for (size_t s = 0; s < o->S; ++s) {
+    if (solid) solid[s] = o->solid[s];
+    if (pid) pid[s] = o->pid[s];
   }
   return LBO_OK;
 }

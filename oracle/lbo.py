@@ -56,6 +56,11 @@ def _load():
         lib.lbo_get_populations.argtypes = [vp, C.c_int, dp]
         lib.lbo_set_populations.argtypes = [vp, C.c_int, dp]
         lib.lbo_get_fields.argtypes = [vp, dp, dp, dp, ip, dp]
+        lib.lbo_set_particles.argtypes = [vp, C.c_int, dp]
+        lib.lbo_get_particles.argtypes = [vp, dp, dp]
+        lib.lbo_set_particle_options.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
+        lib.lbo_set_particle_force.argtypes = [vp, C.c_int, dp, dp]
+        lib.lbo_get_node_map.argtypes = [vp, u8p, ip]
         lib.lbo_constants.argtypes = [ip, ip, dp, dp]
         lib.lbo_constants.restype = None
         _lib = lib
@@ -176,6 +181,33 @@ class Oracle:
     def set_populations(self, comp, f):
         ff = _f64(f).reshape((19,) + self.shape)
         self._ck(self.lib.lbo_set_populations(self.h, comp, _dptr(ff)), "lbo_set_populations")
+
+    # ---- rigid particles (G32-G37)
+    def set_particles(self, state):
+        """state [n, 15]: r[3], u[3], w[3], q[4] (w, x, y, z), R, mass.  Before init."""
+        st = np.ascontiguousarray(state, dtype=np.float64).reshape(-1, 15)
+        self.npart = len(st)
+        self._ck(self.lib.lbo_set_particles(self.h, self.npart, _dptr(st)), "lbo_set_particles")
+
+    def get_particles(self):
+        """(state [n, 15], force [n, 9]: F[3], T[3] from the fluid links of the last step, F_pp[3])."""
+        st = np.zeros((self.npart, 15))
+        fo = np.zeros((self.npart, 9))
+        self._ck(self.lib.lbo_get_particles(self.h, _dptr(st), _dptr(fo)), "lbo_get_particles")
+        return st, fo
+
+    def set_particle_options(self, mobile=True, K=0.0, h_c=0.0, lubrication=False):
+        self._ck(self.lib.lbo_set_particle_options(self.h, int(mobile), float(K), float(h_c), int(lubrication)), "lbo_set_particle_options")
+
+    def set_particle_force(self, p, F=(0, 0, 0), T=(0, 0, 0)):
+        f, t = np.array(F, np.float64), np.array(T, np.float64)
+        self._ck(self.lib.lbo_set_particle_force(self.h, int(p), _dptr(f), _dptr(t)), "lbo_set_particle_force")
+
+    def get_node_map(self):
+        sol = np.zeros(self.shape, np.uint8)
+        pid = np.zeros(self.shape, np.int32)
+        self._ck(self.lib.lbo_get_node_map(self.h, sol.ctypes.data_as(C.POINTER(C.c_uint8)), pid.ctypes.data_as(C.POINTER(C.c_int))), "lbo_get_node_map")
+        return sol, pid
 
     def get_fields(self):
         """dict(phi, G[3], F[3], h (contact distance, 0 = none), margin (G12))."""
