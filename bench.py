@@ -133,7 +133,7 @@ def config_of(w, storage, extra=None):
     if w.rho_b is not None and w.A_nc != 0.0 and w.A > 0.0:
         # N_c = A dx / sigma with sigma = (4/9) A tau of the colour-gradient perturbation (G5)
         c["N_c"] = w.A_nc / ((4.0 / 9.0) * w.A * w.tau_r)
-    c.update(w.info)
+    c.update({k: v for k, v in w.info.items() if k != "particles"})     # (the particle array stays out of the JSON line)
     if extra:
         c.update(extra)
     return c
@@ -155,6 +155,8 @@ def oracle_sample_workload(name, budget_updates):
             return W.c1_droplet()
         if name.startswith("focuser"):
             return W.focuser(128, 48, 24, wd=10, wc=12, t=3, li=24, wo=10, lo=8, walls_z=True, A_nc=0.02)
+        if name.startswith("bijel"):
+            return W.bijel(n)
         return W.c3_spinodal(n)
     best = 32
     for n in (32, 48, 64, 96, 128, 160):
@@ -398,7 +400,7 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
 
 # The other rows of the table: measured in the same run, after the headline, and
 # reported under "configs" in the same JSON line.
-EXTRA_CONFIGS = [("c3", "ab"), ("c4", "ab"), ("c5", "aa"), ("c2", "ab")]
+EXTRA_CONFIGS = [("c3", "ab"), ("c4", "ab"), ("c5", "aa"), ("c2", "ab"), ("bijel", "ab")]
 
 
 def run_ours(args):
@@ -450,7 +452,7 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large"])
+    ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large", "bijel", "bijel-mini"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tune", default="", help="lb_set_tuning settings for experiments, e.g. fixup=0,zc=12")

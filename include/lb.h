@@ -224,6 +224,42 @@ int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi);
 int lb_slab_pack_phi(lb_handle h, void* send_lo, void* send_hi);
 int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi);
 
+/* ---- rigid spherical particles (the paper's section 6) --------------------
+ * "colloidal particles are represented as rigid spheres of radius R, moving under the effect of a
+ * total force F_p and torque T_p ... dr_p/dt = u_p, m_p du_p/dt = F_p, I_p dw_p/dt = T_p (Eq. 15) ...
+ * The force on each particle takes into account the interactions with the fluid and the
+ * inter-particle forces, including the lubrication term.  Hence, the equations of motion are solved
+ * by a leapfrog approach, using quaternion algebra for the rotational component".
+ * The paper gives no coupling rule; G32-G37 state the ones built: a lattice node within R of
+ * the centre is solid; a link from a fluid node into it is reflected half-way at a wall that moves
+ * with u_p + w_p x (x_b - r_p) (both components, as lb_set_wall_velocity does for plane walls) and
+ * hands its momentum change to the particle; leapfrog and quaternion update per step; nodes that
+ * leave a particle are filled with the equilibrium of their neighbours' mean densities, nodes that
+ * enter it give their momentum to it, so that the momentum of fluid + particles is conserved
+ * exactly; between particles a repulsion K (h_c - h)^(3/2) for gaps h < h_c and, if switched on,
+ * the normal lubrication force 6 pi mu R_eff^2 (1/h - 1/h_c) against the approach.
+ * lb_particle: centre r, velocity u, angular velocity w, orientation quaternion q = (w, x, y, z),
+ * radius R, mass (I_p = 2/5 m R^2); doubles, lattice units.
+ * lb_set_particles(h, n, p): HOST array of n particles; before lb_init (n = 0: none).  Needs A/B
+ * storage, the colour-gradient model or one component, no slab (lb_init returns LB_ESTATE
+ * otherwise); the "replicated data" scheme of PAPER.md:312-316 for several ranks is not built.
+ * The particle nodes hold no fluid: lb_init ignores its input there and lb_get_macros returns zeros.
+ * lb_set_particle_options: mobile = 0 holds the particles in place (they still exchange momentum with
+ * the fluid); K, h_c, lubrication: the pair force (h_c <= 0: none).  lb_set_particle_force: a constant
+ * external force and torque on particle i (either may be NULL); before lb_init.
+ * lb_get_particles(h, state, force): current states and, per particle, 9 doubles: force and torque
+ * from the fluid links of the last step, force from the other particles (HOST arrays, either may be
+ * NULL); synchronises; LB_ESTATE if a particle moved so fast that more than 384 of its nodes changed
+ * in one step.  With particles, phi is recomputed by the full sweep every step (the node map
+ * changes under the forwarded moments). */
+typedef struct {
+  double r[3], u[3], w[3], q[4], R, mass;
+} lb_particle;
+int lb_set_particles(lb_handle h, int n, const lb_particle* p);
+int lb_set_particle_options(lb_handle h, int mobile, double K, double h_c, int lubrication);
+int lb_set_particle_force(lb_handle h, int i, const double* F, const double* T);
+int lb_get_particles(lb_handle h, lb_particle* state, double* force);
+
 /* Tuning of lb_step.  key = "forward": 1 (default) = the fused kernel forwards the moments of the
  * next state and a light kernel turns them into phi; 0 = a full
  * phase-field sweep over the populations before every step (same phi to ~1e-8).  "zc": z planes

@@ -120,6 +120,16 @@ struct lb_handle_s {
   bool phi_current = false;  // phi array matches the current populations
   float* mom = nullptr;      // forwarded moments Md, Mt (2 x S floats), written by k_fused
   int forward = 1;           // 1 = phi(t+1) from forwarded moments (k_phase_fwd), 0 = full k_phase sweep
+  // rigid particles (NEXT-4)
+  int np = 0;
+  std::vector<PState> parts_host;   // what lb_set_particles gave (and the external forces)
+  PState* parts = nullptr;          // device
+  int* pid = nullptr;               // particle index per site, -1 elsewhere
+  uint32_t* mask_static = nullptr;  // the walls of lb_set_geometry alone (the live mask also holds the particle nodes)
+  bool user_solid = false, user_moving = false;
+  int* povf = nullptr;              // k_part_remap overflow flag
+  int p_mobile = 1, p_lub = 0;
+  double p_K = 0.0, p_hc = 0.0;
   int tune_zc = 0;           // z planes per CTA (0 = automatic)
   int sm_count = 0;          // SMs of the handle's device (0: not asked yet)
   double* chk = nullptr;     // state check (lb_check_state): {sum rho_r, sum rho_b, non-finite count}
@@ -142,6 +152,7 @@ struct lb_handle_s {
     b.S = S;
     b.mask = has_solid ? mask : nullptr;
     b.gmask = (has_solid && has_moving) ? mask + (size_t)b.nxw * ny * nza() : nullptr;
+    b.pid = np > 0 ? pid : nullptr;
     return b;
   }
   int planes() const { return two ? 2 * Q : Q; }
@@ -217,6 +228,7 @@ StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc, i
   p.z1 = z1 < 0 ? h->zhi() : z1;
   p.src = src; p.dst = dst; p.phi = h->phi;
   p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
+  p.parts = h->np > 0 ? h->parts : nullptr;
   const size_t plane = (h->two ? 2 : 1) * (size_t)h->S;   // floats per direction plane ({T, R} pairs or T)
   for (int q = 0; q < Q; ++q) {
     p.ps[q] = src ? src + (size_t)q * plane : nullptr;
@@ -319,10 +331,12 @@ void launch_fused_g(lb_handle h, const StepParams& p, dim3 grid) {
   const bool g = p.has_g || (MODE != MODE_AB && !HAS_NC) || WALLS == 2;
   const bool edm = p.edm && (HAS_NC || p.has_g);    // no force, no source: nothing to choose
 #ifdef LB_BUILD_SUBSET      // developer builds (LB_BUILD_SUBSET=1 python -m ...build): Guo forcing, walls at rest or none
-  if (edm || WALLS == 2) { h->err = "not in this developer build (LB_BUILD_SUBSET)"; return; }
+  if (edm) { h->err = "not in this developer build (LB_BUILD_SUBSET)"; return; }
   if constexpr (WALLS != 2) {
     if (g) launch_fused_t<MODE, WALLS, HAS_NC, 1>(h, p, grid);
     else launch_fused_t<MODE, WALLS, HAS_NC, 0>(h, p, grid);
+  } else {
+    launch_fused_t<MODE, 2, HAS_NC, 1>(h, p, grid);
   }
 #else
   if (edm) {
@@ -446,11 +460,37 @@ void flip(lb_handle h) {
   h->steps_done++;
 }
 
+PartParams make_part_params(lb_handle h) {
+  PartParams q;
+  memset(&q, 0, sizeof(q));
+  const size_t plane = (h->two ? 2 : 1) * (size_t)h->S;
+  for (int d = 0; d < Q; ++d) { q.ps[d] = h->cur_buf() + (size_t)d * plane; q.pd[d] = next_buf(h) + (size_t)d * plane; }
+  q.box = h->box();
+  q.mask = h->mask; q.pid = h->pid; q.parts = h->parts; q.np = h->np;
+  q.mobile = h->p_mobile; q.K = h->p_K; q.hc = h->p_hc; q.lub = h->p_lub;
+  q.mu = ((double)h->par.tau_r - 0.5) / 3.0;
+  q.overflow = h->povf;
+  return q;
+}
+
+// The particles' part of a step (Eq. 15), between the fused kernel, which applied
+// the link rule to what it stored, and the flip: momentum exchange, leapfrog, node changes.
+void run_particles(lb_handle h) {
+  const PartParams q = make_part_params(h);
+  if (h->two) k_part_force<true><<<h->np, 256, 0, h->stream>>>(q);
+  else k_part_force<false><<<h->np, 256, 0, h->stream>>>(q);
+  k_part_move<<<1, 128, 0, h->stream>>>(q);
+  if (h->two) k_part_remap<true><<<h->np, 256, 0, h->stream>>>(q);
+  else k_part_remap<false><<<h->np, 256, 0, h->stream>>>(q);
+  h->launches += 3;
+}
+
 // One whole step of a box that is periodic in z: K2 (+ K1f) or K2s
 void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
   launch_collide(h, h->zlo(), h->zhi());
   if (after_k2) cudaEventRecord(after_k2, h->stream);
-  if (h->two && h->forward) {
+  if (h->np > 0) run_particles(h);
+  if (h->two && h->forward && h->np == 0) {      // (with particles the node map changes: phi comes from the full sweep)
     launch_phase_forward(h, h->zlo(), h->zhi());
     flip(h);
     h->phi_current = true;
@@ -592,7 +632,7 @@ void lb_destroy(lb_handle h) {
   if (!h) return;
   DeviceGuard guard(h->device);
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
-  for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk}) dev_free(h->al, q);
+  for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk, (void*)h->parts, (void*)h->pid, (void*)h->mask_static, (void*)h->povf}) dev_free(h->al, q);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
   for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
   cudaGetLastError();
@@ -609,7 +649,7 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
   if (!h) return LB_EINVAL;
   DeviceGuard guard(h->device);
   if (h->inited) return fail(h, LB_ESTATE, "lb_set_geometry after lb_init");
-  if (!solid_mask) { h->has_solid = false; return LB_OK; }
+  if (!solid_mask) { h->has_solid = h->user_solid = false; h->has_moving = h->user_moving = false; return LB_OK; }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
     cudaGetLastError();
@@ -638,8 +678,8 @@ int lb_set_geometry(lb_handle h, const uint8_t* solid_mask) {
   cudaError_t e = cudaMemcpyAsync(&moving, flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);   // also: the staged copy dies with `in`
   if (e != cudaSuccess) return cuda_fail(h, e, "lb_set_geometry");
-  h->has_moving = moving != 0;
-  h->has_solid = true;
+  h->has_moving = h->user_moving = moving != 0;
+  h->has_solid = h->user_solid = true;
   return LB_OK;
 }
 
@@ -780,7 +820,112 @@ int allocate_state(lb_handle h, bool two) {
 
 }  // namespace
 
+namespace {
+
+// Particles at lb_init: the live mask = the walls + the particle nodes (G32), the particle index per
+// site, the particle states on the device.
+int init_particles(lb_handle h) {
+  if (h->storage != 0) return fail(h, LB_ESTATE, "particles need A/B storage");
+  if (h->model != 0) return fail(h, LB_ESTATE, "particles are built for the colour-gradient model and for one component");
+  if (h->gz) return fail(h, LB_ESTATE, "particles are not built for slabs");
+  const Box b0 = h->box();
+  const size_t nwords = (size_t)b0.nxw * h->ny * h->nza();
+  const size_t mb = (3 * nwords + 1) * 4;
+  cudaError_t e = cudaSuccess;
+  if (!h->mask) {
+    h->mask = static_cast<uint32_t*>(dev_alloc(h->al, mb));
+    if (!h->mask) return fail(h, LB_ENOMEM, "mask allocation failed");
+    h->bytes += mb;
+    e = cudaMemsetAsync(h->mask, 0, mb, h->stream);
+  }
+  if (!h->mask_static) {       // the walls alone, as lb_set_geometry left them (or none)
+    h->mask_static = static_cast<uint32_t*>(dev_alloc(h->al, nwords * 4));
+    if (!h->mask_static) return fail(h, LB_ENOMEM, "mask allocation failed");
+    h->bytes += nwords * 4;
+    if (e == cudaSuccess) e = h->user_solid ? cudaMemcpyAsync(h->mask_static, h->mask, nwords * 4, cudaMemcpyDeviceToDevice, h->stream)
+                                            : cudaMemsetAsync(h->mask_static, 0, nwords * 4, h->stream);
+  }
+  if (!h->pid) {
+    h->pid = static_cast<int*>(dev_alloc(h->al, (size_t)h->S * sizeof(int)));
+    h->povf = static_cast<int*>(dev_alloc(h->al, sizeof(int)));
+    if (!h->pid || !h->povf) return fail(h, LB_ENOMEM, "particle index allocation failed");
+    h->bytes += (size_t)h->S * sizeof(int) + sizeof(int);
+  }
+  if (!h->parts) {
+    h->parts = static_cast<PState*>(dev_alloc(h->al, (size_t)h->np * sizeof(PState)));
+    if (!h->parts) return fail(h, LB_ENOMEM, "particle state allocation failed");
+    h->bytes += (size_t)h->np * sizeof(PState);
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h->mask, h->mask_static, nwords * 4, cudaMemcpyDeviceToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->pid, 0xff, (size_t)h->S * sizeof(int), h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->povf, 0, sizeof(int), h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h->parts, h->parts_host.data(), (size_t)h->np * sizeof(PState), cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);      // parts_host is pageable
+  if (e != cudaSuccess) return cuda_fail(h, e, "particle set-up");
+  h->has_solid = true;
+  h->has_moving = true;        // the instantiations that look at what kind of solid a link meets
+  const PartParams q = make_part_params(h);
+  k_part_raster<<<h->np, 256, 0, h->stream>>>(q);
+  h->launches++;
+  return check_launch(h, "k_part_raster");
+}
+
+}  // namespace
+
 extern "C" {
+
+int lb_set_particles(lb_handle h, int n, const lb_particle* p) {
+  if (!h || n < 0 || (n > 0 && !p)) return fail(h, LB_EINVAL, "lb_set_particles: n >= 0 and a host array of n particles");
+  if (h->inited) return fail(h, LB_ESTATE, "lb_set_particles after lb_init");
+  h->parts_host.assign((size_t)n, PState{});
+  for (int i = 0; i < n; ++i) {
+    PState& P = h->parts_host[i];
+    for (int a = 0; a < 3; ++a) { P.r[a] = p[i].r[a]; P.u[a] = p[i].u[a]; P.w[a] = p[i].w[a]; P.ro[a] = P.r[a]; P.uo[a] = P.u[a]; P.wo[a] = P.w[a]; }
+    for (int a = 0; a < 4; ++a) P.q[a] = p[i].q[a];
+    P.R = p[i].R; P.mass = p[i].mass;
+    if (!(P.R > 0.0) || !(P.mass > 0.0)) { h->parts_host.clear(); h->np = 0; return fail(h, LB_EINVAL, "particle radius and mass must be positive"); }
+    if (2.0 * P.R + 4.0 > h->nx || 2.0 * P.R + 4.0 > h->ny || 2.0 * P.R + 4.0 > h->nz) { h->parts_host.clear(); h->np = 0; return fail(h, LB_EINVAL, "particle too large for the box"); }
+    P.inertia = 0.4 * P.mass * P.R * P.R;
+  }
+  h->np = n;
+  return LB_OK;
+}
+
+int lb_set_particle_options(lb_handle h, int mobile, double K, double h_c, int lubrication) {
+  if (!h) return LB_EINVAL;
+  h->p_mobile = mobile ? 1 : 0; h->p_K = K; h->p_hc = h_c; h->p_lub = lubrication ? 1 : 0;
+  return LB_OK;
+}
+
+int lb_set_particle_force(lb_handle h, int i, const double* F, const double* T) {
+  if (!h || i < 0 || i >= h->np) return fail(h, LB_EINVAL, "no such particle");
+  if (h->inited) return fail(h, LB_ESTATE, "lb_set_particle_force after lb_init");
+  for (int a = 0; a < 3; ++a) { h->parts_host[i].Fext[a] = F ? F[a] : 0.0; h->parts_host[i].Text[a] = T ? T[a] : 0.0; }
+  return LB_OK;
+}
+
+int lb_get_particles(lb_handle h, lb_particle* state, double* force) {
+  if (!h) return LB_EINVAL;
+  if (!h->inited || h->np == 0) return fail(h, LB_ESTATE, "lb_get_particles needs an initialised state with particles");
+  DeviceGuard guard(h->device);
+  std::vector<PState> tmp((size_t)h->np);
+  int ovf = 0;
+  cudaError_t e = cudaMemcpyAsync(tmp.data(), h->parts, (size_t)h->np * sizeof(PState), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&ovf, h->povf, sizeof(int), cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "lb_get_particles");
+  for (int i = 0; i < h->np; ++i) {
+    const PState& P = tmp[i];
+    if (state) {
+      for (int a = 0; a < 3; ++a) { state[i].r[a] = P.r[a]; state[i].u[a] = P.u[a]; state[i].w[a] = P.w[a]; }
+      for (int a = 0; a < 4; ++a) state[i].q[a] = P.q[a];
+      state[i].R = P.R; state[i].mass = P.mass;
+    }
+    if (force) for (int a = 0; a < 3; ++a) { force[9 * i + a] = P.F[a]; force[9 * i + 3 + a] = P.T[a]; force[9 * i + 6 + a] = P.Fpp[a]; }
+  }
+  if (ovf) return fail(h, LB_ESTATE, "a particle changed more nodes in one step than the node-change kernel holds (384): it moves too fast");
+  return LB_OK;
+}
 
 int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u) {
   if (!h) return LB_EINVAL;
@@ -794,6 +939,7 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   }
   int rc = allocate_state(h, rho_b != nullptr);
   if (rc) return rc;
+  if (h->np > 0 && (rc = init_particles(h))) return rc;
   const size_t fb = (size_t)h->Sx * sizeof(float);
   Staged srr, srb, su;
   if ((rc = stage_in(h, rho_r, fb, srr))) return rc;

@@ -51,6 +51,7 @@ struct StepParams {
   float uw[3][3];     // velocities of groups 2, 3, 4
   int wtype[3];       // what these groups are (G31): 0 moving wall, 1 velocity inlet, 2 reservoir, 3 pressure outlet
   float wrho[3][2];   // prescribed rho_r, rho_b of an inlet / reservoir / outlet
+  const PState* parts; // rigid particles (NEXT-4), or nullptr
   int sc;             // Shan-Chen model (Eq. 5-10 of the paper): the fields are rho_r, rho_b instead of phi
   float G_C;          // its coupling strength, positive = repulsive
 };
@@ -177,6 +178,46 @@ __device__ __forceinline__ void open_link(const StepParams& p, int gi, float rho
   }
 }
 
+// ---- rigid particles (the paper's section 6; G32-G37) ----
+__device__ __forceinline__ double min_image(double d, int n) { return d - n * floor(d / n + 0.5); }
+
+// G32: velocity of particle P's surface at the midpoint of the link that leaves the fluid node
+// (x, y, z) along c_q, projected on c_q.  with_old: the state before the last move.
+template <int q>
+__device__ __forceinline__ float link_cu(const Box& b, const PState& P, int x, int y, int z, bool with_old = false) {
+  const double* r = with_old ? P.ro : P.r;
+  const double* u = with_old ? P.uo : P.u;
+  const double* w = with_old ? P.wo : P.w;
+  const float rx = (float)(min_image(x - r[0], b.nx) + 0.5 * cx(q));
+  const float ry = (float)(min_image(y - r[1], b.ny) + 0.5 * cy(q));
+  const float rz = (float)(min_image(z - r[2], b.nz) + 0.5 * cz(q));
+  const float wx = (float)w[0], wy = (float)w[1], wz = (float)w[2];
+  const float ux = (float)u[0] + (wy * rz - wz * ry), uy = (float)u[1] + (wz * rx - wx * rz), uz = (float)u[2] + (wx * ry - wy * rx);
+  return cdot<q>(ux, uy, uz);
+}
+
+// The same for the fused kernel, out of line (a real call, taken by the few links that meet a particle)
+// so that the wall-group instantiations keep their registers: c_q . u_b for the particle whose phi
+// sentinel is sv.
+__device__ __noinline__ float particle_cu(const PState* parts, int nx, int ny, int nz, float sv, int x, int y, int z, int q) {
+  const PState& P = parts[(int)(sv * 1.0e-30f + 0.5f) - PART_GROUP0];
+  const float rx = (float)(min_image(x - P.r[0], nx) + 0.5 * c_cx[q]);
+  const float ry = (float)(min_image(y - P.r[1], ny) + 0.5 * c_cy[q]);
+  const float rz = (float)(min_image(z - P.r[2], nz) + 0.5 * c_cz[q]);
+  const float wx = (float)P.w[0], wy = (float)P.w[1], wz = (float)P.w[2];
+  const float ux = (float)P.u[0] + (wy * rz - wz * ry), uy = (float)P.u[1] + (wz * rx - wx * rz), uz = (float)P.u[2] + (wx * ry - wy * rx);
+  return (float)c_cx[q] * ux + (float)c_cy[q] * uy + (float)c_cz[q] * uz;
+}
+
+// G33: the stored pair {ts = f* - w, rs = f^r*} of a link into particle `sv` (its phi sentinel) becomes
+// what comes back from the moving surface: f^k <- f^k* - 6 w_q rho^k (c_q . u_b)
+template <int q>
+__device__ __forceinline__ void particle_link(const StepParams& p, float sv, int x, int y, int z, float rho, float rr, float& ts, float& rs) {
+  const float k = -6.0f * wq(q) * particle_cu(p.parts, p.box.nx, p.box.ny, p.box.nz, sv, x, y, z, q);
+  ts = fmaf(k, rho, ts);
+  rs = fmaf(k, rr, rs);
+}
+
 // Solid flags of the 18 neighbours from the bit-packed mask (bit i <=> x + c_i solid).
 __device__ __forceinline__ uint32_t neighbour_mask(const Box& b, int x, int y, int z) {
   const int xs[3] = {wrap_m(x, b.nx), x, wrap_p(x, b.nx)};
@@ -265,7 +306,7 @@ __device__ __forceinline__ void store_field_with_images(float* field, const Box&
 template <bool SC>
 __device__ __forceinline__ void store_fields(const StepParams& p, int x, int y, int z, int H, bool solid, float d, float rho) {
   // the sentinel of a solid site also carries its wall group (1e30, 2e30, 3e30)
-  const float sent = solid ? PHI_SOLID * (float)wall_group_at(p.box, x, y, z) : 0.f;
+  const float sent = solid ? PHI_SOLID * (float)sentinel_code(p.box, x, y, z) : 0.f;
   if constexpr (!SC) {
     store_field_with_images(p.phi, p.box, x, y, z, H, solid ? sent : d / rho);
   } else {
@@ -650,7 +691,8 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
           // a wall pushing on the fluid, an inlet or an outlet changes the mass.
           if ((smask >> q) & 1u) {
             const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
-            if (sv > 1.5f * PHI_SOLID) open_link<q>(p, (int)(sv > 2.5f * PHI_SOLID) + (int)(sv > 3.5f * PHI_SOLID), rho, rr, inv_rho, ux, uy, uz, uu15, ts, rs);
+            if (sv > 4.5f * PHI_SOLID) particle_link<q>(p, sv, x, y, z, rho, rr, ts, rs);   // a rigid particle's node (G33)
+            else if (sv > 1.5f * PHI_SOLID) open_link<q>(p, (int)(sv > 2.5f * PHI_SOLID) + (int)(sv > 3.5f * PHI_SOLID), rho, rr, inv_rho, ux, uy, uz, uu15, ts, rs);
           }
         }
         const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
@@ -1100,6 +1142,12 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
           float rs = 0.f;                      // one component: rho_r is the density
           open_link<q, true>(p, (int)((g2m >> q) & 1u) + 2 * (int)((g3m >> q) & 1u) - 1, rho, rho, inv_rho, ux, uy, uz, uu15, ts, rs);
         }
+        if (b.pid != nullptr && ((smask >> q) & 1u)) {     // a rigid particle's node (G33)
+          const int pi = b.pid[(size_t)(cx(q) > 0 ? wrap_p(x, b.nx) : (cx(q) < 0 ? wrap_m(x, b.nx) : x)) +
+                               (size_t)b.nx * ((size_t)(cy(q) > 0 ? wrap_p(y, b.ny) : (cy(q) < 0 ? wrap_m(y, b.ny) : y)) +
+                                               (size_t)b.ny * (cz(q) > 0 ? wrap_p(z, b.nz) : (cz(q) < 0 ? wrap_m(z, b.nz) : z)))];
+          if (pi >= 0) ts = fmaf(-6.0f * wq(q) * link_cu<q>(b, p.parts[pi], x, y, z), rho, ts);
+        }
       }
       *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask)) = ts;
     });
@@ -1370,6 +1418,379 @@ __global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box
     out[e] = (v - w) / (v + w);
   } else {
     out[e] = v;
+  }
+}
+
+// ----------------------------------------------------------------------------- rigid particles (NEXT-4)
+// The paper's section 6: rigid spheres obeying Newton's equations (Eq. 15), solved
+// "by a leapfrog approach, using quaternion algebra for the rotational component"; the coupling to the
+// fluid is only cited there.  Readings G32-G37 (DESIGN.md section 2 states them in full).  Per
+// time step, between the fused kernel (which applies the link rule G33 to what it stores) and the next
+// step:  k_part_force (momentum the links handed over), k_part_move (pair forces G37, leapfrog and
+// quaternion G35), k_part_remap (nodes that entered or left a particle, G36).  A/B storage only: the
+// kernels read the state of time t from the source buffer and work on the stored post-collision
+// values of the destination buffer, each at its own site.  One CTA per particle; all sums in double
+// precision and in a fixed order (the result does not depend on the scheduling).
+struct PartParams {
+  const float* ps[Q];    // source buffer (state of time t, pull layout)
+  float* pd[Q];          // destination buffer: post-collision values of time t at their own sites
+  Box box;               // mask and pid are those of time t until k_part_remap has changed them
+  uint32_t* mask;        // writable views of box.mask / box.pid
+  int* pid;
+  PState* parts;
+  int np;
+  int mobile;            // 0: the particles are held in place
+  double K, hc, mu;      // pair force (G37); mu = rho_0 nu
+  int lub;
+  int* overflow;         // set if a particle changed more nodes in one step than k_part_remap can list
+};
+
+constexpr int PART_MAXCH = 384;   // changed nodes per particle and step that k_part_remap can hold
+
+struct PartBox { int lo[3], ext[3]; };
+__device__ __forceinline__ PartBox part_box(const Box& b, const double r[3], double reach) {
+  PartBox pb;
+  const int n[3] = {b.nx, b.ny, b.nz};
+  for (int a = 0; a < 3; ++a) {
+    int lo = (int)floor(r[a] - reach), hi = (int)ceil(r[a] + reach);
+    if (hi - lo + 1 > n[a]) { lo = 0; hi = n[a] - 1; }      // never visit a node twice
+    pb.lo[a] = lo; pb.ext[a] = hi - lo + 1;
+  }
+  return pb;
+}
+__device__ __forceinline__ void part_box_node(const Box& b, const PartBox& pb, int i, int& x, int& y, int& z) {
+  const int lx = i % pb.ext[0], ly = (i / pb.ext[0]) % pb.ext[1], lz = i / (pb.ext[0] * pb.ext[1]);
+  x = (pb.lo[0] + lx) % b.nx; if (x < 0) x += b.nx;
+  y = (pb.lo[1] + ly) % b.ny; if (y < 0) y += b.ny;
+  z = (pb.lo[2] + lz) % b.nz; if (z < 0) z += b.nz;
+}
+__device__ __forceinline__ bool inside_particle(const Box& b, const PState& P, int x, int y, int z) {
+  const double dx = min_image(x - P.r[0], b.nx), dy = min_image(y - P.r[1], b.ny), dz = min_image(z - P.r[2], b.nz);
+  return dx * dx + dy * dy + dz * dz < P.R * P.R;
+}
+__device__ __forceinline__ size_t site_of(const Box& b, int x, int y, int z) { return (size_t)x + (size_t)b.nx * ((size_t)y + (size_t)b.ny * z); }
+__device__ __forceinline__ void nbr_of(const Box& b, int x, int y, int z, int q, int& xn, int& yn, int& zn) {
+  xn = x + c_cx[q]; yn = y + c_cy[q]; zn = z + c_cz[q];
+  xn = xn < 0 ? b.nx - 1 : (xn >= b.nx ? 0 : xn);
+  yn = yn < 0 ? b.ny - 1 : (yn >= b.ny ? 0 : yn);
+  zn = zn < 0 ? b.nz - 1 : (zn >= b.nz ? 0 : zn);
+}
+
+// rho_r, rho_b (one component: rho, 0) of the fluid site (x, y, z) at time t (Eq. 3): its
+// pre-collision populations gathered from the source buffer with the pull rule
+template <bool TWO>
+__device__ __forceinline__ void site_density(const PartParams& p, int x, int y, int z, float& rr, float& rb) {
+  Ctx c;
+  make_ctx<TWO ? 8 : 4>(c, p.box, x, y, z);
+  const uint32_t smask = neighbour_mask(p.box, x, y, z);
+  float t = 0.f, r = 0.f;
+  static_for<0, Q>([&](auto qc) {
+    constexpr int q = decltype(qc)::value;
+    const float* src = src_ptr(p, read_slot<MODE_AB, true, q>(c, smask));
+    if constexpr (TWO) { const float2 v = __ldcg(reinterpret_cast<const float2*>(src)); t += v.x; r += v.y; }
+    else t += __ldcg(src);
+  });
+  if constexpr (TWO) { rr = r; rb = (1.0f + t) - r; }
+  else { rr = 1.0f + t; rb = 0.f; }
+}
+
+// stored post-collision pair of direction q at its own site (A/B layout)
+template <bool TWO>
+__device__ __forceinline__ float* own_slot(const PartParams& p, int q, size_t s) { return p.pd[q] + s * (TWO ? 2 : 1); }
+
+// u_b . c_q at the midpoint of the link (x, y, z) -> + c_q, run-time q
+__device__ __forceinline__ double link_cu_rt(const Box& b, const double r[3], const double u[3], const double w[3], int x, int y, int z, int q, double rel[3]) {
+  rel[0] = min_image(x - r[0], b.nx) + 0.5 * c_cx[q];
+  rel[1] = min_image(y - r[1], b.ny) + 0.5 * c_cy[q];
+  rel[2] = min_image(z - r[2], b.nz) + 0.5 * c_cz[q];
+  // in fp32 like k_fused (link_cu), so that undoing a link reproduces the stored value
+  const float rx = (float)rel[0], ry = (float)rel[1], rz = (float)rel[2];
+  const float wx = (float)w[0], wy = (float)w[1], wz = (float)w[2];
+  const float ux = (float)u[0] + (wy * rz - wz * ry), uy = (float)u[1] + (wz * rx - wx * rz), uz = (float)u[2] + (wx * ry - wy * rx);
+  return (double)((float)c_cx[q] * ux + (float)c_cy[q] * uy + (float)c_cz[q] * uz);
+}
+
+// sum of NV doubles per thread over the CTA in a fixed order; result in every thread of warp 0 lane 0 -> out
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* red /* [NV][8] shared */) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] += __shfl_down_sync(0xffffffffu, v[k], o);
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  if (lane == 0)
+    for (int k = 0; k < NV; ++k) red[k * 8 + wp] = v[k];
+  __syncthreads();
+  if (threadIdx.x == 0)
+    for (int k = 0; k < NV; ++k) {
+      double a = 0.0;
+      for (int i = 0; i < 8; ++i) a += red[k * 8 + i];
+      v[k] = a;
+    }
+}
+
+// the nodes of every particle at start-up (G32): solid bit and particle index
+__global__ void __launch_bounds__(256) k_part_raster(const PartParams p) {
+  const Box& b = p.box;
+  const PState& P = p.parts[blockIdx.x];
+  const PartBox pb = part_box(b, P.r, P.R + 1.0);
+  const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
+  for (int i = threadIdx.x; i < nn; i += blockDim.x) {
+    int x, y, z;
+    part_box_node(b, pb, i, x, y, z);
+    if (solid_at(b, x, y, z) || !inside_particle(b, P, x, y, z)) continue;
+    atomicOr(&p.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)], 1u << (x & 31));
+    p.pid[site_of(b, x, y, z)] = blockIdx.x;
+  }
+}
+
+// G33, the particle's side: the momentum and its moment that the links of time t handed over.  For a
+// link j of the fluid site s into the particle the fused kernel stored g = f* - 6 w rho (c.u_b); the
+// particle receives (f* + g) c_j = (2 g + 6 w rho (c.u_b)) c_j, summed over the components.
+template <bool TWO>
+__global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
+  __shared__ double red[6 * 8];
+  const Box& b = p.box;
+  PState& P = p.parts[blockIdx.x];
+  const PartBox pb = part_box(b, P.r, P.R + 2.0);
+  const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
+  double acc[6] = {0, 0, 0, 0, 0, 0};
+  for (int i = threadIdx.x; i < nn; i += blockDim.x) {
+    int x, y, z;
+    part_box_node(b, pb, i, x, y, z);
+    if (solid_at(b, x, y, z)) continue;
+    const size_t s = site_of(b, x, y, z);
+    float rr = 0.f, rb = 0.f;
+    bool have = false;
+    for (int q = 1; q < Q; ++q) {
+      int xn, yn, zn;
+      nbr_of(b, x, y, z, q, xn, yn, zn);
+      if (p.pid[site_of(b, xn, yn, zn)] != (int)blockIdx.x) continue;
+      if (!have) { site_density<TWO>(p, x, y, z, rr, rb); have = true; }
+      double rel[3];
+      const double cu = link_cu_rt(b, P.r, P.u, P.w, x, y, z, q, rel);
+      const float gt = __ldcg(own_slot<TWO>(p, q, s)) + wq(q);          // reflected total (the T plane holds f - w)
+      const double tot = 2.0 * (double)gt + 6.0 * (double)wq(q) * (double)(rr + rb) * cu;
+      const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
+      acc[0] += d[0]; acc[1] += d[1]; acc[2] += d[2];
+      acc[3] += rel[1] * d[2] - rel[2] * d[1];
+      acc[4] += rel[2] * d[0] - rel[0] * d[2];
+      acc[5] += rel[0] * d[1] - rel[1] * d[0];
+    }
+  }
+  block_sum<6>(acc, red);
+  if (threadIdx.x == 0)
+    for (int a = 0; a < 3; ++a) { P.F[a] = acc[a]; P.T[a] = acc[3 + a]; }
+}
+
+// G37 and G35: pair forces, then Eq. 15 by leapfrog with the quaternion update.  One CTA.
+__global__ void __launch_bounds__(128) k_part_move(const PartParams p) {
+  const Box& b = p.box;
+  const int n[3] = {b.nx, b.ny, b.nz};
+  for (int i = threadIdx.x; i < p.np; i += blockDim.x) {
+    PState& A = p.parts[i];
+    double f[3] = {0, 0, 0};
+    if (p.hc > 0.0)
+      for (int j = 0; j < p.np; ++j) {
+        if (j == i) continue;
+        const PState& B = p.parts[j];
+        const double d[3] = {min_image(A.r[0] - B.r[0], n[0]), min_image(A.r[1] - B.r[1], n[1]), min_image(A.r[2] - B.r[2], n[2])};
+        const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        const double h = dist - A.R - B.R;
+        if (h >= p.hc) continue;
+        const double e[3] = {d[0] / dist, d[1] / dist, d[2] / dist};     // from j to i
+        double fm = p.K * pow(p.hc - h, 1.5);
+        if (p.lub) {
+          const double hh = h < 0.1 ? 0.1 : h, Reff = A.R * B.R / (A.R + B.R);
+          const double un = (A.u[0] - B.u[0]) * e[0] + (A.u[1] - B.u[1]) * e[1] + (A.u[2] - B.u[2]) * e[2];
+          fm += -6.0 * 3.14159265358979323846 * p.mu * Reff * Reff * (1.0 / hh - 1.0 / p.hc) * un;
+        }
+        for (int a = 0; a < 3; ++a) f[a] += fm * e[a];
+      }
+    for (int a = 0; a < 3; ++a) A.Fpp[a] = f[a];
+  }
+  __syncthreads();            // every pair force used the positions and velocities of time t
+  if (!p.mobile) return;
+  for (int i = threadIdx.x; i < p.np; i += blockDim.x) {
+    PState& P = p.parts[i];
+    for (int a = 0; a < 3; ++a) {
+      P.ro[a] = P.r[a]; P.uo[a] = P.u[a]; P.wo[a] = P.w[a];
+      P.u[a] += (P.F[a] + P.Fpp[a] + P.Fext[a]) / P.mass;
+      P.w[a] += (P.T[a] + P.Text[a]) / P.inertia;
+      P.r[a] += P.u[a];
+      P.r[a] -= n[a] * floor(P.r[a] / n[a]);
+    }
+    const double th = sqrt(P.w[0] * P.w[0] + P.w[1] * P.w[1] + P.w[2] * P.w[2]);
+    if (th > 0.0) {
+      const double sh = sin(0.5 * th) / th, ch = cos(0.5 * th);
+      const double d[4] = {ch, sh * P.w[0], sh * P.w[1], sh * P.w[2]};
+      const double q0 = P.q[0], q1 = P.q[1], q2 = P.q[2], q3 = P.q[3];
+      double r[4] = {d[0] * q0 - d[1] * q1 - d[2] * q2 - d[3] * q3, d[0] * q1 + d[1] * q0 + d[2] * q3 - d[3] * q2,
+                     d[0] * q2 - d[1] * q3 + d[2] * q0 + d[3] * q1, d[0] * q3 + d[1] * q2 - d[2] * q1 + d[3] * q0};
+      const double nr = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + r[3] * r[3]);
+      for (int a = 0; a < 4; ++a) P.q[a] = r[a] / nr;
+    }
+  }
+}
+
+// G36: the nodes that entered or left particle blockIdx.x when it moved.  Phase 1 lists them (sorted
+// by site, so that the sums below have a fixed order), phase 2 treats one node per thread, phase 3
+// adds the impulses to the particle and rewrites the node map.
+template <bool TWO>
+__global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
+  if (!p.mobile) return;
+  __shared__ int raw[PART_MAXCH], list[PART_MAXCH];     // site index, bit 30 set = entered the particle
+  __shared__ double imp[PART_MAXCH][6];
+  __shared__ int nraw;
+  const Box& b = p.box;
+  const int me = blockIdx.x;
+  PState& P = p.parts[me];
+  if (threadIdx.x == 0) nraw = 0;
+  __syncthreads();
+  const PartBox pb = part_box(b, P.r, P.R + 2.0);
+  const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
+  for (int i = threadIdx.x; i < nn; i += blockDim.x) {
+    int x, y, z;
+    part_box_node(b, pb, i, x, y, z);
+    const size_t s = site_of(b, x, y, z);
+    const bool was = p.pid[s] == me;
+    const bool now = inside_particle(b, P, x, y, z) && (was || !solid_at(b, x, y, z));
+    if (was != now) {
+      const int k = atomicAdd(&nraw, 1);
+      if (k < PART_MAXCH) raw[k] = (int)s | (now ? (1 << 30) : 0);
+    }
+  }
+  __syncthreads();
+  const int nch = min(nraw, PART_MAXCH);
+  if (nraw > PART_MAXCH && threadIdx.x == 0) atomicExch(p.overflow, 1);
+  for (int i = threadIdx.x; i < nch; i += blockDim.x) {       // rank sort by (site, kind)
+    const int v = raw[i] & ~(1 << 30);
+    int rank = 0;
+    for (int j = 0; j < nch; ++j) rank += (raw[j] & ~(1 << 30)) < v;
+    list[rank] = raw[i];
+  }
+  __syncthreads();
+  auto newly_covered = [&](size_t s) {
+    for (int j = 0; j < nch; ++j) if (list[j] == ((int)s | (1 << 30))) return true;
+    return false;
+  };
+  for (int i = threadIdx.x; i < nch; i += blockDim.x) {
+    const bool entered = (list[i] >> 30) & 1;
+    const size_t s = (size_t)(list[i] & ~(1 << 30));
+    const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((size_t)b.nx * b.ny));
+    double dU[3] = {0, 0, 0}, dL[3] = {0, 0, 0};
+    auto give = [&](const double m[3], const double rel[3], double sg) {
+      dU[0] += sg * m[0]; dU[1] += sg * m[1]; dU[2] += sg * m[2];
+      dL[0] += sg * (rel[1] * m[2] - rel[2] * m[1]);
+      dL[1] += sg * (rel[2] * m[0] - rel[0] * m[2]);
+      dL[2] += sg * (rel[0] * m[1] - rel[1] * m[0]);
+    };
+    // G33 with the particle's NEW state on the link (xs, ys, zs) -> + c_q; returns what the particle receives
+    auto reflect = [&](int xs, int ys, int zs, int q, float rr, float rb) {
+      double rel[3];
+      const double cu = link_cu_rt(b, P.r, P.u, P.w, xs, ys, zs, q, rel);
+      float* sl = own_slot<TWO>(p, q, site_of(b, xs, ys, zs));
+      const float k = -6.0f * wq(q) * (float)cu;
+      const float fpt = sl[0] + wq(q);                  // f* (total)
+      const float gt = fmaf(k, rr + rb, fpt);
+      sl[0] = gt - wq(q);
+      if constexpr (TWO) sl[1] = fmaf(k, rr, sl[1]);
+      const double tot = (double)fpt + (double)gt;
+      const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
+      give(d, rel, +1.0);
+    };
+    const double rel0[3] = {min_image(x - P.r[0], b.nx), min_image(y - P.r[1], b.ny), min_image(z - P.r[2], b.nz)};
+    if (!entered) {
+      // the node leaves the particle: equilibrium (Eq. 2) at the mean densities of its fluid neighbours
+      // and the surface velocity; its momentum comes out of the particle's
+      float sr = 0.f, sb = 0.f;
+      int cnt = 0;
+      for (int q = 1; q < Q; ++q) {
+        int xn, yn, zn;
+        nbr_of(b, x, y, z, q, xn, yn, zn);
+        if (solid_at(b, xn, yn, zn) || newly_covered(site_of(b, xn, yn, zn))) continue;
+        float a, c2;
+        site_density<TWO>(p, xn, yn, zn, a, c2);
+        sr += a; sb += c2; ++cnt;
+      }
+      float rr = TWO ? 0.5f : 1.0f, rb = TWO ? 0.5f : 0.0f;
+      if (cnt) { rr = sr / (float)cnt; rb = sb / (float)cnt; }
+      const double wxr[3] = {P.w[1] * rel0[2] - P.w[2] * rel0[1], P.w[2] * rel0[0] - P.w[0] * rel0[2], P.w[0] * rel0[1] - P.w[1] * rel0[0]};
+      const float ux = (float)(P.u[0] + wxr[0]), uy = (float)(P.u[1] + wxr[1]), uz = (float)(P.u[2] + wxr[2]);
+      const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz), rho = rr + rb;
+      for (int q = 0; q < Q; ++q) {
+        const float cu = c_cx[q] * ux + c_cy[q] * uy + c_cz[q] * uz;
+        const float e = 3.0f * cu + 4.5f * cu * cu - uu15;
+        float* sl = own_slot<TWO>(p, q, s);
+        sl[0] = wq(q) * ((rho - 1.0f) + rho * e);
+        if constexpr (TWO) sl[1] = wq(q) * rr * (1.0f + e);
+      }
+      const double mom[3] = {(double)rho * ux, (double)rho * uy, (double)rho * uz};
+      give(mom, rel0, -1.0);
+      for (int q = 1; q < Q; ++q) {                      // its own links into the particle as it stands now
+        int xn, yn, zn;
+        nbr_of(b, x, y, z, q, xn, yn, zn);
+        if (!inside_particle(b, P, xn, yn, zn)) continue;
+        const int pn = p.pid[site_of(b, xn, yn, zn)];
+        if (solid_at(b, xn, yn, zn) && pn != me) continue;    // a wall's or another particle's node
+        reflect(x, y, z, q, rr, rb);
+      }
+      for (int q = 1; q < Q; ++q) {                      // links of fluid neighbours into this node: undone
+        int xs, ys, zs;
+        nbr_of(b, x, y, z, opp(q), xs, ys, zs);          // (xs, ys, zs) + c_q = this node
+        const size_t t = site_of(b, xs, ys, zs);
+        if (solid_at(b, xs, ys, zs) || newly_covered(t)) continue;
+        float a, c2;
+        site_density<TWO>(p, xs, ys, zs, a, c2);
+        double rel[3];
+        const double cu = link_cu_rt(b, P.ro, P.uo, P.wo, xs, ys, zs, q, rel);
+        float* sl = own_slot<TWO>(p, q, t);
+        const float k = 6.0f * wq(q) * (float)cu;
+        const float gt = sl[0] + wq(q);
+        const float fpt = fmaf(k, a + c2, gt);
+        sl[0] = fpt - wq(q);
+        if constexpr (TWO) sl[1] = fmaf(k, a, sl[1]);
+        const double tot = (double)fpt + (double)gt;
+        const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
+        give(d, rel, -1.0);
+      }
+    } else {
+      // the node enters the particle: what it holds goes to the particle.  A stored value stands for a
+      // population that after streaming moves along c_q, or, where the neighbour is solid, along -c_q.
+      double mom[3] = {0, 0, 0};
+      for (int q = 0; q < Q; ++q) {
+        int xn, yn, zn;
+        nbr_of(b, x, y, z, q, xn, yn, zn);
+        const double sg = (q > 0 && solid_at(b, xn, yn, zn)) ? -1.0 : 1.0;
+        const double v = sg * ((double)own_slot<TWO>(p, q, s)[0] + (double)wq(q));
+        mom[0] += v * c_cx[q]; mom[1] += v * c_cy[q]; mom[2] += v * c_cz[q];
+      }
+      give(mom, rel0, +1.0);
+      for (int q = 1; q < Q; ++q) {                      // links of fluid neighbours into this node: reflected
+        int xs, ys, zs;
+        nbr_of(b, x, y, z, opp(q), xs, ys, zs);
+        if (solid_at(b, xs, ys, zs) || newly_covered(site_of(b, xs, ys, zs))) continue;
+        float a, c2;
+        site_density<TWO>(p, xs, ys, zs, a, c2);
+        reflect(xs, ys, zs, q, a, c2);
+      }
+    }
+    for (int a = 0; a < 3; ++a) { imp[i][a] = dU[a]; imp[i][3 + a] = dL[a]; }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t[6] = {0, 0, 0, 0, 0, 0};
+    for (int i = 0; i < nch; ++i)
+      for (int a = 0; a < 6; ++a) t[a] += imp[i][a];
+    for (int a = 0; a < 3; ++a) { P.u[a] += t[a] / P.mass; P.w[a] += t[3 + a] / P.inertia; }
+  }
+  for (int i = threadIdx.x; i < nch; i += blockDim.x) {       // the node map of time t + 1
+    const bool entered = (list[i] >> 30) & 1;
+    const size_t s = (size_t)(list[i] & ~(1 << 30));
+    const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((size_t)b.nx * b.ny));
+    uint32_t* wd = &p.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)];
+    if (entered) { atomicOr(wd, 1u << (x & 31)); p.pid[s] = me; }
+    else { atomicAnd(wd, ~(1u << (x & 31))); p.pid[s] = -1; }
   }
 }
 

@@ -72,7 +72,23 @@ struct Box {
   long long S;           // sites (allocated)
   const uint32_t* mask;  // bit-packed solid mask (bit x&31 of word row*nxw + x>>5), or nullptr
   const uint32_t* gmask; // wall groups: two more bit planes of the same shape behind each other (group - 1 in binary), or nullptr
+  const int* pid;        // rigid particles (NEXT-4): particle index of a particle node, -1 elsewhere; or nullptr
 };
+
+// State of one rigid spherical particle (the paper's section 6, Eq. 15).  Double
+// precision: a position of a few hundred lattice units advanced by ~1e-3 per step loses its
+// increments in fp32.  The first 15 values are lb_particle of include/lb.h.
+struct PState {
+  double r[3], u[3], w[3], q[4];   // centre, velocity, angular velocity, orientation quaternion (w, x, y, z)
+  double R, mass;
+  double inertia;                  // 2/5 m R^2
+  double F[3], T[3];               // force and torque from the fluid links of the last step (G33)
+  double Fpp[3];                   // from the other particles (G37)
+  double Fext[3], Text[3];
+  double ro[3], uo[3], wo[3];      // r, u, w before the last move (the node changes undo links made with them, G36)
+};
+
+constexpr int PART_GROUP0 = 5;     // the phi sentinel of a particle node is 1e30 x (5 + particle index)
 
 __device__ __forceinline__ bool solid_at(const Box& b, int x, int y, int z) {
   return (b.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)] >> (x & 31)) & 1u;
@@ -85,6 +101,15 @@ __device__ __forceinline__ int wall_group_at(const Box& b, int x, int y, int z) 
   const size_t nw = (size_t)b.nxw * b.ny * b.nz;
   const uint32_t g2 = (b.gmask[w] >> (x & 31)) & 1u, g3 = (b.gmask[nw + w] >> (x & 31)) & 1u;
   return 1 + (int)g2 + 2 * (int)g3;
+}
+
+// what the phi sentinel of a solid site encodes: the wall group, or 5 + the particle index
+__device__ __forceinline__ int sentinel_code(const Box& b, int x, int y, int z) {
+  if (b.pid) {
+    const int p = b.pid[(size_t)x + (size_t)b.nx * ((size_t)y + (size_t)b.ny * z)];
+    if (p >= 0) return PART_GROUP0 + p;
+  }
+  return wall_group_at(b, x, y, z);
 }
 
 __device__ __forceinline__ int wrap_m(int a, int n) { return a == 0 ? n - 1 : a - 1; }

@@ -23,6 +23,7 @@ SYMBOLS = [
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
     "lb_set_slab", "lb_slab_halo_bytes", "lb_slab_begin", "lb_slab_interior", "lb_slab_end",
     "lb_slab_pack_phi", "lb_slab_unpack_phi",
+    "lb_set_particles", "lb_set_particle_options", "lb_set_particle_force", "lb_get_particles",
 ]
 
 
@@ -81,6 +82,10 @@ def _load():
     lib.lb_slab_end.argtypes = [vp, fp, fp]
     lib.lb_slab_pack_phi.argtypes = [vp, fp, fp]
     lib.lb_slab_unpack_phi.argtypes = [vp, fp, fp]
+    lib.lb_set_particles.argtypes = [vp, C.c_int, fp]
+    lib.lb_set_particle_options.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
+    lib.lb_set_particle_force.argtypes = [vp, C.c_int, fp, fp]
+    lib.lb_get_particles.argtypes = [vp, fp, fp]
     return lib
 
 
@@ -278,6 +283,28 @@ class LB:
     def slab_unpack_phi(self, recv_lo, recv_hi):
         self._sync_stream()
         self._ck(lib.lb_slab_unpack_phi(self.h, _addr(recv_lo), _addr(recv_hi)))
+
+    # ---- rigid particles (include/lb.h "rigid spherical particles"); state rows = lb_particle:
+    # r[3], u[3], w[3], q[4], R, mass (float64)
+    def set_particles(self, state):
+        st = np.ascontiguousarray(state, dtype=np.float64).reshape(-1, 15)
+        self.npart = len(st)
+        self._ck(lib.lb_set_particles(self.h, self.npart, st.ctypes.data))
+
+    def set_particle_options(self, mobile=True, K=0.0, h_c=0.0, lubrication=False):
+        self._ck(lib.lb_set_particle_options(self.h, int(mobile), float(K), float(h_c), int(lubrication)))
+
+    def set_particle_force(self, p, F=(0, 0, 0), T=(0, 0, 0)):
+        f, t = np.array(F, np.float64), np.array(T, np.float64)
+        self._ck(lib.lb_set_particle_force(self.h, int(p), f.ctypes.data, t.ctypes.data))
+
+    def get_particles(self):
+        """(state [n, 15], force [n, 9]: F[3], T[3] from the fluid links of the last step, F_pp[3])."""
+        self._sync_stream()
+        st = np.zeros((self.npart, 15))
+        fo = np.zeros((self.npart, 9))
+        self._ck(lib.lb_get_particles(self.h, st.ctypes.data, fo.ctypes.data))
+        return st, fo
 
     def launch_count(self):
         return int(lib.lb_launch_count(self.h))

@@ -269,11 +269,48 @@ def focuser(nx=96, ny=48, nz=1, wd=10, wc=12, t=4, li=24, wo=10, lo=8, u_d=0.01,
                     info=dict(alpha=u_d / (2.0 * u_c), wall_groups=walls, li=li, xo=xo, wd=wd, wc=wc))
 
 
+def bijel(n=256, fraction=0.01, R=5.5, density=1.0, steps=2000, index=5):
+    """Colloids in a phase-separating mixture (the paper's section 6 and Fig. 6-7, PAPER.md:286-351:
+    "rigid colloids (of radius R = 5.5 lu) in a bicontinuous fluid"; the phi = 1 % rows of Fig. 6 are a
+    1024^3 box with 15 407 colloids): the C3 spinodal mixture plus N = 3 fraction / (4 pi) (n / R)^3
+     neutrally wetting spheres placed by seeded random sequential addition (gap >= 3
+    lattice units, minimum image), at rest, neutrally buoyant by default; pair repulsion and
+    lubrication on.  Positions only: no LB arithmetic here."""
+    w = c3_spinodal(n, steps=steps, index=index)
+    rng = _rng(index + 100)
+    N = max(1, int(round(3.0 * fraction / (4.0 * np.pi) * (n / R) ** 3)))
+    centres = np.zeros((0, 3))
+    tries = 0
+    while len(centres) < N and tries < 500 * N:
+        tries += 1
+        c = rng.uniform(0.0, n, size=3)
+        if len(centres):
+            d = np.abs(centres - c)
+            d = np.minimum(d, n - d)
+            if (np.sqrt((d ** 2).sum(1)) < 2 * R + 3.0).any():
+                continue
+        centres = np.vstack([centres, c])
+    m = density * 4.0 / 3.0 * np.pi * R ** 3
+    state = np.zeros((len(centres), 15))
+    state[:, 0:3] = centres
+    state[:, 9] = 1.0
+    state[:, 13] = R
+    state[:, 14] = m
+    w.name = "bijel"
+    w.info.update(particles=state, particle_options=dict(mobile=True, K=0.02, h_c=2.0, lubrication=True),
+                  colloids=int(len(centres)), colloid_volume_fraction=float(len(centres) * 4.0 / 3.0 * np.pi * R ** 3 / n ** 3))
+    return w
+
+
 def configure_walls(obj, w):
-    """Apply info["wall_groups"] of a workload to an oracle or an LB (same method names on both)."""
+    """Apply what a workload carries besides its fields to an oracle or an LB (same method names on
+    both): info["wall_groups"] (velocities, open boundaries) and info["particles"] (rigid colloids)."""
     for group, d in sorted(w.info.get("wall_groups", {}).items()):
         obj.set_wall_velocity(group, *d["u"])
         obj.set_wall_type(group, d["kind"], *d["rho"])
+    if "particles" in w.info:
+        obj.set_particles(w.info["particles"])
+        obj.set_particle_options(**w.info["particle_options"])
 
 
 def get(name):
@@ -288,6 +325,8 @@ def get(name):
         "c3-mini": lambda: c3_spinodal(64, steps=100),
         "c4-mini": lambda: c4_channel(128, 32, 32, R=6.0, steps=100),
         "c5-mini": lambda: c5_emulsion(96, 8, steps=100),
+        "bijel": bijel,
+        "bijel-mini": lambda: bijel(48, fraction=0.02, R=4.5, density=2.0, steps=100),
         "focuser": focuser,
         "focuser-3d": lambda: focuser(256, 96, 48, wd=20, wc=24, t=6, li=48, wo=20, lo=16, walls_z=True,
                                       A_nc=0.02, steps=20000),

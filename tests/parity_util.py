@@ -19,6 +19,8 @@ def make_oracle(lbo, w):
         o.set_geometry(w.solid)
     o.set_body_force(*w.g)
     o.set_nc_cutoff(w.phi_c)
+    from paper_2005_12764_b200 import workloads
+    workloads.configure_walls(o, w)            # wall groups, particles
     o.init(w.rho_r, w.rho_b, w.u)
     return o
 
