@@ -479,10 +479,11 @@ void run_particles(lb_handle h) {
   const PartParams q = make_part_params(h);
   if (h->two) k_part_force<true><<<h->np, 256, 0, h->stream>>>(q);
   else k_part_force<false><<<h->np, 256, 0, h->stream>>>(q);
-  k_part_move<<<1, 128, 0, h->stream>>>(q);
+  k_part_pair<<<(h->np + 7) / 8, 256, 0, h->stream>>>(q);
+  k_part_integrate<<<(h->np + 127) / 128, 128, 0, h->stream>>>(q);
   if (h->two) k_part_remap<true><<<h->np, 256, 0, h->stream>>>(q);
   else k_part_remap<false><<<h->np, 256, 0, h->stream>>>(q);
-  h->launches += 3;
+  h->launches += 4;
 }
 
 // One whole step of a box that is periodic in z: K2 (+ K1f) or K2s

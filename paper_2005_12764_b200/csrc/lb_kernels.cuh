@@ -179,7 +179,11 @@ __device__ __forceinline__ void open_link(const StepParams& p, int gi, float rho
 }
 
 // ---- rigid particles (the paper's section 6; G32-G37) ----
-__device__ __forceinline__ double min_image(double d, int n) { return d - n * floor(d / n + 0.5); }
+// nearest periodic image of a difference of two positions inside the box (|d| < n): no division
+__device__ __forceinline__ double min_image(double d, int n) {
+  const double h = 0.5 * n;
+  return d > h ? d - n : (d < -h ? d + n : d);
+}
 
 // G32: velocity of particle P's surface at the midpoint of the link that leaves the fluid node
 // (x, y, z) along c_q, projected on c_q.  with_old: the state before the last move.
@@ -1426,8 +1430,8 @@ __global__ void k_unpad_phi(const float* phi, const float* phi2, float* out, Box
 // "by a leapfrog approach, using quaternion algebra for the rotational component"; the coupling to the
 // fluid is only cited there.  Readings G32-G37 (DESIGN.md section 2 states them in full).  Per
 // time step, between the fused kernel (which applies the link rule G33 to what it stores) and the next
-// step:  k_part_force (momentum the links handed over), k_part_move (pair forces G37, leapfrog and
-// quaternion G35), k_part_remap (nodes that entered or left a particle, G36).  A/B storage only: the
+// step:  k_part_force (momentum the links handed over), k_part_pair (pair forces G37), k_part_integrate
+// (leapfrog and quaternion G35), k_part_remap (nodes that entered or left a particle, G36).  A/B storage only: the
 // kernels read the state of time t from the source buffer and work on the stored post-collision
 // values of the destination buffer, each at its own site.  One CTA per particle; all sums in double
 // precision and in a fixed order (the result does not depend on the scheduling).
@@ -1550,23 +1554,32 @@ __global__ void __launch_bounds__(256) k_part_raster(const PartParams p) {
 template <bool TWO>
 __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
   __shared__ double red[6 * 8];
+  __shared__ int queue[8][64];
   const Box& b = p.box;
   PState& P = p.parts[blockIdx.x];
   const PartBox pb = part_box(b, P.r, P.R + 2.0);
-  const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
   double acc[6] = {0, 0, 0, 0, 0, 0};
-  for (int i = threadIdx.x; i < nn; i += blockDim.x) {
-    int x, y, z;
-    part_box_node(b, pb, i, x, y, z);
-    if (solid_at(b, x, y, z)) continue;
-    const size_t s = site_of(b, x, y, z);
-    float rr = 0.f, rb = 0.f;
-    bool have = false;
+  // everything a candidate site (a fluid node in the shell around the sphere) needs
+  auto process = [&](int site) {
+    const size_t s = (size_t)site;
+    const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((size_t)b.nx * b.ny));
+    const uint32_t smask = neighbour_mask(b, x, y, z);      // 18 independent loads from the (small) bit mask
+    if (smask == 0u) return;
+    // which of the solid neighbours belong to this particle: the index loads are issued together
+    uint32_t mine = 0u;
+    static_for<1, Q>([&](auto qc) {
+      constexpr int q = decltype(qc)::value;
+      if ((smask >> q) & 1u) {
+        int xn, yn, zn;
+        nbr_of(b, x, y, z, q, xn, yn, zn);
+        if (p.pid[site_of(b, xn, yn, zn)] == (int)blockIdx.x) mine |= 1u << q;
+      }
+    });
+    if (mine == 0u) return;
+    float rr, rb;
+    site_density<TWO>(p, x, y, z, rr, rb);
     for (int q = 1; q < Q; ++q) {
-      int xn, yn, zn;
-      nbr_of(b, x, y, z, q, xn, yn, zn);
-      if (p.pid[site_of(b, xn, yn, zn)] != (int)blockIdx.x) continue;
-      if (!have) { site_density<TWO>(p, x, y, z, rr, rb); have = true; }
+      if (!((mine >> q) & 1u)) continue;
       double rel[3];
       const double cu = link_cu_rt(b, P.r, P.u, P.w, x, y, z, q, rel);
       const float gt = __ldcg(own_slot<TWO>(p, q, s)) + wq(q);          // reflected total (the T plane holds f - w)
@@ -1577,59 +1590,113 @@ __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
       acc[4] += rel[2] * d[0] - rel[0] * d[2];
       acc[5] += rel[0] * d[1] - rel[1] * d[0];
     }
+  };
+  const float Rin = (float)P.R - 0.01f, Rout = (float)P.R + 1.75f;     // a fluid node with a link into the sphere lies in this shell
+  // A warp scans rows of the box and queues the few shell nodes it finds; the costly part then runs on
+  // 32 queued nodes at a time, all lanes busy.  Which thread adds which node is fixed by the scan
+  // order, so the sums do not depend on the scheduling.
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nrows = pb.ext[1] * pb.ext[2];
+  const float cxr = (float)P.r[0], cyr = (float)P.r[1], czr = (float)P.r[2];
+  int qn = 0;
+  for (int row = wid; row < nrows; row += 8) {
+    const int ly = row % pb.ext[1], lz = row / pb.ext[1];
+    int y = pb.lo[1] + ly, z = pb.lo[2] + lz;
+    y += y < 0 ? b.ny : (y >= b.ny ? -b.ny : 0);
+    z += z < 0 ? b.nz : (z >= b.nz ? -b.nz : 0);
+    for (int lx0 = 0; lx0 < pb.ext[0]; lx0 += 32) {
+      const int lx = lx0 + lane;
+      int x = pb.lo[0] + lx;
+      x += x < 0 ? b.nx : (x >= b.nx ? -b.nx : 0);
+      bool pass = lx < pb.ext[0];
+      if (pass) {
+        float fx = (float)x - cxr, fy = (float)y - cyr, fz = (float)z - czr;     // fp32 is enough for the prefilter
+        fx += fx > 0.5f * b.nx ? -(float)b.nx : (fx < -0.5f * b.nx ? (float)b.nx : 0.f);
+        fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
+        fz += fz > 0.5f * b.nz ? -(float)b.nz : (fz < -0.5f * b.nz ? (float)b.nz : 0.f);
+        const float d2 = fx * fx + fy * fy + fz * fz;
+        pass = d2 >= Rin * Rin && d2 <= Rout * Rout + 0.5f && !solid_at(b, x, y, z);
+      }
+      const unsigned bal = __ballot_sync(0xffffffffu, pass);
+      if (pass) queue[wid][qn + __popc(bal & ((1u << lane) - 1u))] = (int)site_of(b, x, y, z);
+      qn += __popc(bal);
+      __syncwarp();
+      if (qn >= 32) {
+        process(queue[wid][lane]);
+        const int left = qn - 32;
+        const int v = lane < left ? queue[wid][32 + lane] : 0;
+        __syncwarp();
+        if (lane < left) queue[wid][lane] = v;
+        qn = left;
+        __syncwarp();
+      }
+    }
   }
+  if (lane < qn) process(queue[wid][lane]);
   block_sum<6>(acc, red);
   if (threadIdx.x == 0)
     for (int a = 0; a < 3; ++a) { P.F[a] = acc[a]; P.T[a] = acc[3 + a]; }
 }
 
-// G37 and G35: pair forces, then Eq. 15 by leapfrog with the quaternion update.  One CTA.
-__global__ void __launch_bounds__(128) k_part_move(const PartParams p) {
+// G37: the force on particle i from all others.  One warp per particle, the lanes share the others;
+// the lane sums are added in a fixed order.
+__global__ void __launch_bounds__(256) k_part_pair(const PartParams p) {
   const Box& b = p.box;
   const int n[3] = {b.nx, b.ny, b.nz};
-  for (int i = threadIdx.x; i < p.np; i += blockDim.x) {
-    PState& A = p.parts[i];
-    double f[3] = {0, 0, 0};
-    if (p.hc > 0.0)
-      for (int j = 0; j < p.np; ++j) {
-        if (j == i) continue;
-        const PState& B = p.parts[j];
-        const double d[3] = {min_image(A.r[0] - B.r[0], n[0]), min_image(A.r[1] - B.r[1], n[1]), min_image(A.r[2] - B.r[2], n[2])};
-        const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-        const double h = dist - A.R - B.R;
-        if (h >= p.hc) continue;
-        const double e[3] = {d[0] / dist, d[1] / dist, d[2] / dist};     // from j to i
-        double fm = p.K * pow(p.hc - h, 1.5);
-        if (p.lub) {
-          const double hh = h < 0.1 ? 0.1 : h, Reff = A.R * B.R / (A.R + B.R);
-          const double un = (A.u[0] - B.u[0]) * e[0] + (A.u[1] - B.u[1]) * e[1] + (A.u[2] - B.u[2]) * e[2];
-          fm += -6.0 * 3.14159265358979323846 * p.mu * Reff * Reff * (1.0 / hh - 1.0 / p.hc) * un;
-        }
-        for (int a = 0; a < 3; ++a) f[a] += fm * e[a];
+  const int i = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (i >= p.np) return;
+  PState& A = p.parts[i];
+  double f[3] = {0, 0, 0};
+  if (p.hc > 0.0)
+    for (int j = lane; j < p.np; j += 32) {
+      if (j == i) continue;
+      const PState& B = p.parts[j];
+      const double d[3] = {min_image(A.r[0] - B.r[0], n[0]), min_image(A.r[1] - B.r[1], n[1]), min_image(A.r[2] - B.r[2], n[2])};
+      const double reach = A.R + B.R + p.hc;
+      const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+      if (d2 >= reach * reach) continue;
+      const double dist = sqrt(d2);
+      const double h = dist - A.R - B.R;
+      if (h >= p.hc) continue;
+      const double e[3] = {d[0] / dist, d[1] / dist, d[2] / dist};     // from j to i
+      double fm = p.K * pow(p.hc - h, 1.5);
+      if (p.lub) {
+        const double hh = h < 0.1 ? 0.1 : h, Reff = A.R * B.R / (A.R + B.R);
+        const double un = (A.u[0] - B.u[0]) * e[0] + (A.u[1] - B.u[1]) * e[1] + (A.u[2] - B.u[2]) * e[2];
+        fm += -6.0 * 3.14159265358979323846 * p.mu * Reff * Reff * (1.0 / hh - 1.0 / p.hc) * un;
       }
+      for (int a = 0; a < 3; ++a) f[a] += fm * e[a];
+    }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) f[a] += __shfl_down_sync(0xffffffffu, f[a], o);
+  if (lane == 0)
     for (int a = 0; a < 3; ++a) A.Fpp[a] = f[a];
+}
+
+// G35: Eq. 15 by leapfrog with the quaternion update; one thread per particle
+__global__ void __launch_bounds__(128) k_part_integrate(const PartParams p) {
+  const Box& b = p.box;
+  const int n[3] = {b.nx, b.ny, b.nz};
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= p.np || !p.mobile) return;
+  PState& P = p.parts[i];
+  for (int a = 0; a < 3; ++a) {
+    P.ro[a] = P.r[a]; P.uo[a] = P.u[a]; P.wo[a] = P.w[a];
+    P.u[a] += (P.F[a] + P.Fpp[a] + P.Fext[a]) / P.mass;
+    P.w[a] += (P.T[a] + P.Text[a]) / P.inertia;
+    P.r[a] += P.u[a];
+    P.r[a] -= n[a] * floor(P.r[a] / n[a]);
   }
-  __syncthreads();            // every pair force used the positions and velocities of time t
-  if (!p.mobile) return;
-  for (int i = threadIdx.x; i < p.np; i += blockDim.x) {
-    PState& P = p.parts[i];
-    for (int a = 0; a < 3; ++a) {
-      P.ro[a] = P.r[a]; P.uo[a] = P.u[a]; P.wo[a] = P.w[a];
-      P.u[a] += (P.F[a] + P.Fpp[a] + P.Fext[a]) / P.mass;
-      P.w[a] += (P.T[a] + P.Text[a]) / P.inertia;
-      P.r[a] += P.u[a];
-      P.r[a] -= n[a] * floor(P.r[a] / n[a]);
-    }
-    const double th = sqrt(P.w[0] * P.w[0] + P.w[1] * P.w[1] + P.w[2] * P.w[2]);
-    if (th > 0.0) {
-      const double sh = sin(0.5 * th) / th, ch = cos(0.5 * th);
-      const double d[4] = {ch, sh * P.w[0], sh * P.w[1], sh * P.w[2]};
-      const double q0 = P.q[0], q1 = P.q[1], q2 = P.q[2], q3 = P.q[3];
-      double r[4] = {d[0] * q0 - d[1] * q1 - d[2] * q2 - d[3] * q3, d[0] * q1 + d[1] * q0 + d[2] * q3 - d[3] * q2,
-                     d[0] * q2 - d[1] * q3 + d[2] * q0 + d[3] * q1, d[0] * q3 + d[1] * q2 - d[2] * q1 + d[3] * q0};
-      const double nr = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + r[3] * r[3]);
-      for (int a = 0; a < 4; ++a) P.q[a] = r[a] / nr;
-    }
+  const double th = sqrt(P.w[0] * P.w[0] + P.w[1] * P.w[1] + P.w[2] * P.w[2]);
+  if (th > 0.0) {
+    const double sh = sin(0.5 * th) / th, ch = cos(0.5 * th);
+    const double d[4] = {ch, sh * P.w[0], sh * P.w[1], sh * P.w[2]};
+    const double q0 = P.q[0], q1 = P.q[1], q2 = P.q[2], q3 = P.q[3];
+    double r[4] = {d[0] * q0 - d[1] * q1 - d[2] * q2 - d[3] * q3, d[0] * q1 + d[1] * q0 + d[2] * q3 - d[3] * q2,
+                   d[0] * q2 - d[1] * q3 + d[2] * q0 + d[3] * q1, d[0] * q3 + d[1] * q2 - d[2] * q1 + d[3] * q0};
+    const double nr = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + r[3] * r[3]);
+    for (int a = 0; a < 4; ++a) P.q[a] = r[a] / nr;
   }
 }
 
