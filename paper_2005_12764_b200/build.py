@@ -27,8 +27,17 @@ def _nvcc():
     raise RuntimeError("nvcc not found; cannot build the CUDA extension")
 
 
+SUBSET_STAMP = LIB + ".subset"     # present beside a library that was built with LB_BUILD_SUBSET=1
+
+
+def _subset():
+    return os.environ.get("LB_BUILD_SUBSET") == "1"
+
+
 def stale():
     if not os.path.exists(LIB):
+        return True
+    if os.path.exists(SUBSET_STAMP) != _subset():   # a developer build never stands in for the full one
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS]
@@ -39,11 +48,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         tmp = LIB + ".tmp%d" % os.getpid()
         # LB_BUILD_SUBSET=1: developer builds that compile a fifth of the k_fused instantiations (lb_api.cu)
-        subset = ["-DLB_BUILD_SUBSET"] if os.environ.get("LB_BUILD_SUBSET") == "1" else []
+        subset = ["-DLB_BUILD_SUBSET"] if _subset() else []
         cmd = [_nvcc()] + NVCC_FLAGS + subset + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
+        if _subset():
+            open(SUBSET_STAMP, "w").close()
+        elif os.path.exists(SUBSET_STAMP):
+            os.remove(SUBSET_STAMP)
     return LIB
 
 
