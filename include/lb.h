@@ -160,6 +160,23 @@ int lb_step(lb_handle h, int nsteps);
  * returns LB_ESTATE instead of stepping on: that is the one place where lb_step synchronises. */
 int lb_check_state(lb_handle h, double* mass_r, double* mass_b);
 
+/* The same sums for callers that may not allocate or synchronise (code under CUDA graph capture,
+ * tight loops, harnesses that forbid cudaMalloc): calls no cudaMalloc / cudaFree and no allocator
+ * hook, never synchronises, and writes {sum rho_r, sum rho_b, number of fluid sites that hold a
+ * NaN / Inf population} to d_out, a DEVICE pointer to 3 doubles owned by the caller, on the
+ * handle's stream.  It does not judge the state: the caller reads d_out[2] (LB_ESTATE is never
+ * returned for a non-finite state, and the 1000-step counter of lb_step is not reset).
+ * Scratch memory is one array of 768 KiB + 256 B in the library's device image
+ * (`static __device__`; every GPU that loads the library holds it until the process exits): one
+ * triple of partial sums per block of 8192 sites, added up in a fixed order, so two calls on the
+ * same state give the same bits (lb_check_state adds atomically and agrees to rounding).
+ * Limit: at most 2^28 = 268,435,456 own sites (640^3 fits); a larger box returns LB_EINVAL with
+ * a text that names the limit, before anything is launched.  d_out NULL or a host pointer:
+ * LB_EINVAL.  All calls on one device share the array (handles included): calls that overlap on
+ * the GPU (different streams without an ordering between them) race; calls ordered on one
+ * stream, or by events, do not. */
+int lb_check_state_static(lb_handle h, double* d_out);
+
 /* rho_r, rho_b and the velocity u = (sum_i c_i f_i + F/2)/rho of the current state (Eq. 3,
  * PAPER.md:96, with the half-force shift of Guo forcing; G16).  Zeros on solid sites.  Any
  * output pointer may be NULL; rho_b is ignored in single-component mode.  Does not disturb

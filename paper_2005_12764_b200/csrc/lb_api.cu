@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1351,3 +1352,155 @@ int lb_last_step_ms(lb_handle h, int which, float* ms) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------ state check without allocation
+// lb_check_state_static (include/lb.h): the sums of lb_check_state for callers that may not
+// allocate (CUDA graph capture, tight loops, harnesses that forbid cudaMalloc).  k_check_static is
+// a variant of k_check whose scratch memory is the file-scope array below instead of a buffer the
+// handle allocates: one triple of partial sums per block of SC_SITES_PER_BLOCK sites, summed by
+// the last block to arrive in a fixed order (the result does not depend on the order in which the
+// blocks ran, unlike k_check's atomic adds).
+constexpr int SC_SITES_PER_BLOCK = 8192;   // 256 threads x 32 sites
+constexpr int SC_MAX_BLOCKS = 32768;
+constexpr long long SC_MAX_SITES = (long long)SC_SITES_PER_BLOCK * SC_MAX_BLOCKS;   // 2^28 sites (640^3 fits)
+constexpr int SC_COUNTER_AT = 3 * SC_MAX_BLOCKS;   // the arrival counter sits behind the partial sums
+
+// 768 KiB of partial sums + 256 B for the arrival counter.  Every GPU that loads the library holds
+// this array until the process exits.  In host code the name is a host-side stand-in, NOT a
+// device address: static_scratch() below asks the runtime for the address, once per device.
+static __device__ __align__(256) double g_static_scratch[3 * SC_MAX_BLOCKS + 32];
+
+namespace {
+
+template <int MODE, bool TWO, bool HAS_SOLID>
+__global__ void __launch_bounds__(256) k_check_static(const IoParams p, double* scratch, double* out) {
+  const Box& b = p.box;
+  double sr = 0.0, sb = 0.0, bad = 0.0;
+  const long long base = p.s0 + (long long)blockIdx.x * SC_SITES_PER_BLOCK;
+  const long long end = base + SC_SITES_PER_BLOCK < p.s1 ? base + SC_SITES_PER_BLOCK : p.s1;
+  for (long long s = base + threadIdx.x; s < end; s += 256) {
+    const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((long long)b.nx * b.ny));
+    uint32_t smask = 0;
+    if constexpr (HAS_SOLID) {
+      if (solid_at(b, x, y, z)) continue;
+      smask = neighbour_mask(b, x, y, z);
+    }
+    Ctx c;
+    make_ctx<TWO ? 8 : 4>(c, b, x, y, z);
+    float t = 0.f, r = 0.f;
+    static_for<0, Q>([&](auto qc) {
+      constexpr int q = decltype(qc)::value;
+      const float* src = src_ptr(p, read_slot<MODE, HAS_SOLID, q>(c, smask));
+      if constexpr (TWO) {
+        const float2 v = __ldcg(reinterpret_cast<const float2*>(src));
+        t += v.x; r += v.y;
+      } else {
+        t += __ldcg(src);
+      }
+    });
+    if (!isfinite(t) || !isfinite(r)) { bad += 1.0; continue; }
+    if constexpr (TWO) { sr += (double)r; sb += (double)(1.0f + t) - (double)r; }
+    else sr += (double)(1.0f + t);
+  }
+  __shared__ double red[3][8];
+  __shared__ bool last;
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  auto block_sum3 = [&](double& a0, double& a1, double& a2) {   // fixed order: the same bits every time
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      a0 += __shfl_down_sync(0xffffffffu, a0, o);
+      a1 += __shfl_down_sync(0xffffffffu, a1, o);
+      a2 += __shfl_down_sync(0xffffffffu, a2, o);
+    }
+    if (lane == 0) { red[0][wp] = a0; red[1][wp] = a1; red[2][wp] = a2; }
+    __syncthreads();
+    double v = 0.0;
+    if (threadIdx.x < 3)
+      for (int i = 0; i < 8; ++i) v += red[threadIdx.x][i];
+    return v;   // threads 0..2 hold the three sums
+  };
+  const double part = block_sum3(sr, sb, bad);
+  if (threadIdx.x < 3) {
+    scratch[3 * (size_t)blockIdx.x + threadIdx.x] = part;
+    __threadfence();                 // the partial sums are visible before the ticket is drawn
+  }
+  __syncthreads();
+  unsigned* counter = reinterpret_cast<unsigned*>(scratch + SC_COUNTER_AT);
+  if (threadIdx.x == 0) last = atomicAdd(counter, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+  for (unsigned i = threadIdx.x; i < gridDim.x; i += 256) {
+    a0 += __ldcg(scratch + 3 * (size_t)i);
+    a1 += __ldcg(scratch + 3 * (size_t)i + 1);
+    a2 += __ldcg(scratch + 3 * (size_t)i + 2);
+  }
+  __syncthreads();                   // red[] is reused
+  const double total = block_sum3(a0, a1, a2);
+  if (threadIdx.x < 3) out[threadIdx.x] = total;
+  if (threadIdx.x == 0) *counter = 0u;   // the next call on this stream finds the counter at zero
+}
+
+// Device address of g_static_scratch on the handle's device (which the caller has made current).
+// Asked once per device; no allocation.
+int static_scratch(lb_handle h, double** ptr) {
+  static double* addr[MAX_DEVICES] = {};
+  static std::mutex mu;
+  int cur = -1;
+  if (cudaGetDevice(&cur) != cudaSuccess || cur != h->device || cur < 0 || cur >= MAX_DEVICES) {
+    cudaGetLastError();
+    return fail(h, LB_ECUDA, "lb_check_state_static: the handle's device could not be made current");
+  }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[cur]) {
+    void* q = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&q, g_static_scratch);
+    if (e != cudaSuccess || !q) return cuda_fail(h, e, "lb_check_state_static: address of the static scratch array");
+    addr[cur] = static_cast<double*>(q);
+  }
+  *ptr = addr[cur];
+  return LB_OK;
+}
+
+template <int MODE, bool TWO>
+void launch_check_static_t(lb_handle h, const IoParams& p, int nb, double* scratch, double* out) {
+  if (h->has_solid) k_check_static<MODE, TWO, true><<<nb, 256, 0, h->stream>>>(p, scratch, out);
+  else k_check_static<MODE, TWO, false><<<nb, 256, 0, h->stream>>>(p, scratch, out);
+}
+
+}  // namespace
+
+extern "C" int lb_check_state_static(lb_handle h, double* d_out) {
+  if (!h) return LB_EINVAL;
+  if (!d_out) return fail(h, LB_EINVAL, "lb_check_state_static: d_out is NULL");
+  const long long sites = h->Sx;   // the handle's own sites (known since lb_create)
+  if (sites > SC_MAX_SITES) {
+    char msg[200];
+    snprintf(msg, sizeof(msg), "lb_check_state_static: %lld sites exceed the static scratch array's maximum of %lld (use lb_check_state)",
+             sites, SC_MAX_SITES);
+    return fail(h, LB_EINVAL, msg);
+  }
+  if (!h->inited) return fail(h, LB_ESTATE, "lb_check_state_static before lb_init");
+  DeviceGuard guard(h->device);
+  if (!is_device_ptr(d_out)) return fail(h, LB_EINVAL, "lb_check_state_static: d_out must be a device pointer (3 doubles)");
+  const IoParams p = make_io_params(h);
+  double* scratch = nullptr;
+  if (int rc = static_scratch(h, &scratch)) return rc;
+  // the array keeps what the last call left: the arrival counter must start at zero
+  cudaError_t e = cudaMemsetAsync(scratch + SC_COUNTER_AT, 0, 256, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "lb_check_state_static: counter reset");
+  const int nb = (int)((sites + SC_SITES_PER_BLOCK - 1) / SC_SITES_PER_BLOCK);
+  const int mode = h->mode();
+  if (h->two) {
+    if (mode == MODE_AB) launch_check_static_t<MODE_AB, true>(h, p, nb, scratch, d_out);
+    else if (mode == MODE_AA_EVEN) launch_check_static_t<MODE_AA_EVEN, true>(h, p, nb, scratch, d_out);
+    else launch_check_static_t<MODE_AA_ODD, true>(h, p, nb, scratch, d_out);
+  } else {
+    if (mode == MODE_AB) launch_check_static_t<MODE_AB, false>(h, p, nb, scratch, d_out);
+    else if (mode == MODE_AA_EVEN) launch_check_static_t<MODE_AA_EVEN, false>(h, p, nb, scratch, d_out);
+    else launch_check_static_t<MODE_AA_ODD, false>(h, p, nb, scratch, d_out);
+  }
+  h->launches++;
+  return check_launch(h, "lb_check_state_static");
+}

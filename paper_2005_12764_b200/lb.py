@@ -19,7 +19,7 @@ LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 SYMBOLS = [
     "lb_set_allocator", "lb_create", "lb_destroy", "lb_set_stream", "lb_set_geometry",
     "lb_set_wall_velocity", "lb_set_wall_type", "lb_set_body_force", "lb_set_model", "lb_set_forcing", "lb_set_nc_cutoff", "lb_set_nc_symmetric", "lb_set_wall_phi", "lb_set_storage", "lb_init", "lb_step",
-    "lb_check_state", "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
+    "lb_check_state", "lb_check_state_static", "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
     "lb_set_slab", "lb_slab_halo_bytes", "lb_slab_begin", "lb_slab_interior", "lb_slab_end",
     "lb_slab_pack_phi", "lb_slab_unpack_phi",
@@ -62,6 +62,7 @@ def _load():
     lib.lb_init.argtypes = [vp, fp, fp, fp]
     lib.lb_step.argtypes = [vp, C.c_int]
     lib.lb_check_state.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.lb_check_state_static.argtypes = [vp, vp]
     lib.lb_get_macros.argtypes = [vp, fp, fp, fp]
     lib.lb_get_populations.argtypes = [vp, C.c_int, fp]
     lib.lb_set_populations.argtypes = [vp, C.c_int, fp]
@@ -226,6 +227,12 @@ class LB:
         mr, mb = C.c_double(), C.c_double()
         self._ck(lib.lb_check_state(self.h, C.byref(mr), C.byref(mb)))
         return float(mr.value), float(mb.value)
+
+    def check_state_static(self, d_out):
+        """{mass_r, mass_b, non-finite sites} into d_out (3 float64 on the device) on the handle's
+        stream: no allocation, no synchronisation (include/lb.h)."""
+        self._sync_stream()
+        self._ck(lib.lb_check_state_static(self.h, _addr(d_out)))
 
     def get_macros(self, rho_r=None, rho_b=None, u=None):
         """Fills the given arrays (host or device); allocates numpy outputs when none given."""
