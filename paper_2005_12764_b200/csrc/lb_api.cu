@@ -153,7 +153,6 @@ struct lb_handle_s {
     b.S = S;
     b.mask = has_solid ? mask : nullptr;
     b.gmask = (has_solid && has_moving) ? mask + (size_t)b.nxw * ny * nza() : nullptr;
-    b.pid = np > 0 ? pid : nullptr;
     return b;
   }
   int planes() const { return two ? 2 * Q : Q; }
@@ -491,8 +490,25 @@ void run_particles(lb_handle h) {
 void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
   launch_collide(h, h->zlo(), h->zhi());
   if (after_k2) cudaEventRecord(after_k2, h->stream);
-  if (h->np > 0) run_particles(h);
-  if (h->two && h->forward && h->np == 0) {      // (with particles the node map changes: phi comes from the full sweep)
+  if (h->np > 0) {
+    // phi(t + 1) from the forwarded moments first (they belong to the node map of time t), then the
+    // particles, then phi again in the shells around them (k_part_phi)
+    const bool fwd = h->two && h->forward;
+    if (fwd) launch_phase_forward(h, h->zlo(), h->zhi());
+    run_particles(h);
+    if (fwd) {
+      const StepParams q = make_step_params(h, next_buf(h), nullptr, pick_zc(h), h->zlo(), h->zhi());
+      // rows of the largest particle's box, 32 per CTA (4 per warp)
+      double rmax = 0.0;
+      for (const PState& P : h->parts_host) rmax = std::max(rmax, P.R);
+      const int ext = 2 * (int)std::ceil(rmax + 2.5) + 2;
+      const int slices = std::max(1, std::min(64, (ext * ext + 31) / 32));
+      k_part_phi<<<dim3(h->np, slices), 256, 0, h->stream>>>(q);
+      h->launches++;
+    }
+    flip(h);
+    h->phi_current = fwd;
+  } else if (h->two && h->forward) {
     launch_phase_forward(h, h->zlo(), h->zhi());
     flip(h);
     h->phi_current = true;
@@ -864,8 +880,7 @@ int init_particles(lb_handle h) {
   if (e == cudaSuccess) e = cudaMemcpyAsync(h->parts, h->parts_host.data(), (size_t)h->np * sizeof(PState), cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);      // parts_host is pageable
   if (e != cudaSuccess) return cuda_fail(h, e, "particle set-up");
-  h->has_solid = true;
-  h->has_moving = true;        // the instantiations that look at what kind of solid a link meets
+  h->has_solid = true;         // to the hot kernels a particle's node is a wall at rest (k_part_force applies G33)
   const PartParams q = make_part_params(h);
   k_part_raster<<<h->np, 256, 0, h->stream>>>(q);
   h->launches++;

@@ -179,47 +179,12 @@ __device__ __forceinline__ void open_link(const StepParams& p, int gi, float rho
 }
 
 // ---- rigid particles (the paper's section 6; G32-G37) ----
+// The hot kernels treat a particle's nodes as walls at rest; k_part_force then turns every stored
+// value of a link into a particle into what comes back from the moving surface (G33).
 // nearest periodic image of a difference of two positions inside the box (|d| < n): no division
 __device__ __forceinline__ double min_image(double d, int n) {
   const double h = 0.5 * n;
   return d > h ? d - n : (d < -h ? d + n : d);
-}
-
-// G32: velocity of particle P's surface at the midpoint of the link that leaves the fluid node
-// (x, y, z) along c_q, projected on c_q.  with_old: the state before the last move.
-template <int q>
-__device__ __forceinline__ float link_cu(const Box& b, const PState& P, int x, int y, int z, bool with_old = false) {
-  const double* r = with_old ? P.ro : P.r;
-  const double* u = with_old ? P.uo : P.u;
-  const double* w = with_old ? P.wo : P.w;
-  const float rx = (float)(min_image(x - r[0], b.nx) + 0.5 * cx(q));
-  const float ry = (float)(min_image(y - r[1], b.ny) + 0.5 * cy(q));
-  const float rz = (float)(min_image(z - r[2], b.nz) + 0.5 * cz(q));
-  const float wx = (float)w[0], wy = (float)w[1], wz = (float)w[2];
-  const float ux = (float)u[0] + (wy * rz - wz * ry), uy = (float)u[1] + (wz * rx - wx * rz), uz = (float)u[2] + (wx * ry - wy * rx);
-  return cdot<q>(ux, uy, uz);
-}
-
-// The same for the fused kernel, out of line (a real call, taken by the few links that meet a particle)
-// so that the wall-group instantiations keep their registers: c_q . u_b for the particle whose phi
-// sentinel is sv.
-__device__ __noinline__ float particle_cu(const PState* parts, int nx, int ny, int nz, float sv, int x, int y, int z, int q) {
-  const PState& P = parts[(int)(sv * 1.0e-30f + 0.5f) - PART_GROUP0];
-  const float rx = (float)(min_image(x - P.r[0], nx) + 0.5 * c_cx[q]);
-  const float ry = (float)(min_image(y - P.r[1], ny) + 0.5 * c_cy[q]);
-  const float rz = (float)(min_image(z - P.r[2], nz) + 0.5 * c_cz[q]);
-  const float wx = (float)P.w[0], wy = (float)P.w[1], wz = (float)P.w[2];
-  const float ux = (float)P.u[0] + (wy * rz - wz * ry), uy = (float)P.u[1] + (wz * rx - wx * rz), uz = (float)P.u[2] + (wx * ry - wy * rx);
-  return (float)c_cx[q] * ux + (float)c_cy[q] * uy + (float)c_cz[q] * uz;
-}
-
-// G33: the stored pair {ts = f* - w, rs = f^r*} of a link into particle `sv` (its phi sentinel) becomes
-// what comes back from the moving surface: f^k <- f^k* - 6 w_q rho^k (c_q . u_b)
-template <int q>
-__device__ __forceinline__ void particle_link(const StepParams& p, float sv, int x, int y, int z, float rho, float rr, float& ts, float& rs) {
-  const float k = -6.0f * wq(q) * particle_cu(p.parts, p.box.nx, p.box.ny, p.box.nz, sv, x, y, z, q);
-  ts = fmaf(k, rho, ts);
-  rs = fmaf(k, rr, rs);
 }
 
 // Solid flags of the 18 neighbours from the bit-packed mask (bit i <=> x + c_i solid).
@@ -695,8 +660,7 @@ __global__ void __launch_bounds__(TX* TY, ((MODE == MODE_AA_ODD && SC) || WALLS 
           // a wall pushing on the fluid, an inlet or an outlet changes the mass.
           if ((smask >> q) & 1u) {
             const float sv = plane(cz(q))[(ly + cy(q)) * R_::BX + lx + cx(q)];
-            if (sv > 4.5f * PHI_SOLID) particle_link<q>(p, sv, x, y, z, rho, rr, ts, rs);   // a rigid particle's node (G33)
-            else if (sv > 1.5f * PHI_SOLID) open_link<q>(p, (int)(sv > 2.5f * PHI_SOLID) + (int)(sv > 3.5f * PHI_SOLID), rho, rr, inv_rho, ux, uy, uz, uu15, ts, rs);
+            if (sv > 1.5f * PHI_SOLID) open_link<q>(p, (int)(sv > 2.5f * PHI_SOLID) + (int)(sv > 3.5f * PHI_SOLID), rho, rr, inv_rho, ux, uy, uz, uu15, ts, rs);
           }
         }
         const Slot s = write_slot<MODE, decltype(bounce)::value, q>(c, smask);
@@ -1146,12 +1110,6 @@ __global__ void __launch_bounds__(TX* TY) k_single(const StepParams p) {
           float rs = 0.f;                      // one component: rho_r is the density
           open_link<q, true>(p, (int)((g2m >> q) & 1u) + 2 * (int)((g3m >> q) & 1u) - 1, rho, rho, inv_rho, ux, uy, uz, uu15, ts, rs);
         }
-        if (b.pid != nullptr && ((smask >> q) & 1u)) {     // a rigid particle's node (G33)
-          const int pi = b.pid[(size_t)(cx(q) > 0 ? wrap_p(x, b.nx) : (cx(q) < 0 ? wrap_m(x, b.nx) : x)) +
-                               (size_t)b.nx * ((size_t)(cy(q) > 0 ? wrap_p(y, b.ny) : (cy(q) < 0 ? wrap_m(y, b.ny) : y)) +
-                                               (size_t)b.ny * (cz(q) > 0 ? wrap_p(z, b.nz) : (cz(q) < 0 ? wrap_m(z, b.nz) : z)))];
-          if (pi >= 0) ts = fmaf(-6.0f * wq(q) * link_cu<q>(b, p.parts[pi], x, y, z), rho, ts);
-        }
       }
       *dst_ptr(p, write_slot<MODE, HAS_SOLID, q>(c, smask)) = ts;
     });
@@ -1533,6 +1491,53 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* red /* [NV][8
     }
 }
 
+// A warp scans the rows row0, row0 + stride, ... of the bounding box pb of a sphere centred at r and
+// queues the nodes with rin2 <= d^2 <= rout2 that pass keep(x, y, z); the costly part, process(site),
+// then runs on 32 queued nodes at a time, all lanes busy.  Which lane treats which node is fixed by
+// the scan order, so sums formed in process() do not depend on the scheduling.  queue: 64 ints of
+// shared memory owned by this warp.
+template <class Keep, class Process>
+__device__ __forceinline__ void scan_shell(const Box& b, const PartBox& pb, const double r[3], float rin2, float rout2,
+                                           int row0, int stride, int* queue, Keep keep, Process process) {
+  const int lane = threadIdx.x & 31, nrows = pb.ext[1] * pb.ext[2];
+  const float cxr = (float)r[0], cyr = (float)r[1], czr = (float)r[2];
+  int qn = 0;
+  for (int row = row0; row < nrows; row += stride) {
+    const int ly = row % pb.ext[1], lz = row / pb.ext[1];
+    int y = pb.lo[1] + ly, z = pb.lo[2] + lz;
+    y += y < 0 ? b.ny : (y >= b.ny ? -b.ny : 0);
+    z += z < 0 ? b.nz : (z >= b.nz ? -b.nz : 0);
+    for (int lx0 = 0; lx0 < pb.ext[0]; lx0 += 32) {
+      const int lx = lx0 + lane;
+      int x = pb.lo[0] + lx;
+      x += x < 0 ? b.nx : (x >= b.nx ? -b.nx : 0);
+      bool pass = lx < pb.ext[0];
+      if (pass) {
+        float fx = (float)x - cxr, fy = (float)y - cyr, fz = (float)z - czr;     // fp32 is enough for the prefilter
+        fx += fx > 0.5f * b.nx ? -(float)b.nx : (fx < -0.5f * b.nx ? (float)b.nx : 0.f);
+        fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
+        fz += fz > 0.5f * b.nz ? -(float)b.nz : (fz < -0.5f * b.nz ? (float)b.nz : 0.f);
+        const float d2 = fx * fx + fy * fy + fz * fz;
+        pass = d2 >= rin2 && d2 <= rout2 && keep(x, y, z);
+      }
+      const unsigned bal = __ballot_sync(0xffffffffu, pass);
+      if (pass) queue[qn + __popc(bal & ((1u << lane) - 1u))] = (int)site_of(b, x, y, z);
+      qn += __popc(bal);
+      __syncwarp();
+      if (qn >= 32) {
+        process(queue[lane]);
+        const int left = qn - 32;
+        const int v = lane < left ? queue[32 + lane] : 0;
+        __syncwarp();
+        if (lane < left) queue[lane] = v;
+        qn = left;
+        __syncwarp();
+      }
+    }
+  }
+  if (lane < qn) process(queue[lane]);
+}
+
 // the nodes of every particle at start-up (G32): solid bit and particle index
 __global__ void __launch_bounds__(256) k_part_raster(const PartParams p) {
   const Box& b = p.box;
@@ -1548,9 +1553,12 @@ __global__ void __launch_bounds__(256) k_part_raster(const PartParams p) {
   }
 }
 
-// G33, the particle's side: the momentum and its moment that the links of time t handed over.  For a
-// link j of the fluid site s into the particle the fused kernel stored g = f* - 6 w rho (c.u_b); the
-// particle receives (f* + g) c_j = (2 g + 6 w rho (c.u_b)) c_j, summed over the components.
+// G33: the link rule at a moving surface and the momentum it hands over.  For a link j of the fluid
+// site s into the particle the hot kernel stored f*_j at the site itself (bounce-back at a wall at
+// rest: the site reads it back along -c_j); here it becomes g^k = f^k* - 6 w_j rho^k (c_j . u_b), rho^k
+// the site's own densities of time t and u_b the surface velocity at the midpoint of the link, and
+// the particle receives (f* + g) c_j, summed over the components.  Every link belongs to one
+// particle, so no two threads touch the same value.
 template <bool TWO>
 __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
   __shared__ double red[6 * 8];
@@ -1582,8 +1590,13 @@ __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
       if (!((mine >> q) & 1u)) continue;
       double rel[3];
       const double cu = link_cu_rt(b, P.r, P.u, P.w, x, y, z, q, rel);
-      const float gt = __ldcg(own_slot<TWO>(p, q, s)) + wq(q);          // reflected total (the T plane holds f - w)
-      const double tot = 2.0 * (double)gt + 6.0 * (double)wq(q) * (double)(rr + rb) * cu;
+      float* sl = own_slot<TWO>(p, q, s);
+      const float k = -6.0f * wq(q) * (float)cu;
+      const float ft = __ldcg(sl);                                       // f* - w (the T plane holds deviations)
+      const float gt = fmaf(k, rr + rb, ft);
+      sl[0] = gt;
+      if constexpr (TWO) sl[1] = fmaf(k, rr, __ldcg(sl + 1));
+      const double tot = ((double)ft + (double)wq(q)) + ((double)gt + (double)wq(q));
       const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
       acc[0] += d[0]; acc[1] += d[1]; acc[2] += d[2];
       acc[3] += rel[1] * d[2] - rel[2] * d[1];
@@ -1591,47 +1604,10 @@ __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
       acc[5] += rel[0] * d[1] - rel[1] * d[0];
     }
   };
-  const float Rin = (float)P.R - 0.01f, Rout = (float)P.R + 1.75f;     // a fluid node with a link into the sphere lies in this shell
-  // A warp scans rows of the box and queues the few shell nodes it finds; the costly part then runs on
-  // 32 queued nodes at a time, all lanes busy.  Which thread adds which node is fixed by the scan
-  // order, so the sums do not depend on the scheduling.
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nrows = pb.ext[1] * pb.ext[2];
-  const float cxr = (float)P.r[0], cyr = (float)P.r[1], czr = (float)P.r[2];
-  int qn = 0;
-  for (int row = wid; row < nrows; row += 8) {
-    const int ly = row % pb.ext[1], lz = row / pb.ext[1];
-    int y = pb.lo[1] + ly, z = pb.lo[2] + lz;
-    y += y < 0 ? b.ny : (y >= b.ny ? -b.ny : 0);
-    z += z < 0 ? b.nz : (z >= b.nz ? -b.nz : 0);
-    for (int lx0 = 0; lx0 < pb.ext[0]; lx0 += 32) {
-      const int lx = lx0 + lane;
-      int x = pb.lo[0] + lx;
-      x += x < 0 ? b.nx : (x >= b.nx ? -b.nx : 0);
-      bool pass = lx < pb.ext[0];
-      if (pass) {
-        float fx = (float)x - cxr, fy = (float)y - cyr, fz = (float)z - czr;     // fp32 is enough for the prefilter
-        fx += fx > 0.5f * b.nx ? -(float)b.nx : (fx < -0.5f * b.nx ? (float)b.nx : 0.f);
-        fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
-        fz += fz > 0.5f * b.nz ? -(float)b.nz : (fz < -0.5f * b.nz ? (float)b.nz : 0.f);
-        const float d2 = fx * fx + fy * fy + fz * fz;
-        pass = d2 >= Rin * Rin && d2 <= Rout * Rout + 0.5f && !solid_at(b, x, y, z);
-      }
-      const unsigned bal = __ballot_sync(0xffffffffu, pass);
-      if (pass) queue[wid][qn + __popc(bal & ((1u << lane) - 1u))] = (int)site_of(b, x, y, z);
-      qn += __popc(bal);
-      __syncwarp();
-      if (qn >= 32) {
-        process(queue[wid][lane]);
-        const int left = qn - 32;
-        const int v = lane < left ? queue[wid][32 + lane] : 0;
-        __syncwarp();
-        if (lane < left) queue[wid][lane] = v;
-        qn = left;
-        __syncwarp();
-      }
-    }
-  }
-  if (lane < qn) process(queue[wid][lane]);
+  // a fluid node with a link into the sphere lies in the shell R .. R + 1.75
+  const float Rin = (float)P.R - 0.01f, Rout = (float)P.R + 1.75f;
+  scan_shell(b, pb, P.r, Rin * Rin, Rout * Rout + 0.5f, threadIdx.x >> 5, 8, queue[threadIdx.x >> 5],
+             [&](int x, int y, int z) { return !solid_at(b, x, y, z); }, process);
   block_sum<6>(acc, red);
   if (threadIdx.x == 0)
     for (int a = 0; a < 3; ++a) { P.F[a] = acc[a]; P.T[a] = acc[3 + a]; }
@@ -1859,6 +1835,32 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
     if (entered) { atomicOr(wd, 1u << (x & 31)); p.pid[s] = me; }
     else { atomicAnd(wd, ~(1u << (x & 31))); p.pid[s] = -1; }
   }
+}
+
+// The phase field around the particles.  k_phase_fwd has written phi(t + 1) from the moments k_fused
+// forwarded, i.e. for walls at rest and the node map of time t.  Near a particle both have changed
+// since: k_part_force rewrote the values that come back from the surface, and a node that entered
+// or left the particle (k_part_remap) changes what its neighbours will read.  So phi is formed
+// again, from the stored populations with the node map of time t + 1, in the shell of nodes around
+// every particle's surface, R - 2 <= d <= R + 2.5 from the new centre: a fluid node with a link into
+// the particle lies within R + sqrt(2) of the old centre, a changed node within R of the old or the
+// new one and its neighbours sqrt(2) further, and the centre moves by less than one node per step;
+// nodes deeper inside keep their sentinel.  Shells of two particles may overlap: both write the same
+// values.  A/B storage (the particles' only one).
+// grid = (particles, slices of the box's rows): the gathers are latency-bound, so the rows of a
+// box are spread over several CTAs.
+__global__ void __launch_bounds__(256) k_part_phi(const StepParams p) {
+  __shared__ int queue[8][64];
+  const Box& b = p.box;
+  const PState& P = p.parts[blockIdx.x];
+  const PartBox pb = part_box(b, P.r, P.R + 2.5);
+  const float Rin = P.R > 2.0 ? (float)P.R - 2.0f : 0.f, Rout = (float)P.R + 2.5f;
+  scan_shell(b, pb, P.r, Rin * Rin, Rout * Rout + 0.5f, blockIdx.y * 8 + (threadIdx.x >> 5), 8 * gridDim.y, queue[threadIdx.x >> 5],
+             [](int, int, int) { return true; },
+             [&](int site) {
+               const int x = site % b.nx, y = (site / b.nx) % b.ny, z = site / (b.nx * b.ny);
+               phase_column<MODE_AB, true, false>(p, x, y, z, z + 1);
+             });
 }
 
 // ----------------------------------------------------------------------------- slab halo

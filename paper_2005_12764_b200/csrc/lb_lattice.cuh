@@ -72,7 +72,6 @@ struct Box {
   long long S;           // sites (allocated)
   const uint32_t* mask;  // bit-packed solid mask (bit x&31 of word row*nxw + x>>5), or nullptr
   const uint32_t* gmask; // wall groups: two more bit planes of the same shape behind each other (group - 1 in binary), or nullptr
-  const int* pid;        // rigid particles (NEXT-4): particle index of a particle node, -1 elsewhere; or nullptr
 };
 
 // State of one rigid spherical particle (the paper's section 6, Eq. 15).  Double
@@ -88,8 +87,6 @@ struct PState {
   double ro[3], uo[3], wo[3];      // r, u, w before the last move (the node changes undo links made with them, G36)
 };
 
-constexpr int PART_GROUP0 = 5;     // the phi sentinel of a particle node is 1e30 x (5 + particle index)
-
 __device__ __forceinline__ bool solid_at(const Box& b, int x, int y, int z) {
   return (b.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)] >> (x & 31)) & 1u;
 }
@@ -103,14 +100,8 @@ __device__ __forceinline__ int wall_group_at(const Box& b, int x, int y, int z) 
   return 1 + (int)g2 + 2 * (int)g3;
 }
 
-// what the phi sentinel of a solid site encodes: the wall group, or 5 + the particle index
-__device__ __forceinline__ int sentinel_code(const Box& b, int x, int y, int z) {
-  if (b.pid) {
-    const int p = b.pid[(size_t)x + (size_t)b.nx * ((size_t)y + (size_t)b.ny * z)];
-    if (p >= 0) return PART_GROUP0 + p;
-  }
-  return wall_group_at(b, x, y, z);
-}
+// what the phi sentinel of a solid site encodes: the wall group (a particle's node counts as a wall at rest)
+__device__ __forceinline__ int sentinel_code(const Box& b, int x, int y, int z) { return wall_group_at(b, x, y, z); }
 
 __device__ __forceinline__ int wrap_m(int a, int n) { return a == 0 ? n - 1 : a - 1; }
 __device__ __forceinline__ int wrap_p(int a, int n) { return a == n - 1 ? 0 : a + 1; }
