@@ -288,7 +288,12 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
             sim.set_tuning(**TUNE)
     sim.init(d_rr, d_rb, d_u)
     mass0 = sim.check_state()
-    sim.set_profiling(7)      # every 7th step (odd, so that both AA parities are sampled) is timed kernel by kernel (CUDA events on the stream)
+    # Every 7th step (odd, so that both AA parities are sampled) is timed kernel by kernel (CUDA events
+    # on the stream).  A box of at most 2^21 sites is stepped by replaying a CUDA graph (include/lb.h,
+    # lb_set_tuning "graph"), which event records inside the step would switch off: there the timed
+    # region runs without them and the kernels are timed in a pass of the same length right after it.
+    graphed = (not slabs) and w.sites <= (1 << 21) and TUNE.get("graph", -1) != 0 and w.info.get("particles") is None
+    sim.set_profiling(0 if graphed else 7)
     sim.step(Wu)
     torch.cuda.synchronize()
     if world > 1:
@@ -313,9 +318,15 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
         remeasured = True
         time.sleep(5.0)
     ms = ev0.elapsed_time(ev1)
+    if graphed:
+        sim.set_profiling(7)
+        sim.step(K)
+        torch.cuda.synchronize()
     ms_k2 = sim.last_step_ms(1)
     ms_k1 = sim.last_step_ms(2) if two else 0.0
     kernel_timing = "CUDA events around every 7th step of the timed region"
+    if graphed:
+        kernel_timing = "CUDA events around every 7th step of a pass of the same length right after the timed region (which replays a CUDA graph of 16 steps)"
     if ms_k2 is None:        # slabs: the fused kernel runs as three launches per step; the whole step stands in
         ms_k2, ms_k1 = ms / K, None
         kernel_timing = "slab phases are not timed kernel by kernel: kernel_ms is the whole step (boundary + interior bricks, phase field, packing, exchange)"

@@ -278,9 +278,16 @@ int lb_set_particle_force(lb_handle h, int i, const double* F, const double* T);
 int lb_get_particles(lb_handle h, lb_particle* state, double* force);
 
 /* Tuning of lb_step.  key = "forward": 1 (default) = the fused kernel forwards the moments of the
- * next state and a light kernel turns them into phi; 0 = a full
- * phase-field sweep over the populations before every step (same phi to ~1e-8).  "zc": z planes
- * per CTA, 0 = automatic.  Returns LB_EINVAL for an unknown key. */
+ * next state and a light kernel turns them into phi, except in
+ * boxes so small that a CTA holds a single plane, where the full sweep is faster; 2 = the same
+ * without that exception; 0 = a full phase-field sweep over the populations before every step
+ * (same phi to ~1e-8).  "zc": z planes
+ * per CTA, 0 = automatic.  "graph": lb_step replays a CUDA graph of 16 time steps where it can (no
+ * profiling, no particles, not the first two steps, not while the caller's stream is capturing):
+ * -1 (default) = for boxes of at most 2^21 sites, whose step is bounded by launch latency, 0 = never,
+ * 1 = for every box.  The graph is captured on a stream of the handle's own and launched into the
+ * handle's stream; it is rebuilt when any parameter, buffer or the storage parity changes; results
+ * are bit-identical to plain launches.  Returns LB_EINVAL for an unknown key. */
 int lb_set_tuning(lb_handle h, const char* key, int value);
 
 /* Number of kernel launches this handle has made so far (for the harness' gpu_launches). */

@@ -132,6 +132,13 @@ struct lb_handle_s {
   int p_mobile = 1, p_lub = 0;
   double p_K = 0.0, p_hc = 0.0;
   int tune_zc = 0;           // z planes per CTA (0 = automatic)
+  // CUDA graph of GRAPH_STEPS time steps for boxes whose step is bounded by launch latency (lb_step)
+  int graph = -1;            // tuning key "graph": -1 = automatic (small boxes), 0 = never, 1 = whenever possible
+  cudaGraphExec_t gexec = nullptr;
+  cudaStream_t gstream = nullptr;          // capture stream (the caller's may be the legacy default stream, which cannot capture)
+  std::vector<unsigned char> gkey;         // everything the captured launches depend on (graph_key)
+  long long graph_kernels = 0;             // kernel nodes in the graph
+  bool graph_failed = false;               // capture or instantiation failed once: not tried again
   int sm_count = 0;          // SMs of the handle's device (0: not asked yet)
   double* chk = nullptr;     // state check (lb_check_state): {sum rho_r, sum rho_b, non-finite count}
   long long steps_done = 0;  // time steps since lb_init
@@ -169,6 +176,7 @@ int fail(lb_handle h, int code, const std::string& msg) {
 }
 
 constexpr long long CHECK_EVERY = 1000;   // steps between two state checks inside lb_step (G23)
+constexpr long long GRAPH_AUTO_SITES = 1LL << 21;     // boxes up to 128^3 count as bounded by launch latency (tuning key "graph")
 
 int cuda_fail(lb_handle h, cudaError_t e, const char* what) {
   cudaGetLastError();
@@ -224,6 +232,7 @@ namespace {
 
 StepParams make_step_params(lb_handle h, const float* src, float* dst, int zc, int z0 = -1, int z1 = -1) {
   StepParams p;
+  memset(&p, 0, sizeof(p));      // (padding too: graph_key compares the bytes)
   p.z0 = z0 < 0 ? h->zlo() : z0;
   p.z1 = z1 < 0 ? h->zhi() : z1;
   p.src = src; p.dst = dst; p.phi = h->phi;
@@ -460,6 +469,16 @@ void flip(lb_handle h) {
   h->steps_done++;
 }
 
+// Does phi(t + 1) come from the forwarded moments (k_phase_fwd) in lb_step?  Not for bricks of one
+// plane, which pick_zc gives a box far smaller than one wave of CTAs: there every plane is both z
+// faces of its brick, k_phase_fwd gathers most populations anyway (four sites per thread, a quarter
+// of its lanes busy at nx = 32), and the full sweep k_phase (one site per thread) is faster: 32^3
+// 11.2 -> 7.1 us per step.  With two planes per brick forwarding still wins (128 x 32 x 32: 18.1
+// against 22.6 us).  "forward" = 2 forwards regardless.
+bool forwarding(lb_handle h) {
+  return h->two && h->forward && (h->forward == 2 || h->gz || pick_zc(h) > 1);
+}
+
 PartParams make_part_params(lb_handle h) {
   PartParams q;
   memset(&q, 0, sizeof(q));
@@ -493,7 +512,7 @@ void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
   if (h->np > 0) {
     // phi(t + 1) from the forwarded moments first (they belong to the node map of time t), then the
     // particles, then phi again in the shells around them (k_part_phi)
-    const bool fwd = h->two && h->forward;
+    const bool fwd = forwarding(h);
     if (fwd) launch_phase_forward(h, h->zlo(), h->zhi());
     run_particles(h);
     if (fwd) {
@@ -508,7 +527,7 @@ void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
     }
     flip(h);
     h->phi_current = fwd;
-  } else if (h->two && h->forward) {
+  } else if (forwarding(h)) {
     launch_phase_forward(h, h->zlo(), h->zhi());
     flip(h);
     h->phi_current = true;
@@ -651,6 +670,8 @@ void lb_destroy(lb_handle h) {
   DeviceGuard guard(h->device);
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
   for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk, (void*)h->parts, (void*)h->pid, (void*)h->mask_static, (void*)h->povf}) dev_free(h->al, q);
+  if (h->gexec) cudaGraphExecDestroy(h->gexec);
+  if (h->gstream) cudaStreamDestroy(h->gstream);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
   for (cudaEvent_t e : h->ev_k) cudaEventDestroy(e);
   cudaGetLastError();
@@ -985,6 +1006,65 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   return LB_OK;
 }
 
+namespace {
+
+// A box that one wave of CTAs covers is bounded by the latency of its two dependent launches per step
+// (C1, 32^3: ~8 us per launch), not by memory traffic.  For such boxes lb_step replays a CUDA graph
+// of GRAPH_STEPS steps: the launches then cost the GPU front end a fraction of a stream launch
+// and the host one call per GRAPH_STEPS steps.
+constexpr int GRAPH_STEPS = 16;                       // even: the A/B and in-place parities return to where they were
+
+// Everything the captured launches depend on.  The graph is rebuilt when any of it changes.
+std::vector<unsigned char> graph_key(lb_handle h) {
+  const StepParams p = make_step_params(h, h->cur_buf(), next_buf(h), pick_zc(h), h->zlo(), h->zhi());
+  const long long extra[] = {h->model, h->has_solid, h->has_moving, h->forward, h->storage, h->cur, h->aa_odd, h->two,
+                             (long long)(size_t)h->mom, (long long)(size_t)h->mask, (long long)(size_t)h->buf[0], (long long)(size_t)h->buf[1]};
+  std::vector<unsigned char> k(sizeof(p) + sizeof(extra));
+  memcpy(k.data(), &p, sizeof(p));
+  memcpy(k.data() + sizeof(p), extra, sizeof(extra));
+  return k;
+}
+
+bool graph_eligible(lb_handle h, int remaining) {
+  if (h->graph == 0 || h->graph_failed || remaining < GRAPH_STEPS) return false;
+  if (h->graph < 0 && h->Sx > GRAPH_AUTO_SITES) return false;
+  if (h->profiling || h->np > 0 || h->gz) return false;
+  // the host flags must come back to where they were: with forwarding phi is current at every step's
+  // start (the first step after lb_init / lb_set_populations runs K1 by itself), without it never
+  if (h->two && forwarding(h) != h->phi_current) return false;
+  if (h->steps_done < 2) return false;                              // first launches set function attributes
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(h->stream, &st) != cudaSuccess) { cudaGetLastError(); return false; }
+  return st == cudaStreamCaptureStatusNone;                         // the caller is capturing lb_step itself: plain launches
+}
+
+// Captures GRAPH_STEPS steps from the current parity.  Leaves the handle's host state as it was.
+bool graph_build(lb_handle h, const std::vector<unsigned char>& key) {
+  if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+  if (!h->gstream && cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return false; }
+  const cudaStream_t user = h->stream;
+  const long long l0 = h->launches, s0 = h->steps_done;
+  const int cur0 = h->cur, odd0 = h->aa_odd;
+  const bool pc0 = h->phi_current, pg0 = h->phi_ghost_ok;
+  h->stream = h->gstream;
+  cudaGraph_t g = nullptr;
+  bool ok = cudaStreamBeginCapture(h->gstream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (ok) {
+    for (int t = 0; t < GRAPH_STEPS; ++t) { run_phase(h); run_collide(h); }
+    ok = cudaStreamEndCapture(h->gstream, &g) == cudaSuccess && g != nullptr;
+  }
+  h->stream = user;
+  h->graph_kernels = h->launches - l0;
+  h->launches = l0; h->steps_done = s0; h->cur = cur0; h->aa_odd = odd0; h->phi_current = pc0; h->phi_ghost_ok = pg0;
+  if (ok) ok = cudaGraphInstantiate(&h->gexec, g, 0) == cudaSuccess;
+  if (g) cudaGraphDestroy(g);
+  if (!ok) { cudaGetLastError(); h->gexec = nullptr; return false; }
+  h->gkey = key;
+  return true;
+}
+
+}  // namespace
+
 int lb_step(lb_handle h, int nsteps) {
   if (!h || nsteps < 0) return fail(h, LB_EINVAL, "nsteps must be >= 0");
   DeviceGuard guard(h->device);
@@ -1003,6 +1083,29 @@ int lb_step(lb_handle h, int nsteps) {
   h->ev_steps = nprof;
   cudaEventRecord(h->ev_step[0], h->stream);
   for (int t = 0; t < nsteps; ++t) {
+    // replays of the step graph, as many as fit before the end of the call and the next state check
+    if (graph_eligible(h, nsteps - t)) {
+      const long long room = std::min<long long>(nsteps - t, CHECK_EVERY - (h->steps_done - h->last_check));
+      const int reps = (int)(room / GRAPH_STEPS);
+      if (reps > 0) {
+        const std::vector<unsigned char> key = graph_key(h);
+        if ((h->gexec && key == h->gkey) || graph_build(h, key)) {
+          cudaError_t e = cudaSuccess;
+          for (int r = 0; r < reps && e == cudaSuccess; ++r) e = cudaGraphLaunch(h->gexec, h->stream);
+          if (e != cudaSuccess) return cuda_fail(h, e, "lb_step: graph launch");
+          h->launches += (long long)reps * h->graph_kernels;
+          h->steps_done += (long long)reps * GRAPH_STEPS;
+          t += reps * GRAPH_STEPS - 1;         // (the parities are where they were: GRAPH_STEPS is even)
+          if (h->steps_done - h->last_check >= CHECK_EVERY) {
+            int rc = check_launch(h, "lb_step");
+            if (!rc) rc = state_check(h, nullptr, nullptr);
+            if (rc) { cudaEventRecord(h->ev_step[1], h->stream); return rc; }
+          }
+          continue;
+        }
+        h->graph_failed = true;                // stays on plain launches
+      }
+    }
     const bool prof = stride > 0 && t % stride == 0;
     const int k = prof ? 4 * (t / stride) : 0;
     if (prof) cudaEventRecord(h->ev_k[k + 0], h->stream);
@@ -1324,8 +1427,9 @@ const char* lb_last_error(lb_handle h) { return h ? h->err.c_str() : g_create_er
 int lb_set_tuning(lb_handle h, const char* key, int value) {
   if (!h || !key) return LB_EINVAL;
   const std::string k(key);
-  if (k == "forward") h->forward = value ? 1 : 0;
+  if (k == "forward") h->forward = value < 0 || value > 2 ? 1 : value;
   else if (k == "zc") h->tune_zc = value;
+  else if (k == "graph") h->graph = value < 0 ? -1 : (value ? 1 : 0);
   else return fail(h, LB_EINVAL, "unknown tuning key: " + k);
   return LB_OK;
 }

@@ -256,13 +256,32 @@ def test_forwarding_brick_sizes_agree(lbmod):
     ref = None
     for zc in (0, 1, 5, 96):
         sim = pu.make_gpu(lbmod, w)
-        sim.set_tuning(zc=zc)
+        sim.set_tuning(zc=zc, forward=2)              # (2: also with one plane per brick, where lb_step would sweep)
         sim.step(3)
         phi = sim.get_phi()
         if ref is None:
             ref = phi
         else:
             assert np.abs(phi - ref).max() < 1e-6, (zc, np.abs(phi - ref).max())
+
+
+def test_single_plane_bricks_take_the_full_sweep(lbmod):
+    """A box far smaller than one wave of CTAs gets bricks of one plane, and lb_step then forms phi
+    by the full sweep instead of forwarding (lb_set_tuning "forward"): one launch per step more
+    than the count of k_fused launches either way, and the same phi as forwarding to rounding."""
+    w = W.get("c1")
+    phis, launches = [], []
+    for fwd in (1, 2, 0):
+        sim = pu.make_gpu(lbmod, w)
+        sim.set_tuning(forward=fwd, graph=0)
+        sim.step(1)
+        l0 = sim.launch_count()
+        sim.step(20)
+        launches.append(sim.launch_count() - l0)
+        phis.append(sim.get_phi())
+    assert launches[0] == launches[1] == launches[2] == 40
+    assert np.array_equal(phis[0], phis[2])           # default on this box = the full sweep
+    assert np.abs(phis[0] - phis[1]).max() < 2e-6
 
 
 def test_full_size_c5_sampled_macros_and_conservation(lbmod, lbo):
@@ -962,3 +981,29 @@ def test_state_check_reports_nan_and_masses(lbmod):
     sim.step(3)
     mr, mb = sim.check_state()
     assert abs(mr - w2.sites) / w2.sites < 1e-6 and mb == 0.0
+
+
+@pytest.mark.parametrize("name,storage", [("c1", "ab"), ("c1", "aa"), ("c4-mini", "ab"), ("c4-mini", "aa"), ("c2-mini", "ab")])
+def test_step_graph_is_bit_identical_to_plain_launches(lbmod, name, storage):
+    """lb_set_tuning("graph"): lb_step replays a CUDA graph of 16 steps for small boxes.  Same bits,
+    same launch count and the same state check as plain launches; a changed parameter (here the
+    body force) between two calls rebuilds the graph."""
+    w = W.get(name)
+    two = w.rho_b is not None
+    sims = {}
+    for graph in (0, 1):
+        sim = pu.make_gpu(lbmod, w, storage)
+        sim.set_tuning(graph=graph)
+        sim.step(3)                                   # plain in both (the first steps), odd parity next
+        sim.step(37)                                  # 2 replays + 5 plain steps
+        sim.set_body_force(2e-5, -1e-5, 3e-5)
+        sim.step(64)                                  # new key: rebuilt, 4 replays
+        sim.step(1000)                                # crosses the state check at 1000 steps
+        sims[graph] = sim
+    assert sims[0].launch_count() == sims[1].launch_count()
+    for k in range(2 if two else 1):
+        assert np.array_equal(sims[0].get_populations(k), sims[1].get_populations(k))
+    if two:
+        assert np.array_equal(sims[0].get_phi(), sims[1].get_phi())
+        a, b = sims[0].check_state(), sims[1].check_state()
+        assert abs(a[0] - b[0]) <= 1e-12 * a[0] and abs(a[1] - b[1]) <= 1e-12 * a[1]
