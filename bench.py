@@ -235,6 +235,13 @@ class SlabRunner:
 
     def __init__(self, w, storage, rank, world):
         from paper_2005_12764_b200 import slab
+        if w.info.get("particles") is not None and world > 1:
+            # rigid particles are replicated data (every rank holds all of them): the taller box holds the
+            # workload's particles once per period
+            import dataclasses
+            parts = np.asarray(w.info["particles"], dtype=np.float64)
+            tiled = np.concatenate([parts + np.array([0, 0, k * w.nz] + [0] * (parts.shape[1] - 3)) for k in range(world)])
+            w = dataclasses.replace(w, info=dict(w.info, particles=tiled))
         self.ds = slab.DistributedSlab(slab.Slab.from_workload(w, rank * w.nz, w.nz, storage, nz_global=world * w.nz), rank, world)
         self.sim = self.ds.slab.sim
 

@@ -241,6 +241,32 @@ int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi);
 int lb_slab_pack_phi(lb_handle h, void* send_lo, void* send_hi);
 int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi);
 
+/* Particles in a slab: "replicated data" ("each process stores the physical
+ * variables of all particles ... a global reduction ... each process solves the equation of motion
+ * for all particles").  Every slab handle is given ALL particles (lb_set_particles, positions in
+ * the coordinates of the whole box) and keeps the same state as every other; per step two sums over
+ * the slabs are the caller's (an all-reduce of 6 doubles per particle each):
+ *   lb_slab_begin(h, send_lo, send_hi)   with particles: the fused kernel on EVERY brick, the link
+ *                                        rule (G33) on the slab's own sites and its share of the link
+ *                                        sums; nothing is packed yet (the particles still rewrite
+ *                                        stored values of the boundary planes), so there is no overlap
+ *   lb_slab_part_get(h, d_sums)          the slab's share [np][6] = (F, T) -> caller's DEVICE buffer
+ *   [caller: sum over the slabs]
+ *   lb_slab_part_put(h, d_sums)          the totals; pair forces, leapfrog step, node changes of the
+ *                                        slab's own sites (G36), its share of their impulses
+ *   lb_slab_part_get(h, d_sums)          that share [np][6] = (dU, dL)
+ *   [caller: sum over the slabs]
+ *   lb_slab_part_put(h, d_sums)          the totals go to the particles; the population messages
+ *                                        given to lb_slab_begin are packed now
+ *   [caller: exchange the population messages]   lb_slab_interior, lb_slab_end as above
+ *   (lb_slab_end also forms phi again around the particles)
+ * and the phi messages carry, behind the phi planes, rho_r and rho_b of the boundary plane (G36 fills
+ * a node that leaves a particle at the mean densities of its neighbours, which may lie in a ghost
+ * plane): lb_slab_halo_bytes counts them, and with one component the phi calls then carry only those.
+ * The result equals the undivided box up to the order of the two sums.  LB_ESTATE: out of order. */
+int lb_slab_part_get(lb_handle h, double* d_sums);
+int lb_slab_part_put(lb_handle h, const double* d_sums);
+
 /* ---- rigid spherical particles (the paper's section 6) --------------------
  * "colloidal particles are represented as rigid spheres of radius R, moving under the effect of a
  * total force F_p and torque T_p ... dr_p/dt = u_p, m_p du_p/dt = F_p, I_p dw_p/dt = T_p (Eq. 15) ...

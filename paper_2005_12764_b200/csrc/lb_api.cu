@@ -129,6 +129,12 @@ struct lb_handle_s {
   uint32_t* mask_static = nullptr;  // the walls of lb_set_geometry alone (the live mask also holds the particle nodes)
   bool user_solid = false, user_moving = false;
   int* povf = nullptr;              // k_part_remap overflow flag
+  // particles in a slab (replicated data): lb_slab_part_get / lb_slab_part_put
+  double* pred = nullptr;           // [np][6] this slab's share of the link sums, then of the node-change impulses
+  double* ptot = nullptr;           // [np][6] the sums over all slabs, as the caller gave them back
+  float* ghost_rho = nullptr;       // [2 faces][2 components][ny * nx] densities in the ghost planes (lb_slab_unpack_phi)
+  int part_stage = 0;               // 0 = none pending, 1 = link sums wait for their total, 2 = impulses wait for theirs
+  void* pend_send[2] = {nullptr, nullptr};   // the population messages lb_slab_begin was given, packed once the particles have moved
   int p_mobile = 1, p_lub = 0;
   double p_K = 0.0, p_hc = 0.0;
   int tune_zc = 0;           // z planes per CTA (0 = automatic)
@@ -156,6 +162,7 @@ struct lb_handle_s {
     Box b;
     b.nx = nx; b.ny = ny; b.nz = nza();
     b.zlo = zlo(); b.zhi = zhi(); b.zper = gz == 0;
+    b.gnz = gz ? slab_nzg : nz; b.zoff = gz ? slab_z0 - gz : 0;
     b.nxw = (nx + 31) / 32;
     b.S = S;
     b.mask = has_solid ? mask : nullptr;
@@ -489,20 +496,49 @@ PartParams make_part_params(lb_handle h) {
   q.mobile = h->p_mobile; q.K = h->p_K; q.hc = h->p_hc; q.lub = h->p_lub;
   q.mu = ((double)h->par.tau_r - 0.5) / 3.0;
   q.overflow = h->povf;
+  q.part_out = h->gz ? h->pred : nullptr;
+  q.tot_in = h->gz ? h->ptot : nullptr;
+  q.ghost_rho = h->ghost_rho;
   return q;
 }
 
 // The particles' part of a step (Eq. 15), between the fused kernel, which applied
 // the link rule to what it stored, and the flip: momentum exchange, leapfrog, node changes.
-void run_particles(lb_handle h) {
+// In three parts, because a slab needs the sums over all slabs in between (lb_slab_part_put).
+void particles_force(lb_handle h) {
   const PartParams q = make_part_params(h);
   if (h->two) k_part_force<true><<<h->np, 256, 0, h->stream>>>(q);
   else k_part_force<false><<<h->np, 256, 0, h->stream>>>(q);
+  h->launches++;
+}
+void particles_move(lb_handle h) {
+  const PartParams q = make_part_params(h);
   k_part_pair<<<(h->np + 7) / 8, 256, 0, h->stream>>>(q);
   k_part_integrate<<<(h->np + 127) / 128, 128, 0, h->stream>>>(q);
+  if (h->gz) cudaMemsetAsync(h->pred, 0, (size_t)h->np * 6 * sizeof(double), h->stream);   // (particles held in place list no changes)
   if (h->two) k_part_remap<true><<<h->np, 256, 0, h->stream>>>(q);
   else k_part_remap<false><<<h->np, 256, 0, h->stream>>>(q);
-  h->launches += 4;
+  h->launches += 3;
+}
+void particles_apply(lb_handle h) {     // slabs only
+  const PartParams q = make_part_params(h);
+  k_part_apply<<<(h->np + 127) / 128, 128, 0, h->stream>>>(q);
+  h->launches++;
+}
+void run_particles(lb_handle h) {
+  particles_force(h);
+  particles_move(h);
+}
+// phi again in the shells around the particles, for the state launch_collide has written (before flip())
+void particles_phi(lb_handle h) {
+  const StepParams q = make_step_params(h, next_buf(h), nullptr, pick_zc(h), h->zlo(), h->zhi());
+  // rows of the largest particle's box, 32 per CTA (4 per warp)
+  double rmax = 0.0;
+  for (const PState& P : h->parts_host) rmax = std::max(rmax, P.R);
+  const int ext = 2 * (int)std::ceil(rmax + 2.5) + 2;
+  const int slices = std::max(1, std::min(64, (ext * ext + 31) / 32));
+  k_part_phi<<<dim3(h->np, slices), 256, 0, h->stream>>>(q);
+  h->launches++;
 }
 
 // One whole step of a box that is periodic in z: K2 (+ K1f) or K2s
@@ -515,16 +551,7 @@ void run_collide(lb_handle h, cudaEvent_t after_k2 = nullptr) {
     const bool fwd = forwarding(h);
     if (fwd) launch_phase_forward(h, h->zlo(), h->zhi());
     run_particles(h);
-    if (fwd) {
-      const StepParams q = make_step_params(h, next_buf(h), nullptr, pick_zc(h), h->zlo(), h->zhi());
-      // rows of the largest particle's box, 32 per CTA (4 per warp)
-      double rmax = 0.0;
-      for (const PState& P : h->parts_host) rmax = std::max(rmax, P.R);
-      const int ext = 2 * (int)std::ceil(rmax + 2.5) + 2;
-      const int slices = std::max(1, std::min(64, (ext * ext + 31) / 32));
-      k_part_phi<<<dim3(h->np, slices), 256, 0, h->stream>>>(q);
-      h->launches++;
-    }
+    if (fwd) particles_phi(h);
     flip(h);
     h->phi_current = fwd;
   } else if (forwarding(h)) {
@@ -669,7 +696,7 @@ void lb_destroy(lb_handle h) {
   if (!h) return;
   DeviceGuard guard(h->device);
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
-  for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk, (void*)h->parts, (void*)h->pid, (void*)h->mask_static, (void*)h->povf}) dev_free(h->al, q);
+  for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk, (void*)h->parts, (void*)h->pid, (void*)h->mask_static, (void*)h->povf, (void*)h->pred, (void*)h->ptot, (void*)h->ghost_rho}) dev_free(h->al, q);
   if (h->gexec) cudaGraphExecDestroy(h->gexec);
   if (h->gstream) cudaStreamDestroy(h->gstream);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
@@ -866,7 +893,8 @@ namespace {
 int init_particles(lb_handle h) {
   if (h->storage != 0) return fail(h, LB_ESTATE, "particles need A/B storage");
   if (h->model != 0) return fail(h, LB_ESTATE, "particles are built for the colour-gradient model and for one component");
-  if (h->gz) return fail(h, LB_ESTATE, "particles are not built for slabs");
+  // a slab with its two ghost planes must not hold any plane of the box twice (a ring of one slab would)
+  if (h->gz && h->nz + 2 > h->slab_nzg) return fail(h, LB_ESTATE, "particles in a slab need nz + 2 <= nz_global (at least two slabs)");
   const Box b0 = h->box();
   const size_t nwords = (size_t)b0.nxw * h->ny * h->nza();
   const size_t mb = (3 * nwords + 1) * 4;
@@ -895,6 +923,18 @@ int init_particles(lb_handle h) {
     if (!h->parts) return fail(h, LB_ENOMEM, "particle state allocation failed");
     h->bytes += (size_t)h->np * sizeof(PState);
   }
+  if (h->gz && !h->pred) {     // a slab: the buffers of the two sums over the slabs, the densities of the ghost planes
+    const size_t rb = (size_t)h->np * 6 * sizeof(double), gb = (size_t)4 * h->nx * h->ny * sizeof(float);
+    h->pred = static_cast<double*>(dev_alloc(h->al, rb));
+    h->ptot = static_cast<double*>(dev_alloc(h->al, rb));
+    h->ghost_rho = static_cast<float*>(dev_alloc(h->al, gb));
+    if (!h->pred || !h->ptot || !h->ghost_rho) return fail(h, LB_ENOMEM, "particle reduction buffer allocation failed");
+    h->bytes += 2 * rb + gb;
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->pred, 0, rb, h->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->ptot, 0, rb, h->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->ghost_rho, 0, gb, h->stream);
+  }
+  h->part_stage = 0;
   if (e == cudaSuccess) e = cudaMemcpyAsync(h->mask, h->mask_static, nwords * 4, cudaMemcpyDeviceToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->pid, 0xff, (size_t)h->S * sizeof(int), h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->povf, 0, sizeof(int), h->stream);
@@ -922,7 +962,7 @@ int lb_set_particles(lb_handle h, int n, const lb_particle* p) {
     for (int a = 0; a < 4; ++a) P.q[a] = p[i].q[a];
     P.R = p[i].R; P.mass = p[i].mass;
     if (!(P.R > 0.0) || !(P.mass > 0.0)) { h->parts_host.clear(); h->np = 0; return fail(h, LB_EINVAL, "particle radius and mass must be positive"); }
-    if (2.0 * P.R + 4.0 > h->nx || 2.0 * P.R + 4.0 > h->ny || 2.0 * P.R + 4.0 > h->nz) { h->parts_host.clear(); h->np = 0; return fail(h, LB_EINVAL, "particle too large for the box"); }
+    if (2.0 * P.R + 4.0 > h->nx || 2.0 * P.R + 4.0 > h->ny || 2.0 * P.R + 4.0 > (h->gz ? h->slab_nzg : h->nz)) { h->parts_host.clear(); h->np = 0; return fail(h, LB_EINVAL, "particle too large for the box"); }
     P.inertia = 0.4 * P.mass * P.R * P.R;
   }
   h->np = n;
@@ -1304,6 +1344,12 @@ void slab_copy_populations(lb_handle h, float* buf, const SlabBlocks& b, void* m
 int slab_phi_halo(lb_handle h) { return (h->model == 0 && h->par.A_nc != 0.f) ? H_MAX_NC : 1; }
 size_t slab_phi_plane_floats(lb_handle h) { return (size_t)(h->nx + 2 * HALO) * (h->ny + 2 * HALO); }
 
+// the phi part of a phi message, and the densities of the boundary plane behind it (runs with particles)
+size_t slab_phi_bytes(lb_handle h) {
+  return h->two ? (size_t)(h->model == 1 ? 2 : 1) * slab_phi_halo(h) * slab_phi_plane_floats(h) * sizeof(float) : 0;
+}
+size_t slab_rho_bytes(lb_handle h) { return h->np > 0 ? (size_t)2 * h->nx * h->ny * sizeof(float) : 0; }
+
 int slab_ready(lb_handle h, int phase, const char* what) {
   if (!h) return LB_EINVAL;
   if (!h->gz) return fail(h, LB_ESTATE, std::string(what) + ": not a slab (lb_set_slab)");
@@ -1332,7 +1378,7 @@ int lb_slab_halo_bytes(lb_handle h, size_t* pop_bytes, size_t* phi_bytes) {
   if (!h) return LB_EINVAL;
   if (!h->gz || !h->inited) return fail(h, LB_ESTATE, "lb_slab_halo_bytes needs an initialised slab");
   if (pop_bytes) *pop_bytes = (size_t)5 * h->nx * h->ny * (h->two ? 2 : 1) * sizeof(float);
-  if (phi_bytes) *phi_bytes = h->two ? (size_t)(h->model == 1 ? 2 : 1) * slab_phi_halo(h) * slab_phi_plane_floats(h) * sizeof(float) : 0;
+  if (phi_bytes) *phi_bytes = slab_phi_bytes(h) + slab_rho_bytes(h);
   return LB_OK;
 }
 
@@ -1344,6 +1390,18 @@ int lb_slab_begin(lb_handle h, void* send_lo, void* send_hi) {
     return fail(h, LB_ESTATE, "lb_slab_begin: the phi ghost planes are stale (lb_slab_pack_phi, exchange, lb_slab_unpack_phi first)");
   if (h->two && !h->forward) return fail(h, LB_ESTATE, "slabs need moment forwarding (lb_set_tuning forward = 1)");
   DeviceGuard guard(h->device);
+  if (h->np > 0) {
+    // Particles (replicated data): the link rule and the node changes rewrite stored
+    // values of the boundary planes, so nothing is packed before the particles have moved.  All
+    // bricks now, then this slab's share of the link sums; the messages are packed by the second
+    // lb_slab_part_put.
+    launch_collide(h, h->zlo(), h->zhi());
+    particles_force(h);
+    h->part_stage = 1;
+    h->pend_send[0] = send_lo; h->pend_send[1] = send_hi;
+    h->slab_phase = 1;
+    return check_launch(h, "lb_slab_begin");
+  }
   const SlabBricks b = slab_bricks(h);
   launch_collide(h, b.first0, b.first1);
   launch_collide(h, b.last0, b.last1);
@@ -1356,8 +1414,10 @@ int lb_slab_interior(lb_handle h) {
   int rc = slab_ready(h, 1, "lb_slab_interior");
   if (rc) return rc;
   DeviceGuard guard(h->device);
+  if (h->np > 0 && h->part_stage != 0)
+    return fail(h, LB_ESTATE, "lb_slab_interior: the particles wait for their sums (lb_slab_part_get / lb_slab_part_put, twice per step)");
   const SlabBricks b = slab_bricks(h);
-  launch_collide(h, b.mid0, b.mid1);
+  if (h->np == 0) launch_collide(h, b.mid0, b.mid1);         // (with particles lb_slab_begin has run every brick)
   const int H = slab_phi_halo(h);
   launch_phase_forward(h, h->zlo() + H, h->zhi() - H);     // the planes whose phi does not wait for the halo
   h->slab_phase = 2;
@@ -1374,6 +1434,7 @@ int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi) {
   const int H = slab_phi_halo(h);
   launch_phase_forward(h, h->zlo(), std::min(h->zlo() + H, h->zhi()));
   launch_phase_forward(h, std::max(h->zhi() - H, h->zlo() + H), h->zhi());
+  if (h->np > 0 && h->two) particles_phi(h);                 // phi again around the particles (own planes)
   flip(h);
   h->phi_current = h->two;
   h->phi_ghost_ok = false;
@@ -1386,9 +1447,19 @@ int lb_slab_end(lb_handle h, const void* recv_lo, const void* recv_hi) {
 int lb_slab_pack_phi(lb_handle h, void* send_lo, void* send_hi) {
   int rc = slab_ready(h, 0, "lb_slab_pack_phi");
   if (rc) return rc;
-  if (!h->two) return LB_OK;                       // one component: no phase field
+  if (!h->two && h->np == 0) return LB_OK;         // one component: no phase field
   if ((rc = slab_msg_check(h, send_lo, send_hi))) return rc;
   DeviceGuard guard(h->device);
+  if (h->np > 0) {                                 // the densities of the boundary planes, behind the phi part
+    const PartParams q = make_part_params(h);
+    float* lo = reinterpret_cast<float*>(static_cast<char*>(send_lo) + slab_phi_bytes(h));
+    float* hi = reinterpret_cast<float*>(static_cast<char*>(send_hi) + slab_phi_bytes(h));
+    const dim3 grid((unsigned)(((size_t)h->nx * h->ny + 255) / 256), 2);
+    if (h->two) k_slab_rho<true><<<grid, 256, 0, h->stream>>>(q, lo, hi);
+    else k_slab_rho<false><<<grid, 256, 0, h->stream>>>(q, lo, hi);
+    h->launches++;
+    if (!h->two) return check_launch(h, "lb_slab_pack_phi");
+  }
   run_phase(h);                                    // after lb_init / lb_set_populations: the full sweep
   const int H = slab_phi_halo(h);
   const size_t pf = slab_phi_plane_floats(h), nb = (size_t)H * pf * sizeof(float);
@@ -1404,10 +1475,17 @@ int lb_slab_pack_phi(lb_handle h, void* send_lo, void* send_hi) {
 int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi) {
   int rc = slab_ready(h, 0, "lb_slab_unpack_phi");
   if (rc) return rc;
-  if (!h->two) return LB_OK;
+  if (!h->two && h->np == 0) return LB_OK;
   if ((rc = slab_msg_check(h, recv_lo, recv_hi))) return rc;
-  if (!h->phi_current) return fail(h, LB_ESTATE, "lb_slab_unpack_phi before lb_slab_pack_phi");
+  if (h->two && !h->phi_current) return fail(h, LB_ESTATE, "lb_slab_unpack_phi before lb_slab_pack_phi");
   DeviceGuard guard(h->device);
+  if (h->np > 0) {                                 // ghost densities: below from the message that came up, above from the one that came down
+    const size_t gb = slab_rho_bytes(h);
+    cudaError_t e = cudaMemcpyAsync(h->ghost_rho, static_cast<const char*>(recv_lo) + slab_phi_bytes(h), gb, cudaMemcpyDeviceToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(reinterpret_cast<char*>(h->ghost_rho) + gb, static_cast<const char*>(recv_hi) + slab_phi_bytes(h), gb, cudaMemcpyDeviceToDevice, h->stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "lb_slab_unpack_phi");
+    if (!h->two) { h->phi_ghost_ok = true; return LB_OK; }
+  }
   const int H = slab_phi_halo(h);
   const size_t pf = slab_phi_plane_floats(h), nb = (size_t)H * pf * sizeof(float);
   float* fields[2] = {h->phi, h->phi2};
@@ -1418,6 +1496,36 @@ int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi) {
   }
   h->phi_ghost_ok = true;
   return LB_OK;
+}
+
+int lb_slab_part_get(lb_handle h, double* d_sums) {
+  int rc = slab_ready(h, 1, "lb_slab_part_get");
+  if (rc) return rc;
+  if (h->np == 0 || h->part_stage == 0) return fail(h, LB_ESTATE, "lb_slab_part_get: no particle sums are pending");
+  if (!d_sums || !is_device_ptr(d_sums)) return fail(h, LB_EINVAL, "lb_slab_part_get: a device buffer of 6 doubles per particle");
+  DeviceGuard guard(h->device);
+  cudaError_t e = cudaMemcpyAsync(d_sums, h->pred, (size_t)h->np * 6 * sizeof(double), cudaMemcpyDeviceToDevice, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "lb_slab_part_get");
+  return LB_OK;
+}
+
+int lb_slab_part_put(lb_handle h, const double* d_sums) {
+  int rc = slab_ready(h, 1, "lb_slab_part_put");
+  if (rc) return rc;
+  if (h->np == 0 || h->part_stage == 0) return fail(h, LB_ESTATE, "lb_slab_part_put: no particle sums are pending");
+  if (!d_sums || !is_device_ptr(d_sums)) return fail(h, LB_EINVAL, "lb_slab_part_put: a device buffer of 6 doubles per particle");
+  DeviceGuard guard(h->device);
+  cudaError_t e = cudaMemcpyAsync(h->ptot, d_sums, (size_t)h->np * 6 * sizeof(double), cudaMemcpyDeviceToDevice, h->stream);
+  if (e != cudaSuccess) return cuda_fail(h, e, "lb_slab_part_put");
+  if (h->part_stage == 1) {          // force and torque on every particle: pair forces, the move, this slab's node changes
+    particles_move(h);
+    h->part_stage = 2;
+  } else {                           // impulses of the node changes; the stored values are final: pack
+    particles_apply(h);
+    slab_copy_populations(h, next_buf(h), slab_send_blocks(h, h->mode()), h->pend_send[0], h->pend_send[1], true);
+    h->part_stage = 0;
+  }
+  return check_launch(h, "lb_slab_part_put");
 }
 
 long long lb_launch_count(lb_handle h) { return h ? h->launches : 0; }

@@ -1405,14 +1405,30 @@ struct PartParams {
   double K, hc, mu;      // pair force (G37); mu = rho_0 nu
   int lub;
   int* overflow;         // set if a particle changed more nodes in one step than k_part_remap can list
+  // a slab of a larger box (replicated data): every rank holds all particles and sums
+  // what its own planes contribute; the sums over the ranks come back from the caller's all-reduce
+  double* part_out;      // [np][6] this slab's share of the link sums (k_part_force) / of the impulses (k_part_remap); nullptr: undivided box
+  const double* tot_in;  // [np][6] the sums over all slabs (k_part_pair: F, T; k_part_apply: dU, dL)
+  const float* ghost_rho;   // [2 faces][2 components][ny * nx] densities of time t in the ghost planes (lb_slab_unpack_phi)
 };
 
 constexpr int PART_MAXCH = 384;   // changed nodes per particle and step that k_part_remap can hold
 
-struct PartBox { int lo[3], ext[3]; };
+// Coordinates.  A particle lives in the whole periodic box, nx x ny x gnz, and its state is the same
+// on every rank that holds a slab of that box ("replicated data").  The kernels
+// below index SITES by the handle's allocated planes, z in [0, b.nz), of which [b.zlo, b.zhi) are its
+// own; plane z stands at global z + b.zoff (mod gnz).  Distances to a particle are taken in global
+// coordinates.  Undivided box: gnz = b.nz, zoff = 0, every plane its own.
+__device__ __forceinline__ int global_z(const Box& b, int z) {
+  const int g = z + b.zoff;
+  return g < 0 ? g + b.gnz : (g >= b.gnz ? g - b.gnz : g);
+}
+__device__ __forceinline__ bool own_plane(const Box& b, int z) { return z >= b.zlo && z < b.zhi; }
+
+struct PartBox { int lo[3], ext[3]; };    // in global coordinates
 __device__ __forceinline__ PartBox part_box(const Box& b, const double r[3], double reach) {
   PartBox pb;
-  const int n[3] = {b.nx, b.ny, b.nz};
+  const int n[3] = {b.nx, b.ny, b.gnz};
   for (int a = 0; a < 3; ++a) {
     int lo = (int)floor(r[a] - reach), hi = (int)ceil(r[a] + reach);
     if (hi - lo + 1 > n[a]) { lo = 0; hi = n[a] - 1; }      // never visit a node twice
@@ -1420,28 +1436,46 @@ __device__ __forceinline__ PartBox part_box(const Box& b, const double r[3], dou
   }
   return pb;
 }
-__device__ __forceinline__ void part_box_node(const Box& b, const PartBox& pb, int i, int& x, int& y, int& z) {
+// the allocated plane that holds global plane zg, or -1
+__device__ __forceinline__ int local_z(const Box& b, int zg) {
+  int z = zg - b.zoff;
+  z = z < 0 ? z + b.gnz : (z >= b.gnz ? z - b.gnz : z);
+  return z < b.nz ? z : -1;
+}
+// node i of the box: site coordinates (x, y, z); false if this handle does not hold its plane
+__device__ __forceinline__ bool part_box_node(const Box& b, const PartBox& pb, int i, int& x, int& y, int& z) {
   const int lx = i % pb.ext[0], ly = (i / pb.ext[0]) % pb.ext[1], lz = i / (pb.ext[0] * pb.ext[1]);
   x = (pb.lo[0] + lx) % b.nx; if (x < 0) x += b.nx;
   y = (pb.lo[1] + ly) % b.ny; if (y < 0) y += b.ny;
-  z = (pb.lo[2] + lz) % b.nz; if (z < 0) z += b.nz;
+  int zg = (pb.lo[2] + lz) % b.gnz; if (zg < 0) zg += b.gnz;
+  z = local_z(b, zg);
+  return z >= 0;
 }
 __device__ __forceinline__ bool inside_particle(const Box& b, const PState& P, int x, int y, int z) {
-  const double dx = min_image(x - P.r[0], b.nx), dy = min_image(y - P.r[1], b.ny), dz = min_image(z - P.r[2], b.nz);
+  const double dx = min_image(x - P.r[0], b.nx), dy = min_image(y - P.r[1], b.ny), dz = min_image(global_z(b, z) - P.r[2], b.gnz);
   return dx * dx + dy * dy + dz * dz < P.R * P.R;
 }
 __device__ __forceinline__ size_t site_of(const Box& b, int x, int y, int z) { return (size_t)x + (size_t)b.nx * ((size_t)y + (size_t)b.ny * z); }
-__device__ __forceinline__ void nbr_of(const Box& b, int x, int y, int z, int q, int& xn, int& yn, int& zn) {
+// the neighbour of site (x, y, z) along c_q; false if this handle does not hold its plane (a slab's
+// ghost planes have neighbours on one side only)
+__device__ __forceinline__ bool nbr_of(const Box& b, int x, int y, int z, int q, int& xn, int& yn, int& zn) {
   xn = x + c_cx[q]; yn = y + c_cy[q]; zn = z + c_cz[q];
   xn = xn < 0 ? b.nx - 1 : (xn >= b.nx ? 0 : xn);
   yn = yn < 0 ? b.ny - 1 : (yn >= b.ny ? 0 : yn);
-  zn = zn < 0 ? b.nz - 1 : (zn >= b.nz ? 0 : zn);
+  if (b.zper) { zn = zn < 0 ? b.nz - 1 : (zn >= b.nz ? 0 : zn); return true; }
+  return zn >= 0 && zn < b.nz;
 }
 
 // rho_r, rho_b (one component: rho, 0) of the fluid site (x, y, z) at time t (Eq. 3): its
 // pre-collision populations gathered from the source buffer with the pull rule
 template <bool TWO>
 __device__ __forceinline__ void site_density(const PartParams& p, int x, int y, int z, float& rr, float& rb) {
+  if (!own_plane(p.box, z)) {      // a slab's ghost plane: what the rank that owns it has sent (lb_slab_pack_phi)
+    const size_t n = (size_t)p.box.nx * p.box.ny, o = (size_t)x + (size_t)p.box.nx * y;
+    const float* g = p.ghost_rho + (z < p.box.zlo ? 0 : 2) * n;
+    rr = g[o]; rb = g[n + o];
+    return;
+  }
   Ctx c;
   make_ctx<TWO ? 8 : 4>(c, p.box, x, y, z);
   const uint32_t smask = neighbour_mask(p.box, x, y, z);
@@ -1456,6 +1490,22 @@ __device__ __forceinline__ void site_density(const PartParams& p, int x, int y, 
   else { rr = 1.0f + t; rb = 0.f; }
 }
 
+// A slab with particles: rho_r, rho_b of its lowest and highest own plane (zero at solid sites), which
+// travel with the phi halo and become the neighbours' ghost densities (site_density; G36 fills a node
+// that leaves a particle at the mean densities of its fluid neighbours).  grid = (sites of a plane / 256, 2 faces).
+template <bool TWO>
+__global__ void __launch_bounds__(256) k_slab_rho(const PartParams p, float* out_lo, float* out_hi) {
+  const Box& b = p.box;
+  const int n = b.nx * b.ny, o = blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= n) return;
+  const int x = o % b.nx, y = o / b.nx, z = blockIdx.y == 0 ? b.zlo : b.zhi - 1;
+  float rr = 0.f, rb = 0.f;
+  if (!solid_at(b, x, y, z)) site_density<TWO>(p, x, y, z, rr, rb);
+  float* out = blockIdx.y == 0 ? out_lo : out_hi;
+  out[o] = rr;
+  out[n + o] = rb;
+}
+
 // stored post-collision pair of direction q at its own site (A/B layout)
 template <bool TWO>
 __device__ __forceinline__ float* own_slot(const PartParams& p, int q, size_t s) { return p.pd[q] + s * (TWO ? 2 : 1); }
@@ -1464,7 +1514,7 @@ __device__ __forceinline__ float* own_slot(const PartParams& p, int q, size_t s)
 __device__ __forceinline__ double link_cu_rt(const Box& b, const double r[3], const double u[3], const double w[3], int x, int y, int z, int q, double rel[3]) {
   rel[0] = min_image(x - r[0], b.nx) + 0.5 * c_cx[q];
   rel[1] = min_image(y - r[1], b.ny) + 0.5 * c_cy[q];
-  rel[2] = min_image(z - r[2], b.nz) + 0.5 * c_cz[q];
+  rel[2] = min_image(global_z(b, z) - r[2], b.gnz) + 0.5 * c_cz[q];
   // in fp32 like k_fused (link_cu), so that undoing a link reproduces the stored value
   const float rx = (float)rel[0], ry = (float)rel[1], rz = (float)rel[2];
   const float wx = (float)w[0], wy = (float)w[1], wz = (float)w[2];
@@ -1504,19 +1554,21 @@ __device__ __forceinline__ void scan_shell(const Box& b, const PartBox& pb, cons
   int qn = 0;
   for (int row = row0; row < nrows; row += stride) {
     const int ly = row % pb.ext[1], lz = row / pb.ext[1];
-    int y = pb.lo[1] + ly, z = pb.lo[2] + lz;
+    int y = pb.lo[1] + ly, zg = pb.lo[2] + lz;
     y += y < 0 ? b.ny : (y >= b.ny ? -b.ny : 0);
-    z += z < 0 ? b.nz : (z >= b.nz ? -b.nz : 0);
+    zg += zg < 0 ? b.gnz : (zg >= b.gnz ? -b.gnz : 0);
+    const int z = local_z(b, zg);
+    if (z < 0) continue;                                   // a plane of another slab
     for (int lx0 = 0; lx0 < pb.ext[0]; lx0 += 32) {
       const int lx = lx0 + lane;
       int x = pb.lo[0] + lx;
       x += x < 0 ? b.nx : (x >= b.nx ? -b.nx : 0);
       bool pass = lx < pb.ext[0];
       if (pass) {
-        float fx = (float)x - cxr, fy = (float)y - cyr, fz = (float)z - czr;     // fp32 is enough for the prefilter
+        float fx = (float)x - cxr, fy = (float)y - cyr, fz = (float)zg - czr;    // fp32 is enough for the prefilter
         fx += fx > 0.5f * b.nx ? -(float)b.nx : (fx < -0.5f * b.nx ? (float)b.nx : 0.f);
         fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
-        fz += fz > 0.5f * b.nz ? -(float)b.nz : (fz < -0.5f * b.nz ? (float)b.nz : 0.f);
+        fz += fz > 0.5f * b.gnz ? -(float)b.gnz : (fz < -0.5f * b.gnz ? (float)b.gnz : 0.f);
         const float d2 = fx * fx + fy * fy + fz * fz;
         pass = d2 >= rin2 && d2 <= rout2 && keep(x, y, z);
       }
@@ -1546,7 +1598,7 @@ __global__ void __launch_bounds__(256) k_part_raster(const PartParams p) {
   const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
   for (int i = threadIdx.x; i < nn; i += blockDim.x) {
     int x, y, z;
-    part_box_node(b, pb, i, x, y, z);
+    if (!part_box_node(b, pb, i, x, y, z)) continue;       // (a slab marks its ghost planes too)
     if (solid_at(b, x, y, z) || !inside_particle(b, P, x, y, z)) continue;
     atomicOr(&p.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)], 1u << (x & 31));
     p.pid[site_of(b, x, y, z)] = blockIdx.x;
@@ -1579,7 +1631,7 @@ __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
       constexpr int q = decltype(qc)::value;
       if ((smask >> q) & 1u) {
         int xn, yn, zn;
-        nbr_of(b, x, y, z, q, xn, yn, zn);
+        nbr_of(b, x, y, z, q, xn, yn, zn);                 // (an own site: all its neighbours are held)
         if (p.pid[site_of(b, xn, yn, zn)] == (int)blockIdx.x) mine |= 1u << q;
       }
     });
@@ -1607,20 +1659,28 @@ __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
   // a fluid node with a link into the sphere lies in the shell R .. R + 1.75
   const float Rin = (float)P.R - 0.01f, Rout = (float)P.R + 1.75f;
   scan_shell(b, pb, P.r, Rin * Rin, Rout * Rout + 0.5f, threadIdx.x >> 5, 8, queue[threadIdx.x >> 5],
-             [&](int x, int y, int z) { return !solid_at(b, x, y, z); }, process);
+             [&](int x, int y, int z) { return own_plane(b, z) && !solid_at(b, x, y, z); }, process);
   block_sum<6>(acc, red);
-  if (threadIdx.x == 0)
-    for (int a = 0; a < 3; ++a) { P.F[a] = acc[a]; P.T[a] = acc[3 + a]; }
+  if (threadIdx.x == 0) {
+    if (p.part_out)
+      for (int a = 0; a < 6; ++a) p.part_out[(size_t)blockIdx.x * 6 + a] = acc[a];     // this slab's share
+    else
+      for (int a = 0; a < 3; ++a) { P.F[a] = acc[a]; P.T[a] = acc[3 + a]; }
+  }
 }
 
 // G37: the force on particle i from all others.  One warp per particle, the lanes share the others;
 // the lane sums are added in a fixed order.
 __global__ void __launch_bounds__(256) k_part_pair(const PartParams p) {
   const Box& b = p.box;
-  const int n[3] = {b.nx, b.ny, b.nz};
+  const int n[3] = {b.nx, b.ny, b.gnz};
   const int i = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
   if (i >= p.np) return;
   PState& A = p.parts[i];
+  if (p.tot_in && lane < 6) {      // a slab: the link sums over all slabs
+    if (lane < 3) A.F[lane] = p.tot_in[(size_t)i * 6 + lane];
+    else A.T[lane - 3] = p.tot_in[(size_t)i * 6 + lane];
+  }
   double f[3] = {0, 0, 0};
   if (p.hc > 0.0)
     for (int j = lane; j < p.np; j += 32) {
@@ -1653,7 +1713,7 @@ __global__ void __launch_bounds__(256) k_part_pair(const PartParams p) {
 // G35: Eq. 15 by leapfrog with the quaternion update; one thread per particle
 __global__ void __launch_bounds__(128) k_part_integrate(const PartParams p) {
   const Box& b = p.box;
-  const int n[3] = {b.nx, b.ny, b.nz};
+  const int n[3] = {b.nx, b.ny, b.gnz};
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= p.np || !p.mobile) return;
   PState& P = p.parts[i];
@@ -1694,7 +1754,7 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
   const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
   for (int i = threadIdx.x; i < nn; i += blockDim.x) {
     int x, y, z;
-    part_box_node(b, pb, i, x, y, z);
+    if (!part_box_node(b, pb, i, x, y, z)) continue;       // (a slab lists the changes in its ghost planes too)
     const size_t s = site_of(b, x, y, z);
     const bool was = p.pid[s] == me;
     const bool now = inside_particle(b, P, x, y, z) && (was || !solid_at(b, x, y, z));
@@ -1742,8 +1802,12 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
       const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
       give(d, rel, +1.0);
     };
-    const double rel0[3] = {min_image(x - P.r[0], b.nx), min_image(y - P.r[1], b.ny), min_image(z - P.r[2], b.nz)};
+    const double rel0[3] = {min_image(x - P.r[0], b.nx), min_image(y - P.r[1], b.ny), min_image(global_z(b, z) - P.r[2], b.gnz)};
+    // A slab treats what belongs to its own planes: the node itself if it owns it, and of every changed
+    // node (its ghost planes included) the links of its own fluid sites into that node.
+    const bool own_s = own_plane(b, z);
     if (!entered) {
+      if (own_s) {
       // the node leaves the particle: equilibrium (Eq. 2) at the mean densities of its fluid neighbours
       // and the surface velocity; its momentum comes out of the particle's
       float sr = 0.f, sb = 0.f;
@@ -1778,9 +1842,10 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
         if (solid_at(b, xn, yn, zn) && pn != me) continue;    // a wall's or another particle's node
         reflect(x, y, z, q, rr, rb);
       }
+      }
       for (int q = 1; q < Q; ++q) {                      // links of fluid neighbours into this node: undone
         int xs, ys, zs;
-        nbr_of(b, x, y, z, opp(q), xs, ys, zs);          // (xs, ys, zs) + c_q = this node
+        if (!nbr_of(b, x, y, z, opp(q), xs, ys, zs) || !own_plane(b, zs)) continue;     // (xs, ys, zs) + c_q = this node
         const size_t t = site_of(b, xs, ys, zs);
         if (solid_at(b, xs, ys, zs) || newly_covered(t)) continue;
         float a, c2;
@@ -1800,6 +1865,7 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
     } else {
       // the node enters the particle: what it holds goes to the particle.  A stored value stands for a
       // population that after streaming moves along c_q, or, where the neighbour is solid, along -c_q.
+      if (own_s) {
       double mom[3] = {0, 0, 0};
       for (int q = 0; q < Q; ++q) {
         int xn, yn, zn;
@@ -1809,9 +1875,10 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
         mom[0] += v * c_cx[q]; mom[1] += v * c_cy[q]; mom[2] += v * c_cz[q];
       }
       give(mom, rel0, +1.0);
+      }
       for (int q = 1; q < Q; ++q) {                      // links of fluid neighbours into this node: reflected
         int xs, ys, zs;
-        nbr_of(b, x, y, z, opp(q), xs, ys, zs);
+        if (!nbr_of(b, x, y, z, opp(q), xs, ys, zs) || !own_plane(b, zs)) continue;
         if (solid_at(b, xs, ys, zs) || newly_covered(site_of(b, xs, ys, zs))) continue;
         float a, c2;
         site_density<TWO>(p, xs, ys, zs, a, c2);
@@ -1825,7 +1892,10 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
     double t[6] = {0, 0, 0, 0, 0, 0};
     for (int i = 0; i < nch; ++i)
       for (int a = 0; a < 6; ++a) t[a] += imp[i][a];
-    for (int a = 0; a < 3; ++a) { P.u[a] += t[a] / P.mass; P.w[a] += t[3 + a] / P.inertia; }
+    if (p.part_out)
+      for (int a = 0; a < 6; ++a) p.part_out[(size_t)me * 6 + a] = t[a];      // this slab's share: k_part_apply adds the total
+    else
+      for (int a = 0; a < 3; ++a) { P.u[a] += t[a] / P.mass; P.w[a] += t[3 + a] / P.inertia; }
   }
   for (int i = threadIdx.x; i < nch; i += blockDim.x) {       // the node map of time t + 1
     const bool entered = (list[i] >> 30) & 1;
@@ -1834,6 +1904,18 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
     uint32_t* wd = &p.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)];
     if (entered) { atomicOr(wd, 1u << (x & 31)); p.pid[s] = me; }
     else { atomicAnd(wd, ~(1u << (x & 31))); p.pid[s] = -1; }
+  }
+}
+
+// A slab: the impulses of the node changes, summed over all slabs by the caller, go to the particles
+// (what the last lines of k_part_remap do in an undivided box).  One thread per particle.
+__global__ void __launch_bounds__(128) k_part_apply(const PartParams p) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= p.np || !p.mobile) return;
+  PState& P = p.parts[i];
+  for (int a = 0; a < 3; ++a) {
+    P.u[a] += p.tot_in[(size_t)i * 6 + a] / P.mass;
+    P.w[a] += p.tot_in[(size_t)i * 6 + 3 + a] / P.inertia;
   }
 }
 
@@ -1856,7 +1938,7 @@ __global__ void __launch_bounds__(256) k_part_phi(const StepParams p) {
   const PartBox pb = part_box(b, P.r, P.R + 2.5);
   const float Rin = P.R > 2.0 ? (float)P.R - 2.0f : 0.f, Rout = (float)P.R + 2.5f;
   scan_shell(b, pb, P.r, Rin * Rin, Rout * Rout + 0.5f, blockIdx.y * 8 + (threadIdx.x >> 5), 8 * gridDim.y, queue[threadIdx.x >> 5],
-             [](int, int, int) { return true; },
+             [&](int, int, int z) { return own_plane(b, z); },
              [&](int site) {
                const int x = site % b.nx, y = (site / b.nx) % b.ny, z = site / (b.nx * b.ny);
                phase_column<MODE_AB, true, false>(p, x, y, z, z + 1);

@@ -68,6 +68,7 @@ struct Box {
   int nx, ny, nz;        // allocated extents (a z slab holds one ghost plane below and one above its own planes)
   int zlo, zhi;          // planes this handle updates: [zlo, zhi) = [0, nz), or [1, nz - 1) for a z slab
   int zper;              // z is periodic inside this box (0 for a slab: its z neighbours are other handles)
+  int gnz, zoff;         // z extent of the whole (periodic) box and global z of the allocated plane 0: nz, 0 unless a slab
   int nxw;               // 32-bit mask words per x row
   long long S;           // sites (allocated)
   const uint32_t* mask;  // bit-packed solid mask (bit x&31 of word row*nxw + x>>5), or nullptr

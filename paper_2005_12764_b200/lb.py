@@ -22,7 +22,7 @@ SYMBOLS = [
     "lb_check_state", "lb_check_state_static", "lb_get_macros", "lb_get_populations", "lb_set_populations", "lb_get_phi", "lb_launch_count",
     "lb_device_bytes", "lb_last_error", "lb_set_profiling", "lb_last_step_ms", "lb_set_tuning",
     "lb_set_slab", "lb_slab_halo_bytes", "lb_slab_begin", "lb_slab_interior", "lb_slab_end",
-    "lb_slab_pack_phi", "lb_slab_unpack_phi",
+    "lb_slab_pack_phi", "lb_slab_unpack_phi", "lb_slab_part_get", "lb_slab_part_put",
     "lb_set_particles", "lb_set_particle_options", "lb_set_particle_force", "lb_get_particles",
 ]
 
@@ -83,6 +83,8 @@ def _load():
     lib.lb_slab_end.argtypes = [vp, fp, fp]
     lib.lb_slab_pack_phi.argtypes = [vp, fp, fp]
     lib.lb_slab_unpack_phi.argtypes = [vp, fp, fp]
+    lib.lb_slab_part_get.argtypes = [vp, vp]
+    lib.lb_slab_part_put.argtypes = [vp, vp]
     lib.lb_set_particles.argtypes = [vp, C.c_int, fp]
     lib.lb_set_particle_options.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_int]
     lib.lb_set_particle_force.argtypes = [vp, C.c_int, fp, fp]
@@ -290,6 +292,14 @@ class LB:
     def slab_unpack_phi(self, recv_lo, recv_hi):
         self._sync_stream()
         self._ck(lib.lb_slab_unpack_phi(self.h, _addr(recv_lo), _addr(recv_hi)))
+
+    def slab_part_get(self, d_sums):
+        self._sync_stream()
+        self._ck(lib.lb_slab_part_get(self.h, _addr(d_sums)))
+
+    def slab_part_put(self, d_sums):
+        self._sync_stream()
+        self._ck(lib.lb_slab_part_put(self.h, _addr(d_sums)))
 
     # ---- rigid particles (include/lb.h "rigid spherical particles"); state rows = lb_particle:
     # r[3], u[3], w[3], q[4], R, mass (float64)

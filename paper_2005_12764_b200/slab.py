@@ -3,7 +3,9 @@
 The paper distributes the fluid box equally over its ranks; collision is local and
 streaming reaches first neighbours only.  Here every rank (one process per GPU)
 owns a slab of z planes; per step and face it sends the 5 populations per component that cross the
-face and H planes of the phase field (include/lb.h).  This module holds NO lattice-Boltzmann
+face and H planes of the phase field (include/lb.h); with rigid particles ("replicated data",
+PAPER.md:312-316) every rank holds all of them and two sums of 6 doubles per particle go over the
+ranks per step.  This module holds NO lattice-Boltzmann
 arithmetic and no kernels: it allocates the message buffers (torch device tensors), moves them
 with torch.distributed point-to-point operations (NCCL send/recv over NVLink; gloo in the CPU test
 of the schedule) and orders the phases of a step so that the population exchange runs on a side
@@ -67,6 +69,16 @@ def exchange(send_lo, send_hi, recv_lo, recv_hi, rank=0, world=1, group=None):
         req.wait()
 
 
+def reduce_sums(sums, world=1, group=None):
+    """The sum over the ranks of a [np, 6] float64 tensor, in place (replicated particles: link sums,
+    then the impulses of the node changes).  Every rank must end up with the same bits, or the
+    replicated particle states drift apart: an all-reduce gives that."""
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
+    return sums
+
+
 # ------------------------------------------------------------------------------ one slab
 class Slab:
     """The planes [z0, z0 + nz) of an nx x ny x nz_global box, on the current CUDA device."""
@@ -107,6 +119,9 @@ class Slab:
         self.buf = {k: mk(pop if k.startswith("p") else phi)
                     for k in ("p_send_lo", "p_send_hi", "p_recv_lo", "p_recv_hi", "f_send_lo", "f_send_hi", "f_recv_lo", "f_recv_hi")}
         self.halo_bytes = (pop, phi)
+        self.np = getattr(self.sim, "npart", 0)
+        # the slab's share of the particle sums [np, 6], and where the totals come back
+        self.sums = torch.zeros((max(self.np, 1), 6), dtype=torch.float64, device=dev)
 
     def init_from(self, w):
         z0 = self.z0 % w.nz                      # a box taller than the workload repeats it along z
@@ -130,6 +145,13 @@ class Slab:
 
     def unpack_phi(self):
         self.sim.slab_unpack_phi(self.buf["f_recv_lo"], self.buf["f_recv_hi"])
+
+    def part_get(self):
+        self.sim.slab_part_get(self.sums)
+        return self.sums
+
+    def part_put(self, total):
+        self.sim.slab_part_put(total)
 
 
 # ------------------------------------------------------------------------------ one slab per rank
@@ -168,6 +190,16 @@ class DistributedSlab:
         main = torch.cuda.current_stream()
         for _ in range(int(nsteps)):
             self.slab.begin()
+            if self.slab.np > 0:
+                # replicated particles: link sums, then the impulses of the node changes, summed over
+                # the ranks (every rank gets the same bits back); no overlap in this step
+                for _stage in range(2):
+                    self.slab.part_put(reduce_sums(self.slab.part_get(), self.world, self.group))
+                self._x("p")
+                self.slab.interior()
+                self.slab.end()
+                self.exchange_phi()
+                continue
             if self.side is not None:
                 ready = main.record_event()
                 with torch.cuda.stream(self.side):
@@ -219,6 +251,14 @@ class LocalRing:
         for _ in range(int(nsteps)):
             for s in self.slabs:
                 s.begin()
+            if self.slabs[0].np > 0:
+                for _stage in range(2):        # the two sums over the slabs, in slab order
+                    total = None
+                    for s in self.slabs:
+                        part = s.part_get()
+                        total = part.clone() if total is None else total + part
+                    for s in self.slabs:
+                        s.part_put(total)
             self._x("p")
             for s in self.slabs:
                 s.interior()

@@ -186,3 +186,81 @@ def test_distributed_slab_world1_two_streams(lbmod, slabmod, storage):
     ds.step(4); sim.step(4)
     for k in (0, 1):
         assert np.array_equal(ds.slab.sim.get_populations(k), sim.get_populations(k))
+
+
+# ------------------------------------------------------------------------------- particles over slabs
+def _particle_workload(two, walls=False):
+    """A 40 x 24 x 32 box with three particles: one astride the cut at z = 16 and moving along z, one
+    crossing the periodic z boundary (the ring's wrap), one inside a slab; pair force on; in the
+    two-component case a flat interface that the first particle sits in and the near-contact force."""
+    from test_oracle_colloids import particle
+    nx, ny, nz = 40, 24, 32
+    parts = np.array([particle((11.3, 12.1, 15.6), u=(0.01, -0.01, 0.05), w=(0.003, 0.001, -0.002), R=4.5, density=2.0),
+                      particle((27.2, 11.6, 30.9), u=(-0.02, 0.004, 0.045), w=(0.0, -0.004, 0.001), R=3.6, density=3.0),
+                      particle((26.0, 10.9, 21.3), u=(0.0, 0.01, -0.04), w=(0.002, 0.0, 0.0), R=3.2, density=2.5)])
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    phi = np.tanh((x - 12.3) / 2.0) * np.tanh((30.2 - np.abs(x - 12.3)) / 2.0)
+    rr = ((1 + phi) / 2 if two else np.ones((nz, ny, nx))).astype(np.float32)
+    rb = ((1 - phi) / 2).astype(np.float32) if two else None
+    solid = None
+    if walls:
+        solid = np.zeros((nz, ny, nx), np.uint8)
+        solid[:, 0, :] = 1
+        solid[:, ny - 1, :] = 1
+    params = (0.9, 1.1, 0.01, 0.7, 0.02) if two else (0.8, 0.8, 0.0, 0.0, 0.0)
+    return W.Workload("slab-particles", nx, ny, nz, *params, rr, rb, np.zeros((3, nz, ny, nx), np.float32), solid=solid,
+                      g=(1e-5, 0.0, -2e-5),
+                      info={"particles": parts, "particle_options": dict(mobile=True, K=0.02, h_c=2.5, lubrication=True)})
+
+
+@pytest.mark.parametrize("cuts", [(16, 16), (8, 16, 8), (12, 20)])
+@pytest.mark.parametrize("two,walls", [(True, False), (False, False), (True, True)])
+def test_slabs_with_replicated_particles(lbmod, slabmod, two, walls, cuts):
+    """Replicated data: every slab holds all particles; the link sums and the
+    impulses of the node changes are added over the slabs.  Against the undivided box over 40
+    steps, in which nodes enter and leave the particles on both sides of the cuts: the same node
+    map, particle states to the rounding of the two sums, populations and fields to the rounding
+    that follows from it; and all slabs hold the same particle states bit for bit."""
+    w = _particle_workload(two, walls)
+    sim = lbmod.from_workload(w)
+    sim.set_tuning(zc=8)
+    sim.init(w.rho_r, w.rho_b, w.u)
+    ring = slabmod.LocalRing(w, cuts, "ab", zc=8)
+    ring.init()
+    solid0 = sim.get_macros()[0] == 0
+    changed = 0
+    # cuts at brick faces of the undivided run: the fluid agrees bit for bit and only the order of the
+    # two sums differs; other cuts: the forwarded phi sums round differently (fp32), and the forces follow
+    aligned = all(c % 8 == 0 for c in cuts)
+    tol_state, tol_force = (1e-9, 1e-9) if aligned else (1e-7, 1e-5)
+    for n in range(1, 41):
+        ring.step(1); sim.step(1)
+        if n in (1, 2, 3, 5, 10, 20, 30, 40):
+            st, fo = sim.get_particles()
+            for s in ring.slabs:
+                st_s, fo_s = s.sim.get_particles()
+                assert np.array_equal(st_s, ring.slabs[0].sim.get_particles()[0])      # replicated: the same bits everywhere
+                assert np.abs(st_s - st).max() < tol_state, (n, np.abs(st_s - st).max())
+                assert np.abs(fo_s - fo).max() < tol_force * max(1.0, np.abs(fo).max()), (n, np.abs(fo_s - fo).max())
+            a, b = ring.gather("get_macros"), sim.get_macros()
+            assert np.array_equal(a[0] == 0, b[0] == 0), (n, "node maps differ")
+            changed += int(((b[0] == 0) != solid0).sum())
+            solid0 = b[0] == 0
+            for x, y in zip(a, b):
+                assert (x is None and y is None) or np.abs(x - y).max() < 1e-6, n
+            for k in range(2 if two else 1):
+                d = np.abs(ring.gather("get_populations", k).astype(np.float64) - sim.get_populations(k)) / pu.W19[:, None, None, None]
+                assert d.max() < 1e-6, (n, k, d.max())
+            if two:
+                fluid = b[0] != 0
+                assert np.abs(ring.gather("get_phi") - sim.get_phi())[fluid].max() < 2e-6, n
+    assert changed > 40                       # nodes did enter and leave the particles
+
+
+def test_particles_need_two_slabs(lbmod, slabmod):
+    """A ring of one slab would hold the planes next to its own faces twice: refused at lb_init."""
+    w = _particle_workload(True)
+    ring = slabmod.LocalRing(w, (32,), "ab", zc=8)
+    with pytest.raises(lbmod.LBError) as ei:
+        ring.init()
+    assert ei.value.code == lbmod.LB_ESTATE and "two slabs" in str(ei.value)

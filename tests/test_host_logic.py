@@ -144,6 +144,14 @@ for it in range(3):                      # several rounds: messages of consecuti
     slab.exchange(send_lo, send_hi, recv_lo, recv_hi, rank, world)
     # my lower ghost holds the top planes of the rank below, my upper ghost the bottom planes of the rank above
     ok &= bool((recv_lo == 100.0 * below + 2 + 1000 * it).all()) and bool((recv_hi == 100.0 * above + 1 + 1000 * it).all())
+# replicated particles: the sums over the ranks, the same bits on every rank
+g = torch.Generator().manual_seed(7)
+shares = torch.randn((world, 5, 6), dtype=torch.float64, generator=g) * 10.0 ** torch.randint(-8, 3, (world, 5, 6), generator=g).double()
+mine = slab.reduce_sums(shares[rank].clone(), world)
+ok &= bool(torch.allclose(mine, shares.sum(0), rtol=1e-13, atol=0.0))
+every = [torch.zeros_like(mine) for _ in range(world)]
+dist.all_gather(every, mine)
+ok &= all(bool(torch.equal(e, every[0])) for e in every)
 t = torch.tensor([1.0 if ok else 0.0])
 dist.all_reduce(t, op=dist.ReduceOp.MIN)
 if rank == 0:
@@ -157,7 +165,8 @@ def test_gloo_slab_halo_exchange_schedule(tmp_path, world):
     """The halo exchange of the z-slab decomposition (paper_2005_12764_b200/slab.py: exchange) on a
     ring of 2 and of 3 ranks over gloo: every rank's lower ghost receives the top message of the rank
     below and its upper ghost the bottom message of the rank above; with 2 ranks both neighbours are
-    the same peer and the two messages must not be swapped."""
+    the same peer and the two messages must not be swapped.  And the sums of the replicated particles
+    (slab.reduce_sums): the total on every rank, bit for bit the same everywhere."""
     script = tmp_path / "worker.py"
     script.write_text(_GLOO_SLAB_WORKER)
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
