@@ -1615,8 +1615,16 @@ template <bool TWO>
 __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
   __shared__ double red[6 * 8];
   __shared__ int queue[8][64];
+  // the particle's state in shared memory: this kernel stores to global memory, so the compiler would
+  // load r, u, w of a global PState again for every link (measured: a quarter of the kernel's stall samples)
+  __shared__ PState P;
   const Box& b = p.box;
-  PState& P = p.parts[blockIdx.x];
+  {
+    const double* src = reinterpret_cast<const double*>(&p.parts[blockIdx.x]);
+    double* dst = reinterpret_cast<double*>(&P);
+    for (int i = threadIdx.x; i < (int)(sizeof(PState) / sizeof(double)); i += blockDim.x) dst[i] = src[i];
+  }
+  __syncthreads();
   const PartBox pb = part_box(b, P.r, P.R + 2.0);
   double acc[6] = {0, 0, 0, 0, 0, 0};
   // everything a candidate site (a fluid node in the shell around the sphere) needs
@@ -1665,7 +1673,7 @@ __global__ void __launch_bounds__(256) k_part_force(const PartParams p) {
     if (p.part_out)
       for (int a = 0; a < 6; ++a) p.part_out[(size_t)blockIdx.x * 6 + a] = acc[a];     // this slab's share
     else
-      for (int a = 0; a < 3; ++a) { P.F[a] = acc[a]; P.T[a] = acc[3 + a]; }
+      for (int a = 0; a < 3; ++a) { p.parts[blockIdx.x].F[a] = acc[a]; p.parts[blockIdx.x].T[a] = acc[3 + a]; }
   }
 }
 
