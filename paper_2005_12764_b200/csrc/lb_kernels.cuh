@@ -1785,10 +1785,17 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
     for (int j = 0; j < nch; ++j) if (list[j] == ((int)s | (1 << 30))) return true;
     return false;
   };
-  for (int i = threadIdx.x; i < nch; i += blockDim.x) {
+  // One WARP per changed node, lane q = direction q (lanes 19..31 idle): the work of a node is 18
+  // neighbours, each a chain of dependent loads (mask, densities, stored values), and one thread per
+  // node ran them one after the other (70 us per step at 241 colloids).  The lanes' shares of the
+  // impulse are added by a shuffle tree: a fixed order.
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int i = wid; i < nch; i += 8) {
     const bool entered = (list[i] >> 30) & 1;
     const size_t s = (size_t)(list[i] & ~(1 << 30));
     const int x = (int)(s % b.nx), y = (int)((s / b.nx) % b.ny), z = (int)(s / ((size_t)b.nx * b.ny));
+    const int q = lane;
+    const bool dir = q >= 1 && q < Q;                  // this lane stands for a link direction
     double dU[3] = {0, 0, 0}, dL[3] = {0, 0, 0};
     auto give = [&](const double m[3], const double rel[3], double sg) {
       dU[0] += sg * m[0]; dU[1] += sg * m[1]; dU[2] += sg * m[2];
@@ -1796,104 +1803,113 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
       dL[1] += sg * (rel[2] * m[0] - rel[0] * m[2]);
       dL[2] += sg * (rel[0] * m[1] - rel[1] * m[0]);
     };
-    // G33 with the particle's NEW state on the link (xs, ys, zs) -> + c_q; returns what the particle receives
-    auto reflect = [&](int xs, int ys, int zs, int q, float rr, float rb) {
+    // G33 with the particle's NEW state on the link (xs, ys, zs) -> + c_qq; the particle receives the sum
+    auto reflect = [&](int xs, int ys, int zs, int qq, float rr, float rb) {
       double rel[3];
-      const double cu = link_cu_rt(b, P.r, P.u, P.w, xs, ys, zs, q, rel);
-      float* sl = own_slot<TWO>(p, q, site_of(b, xs, ys, zs));
-      const float k = -6.0f * wq(q) * (float)cu;
-      const float fpt = sl[0] + wq(q);                  // f* (total)
+      const double cu = link_cu_rt(b, P.r, P.u, P.w, xs, ys, zs, qq, rel);
+      float* sl = own_slot<TWO>(p, qq, site_of(b, xs, ys, zs));
+      const float k = -6.0f * wq(qq) * (float)cu;
+      const float fpt = sl[0] + wq(qq);                  // f* (total)
       const float gt = fmaf(k, rr + rb, fpt);
-      sl[0] = gt - wq(q);
+      sl[0] = gt - wq(qq);
       if constexpr (TWO) sl[1] = fmaf(k, rr, sl[1]);
       const double tot = (double)fpt + (double)gt;
-      const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
+      const double d[3] = {tot * c_cx[qq], tot * c_cy[qq], tot * c_cz[qq]};
       give(d, rel, +1.0);
     };
     const double rel0[3] = {min_image(x - P.r[0], b.nx), min_image(y - P.r[1], b.ny), min_image(global_z(b, z) - P.r[2], b.gnz)};
     // A slab treats what belongs to its own planes: the node itself if it owns it, and of every changed
     // node (its ghost planes included) the links of its own fluid sites into that node.
     const bool own_s = own_plane(b, z);
+    // the neighbour along c_q and the one against it (xs + c_q = this node)
+    int xn = 0, yn = 0, zn = 0, xs = 0, ys = 0, zs = 0;
+    const bool has_n = dir && nbr_of(b, x, y, z, q, xn, yn, zn);
+    const bool has_s = dir && nbr_of(b, x, y, z, opp(dir ? q : 1), xs, ys, zs) && own_plane(b, zs);
     if (!entered) {
       if (own_s) {
-      // the node leaves the particle: equilibrium (Eq. 2) at the mean densities of its fluid neighbours
-      // and the surface velocity; its momentum comes out of the particle's
-      float sr = 0.f, sb = 0.f;
-      int cnt = 0;
-      for (int q = 1; q < Q; ++q) {
-        int xn, yn, zn;
-        nbr_of(b, x, y, z, q, xn, yn, zn);
-        if (solid_at(b, xn, yn, zn) || newly_covered(site_of(b, xn, yn, zn))) continue;
-        float a, c2;
-        site_density<TWO>(p, xn, yn, zn, a, c2);
-        sr += a; sb += c2; ++cnt;
+        // the node leaves the particle: equilibrium (Eq. 2) at the mean densities of its fluid neighbours
+        // and the surface velocity; its momentum comes out of the particle's
+        float a = 0.f, c2 = 0.f;
+        int one = 0;
+        if (has_n && !solid_at(b, xn, yn, zn) && !newly_covered(site_of(b, xn, yn, zn))) {
+          site_density<TWO>(p, xn, yn, zn, a, c2);
+          one = 1;
+        }
+        // sums over the directions in the order 1, 2, ..., 18 (what one thread did): lane 0 adds them up
+        float sr = 0.f, sb = 0.f;
+        int cnt = 0;
+        for (int k = 1; k < Q; ++k) {
+          sr += __shfl_sync(0xffffffffu, a, k);
+          sb += __shfl_sync(0xffffffffu, c2, k);
+          cnt += __shfl_sync(0xffffffffu, one, k);
+        }
+        float rr = TWO ? 0.5f : 1.0f, rb = TWO ? 0.5f : 0.0f;
+        if (cnt) { rr = sr / (float)cnt; rb = sb / (float)cnt; }
+        const double wxr[3] = {P.w[1] * rel0[2] - P.w[2] * rel0[1], P.w[2] * rel0[0] - P.w[0] * rel0[2], P.w[0] * rel0[1] - P.w[1] * rel0[0]};
+        const float ux = (float)(P.u[0] + wxr[0]), uy = (float)(P.u[1] + wxr[1]), uz = (float)(P.u[2] + wxr[2]);
+        const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz), rho = rr + rb;
+        if (q < Q) {
+          const float cu = c_cx[q] * ux + c_cy[q] * uy + c_cz[q] * uz;
+          const float e = 3.0f * cu + 4.5f * cu * cu - uu15;
+          float* sl = own_slot<TWO>(p, q, s);
+          sl[0] = wq(q) * ((rho - 1.0f) + rho * e);
+          if constexpr (TWO) sl[1] = wq(q) * rr * (1.0f + e);
+        }
+        if (lane == 0) {
+          const double mom[3] = {(double)rho * ux, (double)rho * uy, (double)rho * uz};
+          give(mom, rel0, -1.0);
+        }
+        // its own links into the particle as it stands now (the lane that wrote slot q reflects it)
+        if (has_n && inside_particle(b, P, xn, yn, zn)) {
+          const int pn = p.pid[site_of(b, xn, yn, zn)];
+          if (!(solid_at(b, xn, yn, zn) && pn != me)) reflect(x, y, z, q, rr, rb);    // (not a wall's or another particle's node)
+        }
       }
-      float rr = TWO ? 0.5f : 1.0f, rb = TWO ? 0.5f : 0.0f;
-      if (cnt) { rr = sr / (float)cnt; rb = sb / (float)cnt; }
-      const double wxr[3] = {P.w[1] * rel0[2] - P.w[2] * rel0[1], P.w[2] * rel0[0] - P.w[0] * rel0[2], P.w[0] * rel0[1] - P.w[1] * rel0[0]};
-      const float ux = (float)(P.u[0] + wxr[0]), uy = (float)(P.u[1] + wxr[1]), uz = (float)(P.u[2] + wxr[2]);
-      const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz), rho = rr + rb;
-      for (int q = 0; q < Q; ++q) {
-        const float cu = c_cx[q] * ux + c_cy[q] * uy + c_cz[q] * uz;
-        const float e = 3.0f * cu + 4.5f * cu * cu - uu15;
-        float* sl = own_slot<TWO>(p, q, s);
-        sl[0] = wq(q) * ((rho - 1.0f) + rho * e);
-        if constexpr (TWO) sl[1] = wq(q) * rr * (1.0f + e);
-      }
-      const double mom[3] = {(double)rho * ux, (double)rho * uy, (double)rho * uz};
-      give(mom, rel0, -1.0);
-      for (int q = 1; q < Q; ++q) {                      // its own links into the particle as it stands now
-        int xn, yn, zn;
-        nbr_of(b, x, y, z, q, xn, yn, zn);
-        if (!inside_particle(b, P, xn, yn, zn)) continue;
-        const int pn = p.pid[site_of(b, xn, yn, zn)];
-        if (solid_at(b, xn, yn, zn) && pn != me) continue;    // a wall's or another particle's node
-        reflect(x, y, z, q, rr, rb);
-      }
-      }
-      for (int q = 1; q < Q; ++q) {                      // links of fluid neighbours into this node: undone
-        int xs, ys, zs;
-        if (!nbr_of(b, x, y, z, opp(q), xs, ys, zs) || !own_plane(b, zs)) continue;     // (xs, ys, zs) + c_q = this node
+      // links of fluid neighbours into this node: undone
+      if (has_s) {
         const size_t t = site_of(b, xs, ys, zs);
-        if (solid_at(b, xs, ys, zs) || newly_covered(t)) continue;
-        float a, c2;
-        site_density<TWO>(p, xs, ys, zs, a, c2);
-        double rel[3];
-        const double cu = link_cu_rt(b, P.ro, P.uo, P.wo, xs, ys, zs, q, rel);
-        float* sl = own_slot<TWO>(p, q, t);
-        const float k = 6.0f * wq(q) * (float)cu;
-        const float gt = sl[0] + wq(q);
-        const float fpt = fmaf(k, a + c2, gt);
-        sl[0] = fpt - wq(q);
-        if constexpr (TWO) sl[1] = fmaf(k, a, sl[1]);
-        const double tot = (double)fpt + (double)gt;
-        const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
-        give(d, rel, -1.0);
+        if (!solid_at(b, xs, ys, zs) && !newly_covered(t)) {
+          float a, c2;
+          site_density<TWO>(p, xs, ys, zs, a, c2);
+          double rel[3];
+          const double cu = link_cu_rt(b, P.ro, P.uo, P.wo, xs, ys, zs, q, rel);
+          float* sl = own_slot<TWO>(p, q, t);
+          const float k = 6.0f * wq(q) * (float)cu;
+          const float gt = sl[0] + wq(q);
+          const float fpt = fmaf(k, a + c2, gt);
+          sl[0] = fpt - wq(q);
+          if constexpr (TWO) sl[1] = fmaf(k, a, sl[1]);
+          const double tot = (double)fpt + (double)gt;
+          const double d[3] = {tot * c_cx[q], tot * c_cy[q], tot * c_cz[q]};
+          give(d, rel, -1.0);
+        }
       }
     } else {
       // the node enters the particle: what it holds goes to the particle.  A stored value stands for a
       // population that after streaming moves along c_q, or, where the neighbour is solid, along -c_q.
-      if (own_s) {
-      double mom[3] = {0, 0, 0};
-      for (int q = 0; q < Q; ++q) {
-        int xn, yn, zn;
-        nbr_of(b, x, y, z, q, xn, yn, zn);
-        const double sg = (q > 0 && solid_at(b, xn, yn, zn)) ? -1.0 : 1.0;
+      if (own_s && q < Q) {
+        const double sg = (dir && has_n && solid_at(b, xn, yn, zn)) ? -1.0 : 1.0;
         const double v = sg * ((double)own_slot<TWO>(p, q, s)[0] + (double)wq(q));
-        mom[0] += v * c_cx[q]; mom[1] += v * c_cy[q]; mom[2] += v * c_cz[q];
+        const double mom[3] = {v * c_cx[q], v * c_cy[q], v * c_cz[q]};
+        give(mom, rel0, +1.0);
       }
-      give(mom, rel0, +1.0);
-      }
-      for (int q = 1; q < Q; ++q) {                      // links of fluid neighbours into this node: reflected
-        int xs, ys, zs;
-        if (!nbr_of(b, x, y, z, opp(q), xs, ys, zs) || !own_plane(b, zs)) continue;
-        if (solid_at(b, xs, ys, zs) || newly_covered(site_of(b, xs, ys, zs))) continue;
+      // links of fluid neighbours into this node: reflected
+      if (has_s && !solid_at(b, xs, ys, zs) && !newly_covered(site_of(b, xs, ys, zs))) {
         float a, c2;
         site_density<TWO>(p, xs, ys, zs, a, c2);
         reflect(xs, ys, zs, q, a, c2);
       }
     }
-    for (int a = 0; a < 3; ++a) { imp[i][a] = dU[a]; imp[i][3 + a] = dL[a]; }
+    // the lanes' shares, added by a tree of fixed shape
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        dU[a] += __shfl_down_sync(0xffffffffu, dU[a], o);
+        dL[a] += __shfl_down_sync(0xffffffffu, dL[a], o);
+      }
+    if (lane == 0)
+      for (int a = 0; a < 3; ++a) { imp[i][a] = dU[a]; imp[i][3 + a] = dL[a]; }
   }
   __syncthreads();
   if (threadIdx.x == 0) {
