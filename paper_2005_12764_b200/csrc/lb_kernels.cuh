@@ -1948,10 +1948,10 @@ __global__ void __launch_bounds__(128) k_part_apply(const PartParams p) {
 // since: k_part_force rewrote the values that come back from the surface, and a node that entered
 // or left the particle (k_part_remap) changes what its neighbours will read.  So phi is formed
 // again, from the stored populations with the node map of time t + 1, in the shell of nodes around
-// every particle's surface, R - 2 <= d <= R + 2.5 from the new centre: a fluid node with a link into
-// the particle lies within R + sqrt(2) of the old centre, a changed node within R of the old or the
-// new one and its neighbours sqrt(2) further, and the centre moves by less than one node per step;
-// nodes deeper inside keep their sentinel.  Shells of two particles may overlap: both write the same
+// every particle's surface, R - dr <= d <= R + sqrt(2) + dr from the new centre, dr = the distance the
+// centre moved in this step: a fluid node with a link into the particle lies within R + sqrt(2) of the
+// old centre, a changed node within R of the old or the new one and its neighbours sqrt(2) further;
+// nodes deeper inside than R - dr were and are the particle's and keep their sentinel.  Shells of two particles may overlap: both write the same
 // values.  A/B storage (the particles' only one).
 // grid = (particles, slices of the box's rows): the gathers are latency-bound, so the rows of a
 // box are spread over several CTAs.
@@ -1959,8 +1959,11 @@ __global__ void __launch_bounds__(256) k_part_phi(const StepParams p) {
   __shared__ int queue[8][64];
   const Box& b = p.box;
   const PState& P = p.parts[blockIdx.x];
-  const PartBox pb = part_box(b, P.r, P.R + 2.5);
-  const float Rin = P.R > 2.0 ? (float)P.R - 2.0f : 0.f, Rout = (float)P.R + 2.5f;
+  // how far the centre moved in this step
+  const double mx = min_image(P.r[0] - P.ro[0], b.nx), my = min_image(P.r[1] - P.ro[1], b.ny), mz = min_image(P.r[2] - P.ro[2], b.gnz);
+  const float dr = (float)sqrt(mx * mx + my * my + mz * mz) + 0.05f;
+  const float Rin = (float)P.R > dr ? (float)P.R - dr : 0.f, Rout = (float)P.R + 1.4143f + dr;
+  const PartBox pb = part_box(b, P.r, (double)Rout + 0.5);
   scan_shell(b, pb, P.r, Rin * Rin, Rout * Rout + 0.5f, blockIdx.y * 8 + (threadIdx.x >> 5), 8 * gridDim.y, queue[threadIdx.x >> 5],
              [&](int, int, int z) { return own_plane(b, z); },
              [&](int site) {
