@@ -1559,17 +1559,20 @@ __device__ __forceinline__ void scan_shell(const Box& b, const PartBox& pb, cons
     zg += zg < 0 ? b.gnz : (zg >= b.gnz ? -b.gnz : 0);
     const int z = local_z(b, zg);
     if (z < 0) continue;                                   // a plane of another slab
+    float fy = (float)y - cyr, fz = (float)zg - czr;       // fp32 is enough for the prefilter
+    fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
+    fz += fz > 0.5f * b.gnz ? -(float)b.gnz : (fz < -0.5f * b.gnz ? (float)b.gnz : 0.f);
+    const float ryz2 = fy * fy + fz * fz;
+    if (ryz2 > rout2) continue;                            // a row in a corner of the box: it misses the shell
     for (int lx0 = 0; lx0 < pb.ext[0]; lx0 += 32) {
       const int lx = lx0 + lane;
       int x = pb.lo[0] + lx;
       x += x < 0 ? b.nx : (x >= b.nx ? -b.nx : 0);
       bool pass = lx < pb.ext[0];
       if (pass) {
-        float fx = (float)x - cxr, fy = (float)y - cyr, fz = (float)zg - czr;    // fp32 is enough for the prefilter
+        float fx = (float)x - cxr;
         fx += fx > 0.5f * b.nx ? -(float)b.nx : (fx < -0.5f * b.nx ? (float)b.nx : 0.f);
-        fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
-        fz += fz > 0.5f * b.gnz ? -(float)b.gnz : (fz < -0.5f * b.gnz ? (float)b.gnz : 0.f);
-        const float d2 = fx * fx + fy * fy + fz * fz;
+        const float d2 = fx * fx + ryz2;
         pass = d2 >= rin2 && d2 <= rout2 && keep(x, y, z);
       }
       const unsigned bal = __ballot_sync(0xffffffffu, pass);
