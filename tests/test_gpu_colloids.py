@@ -177,3 +177,33 @@ def test_bijel_mini_workload_parity(lbmod, lbo):
     so, _ = o.get_particles()
     assert np.abs(st - so).max() < 1e-5
     assert np.abs(st[:, 3:6]).max() > 1e-6          # the demixing fluid does push the colloids
+
+
+@pytest.mark.parametrize("two", [True, False])
+def test_particles_between_sliding_walls_parity(lbmod, lbo, two):
+    """A particle in a channel whose y walls slide in opposite directions (wall groups 2 and 3, G28:
+    the wall-group instantiations of the fused kernel, to which a particle's node is a wall at rest)
+    against the oracle: node map, populations, fields and particle state over 20 steps."""
+    nx, ny, nz = 40, 20, 16
+    solid = np.zeros((nz, ny, nx), np.uint8)
+    solid[:, 0, :] = 2
+    solid[:, ny - 1, :] = 3
+    parts = [particle((14.2, 8.7, 8.1), u=(0.03, 0.02, -0.01), w=(0.0, 0.002, 0.004), R=4.2, density=2.0)]
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    phi = np.tanh((x - 20.3) / 2.0) * np.tanh((15.2 - np.abs(x - 20.3)) / 2.0)
+    rr, rb = ((1 + phi) / 2, (1 - phi) / 2) if two else (np.ones((nz, ny, nx)), None)
+    rr = np.where(solid > 0, 0.0, rr)
+    rb = None if rb is None else np.where(solid > 0, 0.0, rb)
+    params = (0.9, 1.1, 0.01, 0.7, 0.0) if two else (0.8, 0.8, 0.0, 0.0, 0.0)
+    o, sim = _pair(lbmod, lbo, (nx, ny, nz), params, parts, rr, rb, solid=solid, opts=dict(mobile=True, K=0.0, h_c=0.0, lubrication=False))
+    # (wall velocities may be set at any time: they act from the next step)
+    for obj in (o, sim):
+        obj.set_wall_velocity(2, -0.02, 0.0, 0.0)
+        obj.set_wall_velocity(3, 0.02, 0.0, 0.003)
+    for n in range(1, 21):
+        o.step(1); sim.step(1)
+        if n in (1, 2, 5, 10, 20):
+            e, ds, df, dm = _compare(o, sim, two)
+            assert e < pu.POP_TOL * max(1, n / 2), (n, e)
+            assert ds < 2e-6 and dm < pu.MACRO_TOL, (n, ds, dm)
+            assert df < 1e-5 * max(1.0, np.abs(o.get_particles()[1]).max()), (n, df)
