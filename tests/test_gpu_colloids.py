@@ -179,11 +179,12 @@ def test_bijel_mini_workload_parity(lbmod, lbo):
     assert np.abs(st[:, 3:6]).max() > 1e-6          # the demixing fluid does push the colloids
 
 
-@pytest.mark.parametrize("two", [True, False])
-def test_particles_between_sliding_walls_parity(lbmod, lbo, two):
+@pytest.mark.parametrize("two,wet", [(True, False), (True, True), (False, False)])
+def test_particles_between_sliding_walls_parity(lbmod, lbo, two, wet):
     """A particle in a channel whose y walls slide in opposite directions (wall groups 2 and 3, G28:
     the wall-group instantiations of the fused kernel, to which a particle's node is a wall at rest)
-    against the oracle: node map, populations, fields and particle state over 20 steps."""
+    against the oracle: node map, populations, fields and particle state over 20 steps.  wet: walls and
+    particle alike carry a prescribed phi in the colour stencil (G30: a wetting colloid)."""
     nx, ny, nz = 40, 20, 16
     solid = np.zeros((nz, ny, nx), np.uint8)
     solid[:, 0, :] = 2
@@ -200,6 +201,8 @@ def test_particles_between_sliding_walls_parity(lbmod, lbo, two):
     for obj in (o, sim):
         obj.set_wall_velocity(2, -0.02, 0.0, 0.0)
         obj.set_wall_velocity(3, 0.02, 0.0, 0.003)
+        if wet:
+            obj.set_wall_phi(0.3)
     for n in range(1, 21):
         o.step(1); sim.step(1)
         if n in (1, 2, 5, 10, 20):
