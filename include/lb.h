@@ -257,7 +257,8 @@ int lb_slab_unpack_phi(lb_handle h, const void* recv_lo, const void* recv_hi);
  *   lb_slab_part_get(h, d_sums)          that share [np][6] = (dU, dL)
  *   [caller: sum over the slabs]
  *   lb_slab_part_put(h, d_sums)          the totals go to the particles; the population messages
- *                                        given to lb_slab_begin are packed now
+ *                                        given to lb_slab_begin are packed now (send_lo, send_hi
+ *                                        must stay valid until this call returns)
  *   [caller: exchange the population messages]   lb_slab_interior, lb_slab_end as above
  *   (lb_slab_end also forms phi again around the particles)
  * and the phi messages carry, behind the phi planes, rho_r and rho_b of the boundary plane (G36 fills
