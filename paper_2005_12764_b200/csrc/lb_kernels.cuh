@@ -1397,7 +1397,7 @@ struct PartParams {
   const float* ps[Q];    // source buffer (state of time t, pull layout)
   float* pd[Q];          // destination buffer: post-collision values of time t at their own sites
   Box box;               // mask and pid are those of time t until k_part_remap has changed them
-  uint32_t* mask;        // writable views of box.mask / box.pid
+  uint32_t* mask;        // writable view of box.mask; the particle index per site (-1: none)
   int* pid;
   PState* parts;
   int np;
