@@ -47,6 +47,7 @@ void dev_free(const Allocator& a, void* p) {
 }
 
 constexpr int MAX_DEVICES = 64;
+constexpr int IO_CHUNKS = 8;
 
 // Makes the handle's device current for the duration of one C-ABI call (one process may hold
 // handles on several devices) and restores the caller's device afterwards.
@@ -138,6 +139,10 @@ struct lb_handle_s {
   int p_mobile = 1, p_lub = 0;
   double p_K = 0.0, p_hc = 0.0;
   int tune_zc = 0;           // z planes per CTA (0 = automatic)
+  // lb_init / lb_get_macros with HOST arrays: copies in IO_CHUNKS pieces on a stream of their own, so that
+  // the kernel works on one piece while the next one crosses PCIe
+  cudaStream_t cstream = nullptr;
+  cudaEvent_t cev[IO_CHUNKS + 1] = {};
   // CUDA graph of GRAPH_STEPS time steps for boxes whose step is bounded by launch latency (lb_step)
   int graph = -1;            // tuning key "graph": -1 = automatic (small boxes), 0 = never, 1 = whenever possible
   cudaGraphExec_t gexec = nullptr;
@@ -204,15 +209,30 @@ struct Staged {
   ~Staged() { if (owned) dev_free(al, dev); }
 };
 
-int stage_in(lb_handle h, const void* src, size_t bytes, Staged& s) {
+int stage_in(lb_handle h, const void* src, size_t bytes, Staged& s, bool copy = true) {
   if (is_device_ptr(src)) { s.dev = const_cast<void*>(src); return LB_OK; }
   s.al = h->al;
   s.dev = dev_alloc(h->al, bytes);
   if (!s.dev) return fail(h, LB_ENOMEM, "staging buffer allocation failed");
   s.owned = true;
+  if (!copy) return LB_OK;       // (the caller copies piece by piece: io_pipeline)
   cudaError_t e = cudaMemcpyAsync(s.dev, src, bytes, cudaMemcpyHostToDevice, h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "H2D copy");
   return LB_OK;
+}
+
+// The copy stream and the events of the chunked host transfers (created on first use).
+int io_pipeline(lb_handle h) {
+  if (!h->cstream && cudaStreamCreateWithFlags(&h->cstream, cudaStreamNonBlocking) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "copy stream");
+  for (cudaEvent_t& e : h->cev)
+    if (!e && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return cuda_fail(h, cudaGetLastError(), "copy event");
+  return LB_OK;
+}
+// elements [*e0, *e1) of piece c of n elements (pieces start at multiples of 1024 elements)
+void io_chunk(long long n, int c, long long* e0, long long* e1) {
+  const long long per = ((n + IO_CHUNKS - 1) / IO_CHUNKS + 1023) / 1024 * 1024;
+  *e0 = std::min(n, per * c);
+  *e1 = std::min(n, per * (c + 1));
 }
 
 // Output staging: device pointer as is, else a device temporary copied back by finish_out.
@@ -573,6 +593,7 @@ IoParams make_io_params(lb_handle h) {
   p.box = h->box();
   p.s0 = (long long)h->zlo() * h->nx * h->ny;      // the caller's arrays hold the handle's own planes
   p.s1 = (long long)h->zhi() * h->nx * h->ny;
+  p.c0 = 0; p.c1 = p.s1 - p.s0;
   p.phi = h->phi;
   p.phi2 = h->phi2; p.sc = h->model == 1; p.G_C = h->G_C;
   p.tau_r = h->par.tau_r; p.tau_b = h->par.tau_b; p.A = h->par.A; p.beta = h->par.beta;
@@ -590,7 +611,7 @@ IoParams make_io_params(lb_handle h) {
     else KERNEL<MODE, TWO, false><<<nb, 256, 0, h->stream>>>(p);                                     \
   }                                                                                                  \
   void launch_##KERNEL(lb_handle h, const IoParams& p) {                                             \
-    const unsigned nb = (unsigned)((p.s1 - p.s0 + 255) / 256);                                       \
+    const unsigned nb = (unsigned)((p.c1 - p.c0 + 255) / 256);                                       \
     const int mode = h->mode();                                                                      \
     if (h->two) {                                                                                    \
       if (mode == MODE_AB) launch_##KERNEL##_t<MODE_AB, true>(h, p, nb);                             \
@@ -697,6 +718,8 @@ void lb_destroy(lb_handle h) {
   DeviceGuard guard(h->device);
   if (h->inited || h->mask) cudaStreamSynchronize(h->stream);
   for (void* q : {(void*)h->buf[0], (void*)h->buf[1], (void*)h->phi, (void*)h->phi2, (void*)h->mask, (void*)h->mom, (void*)h->chk, (void*)h->parts, (void*)h->pid, (void*)h->mask_static, (void*)h->povf, (void*)h->pred, (void*)h->ptot, (void*)h->ghost_rho}) dev_free(h->al, q);
+  if (h->cstream) cudaStreamDestroy(h->cstream);
+  for (cudaEvent_t e : h->cev) if (e) cudaEventDestroy(e);
   if (h->gexec) cudaGraphExecDestroy(h->gexec);
   if (h->gstream) cudaStreamDestroy(h->gstream);
   for (int i = 0; i < 2; ++i) if (h->ev_step[i]) cudaEventDestroy(h->ev_step[i]);
@@ -1020,9 +1043,10 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   if (h->np > 0 && (rc = init_particles(h))) return rc;
   const size_t fb = (size_t)h->Sx * sizeof(float);
   Staged srr, srb, su;
-  if ((rc = stage_in(h, rho_r, fb, srr))) return rc;
-  if (rho_b && (rc = stage_in(h, rho_b, fb, srb))) return rc;
-  if ((rc = stage_in(h, u, 3 * fb, su))) return rc;
+  // host arrays: staged piece by piece below, under the kernel that turns the piece before into populations
+  if ((rc = stage_in(h, rho_r, fb, srr, false))) return rc;
+  if (rho_b && (rc = stage_in(h, rho_b, fb, srb, false))) return rc;
+  if ((rc = stage_in(h, u, 3 * fb, su, false))) return rc;
   h->cur = 0;
   h->aa_odd = 0;
   h->steps_done = 0;
@@ -1032,10 +1056,35 @@ int lb_init(lb_handle h, const float* rho_r, const float* rho_b, const float* u)
   p.rho_r = static_cast<const float*>(srr.dev);
   p.rho_b = static_cast<const float*>(srb.dev);
   p.u = static_cast<const float*>(su.dev);
-  // solid sites keep zeros so that stray reads are harmless
-  cudaError_t e = cudaMemsetAsync(h->cur_buf(), 0, (size_t)h->planes() * h->S * sizeof(float), h->stream);
+  // solid sites (and the planes of a slab that its own sites do not read) keep zeros so that stray reads
+  // are harmless; in an undivided box without solid sites k_scatter writes every slot of every site, and
+  // clearing 40 GB first costs 12 ms at 640^3
+  cudaError_t e = cudaSuccess;
+  if (h->has_solid || h->gz) e = cudaMemsetAsync(h->cur_buf(), 0, (size_t)h->planes() * h->S * sizeof(float), h->stream);
   if (e != cudaSuccess) return cuda_fail(h, e, "population memset");
-  launch_scatter(h, p);
+  if (srr.owned || srb.owned || su.owned) {
+    if ((rc = io_pipeline(h))) return rc;
+    cudaEventRecord(h->cev[IO_CHUNKS], h->stream);             // (the staging buffers and the cleared populations are ready)
+    cudaStreamWaitEvent(h->cstream, h->cev[IO_CHUNKS], 0);
+    const long long n = h->Sx;
+    for (int c = 0; c < IO_CHUNKS; ++c) {
+      long long e0, e1;
+      io_chunk(n, c, &e0, &e1);
+      if (e1 <= e0) continue;
+      const size_t nb = (size_t)(e1 - e0) * sizeof(float);
+      if (srr.owned) e = cudaMemcpyAsync(static_cast<float*>(srr.dev) + e0, rho_r + e0, nb, cudaMemcpyHostToDevice, h->cstream);
+      if (e == cudaSuccess && srb.owned) e = cudaMemcpyAsync(static_cast<float*>(srb.dev) + e0, rho_b + e0, nb, cudaMemcpyHostToDevice, h->cstream);
+      for (int a = 0; a < 3 && e == cudaSuccess && su.owned; ++a)
+        e = cudaMemcpyAsync(static_cast<float*>(su.dev) + a * n + e0, u + a * n + e0, nb, cudaMemcpyHostToDevice, h->cstream);
+      if (e != cudaSuccess) return cuda_fail(h, e, "H2D copy");
+      cudaEventRecord(h->cev[c], h->cstream);
+      cudaStreamWaitEvent(h->stream, h->cev[c], 0);
+      p.c0 = e0; p.c1 = e1;
+      launch_scatter(h, p);
+    }
+  } else {
+    launch_scatter(h, p);
+  }
   if ((rc = check_launch(h, "k_scatter"))) return rc;
   h->inited = true;
   h->phi_current = false;
@@ -1187,16 +1236,34 @@ int lb_get_macros(lb_handle h, float* rho_r, float* rho_b, float* u) {
   p.out0 = static_cast<float*>(o0.dev);
   p.out1 = static_cast<float*>(o1.dev);
   p.out2 = static_cast<float*>(o2.dev);
-  launch_macros(h, p);
-  if ((rc = check_launch(h, "k_macros"))) return rc;
-  if ((rc = finish_out(h, rho_r, fb, o0))) return rc;
-  if (h->two && (rc = finish_out(h, rho_b, fb, o1))) return rc;
-  if ((rc = finish_out(h, u, 3 * fb, o2))) return rc;
   if (o0.owned || o1.owned || o2.owned) {
-    cudaError_t e = cudaStreamSynchronize(h->stream);
+    // host arrays: the fields piece by piece, each piece on its way over PCIe while the next one is formed
+    if ((rc = io_pipeline(h))) return rc;
+    const long long n = h->Sx;
+    cudaError_t e = cudaSuccess;
+    for (int c = 0; c < IO_CHUNKS; ++c) {
+      long long e0, e1;
+      io_chunk(n, c, &e0, &e1);
+      if (e1 <= e0) continue;
+      p.c0 = e0; p.c1 = e1;
+      launch_macros(h, p);
+      cudaEventRecord(h->cev[c], h->stream);
+      cudaStreamWaitEvent(h->cstream, h->cev[c], 0);
+      const size_t nb = (size_t)(e1 - e0) * sizeof(float);
+      if (rho_r && o0.owned) e = cudaMemcpyAsync(rho_r + e0, static_cast<float*>(o0.dev) + e0, nb, cudaMemcpyDeviceToHost, h->cstream);
+      if (e == cudaSuccess && h->two && rho_b && o1.owned) e = cudaMemcpyAsync(rho_b + e0, static_cast<float*>(o1.dev) + e0, nb, cudaMemcpyDeviceToHost, h->cstream);
+      for (int a = 0; a < 3 && e == cudaSuccess && u && o2.owned; ++a)
+        e = cudaMemcpyAsync(u + a * n + e0, static_cast<float*>(o2.dev) + a * n + e0, nb, cudaMemcpyDeviceToHost, h->cstream);
+      if (e != cudaSuccess) return cuda_fail(h, e, "D2H copy");
+    }
+    if ((rc = check_launch(h, "k_macros"))) return rc;
+    e = cudaStreamSynchronize(h->cstream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return cuda_fail(h, e, "lb_get_macros");
+    return LB_OK;
   }
-  return LB_OK;
+  launch_macros(h, p);
+  return check_launch(h, "k_macros");
 }
 
 int lb_get_populations(lb_handle h, int comp, float* f) {

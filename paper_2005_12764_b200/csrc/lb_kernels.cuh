@@ -1126,7 +1126,8 @@ struct IoParams {
   const float* ps[Q];    // its direction planes, as in StepParams
   float* pd[Q];
   Box box;
-  long long s0, s1;      // allocated site indices this launch covers: [zlo, zhi) x ny x nx
+  long long s0, s1;      // allocated site indices the caller's arrays stand for: [zlo, zhi) x ny x nx
+  long long c0, c1;      // elements [c0, c1) of those arrays that THIS launch treats (all: 0, s1 - s0)
   int comp;              // component of k_scatter / k_gatherf
   const float* in0;      // k_scatter: f[19][Sx] full populations (or nullptr: from rho,u)
   const float* rho_r;    // init fields
@@ -1156,10 +1157,10 @@ template <int ESZ, bool HAS_SOLID>
 __device__ __forceinline__ IoSite io_site(const IoParams& p) {
   IoSite t;
   const Box& b = p.box;
-  t.e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  t.e = p.c0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
   t.s = p.s0 + t.e;
   t.Sx = p.s1 - p.s0;
-  t.inside = t.s < p.s1;
+  t.inside = t.e < p.c1;
   t.solid = false;
   t.smask = 0;
   t.x = t.y = t.z = 0;
