@@ -299,7 +299,7 @@ def measure_config(wl_name, storage, K, Wu, dev, local_rank, world, w=None, with
     # on the stream).  A box of at most 2^21 sites is stepped by replaying a CUDA graph (include/lb.h,
     # lb_set_tuning "graph"), which event records inside the step would switch off: there the timed
     # region runs without them and the kernels are timed in a pass of the same length right after it.
-    graphed = (not slabs) and w.sites <= (1 << 21) and TUNE.get("graph", -1) != 0 and w.info.get("particles") is None
+    graphed = (not slabs) and w.sites <= (1 << 21) and TUNE.get("graph", -1) != 0
     sim.set_profiling(0 if graphed else 7)
     sim.step(Wu)
     torch.cuda.synchronize()

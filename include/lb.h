@@ -310,7 +310,7 @@ int lb_get_particles(lb_handle h, lb_particle* state, double* force);
  * without that exception; 0 = a full phase-field sweep over the populations before every step
  * (same phi to ~1e-8).  "zc": z planes
  * per CTA, 0 = automatic.  "graph": lb_step replays a CUDA graph of 16 time steps where it can (no
- * profiling, no particles, not the first two steps, not while the caller's stream is capturing):
+ * profiling, not the first two steps, not while the caller's stream is capturing):
  * -1 (default) = for boxes of at most 2^21 sites, whose step is bounded by launch latency, 0 = never,
  * 1 = for every box.  The graph is captured on a stream of the handle's own and launched into the
  * handle's stream; it is rebuilt when any parameter, buffer or the storage parity changes; results

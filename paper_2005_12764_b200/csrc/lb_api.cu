@@ -1112,16 +1112,20 @@ std::vector<unsigned char> graph_key(lb_handle h) {
   const StepParams p = make_step_params(h, h->cur_buf(), next_buf(h), pick_zc(h), h->zlo(), h->zhi());
   const long long extra[] = {h->model, h->has_solid, h->has_moving, h->forward, h->storage, h->cur, h->aa_odd, h->two,
                              (long long)(size_t)h->mom, (long long)(size_t)h->mask, (long long)(size_t)h->buf[0], (long long)(size_t)h->buf[1]};
-  std::vector<unsigned char> k(sizeof(p) + sizeof(extra));
+  std::vector<unsigned char> k(sizeof(p) + sizeof(extra) + (h->np > 0 ? sizeof(PartParams) : 0));
   memcpy(k.data(), &p, sizeof(p));
   memcpy(k.data() + sizeof(p), extra, sizeof(extra));
+  if (h->np > 0) {       // the particle kernels' parameters (buffers, options)
+    const PartParams q = make_part_params(h);
+    memcpy(k.data() + sizeof(p) + sizeof(extra), &q, sizeof(q));
+  }
   return k;
 }
 
 bool graph_eligible(lb_handle h, int remaining) {
   if (h->graph == 0 || h->graph_failed || remaining < GRAPH_STEPS) return false;
   if (h->graph < 0 && h->Sx > GRAPH_AUTO_SITES) return false;
-  if (h->profiling || h->np > 0 || h->gz) return false;
+  if (h->profiling || h->gz) return false;
   // the host flags must come back to where they were: with forwarding phi is current at every step's
   // start (the first step after lb_init / lb_set_populations runs K1 by itself), without it never
   if (h->two && forwarding(h) != h->phi_current) return false;

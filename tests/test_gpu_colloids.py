@@ -210,3 +210,21 @@ def test_particles_between_sliding_walls_parity(lbmod, lbo, two, wet):
             assert e < pu.POP_TOL * max(1, n / 2), (n, e)
             assert ds < 2e-6 and dm < pu.MACRO_TOL, (n, ds, dm)
             assert df < 1e-5 * max(1.0, np.abs(o.get_particles()[1]).max()), (n, df)
+
+
+def test_particles_step_graph_is_bit_identical(lbmod):
+    """lb_step replays a CUDA graph of 16 steps for small boxes, with particles too (the particle
+    kernels take no decision on the host): same bits as plain launches, fluid and particles."""
+    from paper_2005_12764_b200 import workloads as W
+    w = W.get("bijel-mini")
+    out = []
+    for graph in (0, 1):
+        sim = lbmod.from_workload(w)
+        sim.set_tuning(graph=graph)
+        sim.init(w.rho_r, w.rho_b, w.u)
+        sim.step(3); sim.step(70); sim.step(1000)
+        out.append((sim.get_populations(0), sim.get_populations(1), sim.get_phi(), sim.get_particles(), sim.launch_count()))
+    a, b = out
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    assert np.array_equal(a[3][0], b[3][0]) and np.array_equal(a[3][1], b[3][1])
+    assert a[4] == b[4]
