@@ -1023,7 +1023,11 @@ __global__ void __launch_bounds__(TX* TY, 8) k_phase_fwd(const StepParams p) {
       }
     });
   }
-  if (x >= H && x + 4 <= b.nx - H && y >= H && y < b.ny - H && (!b.zper || (z >= H && z < b.nz - H))) {   // no ghost image
+  // A row away from the y and z faces of the box (the same answer for a whole warp) has images along x
+  // only, and only in its first and last quad: one 128-bit store, plus the few images of those two
+  // quads.  (A warp spans 128 sites, so in a box of nx <= 256 EVERY warp holds such a quad; sending
+  // the whole warp through the general image code below was 40 % of this kernel's instructions.)
+  if (y >= H && y < b.ny - H && (!b.zper || (z >= H && z < b.nz - H))) {
     float f0[4], f1[4];
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
@@ -1036,9 +1040,26 @@ __global__ void __launch_bounds__(TX* TY, 8) k_phase_fwd(const StepParams p) {
       }
     }
     const size_t px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
-    const size_t o = (size_t)(x + HALO) + px * ((size_t)(y + HALO) + py * (size_t)(z + HALO));
+    const size_t rowo = px * ((size_t)(y + HALO) + py * (size_t)(z + HALO));
+    const size_t o = (size_t)(x + HALO) + rowo;
     *reinterpret_cast<float4*>(p.phi + o) = make_float4(f0[0], f0[1], f0[2], f0[3]);
     if constexpr (SC) *reinterpret_cast<float4*>(p.phi2 + o) = make_float4(f1[0], f1[1], f1[2], f1[3]);
+    if (x < H) {                       // x = 0 (H <= 4 = the quad): sites 0 .. H-1 also stand behind nx - 1
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        if (e < H) {
+          p.phi[o + b.nx + e] = f0[e];
+          if constexpr (SC) p.phi2[o + b.nx + e] = f1[e];
+        }
+    }
+    if (x + 4 > b.nx - H) {            // x = nx - 4: sites nx - H .. nx - 1 also stand before 0
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        if (e >= 4 - H) {
+          p.phi[o - b.nx + e] = f0[e];
+          if constexpr (SC) p.phi2[o - b.nx + e] = f1[e];
+        }
+    }
   } else {
 #pragma unroll
     for (int e = 0; e < 4; ++e) store_fields<SC>(p, x + e, y, z, H, solid[e], d[e], 1.0f + t[e]);
