@@ -920,8 +920,6 @@ namespace {
 int init_particles(lb_handle h) {
   if (h->storage != 0) return fail(h, LB_ESTATE, "particles need A/B storage");
   if (h->model != 0) return fail(h, LB_ESTATE, "particles are built for the colour-gradient model and for one component");
-  // a slab with its two ghost planes must not hold any plane of the box twice (a ring of one slab would)
-  if (h->gz && h->nz + 2 > h->slab_nzg) return fail(h, LB_ESTATE, "particles in a slab need nz + 2 <= nz_global (at least two slabs)");
   const Box b0 = h->box();
   const size_t nwords = (size_t)b0.nxw * h->ny * h->nza();
   const size_t mb = (3 * nwords + 1) * 4;

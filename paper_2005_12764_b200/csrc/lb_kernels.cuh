@@ -1458,19 +1458,22 @@ __device__ __forceinline__ PartBox part_box(const Box& b, const double r[3], dou
   }
   return pb;
 }
-// the allocated plane that holds global plane zg, or -1
-__device__ __forceinline__ int local_z(const Box& b, int zg) {
+// The allocated plane that holds global plane zg, or -1.  A ring of ONE slab holds the planes next to its
+// own faces twice (own plane and the ghost plane on the other side): img = 0 / 1 asks for the first /
+// second copy.
+__device__ __forceinline__ int local_z(const Box& b, int zg, int img = 0) {
   int z = zg - b.zoff;
   z = z < 0 ? z + b.gnz : (z >= b.gnz ? z - b.gnz : z);
+  z += img * b.gnz;
   return z < b.nz ? z : -1;
 }
-// node i of the box: site coordinates (x, y, z); false if this handle does not hold its plane
-__device__ __forceinline__ bool part_box_node(const Box& b, const PartBox& pb, int i, int& x, int& y, int& z) {
+// node i of the box: site coordinates (x, y, z); false if this handle does not hold (that copy of) its plane
+__device__ __forceinline__ bool part_box_node(const Box& b, const PartBox& pb, int i, int& x, int& y, int& z, int img = 0) {
   const int lx = i % pb.ext[0], ly = (i / pb.ext[0]) % pb.ext[1], lz = i / (pb.ext[0] * pb.ext[1]);
   x = (pb.lo[0] + lx) % b.nx; if (x < 0) x += b.nx;
   y = (pb.lo[1] + ly) % b.ny; if (y < 0) y += b.ny;
   int zg = (pb.lo[2] + lz) % b.gnz; if (zg < 0) zg += b.gnz;
-  z = local_z(b, zg);
+  z = local_z(b, zg, img);
   return z >= 0;
 }
 __device__ __forceinline__ bool inside_particle(const Box& b, const PState& P, int x, int y, int z) {
@@ -1579,13 +1582,14 @@ __device__ __forceinline__ void scan_shell(const Box& b, const PartBox& pb, cons
     int y = pb.lo[1] + ly, zg = pb.lo[2] + lz;
     y += y < 0 ? b.ny : (y >= b.ny ? -b.ny : 0);
     zg += zg < 0 ? b.gnz : (zg >= b.gnz ? -b.gnz : 0);
-    const int z = local_z(b, zg);
-    if (z < 0) continue;                                   // a plane of another slab
     float fy = (float)y - cyr, fz = (float)zg - czr;       // fp32 is enough for the prefilter
     fy += fy > 0.5f * b.ny ? -(float)b.ny : (fy < -0.5f * b.ny ? (float)b.ny : 0.f);
     fz += fz > 0.5f * b.gnz ? -(float)b.gnz : (fz < -0.5f * b.gnz ? (float)b.gnz : 0.f);
     const float ryz2 = fy * fy + fz * fz;
     if (ryz2 > rout2) continue;                            // a row in a corner of the box: it misses the shell
+    for (int img = 0; img < 2; ++img) {                    // (the second copy of a plane: a ring of one slab only)
+    const int z = local_z(b, zg, img);
+    if (z < 0) continue;                                   // a plane of another slab
     for (int lx0 = 0; lx0 < pb.ext[0]; lx0 += 32) {
       const int lx = lx0 + lane;
       int x = pb.lo[0] + lx;
@@ -1611,6 +1615,7 @@ __device__ __forceinline__ void scan_shell(const Box& b, const PartBox& pb, cons
         __syncwarp();
       }
     }
+    }
   }
   if (lane < qn) process(queue[lane]);
 }
@@ -1621,9 +1626,9 @@ __global__ void __launch_bounds__(256) k_part_raster(const PartParams p) {
   const PState& P = p.parts[blockIdx.x];
   const PartBox pb = part_box(b, P.r, P.R + 1.0);
   const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
-  for (int i = threadIdx.x; i < nn; i += blockDim.x) {
+  for (int i = threadIdx.x; i < 2 * nn; i += blockDim.x) {
     int x, y, z;
-    if (!part_box_node(b, pb, i, x, y, z)) continue;       // (a slab marks its ghost planes too)
+    if (!part_box_node(b, pb, i % nn, x, y, z, i / nn)) continue;       // (a slab marks its ghost planes too)
     if (solid_at(b, x, y, z) || !inside_particle(b, P, x, y, z)) continue;
     atomicOr(&p.mask[(size_t)(z * b.ny + y) * b.nxw + (x >> 5)], 1u << (x & 31));
     p.pid[site_of(b, x, y, z)] = blockIdx.x;
@@ -1785,9 +1790,9 @@ __global__ void __launch_bounds__(256) k_part_remap(const PartParams p) {
   __syncthreads();
   const PartBox pb = part_box(b, P.r, P.R + 2.0);
   const int nn = pb.ext[0] * pb.ext[1] * pb.ext[2];
-  for (int i = threadIdx.x; i < nn; i += blockDim.x) {
+  for (int i = threadIdx.x; i < 2 * nn; i += blockDim.x) {
     int x, y, z;
-    if (!part_box_node(b, pb, i, x, y, z)) continue;       // (a slab lists the changes in its ghost planes too)
+    if (!part_box_node(b, pb, i % nn, x, y, z, i / nn)) continue;       // (a slab lists the changes in its ghost planes too)
     const size_t s = site_of(b, x, y, z);
     const bool was = p.pid[s] == me;
     const bool now = inside_particle(b, P, x, y, z) && (was || !solid_at(b, x, y, z));

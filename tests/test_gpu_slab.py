@@ -213,14 +213,15 @@ def _particle_workload(two, walls=False):
                       info={"particles": parts, "particle_options": dict(mobile=True, K=0.02, h_c=2.5, lubrication=True)})
 
 
-@pytest.mark.parametrize("cuts", [(16, 16), (8, 16, 8), (12, 20)])
+@pytest.mark.parametrize("cuts", [(16, 16), (8, 16, 8), (12, 20), (32,)])
 @pytest.mark.parametrize("two,walls", [(True, False), (False, False), (True, True)])
 def test_slabs_with_replicated_particles(lbmod, slabmod, two, walls, cuts):
     """Replicated data: every slab holds all particles; the link sums and the
     impulses of the node changes are added over the slabs.  Against the undivided box over 40
     steps, in which nodes enter and leave the particles on both sides of the cuts: the same node
     map, particle states to the rounding of the two sums, populations and fields to the rounding
-    that follows from it; and all slabs hold the same particle states bit for bit."""
+    that follows from it; and all slabs hold the same particle states bit for bit.  (32,): a ring of
+    one slab, which holds the planes next to its faces twice, as own and as ghost planes."""
     w = _particle_workload(two, walls)
     sim = lbmod.from_workload(w)
     sim.set_tuning(zc=8)
@@ -255,12 +256,3 @@ def test_slabs_with_replicated_particles(lbmod, slabmod, two, walls, cuts):
                 fluid = b[0] != 0
                 assert np.abs(ring.gather("get_phi") - sim.get_phi())[fluid].max() < 2e-6, n
     assert changed > 40                       # nodes did enter and leave the particles
-
-
-def test_particles_need_two_slabs(lbmod, slabmod):
-    """A ring of one slab would hold the planes next to its own faces twice: refused at lb_init."""
-    w = _particle_workload(True)
-    ring = slabmod.LocalRing(w, (32,), "ab", zc=8)
-    with pytest.raises(lbmod.LBError) as ei:
-        ring.init()
-    assert ei.value.code == lbmod.LB_ESTATE and "two slabs" in str(ei.value)
