@@ -1023,46 +1023,53 @@ __global__ void __launch_bounds__(TX* TY, 8) k_phase_fwd(const StepParams p) {
       }
     });
   }
-  // A row away from the y and z faces of the box (the same answer for a whole warp) has images along x
-  // only, and only in its first and last quad: one 128-bit store, plus the few images of those two
-  // quads.  (A warp spans 128 sites, so in a box of nx <= 256 EVERY warp holds such a quad; sending
-  // the whole warp through the general image code below was 40 % of this kernel's instructions.)
-  if (y >= H && y < b.ny - H && (!b.zper || (z >= H && z < b.nz - H))) {
-    float f0[4], f1[4];
+  // phi of the quad goes to its home in the padded array and to every periodic image that falls into
+  // the ghost layers (depth H).  Images are taken row by row: a row has at most one image along y and
+  // one along z (two in a box thinner than 2 H), the same for a whole warp, and within a row only the
+  // first and the last quad have images along x: one 128-bit store per row image plus the few x
+  // images of those two quads.  (A warp spans 128 sites, so in a box of nx <= 256 EVERY warp holds
+  // such a quad; sending whole warps through per-site image code, 27 candidates per site, was 40 % of
+  // this kernel's instructions, and all of them in rows within H of a y or z face: C4.)
+  float f0[4], f1[4];
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const float rho = 1.0f + t[e];
-      if constexpr (!SC) {
-        f0[e] = solid[e] ? sent[e] : d[e] / rho;
-      } else {
-        f0[e] = solid[e] ? sent[e] : 0.5f * (rho + d[e]);
-        f1[e] = solid[e] ? 0.f : 0.5f * (rho - d[e]);
+  for (int e = 0; e < 4; ++e) {
+    const float rho = 1.0f + t[e];
+    if constexpr (!SC) {
+      f0[e] = solid[e] ? sent[e] : d[e] / rho;
+    } else {
+      f0[e] = solid[e] ? sent[e] : 0.5f * (rho + d[e]);
+      f1[e] = solid[e] ? 0.f : 0.5f * (rho - d[e]);
+    }
+  }
+  const size_t px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
+  const int sy[3] = {0, y < H ? b.ny : 0, y >= b.ny - H ? -b.ny : 0};
+  const int sz[3] = {0, (b.zper && z < H) ? b.nz : 0, (b.zper && z >= b.nz - H) ? -b.nz : 0};    // (a slab's z ghost planes come from its neighbours)
+#pragma unroll
+  for (int iz = 0; iz < 3; ++iz) {
+    if (iz && !sz[iz]) continue;
+#pragma unroll
+    for (int iy = 0; iy < 3; ++iy) {
+      if (iy && !sy[iy]) continue;
+      const size_t o = (size_t)(x + HALO) + px * ((size_t)(y + sy[iy] + HALO) + py * (size_t)(z + sz[iz] + HALO));
+      *reinterpret_cast<float4*>(p.phi + o) = make_float4(f0[0], f0[1], f0[2], f0[3]);
+      if constexpr (SC) *reinterpret_cast<float4*>(p.phi2 + o) = make_float4(f1[0], f1[1], f1[2], f1[3]);
+      if (x < H) {                       // x = 0 (H <= 4 = the quad): sites 0 .. H-1 also stand behind nx - 1
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          if (e < H) {
+            p.phi[o + b.nx + e] = f0[e];
+            if constexpr (SC) p.phi2[o + b.nx + e] = f1[e];
+          }
+      }
+      if (x + 4 > b.nx - H) {            // x = nx - 4: sites nx - H .. nx - 1 also stand before 0
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          if (e >= 4 - H) {
+            p.phi[o - b.nx + e] = f0[e];
+            if constexpr (SC) p.phi2[o - b.nx + e] = f1[e];
+          }
       }
     }
-    const size_t px = b.nx + 2 * HALO, py = b.ny + 2 * HALO;
-    const size_t rowo = px * ((size_t)(y + HALO) + py * (size_t)(z + HALO));
-    const size_t o = (size_t)(x + HALO) + rowo;
-    *reinterpret_cast<float4*>(p.phi + o) = make_float4(f0[0], f0[1], f0[2], f0[3]);
-    if constexpr (SC) *reinterpret_cast<float4*>(p.phi2 + o) = make_float4(f1[0], f1[1], f1[2], f1[3]);
-    if (x < H) {                       // x = 0 (H <= 4 = the quad): sites 0 .. H-1 also stand behind nx - 1
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        if (e < H) {
-          p.phi[o + b.nx + e] = f0[e];
-          if constexpr (SC) p.phi2[o + b.nx + e] = f1[e];
-        }
-    }
-    if (x + 4 > b.nx - H) {            // x = nx - 4: sites nx - H .. nx - 1 also stand before 0
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        if (e >= 4 - H) {
-          p.phi[o - b.nx + e] = f0[e];
-          if constexpr (SC) p.phi2[o - b.nx + e] = f1[e];
-        }
-    }
-  } else {
-#pragma unroll
-    for (int e = 0; e < 4; ++e) store_fields<SC>(p, x + e, y, z, H, solid[e], d[e], 1.0f + t[e]);
   }
 }
 
