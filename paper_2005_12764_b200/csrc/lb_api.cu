@@ -800,6 +800,9 @@ int lb_set_body_force(lb_handle h, float gx, float gy, float gz) {
 int lb_set_model(lb_handle h, int model, float G_C) {
   if (!h || (model != 0 && model != 1)) return fail(h, LB_EINVAL, "model must be 0 (colour gradient) or 1 (Shan-Chen)");
   if (h->inited) return fail(h, LB_ESTATE, "lb_set_model after lb_init");
+#ifdef LB_BUILD_SUBSET
+  if (model == 1) return fail(h, LB_EINVAL, "the Shan-Chen model is not in this developer build (LB_BUILD_SUBSET)");
+#endif
   h->model = model;
   h->G_C = G_C;
   return LB_OK;
@@ -807,6 +810,9 @@ int lb_set_model(lb_handle h, int model, float G_C) {
 
 int lb_set_forcing(lb_handle h, int mode) {
   if (!h || (mode != 0 && mode != 1)) return fail(h, LB_EINVAL, "forcing must be 0 (Guo) or 1 (exact difference)");
+#ifdef LB_BUILD_SUBSET
+  if (mode == 1) return fail(h, LB_EINVAL, "exact-difference forcing is not in this developer build (LB_BUILD_SUBSET)");
+#endif
   h->forcing = mode;
   return LB_OK;
 }
