@@ -473,9 +473,9 @@ def main(argv=None):
     ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "c2-mini", "c3-mini", "c4-mini", "c5-mini", "focuser", "focuser-3d", "focuser-drip", "focuser-large", "bijel", "bijel-mini"])
     ap.add_argument("--storage", default="ab", choices=["ab", "aa"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--tune", default="", help="lb_set_tuning settings for experiments, e.g. fixup=0,zc=12")
+    ap.add_argument("--tune", default="", help="lb_set_tuning settings for experiments, e.g. forward=0,zc=12,graph=0")
     ap.add_argument("--slabs", action="store_true", help="run the z-slab driver also at N = 1 (the rank is then its own neighbour)")
-    ap.add_argument("--configs", default=None, choices=["all", "none"], help="all = also measure C3 A/B, C4 A/B, C5 AA and C2 and report them under 'configs' (default when --workload is left at c5)")
+    ap.add_argument("--configs", default=None, choices=["all", "none"], help="all = also measure C3 A/B, C4 A/B, C5 AA, C2 and the bijel workload and report them under 'configs' (default when --workload is left at c5)")
     ap.add_argument("--model", default="cg", choices=["cg", "sc"], help="cg = colour gradient (north_star), sc = Shan-Chen + exact difference (Eq. 5-10 of the paper)")
     ap.add_argument("--gc", type=float, default=3.0, help="G_C of the Shan-Chen model")
     ap.add_argument("--windows", type=int, default=0, help="also time N windows of K steps spread over the config's run length")
